@@ -1,0 +1,169 @@
+/* mlpf.h -- C ABI of libmlpf.so: the MLPF transformer-encoder forward pass on one B200 (sm_100a).
+ *
+ * What it computes (citations: /root/reference/PAPER.md = CMS-PFT-25-001, arxiv 2601.17554):
+ *   per collision event, a variable-length *set* of PF elements (tracks, calorimeter clusters; L118-L124)
+ *   -> per-type embedding FFN (L156) -> L pre-LayerNorm transformer encoder blocks with full-event
+ *   scaled-dot-product self-attention  A = softmax(Q K^T / sqrt(d_k)) V  (Eq. 4; computed
+ *   flash-style without the N x N matrix, L154) -> two-layer FFN heads giving particle-id logits and
+ *   the momentum regressions (pT', eta, sin phi, cos phi, E')  (L126, L134-L139, L156, Fig. 2).
+ *   The readings taken where the paper is silent are A1-A19 in DESIGN.md.
+ *
+ * All functions are thread-safe per handle; concurrent mlpf_infer calls on DIFFERENT streams are safe
+ * (each stream owns a grow-only workspace), calls on the same stream serialise in stream order.
+ * Every step runs in hand-written CUDA kernels; there is no CPU fallback: without a CUDA device every
+ * entry point that needs one fails with MLPF_E_CUDA.
+ */
+#ifndef MLPF_H_
+#define MLPF_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mlpf_handle mlpf_handle;
+
+/* ---- error codes (0 = success) ------------------------------------------------------------------ */
+#define MLPF_OK          0
+#define MLPF_E_NULL     -1   /* a required pointer is NULL                                            */
+#define MLPF_E_BLOB     -2   /* bad magic / version / hyper-parameters / size of the weight blob      */
+#define MLPF_E_OFFSETS  -3   /* event_offsets[0] != 0, decreasing, or negative                        */
+#define MLPF_E_ALLOC    -4   /* device or host allocation failed                                      */
+#define MLPF_E_CUDA     -5   /* a CUDA call failed (text in mlpf_last_error)                          */
+#define MLPF_E_ARG      -6   /* unknown option / query key, bad value, capacity too small             */
+
+/* ---- weight blob (little-endian) -------------------------------------------------------------------
+ * 256-byte header, then fp32 tensors, row-major [out,in] (y = x W^T + b), in this order:
+ *   for type t = 1..n_types      : emb.t.W1[d,F] b1[d] W2[d,d] b2[d]                     (L156, A3-A4)
+ *   for layer l = 0..n_layers-1  : ln1.g[d] ln1.b[d] Wqkv[3d,d] bqkv[3d] Wo[d,d] bo[d]
+ *                                  ln2.g[d] ln2.b[d] W1[dff,d] b1[dff] W2[d,dff] b2[d]   (L148-L156)
+ *   lnf.g[d] lnf.b[d]                                                                    (A7)
+ *   cls.W1[d,d] b1[d] W2[C,d] b2[C]                                                      (L156, A11)
+ *   for k = 0..n_reg_heads-1     : reg.k.W1[d,d] b1[d] W2[reg_dims[k],d] b2[reg_dims[k]]
+ * Master weights are fp32.  In BF16 mode the library rounds (RNE) the matrices that feed tensor-core
+ * GEMMs (emb W2, Wqkv, Wo, W1, W2, cls.W1, reg.k.W1); emb W1, the C + sum(reg_dims) output rows
+ * (cls.W2, reg.k.W2) and all vectors stay fp32.
+ */
+#define MLPF_BLOB_MAGIC   "MLPFBLOB"
+#define MLPF_BLOB_VERSION 1u
+#define MLPF_HEADER_BYTES 256
+#define MLPF_MAX_REG_HEADS 4
+
+typedef struct mlpf_blob_header {
+    char     magic[8];       /* "MLPFBLOB" */
+    uint32_t version;        /* 1 */
+    uint32_t n_layers;       /* L  >= 1 */
+    uint32_t d_model;        /* d  in {64,128,256,512}; multiple of 64 */
+    uint32_t n_heads;        /* H ; d/H in {16,32,64} */
+    uint32_t d_ff;           /* multiple of 64 */
+    uint32_t n_feat;         /* F = 55 (A13); 1 <= F <= 64 */
+    uint32_t n_types;        /* T = 4 (A3) */
+    uint32_t n_classes;      /* C = 9 (A13); <= 16 */
+    uint32_t n_reg_heads;    /* <= 4 (A11) */
+    uint32_t reg_dims[MLPF_MAX_REG_HEADS]; /* (1,1,2,1): pT', eta, (sin phi, cos phi), E' ; sum <= 8 */
+    uint32_t activation;     /* 0 = ReLU (L156), 1 = GELU exact-erf form (A6) */
+    uint32_t final_ln;       /* 0/1 (A7) */
+    float    ln_eps;         /* 1e-5 (A8) */
+    /* zero padding up to MLPF_HEADER_BYTES */
+} mlpf_blob_header;
+
+/* mlpf_create: parse + validate `blob` (HOST pointer, borrowed only during the call), upload weights to
+ * the current CUDA device (fp32 masters + BF16 copies).  Returns NULL on error (see mlpf_last_error). */
+mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes);
+
+/* mlpf_infer: one forward pass (steps a0..a8 of DESIGN.md) over n_events packed events.
+ *   elements      DEVICE, [N, n_feat] row-major fp32, N = event_offsets[n_events]; feature 0 is the
+ *                 element type id as a float (0 = pad row, 1 track, 2 ECAL, 3 HCAL, 4 HF; A1-A2).
+ *   event_offsets HOST, n_events+1 int32, [0] = 0, non-decreasing; read before return (caller may free).
+ *   out_logits    DEVICE, [N, n_classes] fp32.   out_regress  DEVICE, [N, sum(reg_dims)] fp32
+ *                 = raw head outputs (pT', eta, sin phi, cos phi, E'), no inverse transform (A12).
+ *                 Pad rows are written as exactly 0 (A2).
+ *   stream        cudaStream_t (NULL = legacy default stream).
+ * Only enqueues work on `stream` (no device synchronisation; the first call on a stream, or a call with a
+ * larger N than before, may cudaMalloc).  n_events == 0 or N == 0: success, nothing written.
+ * Returns MLPF_OK or a negative error code. */
+int mlpf_infer(mlpf_handle* h, const float* elements, const int32_t* event_offsets, int32_t n_events,
+               float* out_logits, float* out_regress, void* stream);
+
+/* mlpf_infer_host: same computation with HOST buffers (pinned memory recommended): copies `elements`
+ * host->device, runs mlpf_infer, copies both outputs device->host, all on `stream`, then synchronises
+ * the stream.  This is the end-to-end entry (the paper's deployment copies per event, L224). */
+int mlpf_infer_host(mlpf_handle* h, const float* elements_host, const int32_t* event_offsets,
+                    int32_t n_events, float* out_logits_host, float* out_regress_host, void* stream);
+
+void mlpf_destroy(mlpf_handle* h);
+
+/* Thread-local text of the last error raised on this thread ("" if none). */
+const char* mlpf_last_error(void);
+
+/* ---- options -------------------------------------------------------------------------------------- */
+#define MLPF_OPT_PRECISION   1   /* MLPF_PREC_BF16 (default) | MLPF_PREC_FP32_DEBUG                    */
+#define MLPF_OPT_TILE_Q      2   /* query-tile rows of the attention work list: 64 | 128 (default 128) */
+#define MLPF_OPT_TAP_LAYER   3   /* -1 (default): full pass.  l >= 0: stop after encoder layer l so that
+                                    mlpf_debug_get_tensor can read that layer's intermediates; outputs
+                                    are then NOT written.  -2: stop after the embedding.                */
+#define MLPF_OPT_KERNELS     4   /* MLPF_KERNELS_TC (default: tcgen05 GEMM + attention) | MLPF_KERNELS_SIMPLE
+                                    (CUDA-core kernels in the same precision; debugging aid)            */
+#define MLPF_PREC_BF16        0
+#define MLPF_PREC_FP32_DEBUG  1
+#define MLPF_KERNELS_TC       0
+#define MLPF_KERNELS_SIMPLE   1
+int mlpf_set_option(mlpf_handle* h, int key, int64_t value);
+
+/* ---- queries -------------------------------------------------------------------------------------- */
+#define MLPF_Q_N_LAYERS        1
+#define MLPF_Q_D_MODEL         2
+#define MLPF_Q_N_HEADS         3
+#define MLPF_Q_D_FF            4
+#define MLPF_Q_N_FEAT          5
+#define MLPF_Q_N_CLASSES       6
+#define MLPF_Q_N_REGRESS       7
+#define MLPF_Q_WEIGHT_BYTES    8   /* device bytes held by weights (fp32 + bf16 copies)                */
+#define MLPF_Q_WORKSPACE_BYTES 9   /* device bytes held by all per-stream workspaces (linear in N)      */
+#define MLPF_Q_N_PARAMS        10
+#define MLPF_Q_LAUNCHES        11  /* kernels launched by the last mlpf_infer on this handle             */
+int64_t mlpf_query(const mlpf_handle* h, int key);   /* < 0 on error */
+
+/* ---- debug taps (tests only; these synchronise `stream`) ------------------------------------------- */
+/* integer schedule arrays of the last mlpf_infer on `stream` (step a0; bit-exact vs the oracle) */
+#define MLPF_SCHED_ROW_EVENT    0   /* [N]                                   */
+#define MLPF_SCHED_ROW_POS      1   /* [N]                                   */
+#define MLPF_SCHED_VALID        2   /* [N] 0/1                               */
+#define MLPF_SCHED_N_VALID      3   /* [E]                                   */
+#define MLPF_SCHED_TYPE_OFFSETS 4   /* [6] segment starts in sorted space, each a multiple of 128 */
+#define MLPF_SCHED_SORTED_ROW   5   /* [N] row -> sorted slot, -1 for pad    */
+#define MLPF_SCHED_TYPE_PERM    6   /* [type_offsets[5]] slot -> row, -1 filler */
+#define MLPF_SCHED_WORK_LIST    7   /* [n_tiles,2] (event, q_tile)           */
+/* returns the number of int32 written, or a negative error (MLPF_E_ARG if capacity is too small) */
+int64_t mlpf_debug_get_schedule(mlpf_handle* h, void* stream, int which, int32_t* host_out, int64_t capacity);
+
+/* intermediates of the last mlpf_infer on `stream`, converted to fp32, row-major:
+ * H [N,d] residual stream; U [N,d] last LayerNorm output; QK [N,2d] (q | k); VT [d,N] (v transposed);
+ * O [N,d] attention output; G [N,gw] last wide hidden (FFN: gw = d_ff; heads: gw = (1+n_reg_heads) d).
+ * Which stage they hold depends on MLPF_OPT_TAP_LAYER.  Returns floats written or a negative error. */
+#define MLPF_TENSOR_H   0
+#define MLPF_TENSOR_U   1
+#define MLPF_TENSOR_QK  2
+#define MLPF_TENSOR_VT  3
+#define MLPF_TENSOR_O   4
+#define MLPF_TENSOR_G   5
+int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which, float* host_out, int64_t capacity);
+
+/* ---- kernel-level entry points (unit tests and micro-benchmarks; device pointers, bf16 = uint16) ---- */
+/* C[M,N] (fp32, ldc = N) = A[M,K] (bf16, row-major) * W[N,K]^T (bf16, row-major) via the tcgen05 GEMM.
+ * K % 64 == 0, N % 64 == 0.  Step a3/a5/a6/a7's contraction (L148-L156) without an epilogue. */
+int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* W, float* C, int32_t M, int32_t N, int32_t K,
+                      void* stream);
+/* O[N,d] (bf16) = per-event multi-head softmax(Q K^T / sqrt(hd)) V (Eq. 4) via the tcgen05 flash kernel.
+ * QK [N,2d] bf16 (q | k), VT [d, ldvt] bf16, key_valid [N] int32 0/1 (NULL = all valid),
+ * event_offsets HOST int32 [n_events+1]. */
+int mlpf_tc_attention_bf16(const uint16_t* QK, const uint16_t* VT, int64_t ldvt, const int32_t* key_valid,
+                           const int32_t* event_offsets, int32_t n_events, int32_t d_model, int32_t n_heads,
+                           uint16_t* O, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MLPF_H_ */

@@ -1,0 +1,182 @@
+"""paper_2601_17554_b200 -- thin ctypes binding over libmlpf.so (include/mlpf.h).
+
+Argument marshalling only: every step of the MLPF encoder forward pass runs in
+the library's CUDA kernels.  torch is used for device memory and streams.  There is no CPU fallback:
+importing works without a GPU (so that the symbols can be checked), creating a model does not.
+"""
+from __future__ import annotations
+import ctypes as C
+import os
+import numpy as np
+
+from .blob import pack_blob
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmlpf.so")
+
+# include/mlpf.h constants
+OK = 0
+OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS = 1, 2, 3, 4
+PREC_BF16, PREC_FP32_DEBUG = 0, 1
+KERNELS_TC, KERNELS_SIMPLE = 0, 1
+Q_N_LAYERS, Q_D_MODEL, Q_N_HEADS, Q_D_FF, Q_N_FEAT, Q_N_CLASSES, Q_N_REGRESS = 1, 2, 3, 4, 5, 6, 7
+Q_WEIGHT_BYTES, Q_WORKSPACE_BYTES, Q_N_PARAMS, Q_LAUNCHES = 8, 9, 10, 11
+SCHED = dict(row_event=0, row_pos=1, valid=2, n_valid=3, type_offsets=4, sorted_row=5, type_perm=6, work_list=7)
+TENSOR = dict(H=0, U=1, QK=2, VT=3, O=4, G=5)
+
+EXPORTS = ["mlpf_create", "mlpf_infer", "mlpf_infer_host", "mlpf_destroy", "mlpf_last_error", "mlpf_set_option",
+           "mlpf_query", "mlpf_debug_get_schedule", "mlpf_debug_get_tensor", "mlpf_tc_gemm_bf16",
+           "mlpf_tc_attention_bf16"]
+
+_lib = None
+
+
+def lib():
+    """Load libmlpf.so (built in-tree by paper_2601_17554_b200.build); fails loudly if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2601_17554_b200.build` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+    L.mlpf_create.restype = vp
+    L.mlpf_create.argtypes = [vp, C.c_size_t]
+    L.mlpf_infer.restype = C.c_int
+    L.mlpf_infer.argtypes = [vp, vp, vp, i32, vp, vp, vp]
+    L.mlpf_infer_host.restype = C.c_int
+    L.mlpf_infer_host.argtypes = [vp, vp, vp, i32, vp, vp, vp]
+    L.mlpf_destroy.restype = None
+    L.mlpf_destroy.argtypes = [vp]
+    L.mlpf_last_error.restype = C.c_char_p
+    L.mlpf_last_error.argtypes = []
+    L.mlpf_set_option.restype = C.c_int
+    L.mlpf_set_option.argtypes = [vp, C.c_int, i64]
+    L.mlpf_query.restype = i64
+    L.mlpf_query.argtypes = [vp, C.c_int]
+    L.mlpf_debug_get_schedule.restype = i64
+    L.mlpf_debug_get_schedule.argtypes = [vp, vp, C.c_int, vp, i64]
+    L.mlpf_debug_get_tensor.restype = i64
+    L.mlpf_debug_get_tensor.argtypes = [vp, vp, C.c_int, vp, i64]
+    L.mlpf_tc_gemm_bf16.restype = C.c_int
+    L.mlpf_tc_gemm_bf16.argtypes = [vp, vp, vp, i32, i32, i32, vp]
+    L.mlpf_tc_attention_bf16.restype = C.c_int
+    L.mlpf_tc_attention_bf16.argtypes = [vp, vp, i64, vp, vp, i32, i32, i32, vp, vp]
+    _lib = L
+    return L
+
+
+class MlpfError(RuntimeError):
+    pass
+
+
+def _check(rc):
+    if rc < 0:
+        raise MlpfError(f"libmlpf error {rc}: {lib().mlpf_last_error().decode()}")
+    return rc
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+class Mlpf:
+    """One model instance (mlpf_create ... mlpf_destroy)."""
+
+    def __init__(self, W: dict, m):
+        self._h = None
+        blob = pack_blob(W, m)
+        self.m = m
+        buf = C.create_string_buffer(blob, len(blob))
+        h = lib().mlpf_create(C.cast(buf, C.c_void_p), len(blob))
+        if not h:
+            raise MlpfError("mlpf_create failed: " + lib().mlpf_last_error().decode())
+        self._h = C.c_void_p(h)
+        self.n_classes = int(self.query(Q_N_CLASSES))
+        self.n_regress = int(self.query(Q_N_REGRESS))
+        self.n_feat = int(self.query(Q_N_FEAT))
+        self.d_model = int(self.query(Q_D_MODEL))
+
+    def close(self):
+        if self._h is not None:
+            lib().mlpf_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_option(self, key, value):
+        _check(lib().mlpf_set_option(self._h, key, int(value)))
+
+    def query(self, key):
+        return _check(lib().mlpf_query(self._h, key))
+
+    def infer(self, elements, event_offsets, out_logits=None, out_regress=None, stream=None):
+        """elements: CUDA float32 tensor [N, n_feat]; event_offsets: host int32 array [E+1].
+        Returns (logits [N,C], regress [N,R]) CUDA float32 tensors (enqueued on `stream`)."""
+        import torch
+        assert elements.is_cuda and elements.dtype == torch.float32 and elements.is_contiguous()
+        off = np.ascontiguousarray(event_offsets, dtype=np.int32)
+        N = elements.shape[0]
+        if out_logits is None:
+            out_logits = torch.empty((N, self.n_classes), dtype=torch.float32, device=elements.device)
+        if out_regress is None:
+            out_regress = torch.empty((N, self.n_regress), dtype=torch.float32, device=elements.device)
+        _check(lib().mlpf_infer(self._h, C.c_void_p(elements.data_ptr()), off.ctypes.data_as(C.c_void_p),
+                                len(off) - 1, C.c_void_p(out_logits.data_ptr()),
+                                C.c_void_p(out_regress.data_ptr()), _stream_ptr(stream)))
+        return out_logits, out_regress
+
+    def infer_host(self, elements_host, event_offsets, out_logits_host, out_regress_host, stream=None):
+        """Host (ideally pinned) torch tensors in and out; copies + compute + synchronise inside."""
+        off = np.ascontiguousarray(event_offsets, dtype=np.int32)
+        _check(lib().mlpf_infer_host(self._h, C.c_void_p(elements_host.data_ptr()),
+                                     off.ctypes.data_as(C.c_void_p), len(off) - 1,
+                                     C.c_void_p(out_logits_host.data_ptr()),
+                                     C.c_void_p(out_regress_host.data_ptr()), _stream_ptr(stream)))
+
+    def schedule(self, which: str, stream=None):
+        cap = 1 << 22
+        out = np.empty(cap, np.int32)
+        n = _check(lib().mlpf_debug_get_schedule(self._h, _stream_ptr(stream), SCHED[which],
+                                                 out.ctypes.data_as(C.c_void_p), cap))
+        out = out[:n].copy()
+        return out.reshape(-1, 2) if which == "work_list" else out
+
+    def tensor(self, which: str, shape, stream=None):
+        out = np.empty(int(np.prod(shape)), np.float32)
+        n = _check(lib().mlpf_debug_get_tensor(self._h, _stream_ptr(stream), TENSOR[which],
+                                               out.ctypes.data_as(C.c_void_p), out.size))
+        assert n == out.size, (n, out.size)
+        return out.reshape(shape)
+
+
+def tc_gemm_bf16(A, W, stream=None):
+    """A [M,K], W [N,K] CUDA bfloat16 tensors -> fp32 [M,N] = A W^T via the tcgen05 GEMM kernel."""
+    import torch
+    M, K = A.shape
+    N = W.shape[0]
+    out = torch.empty((M, N), dtype=torch.float32, device=A.device)
+    _check(lib().mlpf_tc_gemm_bf16(C.c_void_p(A.data_ptr()), C.c_void_p(W.data_ptr()), C.c_void_p(out.data_ptr()),
+                                   M, N, K, _stream_ptr(stream)))
+    return out
+
+
+def tc_attention_bf16(QK, VT, key_valid, event_offsets, d_model, n_heads, stream=None):
+    """QK [N,2d] bf16, VT [d,ldvt] bf16, key_valid [N] int32 or None -> O [N,d] bf16 (Eq. 4 per event/head)."""
+    import torch
+    off = np.ascontiguousarray(event_offsets, dtype=np.int32)
+    N = QK.shape[0]
+    out = torch.zeros((N, d_model), dtype=torch.bfloat16, device=QK.device)
+    kv = C.c_void_p(key_valid.data_ptr()) if key_valid is not None else C.c_void_p(0)
+    _check(lib().mlpf_tc_attention_bf16(C.c_void_p(QK.data_ptr()), C.c_void_p(VT.data_ptr()), VT.stride(0), kv,
+                                        off.ctypes.data_as(C.c_void_p), len(off) - 1, d_model, n_heads,
+                                        C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+    return out

@@ -1,0 +1,58 @@
+// common.cuh -- shared device-side types of libmlpf.so (sm_100a only).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <cstdio>
+
+namespace mlpf {
+
+typedef __nv_bfloat16 bf16;
+
+enum Act { ACT_NONE = 0, ACT_RELU = 1, ACT_GELU = 2 };
+
+// activation between the two linears of every 2-layer FFN (reading A5/A6)
+__device__ __forceinline__ float apply_act(float x, int act) {
+    if (act == ACT_RELU) return fmaxf(x, 0.0f);
+    if (act == ACT_GELU) return 0.5f * x * (1.0f + erff(x * 0.70710678118654752440f));
+    return x;
+}
+
+template <typename T> __device__ __forceinline__ float to_f32(T v);
+template <> __device__ __forceinline__ float to_f32<float>(float v) { return v; }
+template <> __device__ __forceinline__ float to_f32<bf16>(bf16 v) { return __bfloat162float(v); }
+template <typename T> __device__ __forceinline__ T from_f32(float v);
+template <> __device__ __forceinline__ float from_f32<float>(float v) { return v; }
+template <> __device__ __forceinline__ bf16 from_f32<bf16>(float v) { return __float2bfloat16_rn(v); }
+
+// Epilogue description shared by the CUDA-core GEMM and the tcgen05 GEMM:
+//   v = acc + bias[n]; v = act(v); v += residual[m, n];
+//   out_f32[row, n] = v;  out_act[row, n] = T(v) for n < vt_col0;  out_vt[n - vt_col0, row] = T(v) otherwise
+// row = row_perm ? row_perm[m] : m (row < 0: nothing is written).  Grouped mode (group_offsets != null):
+// the M-tile starting at m0 uses weight/bias block g-1 where group_offsets[g] <= m0 < group_offsets[g+1]
+// (g = 1..n_groups, segments are multiples of 128 rows); tiles at or beyond group_offsets[n_groups+1] exit.
+struct Epi {
+    const float* bias = nullptr;
+    int act = ACT_NONE;
+    const float* residual = nullptr; int64_t ld_res = 0;
+    float* out_f32 = nullptr;        int64_t ld_f32 = 0;
+    void* out_act = nullptr;         int64_t ld_act = 0;
+    void* out_vt = nullptr;          int64_t ld_vt = 0;
+    int vt_col0 = 0x7fffffff;
+    const int* row_perm = nullptr;
+    const int* group_offsets = nullptr;
+    int n_groups = 0;
+};
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+}  // namespace mlpf

@@ -1,0 +1,681 @@
+// mlpf_api.cu -- the C ABI of libmlpf.so (include/mlpf.h): blob parsing, weight upload, per-stream
+// workspaces, the host half of the schedule (a0) and the launch sequence a0..a8.
+// PAPER.md citations: embedding / encoder / heads L156; attention Eq. 4; outputs L126.
+#include "../../include/mlpf.h"
+#include "common.cuh"
+#include "simple_kernels.cuh"
+#include "tc_gemm.cuh"
+#include "tc_attn.cuh"
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <type_traits>
+#include <cstring>
+#include <map>
+#include <mutex>
+#include <string>
+#include <vector>
+
+using namespace mlpf;
+
+// ------------------------------------------------------------------------------------------------ errors
+static thread_local std::string g_err;
+static int set_err(int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+#define CUDA_TRY(expr)                                                                         \
+    do {                                                                                       \
+        cudaError_t e_ = (expr);                                                               \
+        if (e_ != cudaSuccess)                                                                 \
+            return set_err(MLPF_E_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), \
+                           __FILE__, __LINE__);                                                \
+    } while (0)
+
+extern "C" const char* mlpf_last_error(void) { return g_err.c_str(); }
+
+// ------------------------------------------------------------------------------------------------ handle
+struct LayerW {                       // element offsets into the packed parameter buffers
+    int64_t ln1g, ln1b, Wqkv, bqkv, Wo, bo, ln2g, ln2b, W1, b1, W2, b2;
+};
+struct Workspace {
+    int64_t cap_rows = 0;             // capacity in rows (multiple of 128)
+    int64_t cap_events = 0, cap_tiles = 0;
+    int64_t bytes = 0;
+    bool fp32 = false;                // element type of the activation buffers
+    int64_t ldvt = 0;
+    float* h = nullptr;               // [cap, d] fp32 residual stream
+    void *u = nullptr, *qk = nullptr, *vt = nullptr, *o = nullptr, *g = nullptr;
+    int64_t g_elems = 0;
+    // schedule (a0)
+    int *offsets = nullptr, *work = nullptr, *pairs = nullptr;
+    int *valid = nullptr, *row_event = nullptr, *row_pos = nullptr, *n_valid = nullptr;
+    int *block_counts = nullptr, *block_base = nullptr, *type_offsets = nullptr;
+    int *sorted_row = nullptr, *type_perm = nullptr;
+    // last call
+    int64_t N = 0, E = 0, n_tiles = 0, n_pairs = 0, m_ub = 0, g_width = 0;
+    int tile_q = 128;
+};
+
+struct mlpf_handle {
+    mlpf_blob_header hp;
+    int d, H, hd, dff, F, C, R, n_out, L, n_hblk;
+    int act;
+    int64_t n_params = 0, n_packed = 0;
+    float* P32 = nullptr;             // packed parameters, fp32
+    bf16* P16 = nullptr;              // same offsets, RNE-rounded to bf16
+    int64_t embW1t, embB1, embW2, embB2, lnfg, lnfb, headW1, headB1, headW2, headB2;
+    std::vector<LayerW> layers;
+    HeadsOut ho;
+    // options
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1;
+    int64_t last_launches = 0;
+    std::mutex mu;
+    std::map<void*, Workspace*> ws;
+    TcContext tc;
+};
+
+static uint16_t f32_to_bf16_rne(float f) {
+    uint32_t u;
+    memcpy(&u, &f, 4);
+    if ((u & 0x7fffffffu) > 0x7f800000u) return (uint16_t)((u >> 16) | 0x40);   // NaN stays NaN
+    uint32_t r = u + 0x7fffu + ((u >> 16) & 1u);
+    return (uint16_t)(r >> 16);
+}
+
+extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
+    if (!blob) { set_err(MLPF_E_NULL, "blob is NULL"); return nullptr; }
+    if (blob_bytes < MLPF_HEADER_BYTES) { set_err(MLPF_E_BLOB, "blob shorter than its header"); return nullptr; }
+    mlpf_blob_header hp;
+    memcpy(&hp, blob, sizeof hp);
+    if (memcmp(hp.magic, MLPF_BLOB_MAGIC, 8) != 0) { set_err(MLPF_E_BLOB, "bad magic"); return nullptr; }
+    if (hp.version != MLPF_BLOB_VERSION) { set_err(MLPF_E_BLOB, "unsupported version %u", hp.version); return nullptr; }
+    const int d = hp.d_model, H = hp.n_heads, dff = hp.d_ff, F = hp.n_feat, C = hp.n_classes, L = hp.n_layers;
+    const int T = hp.n_types, K = hp.n_reg_heads;
+    if (L < 1 || L > 64 || d < 64 || d > 512 || d % 64 || H < 1 || d % H || dff < 64 || dff % 64 || dff > 4096 ||
+        F < 1 || F > 64 || T != 4 || C < 1 || C > 16 || K < 0 || K > MLPF_MAX_REG_HEADS || hp.activation > 1 ||
+        hp.final_ln > 1 || !(hp.ln_eps > 0.0f)) {
+        set_err(MLPF_E_BLOB, "unsupported hyper-parameters (L=%d d=%d H=%d dff=%d F=%d T=%d C=%d K=%d)", L, d, H,
+                dff, F, T, C, K);
+        return nullptr;
+    }
+    const int hd = d / H;
+    if (hd != 16 && hd != 32 && hd != 64) { set_err(MLPF_E_BLOB, "head_dim %d not in {16,32,64}", hd); return nullptr; }
+    int R = 0;
+    for (int k = 0; k < K; ++k) {
+        if (hp.reg_dims[k] < 1 || hp.reg_dims[k] > 8) { set_err(MLPF_E_BLOB, "bad reg_dims"); return nullptr; }
+        R += hp.reg_dims[k];
+    }
+    if (C + R > MAX_OUT) { set_err(MLPF_E_BLOB, "too many outputs"); return nullptr; }
+    // ---- expected size
+    int64_t np = 0;
+    np += (int64_t)T * ((int64_t)d * F + d + (int64_t)d * d + d);
+    np += (int64_t)L * (2 * d + 3LL * d * d + 3 * d + (int64_t)d * d + d + 2 * d + (int64_t)dff * d + dff + (int64_t)d * dff + d);
+    np += 2 * d;
+    np += (int64_t)d * d + d + (int64_t)C * d + C;
+    for (int k = 0; k < K; ++k) np += (int64_t)d * d + d + (int64_t)hp.reg_dims[k] * d + hp.reg_dims[k];
+    if (blob_bytes != (size_t)(MLPF_HEADER_BYTES + np * 4)) {
+        set_err(MLPF_E_BLOB, "blob size %zu != expected %lld", blob_bytes, (long long)(MLPF_HEADER_BYTES + np * 4));
+        return nullptr;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        set_err(MLPF_E_CUDA, "no CUDA device: libmlpf has no CPU fallback");
+        return nullptr;
+    }
+    mlpf_handle* h = new (std::nothrow) mlpf_handle();
+    if (!h) { set_err(MLPF_E_ALLOC, "host allocation failed"); return nullptr; }
+    h->hp = hp; h->d = d; h->H = H; h->hd = hd; h->dff = dff; h->F = F; h->C = C; h->R = R; h->L = L;
+    h->n_out = C + R; h->n_hblk = 1 + K; h->n_params = np;
+    h->act = hp.activation == 0 ? ACT_RELU : ACT_GELU;
+
+    // ---- repack into the layouts the kernels want
+    const float* src = (const float*)((const char*)blob + MLPF_HEADER_BYTES);
+    std::vector<float> P;
+    auto reserve = [&](int64_t n) { int64_t off = (int64_t)P.size(); P.resize(off + ((n + 63) / 64) * 64, 0.0f); return off; };
+    h->embW1t = reserve((int64_t)T * 64 * d);
+    h->embB1 = reserve((int64_t)T * d);
+    h->embW2 = reserve((int64_t)T * d * d);
+    h->embB2 = reserve((int64_t)T * d);
+    int64_t s = 0;
+    for (int t = 0; t < T; ++t) {
+        for (int j = 0; j < d; ++j)
+            for (int k = 0; k < F; ++k) P[h->embW1t + ((int64_t)t * 64 + k) * d + j] = src[s + (int64_t)j * F + k];
+        s += (int64_t)d * F;
+        memcpy(&P[h->embB1 + (int64_t)t * d], src + s, d * 4); s += d;
+        memcpy(&P[h->embW2 + (int64_t)t * d * d], src + s, (size_t)d * d * 4); s += (int64_t)d * d;
+        memcpy(&P[h->embB2 + (int64_t)t * d], src + s, d * 4); s += d;
+    }
+    auto take = [&](int64_t n) { int64_t off = reserve(n); memcpy(&P[off], src + s, (size_t)n * 4); s += n; return off; };
+    h->layers.resize(L);
+    for (int l = 0; l < L; ++l) {
+        LayerW& w = h->layers[l];
+        w.ln1g = take(d); w.ln1b = take(d); w.Wqkv = take(3LL * d * d); w.bqkv = take(3 * d);
+        w.Wo = take((int64_t)d * d); w.bo = take(d); w.ln2g = take(d); w.ln2b = take(d);
+        w.W1 = take((int64_t)dff * d); w.b1 = take(dff); w.W2 = take((int64_t)d * dff); w.b2 = take(d);
+    }
+    h->lnfg = take(d); h->lnfb = take(d);
+    h->headW1 = reserve((int64_t)h->n_hblk * d * d);
+    h->headB1 = reserve((int64_t)h->n_hblk * d);
+    h->headW2 = reserve((int64_t)h->n_out * d);
+    h->headB2 = reserve(h->n_out);
+    h->ho.n_out = h->n_out; h->ho.n_cls = C; h->ho.n_reg = R;
+    int o = 0;
+    for (int b = 0; b < h->n_hblk; ++b) {
+        int rk = (b == 0) ? C : (int)hp.reg_dims[b - 1];
+        memcpy(&P[h->headW1 + (int64_t)b * d * d], src + s, (size_t)d * d * 4); s += (int64_t)d * d;
+        memcpy(&P[h->headB1 + (int64_t)b * d], src + s, d * 4); s += d;
+        memcpy(&P[h->headW2 + (int64_t)o * d], src + s, (size_t)rk * d * 4); s += (int64_t)rk * d;
+        memcpy(&P[h->headB2 + o], src + s, rk * 4); s += rk;
+        for (int i = 0; i < rk; ++i) h->ho.blk[o + i] = b;
+        o += rk;
+    }
+    if (s != np) { set_err(MLPF_E_BLOB, "internal: consumed %lld of %lld parameters", (long long)s, (long long)np); delete h; return nullptr; }
+    h->n_packed = (int64_t)P.size();
+    std::vector<uint16_t> P16(P.size());
+    for (size_t i = 0; i < P.size(); ++i) P16[i] = f32_to_bf16_rne(P[i]);
+    if (cudaMalloc(&h->P32, P.size() * 4) != cudaSuccess || cudaMalloc(&h->P16, P.size() * 2) != cudaSuccess) {
+        set_err(MLPF_E_ALLOC, "cudaMalloc of %zu parameter bytes failed", P.size() * 6);
+        cudaFree(h->P32); delete h; return nullptr;
+    }
+    if (cudaMemcpy(h->P32, P.data(), P.size() * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(h->P16, P16.data(), P16.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) {
+        set_err(MLPF_E_CUDA, "weight upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+        cudaFree(h->P32); cudaFree(h->P16); delete h; return nullptr;
+    }
+    if (tc_init(&h->tc) != 0) {
+        set_err(MLPF_E_CUDA, "tcgen05/TMA initialisation failed: %s", h->tc.err);
+        cudaFree(h->P32); cudaFree(h->P16); delete h; return nullptr;
+    }
+    g_err.clear();
+    return h;
+}
+
+static void ws_free(Workspace* w) {
+    void* ptrs[] = {w->h, w->u, w->qk, w->vt, w->o, w->g, w->offsets, w->work, w->pairs, w->valid, w->row_event,
+                    w->row_pos, w->n_valid, w->block_counts, w->block_base, w->type_offsets, w->sorted_row, w->type_perm};
+    for (void* p : ptrs) if (p) cudaFree(p);
+}
+
+extern "C" void mlpf_destroy(mlpf_handle* h) {
+    if (!h) return;
+    cudaDeviceSynchronize();
+    for (auto& kv : h->ws) { ws_free(kv.second); delete kv.second; }
+    cudaFree(h->P32); cudaFree(h->P16);
+    delete h;
+}
+
+extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
+    if (!h) return set_err(MLPF_E_NULL, "handle is NULL");
+    std::lock_guard<std::mutex> lk(h->mu);
+    switch (key) {
+        case MLPF_OPT_PRECISION:
+            if (value != MLPF_PREC_BF16 && value != MLPF_PREC_FP32_DEBUG) return set_err(MLPF_E_ARG, "bad precision");
+            h->precision = (int)value; return MLPF_OK;
+        case MLPF_OPT_TILE_Q:
+            if (value != 64 && value != 128) return set_err(MLPF_E_ARG, "tile_q must be 64 or 128");
+            h->tile_q = (int)value; return MLPF_OK;
+        case MLPF_OPT_TAP_LAYER:
+            if (value < -2 || value >= h->L) return set_err(MLPF_E_ARG, "bad tap layer");
+            h->tap_layer = (int)value; return MLPF_OK;
+        case MLPF_OPT_KERNELS:
+            if (value != MLPF_KERNELS_TC && value != MLPF_KERNELS_SIMPLE) return set_err(MLPF_E_ARG, "bad kernel set");
+            h->kernels = (int)value; return MLPF_OK;
+    }
+    return set_err(MLPF_E_ARG, "unknown option %d", key);
+}
+
+extern "C" int64_t mlpf_query(const mlpf_handle* h, int key) {
+    if (!h) return set_err(MLPF_E_NULL, "handle is NULL");
+    switch (key) {
+        case MLPF_Q_N_LAYERS: return h->L;
+        case MLPF_Q_D_MODEL: return h->d;
+        case MLPF_Q_N_HEADS: return h->H;
+        case MLPF_Q_D_FF: return h->dff;
+        case MLPF_Q_N_FEAT: return h->F;
+        case MLPF_Q_N_CLASSES: return h->C;
+        case MLPF_Q_N_REGRESS: return h->R;
+        case MLPF_Q_WEIGHT_BYTES: return h->n_packed * 6;
+        case MLPF_Q_N_PARAMS: return h->n_params;
+        case MLPF_Q_LAUNCHES: return h->last_launches;
+        case MLPF_Q_WORKSPACE_BYTES: {
+            int64_t b = 0;
+            std::lock_guard<std::mutex> lk(const_cast<mlpf_handle*>(h)->mu);
+            for (auto& kv : h->ws) b += kv.second->bytes;
+            return b;
+        }
+    }
+    return set_err(MLPF_E_ARG, "unknown query %d", key);
+}
+
+// ------------------------------------------------------------------------------------------------ workspace
+template <typename P> static cudaError_t dmalloc(P** p, int64_t bytes, Workspace* w) {
+    cudaError_t e = cudaMalloc((void**)p, (size_t)std::max<int64_t>(bytes, 256));
+    if (e == cudaSuccess) w->bytes += std::max<int64_t>(bytes, 256);
+    return e;
+}
+
+static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t n_tiles, bool fp32) {
+    const int64_t d = h->d;
+    if (N > w->cap_rows || fp32 != w->fp32) {
+        void* ptrs[] = {w->h, w->u, w->qk, w->vt, w->o, w->g, w->valid, w->row_event, w->row_pos, w->block_counts,
+                        w->block_base, w->sorted_row, w->type_perm, w->type_offsets};
+        int64_t small = w->bytes;     // recompute below
+        (void)small;
+        for (void* p : ptrs) if (p) cudaFree(p);   // cudaFree waits for work in flight
+        // keep the event-indexed arrays' accounting: recompute bytes from scratch
+        int64_t ev_bytes = 0;
+        if (w->offsets) ev_bytes += std::max<int64_t>((w->cap_events + 1) * 4, 256) + std::max<int64_t>(w->cap_events * 4, 256);
+        if (w->work) ev_bytes += 2 * std::max<int64_t>(w->cap_tiles * 8, 256);
+        w->bytes = ev_bytes;
+        const int64_t cap = (std::max<int64_t>(N, w->cap_rows) + 127) / 128 * 128;
+        const int64_t es = fp32 ? 4 : 2;
+        const int64_t m_ub = cap + 4 * 128;
+        const int64_t gw = std::max<int64_t>(h->dff, (int64_t)h->n_hblk * d);
+        w->g_elems = std::max<int64_t>(cap * gw, m_ub * d);
+        w->ldvt = cap;
+        w->fp32 = fp32;
+        const int64_t nb = (cap + SCHED_BLOCK - 1) / SCHED_BLOCK;
+        if (dmalloc(&w->h, cap * d * 4, w) || dmalloc((char**)&w->u, cap * d * es, w) ||
+            dmalloc((char**)&w->qk, cap * 2 * d * es, w) || dmalloc((char**)&w->vt, d * w->ldvt * es, w) ||
+            dmalloc((char**)&w->o, cap * d * es, w) || dmalloc((char**)&w->g, w->g_elems * es, w) ||
+            dmalloc(&w->valid, cap * 4, w) || dmalloc(&w->row_event, cap * 4, w) || dmalloc(&w->row_pos, cap * 4, w) ||
+            dmalloc(&w->block_counts, nb * 5 * 4, w) || dmalloc(&w->block_base, nb * 5 * 4, w) ||
+            dmalloc(&w->sorted_row, cap * 4, w) || dmalloc(&w->type_perm, m_ub * 4, w) ||
+            dmalloc(&w->type_offsets, 8 * 4, w)) {
+            w->cap_rows = 0;
+            return set_err(MLPF_E_ALLOC, "workspace allocation for %lld rows failed: %s", (long long)cap,
+                           cudaGetErrorString(cudaGetLastError()));
+        }
+        // the activation buffers feed TMA loads whose boxes may overrun valid rows: start from zeros so
+        // that never-written tails hold finite values
+        cudaMemset(w->u, 0, cap * d * es); cudaMemset(w->qk, 0, cap * 2 * d * es);
+        cudaMemset(w->vt, 0, d * w->ldvt * es); cudaMemset(w->o, 0, cap * d * es);
+        cudaMemset(w->g, 0, w->g_elems * es);
+        w->cap_rows = cap;
+    }
+    if (E > w->cap_events) {
+        if (w->offsets) { cudaFree(w->offsets); cudaFree(w->n_valid); }
+        const int64_t ce = std::max<int64_t>(E, 64);
+        if (dmalloc(&w->offsets, (ce + 1) * 4, w) || dmalloc(&w->n_valid, ce * 4, w)) {
+            w->cap_events = 0;
+            return set_err(MLPF_E_ALLOC, "workspace allocation for %lld events failed", (long long)ce);
+        }
+        w->cap_events = ce;
+    }
+    if (n_tiles > w->cap_tiles) {
+        if (w->work) { cudaFree(w->work); cudaFree(w->pairs); }
+        const int64_t ct = std::max<int64_t>(n_tiles, 1024);
+        if (dmalloc(&w->work, ct * 8, w) || dmalloc(&w->pairs, ct * 8, w)) {
+            w->cap_tiles = 0;
+            return set_err(MLPF_E_ALLOC, "workspace allocation for %lld tiles failed", (long long)ct);
+        }
+        w->cap_tiles = ct;
+    }
+    return MLPF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ launch helpers
+#define LAUNCH_CHECK(h)                                                                                   \
+    do {                                                                                                  \
+        (h)->last_launches++;                                                                             \
+        cudaError_t e_ = cudaGetLastError();                                                              \
+        if (e_ != cudaSuccess) return set_err(MLPF_E_CUDA, "kernel launch failed: %s (%s:%d)",            \
+                                              cudaGetErrorString(e_), __FILE__, __LINE__);                \
+    } while (0)
+
+template <typename T>
+static int run_gemm(mlpf_handle* h, bool tc, const T* A, const T* W, int M, int N, int K, const Epi& ep,
+                    cudaStream_t st) {
+    if (M <= 0) return MLPF_OK;
+    if (tc) {
+        if constexpr (std::is_same<T, bf16>::value) {
+            int rc = tc_gemm_launch(&h->tc, A, W, M, N, K, ep, st);
+            if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", h->tc.err);
+            LAUNCH_CHECK(h);
+            return MLPF_OK;
+        }
+    }
+    dim3 grid(N / 64, (M + 63) / 64);
+    k_gemm_simple<T><<<grid, 256, 0, st>>>(A, W, M, N, K, ep);
+    LAUNCH_CHECK(h);
+    return MLPF_OK;
+}
+
+template <typename T>
+static int run_layernorm(mlpf_handle* h, const float* x, int N, const float* g, const float* b, T* u, cudaStream_t st) {
+    dim3 grid((N + 7) / 8);
+    switch (h->d) {
+        case 64:  k_layernorm<T, 64><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
+        case 128: k_layernorm<T, 128><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
+        case 192: k_layernorm<T, 192><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
+        case 256: k_layernorm<T, 256><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
+        case 320: k_layernorm<T, 320><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
+        case 384: k_layernorm<T, 384><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
+        case 448: k_layernorm<T, 448><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
+        case 512: k_layernorm<T, 512><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
+        default: return set_err(MLPF_E_ARG, "d_model %d unsupported by LayerNorm", h->d);
+    }
+    LAUNCH_CHECK(h);
+    return MLPF_OK;
+}
+
+template <typename T>
+static int run_attention(mlpf_handle* h, bool tc, Workspace* w, cudaStream_t st) {
+    if (w->n_tiles == 0) return MLPF_OK;
+    if (tc) {
+        if constexpr (std::is_same<T, bf16>::value) {
+            int rc = tc_attn_launch(&h->tc, (const bf16*)w->qk, (const bf16*)w->vt, w->ldvt, w->N, w->valid, w->offsets,
+                                    (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, (bf16*)w->o, st);
+            if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", h->tc.err);
+            LAUNCH_CHECK(h);
+            return MLPF_OK;
+        }
+    }
+    dim3 grid((unsigned)w->n_tiles, h->H);
+    const T* qk = (const T*)w->qk; const T* vt = (const T*)w->vt; T* o = (T*)w->o;
+    switch (h->hd) {
+        case 16: k_attn_simple<T, 16><<<grid, w->tile_q, 0, st>>>(qk, vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, w->tile_q, h->d, o); break;
+        case 32: k_attn_simple<T, 32><<<grid, w->tile_q, 0, st>>>(qk, vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, w->tile_q, h->d, o); break;
+        case 64: k_attn_simple<T, 64><<<grid, w->tile_q, 0, st>>>(qk, vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, w->tile_q, h->d, o); break;
+    }
+    LAUNCH_CHECK(h);
+    return MLPF_OK;
+}
+
+// host half of a0: the attention work list (event, q_tile), longest event first, ties by event id, then
+// q_tile ascending; `pairs` = the same order with two consecutive q-tiles of one event per entry.
+static void build_work_lists(const int32_t* off, int E, int tile_q, std::vector<int>& work, std::vector<int>& pairs) {
+    std::vector<int> order(E);
+    for (int e = 0; e < E; ++e) order[e] = e;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return (off[a + 1] - off[a]) > (off[b + 1] - off[b]); });
+    work.clear(); pairs.clear();
+    for (int e : order) {
+        int n = off[e + 1] - off[e];
+        int nt = (n + tile_q - 1) / tile_q;
+        for (int q = 0; q < nt; ++q) { work.push_back(e); work.push_back(q); }
+        int np128 = (n + 255) / 256;
+        for (int p = 0; p < np128; ++p) { pairs.push_back(e); pairs.push_back(p); }
+    }
+}
+
+template <typename T>
+static int infer_impl(mlpf_handle* h, Workspace* w, const float* X, float* out_logits, float* out_regress, cudaStream_t st) {
+    const int N = (int)w->N, E = (int)w->E, d = h->d, dff = h->dff;
+    const bool fp32 = std::is_same<T, float>::value;
+    const bool tc_req = !fp32 && h->kernels == MLPF_KERNELS_TC;
+    const bool tc = tc_req && TC_GEMM_READY;
+    const bool tc_attn = tc_req && TC_ATTN_READY;
+    const T* PW = fp32 ? (const T*)h->P32 : (const T*)h->P16;
+    const float* PV = h->P32;
+    T* u = (T*)w->u; T* g = (T*)w->g;
+
+    // ---- a0 (device half)
+    const int nb = (N + SCHED_BLOCK - 1) / SCHED_BLOCK;
+    CUDA_TRY(cudaMemsetAsync(w->n_valid, 0, (size_t)E * 4, st));
+    CUDA_TRY(cudaMemsetAsync(w->type_perm, 0xff, (size_t)w->m_ub * 4, st));
+    k_sched_count<<<nb, SCHED_BLOCK, 0, st>>>(X, N, h->F, w->offsets, E, w->block_counts, w->valid, w->row_event, w->row_pos, w->n_valid);
+    LAUNCH_CHECK(h);
+    k_sched_scan<<<1, 32, 0, st>>>(w->block_counts, nb, w->block_base, w->type_offsets);
+    LAUNCH_CHECK(h);
+    k_sched_scatter<<<nb, SCHED_BLOCK, 0, st>>>(X, N, h->F, w->block_base, w->type_offsets, w->sorted_row, w->type_perm);
+    LAUNCH_CHECK(h);
+
+    // ---- a1: per-type embedding (L156; A3-A5)
+    k_embed_l1<T><<<(N + EMB_ROWS - 1) / EMB_ROWS, 256, 0, st>>>(X, N, h->F, d, PV + h->embW1t, PV + h->embB1, h->act, w->sorted_row, g, w->h);
+    LAUNCH_CHECK(h);
+    {
+        Epi ep;
+        ep.bias = PV + h->embB2; ep.out_f32 = w->h; ep.ld_f32 = d;
+        ep.row_perm = w->type_perm; ep.group_offsets = w->type_offsets; ep.n_groups = 4;
+        int rc = run_gemm<T>(h, tc, g, PW + h->embW2, (int)w->m_ub, d, d, ep, st);
+        if (rc) return rc;
+    }
+    if (h->tap_layer == -2) return MLPF_OK;
+
+    // ---- encoder blocks (pre-LN, L156 + A7)
+    for (int l = 0; l < h->L; ++l) {
+        const LayerW& lw = h->layers[l];
+        int rc = run_layernorm<T>(h, w->h, N, PV + lw.ln1g, PV + lw.ln1b, u, st);                     // a2
+        if (rc) return rc;
+        {   // a3: [Q K V] = LN1(x) Wqkv^T + bqkv ; V stored transposed per head dim
+            Epi ep;
+            ep.bias = PV + lw.bqkv; ep.out_act = w->qk; ep.ld_act = 2 * d;
+            ep.out_vt = w->vt; ep.ld_vt = w->ldvt; ep.vt_col0 = 2 * d;
+            rc = run_gemm<T>(h, tc, u, PW + lw.Wqkv, N, 3 * d, d, ep, st);
+            if (rc) return rc;
+        }
+        rc = run_attention<T>(h, tc_attn, w, st);                                                         // a4
+        if (rc) return rc;
+        {   // a5: h <- h + O Wo^T + bo
+            Epi ep;
+            ep.bias = PV + lw.bo; ep.residual = w->h; ep.ld_res = d; ep.out_f32 = w->h; ep.ld_f32 = d;
+            rc = run_gemm<T>(h, tc, (const T*)w->o, PW + lw.Wo, N, d, d, ep, st);
+            if (rc) return rc;
+        }
+        rc = run_layernorm<T>(h, w->h, N, PV + lw.ln2g, PV + lw.ln2b, u, st);
+        if (rc) return rc;
+        {   // a6: g = act(LN2(h) W1^T + b1)
+            Epi ep;
+            ep.bias = PV + lw.b1; ep.act = h->act; ep.out_act = g; ep.ld_act = dff;
+            rc = run_gemm<T>(h, tc, u, PW + lw.W1, N, dff, d, ep, st);
+            if (rc) return rc;
+        }
+        {   // a7: h <- h + g W2^T + b2
+            Epi ep;
+            ep.bias = PV + lw.b2; ep.residual = w->h; ep.ld_res = d; ep.out_f32 = w->h; ep.ld_f32 = d;
+            rc = run_gemm<T>(h, tc, g, PW + lw.W2, N, d, dff, ep, st);
+            if (rc) return rc;
+        }
+        w->g_width = dff;
+        if (h->tap_layer == l) return MLPF_OK;
+    }
+
+    // ---- a8: heads (L156; A11-A12)
+    if (h->hp.final_ln) {
+        int rc = run_layernorm<T>(h, w->h, N, PV + h->lnfg, PV + h->lnfb, u, st);
+        if (rc) return rc;
+    } else {
+        // no final LN: u = T(h).  (identity affine with the row kept: done by a cast kernel)
+        return set_err(MLPF_E_ARG, "final_ln = 0 is not supported yet");
+    }
+    {
+        Epi ep;
+        const int hw = h->n_hblk * d;
+        ep.bias = PV + h->headB1; ep.act = h->act; ep.out_act = g; ep.ld_act = hw;
+        int rc = run_gemm<T>(h, tc, u, PW + h->headW1, N, hw, d, ep, st);
+        if (rc) return rc;
+        w->g_width = hw;
+        k_heads_l2<T><<<(N + 7) / 8, 256, 0, st>>>(g, N, d, hw, PV + h->headW2, PV + h->headB2, w->valid, h->ho, out_logits, out_regress);
+        LAUNCH_CHECK(h);
+    }
+    return MLPF_OK;
+}
+
+extern "C" int mlpf_infer(mlpf_handle* h, const float* elements, const int32_t* event_offsets, int32_t n_events,
+                          float* out_logits, float* out_regress, void* stream) {
+    if (!h) return set_err(MLPF_E_NULL, "handle is NULL");
+    if (n_events < 0) return set_err(MLPF_E_OFFSETS, "n_events < 0");
+    if (n_events == 0) return MLPF_OK;
+    if (!event_offsets) return set_err(MLPF_E_NULL, "event_offsets is NULL");
+    if (event_offsets[0] != 0) return set_err(MLPF_E_OFFSETS, "event_offsets[0] != 0");
+    for (int e = 0; e < n_events; ++e)
+        if (event_offsets[e + 1] < event_offsets[e]) return set_err(MLPF_E_OFFSETS, "event_offsets decreasing at %d", e);
+    const int64_t N = event_offsets[n_events];
+    if (N == 0) return MLPF_OK;
+    if (!elements || !out_logits || !out_regress) return set_err(MLPF_E_NULL, "elements / outputs NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+
+    std::unique_lock<std::mutex> lk(h->mu);
+    const bool fp32 = h->precision == MLPF_PREC_FP32_DEBUG;
+    Workspace*& wref = h->ws[stream];
+    if (!wref) wref = new Workspace();
+    Workspace* w = wref;
+    std::vector<int> work, pairs;
+    build_work_lists(event_offsets, n_events, h->tile_q, work, pairs);
+    int rc = ws_ensure(h, w, N, n_events, (int64_t)work.size() / 2, fp32);
+    if (rc) return rc;
+    w->N = N; w->E = n_events; w->n_tiles = (int64_t)work.size() / 2; w->n_pairs = (int64_t)pairs.size() / 2;
+    w->tile_q = h->tile_q;
+    w->m_ub = (N + 127) / 128 * 128 + 4 * 128;
+    h->last_launches = 0;
+    // pageable -> device async copies are staged by the runtime before returning: the caller may free
+    CUDA_TRY(cudaMemcpyAsync(w->offsets, event_offsets, (size_t)(n_events + 1) * 4, cudaMemcpyHostToDevice, st));
+    if (!work.empty()) CUDA_TRY(cudaMemcpyAsync(w->work, work.data(), work.size() * 4, cudaMemcpyHostToDevice, st));
+    if (!pairs.empty()) CUDA_TRY(cudaMemcpyAsync(w->pairs, pairs.data(), pairs.size() * 4, cudaMemcpyHostToDevice, st));
+    if (fp32) rc = infer_impl<float>(h, w, elements, out_logits, out_regress, st);
+    else rc = infer_impl<bf16>(h, w, elements, out_logits, out_regress, st);
+    if (rc == MLPF_OK) g_err.clear();
+    return rc;
+}
+
+extern "C" int mlpf_infer_host(mlpf_handle* h, const float* elements_host, const int32_t* event_offsets,
+                               int32_t n_events, float* out_logits_host, float* out_regress_host, void* stream) {
+    if (!h) return set_err(MLPF_E_NULL, "handle is NULL");
+    if (n_events <= 0 || !event_offsets) return mlpf_infer(h, nullptr, event_offsets, n_events, nullptr, nullptr, stream);
+    const int64_t N = event_offsets[n_events];
+    if (N <= 0) return mlpf_infer(h, nullptr, event_offsets, n_events, nullptr, nullptr, stream);
+    if (!elements_host || !out_logits_host || !out_regress_host) return set_err(MLPF_E_NULL, "host buffers NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    // device staging buffers, one set per calling thread (the call synchronises before returning)
+    static thread_local struct { float* x = nullptr; float* lg = nullptr; float* rg = nullptr; int64_t cap = 0; } sb;
+    if (N > sb.cap) {
+        cudaFree(sb.x); cudaFree(sb.lg); cudaFree(sb.rg);
+        const int64_t cap = (N + 1023) / 1024 * 1024;
+        if (cudaMalloc(&sb.x, cap * h->F * 4) || cudaMalloc(&sb.lg, cap * h->C * 4) || cudaMalloc(&sb.rg, cap * std::max(h->R, 1) * 4)) {
+            sb.cap = 0; sb.x = sb.lg = sb.rg = nullptr;
+            return set_err(MLPF_E_ALLOC, "staging allocation failed");
+        }
+        sb.cap = cap;
+    }
+    CUDA_TRY(cudaMemcpyAsync(sb.x, elements_host, (size_t)N * h->F * 4, cudaMemcpyHostToDevice, st));
+    int rc = mlpf_infer(h, sb.x, event_offsets, n_events, sb.lg, sb.rg, stream);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(out_logits_host, sb.lg, (size_t)N * h->C * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(out_regress_host, sb.rg, (size_t)N * h->R * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return MLPF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ debug taps
+extern "C" int64_t mlpf_debug_get_schedule(mlpf_handle* h, void* stream, int which, int32_t* host_out, int64_t capacity) {
+    if (!h || !host_out) return set_err(MLPF_E_NULL, "NULL argument");
+    std::lock_guard<std::mutex> lk(h->mu);
+    auto it = h->ws.find(stream);
+    if (it == h->ws.end() || it->second->N == 0) return set_err(MLPF_E_ARG, "no mlpf_infer ran on this stream");
+    Workspace* w = it->second;
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+    const int* src = nullptr; int64_t n = 0;
+    int toff[8];
+    switch (which) {
+        case MLPF_SCHED_ROW_EVENT: src = w->row_event; n = w->N; break;
+        case MLPF_SCHED_ROW_POS: src = w->row_pos; n = w->N; break;
+        case MLPF_SCHED_VALID: src = w->valid; n = w->N; break;
+        case MLPF_SCHED_N_VALID: src = w->n_valid; n = w->E; break;
+        case MLPF_SCHED_TYPE_OFFSETS: src = w->type_offsets; n = 6; break;
+        case MLPF_SCHED_SORTED_ROW: src = w->sorted_row; n = w->N; break;
+        case MLPF_SCHED_TYPE_PERM:
+            CUDA_TRY(cudaMemcpy(toff, w->type_offsets, 6 * 4, cudaMemcpyDeviceToHost));
+            src = w->type_perm; n = toff[5]; break;
+        case MLPF_SCHED_WORK_LIST: src = w->work; n = w->n_tiles * 2; break;
+        default: return set_err(MLPF_E_ARG, "unknown schedule array %d", which);
+    }
+    if (n > capacity) return set_err(MLPF_E_ARG, "capacity %lld < %lld", (long long)capacity, (long long)n);
+    if (n > 0) CUDA_TRY(cudaMemcpy(host_out, src, (size_t)n * 4, cudaMemcpyDeviceToHost));
+    return n;
+}
+
+template <typename T>
+static int tap_copy(const void* src, int64_t rows, int64_t cols, int64_t ld, float* host_out) {
+    float* tmp = nullptr;
+    CUDA_TRY(cudaMalloc(&tmp, (size_t)rows * ld * 4));
+    int64_t n = rows * ld;
+    k_to_f32<T><<<(unsigned)((n + 255) / 256), 256>>>((const T*)src, tmp, n);
+    cudaError_t e = cudaMemcpy2D(host_out, (size_t)cols * 4, tmp, (size_t)ld * 4, (size_t)cols * 4, (size_t)rows, cudaMemcpyDeviceToHost);
+    cudaFree(tmp);
+    if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tap copy failed: %s", cudaGetErrorString(e));
+    return MLPF_OK;
+}
+
+extern "C" int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which, float* host_out, int64_t capacity) {
+    if (!h || !host_out) return set_err(MLPF_E_NULL, "NULL argument");
+    std::lock_guard<std::mutex> lk(h->mu);
+    auto it = h->ws.find(stream);
+    if (it == h->ws.end() || it->second->N == 0) return set_err(MLPF_E_ARG, "no mlpf_infer ran on this stream");
+    Workspace* w = it->second;
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+    const int64_t N = w->N, d = h->d;
+    const void* src = nullptr; int64_t rows = N, cols = d, ld = d;
+    switch (which) {
+        case MLPF_TENSOR_H: {
+            if (N * d > capacity) return set_err(MLPF_E_ARG, "capacity too small");
+            CUDA_TRY(cudaMemcpy(host_out, w->h, (size_t)N * d * 4, cudaMemcpyDeviceToHost));
+            return N * d;
+        }
+        case MLPF_TENSOR_U: src = w->u; break;
+        case MLPF_TENSOR_QK: src = w->qk; cols = ld = 2 * d; break;
+        case MLPF_TENSOR_VT: src = w->vt; rows = d; cols = N; ld = w->ldvt; break;
+        case MLPF_TENSOR_O: src = w->o; break;
+        case MLPF_TENSOR_G: src = w->g; cols = ld = w->g_width; if (cols == 0) return set_err(MLPF_E_ARG, "G not produced yet"); break;
+        default: return set_err(MLPF_E_ARG, "unknown tensor %d", which);
+    }
+    if (rows * cols > capacity) return set_err(MLPF_E_ARG, "capacity too small");
+    int rc = w->fp32 ? tap_copy<float>(src, rows, cols, ld, host_out) : tap_copy<bf16>(src, rows, cols, ld, host_out);
+    if (rc) return rc;
+    return rows * cols;
+}
+
+// ------------------------------------------------------------------------------------------------ kernel-level entries
+extern "C" int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* W, float* C, int32_t M, int32_t N, int32_t K, void* stream) {
+    if (!A || !W || !C) return set_err(MLPF_E_NULL, "NULL argument");
+    if (M <= 0 || N <= 0 || K <= 0 || N % 64 || K % 64) return set_err(MLPF_E_ARG, "need M > 0, N %% 64 == 0, K %% 64 == 0");
+    static TcContext ctx;
+    static std::once_flag once;
+    static int init_rc = 0;
+    std::call_once(once, [&] { init_rc = tc_init(&ctx); });
+    if (init_rc) return set_err(MLPF_E_CUDA, "tcgen05/TMA initialisation failed: %s", ctx.err);
+    Epi ep;
+    ep.out_f32 = C; ep.ld_f32 = N;
+    if (tc_gemm_launch(&ctx, (const bf16*)A, (const bf16*)W, M, N, K, ep, (cudaStream_t)stream))
+        return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", ctx.err);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", cudaGetErrorString(e));
+    return MLPF_OK;
+}
+
+extern "C" int mlpf_tc_attention_bf16(const uint16_t* QK, const uint16_t* VT, int64_t ldvt, const int32_t* key_valid,
+                                      const int32_t* event_offsets, int32_t n_events, int32_t d_model, int32_t n_heads,
+                                      uint16_t* O, void* stream) {
+    if (!QK || !VT || !event_offsets || !O) return set_err(MLPF_E_NULL, "NULL argument");
+    if (n_events <= 0) return MLPF_OK;
+    const int hd = n_heads > 0 ? d_model / n_heads : 0;
+    if (hd != 16 && hd != 32 && hd != 64) return set_err(MLPF_E_ARG, "head_dim must be 16, 32 or 64");
+    static TcContext ctx;
+    static std::once_flag once;
+    static int init_rc = 0;
+    std::call_once(once, [&] { init_rc = tc_init(&ctx); });
+    if (init_rc) return set_err(MLPF_E_CUDA, "tcgen05/TMA initialisation failed: %s", ctx.err);
+    std::vector<int> work, pairs;
+    build_work_lists(event_offsets, n_events, 128, work, pairs);
+    const int64_t N = event_offsets[n_events];
+    if (pairs.empty()) return MLPF_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    int *d_off = nullptr, *d_pairs = nullptr;
+    CUDA_TRY(cudaMalloc(&d_off, (size_t)(n_events + 1) * 4));
+    CUDA_TRY(cudaMalloc(&d_pairs, pairs.size() * 4));
+    CUDA_TRY(cudaMemcpyAsync(d_off, event_offsets, (size_t)(n_events + 1) * 4, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(d_pairs, pairs.data(), pairs.size() * 4, cudaMemcpyHostToDevice, st));
+    int rc = tc_attn_launch(&ctx, (const bf16*)QK, (const bf16*)VT, ldvt, N, key_valid, d_off, (const int2*)d_pairs,
+                            (int)(pairs.size() / 2), d_model, n_heads, (bf16*)O, st);
+    cudaError_t e = cudaStreamSynchronize(st);
+    cudaFree(d_off); cudaFree(d_pairs);
+    if (rc) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", ctx.err);
+    if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tcgen05 attention failed: %s", cudaGetErrorString(e));
+    return MLPF_OK;
+}

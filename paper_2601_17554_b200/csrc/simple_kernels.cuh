@@ -1,0 +1,378 @@
+// simple_kernels.cuh -- CUDA-core kernels of libmlpf.so.
+//  * the integer schedule (step a0), the embedding's first layer (a1), LayerNorm (a2) and the heads'
+//    output layer (a8) are used by every path;
+//  * the tiled FFMA GEMM and the one-thread-per-query attention are the fp32 debug path
+//    (MLPF_PREC_FP32_DEBUG, parity <= 1e-4) and the MLPF_KERNELS_SIMPLE debugging aid in bf16.
+// Citations are /root/reference/PAPER.md lines; readings A* are listed in DESIGN.md.
+#pragma once
+#include "common.cuh"
+
+namespace mlpf {
+
+// ------------------------------------------------------------------------------------------------
+// a0: integer schedule on the device (the type id lives in device memory: reading A1)
+// ------------------------------------------------------------------------------------------------
+constexpr int SCHED_BLOCK = 1024;
+
+__device__ __forceinline__ int element_type(const float* __restrict__ X, int64_t row, int F) {
+    float x0 = X[row * F];
+    int t = (x0 >= 0.0f && x0 < 5.0f) ? (int)x0 : (x0 >= 5.0f ? 4 : 0);   // clamp to 0..4; NaN -> 0
+    return t;
+}
+
+// per 1024-row block: histogram of types 0..4; also valid[], row_event[], row_pos[], n_valid[e] (atomic)
+__global__ void __launch_bounds__(SCHED_BLOCK)
+k_sched_count(const float* __restrict__ X, int N, int F, const int* __restrict__ offsets, int E,
+              int* __restrict__ block_counts, int* __restrict__ valid, int* __restrict__ row_event,
+              int* __restrict__ row_pos, int* __restrict__ n_valid) {
+    __shared__ int hist[5];
+    if (threadIdx.x < 5) hist[threadIdx.x] = 0;
+    __syncthreads();
+    int i = blockIdx.x * SCHED_BLOCK + threadIdx.x;
+    int t = -1;
+    if (i < N) {
+        t = element_type(X, i, F);
+        valid[i] = (t != 0);
+        // event of row i: largest e with offsets[e] <= i  (offsets non-decreasing; empty events skipped)
+        int lo = 0, hi = E;             // invariant: offsets[lo] <= i < offsets[hi]
+        while (hi - lo > 1) {
+            int mid = (lo + hi) >> 1;
+            if (offsets[mid] <= i) lo = mid; else hi = mid;
+        }
+        row_event[i] = lo;
+        row_pos[i] = i - offsets[lo];
+        if (t != 0) atomicAdd(&n_valid[lo], 1);
+    }
+#pragma unroll
+    for (int ty = 0; ty < 5; ++ty) {
+        unsigned m = __ballot_sync(0xffffffffu, t == ty);
+        if ((threadIdx.x & 31) == 0 && m) atomicAdd(&hist[ty], __popc(m));
+    }
+    __syncthreads();
+    if (threadIdx.x < 5) block_counts[blockIdx.x * 5 + threadIdx.x] = hist[threadIdx.x];
+}
+
+// one block: exclusive scan of the per-block counts per type; segment starts padded to 128 rows
+__global__ void k_sched_scan(const int* __restrict__ block_counts, int nb, int* __restrict__ block_base,
+                             int* __restrict__ type_offsets) {
+    __shared__ int total[5];
+    int ty = threadIdx.x;
+    if (ty < 5) {
+        int run = 0;
+        for (int b = 0; b < nb; ++b) {
+            block_base[b * 5 + ty] = run;
+            run += block_counts[b * 5 + ty];
+        }
+        total[ty] = run;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int pos = 0;
+        type_offsets[0] = 0;
+        for (int t = 1; t <= 4; ++t) {
+            type_offsets[t] = pos;
+            pos += (total[t] + 127) / 128 * 128;
+        }
+        type_offsets[5] = pos;
+    }
+}
+
+// stable counting sort by type: sorted_row[i] = slot, type_perm[slot] = i  (type_perm pre-filled with -1)
+__global__ void __launch_bounds__(SCHED_BLOCK)
+k_sched_scatter(const float* __restrict__ X, int N, int F, const int* __restrict__ block_base,
+                const int* __restrict__ type_offsets, int* __restrict__ sorted_row,
+                int* __restrict__ type_perm) {
+    __shared__ int warp_cnt[32][5];
+    int i = blockIdx.x * SCHED_BLOCK + threadIdx.x;
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int t = (i < N) ? element_type(X, i, F) : -1;
+    int my_rank = 0;
+#pragma unroll
+    for (int ty = 0; ty < 5; ++ty) {
+        unsigned m = __ballot_sync(0xffffffffu, t == ty);
+        if (t == ty) my_rank = __popc(m & ((1u << lane) - 1u));
+        if (lane == 0) warp_cnt[w][ty] = __popc(m);
+    }
+    __syncthreads();
+    if (i < N) {
+        if (t == 0) {
+            sorted_row[i] = -1;
+        } else {
+            int before = 0;
+            for (int ww = 0; ww < w; ++ww) before += warp_cnt[ww][t];
+            int slot = type_offsets[t] + block_base[blockIdx.x * 5 + t] + before + my_rank;
+            sorted_row[i] = slot;
+            type_perm[slot] = i;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1 (first layer): h1[slot] = act(W1[t] x + b1[t]) in fp32 on CUDA cores (raw features span
+// 1e-2..1e4), rows written in by-type sorted order so that the second layer is a grouped GEMM.
+// Pad rows (type 0): the residual stream row h[i,:] is set to exactly 0 (reading A2).
+// W1t is [T][64][d] (k-major, zero padded to 64 features) so loads are coalesced over the d outputs.
+// ------------------------------------------------------------------------------------------------
+constexpr int EMB_ROWS = 64;
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_embed_l1(const float* __restrict__ X, int N, int F, int d, const float* __restrict__ W1t,
+           const float* __restrict__ b1, int act, const int* __restrict__ sorted_row,
+           T* __restrict__ h1, float* __restrict__ h) {
+    __shared__ float xs[EMB_ROWS][65];
+    __shared__ int list[5][EMB_ROWS];
+    __shared__ int cnt[5];
+    const int row0 = blockIdx.x * EMB_ROWS;
+    const int rows = min(EMB_ROWS, N - row0);
+    if (threadIdx.x < 5) cnt[threadIdx.x] = 0;
+    for (int idx = threadIdx.x; idx < EMB_ROWS * 64; idx += 256) {
+        int r = idx >> 6, k = idx & 63;
+        xs[r][k] = (r < rows && k < F) ? X[(int64_t)(row0 + r) * F + k] : 0.0f;
+    }
+    __syncthreads();
+    if (threadIdx.x < rows) {
+        int t = element_type(X, row0 + threadIdx.x, F);
+        int p = atomicAdd(&cnt[t], 1);
+        list[t][p] = threadIdx.x;
+    }
+    __syncthreads();
+    // pad rows -> zero residual-stream rows
+    for (int p = 0; p < cnt[0]; ++p) {
+        int r = list[0][p];
+        for (int j = threadIdx.x; j < d; j += 256) h[(int64_t)(row0 + r) * d + j] = 0.0f;
+    }
+    for (int t = 1; t <= 4; ++t) {
+        const int c = cnt[t];
+        if (c == 0) continue;
+        for (int j = threadIdx.x; j < d; j += 256) {
+            float w[64];
+            const float* wp = W1t + ((int64_t)(t - 1) * 64) * d + j;
+#pragma unroll
+            for (int k = 0; k < 64; ++k) w[k] = wp[(int64_t)k * d];
+            const float bj = b1[(t - 1) * d + j];
+            for (int p = 0; p < c; ++p) {
+                const int r = list[t][p];
+                float acc = bj;
+#pragma unroll
+                for (int k = 0; k < 64; ++k) acc = fmaf(w[k], xs[r][k], acc);
+                int slot = sorted_row[row0 + r];
+                h1[(int64_t)slot * d + j] = from_f32<T>(apply_act(acc, act));
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2: LayerNorm (L156; A8: biased variance, eps, affine).  One warp per row, fp32 statistics,
+// two passes over registers (mean, then centred second moment).
+// ------------------------------------------------------------------------------------------------
+template <typename T, int D>
+__global__ void __launch_bounds__(256)
+k_layernorm(const float* __restrict__ h, int N, const float* __restrict__ gamma,
+            const float* __restrict__ beta, float eps, T* __restrict__ u) {
+    constexpr int PER = D / 32;
+    int row = blockIdx.x * 8 + (threadIdx.x >> 5);
+    int lane = threadIdx.x & 31;
+    if (row >= N) return;
+    const float* hp = h + (int64_t)row * D;
+    float v[PER];
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) { v[i] = hp[lane + 32 * i]; s += v[i]; }
+    float mean = warp_sum(s) * (1.0f / D);
+    float q = 0.f;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) { float c = v[i] - mean; q = fmaf(c, c, q); }
+    float rstd = rsqrtf(warp_sum(q) * (1.0f / D) + eps);
+    T* up = u + (int64_t)row * D;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+        int c = lane + 32 * i;
+        up[c] = from_f32<T>((v[i] - mean) * rstd * gamma[c] + beta[c]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// CUDA-core GEMM  C = A[M,K] W[N,K]^T with the shared epilogue (fp32 debug path / debugging aid).
+// 64x64 tile, BK = 16, 256 threads x (4x4) outputs, fp32 accumulate.  K % 16 == 0, N % 64 == 0.
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_gemm_simple(const T* __restrict__ A, const T* __restrict__ W, int M, int N, int K, Epi ep) {
+    __shared__ float As[16][64 + 4];
+    __shared__ float Ws[16][64 + 4];
+    const int m0 = blockIdx.y * 64, n0 = blockIdx.x * 64;
+    int64_t w_row0 = 0;
+    if (ep.group_offsets) {
+        int g = 1;
+        if (m0 >= ep.group_offsets[ep.n_groups + 1]) return;
+        while (g < ep.n_groups && m0 >= ep.group_offsets[g + 1]) ++g;
+        w_row0 = (int64_t)(g - 1) * N;
+    }
+    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+    float acc[4][4] = {};
+    const int lr = threadIdx.x >> 2, lk = (threadIdx.x & 3) * 4;   // 64 rows x 16 k, 4 k per thread
+    for (int k0 = 0; k0 < K; k0 += 16) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            int m = m0 + lr;
+            As[lk + i][lr] = (m < M) ? to_f32<T>(A[(int64_t)m * K + k0 + lk + i]) : 0.0f;
+            Ws[lk + i][lr] = to_f32<T>(W[(w_row0 + n0 + lr) * K + k0 + lk + i]);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            float a[4], b[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) { a[i] = As[k][ty * 4 + i]; b[i] = Ws[k][tx * 4 + i]; }
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        int m = m0 + ty * 4 + i;
+        if (m >= M) continue;
+        int row = ep.row_perm ? ep.row_perm[m] : m;
+        if (row < 0) continue;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            int n = n0 + tx * 4 + j;
+            float v = acc[i][j];
+            if (ep.bias) v += ep.bias[w_row0 + n];
+            v = apply_act(v, ep.act);
+            if (ep.residual) v += ep.residual[(int64_t)row * ep.ld_res + n];
+            if (ep.out_f32) ep.out_f32[(int64_t)row * ep.ld_f32 + n] = v;
+            if (n < ep.vt_col0) {
+                if (ep.out_act) ((T*)ep.out_act)[(int64_t)row * ep.ld_act + n] = from_f32<T>(v);
+            } else {
+                ((T*)ep.out_vt)[(int64_t)(n - ep.vt_col0) * ep.ld_vt + row] = from_f32<T>(v);
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a4 (debug path): per event, per head  O = softmax(Q K^T / sqrt(hd)) V  (Eq. 4) with the
+// FlashAttention recurrence (L154) over key tiles of 32; one thread per query row, fp32 state.
+// Keys outside the event or with valid == 0 get weight exactly 0 (A2); no valid key -> O = 0 (A15).
+// grid = (n_tiles, H), block = tile_q threads; work = (event, q_tile) list.
+// ------------------------------------------------------------------------------------------------
+template <typename T, int HD>
+__global__ void __launch_bounds__(128)
+k_attn_simple(const T* __restrict__ QK, const T* __restrict__ VT, int64_t ldvt,
+              const int* __restrict__ key_valid, const int* __restrict__ offsets,
+              const int2* __restrict__ work, int tile_q, int d, T* __restrict__ O) {
+    __shared__ float Ks[32][HD + 1];
+    __shared__ float Vs[32][HD + 1];
+    __shared__ int vs[32];
+    const int2 wk = work[blockIdx.x];
+    const int head = blockIdx.y;
+    const int ev0 = offsets[wk.x], ev1 = offsets[wk.x + 1];
+    const int qrow = ev0 + wk.y * tile_q + threadIdx.x;
+    const bool active = (int)threadIdx.x < tile_q && qrow < ev1;
+    const float scale = rsqrtf((float)HD);
+    float q[HD], acc[HD];
+#pragma unroll
+    for (int c = 0; c < HD; ++c) {
+        q[c] = active ? to_f32<T>(QK[(int64_t)qrow * (2 * d) + head * HD + c]) * scale : 0.0f;
+        acc[c] = 0.0f;
+    }
+    float m = -INFINITY, l = 0.0f;
+    for (int k0 = ev0; k0 < ev1; k0 += 32) {
+        __syncthreads();
+        for (int idx = threadIdx.x; idx < 32 * HD; idx += blockDim.x) {
+            int j = idx / HD, c = idx % HD;          // K rows: contiguous over c
+            int key = k0 + j;
+            Ks[j][c] = (key < ev1) ? to_f32<T>(QK[(int64_t)key * (2 * d) + d + head * HD + c]) : 0.0f;
+        }
+        for (int idx = threadIdx.x; idx < 32 * HD; idx += blockDim.x) {
+            int c = idx / 32, j = idx % 32;          // V^T rows: contiguous over keys
+            int key = k0 + j;
+            Vs[j][c] = (key < ev1) ? to_f32<T>(VT[(int64_t)(head * HD + c) * ldvt + key]) : 0.0f;
+        }
+        if (threadIdx.x < 32) {
+            int key = k0 + threadIdx.x;
+            vs[threadIdx.x] = (key < ev1) && (key_valid == nullptr || key_valid[key] != 0);
+        }
+        __syncthreads();
+        float s[32];
+        float tmax = -INFINITY;
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+            float a = 0.0f;
+#pragma unroll
+            for (int c = 0; c < HD; ++c) a = fmaf(q[c], Ks[j][c], a);
+            s[j] = vs[j] ? a : -INFINITY;
+            tmax = fmaxf(tmax, s[j]);
+        }
+        if (tmax == -INFINITY) continue;             // block-uniform only per thread; no barrier inside
+        float mnew = fmaxf(m, tmax);
+        float corr = expf(m - mnew);                 // m = -inf -> 0
+        l *= corr;
+#pragma unroll
+        for (int c = 0; c < HD; ++c) acc[c] *= corr;
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+            float p = expf(s[j] - mnew);             // -inf -> 0
+            l += p;
+#pragma unroll
+            for (int c = 0; c < HD; ++c) acc[c] = fmaf(p, Vs[j][c], acc[c]);
+        }
+        m = mnew;
+    }
+    if (active) {
+        float inv = (l > 0.0f) ? 1.0f / l : 0.0f;
+#pragma unroll
+        for (int c = 0; c < HD; ++c) O[(int64_t)qrow * d + head * HD + c] = from_f32<T>(acc[c] * inv);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a8 (output layer): out[row, o] = W2[o,:] . hidden[row, head(o) block] + b2[o] in fp32; one warp per
+// row; rows with valid == 0 are written as exactly 0 (A2).  hidden = [N, n_blocks*d]; output o reads
+// hidden block blk[o].  Outputs 0..C-1 -> logits, C.. -> regress.
+// ------------------------------------------------------------------------------------------------
+constexpr int MAX_OUT = 24;
+struct HeadsOut {
+    int n_out; int n_cls; int n_reg;
+    int blk[MAX_OUT];
+};
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_heads_l2(const T* __restrict__ hidden, int N, int d, int ld_hidden, const float* __restrict__ W2,
+           const float* __restrict__ b2, const int* __restrict__ valid, HeadsOut ho,
+           float* __restrict__ out_logits, float* __restrict__ out_regress) {
+    int row = blockIdx.x * 8 + (threadIdx.x >> 5);
+    int lane = threadIdx.x & 31;
+    if (row >= N) return;
+    const bool ok = valid[row] != 0;
+    const T* hp = hidden + (int64_t)row * ld_hidden;
+    for (int o = 0; o < ho.n_out; ++o) {
+        float a = 0.0f;
+        if (ok) {
+            const T* hb = hp + ho.blk[o] * d;
+            const float* w = W2 + (int64_t)o * d;
+            for (int c = lane; c < d; c += 32) a = fmaf(to_f32<T>(hb[c]), w[c], a);
+            a = warp_sum(a) + b2[o];
+        }
+        if (lane == 0) {
+            if (o < ho.n_cls) out_logits[(int64_t)row * ho.n_cls + o] = a;
+            else out_regress[(int64_t)row * ho.n_reg + (o - ho.n_cls)] = a;
+        }
+    }
+}
+
+// fp32 <- T conversion for the debug taps
+template <typename T>
+__global__ void k_to_f32(const T* __restrict__ src, float* __restrict__ dst, int64_t n) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = to_f32<T>(src[i]);
+}
+
+}  // namespace mlpf

@@ -1,0 +1,241 @@
+"""GPU parity: libmlpf.so (through the C ABI) against the fp64 CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star; metric = DESIGN.md reading A14): max relative error <= 2e-2 on
+logits and regressions in BF16, <= 1e-4 on the fp32 debug path, argmax agreement >= 99.9 % over
+decidable rows, integer schedule arrays bit-exact."""
+import numpy as np
+import pytest
+
+import synth
+import oracle
+from synth.configs import ModelCfg
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+import paper_2601_17554_b200 as P
+
+TOL_BF16 = 2e-2
+TOL_FP32 = 1e-4
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    assert P.lib() is not None          # fail loudly if the extension is missing
+
+
+def gpu_forward(W, m, X, off, precision=P.PREC_BF16, kernels=P.KERNELS_TC, tap=None):
+    mod = P.Mlpf(W, m)
+    mod.set_option(P.OPT_PRECISION, precision)
+    mod.set_option(P.OPT_KERNELS, kernels)
+    if tap is not None:
+        mod.set_option(P.OPT_TAP_LAYER, tap)
+    Xd = torch.from_numpy(X).cuda()
+    lg, rg = mod.infer(Xd, off)
+    torch.cuda.synchronize()
+    return mod, lg.cpu().numpy(), rg.cpu().numpy()
+
+
+def oracle_events(W, m, X, off, events, quantized):
+    """Oracle outputs for a subset of events (events are independent: pin P4)."""
+    Wq = oracle.quantize_weights(W) if quantized else W
+    rows, lgs, rgs = [], [], []
+    for e in events:
+        a, b = int(off[e]), int(off[e + 1])
+        lg, rg = oracle.forward(X[a:b], np.array([0, b - a]), Wq, m)
+        rows.append(np.arange(a, b)); lgs.append(lg); rgs.append(rg)
+    return np.concatenate(rows), np.concatenate(lgs), np.concatenate(rgs)
+
+
+def check(lg_gpu, rg_gpu, rows, lg_ref, rg_ref, X, tol, argmax=True):
+    valid = X[rows, 0] != 0
+    e_lg, _ = oracle.parity_metrics(lg_gpu[rows], lg_ref, valid)
+    e_rg, _ = oracle.parity_metrics(rg_gpu[rows], rg_ref, valid)
+    assert np.isfinite(lg_gpu).all() and np.isfinite(rg_gpu).all()
+    assert (lg_gpu[X[:, 0] == 0] == 0).all() and (rg_gpu[X[:, 0] == 0] == 0).all()    # pad rows exactly 0
+    assert e_lg <= tol and e_rg <= tol, (e_lg, e_rg)
+    if argmax:
+        agree, dec_frac, raw = oracle.argmax_agreement(lg_gpu[rows], lg_ref, valid, tol_rel=tol)
+        assert agree >= 0.999, (agree, dec_frac, raw)
+    return e_lg, e_rg
+
+
+# ------------------------------------------------------------------------------------------- a0 schedule
+@pytest.mark.parametrize("lens,pad", [((64, 192), 0.0), ((0, 5, 0, 300, 129, 1, 0), 0.3), ((1,), 0.0),
+                                      ((1500, 700, 1500, 2049), 0.1)])
+@pytest.mark.parametrize("tile_q", [64, 128])
+def test_schedule_bit_exact(lens, pad, tile_q):
+    m = synth.model_cfg("cfg1")
+    W = synth.make_weights("cfg1")
+    X, off = synth.make_events(lens, seed=11, pad_frac=pad)
+    mod = P.Mlpf(W, m)
+    mod.set_option(P.OPT_TILE_Q, tile_q)
+    mod.set_option(P.OPT_TAP_LAYER, -2)
+    mod.infer(torch.from_numpy(X).cuda(), off)
+    ref = oracle.schedule(X, off, tile_q)
+    for k in ("row_event", "row_pos", "valid", "n_valid", "type_offsets", "sorted_row", "type_perm", "work_list"):
+        got = mod.schedule(k)
+        assert got.dtype == np.int32
+        np.testing.assert_array_equal(got, ref[k], err_msg=k)
+
+
+# ------------------------------------------------------------------------------------------- fp32 debug path
+@pytest.mark.parametrize("name,events", [("cfg1", None), ("cfg2", [0, 5])])
+def test_fp32_debug_path(name, events):
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    X, off = synth.make_named_events(name)
+    _, lg, rg = gpu_forward(W, m, X, off, precision=P.PREC_FP32_DEBUG)
+    ev = range(len(off) - 1) if events is None else events
+    rows, lr, rr = oracle_events(W, m, X, off, ev, quantized=False)
+    check(lg, rg, rows, lr, rr, X, TOL_FP32)
+
+
+# ------------------------------------------------------------------------------------------- bf16 path
+BF16_CASES = [("cfg1", None), ("cfg2", None), ("cfg3", [0, 3]), ("cfg4", [2, 17]), ("cfg5b", [31])]
+
+
+@pytest.mark.parametrize("kernels", [P.KERNELS_TC, P.KERNELS_SIMPLE])
+@pytest.mark.parametrize("name,events", BF16_CASES)
+def test_bf16_parity(name, events, kernels):
+    if kernels == P.KERNELS_SIMPLE and name not in ("cfg1", "cfg2"):
+        pytest.skip("CUDA-core debugging kernels are only exercised on the small configs")
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    X, off = synth.make_named_events(name)
+    mod, lg, rg = gpu_forward(W, m, X, off, kernels=kernels)
+    ev = range(len(off) - 1) if events is None else events
+    rows, lr, rr = oracle_events(W, m, X, off, ev, quantized=True)
+    e = check(lg, rg, rows, lr, rr, X, TOL_BF16)
+    print(name, "max rel err (logits, regress) =", e, "launches", mod.query(P.Q_LAUNCHES))
+
+
+def test_bf16_parity_sharp_attention():
+    """Pin P15's weight set: W_q x4 makes attention far from uniform so masking/leak bugs show."""
+    name = "cfg2"
+    m = synth.model_cfg(name)
+    W = synth.sharpen(synth.make_weights(name), m, 4.0)
+    X, off = synth.make_named_events(name, max_events=4)
+    _, lg, rg = gpu_forward(W, m, X, off)
+    rows, lr, rr = oracle_events(W, m, X, off, range(len(off) - 1), quantized=True)
+    check(lg, rg, rows, lr, rr, X, TOL_BF16)
+
+
+# ------------------------------------------------------------------------------------------- per-step parity
+def _rel(got, ref, valid):
+    ref = ref[valid]; got = got[valid]
+    rms = np.sqrt((ref ** 2).mean())
+    return float((np.abs(got - ref) / np.maximum(np.abs(ref), rms)).max())
+
+
+@pytest.mark.parametrize("precision,tol", [(P.PREC_FP32_DEBUG, 1e-4), (P.PREC_BF16, 2e-2)])
+@pytest.mark.parametrize("name,max_events", [("cfg1", None), ("cfg2", 3)])
+def test_per_step_intermediates(name, max_events, precision, tol):
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    X, off = synth.make_named_events(name, max_events=max_events)
+    N, d = X.shape[0], m.d_model
+    valid = X[:, 0] != 0
+    dump = {}
+    Wq = oracle.quantize_weights(W) if precision == P.PREC_BF16 else W
+    oracle.forward(X, off, Wq, m, dump=dump)
+    # after the embedding
+    mod, _, _ = gpu_forward(W, m, X, off, precision=precision, tap=-2)
+    assert _rel(mod.tensor("H", (N, d)), dump["h0"], valid) <= tol
+    for l in (0, m.n_layers - 1):
+        mod, _, _ = gpu_forward(W, m, X, off, precision=precision, tap=l)
+        p = f"layer.{l}."
+        qkv = dump[p + "qkv"]
+        assert _rel(mod.tensor("QK", (N, 2 * d)), qkv[:, :2 * d], valid) <= tol, "qk"
+        assert _rel(mod.tensor("VT", (d, N)).T, qkv[:, 2 * d:], valid) <= tol, "v"
+        assert _rel(mod.tensor("O", (N, d)), dump[p + "o"], valid) <= tol, "o"
+        assert _rel(mod.tensor("U", (N, d)), dump[p + "u2"], valid) <= tol, "u2"
+        assert _rel(mod.tensor("G", (N, m.d_ff)), dump[p + "g"], valid) <= tol, "g"
+        assert _rel(mod.tensor("H", (N, d)), dump[p + "h"], valid) <= tol, "h"
+
+
+# ------------------------------------------------------------------------------------------- edge cases
+TINY = ModelCfg(n_layers=2, d_model=64, n_heads=4, d_ff=256)
+
+
+@pytest.mark.parametrize("lens,pad", [((1,), 0.0), ((0, 7, 0), 0.0), ((129, 1, 257, 128), 0.0), ((40, 300), 0.5),
+                                      ((5, 6), 1.0)])
+@pytest.mark.parametrize("precision,tol", [(P.PREC_FP32_DEBUG, TOL_FP32), (P.PREC_BF16, TOL_BF16)])
+def test_edge_cases(lens, pad, precision, tol):
+    W = synth.make_weights(TINY, seed=5)
+    X, off = synth.make_events(lens, seed=9, pad_frac=pad)
+    if pad == 0.5:
+        X[X[:, 0] == 0, 1:] = 1e30            # garbage in pad rows must be ignored (P4 iii)
+    _, lg, rg = gpu_forward(W, TINY, X, off, precision=precision)
+    Wq = oracle.quantize_weights(W) if precision == P.PREC_BF16 else W
+    lr, rr = oracle.forward(X, off, Wq, TINY)
+    check(lg, rg, np.arange(X.shape[0]), lr, rr, X, tol, argmax=False)
+
+
+def test_empty_calls_and_bad_offsets():
+    W = synth.make_weights(TINY, seed=5)
+    mod = P.Mlpf(W, TINY)
+    X = torch.zeros((4, 55), device="cuda")
+    lg, rg = mod.infer(X[:0], np.array([0], np.int32))                 # zero events
+    lg, rg = mod.infer(X[:0], np.array([0, 0, 0], np.int32))           # zero rows
+    with pytest.raises(P.MlpfError, match="-3"):
+        mod.infer(X, np.array([1, 4], np.int32))
+    with pytest.raises(P.MlpfError, match="-3"):
+        mod.infer(X, np.array([0, 3, 2, 4], np.int32))
+
+
+def test_determinism_and_packing_invariance():
+    """L232: the same event gives identical outputs; per-event tile schedule -> also when packed."""
+    name = "cfg2"
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    X, off = synth.make_named_events(name, max_events=5)
+    mod = P.Mlpf(W, m)
+    Xd = torch.from_numpy(X).cuda()
+    a = [t.clone() for t in mod.infer(Xd, off)]
+    b = [t.clone() for t in mod.infer(Xd, off)]
+    torch.cuda.synchronize()
+    assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])
+    s0, s1 = int(off[2]), int(off[3])
+    c = mod.infer(Xd[s0:s1].contiguous(), np.array([0, s1 - s0], np.int32))
+    torch.cuda.synchronize()
+    assert torch.equal(c[0], a[0][s0:s1]) and torch.equal(c[1], a[1][s0:s1])
+
+
+def test_concurrent_streams_match_single_stream():
+    name = "cfg2"
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    X, off = synth.make_named_events(name)
+    mod = P.Mlpf(W, m)
+    Xd = torch.from_numpy(X).cuda()
+    ref = [t.clone() for t in mod.infer(Xd, off)]
+    torch.cuda.synchronize()
+    E = len(off) - 1
+    streams = [torch.cuda.Stream() for _ in range(4)]
+    outs = []
+    for i, s in enumerate(streams):
+        e0, e1 = i * E // 4, (i + 1) * E // 4
+        r0, r1 = int(off[e0]), int(off[e1])
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            outs.append((r0, r1, mod.infer(Xd[r0:r1], off[e0:e1 + 1] - off[e0], stream=s)))
+    torch.cuda.synchronize()
+    for r0, r1, (lg, rg) in outs:
+        assert torch.equal(lg, ref[0][r0:r1]) and torch.equal(rg, ref[1][r0:r1])
+    assert mod.query(P.Q_WORKSPACE_BYTES) > 0
+
+
+def test_host_entry_point_matches_device_entry_point():
+    m = synth.model_cfg("cfg1")
+    W = synth.make_weights("cfg1")
+    X, off = synth.make_named_events("cfg1")
+    mod = P.Mlpf(W, m)
+    lg, rg = mod.infer(torch.from_numpy(X).cuda(), off)
+    xh = torch.from_numpy(X).pin_memory()
+    lh = torch.empty((X.shape[0], 9)).pin_memory()
+    rh = torch.empty((X.shape[0], 5)).pin_memory()
+    mod.infer_host(xh, off, lh, rh)
+    assert torch.equal(lh, lg.cpu()) and torch.equal(rh, rg.cpu())
