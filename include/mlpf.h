@@ -106,6 +106,10 @@ const char* mlpf_last_error(void);
                                     are then NOT written.  -2: stop after the embedding.                */
 #define MLPF_OPT_KERNELS     4   /* MLPF_KERNELS_TC (default: tcgen05 GEMM + attention) | MLPF_KERNELS_SIMPLE
                                     (CUDA-core kernels in the same precision; debugging aid)            */
+#define MLPF_OPT_SPLIT       5   /* 1 (default): in BF16 mode the activations that feed the residual stream
+                                    (embedding hidden, attention output, LN2 / final-LN output, FFN hidden, head
+                                    hidden) are carried as two bf16 terms hi + lo and multiplied as two MMAs
+                                    (DESIGN.md "error budget").  0: single bf16 term everywhere.          */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0
@@ -152,10 +156,10 @@ int64_t mlpf_debug_get_schedule(mlpf_handle* h, void* stream, int which, int32_t
 int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which, float* host_out, int64_t capacity);
 
 /* ---- kernel-level entry points (unit tests and micro-benchmarks; device pointers, bf16 = uint16) ---- */
-/* C[M,N] (fp32, ldc = N) = A[M,K] (bf16, row-major) * W[N,K]^T (bf16, row-major) via the tcgen05 GEMM.
- * K % 64 == 0, N % 64 == 0.  Step a3/a5/a6/a7's contraction (L148-L156) without an epilogue. */
-int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* W, float* C, int32_t M, int32_t N, int32_t K,
-                      void* stream);
+/* C[M,N] (fp32, ldc = N) = (A + A_lo)[M,K] (bf16, row-major; A_lo may be NULL) * W[N,K]^T (bf16, row-major)
+ * via the tcgen05 GEMM.  K % 64 == 0, N % 64 == 0.  Step a3/a5/a6/a7's contraction (L148-L156), no epilogue. */
+int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* A_lo, const uint16_t* W, float* C, int32_t M, int32_t N,
+                      int32_t K, void* stream);
 /* O[N,d] (bf16) = per-event multi-head softmax(Q K^T / sqrt(hd)) V (Eq. 4) via the tcgen05 flash kernel.
  * QK [N,2d] bf16 (q | k), VT [d, ldvt] bf16, key_valid [N] int32 0/1 (NULL = all valid),
  * event_offsets HOST int32 [n_events+1]. */

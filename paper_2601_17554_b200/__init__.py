@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmlpf.so")
 
 # include/mlpf.h constants
 OK = 0
-OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS = 1, 2, 3, 4
+OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT = 1, 2, 3, 4, 5
 PREC_BF16, PREC_FP32_DEBUG = 0, 1
 KERNELS_TC, KERNELS_SIMPLE = 0, 1
 Q_N_LAYERS, Q_D_MODEL, Q_N_HEADS, Q_D_FF, Q_N_FEAT, Q_N_CLASSES, Q_N_REGRESS = 1, 2, 3, 4, 5, 6, 7
@@ -60,7 +60,7 @@ def lib():
     L.mlpf_debug_get_tensor.restype = i64
     L.mlpf_debug_get_tensor.argtypes = [vp, vp, C.c_int, vp, i64]
     L.mlpf_tc_gemm_bf16.restype = C.c_int
-    L.mlpf_tc_gemm_bf16.argtypes = [vp, vp, vp, i32, i32, i32, vp]
+    L.mlpf_tc_gemm_bf16.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp]
     L.mlpf_tc_attention_bf16.restype = C.c_int
     L.mlpf_tc_attention_bf16.argtypes = [vp, vp, i64, vp, vp, i32, i32, i32, vp, vp]
     _lib = L
@@ -158,13 +158,14 @@ class Mlpf:
         return out.reshape(shape)
 
 
-def tc_gemm_bf16(A, W, stream=None):
-    """A [M,K], W [N,K] CUDA bfloat16 tensors -> fp32 [M,N] = A W^T via the tcgen05 GEMM kernel."""
+def tc_gemm_bf16(A, W, A_lo=None, stream=None):
+    """A (+ A_lo) [M,K], W [N,K] CUDA bfloat16 tensors -> fp32 [M,N] = (A + A_lo) W^T via the tcgen05 GEMM."""
     import torch
     M, K = A.shape
     N = W.shape[0]
     out = torch.empty((M, N), dtype=torch.float32, device=A.device)
-    _check(lib().mlpf_tc_gemm_bf16(C.c_void_p(A.data_ptr()), C.c_void_p(W.data_ptr()), C.c_void_p(out.data_ptr()),
+    _check(lib().mlpf_tc_gemm_bf16(C.c_void_p(A.data_ptr()), C.c_void_p(A_lo.data_ptr() if A_lo is not None else 0),
+                                   C.c_void_p(W.data_ptr()), C.c_void_p(out.data_ptr()),
                                    M, N, K, _stream_ptr(stream)))
     return out
 

@@ -52,6 +52,7 @@ struct Workspace {
     int64_t ldvt = 0;
     float* h = nullptr;               // [cap, d] fp32 residual stream
     void *u = nullptr, *qk = nullptr, *vt = nullptr, *o = nullptr, *g = nullptr;
+    void *u_lo = nullptr, *o_lo = nullptr, *g_lo = nullptr;   // second bf16 term of split activations
     int64_t g_elems = 0;
     // schedule (a0)
     int *offsets = nullptr, *work = nullptr, *pairs = nullptr;
@@ -74,7 +75,7 @@ struct mlpf_handle {
     std::vector<LayerW> layers;
     HeadsOut ho;
     // options
-    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1;
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = 1;
     int64_t last_launches = 0;
     std::mutex mu;
     std::map<void*, Workspace*> ws;
@@ -198,7 +199,7 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
 }
 
 static void ws_free(Workspace* w) {
-    void* ptrs[] = {w->h, w->u, w->qk, w->vt, w->o, w->g, w->offsets, w->work, w->pairs, w->valid, w->row_event,
+    void* ptrs[] = {w->h, w->u, w->qk, w->vt, w->o, w->g, w->u_lo, w->o_lo, w->g_lo, w->offsets, w->work, w->pairs, w->valid, w->row_event,
                     w->row_pos, w->n_valid, w->block_counts, w->block_base, w->type_offsets, w->sorted_row, w->type_perm};
     for (void* p : ptrs) if (p) cudaFree(p);
 }
@@ -224,6 +225,9 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_TAP_LAYER:
             if (value < -2 || value >= h->L) return set_err(MLPF_E_ARG, "bad tap layer");
             h->tap_layer = (int)value; return MLPF_OK;
+        case MLPF_OPT_SPLIT:
+            if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "split must be 0 or 1");
+            h->split = (int)value; return MLPF_OK;
         case MLPF_OPT_KERNELS:
             if (value != MLPF_KERNELS_TC && value != MLPF_KERNELS_SIMPLE) return set_err(MLPF_E_ARG, "bad kernel set");
             h->kernels = (int)value; return MLPF_OK;
@@ -264,7 +268,7 @@ template <typename P> static cudaError_t dmalloc(P** p, int64_t bytes, Workspace
 static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t n_tiles, bool fp32) {
     const int64_t d = h->d;
     if (N > w->cap_rows || fp32 != w->fp32) {
-        void* ptrs[] = {w->h, w->u, w->qk, w->vt, w->o, w->g, w->valid, w->row_event, w->row_pos, w->block_counts,
+        void* ptrs[] = {w->h, w->u, w->qk, w->vt, w->o, w->g, w->u_lo, w->o_lo, w->g_lo, w->valid, w->row_event, w->row_pos, w->block_counts,
                         w->block_base, w->sorted_row, w->type_perm, w->type_offsets};
         int64_t small = w->bytes;     // recompute below
         (void)small;
@@ -285,6 +289,8 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
         if (dmalloc(&w->h, cap * d * 4, w) || dmalloc((char**)&w->u, cap * d * es, w) ||
             dmalloc((char**)&w->qk, cap * 2 * d * es, w) || dmalloc((char**)&w->vt, d * w->ldvt * es, w) ||
             dmalloc((char**)&w->o, cap * d * es, w) || dmalloc((char**)&w->g, w->g_elems * es, w) ||
+            dmalloc((char**)&w->u_lo, cap * d * es, w) || dmalloc((char**)&w->o_lo, cap * d * es, w) ||
+            dmalloc((char**)&w->g_lo, w->g_elems * es, w) ||
             dmalloc(&w->valid, cap * 4, w) || dmalloc(&w->row_event, cap * 4, w) || dmalloc(&w->row_pos, cap * 4, w) ||
             dmalloc(&w->block_counts, nb * 5 * 4, w) || dmalloc(&w->block_base, nb * 5 * 4, w) ||
             dmalloc(&w->sorted_row, cap * 4, w) || dmalloc(&w->type_perm, m_ub * 4, w) ||
@@ -298,6 +304,7 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
         cudaMemset(w->u, 0, cap * d * es); cudaMemset(w->qk, 0, cap * 2 * d * es);
         cudaMemset(w->vt, 0, d * w->ldvt * es); cudaMemset(w->o, 0, cap * d * es);
         cudaMemset(w->g, 0, w->g_elems * es);
+        cudaMemset(w->u_lo, 0, cap * d * es); cudaMemset(w->o_lo, 0, cap * d * es); cudaMemset(w->g_lo, 0, w->g_elems * es);
         w->cap_rows = cap;
     }
     if (E > w->cap_events) {
@@ -331,35 +338,35 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
     } while (0)
 
 template <typename T>
-static int run_gemm(mlpf_handle* h, bool tc, const T* A, const T* W, int M, int N, int K, const Epi& ep,
+static int run_gemm(mlpf_handle* h, bool tc, const T* A, const T* A_lo, const T* W, int M, int N, int K, const Epi& ep,
                     cudaStream_t st) {
     if (M <= 0) return MLPF_OK;
     if (tc) {
         if constexpr (std::is_same<T, bf16>::value) {
-            int rc = tc_gemm_launch(&h->tc, A, W, M, N, K, ep, st);
+            int rc = tc_gemm_launch(&h->tc, A, A_lo, W, M, N, K, ep, st);
             if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", h->tc.err);
             LAUNCH_CHECK(h);
             return MLPF_OK;
         }
     }
     dim3 grid(N / 64, (M + 63) / 64);
-    k_gemm_simple<T><<<grid, 256, 0, st>>>(A, W, M, N, K, ep);
+    k_gemm_simple<T><<<grid, 256, 0, st>>>(A, A_lo, W, M, N, K, ep);
     LAUNCH_CHECK(h);
     return MLPF_OK;
 }
 
 template <typename T>
-static int run_layernorm(mlpf_handle* h, const float* x, int N, const float* g, const float* b, T* u, cudaStream_t st) {
+static int run_layernorm(mlpf_handle* h, const float* x, int N, const float* g, const float* b, T* u, T* u_lo, cudaStream_t st) {
     dim3 grid((N + 7) / 8);
     switch (h->d) {
-        case 64:  k_layernorm<T, 64><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
-        case 128: k_layernorm<T, 128><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
-        case 192: k_layernorm<T, 192><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
-        case 256: k_layernorm<T, 256><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
-        case 320: k_layernorm<T, 320><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
-        case 384: k_layernorm<T, 384><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
-        case 448: k_layernorm<T, 448><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
-        case 512: k_layernorm<T, 512><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u); break;
+        case 64:  k_layernorm<T, 64><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
+        case 128: k_layernorm<T, 128><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
+        case 192: k_layernorm<T, 192><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
+        case 256: k_layernorm<T, 256><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
+        case 320: k_layernorm<T, 320><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
+        case 384: k_layernorm<T, 384><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
+        case 448: k_layernorm<T, 448><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
+        case 512: k_layernorm<T, 512><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
         default: return set_err(MLPF_E_ARG, "d_model %d unsupported by LayerNorm", h->d);
     }
     LAUNCH_CHECK(h);
@@ -367,23 +374,23 @@ static int run_layernorm(mlpf_handle* h, const float* x, int N, const float* g, 
 }
 
 template <typename T>
-static int run_attention(mlpf_handle* h, bool tc, Workspace* w, cudaStream_t st) {
+static int run_attention(mlpf_handle* h, bool tc, bool split, Workspace* w, cudaStream_t st) {
     if (w->n_tiles == 0) return MLPF_OK;
     if (tc) {
         if constexpr (std::is_same<T, bf16>::value) {
             int rc = tc_attn_launch(&h->tc, (const bf16*)w->qk, (const bf16*)w->vt, w->ldvt, w->N, w->valid, w->offsets,
-                                    (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, (bf16*)w->o, st);
+                                    (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, (bf16*)w->o, split ? (bf16*)w->o_lo : nullptr, st);
             if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", h->tc.err);
             LAUNCH_CHECK(h);
             return MLPF_OK;
         }
     }
     dim3 grid((unsigned)w->n_tiles, h->H);
-    const T* qk = (const T*)w->qk; const T* vt = (const T*)w->vt; T* o = (T*)w->o;
+    const T* qk = (const T*)w->qk; const T* vt = (const T*)w->vt; T* o = (T*)w->o; T* o_lo = split ? (T*)w->o_lo : nullptr;
     switch (h->hd) {
-        case 16: k_attn_simple<T, 16><<<grid, w->tile_q, 0, st>>>(qk, vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, w->tile_q, h->d, o); break;
-        case 32: k_attn_simple<T, 32><<<grid, w->tile_q, 0, st>>>(qk, vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, w->tile_q, h->d, o); break;
-        case 64: k_attn_simple<T, 64><<<grid, w->tile_q, 0, st>>>(qk, vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, w->tile_q, h->d, o); break;
+        case 16: k_attn_simple<T, 16><<<grid, w->tile_q, 0, st>>>(qk, vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, w->tile_q, h->d, o, o_lo); break;
+        case 32: k_attn_simple<T, 32><<<grid, w->tile_q, 0, st>>>(qk, vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, w->tile_q, h->d, o, o_lo); break;
+        case 64: k_attn_simple<T, 64><<<grid, w->tile_q, 0, st>>>(qk, vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, w->tile_q, h->d, o, o_lo); break;
     }
     LAUNCH_CHECK(h);
     return MLPF_OK;
@@ -414,7 +421,9 @@ static int infer_impl(mlpf_handle* h, Workspace* w, const float* X, float* out_l
     const bool tc_attn = tc_req && TC_ATTN_READY;
     const T* PW = fp32 ? (const T*)h->P32 : (const T*)h->P16;
     const float* PV = h->P32;
+    const bool split = !fp32 && h->split != 0;     // bf16 activations carried as hi + lo where they feed the residual stream
     T* u = (T*)w->u; T* g = (T*)w->g;
+    T* u_lo = split ? (T*)w->u_lo : nullptr; T* g_lo = split ? (T*)w->g_lo : nullptr; T* o_lo = split ? (T*)w->o_lo : nullptr;
 
     // ---- a0 (device half)
     const int nb = (N + SCHED_BLOCK - 1) / SCHED_BLOCK;
@@ -428,13 +437,13 @@ static int infer_impl(mlpf_handle* h, Workspace* w, const float* X, float* out_l
     LAUNCH_CHECK(h);
 
     // ---- a1: per-type embedding (L156; A3-A5)
-    k_embed_l1<T><<<(N + EMB_ROWS - 1) / EMB_ROWS, 256, 0, st>>>(X, N, h->F, d, PV + h->embW1t, PV + h->embB1, h->act, w->sorted_row, g, w->h);
+    k_embed_l1<T><<<(N + EMB_ROWS - 1) / EMB_ROWS, 256, 0, st>>>(X, N, h->F, d, PV + h->embW1t, PV + h->embB1, h->act, w->sorted_row, g, g_lo, w->h);
     LAUNCH_CHECK(h);
     {
         Epi ep;
         ep.bias = PV + h->embB2; ep.out_f32 = w->h; ep.ld_f32 = d;
         ep.row_perm = w->type_perm; ep.group_offsets = w->type_offsets; ep.n_groups = 4;
-        int rc = run_gemm<T>(h, tc, g, PW + h->embW2, (int)w->m_ub, d, d, ep, st);
+        int rc = run_gemm<T>(h, tc, g, g_lo, PW + h->embW2, (int)w->m_ub, d, d, ep, st);
         if (rc) return rc;
     }
     if (h->tap_layer == -2) return MLPF_OK;
@@ -442,35 +451,35 @@ static int infer_impl(mlpf_handle* h, Workspace* w, const float* X, float* out_l
     // ---- encoder blocks (pre-LN, L156 + A7)
     for (int l = 0; l < h->L; ++l) {
         const LayerW& lw = h->layers[l];
-        int rc = run_layernorm<T>(h, w->h, N, PV + lw.ln1g, PV + lw.ln1b, u, st);                     // a2
+        int rc = run_layernorm<T>(h, w->h, N, PV + lw.ln1g, PV + lw.ln1b, u, (T*)nullptr, st);                     // a2
         if (rc) return rc;
         {   // a3: [Q K V] = LN1(x) Wqkv^T + bqkv ; V stored transposed per head dim
             Epi ep;
             ep.bias = PV + lw.bqkv; ep.out_act = w->qk; ep.ld_act = 2 * d;
             ep.out_vt = w->vt; ep.ld_vt = w->ldvt; ep.vt_col0 = 2 * d;
-            rc = run_gemm<T>(h, tc, u, PW + lw.Wqkv, N, 3 * d, d, ep, st);
+            rc = run_gemm<T>(h, tc, u, (const T*)nullptr, PW + lw.Wqkv, N, 3 * d, d, ep, st);
             if (rc) return rc;
         }
-        rc = run_attention<T>(h, tc_attn, w, st);                                                         // a4
+        rc = run_attention<T>(h, tc_attn, split, w, st);                                                         // a4
         if (rc) return rc;
         {   // a5: h <- h + O Wo^T + bo
             Epi ep;
             ep.bias = PV + lw.bo; ep.residual = w->h; ep.ld_res = d; ep.out_f32 = w->h; ep.ld_f32 = d;
-            rc = run_gemm<T>(h, tc, (const T*)w->o, PW + lw.Wo, N, d, d, ep, st);
+            rc = run_gemm<T>(h, tc, (const T*)w->o, o_lo, PW + lw.Wo, N, d, d, ep, st);
             if (rc) return rc;
         }
-        rc = run_layernorm<T>(h, w->h, N, PV + lw.ln2g, PV + lw.ln2b, u, st);
+        rc = run_layernorm<T>(h, w->h, N, PV + lw.ln2g, PV + lw.ln2b, u, u_lo, st);
         if (rc) return rc;
         {   // a6: g = act(LN2(h) W1^T + b1)
             Epi ep;
-            ep.bias = PV + lw.b1; ep.act = h->act; ep.out_act = g; ep.ld_act = dff;
-            rc = run_gemm<T>(h, tc, u, PW + lw.W1, N, dff, d, ep, st);
+            ep.bias = PV + lw.b1; ep.act = h->act; ep.out_act = g; ep.out_act_lo = g_lo; ep.ld_act = dff;
+            rc = run_gemm<T>(h, tc, u, u_lo, PW + lw.W1, N, dff, d, ep, st);
             if (rc) return rc;
         }
         {   // a7: h <- h + g W2^T + b2
             Epi ep;
             ep.bias = PV + lw.b2; ep.residual = w->h; ep.ld_res = d; ep.out_f32 = w->h; ep.ld_f32 = d;
-            rc = run_gemm<T>(h, tc, g, PW + lw.W2, N, d, dff, ep, st);
+            rc = run_gemm<T>(h, tc, g, g_lo, PW + lw.W2, N, d, dff, ep, st);
             if (rc) return rc;
         }
         w->g_width = dff;
@@ -479,7 +488,7 @@ static int infer_impl(mlpf_handle* h, Workspace* w, const float* X, float* out_l
 
     // ---- a8: heads (L156; A11-A12)
     if (h->hp.final_ln) {
-        int rc = run_layernorm<T>(h, w->h, N, PV + h->lnfg, PV + h->lnfb, u, st);
+        int rc = run_layernorm<T>(h, w->h, N, PV + h->lnfg, PV + h->lnfb, u, u_lo, st);
         if (rc) return rc;
     } else {
         // no final LN: u = T(h).  (identity affine with the row kept: done by a cast kernel)
@@ -488,11 +497,11 @@ static int infer_impl(mlpf_handle* h, Workspace* w, const float* X, float* out_l
     {
         Epi ep;
         const int hw = h->n_hblk * d;
-        ep.bias = PV + h->headB1; ep.act = h->act; ep.out_act = g; ep.ld_act = hw;
-        int rc = run_gemm<T>(h, tc, u, PW + h->headW1, N, hw, d, ep, st);
+        ep.bias = PV + h->headB1; ep.act = h->act; ep.out_act = g; ep.out_act_lo = g_lo; ep.ld_act = hw;
+        int rc = run_gemm<T>(h, tc, u, u_lo, PW + h->headW1, N, hw, d, ep, st);
         if (rc) return rc;
         w->g_width = hw;
-        k_heads_l2<T><<<(N + 7) / 8, 256, 0, st>>>(g, N, d, hw, PV + h->headW2, PV + h->headB2, w->valid, h->ho, out_logits, out_regress);
+        k_heads_l2<T><<<(N + 7) / 8, 256, 0, st>>>(g, g_lo, N, d, hw, PV + h->headW2, PV + h->headB2, w->valid, h->ho, out_logits, out_regress);
         LAUNCH_CHECK(h);
     }
     return MLPF_OK;
@@ -632,7 +641,7 @@ extern "C" int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which
 }
 
 // ------------------------------------------------------------------------------------------------ kernel-level entries
-extern "C" int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* W, float* C, int32_t M, int32_t N, int32_t K, void* stream) {
+extern "C" int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* A_lo, const uint16_t* W, float* C, int32_t M, int32_t N, int32_t K, void* stream) {
     if (!A || !W || !C) return set_err(MLPF_E_NULL, "NULL argument");
     if (M <= 0 || N <= 0 || K <= 0 || N % 64 || K % 64) return set_err(MLPF_E_ARG, "need M > 0, N %% 64 == 0, K %% 64 == 0");
     static TcContext ctx;
@@ -642,7 +651,7 @@ extern "C" int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* W, float* C,
     if (init_rc) return set_err(MLPF_E_CUDA, "tcgen05/TMA initialisation failed: %s", ctx.err);
     Epi ep;
     ep.out_f32 = C; ep.ld_f32 = N;
-    if (tc_gemm_launch(&ctx, (const bf16*)A, (const bf16*)W, M, N, K, ep, (cudaStream_t)stream))
+    if (tc_gemm_launch(&ctx, (const bf16*)A, (const bf16*)A_lo, (const bf16*)W, M, N, K, ep, (cudaStream_t)stream))
         return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", ctx.err);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", cudaGetErrorString(e));
@@ -672,7 +681,7 @@ extern "C" int mlpf_tc_attention_bf16(const uint16_t* QK, const uint16_t* VT, in
     CUDA_TRY(cudaMemcpyAsync(d_off, event_offsets, (size_t)(n_events + 1) * 4, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(d_pairs, pairs.data(), pairs.size() * 4, cudaMemcpyHostToDevice, st));
     int rc = tc_attn_launch(&ctx, (const bf16*)QK, (const bf16*)VT, ldvt, N, key_valid, d_off, (const int2*)d_pairs,
-                            (int)(pairs.size() / 2), d_model, n_heads, (bf16*)O, st);
+                            (int)(pairs.size() / 2), d_model, n_heads, (bf16*)O, (bf16*)nullptr, st);
     cudaError_t e = cudaStreamSynchronize(st);
     cudaFree(d_off); cudaFree(d_pairs);
     if (rc) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", ctx.err);

@@ -119,7 +119,7 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 k_embed_l1(const float* __restrict__ X, int N, int F, int d, const float* __restrict__ W1t,
            const float* __restrict__ b1, int act, const int* __restrict__ sorted_row,
-           T* __restrict__ h1, float* __restrict__ h) {
+           T* __restrict__ h1, T* __restrict__ h1_lo, float* __restrict__ h) {
     __shared__ float xs[EMB_ROWS][65];
     __shared__ int list[5][EMB_ROWS];
     __shared__ int cnt[5];
@@ -157,7 +157,10 @@ k_embed_l1(const float* __restrict__ X, int N, int F, int d, const float* __rest
 #pragma unroll
                 for (int k = 0; k < 64; ++k) acc = fmaf(w[k], xs[r][k], acc);
                 int slot = sorted_row[row0 + r];
-                h1[(int64_t)slot * d + j] = from_f32<T>(apply_act(acc, act));
+                const float a = apply_act(acc, act);
+                const T hi = from_f32<T>(a);
+                h1[(int64_t)slot * d + j] = hi;
+                if (h1_lo) h1_lo[(int64_t)slot * d + j] = from_f32<T>(a - to_f32<T>(hi));
             }
         }
     }
@@ -170,7 +173,7 @@ k_embed_l1(const float* __restrict__ X, int N, int F, int d, const float* __rest
 template <typename T, int D>
 __global__ void __launch_bounds__(256)
 k_layernorm(const float* __restrict__ h, int N, const float* __restrict__ gamma,
-            const float* __restrict__ beta, float eps, T* __restrict__ u) {
+            const float* __restrict__ beta, float eps, T* __restrict__ u, T* __restrict__ u_lo) {
     constexpr int PER = D / 32;
     int row = blockIdx.x * 8 + (threadIdx.x >> 5);
     int lane = threadIdx.x & 31;
@@ -189,7 +192,10 @@ k_layernorm(const float* __restrict__ h, int N, const float* __restrict__ gamma,
 #pragma unroll
     for (int i = 0; i < PER; ++i) {
         int c = lane + 32 * i;
-        up[c] = from_f32<T>((v[i] - mean) * rstd * gamma[c] + beta[c]);
+        const float y = (v[i] - mean) * rstd * gamma[c] + beta[c];
+        const T hi = from_f32<T>(y);
+        up[c] = hi;
+        if (u_lo) u_lo[(int64_t)row * D + c] = from_f32<T>(y - to_f32<T>(hi));
     }
 }
 
@@ -199,7 +205,7 @@ k_layernorm(const float* __restrict__ h, int N, const float* __restrict__ gamma,
 // ------------------------------------------------------------------------------------------------
 template <typename T>
 __global__ void __launch_bounds__(256)
-k_gemm_simple(const T* __restrict__ A, const T* __restrict__ W, int M, int N, int K, Epi ep) {
+k_gemm_simple(const T* __restrict__ A, const T* __restrict__ A_lo, const T* __restrict__ W, int M, int N, int K, Epi ep) {
     __shared__ float As[16][64 + 4];
     __shared__ float Ws[16][64 + 4];
     const int m0 = blockIdx.y * 64, n0 = blockIdx.x * 64;
@@ -217,7 +223,9 @@ k_gemm_simple(const T* __restrict__ A, const T* __restrict__ W, int M, int N, in
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             int m = m0 + lr;
-            As[lk + i][lr] = (m < M) ? to_f32<T>(A[(int64_t)m * K + k0 + lk + i]) : 0.0f;
+            float a = (m < M) ? to_f32<T>(A[(int64_t)m * K + k0 + lk + i]) : 0.0f;
+            if (A_lo && m < M) a += to_f32<T>(A_lo[(int64_t)m * K + k0 + lk + i]);
+            As[lk + i][lr] = a;
             Ws[lk + i][lr] = to_f32<T>(W[(w_row0 + n0 + lr) * K + k0 + lk + i]);
         }
         __syncthreads();
@@ -248,7 +256,11 @@ k_gemm_simple(const T* __restrict__ A, const T* __restrict__ W, int M, int N, in
             if (ep.residual) v += ep.residual[(int64_t)row * ep.ld_res + n];
             if (ep.out_f32) ep.out_f32[(int64_t)row * ep.ld_f32 + n] = v;
             if (n < ep.vt_col0) {
-                if (ep.out_act) ((T*)ep.out_act)[(int64_t)row * ep.ld_act + n] = from_f32<T>(v);
+                if (ep.out_act) {
+                    const T hi = from_f32<T>(v);
+                    ((T*)ep.out_act)[(int64_t)row * ep.ld_act + n] = hi;
+                    if (ep.out_act_lo) ((T*)ep.out_act_lo)[(int64_t)row * ep.ld_act + n] = from_f32<T>(v - to_f32<T>(hi));
+                }
             } else {
                 ((T*)ep.out_vt)[(int64_t)(n - ep.vt_col0) * ep.ld_vt + row] = from_f32<T>(v);
             }
@@ -266,7 +278,7 @@ template <typename T, int HD>
 __global__ void __launch_bounds__(128)
 k_attn_simple(const T* __restrict__ QK, const T* __restrict__ VT, int64_t ldvt,
               const int* __restrict__ key_valid, const int* __restrict__ offsets,
-              const int2* __restrict__ work, int tile_q, int d, T* __restrict__ O) {
+              const int2* __restrict__ work, int tile_q, int d, T* __restrict__ O, T* __restrict__ O_lo) {
     __shared__ float Ks[32][HD + 1];
     __shared__ float Vs[32][HD + 1];
     __shared__ int vs[32];
@@ -328,7 +340,12 @@ k_attn_simple(const T* __restrict__ QK, const T* __restrict__ VT, int64_t ldvt,
     if (active) {
         float inv = (l > 0.0f) ? 1.0f / l : 0.0f;
 #pragma unroll
-        for (int c = 0; c < HD; ++c) O[(int64_t)qrow * d + head * HD + c] = from_f32<T>(acc[c] * inv);
+        for (int c = 0; c < HD; ++c) {
+            const float y = acc[c] * inv;
+            const T hi = from_f32<T>(y);
+            O[(int64_t)qrow * d + head * HD + c] = hi;
+            if (O_lo) O_lo[(int64_t)qrow * d + head * HD + c] = from_f32<T>(y - to_f32<T>(hi));
+        }
     }
 }
 
@@ -345,7 +362,7 @@ struct HeadsOut {
 
 template <typename T>
 __global__ void __launch_bounds__(256)
-k_heads_l2(const T* __restrict__ hidden, int N, int d, int ld_hidden, const float* __restrict__ W2,
+k_heads_l2(const T* __restrict__ hidden, const T* __restrict__ hidden_lo, int N, int d, int ld_hidden, const float* __restrict__ W2,
            const float* __restrict__ b2, const int* __restrict__ valid, HeadsOut ho,
            float* __restrict__ out_logits, float* __restrict__ out_regress) {
     int row = blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -358,7 +375,12 @@ k_heads_l2(const T* __restrict__ hidden, int N, int d, int ld_hidden, const floa
         if (ok) {
             const T* hb = hp + ho.blk[o] * d;
             const float* w = W2 + (int64_t)o * d;
-            for (int c = lane; c < d; c += 32) a = fmaf(to_f32<T>(hb[c]), w[c], a);
+            if (hidden_lo) {
+                const T* lb = hidden_lo + (int64_t)row * ld_hidden + ho.blk[o] * d;
+                for (int c = lane; c < d; c += 32) a = fmaf(to_f32<T>(hb[c]) + to_f32<T>(lb[c]), w[c], a);
+            } else {
+                for (int c = lane; c < d; c += 32) a = fmaf(to_f32<T>(hb[c]), w[c], a);
+            }
             a = warp_sum(a) + b2[o];
         }
         if (lane == 0) {

@@ -3,7 +3,7 @@
 #include "common.cuh"
 namespace mlpf {
 constexpr bool TC_ATTN_READY = false;
-static int tc_attn_launch(TcContext* c, const bf16*, const bf16*, int64_t, int64_t, const int*, const int*, const int2*, int, int, int, bf16*, cudaStream_t) {
+static int tc_attn_launch(TcContext* c, const bf16*, const bf16*, int64_t, int64_t, const int*, const int*, const int2*, int, int, int, bf16*, bf16*, cudaStream_t) {
     snprintf(c->err, sizeof c->err, "tcgen05 attention not built"); return -1;
 }
 }
