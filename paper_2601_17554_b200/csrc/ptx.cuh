@@ -19,6 +19,13 @@ __device__ __forceinline__ bool elect_one() {
     return pred != 0;
 }
 
+// 2^x on the MUFU (ex2.approx.ftz): 2^-inf = +0; relative error ~2^-22
+__device__ __forceinline__ float fast_exp2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 // ---------------------------------------------------------------- mbarrier
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");

@@ -171,7 +171,16 @@ def test_edge_cases(lens, pad, precision, tol):
     _, lg, rg = gpu_forward(W, TINY, X, off, precision=precision)
     Wq = oracle.quantize_weights(W) if precision == P.PREC_BF16 else W
     lr, rr = oracle.forward(X, off, Wq, TINY)
-    check(lg, rg, np.arange(X.shape[0]), lr, rr, X, tol, argmax=False)
+    # with a handful of rows the per-column rms of A14 degenerates (one row: rms = |value|), so the floor is
+    # the rms over all valid outputs of the case
+    valid = X[:, 0] != 0
+    assert np.isfinite(lg).all() and np.isfinite(rg).all()
+    assert (lg[~valid] == 0).all() and (rg[~valid] == 0).all()
+    for got, ref in ((lg, lr), (rg, rr)):
+        if valid.any():
+            floor = np.sqrt((ref[valid] ** 2).mean())
+            rel = np.abs(got[valid] - ref[valid]) / np.maximum(np.abs(ref[valid]), floor)
+            assert rel.max() <= tol, rel.max()
 
 
 def test_empty_calls_and_bad_offsets():
