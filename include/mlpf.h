@@ -110,6 +110,8 @@ const char* mlpf_last_error(void);
                                     (embedding hidden, attention output, LN2 / final-LN output, FFN hidden, head
                                     hidden) are carried as two bf16 terms hi + lo and multiplied as two MMAs
                                     (DESIGN.md "error budget").  0: single bf16 term everywhere.          */
+#define MLPF_OPT_PROFILE     6   /* 1: record a CUDA event pair around every kernel class inside mlpf_infer
+                                    (read back with mlpf_debug_get_profile); 0 (default): off            */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0
@@ -154,6 +156,22 @@ int64_t mlpf_debug_get_schedule(mlpf_handle* h, void* stream, int which, int32_t
 #define MLPF_TENSOR_O   4
 #define MLPF_TENSOR_G   5
 int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which, float* host_out, int64_t capacity);
+
+/* per-kernel-class device time of the last mlpf_infer on `stream` run with MLPF_OPT_PROFILE = 1:
+ * ms_out[MLPF_KC_COUNT] (sum over the call's launches of that class) and count_out[MLPF_KC_COUNT]. */
+#define MLPF_KC_SCHED      0   /* a0 */
+#define MLPF_KC_EMBED_L1   1   /* a1 first layer (fp32, CUDA cores) */
+#define MLPF_KC_EMBED_L2   2   /* a1 second layer (grouped GEMM) */
+#define MLPF_KC_LAYERNORM  3   /* a2 */
+#define MLPF_KC_QKV        4   /* a3 */
+#define MLPF_KC_ATTENTION  5   /* a4 */
+#define MLPF_KC_OUTPROJ    6   /* a5 */
+#define MLPF_KC_FFN1       7   /* a6 */
+#define MLPF_KC_FFN2       8   /* a7 */
+#define MLPF_KC_HEADS_L1   9   /* a8 first layers */
+#define MLPF_KC_HEADS_L2   10  /* a8 output rows */
+#define MLPF_KC_COUNT      11
+int mlpf_debug_get_profile(mlpf_handle* h, void* stream, float* ms_out, int32_t* count_out);
 
 /* ---- kernel-level entry points (unit tests and micro-benchmarks; device pointers, bf16 = uint16) ---- */
 /* C[M,N] (fp32, ldc = N) = (A + A_lo)[M,K] (bf16, row-major; A_lo may be NULL) * W[N,K]^T (bf16, row-major)

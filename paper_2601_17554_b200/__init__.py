@@ -16,16 +16,18 @@ LIB_PATH = os.path.join(_HERE, "libmlpf.so")
 
 # include/mlpf.h constants
 OK = 0
-OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT = 1, 2, 3, 4, 5
+OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE = 1, 2, 3, 4, 5, 6
 PREC_BF16, PREC_FP32_DEBUG = 0, 1
 KERNELS_TC, KERNELS_SIMPLE = 0, 1
 Q_N_LAYERS, Q_D_MODEL, Q_N_HEADS, Q_D_FF, Q_N_FEAT, Q_N_CLASSES, Q_N_REGRESS = 1, 2, 3, 4, 5, 6, 7
 Q_WEIGHT_BYTES, Q_WORKSPACE_BYTES, Q_N_PARAMS, Q_LAUNCHES = 8, 9, 10, 11
 SCHED = dict(row_event=0, row_pos=1, valid=2, n_valid=3, type_offsets=4, sorted_row=5, type_perm=6, work_list=7)
 TENSOR = dict(H=0, U=1, QK=2, VT=3, O=4, G=5)
+KERNEL_CLASSES = ["sched", "embed_l1", "embed_l2", "layernorm", "qkv", "attention", "outproj", "ffn1", "ffn2",
+                  "heads_l1", "heads_l2"]
 
 EXPORTS = ["mlpf_create", "mlpf_infer", "mlpf_infer_host", "mlpf_destroy", "mlpf_last_error", "mlpf_set_option",
-           "mlpf_query", "mlpf_debug_get_schedule", "mlpf_debug_get_tensor", "mlpf_tc_gemm_bf16",
+           "mlpf_query", "mlpf_debug_get_schedule", "mlpf_debug_get_tensor", "mlpf_debug_get_profile", "mlpf_tc_gemm_bf16",
            "mlpf_tc_attention_bf16"]
 
 _lib = None
@@ -59,6 +61,8 @@ def lib():
     L.mlpf_debug_get_schedule.argtypes = [vp, vp, C.c_int, vp, i64]
     L.mlpf_debug_get_tensor.restype = i64
     L.mlpf_debug_get_tensor.argtypes = [vp, vp, C.c_int, vp, i64]
+    L.mlpf_debug_get_profile.restype = C.c_int
+    L.mlpf_debug_get_profile.argtypes = [vp, vp, vp, vp]
     L.mlpf_tc_gemm_bf16.restype = C.c_int
     L.mlpf_tc_gemm_bf16.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp]
     L.mlpf_tc_attention_bf16.restype = C.c_int
@@ -149,6 +153,13 @@ class Mlpf:
                                                  out.ctypes.data_as(C.c_void_p), cap))
         out = out[:n].copy()
         return out.reshape(-1, 2) if which == "work_list" else out
+
+    def profile(self, stream=None):
+        """{kernel class: (ms, launches)} of the last infer on `stream` (needs OPT_PROFILE = 1)."""
+        ms = (C.c_float * len(KERNEL_CLASSES))()
+        cnt = (C.c_int32 * len(KERNEL_CLASSES))()
+        _check(lib().mlpf_debug_get_profile(self._h, _stream_ptr(stream), ms, cnt))
+        return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(KERNEL_CLASSES)}
 
     def tensor(self, which: str, shape, stream=None):
         out = np.empty(int(np.prod(shape)), np.float32)

@@ -3,9 +3,8 @@
 // PAPER.md citations: embedding / encoder / heads L156; attention Eq. 4; outputs L126.
 #include "../../include/mlpf.h"
 #include "common.cuh"
-#include "simple_kernels.cuh"
-#include "tc_gemm.cuh"
-#include "tc_attn.cuh"
+#include "simple_api.h"
+#include "tc_api.h"
 
 #include <algorithm>
 #include <cstdarg>
@@ -59,6 +58,9 @@ struct Workspace {
     int *valid = nullptr, *row_event = nullptr, *row_pos = nullptr, *n_valid = nullptr;
     int *block_counts = nullptr, *block_base = nullptr, *type_offsets = nullptr;
     int *sorted_row = nullptr, *type_perm = nullptr;
+    // per-kernel-class CUDA-event timing of the last call (MLPF_OPT_PROFILE)
+    std::vector<cudaEvent_t> ev_pool;
+    std::vector<int> prof_cls;          // class of record i; events 2i, 2i+1
     // last call
     int64_t N = 0, E = 0, n_tiles = 0, n_pairs = 0, m_ub = 0, g_width = 0;
     int tile_q = 128;
@@ -75,7 +77,7 @@ struct mlpf_handle {
     std::vector<LayerW> layers;
     HeadsOut ho;
     // options
-    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = 1;
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = 1, profile = 0;
     int64_t last_launches = 0;
     std::mutex mu;
     std::map<void*, Workspace*> ws;
@@ -228,6 +230,9 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_SPLIT:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "split must be 0 or 1");
             h->split = (int)value; return MLPF_OK;
+        case MLPF_OPT_PROFILE:
+            if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "profile must be 0 or 1");
+            h->profile = (int)value; return MLPF_OK;
         case MLPF_OPT_KERNELS:
             if (value != MLPF_KERNELS_TC && value != MLPF_KERNELS_SIMPLE) return set_err(MLPF_E_ARG, "bad kernel set");
             h->kernels = (int)value; return MLPF_OK;
@@ -337,60 +342,49 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
                                               cudaGetErrorString(e_), __FILE__, __LINE__);                \
     } while (0)
 
-template <typename T>
-static int run_gemm(mlpf_handle* h, bool tc, const T* A, const T* A_lo, const T* W, int M, int N, int K, const Epi& ep,
-                    cudaStream_t st) {
+struct ProfScope {           // records a CUDA event pair around one kernel class when profiling is on
+    Workspace* w; cudaStream_t st; bool on;
+    ProfScope(mlpf_handle* h, Workspace* w_, cudaStream_t st_, int cls) : w(w_), st(st_), on(h->profile != 0) {
+        if (!on) return;
+        size_t i = w->prof_cls.size();
+        while (w->ev_pool.size() < 2 * (i + 1)) { cudaEvent_t e; cudaEventCreate(&e); w->ev_pool.push_back(e); }
+        w->prof_cls.push_back(cls);
+        cudaEventRecord(w->ev_pool[2 * i], st);
+    }
+    ~ProfScope() { if (on) cudaEventRecord(w->ev_pool[2 * w->prof_cls.size() - 1], st); }
+};
+
+static int run_gemm(mlpf_handle* h, bool fp32, bool tc, const void* A, const void* A_lo, const void* W, int M, int N, int K,
+                    const Epi& ep, cudaStream_t st) {
     if (M <= 0) return MLPF_OK;
-    if (tc) {
-        if constexpr (std::is_same<T, bf16>::value) {
-            int rc = tc_gemm_launch(&h->tc, A, A_lo, W, M, N, K, ep, st);
-            if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", h->tc.err);
-            LAUNCH_CHECK(h);
-            return MLPF_OK;
-        }
-    }
-    dim3 grid(N / 64, (M + 63) / 64);
-    k_gemm_simple<T><<<grid, 256, 0, st>>>(A, A_lo, W, M, N, K, ep);
-    LAUNCH_CHECK(h);
-    return MLPF_OK;
-}
-
-template <typename T>
-static int run_layernorm(mlpf_handle* h, const float* x, int N, const float* g, const float* b, T* u, T* u_lo, cudaStream_t st) {
-    dim3 grid((N + 7) / 8);
-    switch (h->d) {
-        case 64:  k_layernorm<T, 64><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
-        case 128: k_layernorm<T, 128><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
-        case 192: k_layernorm<T, 192><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
-        case 256: k_layernorm<T, 256><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
-        case 320: k_layernorm<T, 320><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
-        case 384: k_layernorm<T, 384><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
-        case 448: k_layernorm<T, 448><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
-        case 512: k_layernorm<T, 512><<<grid, 256, 0, st>>>(x, N, g, b, h->hp.ln_eps, u, u_lo); break;
-        default: return set_err(MLPF_E_ARG, "d_model %d unsupported by LayerNorm", h->d);
+    if (tc && !fp32) {
+        int rc = tc_gemm_launch(&h->tc, (const bf16*)A, (const bf16*)A_lo, (const bf16*)W, M, N, K, ep, st);
+        if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", h->tc.err);
+    } else {
+        launch_gemm_simple(fp32, A, A_lo, W, M, N, K, ep, st);
     }
     LAUNCH_CHECK(h);
     return MLPF_OK;
 }
 
-template <typename T>
-static int run_attention(mlpf_handle* h, bool tc, bool split, Workspace* w, cudaStream_t st) {
+static int run_layernorm(mlpf_handle* h, bool fp32, const float* x, int N, const float* g, const float* b, void* u, void* u_lo,
+                         cudaStream_t st) {
+    if (launch_layernorm(fp32, h->d, x, N, g, b, h->hp.ln_eps, u, u_lo, st))
+        return set_err(MLPF_E_ARG, "d_model %d unsupported by LayerNorm", h->d);
+    LAUNCH_CHECK(h);
+    return MLPF_OK;
+}
+
+static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspace* w, cudaStream_t st) {
     if (w->n_tiles == 0) return MLPF_OK;
-    if (tc) {
-        if constexpr (std::is_same<T, bf16>::value) {
-            int rc = tc_attn_launch(&h->tc, (const bf16*)w->qk, (const bf16*)w->vt, w->ldvt, w->N, w->valid, w->offsets,
-                                    (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, (bf16*)w->o, split ? (bf16*)w->o_lo : nullptr, st);
-            if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", h->tc.err);
-            LAUNCH_CHECK(h);
-            return MLPF_OK;
-        }
-    }
-    dim3 grid((unsigned)w->n_tiles, h->H);
-    const T* qk = (const T*)w->qk; const T* vt = (const T*)w->vt; T* o = (T*)w->o; T* o_lo = split ? (T*)w->o_lo : nullptr;
-    switch (h->hd) {
-        case 16: k_attn_simple<T, 16><<<grid, w->tile_q, 0, st>>>(qk, vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, w->tile_q, h->d, o, o_lo); break;
-        case 32: k_attn_simple<T, 32><<<grid, w->tile_q, 0, st>>>(qk, vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, w->tile_q, h->d, o, o_lo); break;
-        case 64: k_attn_simple<T, 64><<<grid, w->tile_q, 0, st>>>(qk, vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, w->tile_q, h->d, o, o_lo); break;
+    if (tc && !fp32) {
+        int rc = tc_attn_launch(&h->tc, (const bf16*)w->qk, (const bf16*)w->vt, w->ldvt, w->N, w->valid, w->offsets,
+                                (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, (bf16*)w->o,
+                                split ? (bf16*)w->o_lo : nullptr, st);
+        if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", h->tc.err);
+    } else {
+        launch_attn_simple(fp32, h->hd, w->qk, w->vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, (int)w->n_tiles,
+                           h->H, w->tile_q, h->d, w->o, split ? w->o_lo : nullptr, st);
     }
     LAUNCH_CHECK(h);
     return MLPF_OK;
@@ -412,38 +406,41 @@ static void build_work_lists(const int32_t* off, int E, int tile_q, std::vector<
     }
 }
 
-template <typename T>
-static int infer_impl(mlpf_handle* h, Workspace* w, const float* X, float* out_logits, float* out_regress, cudaStream_t st) {
+static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, float* out_logits, float* out_regress, cudaStream_t st) {
     const int N = (int)w->N, E = (int)w->E, d = h->d, dff = h->dff;
-    const bool fp32 = std::is_same<T, float>::value;
     const bool tc_req = !fp32 && h->kernels == MLPF_KERNELS_TC;
-    const bool tc = tc_req && TC_GEMM_READY;
-    const bool tc_attn = tc_req && TC_ATTN_READY;
-    const T* PW = fp32 ? (const T*)h->P32 : (const T*)h->P16;
+    const bool tc = tc_req, tc_attn = tc_req;
+    const int64_t es = fp32 ? 4 : 2;
+    const char* PWb = fp32 ? (const char*)h->P32 : (const char*)h->P16;
+    auto PW = [&](int64_t off) { return (const void*)(PWb + off * es); };
     const float* PV = h->P32;
     const bool split = !fp32 && h->split != 0;     // bf16 activations carried as hi + lo where they feed the residual stream
-    T* u = (T*)w->u; T* g = (T*)w->g;
-    T* u_lo = split ? (T*)w->u_lo : nullptr; T* g_lo = split ? (T*)w->g_lo : nullptr; T* o_lo = split ? (T*)w->o_lo : nullptr;
+    void* u = w->u; void* g = w->g;
+    void* u_lo = split ? w->u_lo : nullptr; void* g_lo = split ? w->g_lo : nullptr; void* o_lo = split ? w->o_lo : nullptr;
 
     // ---- a0 (device half)
-    const int nb = (N + SCHED_BLOCK - 1) / SCHED_BLOCK;
+    w->prof_cls.clear();
+    {
+    ProfScope ps(h, w, st, MLPF_KC_SCHED);
     CUDA_TRY(cudaMemsetAsync(w->n_valid, 0, (size_t)E * 4, st));
     CUDA_TRY(cudaMemsetAsync(w->type_perm, 0xff, (size_t)w->m_ub * 4, st));
-    k_sched_count<<<nb, SCHED_BLOCK, 0, st>>>(X, N, h->F, w->offsets, E, w->block_counts, w->valid, w->row_event, w->row_pos, w->n_valid);
+    h->last_launches += launch_schedule(X, N, h->F, w->offsets, E, w->block_counts, w->block_base, w->valid, w->row_event,
+                                        w->row_pos, w->n_valid, w->type_offsets, w->sorted_row, w->type_perm, st) - 1;
     LAUNCH_CHECK(h);
-    k_sched_scan<<<1, 32, 0, st>>>(w->block_counts, nb, w->block_base, w->type_offsets);
-    LAUNCH_CHECK(h);
-    k_sched_scatter<<<nb, SCHED_BLOCK, 0, st>>>(X, N, h->F, w->block_base, w->type_offsets, w->sorted_row, w->type_perm);
-    LAUNCH_CHECK(h);
+    }
 
     // ---- a1: per-type embedding (L156; A3-A5)
-    k_embed_l1<T><<<(N + EMB_ROWS - 1) / EMB_ROWS, 256, 0, st>>>(X, N, h->F, d, PV + h->embW1t, PV + h->embB1, h->act, w->sorted_row, g, g_lo, w->h);
-    LAUNCH_CHECK(h);
     {
+    ProfScope ps(h, w, st, MLPF_KC_EMBED_L1);
+    launch_embed_l1(fp32, X, N, h->F, d, PV + h->embW1t, PV + h->embB1, h->act, w->sorted_row, g, g_lo, w->h, st);
+    LAUNCH_CHECK(h);
+    }
+    {
+        ProfScope ps(h, w, st, MLPF_KC_EMBED_L2);
         Epi ep;
         ep.bias = PV + h->embB2; ep.out_f32 = w->h; ep.ld_f32 = d;
         ep.row_perm = w->type_perm; ep.group_offsets = w->type_offsets; ep.n_groups = 4;
-        int rc = run_gemm<T>(h, tc, g, g_lo, PW + h->embW2, (int)w->m_ub, d, d, ep, st);
+        int rc = run_gemm(h, fp32, tc, g, g_lo, PW(h->embW2), (int)w->m_ub, d, d, ep, st);
         if (rc) return rc;
     }
     if (h->tap_layer == -2) return MLPF_OK;
@@ -451,35 +448,49 @@ static int infer_impl(mlpf_handle* h, Workspace* w, const float* X, float* out_l
     // ---- encoder blocks (pre-LN, L156 + A7)
     for (int l = 0; l < h->L; ++l) {
         const LayerW& lw = h->layers[l];
-        int rc = run_layernorm<T>(h, w->h, N, PV + lw.ln1g, PV + lw.ln1b, u, (T*)nullptr, st);                     // a2
+        int rc;
+        {
+            ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);
+            rc = run_layernorm(h, fp32, w->h, N, PV + lw.ln1g, PV + lw.ln1b, u, nullptr, st);                     // a2
+        }
         if (rc) return rc;
         {   // a3: [Q K V] = LN1(x) Wqkv^T + bqkv ; V stored transposed per head dim
+            ProfScope ps(h, w, st, MLPF_KC_QKV);
             Epi ep;
             ep.bias = PV + lw.bqkv; ep.out_act = w->qk; ep.ld_act = 2 * d;
             ep.out_vt = w->vt; ep.ld_vt = w->ldvt; ep.vt_col0 = 2 * d;
-            rc = run_gemm<T>(h, tc, u, (const T*)nullptr, PW + lw.Wqkv, N, 3 * d, d, ep, st);
+            rc = run_gemm(h, fp32, tc, u, nullptr, PW(lw.Wqkv), N, 3 * d, d, ep, st);
             if (rc) return rc;
         }
-        rc = run_attention<T>(h, tc_attn, split, w, st);                                                         // a4
+        {
+            ProfScope ps(h, w, st, MLPF_KC_ATTENTION);
+            rc = run_attention(h, fp32, tc_attn, split, w, st);                                                     // a4
+        }
         if (rc) return rc;
         {   // a5: h <- h + O Wo^T + bo
+            ProfScope ps(h, w, st, MLPF_KC_OUTPROJ);
             Epi ep;
             ep.bias = PV + lw.bo; ep.residual = w->h; ep.ld_res = d; ep.out_f32 = w->h; ep.ld_f32 = d;
-            rc = run_gemm<T>(h, tc, (const T*)w->o, o_lo, PW + lw.Wo, N, d, d, ep, st);
+            rc = run_gemm(h, fp32, tc, w->o, o_lo, PW(lw.Wo), N, d, d, ep, st);
             if (rc) return rc;
         }
-        rc = run_layernorm<T>(h, w->h, N, PV + lw.ln2g, PV + lw.ln2b, u, u_lo, st);
+        {
+            ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);
+            rc = run_layernorm(h, fp32, w->h, N, PV + lw.ln2g, PV + lw.ln2b, u, u_lo, st);
+        }
         if (rc) return rc;
         {   // a6: g = act(LN2(h) W1^T + b1)
+            ProfScope ps(h, w, st, MLPF_KC_FFN1);
             Epi ep;
             ep.bias = PV + lw.b1; ep.act = h->act; ep.out_act = g; ep.out_act_lo = g_lo; ep.ld_act = dff;
-            rc = run_gemm<T>(h, tc, u, u_lo, PW + lw.W1, N, dff, d, ep, st);
+            rc = run_gemm(h, fp32, tc, u, u_lo, PW(lw.W1), N, dff, d, ep, st);
             if (rc) return rc;
         }
         {   // a7: h <- h + g W2^T + b2
+            ProfScope ps(h, w, st, MLPF_KC_FFN2);
             Epi ep;
             ep.bias = PV + lw.b2; ep.residual = w->h; ep.ld_res = d; ep.out_f32 = w->h; ep.ld_f32 = d;
-            rc = run_gemm<T>(h, tc, g, g_lo, PW + lw.W2, N, d, dff, ep, st);
+            rc = run_gemm(h, fp32, tc, g, g_lo, PW(lw.W2), N, d, dff, ep, st);
             if (rc) return rc;
         }
         w->g_width = dff;
@@ -488,7 +499,8 @@ static int infer_impl(mlpf_handle* h, Workspace* w, const float* X, float* out_l
 
     // ---- a8: heads (L156; A11-A12)
     if (h->hp.final_ln) {
-        int rc = run_layernorm<T>(h, w->h, N, PV + h->lnfg, PV + h->lnfb, u, u_lo, st);
+        ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);
+        int rc = run_layernorm(h, fp32, w->h, N, PV + h->lnfg, PV + h->lnfb, u, u_lo, st);
         if (rc) return rc;
     } else {
         // no final LN: u = T(h).  (identity affine with the row kept: done by a cast kernel)
@@ -498,10 +510,15 @@ static int infer_impl(mlpf_handle* h, Workspace* w, const float* X, float* out_l
         Epi ep;
         const int hw = h->n_hblk * d;
         ep.bias = PV + h->headB1; ep.act = h->act; ep.out_act = g; ep.out_act_lo = g_lo; ep.ld_act = hw;
-        int rc = run_gemm<T>(h, tc, u, u_lo, PW + h->headW1, N, hw, d, ep, st);
+        int rc;
+        {
+            ProfScope ps(h, w, st, MLPF_KC_HEADS_L1);
+            rc = run_gemm(h, fp32, tc, u, u_lo, PW(h->headW1), N, hw, d, ep, st);
+        }
         if (rc) return rc;
         w->g_width = hw;
-        k_heads_l2<T><<<(N + 7) / 8, 256, 0, st>>>(g, g_lo, N, d, hw, PV + h->headW2, PV + h->headB2, w->valid, h->ho, out_logits, out_regress);
+        ProfScope ps(h, w, st, MLPF_KC_HEADS_L2);
+        launch_heads_l2(fp32, g, g_lo, N, d, hw, PV + h->headW2, PV + h->headB2, w->valid, h->ho, out_logits, out_regress, st);
         LAUNCH_CHECK(h);
     }
     return MLPF_OK;
@@ -538,8 +555,7 @@ extern "C" int mlpf_infer(mlpf_handle* h, const float* elements, const int32_t* 
     CUDA_TRY(cudaMemcpyAsync(w->offsets, event_offsets, (size_t)(n_events + 1) * 4, cudaMemcpyHostToDevice, st));
     if (!work.empty()) CUDA_TRY(cudaMemcpyAsync(w->work, work.data(), work.size() * 4, cudaMemcpyHostToDevice, st));
     if (!pairs.empty()) CUDA_TRY(cudaMemcpyAsync(w->pairs, pairs.data(), pairs.size() * 4, cudaMemcpyHostToDevice, st));
-    if (fp32) rc = infer_impl<float>(h, w, elements, out_logits, out_regress, st);
-    else rc = infer_impl<bf16>(h, w, elements, out_logits, out_regress, st);
+    rc = infer_impl(h, fp32, w, elements, out_logits, out_regress, st);
     if (rc == MLPF_OK) g_err.clear();
     return rc;
 }
@@ -600,12 +616,10 @@ extern "C" int64_t mlpf_debug_get_schedule(mlpf_handle* h, void* stream, int whi
     return n;
 }
 
-template <typename T>
-static int tap_copy(const void* src, int64_t rows, int64_t cols, int64_t ld, float* host_out) {
+static int tap_copy(bool fp32, const void* src, int64_t rows, int64_t cols, int64_t ld, float* host_out) {
     float* tmp = nullptr;
     CUDA_TRY(cudaMalloc(&tmp, (size_t)rows * ld * 4));
-    int64_t n = rows * ld;
-    k_to_f32<T><<<(unsigned)((n + 255) / 256), 256>>>((const T*)src, tmp, n);
+    launch_to_f32(fp32, src, tmp, rows * ld, 0);
     cudaError_t e = cudaMemcpy2D(host_out, (size_t)cols * 4, tmp, (size_t)ld * 4, (size_t)cols * 4, (size_t)rows, cudaMemcpyDeviceToHost);
     cudaFree(tmp);
     if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tap copy failed: %s", cudaGetErrorString(e));
@@ -635,9 +649,26 @@ extern "C" int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which
         default: return set_err(MLPF_E_ARG, "unknown tensor %d", which);
     }
     if (rows * cols > capacity) return set_err(MLPF_E_ARG, "capacity too small");
-    int rc = w->fp32 ? tap_copy<float>(src, rows, cols, ld, host_out) : tap_copy<bf16>(src, rows, cols, ld, host_out);
+    int rc = tap_copy(w->fp32, src, rows, cols, ld, host_out);
     if (rc) return rc;
     return rows * cols;
+}
+
+extern "C" int mlpf_debug_get_profile(mlpf_handle* h, void* stream, float* ms_out, int32_t* count_out) {
+    if (!h || !ms_out || !count_out) return set_err(MLPF_E_NULL, "NULL argument");
+    std::lock_guard<std::mutex> lk(h->mu);
+    auto it = h->ws.find(stream);
+    if (it == h->ws.end()) return set_err(MLPF_E_ARG, "no mlpf_infer ran on this stream");
+    Workspace* w = it->second;
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+    for (int i = 0; i < MLPF_KC_COUNT; ++i) { ms_out[i] = 0.0f; count_out[i] = 0; }
+    for (size_t i = 0; i < w->prof_cls.size(); ++i) {
+        float ms = 0.0f;
+        CUDA_TRY(cudaEventElapsedTime(&ms, w->ev_pool[2 * i], w->ev_pool[2 * i + 1]));
+        ms_out[w->prof_cls[i]] += ms;
+        count_out[w->prof_cls[i]] += 1;
+    }
+    return MLPF_OK;
 }
 
 // ------------------------------------------------------------------------------------------------ kernel-level entries

@@ -1,0 +1,34 @@
+// simple_api.h -- host-side launchers of the CUDA-core kernels (simple_kernels.cu).  `fp32` selects the
+// element type of activations / weights (float for the fp32 debug path, bf16 otherwise).
+#pragma once
+#include "common.cuh"
+
+namespace mlpf {
+
+constexpr int SCHED_BLOCK = 1024;
+constexpr int EMB_ROWS = 64;
+constexpr int MAX_OUT = 24;
+struct HeadsOut {
+    int n_out; int n_cls; int n_reg;
+    int blk[MAX_OUT];
+};
+
+// a0 device half: 3 launches.  Returns the number of kernels launched.
+int launch_schedule(const float* X, int N, int F, const int* offsets, int E, int* block_counts, int* block_base,
+                    int* valid, int* row_event, int* row_pos, int* n_valid, int* type_offsets, int* sorted_row,
+                    int* type_perm, cudaStream_t st);
+void launch_embed_l1(bool fp32, const float* X, int N, int F, int d, const float* W1t, const float* b1, int act,
+                     const int* sorted_row, void* h1, void* h1_lo, float* h, cudaStream_t st);
+int launch_layernorm(bool fp32, int d, const float* x, int N, const float* g, const float* b, float eps, void* u,
+                     void* u_lo, cudaStream_t st);
+void launch_gemm_simple(bool fp32, const void* A, const void* A_lo, const void* W, int M, int N, int K, const Epi& ep,
+                        cudaStream_t st);
+void launch_attn_simple(bool fp32, int hd, const void* QK, const void* VT, int64_t ldvt, const int* key_valid,
+                        const int* offsets, const int2* work, int n_tiles, int H, int tile_q, int d, void* O,
+                        void* O_lo, cudaStream_t st);
+void launch_heads_l2(bool fp32, const void* hidden, const void* hidden_lo, int N, int d, int ld_hidden,
+                     const float* W2, const float* b2, const int* valid, const HeadsOut& ho, float* out_logits,
+                     float* out_regress, cudaStream_t st);
+void launch_to_f32(bool fp32, const void* src, float* dst, int64_t n, cudaStream_t st);
+
+}  // namespace mlpf

@@ -4,15 +4,13 @@
 //  * the tiled FFMA GEMM and the one-thread-per-query attention are the fp32 debug path
 //    (MLPF_PREC_FP32_DEBUG, parity <= 1e-4) and the MLPF_KERNELS_SIMPLE debugging aid in bf16.
 // Citations are /root/reference/PAPER.md lines; readings A* are listed in DESIGN.md.
-#pragma once
-#include "common.cuh"
+#include "simple_api.h"
 
 namespace mlpf {
 
 // ------------------------------------------------------------------------------------------------
 // a0: integer schedule on the device (the type id lives in device memory: reading A1)
 // ------------------------------------------------------------------------------------------------
-constexpr int SCHED_BLOCK = 1024;
 
 __device__ __forceinline__ int element_type(const float* __restrict__ X, int64_t row, int F) {
     float x0 = X[row * F];
@@ -113,7 +111,6 @@ k_sched_scatter(const float* __restrict__ X, int N, int F, const int* __restrict
 // Pad rows (type 0): the residual stream row h[i,:] is set to exactly 0 (reading A2).
 // W1t is [T][64][d] (k-major, zero padded to 64 features) so loads are coalesced over the d outputs.
 // ------------------------------------------------------------------------------------------------
-constexpr int EMB_ROWS = 64;
 
 template <typename T>
 __global__ void __launch_bounds__(256)
@@ -354,11 +351,6 @@ k_attn_simple(const T* __restrict__ QK, const T* __restrict__ VT, int64_t ldvt,
 // row; rows with valid == 0 are written as exactly 0 (A2).  hidden = [N, n_blocks*d]; output o reads
 // hidden block blk[o].  Outputs 0..C-1 -> logits, C.. -> regress.
 // ------------------------------------------------------------------------------------------------
-constexpr int MAX_OUT = 24;
-struct HeadsOut {
-    int n_out; int n_cls; int n_reg;
-    int blk[MAX_OUT];
-};
 
 template <typename T>
 __global__ void __launch_bounds__(256)
@@ -395,6 +387,84 @@ template <typename T>
 __global__ void k_to_f32(const T* __restrict__ src, float* __restrict__ dst, int64_t n) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) dst[i] = to_f32<T>(src[i]);
+}
+
+// ------------------------------------------------------------------------------------------------ launchers
+int launch_schedule(const float* X, int N, int F, const int* offsets, int E, int* block_counts, int* block_base,
+                    int* valid, int* row_event, int* row_pos, int* n_valid, int* type_offsets, int* sorted_row,
+                    int* type_perm, cudaStream_t st) {
+    const int nb = (N + SCHED_BLOCK - 1) / SCHED_BLOCK;
+    k_sched_count<<<nb, SCHED_BLOCK, 0, st>>>(X, N, F, offsets, E, block_counts, valid, row_event, row_pos, n_valid);
+    k_sched_scan<<<1, 32, 0, st>>>(block_counts, nb, block_base, type_offsets);
+    k_sched_scatter<<<nb, SCHED_BLOCK, 0, st>>>(X, N, F, block_base, type_offsets, sorted_row, type_perm);
+    return 3;
+}
+
+void launch_embed_l1(bool fp32, const float* X, int N, int F, int d, const float* W1t, const float* b1, int act,
+                     const int* sorted_row, void* h1, void* h1_lo, float* h, cudaStream_t st) {
+    dim3 grid((N + EMB_ROWS - 1) / EMB_ROWS);
+    if (fp32) k_embed_l1<float><<<grid, 256, 0, st>>>(X, N, F, d, W1t, b1, act, sorted_row, (float*)h1, (float*)h1_lo, h);
+    else k_embed_l1<bf16><<<grid, 256, 0, st>>>(X, N, F, d, W1t, b1, act, sorted_row, (bf16*)h1, (bf16*)h1_lo, h);
+}
+
+template <typename T>
+static int layernorm_d(int d, const float* x, int N, const float* g, const float* b, float eps, T* u, T* u_lo, cudaStream_t st) {
+    dim3 grid((N + 7) / 8);
+    switch (d) {
+        case 64:  k_layernorm<T, 64><<<grid, 256, 0, st>>>(x, N, g, b, eps, u, u_lo); break;
+        case 128: k_layernorm<T, 128><<<grid, 256, 0, st>>>(x, N, g, b, eps, u, u_lo); break;
+        case 192: k_layernorm<T, 192><<<grid, 256, 0, st>>>(x, N, g, b, eps, u, u_lo); break;
+        case 256: k_layernorm<T, 256><<<grid, 256, 0, st>>>(x, N, g, b, eps, u, u_lo); break;
+        case 320: k_layernorm<T, 320><<<grid, 256, 0, st>>>(x, N, g, b, eps, u, u_lo); break;
+        case 384: k_layernorm<T, 384><<<grid, 256, 0, st>>>(x, N, g, b, eps, u, u_lo); break;
+        case 448: k_layernorm<T, 448><<<grid, 256, 0, st>>>(x, N, g, b, eps, u, u_lo); break;
+        case 512: k_layernorm<T, 512><<<grid, 256, 0, st>>>(x, N, g, b, eps, u, u_lo); break;
+        default: return -1;
+    }
+    return 0;
+}
+int launch_layernorm(bool fp32, int d, const float* x, int N, const float* g, const float* b, float eps, void* u,
+                     void* u_lo, cudaStream_t st) {
+    return fp32 ? layernorm_d<float>(d, x, N, g, b, eps, (float*)u, (float*)u_lo, st)
+                : layernorm_d<bf16>(d, x, N, g, b, eps, (bf16*)u, (bf16*)u_lo, st);
+}
+
+void launch_gemm_simple(bool fp32, const void* A, const void* A_lo, const void* W, int M, int N, int K, const Epi& ep,
+                        cudaStream_t st) {
+    dim3 grid(N / 64, (M + 63) / 64);
+    if (fp32) k_gemm_simple<float><<<grid, 256, 0, st>>>((const float*)A, (const float*)A_lo, (const float*)W, M, N, K, ep);
+    else k_gemm_simple<bf16><<<grid, 256, 0, st>>>((const bf16*)A, (const bf16*)A_lo, (const bf16*)W, M, N, K, ep);
+}
+
+template <typename T>
+static void attn_simple_hd(int hd, const T* QK, const T* VT, int64_t ldvt, const int* key_valid, const int* offsets,
+                           const int2* work, int n_tiles, int H, int tile_q, int d, T* O, T* O_lo, cudaStream_t st) {
+    dim3 grid((unsigned)n_tiles, H);
+    switch (hd) {
+        case 16: k_attn_simple<T, 16><<<grid, tile_q, 0, st>>>(QK, VT, ldvt, key_valid, offsets, work, tile_q, d, O, O_lo); break;
+        case 32: k_attn_simple<T, 32><<<grid, tile_q, 0, st>>>(QK, VT, ldvt, key_valid, offsets, work, tile_q, d, O, O_lo); break;
+        case 64: k_attn_simple<T, 64><<<grid, tile_q, 0, st>>>(QK, VT, ldvt, key_valid, offsets, work, tile_q, d, O, O_lo); break;
+    }
+}
+void launch_attn_simple(bool fp32, int hd, const void* QK, const void* VT, int64_t ldvt, const int* key_valid,
+                        const int* offsets, const int2* work, int n_tiles, int H, int tile_q, int d, void* O,
+                        void* O_lo, cudaStream_t st) {
+    if (fp32) attn_simple_hd<float>(hd, (const float*)QK, (const float*)VT, ldvt, key_valid, offsets, work, n_tiles, H, tile_q, d, (float*)O, (float*)O_lo, st);
+    else attn_simple_hd<bf16>(hd, (const bf16*)QK, (const bf16*)VT, ldvt, key_valid, offsets, work, n_tiles, H, tile_q, d, (bf16*)O, (bf16*)O_lo, st);
+}
+
+void launch_heads_l2(bool fp32, const void* hidden, const void* hidden_lo, int N, int d, int ld_hidden,
+                     const float* W2, const float* b2, const int* valid, const HeadsOut& ho, float* out_logits,
+                     float* out_regress, cudaStream_t st) {
+    dim3 grid((N + 7) / 8);
+    if (fp32) k_heads_l2<float><<<grid, 256, 0, st>>>((const float*)hidden, (const float*)hidden_lo, N, d, ld_hidden, W2, b2, valid, ho, out_logits, out_regress);
+    else k_heads_l2<bf16><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, W2, b2, valid, ho, out_logits, out_regress);
+}
+
+void launch_to_f32(bool fp32, const void* src, float* dst, int64_t n, cudaStream_t st) {
+    unsigned grid = (unsigned)((n + 255) / 256);
+    if (fp32) k_to_f32<float><<<grid, 256, 0, st>>>((const float*)src, dst, n);
+    else k_to_f32<bf16><<<grid, 256, 0, st>>>((const bf16*)src, dst, n);
 }
 
 }  // namespace mlpf

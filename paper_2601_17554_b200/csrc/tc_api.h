@@ -1,0 +1,49 @@
+// tc_api.h -- host-side interface of the tensor-core kernels (tc_gemm.cu, tc_attn.cu).
+#pragma once
+#include <cuda.h>
+#include <mutex>
+#include <unordered_map>
+#include "common.cuh"
+
+namespace mlpf {
+
+// ------------------------------------------------------------------------------------------------ host context
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct TcContext {
+    char err[256] = {0};
+    PFN_encodeTiled encode = nullptr;
+    int num_sms = 148;
+    std::mutex mu;
+    struct Key {
+        const void* p; uint64_t d0, d1, ld; uint32_t b0, b1, sw;
+        bool operator==(const Key& o) const { return p == o.p && d0 == o.d0 && d1 == o.d1 && ld == o.ld && b0 == o.b0 && b1 == o.b1 && sw == o.sw; }
+    };
+    struct KeyHash {
+        size_t operator()(const Key& k) const {
+            uint64_t h = (uint64_t)k.p * 0x9E3779B97F4A7C15ull;
+            h ^= k.d0 + 0x9E3779B97F4A7C15ull + (h << 6) + (h >> 2);
+            h ^= k.d1 + 0x9E3779B97F4A7C15ull + (h << 6) + (h >> 2);
+            h ^= k.ld + (h << 6) + (h >> 2);
+            h ^= ((uint64_t)k.b0 << 32 | k.b1) + (h << 6) + (h >> 2);
+            return (size_t)(h ^ k.sw);
+        }
+    };
+    std::unordered_map<Key, CUtensorMap, KeyHash> cache;
+};
+
+
+int tc_init(TcContext* c);
+// 2D bf16 tensor map: dims (d0 inner, d1 outer), row pitch ld elements, box (b0, b1), swizzle = b0 * 2 bytes
+int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64_t ld,
+                  uint32_t b0, uint32_t b1);
+// C = (A + A_lo) W^T with the shared epilogue; A_lo == nullptr -> plain bf16 A.  N % 64 == 0, K % 64 == 0.
+int tc_gemm_launch(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W, int M, int N, int K,
+                   const Epi& ep, cudaStream_t st);
+int tc_attn_launch(TcContext* c, const bf16* QK, const bf16* VT, int64_t ldvt, int64_t N, const int* key_valid,
+                   const int* offsets, const int2* pairs, int n_pairs, int d, int H, bf16* O, bf16* O_lo,
+                   cudaStream_t st);
+
+}  // namespace mlpf

@@ -14,14 +14,11 @@
 // The two warpgroups run half a period apart (S_t(j+1) is issued right after P_t(j) V_j), so one of
 // them is exponentiating while the other waits for the tensor pipe.
 // TMEM columns: S_a [0,128) S_b [128,256) (P_t aliases the first 64 columns of S_t), O_t[buf] at 256 + (2t+buf) hd.
-#pragma once
-#include "common.cuh"
+#include "tc_api.h"
 #include "ptx.cuh"
-#include "tc_gemm.cuh"
 
 namespace mlpf {
 
-constexpr bool TC_ATTN_READY = true;
 constexpr int ATT_THREADS = 320;
 constexpr int ATT_BQ = 128, ATT_BK = 128;
 
@@ -235,13 +232,16 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__ CUte
                 }
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
+                // O_t(j-1) was issued a whole softmax period ago: this wait does not stall, but it must come
+                // BEFORE P_t(j) is published -- afterwards O_t(j) could complete too and the barrier would be two
+                // phases ahead of this waiter (parity aliasing).
+                if (j > 0) ptx::mbar_wait(bar_o + 8 * t, (j - 1) & 1);
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(bar_p + 8 * t);
                 l_run = l_run * corr + rsum;
                 m_run = m_new;
                 // fold the previous tile's P V into the register accumulator
                 if (j > 0) {
-                    ptx::mbar_wait(bar_o + 8 * t, (j - 1) & 1);
                     ptx::tc_fence_after();
                     const uint32_t o_addr = lane_addr + 256 + (2 * t + ((j - 1) & 1)) * HD;
 #pragma unroll
@@ -315,7 +315,7 @@ static int tc_attn_launch_hd(TcContext* c, const bf16* QK, const bf16* VT, int64
     return 0;
 }
 
-static int tc_attn_launch(TcContext* c, const bf16* QK, const bf16* VT, int64_t ldvt, int64_t N, const int* key_valid,
+int tc_attn_launch(TcContext* c, const bf16* QK, const bf16* VT, int64_t ldvt, int64_t N, const int* key_valid,
                           const int* offsets, const int2* pairs, int n_pairs, int d, int H, bf16* O, bf16* O_lo,
                           cudaStream_t st) {
     const int hd = d / H;

@@ -7,45 +7,12 @@
 // Two CTAs are co-resident per SM so one tile's epilogue overlaps the other's main loop.
 // SPLIT: A is given as two bf16 terms (A = A_hi + A_lo); both are multiplied by the same W tile into the
 // same accumulator, so activation rounding is ~2^-17 instead of 2^-9.
-#pragma once
-#include <cuda.h>
-#include <mutex>
-#include <unordered_map>
-#include "common.cuh"
+#include "tc_api.h"
 #include "ptx.cuh"
 
 namespace mlpf {
 
-constexpr bool TC_GEMM_READY = true;
-
-// ------------------------------------------------------------------------------------------------ host context
-typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-struct TcContext {
-    char err[256] = {0};
-    PFN_encodeTiled encode = nullptr;
-    int num_sms = 148;
-    std::mutex mu;
-    struct Key {
-        const void* p; uint64_t d0, d1, ld; uint32_t b0, b1, sw;
-        bool operator==(const Key& o) const { return p == o.p && d0 == o.d0 && d1 == o.d1 && ld == o.ld && b0 == o.b0 && b1 == o.b1 && sw == o.sw; }
-    };
-    struct KeyHash {
-        size_t operator()(const Key& k) const {
-            uint64_t h = (uint64_t)k.p * 0x9E3779B97F4A7C15ull;
-            h ^= k.d0 + 0x9E3779B97F4A7C15ull + (h << 6) + (h >> 2);
-            h ^= k.d1 + 0x9E3779B97F4A7C15ull + (h << 6) + (h >> 2);
-            h ^= k.ld + (h << 6) + (h >> 2);
-            h ^= ((uint64_t)k.b0 << 32 | k.b1) + (h << 6) + (h >> 2);
-            return (size_t)(h ^ k.sw);
-        }
-    };
-    std::unordered_map<Key, CUtensorMap, KeyHash> cache;
-};
-
-static int tc_init(TcContext* c) {
+int tc_init(TcContext* c) {
     c->err[0] = 0;
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult q;
@@ -61,8 +28,7 @@ static int tc_init(TcContext* c) {
     return 0;
 }
 
-// 2D bf16 tensor map: dims (d0 inner, d1 outer), row pitch ld elements, box (b0, b1), swizzle = b0 * 2 bytes
-static int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64_t ld,
+int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64_t ld,
                          uint32_t b0, uint32_t b1) {
     const uint32_t sw_bytes = b0 * 2;
     TcContext::Key key{ptr, d0, d1, ld, b0, b1, sw_bytes};
@@ -280,8 +246,7 @@ static int tc_gemm_launch_cfg(TcContext* c, const bf16* A, const bf16* A_lo, con
     return 0;
 }
 
-// A_lo == nullptr -> plain bf16 A.  N % 64 == 0, K % 64 == 0.
-static int tc_gemm_launch(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W, int M, int N, int K,
+int tc_gemm_launch(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W, int M, int N, int K,
                           const Epi& ep, cudaStream_t st) {
     if (N % 64 || K % 64) { snprintf(c->err, sizeof c->err, "tc_gemm: N=%d, K=%d must be multiples of 64", N, K); return -1; }
     const int w_rows = ep.group_offsets ? ep.n_groups * N : N;
