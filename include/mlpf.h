@@ -146,13 +146,13 @@ int64_t mlpf_query(const mlpf_handle* h, int key);   /* < 0 on error */
 int64_t mlpf_debug_get_schedule(mlpf_handle* h, void* stream, int which, int32_t* host_out, int64_t capacity);
 
 /* intermediates of the last mlpf_infer on `stream`, converted to fp32, row-major:
- * H [N,d] residual stream; U [N,d] last LayerNorm output; QK [N,2d] (q | k); VT [d,N] (v transposed);
+ * H [N,d] residual stream; U [N,d] last LayerNorm output; QK [N,2d] (q | k); V [N,d];
  * O [N,d] attention output; G [N,gw] last wide hidden (FFN: gw = d_ff; heads: gw = (1+n_reg_heads) d).
  * Which stage they hold depends on MLPF_OPT_TAP_LAYER.  Returns floats written or a negative error. */
 #define MLPF_TENSOR_H   0
 #define MLPF_TENSOR_U   1
 #define MLPF_TENSOR_QK  2
-#define MLPF_TENSOR_VT  3
+#define MLPF_TENSOR_V   3
 #define MLPF_TENSOR_O   4
 #define MLPF_TENSOR_G   5
 int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which, float* host_out, int64_t capacity);
@@ -179,9 +179,9 @@ int mlpf_debug_get_profile(mlpf_handle* h, void* stream, float* ms_out, int32_t*
 int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* A_lo, const uint16_t* W, float* C, int32_t M, int32_t N,
                       int32_t K, void* stream);
 /* O[N,d] (bf16) = per-event multi-head softmax(Q K^T / sqrt(hd)) V (Eq. 4) via the tcgen05 flash kernel.
- * QK [N,2d] bf16 (q | k), VT [d, ldvt] bf16, key_valid [N] int32 0/1 (NULL = all valid),
- * event_offsets HOST int32 [n_events+1]. */
-int mlpf_tc_attention_bf16(const uint16_t* QK, const uint16_t* VT, int64_t ldvt, const int32_t* key_valid,
+ * QKV [N,3d] bf16 row-major (q | k | v), key_valid [N] int32 0/1 (NULL = all valid),
+ * event_offsets HOST int32 [n_events+1]; events may start at any row. */
+int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_valid,
                            const int32_t* event_offsets, int32_t n_events, int32_t d_model, int32_t n_heads,
                            uint16_t* O, void* stream);
 

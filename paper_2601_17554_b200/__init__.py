@@ -22,7 +22,7 @@ KERNELS_TC, KERNELS_SIMPLE = 0, 1
 Q_N_LAYERS, Q_D_MODEL, Q_N_HEADS, Q_D_FF, Q_N_FEAT, Q_N_CLASSES, Q_N_REGRESS = 1, 2, 3, 4, 5, 6, 7
 Q_WEIGHT_BYTES, Q_WORKSPACE_BYTES, Q_N_PARAMS, Q_LAUNCHES = 8, 9, 10, 11
 SCHED = dict(row_event=0, row_pos=1, valid=2, n_valid=3, type_offsets=4, sorted_row=5, type_perm=6, work_list=7)
-TENSOR = dict(H=0, U=1, QK=2, VT=3, O=4, G=5)
+TENSOR = dict(H=0, U=1, QK=2, V=3, O=4, G=5)
 KERNEL_CLASSES = ["sched", "embed_l1", "embed_l2", "layernorm", "qkv", "attention", "outproj", "ffn1", "ffn2",
                   "heads_l1", "heads_l2"]
 
@@ -66,7 +66,7 @@ def lib():
     L.mlpf_tc_gemm_bf16.restype = C.c_int
     L.mlpf_tc_gemm_bf16.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp]
     L.mlpf_tc_attention_bf16.restype = C.c_int
-    L.mlpf_tc_attention_bf16.argtypes = [vp, vp, i64, vp, vp, i32, i32, i32, vp, vp]
+    L.mlpf_tc_attention_bf16.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     _lib = L
     return L
 
@@ -181,14 +181,15 @@ def tc_gemm_bf16(A, W, A_lo=None, stream=None):
     return out
 
 
-def tc_attention_bf16(QK, VT, key_valid, event_offsets, d_model, n_heads, stream=None):
-    """QK [N,2d] bf16, VT [d,ldvt] bf16, key_valid [N] int32 or None -> O [N,d] bf16 (Eq. 4 per event/head)."""
+def tc_attention_bf16(QKV, key_valid, event_offsets, d_model, n_heads, stream=None):
+    """QKV [N,3d] bf16 (q | k | v), key_valid [N] int32 or None -> O [N,d] bf16 (Eq. 4 per event/head)."""
     import torch
     off = np.ascontiguousarray(event_offsets, dtype=np.int32)
-    N = QK.shape[0]
-    out = torch.zeros((N, d_model), dtype=torch.bfloat16, device=QK.device)
+    assert QKV.is_contiguous() and QKV.shape[1] == 3 * d_model
+    N = QKV.shape[0]
+    out = torch.zeros((N, d_model), dtype=torch.bfloat16, device=QKV.device)
     kv = C.c_void_p(key_valid.data_ptr()) if key_valid is not None else C.c_void_p(0)
-    _check(lib().mlpf_tc_attention_bf16(C.c_void_p(QK.data_ptr()), C.c_void_p(VT.data_ptr()), VT.stride(0), kv,
+    _check(lib().mlpf_tc_attention_bf16(C.c_void_p(QKV.data_ptr()), kv,
                                         off.ctypes.data_as(C.c_void_p), len(off) - 1, d_model, n_heads,
                                         C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
     return out

@@ -27,7 +27,7 @@ template <> __device__ __forceinline__ bf16 from_f32<bf16>(float v) { return __f
 
 // Epilogue description shared by the CUDA-core GEMM and the tcgen05 GEMM:
 //   v = acc + bias[n]; v = act(v); v += residual[m, n];
-//   out_f32[row, n] = v;  out_act[row, n] = T(v) (+ out_act_lo = T(v - T(v))) for n < vt_col0;  out_vt[n - vt_col0, row] = T(v) otherwise
+//   out_f32[row, n] = v;  out_act[row, n] = T(v) (+ out_act_lo[row, n] = T(v - T(v)))
 // row = row_perm ? row_perm[m] : m (row < 0: nothing is written).  Grouped mode (group_offsets != null):
 // the M-tile starting at m0 uses weight/bias block g-1 where group_offsets[g] <= m0 < group_offsets[g+1]
 // (g = 1..n_groups, segments are multiples of 128 rows); tiles at or beyond group_offsets[n_groups+1] exit.
@@ -38,8 +38,6 @@ struct Epi {
     float* out_f32 = nullptr;        int64_t ld_f32 = 0;
     void* out_act = nullptr;         int64_t ld_act = 0;
     void* out_act_lo = nullptr;      // optional second bf16 term: out_act_lo = T(v - out_act), same ld
-    void* out_vt = nullptr;          int64_t ld_vt = 0;
-    int vt_col0 = 0x7fffffff;
     const int* row_perm = nullptr;
     const int* group_offsets = nullptr;
     int n_groups = 0;

@@ -48,9 +48,8 @@ struct Workspace {
     int64_t cap_events = 0, cap_tiles = 0;
     int64_t bytes = 0;
     bool fp32 = false;                // element type of the activation buffers
-    int64_t ldvt = 0;
     float* h = nullptr;               // [cap, d] fp32 residual stream
-    void *u = nullptr, *qk = nullptr, *vt = nullptr, *o = nullptr, *g = nullptr;
+    void *u = nullptr, *qkv = nullptr, *o = nullptr, *g = nullptr;   // qkv: [cap, 3d] (q | k | v)
     void *u_lo = nullptr, *o_lo = nullptr, *g_lo = nullptr;   // second bf16 term of split activations
     int64_t g_elems = 0;
     // schedule (a0)
@@ -201,7 +200,7 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
 }
 
 static void ws_free(Workspace* w) {
-    void* ptrs[] = {w->h, w->u, w->qk, w->vt, w->o, w->g, w->u_lo, w->o_lo, w->g_lo, w->offsets, w->work, w->pairs, w->valid, w->row_event,
+    void* ptrs[] = {w->h, w->u, w->qkv, w->o, w->g, w->u_lo, w->o_lo, w->g_lo, w->offsets, w->work, w->pairs, w->valid, w->row_event,
                     w->row_pos, w->n_valid, w->block_counts, w->block_base, w->type_offsets, w->sorted_row, w->type_perm};
     for (void* p : ptrs) if (p) cudaFree(p);
 }
@@ -273,10 +272,8 @@ template <typename P> static cudaError_t dmalloc(P** p, int64_t bytes, Workspace
 static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t n_tiles, bool fp32) {
     const int64_t d = h->d;
     if (N > w->cap_rows || fp32 != w->fp32) {
-        void* ptrs[] = {w->h, w->u, w->qk, w->vt, w->o, w->g, w->u_lo, w->o_lo, w->g_lo, w->valid, w->row_event, w->row_pos, w->block_counts,
+        void* ptrs[] = {w->h, w->u, w->qkv, w->o, w->g, w->u_lo, w->o_lo, w->g_lo, w->valid, w->row_event, w->row_pos, w->block_counts,
                         w->block_base, w->sorted_row, w->type_perm, w->type_offsets};
-        int64_t small = w->bytes;     // recompute below
-        (void)small;
         for (void* p : ptrs) if (p) cudaFree(p);   // cudaFree waits for work in flight
         // keep the event-indexed arrays' accounting: recompute bytes from scratch
         int64_t ev_bytes = 0;
@@ -288,11 +285,10 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
         const int64_t m_ub = cap + 4 * 128;
         const int64_t gw = std::max<int64_t>(h->dff, (int64_t)h->n_hblk * d);
         w->g_elems = std::max<int64_t>(cap * gw, m_ub * d);
-        w->ldvt = cap;
         w->fp32 = fp32;
         const int64_t nb = (cap + SCHED_BLOCK - 1) / SCHED_BLOCK;
         if (dmalloc(&w->h, cap * d * 4, w) || dmalloc((char**)&w->u, cap * d * es, w) ||
-            dmalloc((char**)&w->qk, cap * 2 * d * es, w) || dmalloc((char**)&w->vt, d * w->ldvt * es, w) ||
+            dmalloc((char**)&w->qkv, cap * 3 * d * es, w) ||
             dmalloc((char**)&w->o, cap * d * es, w) || dmalloc((char**)&w->g, w->g_elems * es, w) ||
             dmalloc((char**)&w->u_lo, cap * d * es, w) || dmalloc((char**)&w->o_lo, cap * d * es, w) ||
             dmalloc((char**)&w->g_lo, w->g_elems * es, w) ||
@@ -306,8 +302,8 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
         }
         // the activation buffers feed TMA loads whose boxes may overrun valid rows: start from zeros so
         // that never-written tails hold finite values
-        cudaMemset(w->u, 0, cap * d * es); cudaMemset(w->qk, 0, cap * 2 * d * es);
-        cudaMemset(w->vt, 0, d * w->ldvt * es); cudaMemset(w->o, 0, cap * d * es);
+        cudaMemset(w->u, 0, cap * d * es); cudaMemset(w->qkv, 0, cap * 3 * d * es);
+        cudaMemset(w->o, 0, cap * d * es);
         cudaMemset(w->g, 0, w->g_elems * es);
         cudaMemset(w->u_lo, 0, cap * d * es); cudaMemset(w->o_lo, 0, cap * d * es); cudaMemset(w->g_lo, 0, w->g_elems * es);
         w->cap_rows = cap;
@@ -378,12 +374,12 @@ static int run_layernorm(mlpf_handle* h, bool fp32, const float* x, int N, const
 static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspace* w, cudaStream_t st) {
     if (w->n_tiles == 0) return MLPF_OK;
     if (tc && !fp32) {
-        int rc = tc_attn_launch(&h->tc, (const bf16*)w->qk, (const bf16*)w->vt, w->ldvt, w->N, w->valid, w->offsets,
+        int rc = tc_attn_launch(&h->tc, (const bf16*)w->qkv, w->N, w->valid, w->offsets,
                                 (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, (bf16*)w->o,
                                 split ? (bf16*)w->o_lo : nullptr, st);
         if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", h->tc.err);
     } else {
-        launch_attn_simple(fp32, h->hd, w->qk, w->vt, w->ldvt, w->valid, w->offsets, (const int2*)w->work, (int)w->n_tiles,
+        launch_attn_simple(fp32, h->hd, w->qkv, w->valid, w->offsets, (const int2*)w->work, (int)w->n_tiles,
                            h->H, w->tile_q, h->d, w->o, split ? w->o_lo : nullptr, st);
     }
     LAUNCH_CHECK(h);
@@ -454,11 +450,10 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
             rc = run_layernorm(h, fp32, w->h, N, PV + lw.ln1g, PV + lw.ln1b, u, nullptr, st);                     // a2
         }
         if (rc) return rc;
-        {   // a3: [Q K V] = LN1(x) Wqkv^T + bqkv ; V stored transposed per head dim
+        {   // a3: [Q K V] = LN1(x) Wqkv^T + bqkv
             ProfScope ps(h, w, st, MLPF_KC_QKV);
             Epi ep;
-            ep.bias = PV + lw.bqkv; ep.out_act = w->qk; ep.ld_act = 2 * d;
-            ep.out_vt = w->vt; ep.ld_vt = w->ldvt; ep.vt_col0 = 2 * d;
+            ep.bias = PV + lw.bqkv; ep.out_act = w->qkv; ep.ld_act = 3 * d;
             rc = run_gemm(h, fp32, tc, u, nullptr, PW(lw.Wqkv), N, 3 * d, d, ep, st);
             if (rc) return rc;
         }
@@ -619,7 +614,7 @@ extern "C" int64_t mlpf_debug_get_schedule(mlpf_handle* h, void* stream, int whi
 static int tap_copy(bool fp32, const void* src, int64_t rows, int64_t cols, int64_t ld, float* host_out) {
     float* tmp = nullptr;
     CUDA_TRY(cudaMalloc(&tmp, (size_t)rows * ld * 4));
-    launch_to_f32(fp32, src, tmp, rows * ld, 0);
+    launch_to_f32(fp32, src, tmp, (rows - 1) * ld + cols, 0);     // src may be a column block of a wider buffer
     cudaError_t e = cudaMemcpy2D(host_out, (size_t)cols * 4, tmp, (size_t)ld * 4, (size_t)cols * 4, (size_t)rows, cudaMemcpyDeviceToHost);
     cudaFree(tmp);
     if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tap copy failed: %s", cudaGetErrorString(e));
@@ -642,8 +637,8 @@ extern "C" int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which
             return N * d;
         }
         case MLPF_TENSOR_U: src = w->u; break;
-        case MLPF_TENSOR_QK: src = w->qk; cols = ld = 2 * d; break;
-        case MLPF_TENSOR_VT: src = w->vt; rows = d; cols = N; ld = w->ldvt; break;
+        case MLPF_TENSOR_QK: src = w->qkv; cols = 2 * d; ld = 3 * d; break;
+        case MLPF_TENSOR_V: src = (const char*)w->qkv + 2 * d * (w->fp32 ? 4 : 2); cols = d; ld = 3 * d; break;
         case MLPF_TENSOR_O: src = w->o; break;
         case MLPF_TENSOR_G: src = w->g; cols = ld = w->g_width; if (cols == 0) return set_err(MLPF_E_ARG, "G not produced yet"); break;
         default: return set_err(MLPF_E_ARG, "unknown tensor %d", which);
@@ -689,10 +684,10 @@ extern "C" int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* A_lo, const 
     return MLPF_OK;
 }
 
-extern "C" int mlpf_tc_attention_bf16(const uint16_t* QK, const uint16_t* VT, int64_t ldvt, const int32_t* key_valid,
+extern "C" int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_valid,
                                       const int32_t* event_offsets, int32_t n_events, int32_t d_model, int32_t n_heads,
                                       uint16_t* O, void* stream) {
-    if (!QK || !VT || !event_offsets || !O) return set_err(MLPF_E_NULL, "NULL argument");
+    if (!QKV || !event_offsets || !O) return set_err(MLPF_E_NULL, "NULL argument");
     if (n_events <= 0) return MLPF_OK;
     const int hd = n_heads > 0 ? d_model / n_heads : 0;
     if (hd != 16 && hd != 32 && hd != 64) return set_err(MLPF_E_ARG, "head_dim must be 16, 32 or 64");
@@ -711,7 +706,7 @@ extern "C" int mlpf_tc_attention_bf16(const uint16_t* QK, const uint16_t* VT, in
     CUDA_TRY(cudaMalloc(&d_pairs, pairs.size() * 4));
     CUDA_TRY(cudaMemcpyAsync(d_off, event_offsets, (size_t)(n_events + 1) * 4, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(d_pairs, pairs.data(), pairs.size() * 4, cudaMemcpyHostToDevice, st));
-    int rc = tc_attn_launch(&ctx, (const bf16*)QK, (const bf16*)VT, ldvt, N, key_valid, d_off, (const int2*)d_pairs,
+    int rc = tc_attn_launch(&ctx, (const bf16*)QKV, N, key_valid, d_off, (const int2*)d_pairs,
                             (int)(pairs.size() / 2), d_model, n_heads, (bf16*)O, (bf16*)nullptr, st);
     cudaError_t e = cudaStreamSynchronize(st);
     cudaFree(d_off); cudaFree(d_pairs);

@@ -153,6 +153,15 @@ __device__ __forceinline__ uint64_t umma_desc_kmajor(uint32_t smem_addr, uint32_
     const uint64_t sbo = (8u * swizzle_bytes) >> 4;
     return (uint64_t)((smem_addr >> 4) & 0x3FFF) | (1ull << 16) | (sbo << 32) | (1ull << 46) | (layout << 61);
 }
+// MN-major operand tile (the contraction index runs over ROWS of the shared-memory tile, the M/N index
+// is contiguous): rows of `swizzle_bytes` = one swizzle atom along M/N, 8-row (8 x K) groups
+// `8 * swizzle_bytes` apart (SBO); LBO (stride between atoms along M/N) is unused for a single atom.
+__device__ __forceinline__ uint64_t umma_desc_mnmajor(uint32_t smem_addr, uint32_t swizzle_bytes) {
+    const uint64_t layout = swizzle_bytes == 128 ? 2ull : (swizzle_bytes == 64 ? 4ull : 6ull);
+    const uint64_t sbo = (8u * swizzle_bytes) >> 4;
+    return (uint64_t)((smem_addr >> 4) & 0x3FFF) | (sbo << 16) | (sbo << 32) | (1ull << 46) | (layout << 61);
+}
+constexpr uint32_t UMMA_A_MN_MAJOR = 1u << 15, UMMA_B_MN_MAJOR = 1u << 16;   // instruction-descriptor bits
 // instruction descriptor, kind::f16, A and B bf16 K-major, D fp32, M x N tile
 __device__ __host__ constexpr uint32_t umma_idesc_bf16(int M, int N) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);

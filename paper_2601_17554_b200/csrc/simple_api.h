@@ -23,7 +23,7 @@ int launch_layernorm(bool fp32, int d, const float* x, int N, const float* g, co
                      void* u_lo, cudaStream_t st);
 void launch_gemm_simple(bool fp32, const void* A, const void* A_lo, const void* W, int M, int N, int K, const Epi& ep,
                         cudaStream_t st);
-void launch_attn_simple(bool fp32, int hd, const void* QK, const void* VT, int64_t ldvt, const int* key_valid,
+void launch_attn_simple(bool fp32, int hd, const void* QKV, const int* key_valid,
                         const int* offsets, const int2* work, int n_tiles, int H, int tile_q, int d, void* O,
                         void* O_lo, cudaStream_t st);
 void launch_heads_l2(bool fp32, const void* hidden, const void* hidden_lo, int N, int d, int ld_hidden,

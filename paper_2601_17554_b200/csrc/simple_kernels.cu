@@ -252,14 +252,10 @@ k_gemm_simple(const T* __restrict__ A, const T* __restrict__ A_lo, const T* __re
             v = apply_act(v, ep.act);
             if (ep.residual) v += ep.residual[(int64_t)row * ep.ld_res + n];
             if (ep.out_f32) ep.out_f32[(int64_t)row * ep.ld_f32 + n] = v;
-            if (n < ep.vt_col0) {
-                if (ep.out_act) {
-                    const T hi = from_f32<T>(v);
-                    ((T*)ep.out_act)[(int64_t)row * ep.ld_act + n] = hi;
-                    if (ep.out_act_lo) ((T*)ep.out_act_lo)[(int64_t)row * ep.ld_act + n] = from_f32<T>(v - to_f32<T>(hi));
-                }
-            } else {
-                ((T*)ep.out_vt)[(int64_t)(n - ep.vt_col0) * ep.ld_vt + row] = from_f32<T>(v);
+            if (ep.out_act) {
+                const T hi = from_f32<T>(v);
+                ((T*)ep.out_act)[(int64_t)row * ep.ld_act + n] = hi;
+                if (ep.out_act_lo) ((T*)ep.out_act_lo)[(int64_t)row * ep.ld_act + n] = from_f32<T>(v - to_f32<T>(hi));
             }
         }
     }
@@ -273,8 +269,7 @@ k_gemm_simple(const T* __restrict__ A, const T* __restrict__ A_lo, const T* __re
 // ------------------------------------------------------------------------------------------------
 template <typename T, int HD>
 __global__ void __launch_bounds__(128)
-k_attn_simple(const T* __restrict__ QK, const T* __restrict__ VT, int64_t ldvt,
-              const int* __restrict__ key_valid, const int* __restrict__ offsets,
+k_attn_simple(const T* __restrict__ QKV, const int* __restrict__ key_valid, const int* __restrict__ offsets,
               const int2* __restrict__ work, int tile_q, int d, T* __restrict__ O, T* __restrict__ O_lo) {
     __shared__ float Ks[32][HD + 1];
     __shared__ float Vs[32][HD + 1];
@@ -288,7 +283,7 @@ k_attn_simple(const T* __restrict__ QK, const T* __restrict__ VT, int64_t ldvt,
     float q[HD], acc[HD];
 #pragma unroll
     for (int c = 0; c < HD; ++c) {
-        q[c] = active ? to_f32<T>(QK[(int64_t)qrow * (2 * d) + head * HD + c]) * scale : 0.0f;
+        q[c] = active ? to_f32<T>(QKV[(int64_t)qrow * (3 * d) + head * HD + c]) * scale : 0.0f;
         acc[c] = 0.0f;
     }
     float m = -INFINITY, l = 0.0f;
@@ -297,12 +292,12 @@ k_attn_simple(const T* __restrict__ QK, const T* __restrict__ VT, int64_t ldvt,
         for (int idx = threadIdx.x; idx < 32 * HD; idx += blockDim.x) {
             int j = idx / HD, c = idx % HD;          // K rows: contiguous over c
             int key = k0 + j;
-            Ks[j][c] = (key < ev1) ? to_f32<T>(QK[(int64_t)key * (2 * d) + d + head * HD + c]) : 0.0f;
+            Ks[j][c] = (key < ev1) ? to_f32<T>(QKV[(int64_t)key * (3 * d) + d + head * HD + c]) : 0.0f;
         }
         for (int idx = threadIdx.x; idx < 32 * HD; idx += blockDim.x) {
-            int c = idx / 32, j = idx % 32;          // V^T rows: contiguous over keys
+            int j = idx / HD, c = idx % HD;
             int key = k0 + j;
-            Vs[j][c] = (key < ev1) ? to_f32<T>(VT[(int64_t)(head * HD + c) * ldvt + key]) : 0.0f;
+            Vs[j][c] = (key < ev1) ? to_f32<T>(QKV[(int64_t)key * (3 * d) + 2 * d + head * HD + c]) : 0.0f;
         }
         if (threadIdx.x < 32) {
             int key = k0 + threadIdx.x;
@@ -437,20 +432,20 @@ void launch_gemm_simple(bool fp32, const void* A, const void* A_lo, const void* 
 }
 
 template <typename T>
-static void attn_simple_hd(int hd, const T* QK, const T* VT, int64_t ldvt, const int* key_valid, const int* offsets,
+static void attn_simple_hd(int hd, const T* QKV, const int* key_valid, const int* offsets,
                            const int2* work, int n_tiles, int H, int tile_q, int d, T* O, T* O_lo, cudaStream_t st) {
     dim3 grid((unsigned)n_tiles, H);
     switch (hd) {
-        case 16: k_attn_simple<T, 16><<<grid, tile_q, 0, st>>>(QK, VT, ldvt, key_valid, offsets, work, tile_q, d, O, O_lo); break;
-        case 32: k_attn_simple<T, 32><<<grid, tile_q, 0, st>>>(QK, VT, ldvt, key_valid, offsets, work, tile_q, d, O, O_lo); break;
-        case 64: k_attn_simple<T, 64><<<grid, tile_q, 0, st>>>(QK, VT, ldvt, key_valid, offsets, work, tile_q, d, O, O_lo); break;
+        case 16: k_attn_simple<T, 16><<<grid, tile_q, 0, st>>>(QKV, key_valid, offsets, work, tile_q, d, O, O_lo); break;
+        case 32: k_attn_simple<T, 32><<<grid, tile_q, 0, st>>>(QKV, key_valid, offsets, work, tile_q, d, O, O_lo); break;
+        case 64: k_attn_simple<T, 64><<<grid, tile_q, 0, st>>>(QKV, key_valid, offsets, work, tile_q, d, O, O_lo); break;
     }
 }
-void launch_attn_simple(bool fp32, int hd, const void* QK, const void* VT, int64_t ldvt, const int* key_valid,
+void launch_attn_simple(bool fp32, int hd, const void* QKV, const int* key_valid,
                         const int* offsets, const int2* work, int n_tiles, int H, int tile_q, int d, void* O,
                         void* O_lo, cudaStream_t st) {
-    if (fp32) attn_simple_hd<float>(hd, (const float*)QK, (const float*)VT, ldvt, key_valid, offsets, work, n_tiles, H, tile_q, d, (float*)O, (float*)O_lo, st);
-    else attn_simple_hd<bf16>(hd, (const bf16*)QK, (const bf16*)VT, ldvt, key_valid, offsets, work, n_tiles, H, tile_q, d, (bf16*)O, (bf16*)O_lo, st);
+    if (fp32) attn_simple_hd<float>(hd, (const float*)QKV, key_valid, offsets, work, n_tiles, H, tile_q, d, (float*)O, (float*)O_lo, st);
+    else attn_simple_hd<bf16>(hd, (const bf16*)QKV, key_valid, offsets, work, n_tiles, H, tile_q, d, (bf16*)O, (bf16*)O_lo, st);
 }
 
 void launch_heads_l2(bool fp32, const void* hidden, const void* hidden_lo, int N, int d, int ld_hidden,

@@ -5,9 +5,12 @@
 // exactly 0 (reading A2); a query with no valid key gets O = 0 (A15).
 //
 // One CTA = one head x two consecutive 128-row query tiles (a, b) of one event, sharing every K / V^T tile.
-//   warp 0      TMA producer: Q_a, Q_b once; then (K_j [128 keys x hd], V^T_j [hd x 128 keys]) into a ring.
+//   warp 0      TMA producer: Q_a, Q_b once; then (K_j, V_j), each [128 keys x hd] row-major, into a ring.
+//               Q, K, V are column blocks of one row-major [N, 3d] buffer, so an event may start at any row
+//               (TMA needs 16-byte alignment only along the innermost, head-dim, coordinate).
 //   warp 1      MMA issuer:   S_t = Q_t K_j^T  (M=128, N=128, K=hd)  -> TMEM (fp32);
-//                             O_t(j) = P_t V_j (A = P_t read from TMEM, K=128, N=hd) -> TMEM, fresh each tile.
+//                             O_t(j) = P_t V_j (A = P_t read from TMEM, B = V_j as an MN-major operand,
+//                             K=128, N=hd) -> TMEM, fresh each tile.
 //   warps 2-5   softmax warpgroup of tile a, warps 6-9 of tile b: one query row per thread:
 //               S -> (mask) -> running max -> exp2 -> bf16 P written back over S's columns in TMEM;
 //               then acc = acc * corr + O_t(j-1) in registers (no read-modify-write of O in TMEM).
@@ -44,7 +47,7 @@ struct AttnParams {
 
 template <int HD>
 __global__ void __launch_bounds__(ATT_THREADS, 1)
-k_tc_attn(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__ CUtensorMap tmVT, AttnParams prm) {
+k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     using Cfg = AttnCfg<HD>;
     constexpr int ST = Cfg::STAGES;
     extern __shared__ uint8_t smem_raw[];
@@ -78,8 +81,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__ CUte
             ptx::mbar_init(bar_o + 8 * t, 1);
         }
         ptx::fence_barrier_init();
-        ptx::tma_prefetch_desc(&tmQK);
-        ptx::tma_prefetch_desc(&tmVT);
+        ptx::tma_prefetch_desc(&tmQKV);
     }
     if (warp == 1) {
         ptx::tmem_alloc(ptx::smem_u32(&tmem_base_slot), 512);
@@ -94,8 +96,8 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__ CUte
         // ------------------------------------------------------------ TMA producer
         if (lane == 0) {
             ptx::mbar_expect_tx(bar_q, Cfg::Q_BYTES * (has_b ? 2 : 1));
-            ptx::tma_load_2d(sQ, &tmQK, bar_q, head * HD, q0a);
-            if (has_b) ptx::tma_load_2d(sQ + Cfg::Q_BYTES, &tmQK, bar_q, head * HD, q0b);
+            ptx::tma_load_2d(sQ, &tmQKV, bar_q, head * HD, q0a);
+            if (has_b) ptx::tma_load_2d(sQ + Cfg::Q_BYTES, &tmQKV, bar_q, head * HD, q0b);
         }
         for (int j = 0; j < nkv; ++j) {
             const int s = j % ST;
@@ -104,16 +106,15 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__ CUte
                 const uint32_t st = sKV + s * Cfg::STAGE_BYTES;
                 const int k0 = ev0 + j * ATT_BK;
                 ptx::mbar_expect_tx(bar_kv_full + 8 * s, Cfg::STAGE_BYTES);
-                ptx::tma_load_2d(st, &tmQK, bar_kv_full + 8 * s, prm.d + head * HD, k0);
-                ptx::tma_load_2d(st + Cfg::K_BYTES, &tmVT, bar_kv_full + 8 * s, k0, head * HD);
-                ptx::tma_load_2d(st + Cfg::K_BYTES + HD * 128, &tmVT, bar_kv_full + 8 * s, k0 + 64, head * HD);
+                ptx::tma_load_2d(st, &tmQKV, bar_kv_full + 8 * s, prm.d + head * HD, k0);
+                ptx::tma_load_2d(st + Cfg::K_BYTES, &tmQKV, bar_kv_full + 8 * s, 2 * prm.d + head * HD, k0);
             }
             __syncwarp();
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------ MMA issuer
         constexpr uint32_t idesc_s = ptx::umma_idesc_bf16(128, ATT_BK);
-        constexpr uint32_t idesc_o = ptx::umma_idesc_bf16(128, HD);
+        constexpr uint32_t idesc_o = ptx::umma_idesc_bf16(128, HD) | ptx::UMMA_B_MN_MAJOR;
         auto issue_s = [&](int t, int j) {          // S_t = Q_t K_j^T
             const uint32_t kb = sKV + (j % ST) * Cfg::STAGE_BYTES;
             const uint32_t qb = sQ + t * Cfg::Q_BYTES;
@@ -129,7 +130,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__ CUte
 #pragma unroll
             for (int k = 0; k < ATT_BK / 16; ++k)
                 ptx::mma_ts(tmem_base + o_col, tmem_base + t * 128 + k * 8,
-                            ptx::umma_desc_kmajor(vb + (k >> 2) * (HD * 128) + (k & 3) * 32, 128), idesc_o, k != 0);
+                            ptx::umma_desc_mnmajor(vb + k * 16 * Cfg::SW, Cfg::SW), idesc_o, k != 0);
             ptx::mma_commit(bar_o + 8 * t);
         };
         ptx::mbar_wait(bar_q, 0);
@@ -298,12 +299,11 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__ CUte
 }
 
 template <int HD>
-static int tc_attn_launch_hd(TcContext* c, const bf16* QK, const bf16* VT, int64_t ldvt, int64_t N, const AttnParams& prm,
+static int tc_attn_launch_hd(TcContext* c, const bf16* QKV, int64_t N, const AttnParams& prm,
                              cudaStream_t st) {
     using Cfg = AttnCfg<HD>;
-    CUtensorMap tmQK, tmVT;
-    if (tc_tensor_map(c, &tmQK, QK, 2 * prm.d, N, 2 * prm.d, HD, ATT_BQ)) return -1;
-    if (tc_tensor_map(c, &tmVT, VT, N, prm.d, ldvt, 64, HD)) return -1;
+    CUtensorMap tmQKV;
+    if (tc_tensor_map(c, &tmQKV, QKV, 3 * prm.d, N, 3 * prm.d, HD, ATT_BQ)) return -1;
     auto kern = k_tc_attn<HD>;
     static bool attr_set = false;
     if (!attr_set) {
@@ -311,11 +311,11 @@ static int tc_attn_launch_hd(TcContext* c, const bf16* QK, const bf16* VT, int64
         if (e != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return -1; }
         attr_set = true;
     }
-    kern<<<prm.n_pairs * prm.H, ATT_THREADS, Cfg::SMEM_BYTES, st>>>(tmQK, tmVT, prm);
+    kern<<<prm.n_pairs * prm.H, ATT_THREADS, Cfg::SMEM_BYTES, st>>>(tmQKV, prm);
     return 0;
 }
 
-int tc_attn_launch(TcContext* c, const bf16* QK, const bf16* VT, int64_t ldvt, int64_t N, const int* key_valid,
+int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const int* key_valid,
                           const int* offsets, const int2* pairs, int n_pairs, int d, int H, bf16* O, bf16* O_lo,
                           cudaStream_t st) {
     const int hd = d / H;
@@ -323,11 +323,10 @@ int tc_attn_launch(TcContext* c, const bf16* QK, const bf16* VT, int64_t ldvt, i
     prm.key_valid = key_valid; prm.offsets = offsets; prm.pairs = pairs; prm.n_pairs = n_pairs; prm.H = H; prm.d = d;
     prm.O = O; prm.O_lo = O_lo;
     prm.scale_log2 = 1.4426950408889634f / sqrtf((float)hd);
-    if (ldvt % 8) { snprintf(c->err, sizeof c->err, "tc_attn: ldvt must be a multiple of 8"); return -1; }
     switch (hd) {
-        case 16: return tc_attn_launch_hd<16>(c, QK, VT, ldvt, N, prm, st);
-        case 32: return tc_attn_launch_hd<32>(c, QK, VT, ldvt, N, prm, st);
-        case 64: return tc_attn_launch_hd<64>(c, QK, VT, ldvt, N, prm, st);
+        case 16: return tc_attn_launch_hd<16>(c, QKV, N, prm, st);
+        case 32: return tc_attn_launch_hd<32>(c, QKV, N, prm, st);
+        case 64: return tc_attn_launch_hd<64>(c, QKV, N, prm, st);
     }
     snprintf(c->err, sizeof c->err, "tc_attn: head_dim %d unsupported", hd);
     return -1;

@@ -95,31 +95,25 @@ __device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[32], c
 #pragma unroll
         for (int j = 0; j < 8; ++j) op[j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
     }
-    if (n_base < ep.vt_col0) {
-        if (ep.out_act) {
-            uint32_t hi[16], lo[16];
+    if (ep.out_act) {
+        uint32_t hi[16], lo[16];
 #pragma unroll
-            for (int j = 0; j < 16; ++j) {
-                __nv_bfloat162 h2 = __floats2bfloat162_rn(v[2 * j], v[2 * j + 1]);
-                hi[j] = *reinterpret_cast<uint32_t*>(&h2);
-                if (ep.out_act_lo) {
-                    __nv_bfloat162 l2 = __floats2bfloat162_rn(v[2 * j] - __low2float(h2), v[2 * j + 1] - __high2float(h2));
-                    lo[j] = *reinterpret_cast<uint32_t*>(&l2);
-                }
-            }
-            uint4* op = reinterpret_cast<uint4*>((bf16*)ep.out_act + (int64_t)row * ep.ld_act + n_base);
-#pragma unroll
-            for (int j = 0; j < 4; ++j) op[j] = make_uint4(hi[4 * j], hi[4 * j + 1], hi[4 * j + 2], hi[4 * j + 3]);
+        for (int j = 0; j < 16; ++j) {
+            __nv_bfloat162 h2 = __floats2bfloat162_rn(v[2 * j], v[2 * j + 1]);
+            hi[j] = *reinterpret_cast<uint32_t*>(&h2);
             if (ep.out_act_lo) {
-                uint4* lp = reinterpret_cast<uint4*>((bf16*)ep.out_act_lo + (int64_t)row * ep.ld_act + n_base);
-#pragma unroll
-                for (int j = 0; j < 4; ++j) lp[j] = make_uint4(lo[4 * j], lo[4 * j + 1], lo[4 * j + 2], lo[4 * j + 3]);
+                __nv_bfloat162 l2 = __floats2bfloat162_rn(v[2 * j] - __low2float(h2), v[2 * j + 1] - __high2float(h2));
+                lo[j] = *reinterpret_cast<uint32_t*>(&l2);
             }
         }
-    } else {
-        bf16* vt = (bf16*)ep.out_vt + (int64_t)(n_base - ep.vt_col0) * ep.ld_vt + row;
+        uint4* op = reinterpret_cast<uint4*>((bf16*)ep.out_act + (int64_t)row * ep.ld_act + n_base);
 #pragma unroll
-        for (int j = 0; j < 32; ++j) vt[(int64_t)j * ep.ld_vt] = __float2bfloat16_rn(v[j]);   // lanes = consecutive rows
+        for (int j = 0; j < 4; ++j) op[j] = make_uint4(hi[4 * j], hi[4 * j + 1], hi[4 * j + 2], hi[4 * j + 3]);
+        if (ep.out_act_lo) {
+            uint4* lp = reinterpret_cast<uint4*>((bf16*)ep.out_act_lo + (int64_t)row * ep.ld_act + n_base);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) lp[j] = make_uint4(lo[4 * j], lo[4 * j + 1], lo[4 * j + 2], lo[4 * j + 3]);
+        }
     }
 }
 

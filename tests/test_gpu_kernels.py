@@ -56,21 +56,18 @@ def test_tc_attention_matches_dense_softmax(hd, H, lens, pad):
     qkv = rng.standard_normal((N, 3 * d)).astype(np.float32)
     qkv[:, :d] *= 2.0                                     # sharper than unit-variance scores
     valid = (rng.random(N) >= pad)
-    QK = _bf16(np.ascontiguousarray(qkv[:, :2 * d]))
-    ldvt = (N + 7) // 8 * 8
-    VT = torch.zeros((d, ldvt), dtype=torch.bfloat16, device="cuda")
-    VT[:, :N] = _bf16(qkv[:, 2 * d:]).T
+    QKV = _bf16(qkv)
     kv = torch.from_numpy(valid.astype(np.int32)).cuda()
-    O = P.tc_attention_bf16(QK, VT, kv if pad > 0 else None, off, d, H).float().cpu().numpy()
+    O = P.tc_attention_bf16(QKV, kv if pad > 0 else None, off, d, H).float().cpu().numpy()
     if pad == 0:
         valid[:] = True
-    qk64 = QK.float().cpu().numpy().astype(np.float64)
-    v64 = VT[:, :N].T.float().cpu().numpy().astype(np.float64)
+    qk64 = QKV.float().cpu().numpy().astype(np.float64)
+    v64 = qk64[:, 2 * d:]
     for e in range(len(lens)):
         a, b = off[e], off[e + 1]
         if b == a:
             continue
-        ref = oracle.attention_event(qk64[a:b, :d], qk64[a:b, d:], v64[a:b], valid[a:b], H)
+        ref = oracle.attention_event(qk64[a:b, :d], qk64[a:b, d:2 * d], v64[a:b], valid[a:b], H)
         err = np.abs(O[a:b] - ref)
         scale = np.sqrt((ref ** 2).mean()) + 1e-6
         assert (err / np.maximum(np.abs(ref), scale)).max() <= 2e-2, (e, err.max(), scale)

@@ -149,7 +149,7 @@ def test_per_step_intermediates(name, max_events, precision, tol):
         p = f"layer.{l}."
         qkv = dump[p + "qkv"]
         assert _rel(mod.tensor("QK", (N, 2 * d)), qkv[:, :2 * d], valid) <= tol, "qk"
-        assert _rel(mod.tensor("VT", (d, N)).T, qkv[:, 2 * d:], valid) <= tol, "v"
+        assert _rel(mod.tensor("V", (N, d)), qkv[:, 2 * d:], valid) <= tol, "v"
         assert _rel(mod.tensor("O", (N, d)), dump[p + "o"], valid) <= tol, "o"
         assert _rel(mod.tensor("U", (N, d)), dump[p + "u2"], valid) <= tol, "u2"
         assert _rel(mod.tensor("G", (N, m.d_ff)), dump[p + "g"], valid) <= tol, "g"
