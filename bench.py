@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""bench.py -- MLPF encoder forward (steps a0..a8) on synthetic CMS-like events.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl ours|reference]
+
+One "step" = one mlpf_infer call over one batch of the workload (default: BASELINE.json configs[2],
+the CMS-scale config the metric is quoted on: 8 events, ~5000 PF elements each, L=6, d=256, H=8).
+Prints ONE JSON line (rank 0).  `value` = events/s with inputs resident in HBM; `e2e` = the same through
+mlpf_infer_host (pinned host buffers, H2D + D2H inside the timed region); `roofline` = the attention
+kernel (a4, the dominant kernel) against the measured dense-bf16 peak; `cpu_baseline` = the fp64 numpy
+oracle timed on this box's host cores on a bounded sample.  N > 1: events are independent, so every rank
+runs its own batch (weak scaling, no data-path collective); time = max over ranks.
+"""
+from __future__ import annotations
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, HERE)
+
+import synth  # noqa: E402
+
+METRIC = "events_per_s"
+UNIT = "events/s"
+L2_FLUSH_BYTES = 256 << 20          # > 126 MB L2
+
+
+def load_peaks():
+    p = os.path.join(HERE, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return dict(hbm_gbs=d["hbm_gbs"], tflops_burst=d["bf16_tflops"],
+                    tflops_sustained=d.get("bf16_tflops_sustained", d["bf16_tflops"]), source="measured")
+    return dict(hbm_gbs=6650.0, tflops_burst=1590.0, tflops_sustained=1400.0, source="fallback")
+
+
+def workload(name, rank=0):
+    """Seeded synthetic batch; rank r > 0 draws its own batch of the same recipe."""
+    seed = None if rank == 0 else synth.BASE_SEED + 100 * rank + synth.configs.CFG_INDEX[name]
+    X, off = synth.make_named_events(name, seed=seed)
+    return X, off
+
+
+def flop_model(m, off):
+    """Algorithmic FLOPs of one forward pass (linear 2*M*N*K, attention 4*d*sum n_e^2 per layer)."""
+    n = np.diff(off).astype(np.float64)
+    N, s2 = n.sum(), (n * n).sum()
+    d, dff, L, F = m.d_model, m.d_ff, m.n_layers, m.n_feat
+    attn_layer = 4.0 * d * s2
+    lin_layer = 2.0 * N * (3 * d * d + d * d + 2 * d * dff)
+    emb = 2.0 * N * (F * d + d * d)
+    heads = 2.0 * N * ((1 + len(m.reg_dims)) * d * d + (m.n_classes + sum(m.reg_dims)) * d)
+    return dict(attn_per_launch=attn_layer, total=L * (attn_layer + lin_layer) + emb + heads,
+                gemm_per_layer=lin_layer)
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock + throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.sm, self.reasons, self.sm_max, self.ok = index, False, [], set(), None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+                 0x80: "hw_power_brake", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting"}
+        while not self.stop_flag:
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def result(self):
+        if not self.ok or not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": ["nvml_unavailable"]}
+        return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": self.sm_max, "reasons": sorted(self.reasons)}
+
+
+# ------------------------------------------------------------------------------------------------ CPU oracle leg
+def oracle_sample(name, X, off, m, budget_s):
+    """Bounded sample of the workload for the oracle: the shortest event, or a prefix of it when even that
+    would not fit `budget_s` (the oracle runs at roughly 10 GFLOP/s per host core in fp64 numpy)."""
+    n = np.diff(off)
+    e = int(np.argmin(np.where(n > 0, n, n.max() + 1)))
+    a, b = int(off[e]), int(off[e + 1])
+    cores = os.cpu_count() or 1
+    est_rate = 1.2e10 * min(cores, 8) / 8 * 1.0          # FLOP/s, calibrated on 8 cores: 21 s for a 5048-row cfg3 event
+    ns = b - a
+    while ns > 256:
+        f = flop_model(m, np.array([0, ns]))["total"]
+        if f / est_rate <= budget_s:
+            break
+        ns = int(ns * 0.85)
+    whole = ns == b - a
+    desc = (f"{name} event {e} ({'whole, ' if whole else 'first '}{ns} of {b - a} elements), fp64 numpy oracle; "
+            f"events/s = (model FLOPs of the sample / seconds) / (model FLOPs per mean event of the batch)")
+    return X[a:a + ns], np.array([0, ns], np.int32), desc
+
+
+def time_oracle(Xs, offs, W, m, flops_per_event):
+    import oracle
+    t0 = time.perf_counter()
+    oracle.forward(Xs, offs, W, m)
+    dt = time.perf_counter() - t0
+    return flop_model(m, offs)["total"] / dt / flops_per_event, dt
+
+
+def numpy_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        ns = [p.get("num_threads", 1) for p in threadpool_info()]
+        return max(ns) if ns else 1
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    name = args.workload
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    X, off = workload(name)
+    E = len(off) - 1
+    fl = flop_model(m, off)
+    per_step_budget = max(2.0, min(25.0, 240.0 / (args.steps + args.warmup)))
+    Xs, offs, desc = oracle_sample(name, X, off, m, per_step_budget)
+    for _ in range(args.warmup):
+        time_oracle(Xs, offs, W, m, fl["total"] / E)
+    times = []
+    for _ in range(args.steps):
+        _, dt = time_oracle(Xs, offs, W, m, fl["total"] / E)
+        times.append(dt)
+    tot = float(np.sum(times))
+    sample_events = flop_model(m, offs)["total"] / (fl["total"] / E)      # the sample, in mean-event units
+    value = sample_events * args.steps / tot
+    cores = numpy_threads()
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "events": E, "elements": int(off[-1]), "n_layers": m.n_layers,
+                       "d_model": m.d_model, "n_heads": m.n_heads, "d_ff": m.d_ff, "step": "one oracle pass over the sample"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------ GPU arm
+def run_ours(args):
+    import torch
+    import paper_2601_17554_b200 as P
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (libmlpf has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    name = args.workload
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    X, off = workload(name, rank)
+    E, N = len(off) - 1, int(off[-1])
+    fl = flop_model(m, off)
+    peaks = load_peaks()
+
+    mod = P.Mlpf(W, m)
+    st = torch.cuda.Stream()
+    Xd = torch.from_numpy(X).cuda()
+    lg = torch.empty((N, mod.n_classes), dtype=torch.float32, device="cuda")
+    rg = torch.empty((N, mod.n_regress), dtype=torch.float32, device="cuda")
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
+    torch.cuda.synchronize()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed_steps(k, profile):
+        """k steps; L2 flushed (untimed) before each; returns per-step ms (CUDA events on `st`) and per-class ms."""
+        mod.set_option(P.OPT_PROFILE, 1 if profile else 0)
+        ms, cls = [], {c: [0.0, 0] for c in P.KERNEL_CLASSES}
+        with torch.cuda.stream(st):
+            for _ in range(k):
+                flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(st)
+                mod.infer(Xd, off, lg, rg, stream=st)
+                e1.record(st)
+                e1.synchronize()
+                ms.append(e0.elapsed_time(e1))
+                if profile:
+                    for c, (t, n) in mod.profile(stream=st).items():
+                        cls[c][0] += t
+                        cls[c][1] += n
+        mod.set_option(P.OPT_PROFILE, 0)
+        return np.array(ms), cls
+
+    timed_steps(args.warmup, False)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    t_wall0 = time.perf_counter()
+    ms, _ = timed_steps(args.steps, False)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    # the same K steps again with a CUDA-event pair around every kernel class (roofline numerator)
+    ms_prof, cls = timed_steps(args.steps, True)
+    sampler.stop_flag = True
+    sampler.join()
+    launches_per_step = int(mod.query(P.Q_LAUNCHES))
+    total_ms = float(ms.sum())
+    if dist is not None:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = world * E * args.steps / (total_ms * 1e-3)
+
+    # ---- end to end: pinned host buffers in, host buffers out, copies inside the timed region
+    xh = torch.from_numpy(X).pin_memory()
+    lh = torch.empty((N, mod.n_classes), dtype=torch.float32).pin_memory()
+    rh = torch.empty((N, mod.n_regress), dtype=torch.float32).pin_memory()
+    for _ in range(max(3, args.warmup // 2)):
+        mod.infer_host(xh, off, lh, rh, stream=st)
+    barrier()
+    e2e_ms = []
+    for _ in range(args.steps):
+        with torch.cuda.stream(st):
+            flush.zero_()
+        st.synchronize()
+        t0 = time.perf_counter()
+        mod.infer_host(xh, off, lh, rh, stream=st)            # synchronises the stream before returning
+        e2e_ms.append(1e3 * (time.perf_counter() - t0))
+    e2e_total = float(np.sum(e2e_ms))
+    if dist is not None:
+        t = torch.tensor([e2e_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_total = float(t.item())
+    e2e_value = world * E * args.steps / (e2e_total * 1e-3)
+    result_check = float(lh.abs().sum() + rh.abs().sum())     # the device->host result is read
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- single-event latency (one event per call, as the paper deploys it, L224): p50 / p90 over events x repeats
+    lat = []
+    reps = max(2, min(10, args.steps // 2))
+    with torch.cuda.stream(st):
+        for _ in range(reps):
+            for e in range(E):
+                a, b = int(off[e]), int(off[e + 1])
+                if b == a:
+                    continue
+                o1 = np.array([0, b - a], np.int32)
+                flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(st)
+                mod.infer(Xd[a:b], o1, lg[a:b], rg[a:b], stream=st)
+                e1.record(st)
+                e1.synchronize()
+                lat.append(e0.elapsed_time(e1))
+    lat = np.array(lat[E:]) if len(lat) > E else np.array(lat)    # first sweep = warm-up
+
+    # ---- roofline of the dominant kernel (a4 attention): algorithmic FLOPs per launch / mean launch duration
+    at_ms, at_n = cls["attention"]
+    per_launch_s = at_ms * 1e-3 / max(at_n, 1)
+    achieved = fl["attn_per_launch"] / per_launch_s / 1e12 if at_n else None
+    peak = peaks["tflops_sustained"]
+    share = {c: round(t / max(sum(v[0] for v in cls.values()), 1e-9), 4) for c, (t, n) in cls.items()}
+    gemm_ms = sum(cls[c][0] for c in ("qkv", "outproj", "ffn1", "ffn2"))
+    gemm_tflops = fl["gemm_per_layer"] * m.n_layers * args.steps / (gemm_ms * 1e-3) / 1e12 if gemm_ms else None
+    roofline = {"bound": "tensor", "kernel": "k_tc_attn (a4)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": (achieved / peak) if achieved else None, "traffic": None,
+                "peak_source": f"{peaks['source']} bf16_tflops_sustained",
+                "flops_per_launch": fl["attn_per_launch"], "ms_per_launch": per_launch_s * 1e3,
+                "class_time_share": share,
+                "class_ms_per_step": {c: round(t / args.steps, 4) for c, (t, n) in cls.items()},
+                "gemm_tflops": gemm_tflops, "gemm_frac": (gemm_tflops / peak) if gemm_tflops else None,
+                "whole_step_tflops": fl["total"] * args.steps / (total_ms * 1e-3) / 1e12}
+
+    # ---- CPU oracle on a bounded sample (rank 0, N = 1 only)
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        Xs, offs, desc = oracle_sample(name, X, off, m, 25.0)
+        v, dt = time_oracle(Xs, offs, W, m, fl["total"] / E)
+        cpu = {"value": v, "unit": UNIT, "cores": numpy_threads(), "kind": "oracle", "sample": desc, "seconds": dt}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": name, "events": E, "elements": N, "max_event": int(np.diff(off).max()),
+                       "n_layers": m.n_layers, "d_model": m.d_model, "n_heads": m.n_heads, "d_ff": m.d_ff,
+                       "activation": m.activation, "parallelism": f"events sharded over {world} GPU(s), no collective",
+                       "l2": "flushed (256 MB memset) before every timed step", "split_activations": 1},
+            "ms_per_event": total_ms / args.steps / E,
+            "step_ms_p50": float(np.percentile(ms, 50)), "step_ms_p90": float(np.percentile(ms, 90)),
+            "ms_per_step_with_class_events": float(ms_prof.mean()),
+            "single_event_ms_p50": float(np.percentile(lat, 50)), "single_event_ms_p90": float(np.percentile(lat, 90)),
+            "wall_s_timed_region": t_wall,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(N * mod.n_feat * 4),
+                    "d2h_bytes_per_step": int(N * (mod.n_classes + mod.n_regress) * 4),
+                    "ms_per_step": e2e_total / args.steps, "result_checksum": result_check},
+            "gpu_launches": launches_per_step * args.steps, "launches_per_step": launches_per_step,
+            "peak_bytes": {"weights": int(mod.query(P.Q_WEIGHT_BYTES)), "workspace": int(mod.query(P.Q_WORKSPACE_BYTES)),
+                           "torch_max_allocated": int(torch.cuda.max_memory_allocated())},
+            "clocks": sampler.result(), "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5a", "cfg5b", "paper"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
