@@ -171,6 +171,16 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def max_over_ranks(x, dist, device):
+    """Time of a multi-rank region = the slowest rank's (no-op without a process group)."""
+    if dist is None:
+        return x
+    import torch
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 # ------------------------------------------------------------------------------------------------ GPU arm
 def run_ours(args):
     import torch
@@ -241,11 +251,7 @@ def run_ours(args):
     sampler.stop_flag = True
     sampler.join()
     launches_per_step = int(mod.query(P.Q_LAUNCHES))
-    total_ms = float(ms.sum())
-    if dist is not None:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(float(ms.sum()), dist, "cuda")
     value = world * E * args.steps / (total_ms * 1e-3)
 
     # ---- end to end: pinned host buffers in, host buffers out, copies inside the timed region
@@ -263,11 +269,7 @@ def run_ours(args):
         t0 = time.perf_counter()
         mod.infer_host(xh, off, lh, rh, stream=st)            # synchronises the stream before returning
         e2e_ms.append(1e3 * (time.perf_counter() - t0))
-    e2e_total = float(np.sum(e2e_ms))
-    if dist is not None:
-        t = torch.tensor([e2e_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_total = float(t.item())
+    e2e_total = max_over_ranks(float(np.sum(e2e_ms)), dist, "cuda")
     e2e_value = world * E * args.steps / (e2e_total * 1e-3)
     result_check = float(lh.abs().sum() + rh.abs().sum())     # the device->host result is read
 
