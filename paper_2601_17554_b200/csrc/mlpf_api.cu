@@ -374,7 +374,7 @@ static int run_layernorm(mlpf_handle* h, bool fp32, const float* x, int N, const
 static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspace* w, cudaStream_t st) {
     if (w->n_tiles == 0) return MLPF_OK;
     if (tc && !fp32) {
-        int rc = tc_attn_launch(&h->tc, (const bf16*)w->qkv, w->N, w->valid, w->offsets,
+        int rc = tc_attn_launch(&h->tc, (const bf16*)w->qkv, w->N, w->valid, w->n_valid, w->offsets,
                                 (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, (bf16*)w->o,
                                 split ? (bf16*)w->o_lo : nullptr, st);
         if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", h->tc.err);
@@ -706,7 +706,7 @@ extern "C" int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_va
     CUDA_TRY(cudaMalloc(&d_pairs, pairs.size() * 4));
     CUDA_TRY(cudaMemcpyAsync(d_off, event_offsets, (size_t)(n_events + 1) * 4, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(d_pairs, pairs.data(), pairs.size() * 4, cudaMemcpyHostToDevice, st));
-    int rc = tc_attn_launch(&ctx, (const bf16*)QKV, N, key_valid, d_off, (const int2*)d_pairs,
+    int rc = tc_attn_launch(&ctx, (const bf16*)QKV, N, key_valid, nullptr, d_off, (const int2*)d_pairs,
                             (int)(pairs.size() / 2), d_model, n_heads, (bf16*)O, (bf16*)nullptr, st);
     cudaError_t e = cudaStreamSynchronize(st);
     cudaFree(d_off); cudaFree(d_pairs);

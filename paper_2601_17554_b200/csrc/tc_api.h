@@ -43,7 +43,8 @@ int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, 
 int tc_gemm_launch(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W, int M, int N, int K,
                    const Epi& ep, cudaStream_t st);
 // QKV [N, 3d] row-major bf16 (q | k | v)
-int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const int* key_valid,
+// n_valid [E] (valid rows per event) may be null
+int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const int* key_valid, const int* n_valid,
                    const int* offsets, const int2* pairs, int n_pairs, int d, int H, bf16* O, bf16* O_lo,
                    cudaStream_t st);
 

@@ -1,43 +1,48 @@
-// tc_attn.cuh -- varlen, key-padding-masked flash-attention forward on tcgen05 / TMEM / TMA (sm_100a).
+// tc_attn.cu -- varlen, key-padding-masked flash-attention forward on tcgen05 / TMEM / TMA (sm_100a).
 // Step a4 of DESIGN.md:  per event, per head  O = softmax(Q K^T / sqrt(hd) + mask) V   (Eq. 4),
 // computed with the FlashAttention recurrence (running max / running sum over key tiles, L154) so the
 // n x n weight matrix never leaves the SM.  Keys outside the event or with key_valid == 0 get weight
 // exactly 0 (reading A2); a query with no valid key gets O = 0 (A15).
 //
-// One CTA = one head x two consecutive 128-row query tiles (a, b) of one event, sharing every K / V^T tile.
-//   warp 0      TMA producer: Q_a, Q_b once; then (K_j, V_j), each [128 keys x hd] row-major, into a ring.
-//               Q, K, V are column blocks of one row-major [N, 3d] buffer, so an event may start at any row
-//               (TMA needs 16-byte alignment only along the innermost, head-dim, coordinate).
-//   warp 1      MMA issuer:   S_t = Q_t K_j^T  (M=128, N=128, K=hd)  -> TMEM (fp32);
-//                             O_t(j) = P_t V_j (A = P_t read from TMEM, B = V_j as an MN-major operand,
-//                             K=128, N=hd) -> TMEM, fresh each tile.
-//   warps 2-5   softmax warpgroup of tile a, warps 6-9 of tile b: one query row per thread:
-//               S -> (mask) -> running max -> exp2 -> bf16 P written back over S's columns in TMEM;
-//               then acc = acc * corr + O_t(j-1) in registers (no read-modify-write of O in TMEM).
-// The two warpgroups run half a period apart (S_t(j+1) is issued right after P_t(j) V_j), so one of
-// them is exponentiating while the other waits for the tensor pipe.
-// TMEM columns: S_a [0,128) S_b [128,256) (P_t aliases the first 64 columns of S_t), O_t[buf] at 256 + (2t+buf) hd.
+// One CTA = one head x two consecutive 128-row query tiles (a, b) of one event, sharing every K / V tile.
+// Key tiles are 64 keys wide and S is DOUBLE-BUFFERED in TMEM, so the tensor pipe computes S_t(j+1) while the
+// softmax warps work on S_t(j): the MMA chain (measured: ~1400 cycles of issue + hand-off latency per tile at
+// hd = 32, because one thread issues at most one tcgen05.mma per ~50 cycles whatever its N) is off the softmax
+// warps' critical path, and the exponentials (MUFU, the binding unit at hd = 32) run back to back.
+//   warps 0-3   softmax warpgroup of query tile a, warps 4-7 of tile b: one query row per thread, the tile's 64
+//               scores in registers:  S -> (mask) -> running max -> exp2 -> bf16 P written back over S's TMEM
+//               columns; then acc = acc * corr + O_t(j-1) in registers (no read-modify-write of O in TMEM).
+//   warp 8      TMA producer: Q_a, Q_b once; then stages of (K, V), each [128 keys x hd] row-major (two key tiles
+//               per stage).  Q, K, V are column blocks of one row-major [N, 3d] buffer, so an event may start at
+//               any row (TMA needs 16-byte alignment only along the innermost, head-dim, coordinate).
+//   warps 9,10  MMA issuers of tile a / b:  S_t(j) = Q_t K_j^T  (M=128, N=64, K=hd) -> TMEM buffer j&1;
+//               O_t(j) = P_t(j) V_j (A = P read from TMEM, B = V_j as an MN-major operand, K=64, N=hd)
+//               -> TMEM O buffer j&1, fresh each tile.
+//   warp 11     idle (it only makes warpgroup 2 complete for setmaxnreg).
+// TMEM columns: S_t[b] at (2t+b) 64 (P_t[b] aliases its first 32 columns); O_t[b] at 256 + (2t+b) hd.
 #include "tc_api.h"
 #include "ptx.cuh"
 
 namespace mlpf {
 
-constexpr int ATT_THREADS = 320;
-constexpr int ATT_BQ = 128, ATT_BK = 128;
+constexpr int ATT_THREADS = 384;
+constexpr int ATT_WARP_TMA = 8, ATT_WARP_MMA = 9;       // MMA issuers: warp 9 (tile a), warp 10 (tile b)
+constexpr int ATT_BQ = 128, ATT_BK = 64, ATT_SK = 128;  // query tile, key tile, keys per TMA stage
 
 template <int HD>
 struct AttnCfg {
     static constexpr int Q_BYTES = ATT_BQ * HD * 2;
-    static constexpr int K_BYTES = ATT_BK * HD * 2;
-    static constexpr int V_BYTES = HD * ATT_BK * 2;
+    static constexpr int K_BYTES = ATT_SK * HD * 2;
+    static constexpr int V_BYTES = ATT_SK * HD * 2;
     static constexpr int STAGE_BYTES = K_BYTES + V_BYTES;
     static constexpr int STAGES = HD == 64 ? 4 : 6;
     static constexpr int SMEM_BYTES = 2 * Q_BYTES + STAGES * STAGE_BYTES + 1024;
-    static constexpr int SW = HD * 2;                       // swizzle width of Q / K rows in bytes
+    static constexpr int SW = HD * 2;                       // swizzle width of Q / K / V rows in bytes
 };
 
 struct AttnParams {
     const int* key_valid;      // [N] or null
+    const int* n_valid;        // [E] valid rows per event, or null: events without pad rows skip the key_valid loads
     const int* offsets;        // [E+1]
     const int2* pairs;         // (event, pair index)
     int n_pairs, H, d;
@@ -45,22 +50,77 @@ struct AttnParams {
     float scale_log2;          // log2(e) / sqrt(hd)
 };
 
+// 32 scores of one row (registers r[0..31]) -> running max
+template <bool FULL>
+__device__ __forceinline__ float max32(const uint32_t* r, uint32_t mask, float mx) {
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+        const float v = __uint_as_float(r[i]);
+        mx = fmaxf(mx, FULL ? v : ((mask >> i) & 1u ? v : -INFINITY));
+    }
+    return mx;
+}
+// p = 2^(s c - m c) for 32 scores -> 16 bf16 pairs; their fp32 sums go to two packed accumulators (short chains)
+template <bool FULL>
+__device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c, float neg_mc, uint32_t (&pk)[16],
+                                      float2 (&rs)[2]) {
+    const float2 c2 = make_float2(c, c), m2 = make_float2(neg_mc, neg_mc);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const float2 x = ptx::ffma2(make_float2(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1])), c2, m2);
+        float2 p = make_float2(ptx::fast_exp2(x.x), ptx::fast_exp2(x.y));
+        if (!FULL) {
+            p.x = (mask >> (2 * i)) & 1u ? p.x : 0.0f;
+            p.y = (mask >> (2 * i + 1)) & 1u ? p.y : 0.0f;
+        }
+        rs[i & 1] = ptx::fadd2(rs[i & 1], p);
+        __nv_bfloat162 b2 = __floats2bfloat162_rn(p.x, p.y);
+        pk[i] = *reinterpret_cast<uint32_t*>(&b2);
+    }
+}
+
+// One 64-key tile of one query row, scores already in registers s[0..63]:
+// running max -> P = 2^(S c - m c) as bf16, written over S's first 32 TMEM columns at s_addr.
+// Returns corr = 2^((m_old - m_new) c) and the row sum of P in rsum.
+template <bool FULL>
+__device__ __forceinline__ float softmax_tile(const uint32_t (&s)[64], uint32_t s_addr, const uint32_t (&mask)[2], float c,
+                                              float& m_run, float& rsum) {
+    float mx = max32<FULL>(&s[0], mask[0], -INFINITY);
+    mx = max32<FULL>(&s[32], mask[1], mx);
+    const float m_new = fmaxf(m_run, mx);
+    const float m_use = (m_new == -INFINITY) ? 0.0f : m_new;
+    const float corr = ptx::fast_exp2((m_run - m_use) * c);      // m_run = -inf -> 0
+    const float neg_mc = -m_use * c;
+    m_run = m_new;
+    float2 rs[2] = {make_float2(0.0f, 0.0f), make_float2(0.0f, 0.0f)};
+#pragma unroll
+    for (int w = 0; w < 2; ++w) {
+        uint32_t pk[16];
+        exp32<FULL>(&s[32 * w], mask[w], c, neg_mc, pk, rs);
+        ptx::tmem_st16(s_addr + 16 * w, pk);
+    }
+    rsum = (rs[0].x + rs[0].y) + (rs[1].x + rs[1].y);
+    return corr;
+}
+
 template <int HD>
 __global__ void __launch_bounds__(ATT_THREADS, 1)
 k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     using Cfg = AttnCfg<HD>;
     constexpr int ST = Cfg::STAGES;
     extern __shared__ uint8_t smem_raw[];
-    __shared__ uint64_t bars[1 + 2 * ST + 6];
+    __shared__ uint64_t bars[1 + 2 * ST + 10];
     __shared__ uint32_t tmem_base_slot;
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
     const int item = blockIdx.x / prm.H, head = blockIdx.x % prm.H;
     const int2 pr = prm.pairs[item];
     const int ev0 = prm.offsets[pr.x], ev1 = prm.offsets[pr.x + 1];
     const int q0a = ev0 + pr.y * 2 * ATT_BQ, q0b = q0a + ATT_BQ;
     const bool has_b = q0b < ev1;
-    const int nkv = (ev1 - ev0 + ATT_BK - 1) / ATT_BK;
+    const int nkv = (ev1 - ev0 + ATT_BK - 1) / ATT_BK;              // 64-key tiles
+    const int* key_valid = (prm.key_valid && !(prm.n_valid && prm.n_valid[pr.x] == ev1 - ev0)) ? prm.key_valid : nullptr;
+    const int nst = (ev1 - ev0 + ATT_SK - 1) / ATT_SK;              // 128-key TMA stages
 
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t sQ = smem_base;                                  // Q_a, Q_b
@@ -68,22 +128,26 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     const uint32_t bar_q = ptx::smem_u32(&bars[0]);
     const uint32_t bar_kv_full = ptx::smem_u32(&bars[1]);
     const uint32_t bar_kv_empty = ptx::smem_u32(&bars[1 + ST]);
-    const uint32_t bar_s = ptx::smem_u32(&bars[1 + 2 * ST]);        // [t]
-    const uint32_t bar_p = ptx::smem_u32(&bars[1 + 2 * ST + 2]);    // [t]
-    const uint32_t bar_o = ptx::smem_u32(&bars[1 + 2 * ST + 4]);    // [t]
+    const uint32_t bar_s = ptx::smem_u32(&bars[1 + 2 * ST]);        // [2t + b]: S_t(j) landed in buffer b = j & 1
+    const uint32_t bar_p = ptx::smem_u32(&bars[1 + 2 * ST + 4]);    // [2t + b]: P_t(j) written over buffer b
+    const uint32_t bar_o = ptx::smem_u32(&bars[1 + 2 * ST + 8]);    // [t]: O_t(j) complete
 
-    if (warp == 0 && lane == 0) {
+    if (warp == ATT_WARP_TMA && lane == 0) {
         ptx::mbar_init(bar_q, 1);
-        for (int s = 0; s < ST; ++s) { ptx::mbar_init(bar_kv_full + 8 * s, 1); ptx::mbar_init(bar_kv_empty + 8 * s, 1); }
-        for (int t = 0; t < 2; ++t) {
-            ptx::mbar_init(bar_s + 8 * t, 1);
-            ptx::mbar_init(bar_p + 8 * t, 4);                        // one arrival per softmax warp
-            ptx::mbar_init(bar_o + 8 * t, 1);
+        for (int s = 0; s < ST; ++s) {
+            ptx::mbar_init(bar_kv_full + 8 * s, 1);
+            ptx::mbar_init(bar_kv_empty + 8 * s, has_b ? 2 : 1);     // one commit per query tile
         }
+        for (int i = 0; i < 4; ++i) {
+            ptx::mbar_init(bar_s + 8 * i, 1);
+            ptx::mbar_init(bar_p + 8 * i, 4);                        // one arrival per softmax warp
+        }
+        ptx::mbar_init(bar_o, 1);
+        ptx::mbar_init(bar_o + 8, 1);
         ptx::fence_barrier_init();
         ptx::tma_prefetch_desc(&tmQKV);
     }
-    if (warp == 1) {
+    if (warp == ATT_WARP_MMA) {
         ptx::tmem_alloc(ptx::smem_u32(&tmem_base_slot), 512);
         ptx::tmem_relinquish();
     }
@@ -92,185 +156,160 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     ptx::tc_fence_after();
     const uint32_t tmem_base = tmem_base_slot;
 
-    if (warp == 0) {
+    if (warp >= 8) {
+    ptx::setmaxnreg_dec<40>();
+    if (warp == ATT_WARP_TMA) {
         // ------------------------------------------------------------ TMA producer
         if (lane == 0) {
             ptx::mbar_expect_tx(bar_q, Cfg::Q_BYTES * (has_b ? 2 : 1));
             ptx::tma_load_2d(sQ, &tmQKV, bar_q, head * HD, q0a);
             if (has_b) ptx::tma_load_2d(sQ + Cfg::Q_BYTES, &tmQKV, bar_q, head * HD, q0b);
         }
-        for (int j = 0; j < nkv; ++j) {
-            const int s = j % ST;
-            ptx::mbar_wait(bar_kv_empty + 8 * s, ((j / ST) & 1) ^ 1);
+        for (int i = 0; i < nst; ++i) {
+            const int s = i % ST;
+            ptx::mbar_wait(bar_kv_empty + 8 * s, ((i / ST) & 1) ^ 1);
             if (lane == 0) {
                 const uint32_t st = sKV + s * Cfg::STAGE_BYTES;
-                const int k0 = ev0 + j * ATT_BK;
+                const int k0 = ev0 + i * ATT_SK;
                 ptx::mbar_expect_tx(bar_kv_full + 8 * s, Cfg::STAGE_BYTES);
                 ptx::tma_load_2d(st, &tmQKV, bar_kv_full + 8 * s, prm.d + head * HD, k0);
                 ptx::tma_load_2d(st + Cfg::K_BYTES, &tmQKV, bar_kv_full + 8 * s, 2 * prm.d + head * HD, k0);
             }
             __syncwarp();
         }
-    } else if (warp == 1) {
-        // ------------------------------------------------------------ MMA issuer
+    } else if (warp == ATT_WARP_MMA || warp == ATT_WARP_MMA + 1) {
+        // ------------------------------------------------------------ MMA issuers (one per query tile)
+        const int t = warp - ATT_WARP_MMA;
         constexpr uint32_t idesc_s = ptx::umma_idesc_bf16(128, ATT_BK);
         constexpr uint32_t idesc_o = ptx::umma_idesc_bf16(128, HD) | ptx::UMMA_B_MN_MAJOR;
-        auto issue_s = [&](int t, int j) {          // S_t = Q_t K_j^T
-            const uint32_t kb = sKV + (j % ST) * Cfg::STAGE_BYTES;
+        constexpr uint32_t HALF = ATT_BK * Cfg::SW;                  // bytes of a 64-key half of a K or V stage
+        auto issue_s = [&](int j) {                 // S_t(j) = Q_t K_j^T -> S buffer j & 1
+            const uint32_t kb = sKV + ((j >> 1) % ST) * Cfg::STAGE_BYTES + (j & 1) * HALF;
             const uint32_t qb = sQ + t * Cfg::Q_BYTES;
 #pragma unroll
             for (int k = 0; k < HD / 16; ++k)
-                ptx::mma_ss(tmem_base + t * 128, ptx::umma_desc_kmajor(qb + k * 32, Cfg::SW),
+                ptx::mma_ss(tmem_base + (2 * t + (j & 1)) * 64, ptx::umma_desc_kmajor(qb + k * 32, Cfg::SW),
                             ptx::umma_desc_kmajor(kb + k * 32, Cfg::SW), idesc_s, k != 0);
-            ptx::mma_commit(bar_s + 8 * t);
+            ptx::mma_commit(bar_s + 8 * (2 * t + (j & 1)));
         };
-        auto issue_o = [&](int t, int j) {          // O_t(j) = P_t V_j
-            const uint32_t vb = sKV + (j % ST) * Cfg::STAGE_BYTES + Cfg::K_BYTES;
+        auto issue_o = [&](int j) {                 // O_t(j) = P_t(j) V_j -> O buffer j & 1
+            const uint32_t vb = sKV + ((j >> 1) % ST) * Cfg::STAGE_BYTES + Cfg::K_BYTES + (j & 1) * HALF;
             const uint32_t o_col = 256 + (2 * t + (j & 1)) * HD;
 #pragma unroll
             for (int k = 0; k < ATT_BK / 16; ++k)
-                ptx::mma_ts(tmem_base + o_col, tmem_base + t * 128 + k * 8,
+                ptx::mma_ts(tmem_base + o_col, tmem_base + (2 * t + (j & 1)) * 64 + k * 8,
                             ptx::umma_desc_mnmajor(vb + k * 16 * Cfg::SW, Cfg::SW), idesc_o, k != 0);
             ptx::mma_commit(bar_o + 8 * t);
         };
-        ptx::mbar_wait(bar_q, 0);
-        ptx::mbar_wait(bar_kv_full, 0);
-        ptx::tc_fence_after();
-        if (lane == 0) { issue_s(0, 0); if (has_b) issue_s(1, 0); }
-        __syncwarp();
-        for (int j = 0; j < nkv; ++j) {
-            const uint32_t par = j & 1;
-            const bool more = j + 1 < nkv;
-            if (more) ptx::mbar_wait(bar_kv_full + 8 * ((j + 1) % ST), ((j + 1) / ST) & 1);
-            ptx::mbar_wait(bar_p, par);                           // P_a(j) is in TMEM
+        if (t == 0 || has_b) {
+            ptx::mbar_wait(bar_q, 0);
+            ptx::mbar_wait(bar_kv_full, 0);
             ptx::tc_fence_after();
-            if (lane == 0) {
-                issue_o(0, j);
-                if (!has_b) ptx::mma_commit(bar_kv_empty + 8 * (j % ST));
-                if (more) issue_s(0, j + 1);
-            }
-            __syncwarp();
-            if (has_b) {
-                ptx::mbar_wait(bar_p + 8, par);
+            issue_s(0);                             // all lanes: one is elected inside the MMA / commit wrappers
+            if (nkv > 1) issue_s(1);
+            for (int j = 0; j < nkv; ++j) {
+                ptx::mbar_wait(bar_p + 8 * (2 * t + (j & 1)), (j >> 1) & 1);     // P_t(j) is in TMEM
                 ptx::tc_fence_after();
-                if (lane == 0) {
-                    issue_o(1, j);
-                    ptx::mma_commit(bar_kv_empty + 8 * (j % ST));
-                    if (more) issue_s(1, j + 1);
+                issue_o(j);
+                // K and V of stage j >> 1 are no longer needed by this tile after its second half
+                if ((j & 1) || j == nkv - 1) ptx::mma_commit(bar_kv_empty + 8 * ((j >> 1) % ST));
+                if (j + 2 < nkv) {                   // S_t(j+2) reuses S buffer j & 1: in order after P_t(j) V_j
+                    const int i2 = (j + 2) >> 1;
+                    if (((j + 2) & 1) == 0) ptx::mbar_wait(bar_kv_full + 8 * (i2 % ST), (i2 / ST) & 1);
+                    ptx::tc_fence_after();
+                    issue_s(j + 2);
                 }
-                __syncwarp();
             }
         }
+    }
     } else {
         // ------------------------------------------------------------ softmax warpgroups
-        const int t = (warp - 2) >> 2;                 // 0: tile a, 1: tile b
+        ptx::setmaxnreg_inc<232>();
+        const int t = warp >> 2;                       // 0: tile a, 1: tile b
         const int q = warp & 3;                        // TMEM lane quarter this warp may access
         const int row_in_tile = q * 32 + lane;
         const int qrow = (t == 0 ? q0a : q0b) + row_in_tile;
         if (t == 0 || has_b) {
             const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16);
-            const uint32_t s_addr = lane_addr + t * 128;
             const float c = prm.scale_log2;
             float acc[HD];
 #pragma unroll
             for (int i = 0; i < HD; ++i) acc[i] = 0.0f;
-            float m_run = -INFINITY, l_run = 0.0f, corr_prev = 0.0f;
-            for (int j = 0; j < nkv; ++j) {
-                // key mask of this tile: 4 x 32 bits, computed redundantly per warp (no cross-warp sync)
-                const int k0 = ev0 + j * ATT_BK;
-                uint32_t mask[4];
-#pragma unroll
-                for (int w = 0; w < 4; ++w) {
-                    const int key = k0 + w * 32 + lane;
-                    bool ok = key < ev1;
-                    if (ok && prm.key_valid) ok = prm.key_valid[key] != 0;
-                    mask[w] = __ballot_sync(0xffffffffu, ok);
-                }
-                const bool full = (mask[0] & mask[1] & mask[2] & mask[3]) == 0xffffffffu;
-                ptx::mbar_wait(bar_s + 8 * t, j & 1);
-                ptx::tc_fence_after();
-                // pass 1: row max
-                float mx = -INFINITY;
-#pragma unroll
-                for (int w = 0; w < 4; ++w) {
-                    uint32_t r[32];
-                    ptx::tmem_ld32(s_addr + w * 32, r);
-                    ptx::tmem_ld_wait();
-                    if (full) {
-#pragma unroll
-                        for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(r[i]));
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 32; ++i)
-                            mx = fmaxf(mx, (mask[w] >> i) & 1u ? __uint_as_float(r[i]) : -INFINITY);
-                    }
-                }
-                const float m_new = fmaxf(m_run, mx);
-                const float m_use = (m_new == -INFINITY) ? 0.0f : m_new;
-                const float corr = ptx::fast_exp2((m_run - m_use) * c);          // m_run = -inf -> 0
-                const float neg_mc = -m_use * c;
-                float rsum = 0.0f;
-                // pass 2: P = exp2(S c - m c) as bf16 pairs, written over S's first 64 columns
-#pragma unroll
-                for (int w = 0; w < 4; ++w) {
-                    uint32_t r[32];
-                    ptx::tmem_ld32(s_addr + w * 32, r);
-                    ptx::tmem_ld_wait();
-                    uint32_t pk[16];
-#pragma unroll
-                    for (int i = 0; i < 16; ++i) {
-                        float p0 = ptx::fast_exp2(fmaf(__uint_as_float(r[2 * i]), c, neg_mc));
-                        float p1 = ptx::fast_exp2(fmaf(__uint_as_float(r[2 * i + 1]), c, neg_mc));
-                        if (!full) {
-                            p0 = (mask[w] >> (2 * i)) & 1u ? p0 : 0.0f;
-                            p1 = (mask[w] >> (2 * i + 1)) & 1u ? p1 : 0.0f;
-                        }
-                        rsum += p0 + p1;
-                        __nv_bfloat162 b2 = __floats2bfloat162_rn(p0, p1);
-                        pk[i] = *reinterpret_cast<uint32_t*>(&b2);
-                    }
-                    ptx::tmem_st16(s_addr + w * 16, pk);
-                }
-                ptx::tmem_st_wait();
-                ptx::tc_fence_before();
-                // O_t(j-1) was issued a whole softmax period ago: this wait does not stall, but it must come
-                // BEFORE P_t(j) is published -- afterwards O_t(j) could complete too and the barrier would be two
-                // phases ahead of this waiter (parity aliasing).
-                if (j > 0) ptx::mbar_wait(bar_o + 8 * t, (j - 1) & 1);
-                __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(bar_p + 8 * t);
-                l_run = l_run * corr + rsum;
-                m_run = m_new;
-                // fold the previous tile's P V into the register accumulator
-                if (j > 0) {
-                    ptx::tc_fence_after();
-                    const uint32_t o_addr = lane_addr + 256 + (2 * t + ((j - 1) & 1)) * HD;
-#pragma unroll
-                    for (int w = 0; w < HD / 16; ++w) {
-                        uint32_t r[16];
-                        ptx::tmem_ld16(o_addr + w * 16, r);
-                        ptx::tmem_ld_wait();
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) acc[w * 16 + i] = fmaf(acc[w * 16 + i], corr_prev, __uint_as_float(r[i]));
-                    }
-                }
-                corr_prev = corr;
-            }
-            // last tile's P V
-            {
-                const int j = nkv - 1;
-                ptx::mbar_wait(bar_o + 8 * t, j & 1);
-                ptx::tc_fence_after();
+            float m_run = -INFINITY, l_run = 0.0f, corr_prev = 0.0f, rsum_prev = 0.0f;
+            // O_t(j) of a finished P V product: issue the TMEM loads ...
+            uint32_t o_r[HD];
+            auto fold_load = [&](int j) {
                 const uint32_t o_addr = lane_addr + 256 + (2 * t + (j & 1)) * HD;
 #pragma unroll
-                for (int w = 0; w < HD / 16; ++w) {
-                    uint32_t r[16];
-                    ptx::tmem_ld16(o_addr + w * 16, r);
-                    ptx::tmem_ld_wait();
+                for (int w = 0; w < HD / 16; ++w) ptx::tmem_ld16(o_addr + w * 16, *reinterpret_cast<uint32_t(*)[16]>(&o_r[w * 16]));
+            };
+            // ... and (after tcgen05.wait::ld) fold them in: acc = acc * corr + O_t(j), l = l * corr + rowsum(P_t(j))
+            auto fold = [&](float corr_j, float rsum_j) {
+                const float2 c2 = make_float2(corr_j, corr_j);
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) acc[w * 16 + i] = fmaf(acc[w * 16 + i], corr_prev, __uint_as_float(r[i]));
+                for (int i = 0; i < HD / 2; ++i) {
+                    const float2 a2 = ptx::ffma2(make_float2(acc[2 * i], acc[2 * i + 1]), c2,
+                                                 make_float2(__uint_as_float(o_r[2 * i]), __uint_as_float(o_r[2 * i + 1])));
+                    acc[2 * i] = a2.x; acc[2 * i + 1] = a2.y;
                 }
+                l_run = fmaf(l_run, corr_j, rsum_j);
+            };
+            // scores of the current tile live in registers; the next tile's are loaded while this one is finished
+            uint32_t s[64];
+            auto load_s = [&](int j) {
+                ptx::mbar_wait(bar_s + 8 * (2 * t + (j & 1)), (j >> 1) & 1);
+                ptx::tc_fence_after();
+                const uint32_t s_addr = lane_addr + (2 * t + (j & 1)) * 64;
+                ptx::tmem_ld32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
+                ptx::tmem_ld32(s_addr + 32, *reinterpret_cast<uint32_t(*)[32]>(&s[32]));
+            };
+            load_s(0);
+            ptx::tmem_ld_wait();
+            for (int j = 0; j < nkv; ++j) {
+                // key mask of this tile: 2 x 32 bits, computed redundantly per warp (no cross-warp sync)
+                const int k0 = ev0 + j * ATT_BK;
+                uint32_t mask[2];
+                bool full = k0 + ATT_BK <= ev1;
+                if (!full || key_valid) {
+#pragma unroll
+                    for (int w = 0; w < 2; ++w) {
+                        const int key = k0 + w * 32 + lane;
+                        bool ok = key < ev1;
+                        if (ok && key_valid) ok = key_valid[key] != 0;
+                        mask[w] = __ballot_sync(0xffffffffu, ok);
+                    }
+                    full = (mask[0] & mask[1]) == 0xffffffffu;
+                } else {
+                    mask[0] = mask[1] = 0xffffffffu;
+                }
+                const uint32_t s_addr = lane_addr + (2 * t + (j & 1)) * 64;
+                float rsum;
+                const float corr = full ? softmax_tile<true>(s, s_addr, mask, c, m_run, rsum)
+                                        : softmax_tile<false>(s, s_addr, mask, c, m_run, rsum);
+                // O_t(j-1) was issued about a softmax period ago: this wait does not stall, but it must come BEFORE
+                // P_t(j) is published -- afterwards O_t(j) could complete too and the barrier would be two phases
+                // ahead of this waiter (parity aliasing)
+                if (j > 0) {
+                    ptx::mbar_wait(bar_o + 8 * t, (j - 1) & 1);
+                    ptx::tc_fence_after();
+                    fold_load(j - 1);
+                }
+                if (j + 1 < nkv) load_s(j + 1);         // S_t(j+1) is double-buffered: usually long complete
+                ptx::tmem_st_wait();                      // the loads above fly while the P stores drain
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(bar_p + 8 * (2 * t + (j & 1)));      // P_t(j) is in TMEM
+                ptx::tmem_ld_wait();
+                if (j > 0) fold(corr_prev, rsum_prev);
+                corr_prev = corr;
+                rsum_prev = rsum;
             }
+            // last tile's P V
+            ptx::mbar_wait(bar_o + 8 * t, (nkv - 1) & 1);
+            ptx::tc_fence_after();
+            fold_load(nkv - 1);
+            ptx::tmem_ld_wait();
+            fold(corr_prev, rsum_prev);
             if (qrow < ev1) {
                 const float inv = l_run > 0.0f ? 1.0f / l_run : 0.0f;
                 uint32_t hi[HD / 2], lo[HD / 2];
@@ -295,7 +334,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     }
     ptx::tc_fence_before();
     __syncthreads();
-    if (warp == 1) ptx::tmem_dealloc(tmem_base, 512);
+    if (warp == ATT_WARP_MMA) ptx::tmem_dealloc(tmem_base, 512);
 }
 
 template <int HD>
@@ -303,7 +342,7 @@ static int tc_attn_launch_hd(TcContext* c, const bf16* QKV, int64_t N, const Att
                              cudaStream_t st) {
     using Cfg = AttnCfg<HD>;
     CUtensorMap tmQKV;
-    if (tc_tensor_map(c, &tmQKV, QKV, 3 * prm.d, N, 3 * prm.d, HD, ATT_BQ)) return -1;
+    if (tc_tensor_map(c, &tmQKV, QKV, 3 * prm.d, N, 3 * prm.d, HD, ATT_SK)) return -1;
     auto kern = k_tc_attn<HD>;
     static bool attr_set = false;
     if (!attr_set) {
@@ -315,12 +354,12 @@ static int tc_attn_launch_hd(TcContext* c, const bf16* QKV, int64_t N, const Att
     return 0;
 }
 
-int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const int* key_valid,
+int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const int* key_valid, const int* n_valid,
                           const int* offsets, const int2* pairs, int n_pairs, int d, int H, bf16* O, bf16* O_lo,
                           cudaStream_t st) {
     const int hd = d / H;
     AttnParams prm;
-    prm.key_valid = key_valid; prm.offsets = offsets; prm.pairs = pairs; prm.n_pairs = n_pairs; prm.H = H; prm.d = d;
+    prm.key_valid = key_valid; prm.n_valid = n_valid; prm.offsets = offsets; prm.pairs = pairs; prm.n_pairs = n_pairs; prm.H = H; prm.d = d;
     prm.O = O; prm.O_lo = O_lo;
     prm.scale_log2 = 1.4426950408889634f / sqrtf((float)hd);
     switch (hd) {

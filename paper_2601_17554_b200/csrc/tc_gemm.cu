@@ -126,7 +126,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     __shared__ uint64_t bars[2 * STAGES + 1];
     __shared__ uint32_t tmem_base_slot;
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
     const int m0 = blockIdx.y * GEMM_BM, n0 = blockIdx.x * BLOCK_N;
     int64_t w_row0 = 0;
     if (ep.group_offsets) {                                   // grouped GEMM (per-type embedding weights)
@@ -181,7 +181,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             const uint32_t ph = (kb / STAGES) & 1;
             ptx::mbar_wait(bar_full + 8 * s, ph);
             ptx::tc_fence_after();
-            if (lane == 0) {
+            {   // all lanes, warp-uniform operands: one lane is elected inside the MMA / commit wrappers
                 const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
                 const uint32_t b_addr = a_addr + Cfg::A_BYTES * (SPLIT ? 2 : 1);
 #pragma unroll
@@ -193,7 +193,6 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 ptx::mma_commit(bar_empty + 8 * s);           // frees the stage when these MMAs retire
                 if (kb == num_kb - 1) ptx::mma_commit(bar_acc);
             }
-            __syncwarp();
         }
     } else {
         // ---------------- epilogue: warp w reads TMEM lanes 32*(w%4) .. +31
