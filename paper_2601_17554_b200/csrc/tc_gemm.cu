@@ -1,10 +1,12 @@
-// tc_gemm.cuh -- tcgen05 / TMEM / TMA GEMM for sm_100a:  C[M,N] = A[M,K] W[N,K]^T  (+ shared epilogue).
+// tc_gemm.cu -- tcgen05 / TMEM / TMA GEMM for sm_100a:  C[M,N] = A[M,K] W[N,K]^T  (+ shared epilogue).
 // Steps a1 (second layer), a3, a5, a6, a7, a8 (first layer) of DESIGN.md; contractions of PAPER.md L148-L156.
 //
-// One CTA computes a 128 x BLOCK_N tile.  Warp 0 = TMA producer (128B-swizzled K-major tiles of 64 bf16
-// columns into a ring of shared-memory stages), warp 1 = MMA issuer (one elected thread, tcgen05.mma
-// kind::f16, fp32 accumulator in TMEM), warps 2..5 = epilogue (tcgen05.ld, one accumulator row per thread).
-// Two CTAs are co-resident per SM so one tile's epilogue overlaps the other's main loop.
+// Persistent kernel, one CTA per SM looping over 128 x BLOCK_N output tiles (n fastest, so the CTAs running
+// at the same time share A tiles in L2).  Warp 0 = TMA producer (128B-swizzled K-major tiles of 64 bf16
+// columns into a ring of shared-memory stages that runs on across tiles), warp 1 = MMA issuer (tcgen05.mma
+// kind::f16, fp32 accumulators in TWO TMEM buffers), warps 2-5 and 6-9 = two epilogue warpgroups, one per
+// accumulator buffer (tcgen05.ld, one accumulator row per thread): the epilogue of tile i overlaps the main
+// loop of tile i+1 and the epilogue of tile i+1.
 // SPLIT: A is given as two bf16 terms (A = A_hi + A_lo); both are multiplied by the same W tile into the
 // same accumulator, so activation rounding is ~2^-17 instead of 2^-9.
 #include "tc_api.h"
@@ -59,7 +61,7 @@ int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, 
 
 // ------------------------------------------------------------------------------------------------ kernel
 constexpr int GEMM_BM = 128, GEMM_BK = 64;
-constexpr int GEMM_THREADS = 192;
+constexpr int GEMM_THREADS = 320;                              // TMA, MMA, 2 x 4 epilogue warps
 
 template <int BLOCK_N, int STAGES, bool SPLIT>
 struct GemmCfg {
@@ -67,19 +69,43 @@ struct GemmCfg {
     static constexpr int B_BYTES = BLOCK_N * GEMM_BK * 2;
     static constexpr int STAGE_BYTES = A_BYTES * (SPLIT ? 2 : 1) + B_BYTES;
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024;   // + slack for 1024 B alignment
-    static constexpr int TMEM_COLS = BLOCK_N < 32 ? 32 : BLOCK_N;
+    static constexpr int TMEM_COLS = 2 * BLOCK_N < 32 ? 32 : 2 * BLOCK_N;   // two accumulator buffers (power of 2)
 };
 
-// epilogue of one 32-column chunk held in registers (thread = one row)
-template <typename = void>
-__device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[32], const Epi& ep, int64_t w_row0, int row,
+// exact-erf GELU (reading A6) with erf from Abramowitz & Stegun 7.1.26 (|error| <= 1.5e-7): 2 MUFU + ~12 FMA-pipe
+// instructions instead of erff's ~40 (the activation epilogues are issue-bound).  For x < 0 the form
+// 0.5 x (1 - erf|x|) = 0.5 x p e avoids the cancellation in 1 + erf(x).
+__device__ __forceinline__ float gelu_fast(float x) {
+    const float ax = fabsf(x) * 0.70710678118654752440f;
+    float t;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t) : "f"(fmaf(0.3275911f, ax, 1.0f)));
+    float p = fmaf(t, 1.061405429f, -1.453152027f);
+    p = fmaf(p, t, 1.421413741f);
+    p = fmaf(p, t, -0.284496736f);
+    p = fmaf(p, t, 0.254829592f);
+    p *= t;
+    const float e = ptx::fast_exp2(ax * ax * -1.4426950408889634f);
+    const float h = 0.5f * x * p * e;                  // 0.5 x (1 - erf|x|)
+    return x >= 0.0f ? x - h : h;
+}
+__device__ __forceinline__ float act_fast(float x, int act) {
+    if (act == ACT_RELU) return fmaxf(x, 0.0f);
+    if (act == ACT_GELU) return gelu_fast(x);
+    return x;
+}
+
+// epilogue of one 32-column chunk held in registers (thread = one row); bias_s = this tile's bias in shared memory
+__device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[32], const Epi& ep, const float* bias_s, int row,
                                                     int n_base, bool row_ok) {
     float v[32];
 #pragma unroll
-    for (int j = 0; j < 32; ++j) {
-        float x = __uint_as_float(acc[j]);
-        if (ep.bias) x += __ldg(ep.bias + w_row0 + n_base + j);
-        v[j] = apply_act(x, ep.act);
+    for (int j = 0; j < 8; ++j) {
+        float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (bias_s) b = *reinterpret_cast<const float4*>(bias_s + 4 * j);       // broadcast LDS.128
+        v[4 * j] = act_fast(__uint_as_float(acc[4 * j]) + b.x, ep.act);
+        v[4 * j + 1] = act_fast(__uint_as_float(acc[4 * j + 1]) + b.y, ep.act);
+        v[4 * j + 2] = act_fast(__uint_as_float(acc[4 * j + 2]) + b.z, ep.act);
+        v[4 * j + 3] = act_fast(__uint_as_float(acc[4 * j + 3]) + b.w, ep.act);
     }
     if (!row_ok) return;
     if (ep.residual) {
@@ -118,31 +144,28 @@ __device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[32], c
 }
 
 template <int BLOCK_N, int STAGES, bool SPLIT>
-__global__ void __launch_bounds__(GEMM_THREADS)
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
 k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmA_lo,
           const __grid_constant__ CUtensorMap tmB, int M, int N, int K, Epi ep) {
     using Cfg = GemmCfg<BLOCK_N, STAGES, SPLIT>;
     extern __shared__ uint8_t smem_raw[];
-    __shared__ uint64_t bars[2 * STAGES + 1];
+    __shared__ uint64_t bars[2 * STAGES + 4];
     __shared__ uint32_t tmem_base_slot;
+    __shared__ __align__(16) float bias_s[2][BLOCK_N];
 
     const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
-    const int m0 = blockIdx.y * GEMM_BM, n0 = blockIdx.x * BLOCK_N;
-    int64_t w_row0 = 0;
-    if (ep.group_offsets) {                                   // grouped GEMM (per-type embedding weights)
-        if (m0 >= ep.group_offsets[ep.n_groups + 1]) return;  // CTA-uniform, before any barrier / allocation
-        int g = 1;
-        while (g < ep.n_groups && m0 >= ep.group_offsets[g + 1]) ++g;
-        w_row0 = (int64_t)(g - 1) * N;
-    }
+    const int n_tiles_n = N / BLOCK_N;
+    const int total_tiles = ((M + GEMM_BM - 1) / GEMM_BM) * n_tiles_n;
+    const int m_end = ep.group_offsets ? ep.group_offsets[ep.n_groups + 1] : M;   // grouped: rows beyond the last group
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_full = ptx::smem_u32(&bars[0]);
     const uint32_t bar_empty = ptx::smem_u32(&bars[STAGES]);
-    const uint32_t bar_acc = ptx::smem_u32(&bars[2 * STAGES]);
+    const uint32_t bar_acc_full = ptx::smem_u32(&bars[2 * STAGES]);        // [buf]
+    const uint32_t bar_acc_empty = ptx::smem_u32(&bars[2 * STAGES + 2]);   // [buf]
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < STAGES; ++s) { ptx::mbar_init(bar_full + 8 * s, 1); ptx::mbar_init(bar_empty + 8 * s, 1); }
-        ptx::mbar_init(bar_acc, 1);
+        for (int b = 0; b < 2; ++b) { ptx::mbar_init(bar_acc_full + 8 * b, 1); ptx::mbar_init(bar_acc_empty + 8 * b, 4); }
         ptx::fence_barrier_init();
         ptx::tma_prefetch_desc(&tmA);
         ptx::tma_prefetch_desc(&tmB);
@@ -159,57 +182,104 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     const int num_kb = K / GEMM_BK;
 
     if (warp == 0) {
-        // ---------------- TMA producer
-        for (int kb = 0; kb < num_kb; ++kb) {
-            const int s = kb % STAGES;
-            const uint32_t ph = (kb / STAGES) & 1;
-            ptx::mbar_wait(bar_empty + 8 * s, ph ^ 1);
-            if (lane == 0) {
-                const uint32_t st = smem_base + s * Cfg::STAGE_BYTES;
-                ptx::mbar_expect_tx(bar_full + 8 * s, Cfg::STAGE_BYTES);
-                ptx::tma_load_2d(st, &tmA, bar_full + 8 * s, kb * GEMM_BK, m0);
-                if (SPLIT) ptx::tma_load_2d(st + Cfg::A_BYTES, &tmA_lo, bar_full + 8 * s, kb * GEMM_BK, m0);
-                ptx::tma_load_2d(st + Cfg::A_BYTES * (SPLIT ? 2 : 1), &tmB, bar_full + 8 * s, kb * GEMM_BK, (int)(w_row0 + n0));
+        // ---------------- TMA producer: the stage ring runs on across tiles
+        uint32_t kbg = 0;
+        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+            const int m0 = (tile / n_tiles_n) * GEMM_BM, n0 = (tile % n_tiles_n) * BLOCK_N;
+            if (m0 >= m_end) continue;
+            int w_row0 = 0;
+            if (ep.group_offsets) {                               // grouped GEMM (per-type embedding weights)
+                int g = 1;
+                while (g < ep.n_groups && m0 >= ep.group_offsets[g + 1]) ++g;
+                w_row0 = (g - 1) * N;
             }
-            __syncwarp();
+            for (int kb = 0; kb < num_kb; ++kb, ++kbg) {
+                const uint32_t s = kbg % STAGES;
+                ptx::mbar_wait(bar_empty + 8 * s, ((kbg / STAGES) & 1) ^ 1);
+                if (lane == 0) {
+                    const uint32_t st = smem_base + s * Cfg::STAGE_BYTES;
+                    ptx::mbar_expect_tx(bar_full + 8 * s, Cfg::STAGE_BYTES);
+                    ptx::tma_load_2d(st, &tmA, bar_full + 8 * s, kb * GEMM_BK, m0);
+                    if (SPLIT) ptx::tma_load_2d(st + Cfg::A_BYTES, &tmA_lo, bar_full + 8 * s, kb * GEMM_BK, m0);
+                    ptx::tma_load_2d(st + Cfg::A_BYTES * (SPLIT ? 2 : 1), &tmB, bar_full + 8 * s, kb * GEMM_BK, w_row0 + n0);
+                }
+                __syncwarp();
+            }
         }
     } else if (warp == 1) {
-        // ---------------- MMA issuer
+        // ---------------- MMA issuer (all lanes, warp-uniform operands; one lane elected inside the wrappers)
         constexpr uint32_t idesc = ptx::umma_idesc_bf16(GEMM_BM, BLOCK_N);
-        for (int kb = 0; kb < num_kb; ++kb) {
-            const int s = kb % STAGES;
-            const uint32_t ph = (kb / STAGES) & 1;
-            ptx::mbar_wait(bar_full + 8 * s, ph);
+        uint32_t kbg = 0;
+        int it = 0;
+        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+            if ((tile / n_tiles_n) * GEMM_BM >= m_end) continue;
+            const int buf = it & 1;
+            ptx::mbar_wait(bar_acc_empty + 8 * buf, ((it >> 1) & 1) ^ 1);      // the epilogue drained this buffer
             ptx::tc_fence_after();
-            {   // all lanes, warp-uniform operands: one lane is elected inside the MMA / commit wrappers
+            const uint32_t d_tmem = tmem_base + buf * BLOCK_N;
+            for (int kb = 0; kb < num_kb; ++kb, ++kbg) {
+                const uint32_t s = kbg % STAGES;
+                ptx::mbar_wait(bar_full + 8 * s, (kbg / STAGES) & 1);
+                ptx::tc_fence_after();
                 const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
                 const uint32_t b_addr = a_addr + Cfg::A_BYTES * (SPLIT ? 2 : 1);
 #pragma unroll
                 for (int k = 0; k < GEMM_BK / 16; ++k) {
                     const uint64_t bd = ptx::umma_desc_kmajor(b_addr + k * 32, 128);
-                    ptx::mma_ss(tmem_base, ptx::umma_desc_kmajor(a_addr + k * 32, 128), bd, idesc, (kb | k) != 0);
-                    if (SPLIT) ptx::mma_ss(tmem_base, ptx::umma_desc_kmajor(a_addr + Cfg::A_BYTES + k * 32, 128), bd, idesc, 1);
+                    ptx::mma_ss(d_tmem, ptx::umma_desc_kmajor(a_addr + k * 32, 128), bd, idesc, (kb | k) != 0);
+                    if (SPLIT) ptx::mma_ss(d_tmem, ptx::umma_desc_kmajor(a_addr + Cfg::A_BYTES + k * 32, 128), bd, idesc, 1);
                 }
-                ptx::mma_commit(bar_empty + 8 * s);           // frees the stage when these MMAs retire
-                if (kb == num_kb - 1) ptx::mma_commit(bar_acc);
+                ptx::mma_commit(bar_empty + 8 * s);               // frees the stage when these MMAs retire
             }
+            ptx::mma_commit(bar_acc_full + 8 * buf);
+            ++it;
         }
     } else {
-        // ---------------- epilogue: warp w reads TMEM lanes 32*(w%4) .. +31
-        const int q = warp & 3;
-        const int m = m0 + q * 32 + lane;
-        const bool row_ok = m < M;
-        int row = m;
-        if (row_ok && ep.row_perm) row = ep.row_perm[m];
-        const bool write_ok = row_ok && row >= 0;
-        ptx::mbar_wait(bar_acc, 0);
-        ptx::tc_fence_after();
-#pragma unroll 1
-        for (int c = 0; c < BLOCK_N; c += 32) {
-            uint32_t acc[32];
-            ptx::tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + c, acc);
-            ptx::tmem_ld_wait();
-            gemm_epilogue_chunk(acc, ep, w_row0, row, n0 + c, write_ok);
+        // ---------------- epilogue warpgroup e handles the tiles whose accumulator sits in buffer e
+        const int e = (warp - 2) >> 2;
+        const int q = warp & 3;                                   // TMEM lane quarter this warp may access
+        const int tid = ((warp - 2) & 3) * 32 + lane;             // 0..127 inside the warpgroup
+        int it = 0;
+        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+            const int m0 = (tile / n_tiles_n) * GEMM_BM, n0 = (tile % n_tiles_n) * BLOCK_N;
+            if (m0 >= m_end) continue;
+            if ((it & 1) != e) { ++it; continue; }
+            int w_row0 = 0;
+            if (ep.group_offsets) {
+                int g = 1;
+                while (g < ep.n_groups && m0 >= ep.group_offsets[g + 1]) ++g;
+                w_row0 = (g - 1) * N;
+            }
+            // this tile's bias -> shared memory (read back as broadcast 128-bit loads)
+            asm volatile("bar.sync %0, 128;" ::"r"(1 + e) : "memory");          // everyone is done with the last tile's
+            if (ep.bias)
+                for (int c = tid; c < BLOCK_N; c += 128) bias_s[e][c] = __ldg(ep.bias + w_row0 + n0 + c);
+            asm volatile("bar.sync %0, 128;" ::"r"(1 + e) : "memory");
+            const int m = m0 + q * 32 + lane;
+            const bool row_ok = m < M;
+            int row = m;
+            if (row_ok && ep.row_perm) row = ep.row_perm[m];
+            const bool write_ok = row_ok && row >= 0;
+            ptx::mbar_wait(bar_acc_full + 8 * e, (it >> 1) & 1);
+            ptx::tc_fence_after();
+            const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + e * BLOCK_N;
+            uint32_t ra[32], rb[32];
+            ptx::tmem_ld32(t_addr, ra);
+#pragma unroll
+            for (int c = 0; c < BLOCK_N; c += 64) {               // two chunks per iteration, next load in flight
+                ptx::tmem_ld_wait();
+                if (c + 32 < BLOCK_N) ptx::tmem_ld32(t_addr + c + 32, rb);
+                gemm_epilogue_chunk(ra, ep, ep.bias ? &bias_s[e][c] : nullptr, row, n0 + c, write_ok);
+                if (c + 32 < BLOCK_N) {
+                    ptx::tmem_ld_wait();
+                    if (c + 64 < BLOCK_N) ptx::tmem_ld32(t_addr + c + 64, ra);
+                    gemm_epilogue_chunk(rb, ep, ep.bias ? &bias_s[e][c + 32] : nullptr, row, n0 + c + 32, write_ok);
+                }
+            }
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(bar_acc_empty + 8 * e);
+            ++it;
         }
     }
     ptx::tc_fence_before();
@@ -234,7 +304,8 @@ static int tc_gemm_launch_cfg(TcContext* c, const bf16* A, const bf16* A_lo, con
         if (e != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return -1; }
         attr_set = true;
     }
-    dim3 grid(N / BLOCK_N, (M + GEMM_BM - 1) / GEMM_BM);
+    const int total_tiles = ((M + GEMM_BM - 1) / GEMM_BM) * (N / BLOCK_N);
+    const int grid = total_tiles < c->num_sms ? total_tiles : c->num_sms;
     kern<<<grid, GEMM_THREADS, Cfg::SMEM_BYTES, st>>>(tmA, tmAlo, tmB, M, N, K, ep);
     return 0;
 }
@@ -244,11 +315,11 @@ int tc_gemm_launch(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W,
     if (N % 64 || K % 64) { snprintf(c->err, sizeof c->err, "tc_gemm: N=%d, K=%d must be multiples of 64", N, K); return -1; }
     const int w_rows = ep.group_offsets ? ep.n_groups * N : N;
     if (N % 128 == 0) {
-        return A_lo ? tc_gemm_launch_cfg<128, 2, true>(c, A, A_lo, W, M, N, K, w_rows, ep, st)
-                    : tc_gemm_launch_cfg<128, 3, false>(c, A, nullptr, W, M, N, K, w_rows, ep, st);
+        return A_lo ? tc_gemm_launch_cfg<128, 4, true>(c, A, A_lo, W, M, N, K, w_rows, ep, st)
+                    : tc_gemm_launch_cfg<128, 6, false>(c, A, nullptr, W, M, N, K, w_rows, ep, st);
     }
-    return A_lo ? tc_gemm_launch_cfg<64, 4, true>(c, A, A_lo, W, M, N, K, w_rows, ep, st)
-                : tc_gemm_launch_cfg<64, 4, false>(c, A, nullptr, W, M, N, K, w_rows, ep, st);
+    return A_lo ? tc_gemm_launch_cfg<64, 5, true>(c, A, A_lo, W, M, N, K, w_rows, ep, st)
+                : tc_gemm_launch_cfg<64, 8, false>(c, A, nullptr, W, M, N, K, w_rows, ep, st);
 }
 
 }  // namespace mlpf
