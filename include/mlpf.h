@@ -106,10 +106,16 @@ const char* mlpf_last_error(void);
                                     are then NOT written.  -2: stop after the embedding.                */
 #define MLPF_OPT_KERNELS     4   /* MLPF_KERNELS_TC (default: tcgen05 GEMM + attention) | MLPF_KERNELS_SIMPLE
                                     (CUDA-core kernels in the same precision; debugging aid)            */
-#define MLPF_OPT_SPLIT       5   /* 1 (default): in BF16 mode the activations that feed the residual stream
-                                    (embedding hidden, attention output, LN2 / final-LN output, FFN hidden, head
-                                    hidden) are carried as two bf16 terms hi + lo and multiplied as two MMAs
-                                    (DESIGN.md "error budget").  0: single bf16 term everywhere.          */
+#define MLPF_OPT_SPLIT       5   /* bit mask (default MLPF_SPLIT_ALL): which bf16 activations of the BF16 path are carried
+                                    as two bf16 terms hi + lo and multiplied as two MMAs into one fp32 accumulator
+                                    (DESIGN.md "error budget").  0: single bf16 term everywhere.             */
+#define MLPF_SPLIT_EMB   1       /* embedding hidden layer (input of the embedding's second linear)          */
+#define MLPF_SPLIT_O     2       /* attention output (input of the out-projection)                           */
+#define MLPF_SPLIT_U2    4       /* LN2 output (input of FFN1)                                               */
+#define MLPF_SPLIT_G     8       /* FFN hidden layer (input of FFN2)                                         */
+#define MLPF_SPLIT_UF    16      /* final-LN output (input of the heads' first layers)                       */
+#define MLPF_SPLIT_HEAD  32      /* heads' hidden layers (input of the fp32 output rows)                     */
+#define MLPF_SPLIT_ALL   63
 #define MLPF_OPT_PROFILE     6   /* 1: record a CUDA event pair around every kernel class inside mlpf_infer
                                     (read back with mlpf_debug_get_profile); 0 (default): off            */
 #define MLPF_PREC_BF16        0

@@ -76,7 +76,7 @@ struct mlpf_handle {
     std::vector<LayerW> layers;
     HeadsOut ho;
     // options
-    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = 1, profile = 0;
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0;
     int64_t last_launches = 0;
     std::mutex mu;
     std::map<void*, Workspace*> ws;
@@ -227,7 +227,7 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
             if (value < -2 || value >= h->L) return set_err(MLPF_E_ARG, "bad tap layer");
             h->tap_layer = (int)value; return MLPF_OK;
         case MLPF_OPT_SPLIT:
-            if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "split must be 0 or 1");
+            if (value < 0 || value > MLPF_SPLIT_ALL) return set_err(MLPF_E_ARG, "split must be a mask in 0..63");
             h->split = (int)value; return MLPF_OK;
         case MLPF_OPT_PROFILE:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "profile must be 0 or 1");
@@ -410,9 +410,10 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     const char* PWb = fp32 ? (const char*)h->P32 : (const char*)h->P16;
     auto PW = [&](int64_t off) { return (const void*)(PWb + off * es); };
     const float* PV = h->P32;
-    const bool split = !fp32 && h->split != 0;     // bf16 activations carried as hi + lo where they feed the residual stream
+    // bf16 activations carried as hi + lo where they feed the residual stream (mask MLPF_OPT_SPLIT)
+    const int sm = fp32 ? 0 : h->split;
     void* u = w->u; void* g = w->g;
-    void* u_lo = split ? w->u_lo : nullptr; void* g_lo = split ? w->g_lo : nullptr; void* o_lo = split ? w->o_lo : nullptr;
+    auto lo = [&](int bit, void* p) { return (sm & bit) ? p : (void*)nullptr; };
 
     // ---- a0 (device half)
     w->prof_cls.clear();
@@ -428,7 +429,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     // ---- a1: per-type embedding (L156; A3-A5)
     {
     ProfScope ps(h, w, st, MLPF_KC_EMBED_L1);
-    launch_embed_l1(fp32, X, N, h->F, d, PV + h->embW1t, PV + h->embB1, h->act, w->sorted_row, g, g_lo, w->h, st);
+    launch_embed_l1(fp32, X, N, h->F, d, PV + h->embW1t, PV + h->embB1, h->act, w->sorted_row, g, lo(MLPF_SPLIT_EMB, w->g_lo), w->h, st);
     LAUNCH_CHECK(h);
     }
     {
@@ -436,7 +437,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         Epi ep;
         ep.bias = PV + h->embB2; ep.out_f32 = w->h; ep.ld_f32 = d;
         ep.row_perm = w->type_perm; ep.group_offsets = w->type_offsets; ep.n_groups = 4;
-        int rc = run_gemm(h, fp32, tc, g, g_lo, PW(h->embW2), (int)w->m_ub, d, d, ep, st);
+        int rc = run_gemm(h, fp32, tc, g, lo(MLPF_SPLIT_EMB, w->g_lo), PW(h->embW2), (int)w->m_ub, d, d, ep, st);
         if (rc) return rc;
     }
     if (h->tap_layer == -2) return MLPF_OK;
@@ -459,33 +460,33 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         }
         {
             ProfScope ps(h, w, st, MLPF_KC_ATTENTION);
-            rc = run_attention(h, fp32, tc_attn, split, w, st);                                                     // a4
+            rc = run_attention(h, fp32, tc_attn, (sm & MLPF_SPLIT_O) != 0, w, st);                                                     // a4
         }
         if (rc) return rc;
         {   // a5: h <- h + O Wo^T + bo
             ProfScope ps(h, w, st, MLPF_KC_OUTPROJ);
             Epi ep;
             ep.bias = PV + lw.bo; ep.residual = w->h; ep.ld_res = d; ep.out_f32 = w->h; ep.ld_f32 = d;
-            rc = run_gemm(h, fp32, tc, w->o, o_lo, PW(lw.Wo), N, d, d, ep, st);
+            rc = run_gemm(h, fp32, tc, w->o, lo(MLPF_SPLIT_O, w->o_lo), PW(lw.Wo), N, d, d, ep, st);
             if (rc) return rc;
         }
         {
             ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);
-            rc = run_layernorm(h, fp32, w->h, N, PV + lw.ln2g, PV + lw.ln2b, u, u_lo, st);
+            rc = run_layernorm(h, fp32, w->h, N, PV + lw.ln2g, PV + lw.ln2b, u, lo(MLPF_SPLIT_U2, w->u_lo), st);
         }
         if (rc) return rc;
         {   // a6: g = act(LN2(h) W1^T + b1)
             ProfScope ps(h, w, st, MLPF_KC_FFN1);
             Epi ep;
-            ep.bias = PV + lw.b1; ep.act = h->act; ep.out_act = g; ep.out_act_lo = g_lo; ep.ld_act = dff;
-            rc = run_gemm(h, fp32, tc, u, u_lo, PW(lw.W1), N, dff, d, ep, st);
+            ep.bias = PV + lw.b1; ep.act = h->act; ep.out_act = g; ep.out_act_lo = lo(MLPF_SPLIT_G, w->g_lo); ep.ld_act = dff;
+            rc = run_gemm(h, fp32, tc, u, lo(MLPF_SPLIT_U2, w->u_lo), PW(lw.W1), N, dff, d, ep, st);
             if (rc) return rc;
         }
         {   // a7: h <- h + g W2^T + b2
             ProfScope ps(h, w, st, MLPF_KC_FFN2);
             Epi ep;
             ep.bias = PV + lw.b2; ep.residual = w->h; ep.ld_res = d; ep.out_f32 = w->h; ep.ld_f32 = d;
-            rc = run_gemm(h, fp32, tc, g, g_lo, PW(lw.W2), N, d, dff, ep, st);
+            rc = run_gemm(h, fp32, tc, g, lo(MLPF_SPLIT_G, w->g_lo), PW(lw.W2), N, d, dff, ep, st);
             if (rc) return rc;
         }
         w->g_width = dff;
@@ -495,7 +496,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     // ---- a8: heads (L156; A11-A12)
     if (h->hp.final_ln) {
         ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);
-        int rc = run_layernorm(h, fp32, w->h, N, PV + h->lnfg, PV + h->lnfb, u, u_lo, st);
+        int rc = run_layernorm(h, fp32, w->h, N, PV + h->lnfg, PV + h->lnfb, u, lo(MLPF_SPLIT_UF, w->u_lo), st);
         if (rc) return rc;
     } else {
         // no final LN: u = T(h).  (identity affine with the row kept: done by a cast kernel)
@@ -504,16 +505,16 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     {
         Epi ep;
         const int hw = h->n_hblk * d;
-        ep.bias = PV + h->headB1; ep.act = h->act; ep.out_act = g; ep.out_act_lo = g_lo; ep.ld_act = hw;
+        ep.bias = PV + h->headB1; ep.act = h->act; ep.out_act = g; ep.out_act_lo = lo(MLPF_SPLIT_HEAD, w->g_lo); ep.ld_act = hw;
         int rc;
         {
             ProfScope ps(h, w, st, MLPF_KC_HEADS_L1);
-            rc = run_gemm(h, fp32, tc, u, u_lo, PW(h->headW1), N, hw, d, ep, st);
+            rc = run_gemm(h, fp32, tc, u, lo(MLPF_SPLIT_UF, w->u_lo), PW(h->headW1), N, hw, d, ep, st);
         }
         if (rc) return rc;
         w->g_width = hw;
         ProfScope ps(h, w, st, MLPF_KC_HEADS_L2);
-        launch_heads_l2(fp32, g, g_lo, N, d, hw, PV + h->headW2, PV + h->headB2, w->valid, h->ho, out_logits, out_regress, st);
+        launch_heads_l2(fp32, g, lo(MLPF_SPLIT_HEAD, w->g_lo), N, d, hw, PV + h->headW2, PV + h->headB2, w->valid, h->ho, out_logits, out_regress, st);
         LAUNCH_CHECK(h);
     }
     return MLPF_OK;

@@ -61,7 +61,7 @@ int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, 
 
 // ------------------------------------------------------------------------------------------------ kernel
 constexpr int GEMM_BM = 128, GEMM_BK = 64;
-constexpr int GEMM_THREADS = 320;                              // TMA, MMA, 2 x 4 epilogue warps
+constexpr int GEMM_THREADS = 576;                              // TMA, MMA, 4 x 4 epilogue warps
 
 template <int BLOCK_N, int STAGES, bool SPLIT>
 struct GemmCfg {
@@ -72,78 +72,83 @@ struct GemmCfg {
     static constexpr int TMEM_COLS = 2 * BLOCK_N < 32 ? 32 : 2 * BLOCK_N;   // two accumulator buffers (power of 2)
 };
 
-// exact-erf GELU (reading A6) with erf from Abramowitz & Stegun 7.1.26 (|error| <= 1.5e-7): 2 MUFU + ~12 FMA-pipe
-// instructions instead of erff's ~40 (the activation epilogues are issue-bound).  For x < 0 the form
-// 0.5 x (1 - erf|x|) = 0.5 x p e avoids the cancellation in 1 + erf(x).
-__device__ __forceinline__ float gelu_fast(float x) {
-    const float ax = fabsf(x) * 0.70710678118654752440f;
-    float t;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t) : "f"(fmaf(0.3275911f, ax, 1.0f)));
-    float p = fmaf(t, 1.061405429f, -1.453152027f);
-    p = fmaf(p, t, 1.421413741f);
-    p = fmaf(p, t, -0.284496736f);
-    p = fmaf(p, t, 0.254829592f);
-    p *= t;
-    const float e = ptx::fast_exp2(ax * ax * -1.4426950408889634f);
-    const float h = 0.5f * x * p * e;                  // 0.5 x (1 - erf|x|)
-    return x >= 0.0f ? x - h : h;
-}
-__device__ __forceinline__ float act_fast(float x, int act) {
-    if (act == ACT_RELU) return fmaxf(x, 0.0f);
-    if (act == ACT_GELU) return gelu_fast(x);
-    return x;
+// exact-erf GELU (reading A6) on two values, erf from Abramowitz & Stegun 7.1.26 (|error| <= 1.5e-7):
+//   GELU(x) = max(x, 0) - 0.5 |x| p(t) e^{-x^2/2},  t = 1 / (1 + 0.3275911 |x| / sqrt 2)
+// (for x < 0 this is 0.5 x (1 - erf|x/sqrt 2|) with no cancellation).  4 MUFU + ~18 FMA-pipe issue slots per
+// PAIR (packed FFMA2 / FMUL2) instead of erff's ~40 per value: the activation epilogues are issue-bound.
+__device__ __forceinline__ float2 gelu2(float2 x) {
+    float2 t;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t.x) : "f"(fmaf(fabsf(x.x), 0.23164189f, 1.0f)));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t.y) : "f"(fmaf(fabsf(x.y), 0.23164189f, 1.0f)));
+    float2 p = ptx::ffma2(t, make_float2(1.061405429f, 1.061405429f), make_float2(-1.453152027f, -1.453152027f));
+    p = ptx::ffma2(p, t, make_float2(1.421413741f, 1.421413741f));
+    p = ptx::ffma2(p, t, make_float2(-0.284496736f, -0.284496736f));
+    p = ptx::ffma2(p, t, make_float2(0.254829592f, 0.254829592f));
+    p = ptx::fmul2(p, t);
+    const float2 xx = ptx::fmul2(ptx::fmul2(x, x), make_float2(-0.72134752044448170f, -0.72134752044448170f));  // -x^2/2 log2 e
+    const float2 e = make_float2(ptx::fast_exp2(xx.x), ptx::fast_exp2(xx.y));
+    const float2 a = make_float2(fabsf(x.x) * -0.5f, fabsf(x.y) * -0.5f);
+    const float2 h = ptx::fmul2(ptx::fmul2(p, e), a);                     // -0.5 |x| p e
+    return ptx::fadd2(make_float2(fmaxf(x.x, 0.0f), fmaxf(x.y, 0.0f)), h);
 }
 
-// epilogue of one 32-column chunk held in registers (thread = one row); bias_s = this tile's bias in shared memory
-__device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[32], const Epi& ep, const float* bias_s, int row,
+// epilogue of one 16-column chunk held in registers (thread = one row); bias_s = this chunk's bias in shared memory
+template <int ACT>
+__device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[16], const Epi& ep, const float* bias_s, int row,
                                                     int n_base, bool row_ok) {
-    float v[32];
+    float2 v[8];
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
+    for (int j = 0; j < 4; ++j) {
         float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
         if (bias_s) b = *reinterpret_cast<const float4*>(bias_s + 4 * j);       // broadcast LDS.128
-        v[4 * j] = act_fast(__uint_as_float(acc[4 * j]) + b.x, ep.act);
-        v[4 * j + 1] = act_fast(__uint_as_float(acc[4 * j + 1]) + b.y, ep.act);
-        v[4 * j + 2] = act_fast(__uint_as_float(acc[4 * j + 2]) + b.z, ep.act);
-        v[4 * j + 3] = act_fast(__uint_as_float(acc[4 * j + 3]) + b.w, ep.act);
+        v[2 * j] = ptx::fadd2(make_float2(__uint_as_float(acc[4 * j]), __uint_as_float(acc[4 * j + 1])), make_float2(b.x, b.y));
+        v[2 * j + 1] = ptx::fadd2(make_float2(__uint_as_float(acc[4 * j + 2]), __uint_as_float(acc[4 * j + 3])), make_float2(b.z, b.w));
+    }
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        if (ACT == ACT_GELU) v[j] = gelu2(v[j]);
+        if (ACT == ACT_RELU) v[j] = make_float2(fmaxf(v[j].x, 0.0f), fmaxf(v[j].y, 0.0f));
     }
     if (!row_ok) return;
     if (ep.residual) {
         const float4* rp = reinterpret_cast<const float4*>(ep.residual + (int64_t)row * ep.ld_res + n_base);
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            float4 r = rp[j];
-            v[4 * j] += r.x; v[4 * j + 1] += r.y; v[4 * j + 2] += r.z; v[4 * j + 3] += r.w;
+        for (int j = 0; j < 4; ++j) {
+            const float4 r = rp[j];
+            v[2 * j] = ptx::fadd2(v[2 * j], make_float2(r.x, r.y));
+            v[2 * j + 1] = ptx::fadd2(v[2 * j + 1], make_float2(r.z, r.w));
         }
     }
     if (ep.out_f32) {
         float4* op = reinterpret_cast<float4*>(ep.out_f32 + (int64_t)row * ep.ld_f32 + n_base);
 #pragma unroll
-        for (int j = 0; j < 8; ++j) op[j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+        for (int j = 0; j < 4; ++j) op[j] = make_float4(v[2 * j].x, v[2 * j].y, v[2 * j + 1].x, v[2 * j + 1].y);
     }
     if (ep.out_act) {
-        uint32_t hi[16], lo[16];
+        uint32_t hi[8], lo[8];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-            __nv_bfloat162 h2 = __floats2bfloat162_rn(v[2 * j], v[2 * j + 1]);
+        for (int j = 0; j < 8; ++j) {
+            __nv_bfloat162 h2 = __floats2bfloat162_rn(v[j].x, v[j].y);
             hi[j] = *reinterpret_cast<uint32_t*>(&h2);
             if (ep.out_act_lo) {
-                __nv_bfloat162 l2 = __floats2bfloat162_rn(v[2 * j] - __low2float(h2), v[2 * j + 1] - __high2float(h2));
+                // bf16 -> fp32 is a 16-bit shift: v - hi as two integer ops + one packed subtract
+                const float2 d = ptx::fadd2(v[j], make_float2(-__uint_as_float(hi[j] << 16), -__uint_as_float(hi[j] & 0xffff0000u)));
+                __nv_bfloat162 l2 = __floats2bfloat162_rn(d.x, d.y);
                 lo[j] = *reinterpret_cast<uint32_t*>(&l2);
             }
         }
         uint4* op = reinterpret_cast<uint4*>((bf16*)ep.out_act + (int64_t)row * ep.ld_act + n_base);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) op[j] = make_uint4(hi[4 * j], hi[4 * j + 1], hi[4 * j + 2], hi[4 * j + 3]);
+        for (int j = 0; j < 2; ++j) op[j] = make_uint4(hi[4 * j], hi[4 * j + 1], hi[4 * j + 2], hi[4 * j + 3]);
         if (ep.out_act_lo) {
             uint4* lp = reinterpret_cast<uint4*>((bf16*)ep.out_act_lo + (int64_t)row * ep.ld_act + n_base);
 #pragma unroll
-            for (int j = 0; j < 4; ++j) lp[j] = make_uint4(lo[4 * j], lo[4 * j + 1], lo[4 * j + 2], lo[4 * j + 3]);
+            for (int j = 0; j < 2; ++j) lp[j] = make_uint4(lo[4 * j], lo[4 * j + 1], lo[4 * j + 2], lo[4 * j + 3]);
         }
     }
 }
 
-template <int BLOCK_N, int STAGES, bool SPLIT>
+template <int BLOCK_N, int STAGES, bool SPLIT, int ACT>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmA_lo,
           const __grid_constant__ CUtensorMap tmB, int M, int N, int K, Epi ep) {
@@ -165,7 +170,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < STAGES; ++s) { ptx::mbar_init(bar_full + 8 * s, 1); ptx::mbar_init(bar_empty + 8 * s, 1); }
-        for (int b = 0; b < 2; ++b) { ptx::mbar_init(bar_acc_full + 8 * b, 1); ptx::mbar_init(bar_acc_empty + 8 * b, 4); }
+        for (int b = 0; b < 2; ++b) { ptx::mbar_init(bar_acc_full + 8 * b, 1); ptx::mbar_init(bar_acc_empty + 8 * b, 8); }
         ptx::fence_barrier_init();
         ptx::tma_prefetch_desc(&tmA);
         ptx::tma_prefetch_desc(&tmB);
@@ -235,10 +240,13 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             ++it;
         }
     } else {
-        // ---------------- epilogue warpgroup e handles the tiles whose accumulator sits in buffer e
-        const int e = (warp - 2) >> 2;
+        // ---------------- epilogue: 4 warpgroups = (accumulator buffer e) x (column half): 4 warps per SM
+        // sub-partition keep the issue-bound activation epilogues busy
+        const int ew = warp - 2;
+        const int e = (ew >> 2) & 1;
+        const int hcol = (ew >> 3) * (BLOCK_N / 2);
         const int q = warp & 3;                                   // TMEM lane quarter this warp may access
-        const int tid = ((warp - 2) & 3) * 32 + lane;             // 0..127 inside the warpgroup
+        const int tid = ((ew >> 3) * 4 + (ew & 3)) * 32 + lane;   // 0..255 among the threads serving buffer e
         int it = 0;
         for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
             const int m0 = (tile / n_tiles_n) * GEMM_BM, n0 = (tile % n_tiles_n) * BLOCK_N;
@@ -251,10 +259,10 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 w_row0 = (g - 1) * N;
             }
             // this tile's bias -> shared memory (read back as broadcast 128-bit loads)
-            asm volatile("bar.sync %0, 128;" ::"r"(1 + e) : "memory");          // everyone is done with the last tile's
+            asm volatile("bar.sync %0, 256;" ::"r"(1 + e) : "memory");          // everyone is done with the last tile's
             if (ep.bias)
-                for (int c = tid; c < BLOCK_N; c += 128) bias_s[e][c] = __ldg(ep.bias + w_row0 + n0 + c);
-            asm volatile("bar.sync %0, 128;" ::"r"(1 + e) : "memory");
+                for (int c = tid; c < BLOCK_N; c += 256) bias_s[e][c] = __ldg(ep.bias + w_row0 + n0 + c);
+            asm volatile("bar.sync %0, 256;" ::"r"(1 + e) : "memory");
             const int m = m0 + q * 32 + lane;
             const bool row_ok = m < M;
             int row = m;
@@ -262,19 +270,17 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             const bool write_ok = row_ok && row >= 0;
             ptx::mbar_wait(bar_acc_full + 8 * e, (it >> 1) & 1);
             ptx::tc_fence_after();
-            const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + e * BLOCK_N;
-            uint32_t ra[32], rb[32];
-            ptx::tmem_ld32(t_addr, ra);
+            const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + e * BLOCK_N + hcol;
+            uint32_t ra[16], rb[16];
+            ptx::tmem_ld16(t_addr, ra);
 #pragma unroll
-            for (int c = 0; c < BLOCK_N; c += 64) {               // two chunks per iteration, next load in flight
+            for (int c = 0; c < BLOCK_N / 2; c += 32) {           // two 16-column chunks per iteration, next load in flight
                 ptx::tmem_ld_wait();
-                if (c + 32 < BLOCK_N) ptx::tmem_ld32(t_addr + c + 32, rb);
-                gemm_epilogue_chunk(ra, ep, ep.bias ? &bias_s[e][c] : nullptr, row, n0 + c, write_ok);
-                if (c + 32 < BLOCK_N) {
-                    ptx::tmem_ld_wait();
-                    if (c + 64 < BLOCK_N) ptx::tmem_ld32(t_addr + c + 64, ra);
-                    gemm_epilogue_chunk(rb, ep, ep.bias ? &bias_s[e][c + 32] : nullptr, row, n0 + c + 32, write_ok);
-                }
+                ptx::tmem_ld16(t_addr + c + 16, rb);
+                gemm_epilogue_chunk<ACT>(ra, ep, ep.bias ? &bias_s[e][hcol + c] : nullptr, row, n0 + hcol + c, write_ok);
+                ptx::tmem_ld_wait();
+                if (c + 32 < BLOCK_N / 2) ptx::tmem_ld16(t_addr + c + 32, ra);
+                gemm_epilogue_chunk<ACT>(rb, ep, ep.bias ? &bias_s[e][hcol + c + 16] : nullptr, row, n0 + hcol + c + 16, write_ok);
             }
             ptx::tc_fence_before();
             __syncwarp();
@@ -288,8 +294,8 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 }
 
 // ------------------------------------------------------------------------------------------------ launch
-template <int BLOCK_N, int STAGES, bool SPLIT>
-static int tc_gemm_launch_cfg(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W, int M, int N, int K,
+template <int BLOCK_N, int STAGES, bool SPLIT, int ACT>
+static int tc_gemm_launch_act(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W, int M, int N, int K,
                               int w_rows, const Epi& ep, cudaStream_t st) {
     using Cfg = GemmCfg<BLOCK_N, STAGES, SPLIT>;
     CUtensorMap tmA, tmAlo, tmB;
@@ -297,7 +303,7 @@ static int tc_gemm_launch_cfg(TcContext* c, const bf16* A, const bf16* A_lo, con
     if (SPLIT) { if (tc_tensor_map(c, &tmAlo, A_lo, K, M, K, GEMM_BK, GEMM_BM)) return -1; }
     else tmAlo = tmA;
     if (tc_tensor_map(c, &tmB, W, K, w_rows, K, GEMM_BK, BLOCK_N)) return -1;
-    auto kern = k_tc_gemm<BLOCK_N, STAGES, SPLIT>;
+    auto kern = k_tc_gemm<BLOCK_N, STAGES, SPLIT, ACT>;
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
@@ -308,6 +314,16 @@ static int tc_gemm_launch_cfg(TcContext* c, const bf16* A, const bf16* A_lo, con
     const int grid = total_tiles < c->num_sms ? total_tiles : c->num_sms;
     kern<<<grid, GEMM_THREADS, Cfg::SMEM_BYTES, st>>>(tmA, tmAlo, tmB, M, N, K, ep);
     return 0;
+}
+
+template <int BLOCK_N, int STAGES, bool SPLIT>
+static int tc_gemm_launch_cfg(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W, int M, int N, int K,
+                              int w_rows, const Epi& ep, cudaStream_t st) {
+    switch (ep.act) {                                 // the activation is compiled into the epilogue
+        case ACT_GELU: return tc_gemm_launch_act<BLOCK_N, STAGES, SPLIT, ACT_GELU>(c, A, A_lo, W, M, N, K, w_rows, ep, st);
+        case ACT_RELU: return tc_gemm_launch_act<BLOCK_N, STAGES, SPLIT, ACT_RELU>(c, A, A_lo, W, M, N, K, w_rows, ep, st);
+    }
+    return tc_gemm_launch_act<BLOCK_N, STAGES, SPLIT, ACT_NONE>(c, A, A_lo, W, M, N, K, w_rows, ep, st);
 }
 
 int tc_gemm_launch(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W, int M, int N, int K,
