@@ -48,6 +48,9 @@ struct AttnParams {
     int n_pairs, H, d;
     bf16* O; bf16* O_lo;
     float scale_log2;          // log2(e) / sqrt(hd)
+#ifdef MLPF_ATT_LOG
+    long long* prof;           // build with MLPF_NVCC_FLAGS=-DMLPF_ATT_LOG: per-warp clock64 timeline of CTA 200
+#endif
 };
 
 // 32 scores of one row (registers r[0..31]) -> running max
@@ -84,7 +87,7 @@ __device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c,
 // Returns corr = 2^((m_old - m_new) c) and the row sum of P in rsum.
 template <bool FULL>
 __device__ __forceinline__ float softmax_tile(const uint32_t (&s)[64], uint32_t s_addr, const uint32_t (&mask)[2], float c,
-                                              float& m_run, float& rsum) {
+                                              float& m_run, float& rsum, uint32_t mid_bar = 0) {
     float mx = max32<FULL>(&s[0], mask[0], -INFINITY);
     mx = max32<FULL>(&s[32], mask[1], mx);
     const float m_new = fmaxf(m_run, mx);
@@ -98,6 +101,10 @@ __device__ __forceinline__ float softmax_tile(const uint32_t (&s)[64], uint32_t 
         uint32_t pk[16];
         exp32<FULL>(&s[32 * w], mask[w], c, neg_mc, pk, rs);
         ptx::tmem_st16(s_addr + 16 * w, pk);
+        if (w == 0 && mid_bar) {                                 // half-way through this tile (see bar_stagger)
+            __syncwarp();
+            if ((threadIdx.x & 31) == 0) ptx::mbar_arrive(mid_bar);
+        }
     }
     rsum = (rs[0].x + rs[0].y) + (rs[1].x + rs[1].y);
     return corr;
@@ -109,8 +116,15 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     using Cfg = AttnCfg<HD>;
     constexpr int ST = Cfg::STAGES;
     extern __shared__ uint8_t smem_raw[];
-    __shared__ uint64_t bars[1 + 2 * ST + 10];
+    __shared__ uint64_t bars[1 + 2 * ST + 11];
     __shared__ uint32_t tmem_base_slot;
+#ifdef MLPF_ATT_LOG
+    __shared__ long long tlog[4][32][6];
+    const bool logging = prm.prof && blockIdx.x == 200;
+#define TLOG(r, j, k) do { if (logging && (j) < 32 && (threadIdx.x & 31) == 0) tlog[r][j][k] = clock64(); } while (0)
+#else
+#define TLOG(r, j, k) do {} while (0)
+#endif
 
     const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
     const int item = blockIdx.x / prm.H, head = blockIdx.x % prm.H;
@@ -131,6 +145,9 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     const uint32_t bar_s = ptx::smem_u32(&bars[1 + 2 * ST]);        // [2t + b]: S_t(j) landed in buffer b = j & 1
     const uint32_t bar_p = ptx::smem_u32(&bars[1 + 2 * ST + 4]);    // [2t + b]: P_t(j) written over buffer b
     const uint32_t bar_o = ptx::smem_u32(&bars[1 + 2 * ST + 8]);    // [t]: O_t(j) complete
+    // tile b's softmax starts half a tile period after tile a's, so that one tile's exponentials (MUFU) overlap the
+    // other's max pass, TMEM traffic and barrier latencies instead of both contending for the same unit in lockstep
+    const uint32_t bar_stagger = ptx::smem_u32(&bars[1 + 2 * ST + 10]);
 
     if (warp == ATT_WARP_TMA && lane == 0) {
         ptx::mbar_init(bar_q, 1);
@@ -144,6 +161,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
         }
         ptx::mbar_init(bar_o, 1);
         ptx::mbar_init(bar_o + 8, 1);
+        ptx::mbar_init(bar_stagger, 4);
         ptx::fence_barrier_init();
         ptx::tma_prefetch_desc(&tmQKV);
     }
@@ -208,16 +226,21 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
             issue_s(0);                             // all lanes: one is elected inside the MMA / commit wrappers
             if (nkv > 1) issue_s(1);
             for (int j = 0; j < nkv; ++j) {
+                TLOG(2 + t, j, 0);
                 ptx::mbar_wait(bar_p + 8 * (2 * t + (j & 1)), (j >> 1) & 1);     // P_t(j) is in TMEM
                 ptx::tc_fence_after();
+                TLOG(2 + t, j, 1);
                 issue_o(j);
                 // K and V of stage j >> 1 are no longer needed by this tile after its second half
                 if ((j & 1) || j == nkv - 1) ptx::mma_commit(bar_kv_empty + 8 * ((j >> 1) % ST));
+                TLOG(2 + t, j, 2);
                 if (j + 2 < nkv) {                   // S_t(j+2) reuses S buffer j & 1: in order after P_t(j) V_j
                     const int i2 = (j + 2) >> 1;
                     if (((j + 2) & 1) == 0) ptx::mbar_wait(bar_kv_full + 8 * (i2 % ST), (i2 / ST) & 1);
                     ptx::tc_fence_after();
+                    TLOG(2 + t, j, 3);
                     issue_s(j + 2);
+                    TLOG(2 + t, j, 4);
                 }
             }
         }
@@ -263,6 +286,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                 ptx::tmem_ld32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
                 ptx::tmem_ld32(s_addr + 32, *reinterpret_cast<uint32_t(*)[32]>(&s[32]));
             };
+            if (t == 1) ptx::mbar_wait(bar_stagger, 0);
             load_s(0);
             ptx::tmem_ld_wait();
             for (int j = 0; j < nkv; ++j) {
@@ -283,24 +307,31 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                     mask[0] = mask[1] = 0xffffffffu;
                 }
                 const uint32_t s_addr = lane_addr + (2 * t + (j & 1)) * 64;
+                if (q == 0) TLOG(t, j, 0);
                 float rsum;
-                const float corr = full ? softmax_tile<true>(s, s_addr, mask, c, m_run, rsum)
-                                        : softmax_tile<false>(s, s_addr, mask, c, m_run, rsum);
+                const uint32_t mid = (t == 0 && j == 0 && has_b) ? bar_stagger : 0u;
+                const float corr = full ? softmax_tile<true>(s, s_addr, mask, c, m_run, rsum, mid)
+                                        : softmax_tile<false>(s, s_addr, mask, c, m_run, rsum, mid);
                 // O_t(j-1) was issued about a softmax period ago: this wait does not stall, but it must come BEFORE
                 // P_t(j) is published -- afterwards O_t(j) could complete too and the barrier would be two phases
                 // ahead of this waiter (parity aliasing)
+                if (q == 0) TLOG(t, j, 1);
                 if (j > 0) {
                     ptx::mbar_wait(bar_o + 8 * t, (j - 1) & 1);
                     ptx::tc_fence_after();
                     fold_load(j - 1);
                 }
-                if (j + 1 < nkv) load_s(j + 1);         // S_t(j+1) is double-buffered: usually long complete
+                if (q == 0) TLOG(t, j, 2);
+                if (j + 1 < nkv) load_s(j + 1);
+                if (q == 0) TLOG(t, j, 3);         // S_t(j+1) is double-buffered: usually long complete
                 ptx::tmem_st_wait();                      // the loads above fly while the P stores drain
                 ptx::tc_fence_before();
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(bar_p + 8 * (2 * t + (j & 1)));      // P_t(j) is in TMEM
+                if (q == 0) TLOG(t, j, 4);
                 ptx::tmem_ld_wait();
                 if (j > 0) fold(corr_prev, rsum_prev);
+                if (q == 0) TLOG(t, j, 5);
                 corr_prev = corr;
                 rsum_prev = rsum;
             }
@@ -335,6 +366,9 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == ATT_WARP_MMA) ptx::tmem_dealloc(tmem_base, 512);
+#ifdef MLPF_ATT_LOG
+    if (logging) for (int i = threadIdx.x; i < 4 * 32 * 6; i += ATT_THREADS) prm.prof[i] = (&tlog[0][0][0])[i];
+#endif
 }
 
 template <int HD>
@@ -351,6 +385,14 @@ static int tc_attn_launch_hd(TcContext* c, const bf16* QKV, int64_t N, const Att
         attr_set = true;
     }
     kern<<<prm.n_pairs * prm.H, ATT_THREADS, Cfg::SMEM_BYTES, st>>>(tmQKV, prm);
+#ifdef MLPF_ATT_LOG
+    {   // rows 0,1: softmax warp 0 of tile a / b; rows 2,3: MMA issuers; one line per key tile
+        long long h[768];
+        cudaMemcpy(h, prm.prof, sizeof h, cudaMemcpyDeviceToHost);
+        FILE* f = fopen("gpurun_out/att_log.txt", "w");
+        if (f) { for (int r = 0; r < 4; ++r) for (int j = 0; j < 32; ++j) { fprintf(f, "%d %d", r, j); for (int k = 0; k < 6; ++k) fprintf(f, " %lld", h[(r * 32 + j) * 6 + k]); fprintf(f, "\n"); } fclose(f); }
+    }
+#endif
     return 0;
 }
 
@@ -362,6 +404,12 @@ int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const int* key_vali
     prm.key_valid = key_valid; prm.n_valid = n_valid; prm.offsets = offsets; prm.pairs = pairs; prm.n_pairs = n_pairs; prm.H = H; prm.d = d;
     prm.O = O; prm.O_lo = O_lo;
     prm.scale_log2 = 1.4426950408889634f / sqrtf((float)hd);
+#ifdef MLPF_ATT_LOG
+    static long long* pbuf = nullptr;
+    if (!pbuf) cudaMalloc(&pbuf, 768 * 8);
+    cudaMemsetAsync(pbuf, 0, 768 * 8, st);
+    prm.prof = pbuf;
+#endif
     switch (hd) {
         case 16: return tc_attn_launch_hd<16>(c, QKV, N, prm, st);
         case 32: return tc_attn_launch_hd<32>(c, QKV, N, prm, st);
