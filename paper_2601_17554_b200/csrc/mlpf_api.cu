@@ -388,7 +388,7 @@ static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspa
 
 // host half of a0: the attention work list (event, q_tile), longest event first, ties by event id, then
 // q_tile ascending; `pairs` = the same order with two consecutive q-tiles of one event per entry.
-static void build_work_lists(const int32_t* off, int E, int tile_q, std::vector<int>& work, std::vector<int>& pairs) {
+static void build_work_lists(const int32_t* off, int E, int tile_q, int rows_per_item, std::vector<int>& work, std::vector<int>& pairs) {
     std::vector<int> order(E);
     for (int e = 0; e < E; ++e) order[e] = e;
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return (off[a + 1] - off[a]) > (off[b + 1] - off[b]); });
@@ -397,7 +397,7 @@ static void build_work_lists(const int32_t* off, int E, int tile_q, std::vector<
         int n = off[e + 1] - off[e];
         int nt = (n + tile_q - 1) / tile_q;
         for (int q = 0; q < nt; ++q) { work.push_back(e); work.push_back(q); }
-        int np128 = (n + 255) / 256;
+        int np128 = (n + rows_per_item - 1) / rows_per_item;
         for (int p = 0; p < np128; ++p) { pairs.push_back(e); pairs.push_back(p); }
     }
 }
@@ -540,7 +540,7 @@ extern "C" int mlpf_infer(mlpf_handle* h, const float* elements, const int32_t* 
     if (!wref) wref = new Workspace();
     Workspace* w = wref;
     std::vector<int> work, pairs;
-    build_work_lists(event_offsets, n_events, h->tile_q, work, pairs);
+    build_work_lists(event_offsets, n_events, h->tile_q, tc_attn_rows_per_cta(h->hd), work, pairs);
     int rc = ws_ensure(h, w, N, n_events, (int64_t)work.size() / 2, fp32);
     if (rc) return rc;
     w->N = N; w->E = n_events; w->n_tiles = (int64_t)work.size() / 2; w->n_pairs = (int64_t)pairs.size() / 2;
@@ -698,7 +698,7 @@ extern "C" int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_va
     std::call_once(once, [&] { init_rc = tc_init(&ctx); });
     if (init_rc) return set_err(MLPF_E_CUDA, "tcgen05/TMA initialisation failed: %s", ctx.err);
     std::vector<int> work, pairs;
-    build_work_lists(event_offsets, n_events, 128, work, pairs);
+    build_work_lists(event_offsets, n_events, 128, tc_attn_rows_per_cta(hd), work, pairs);
     const int64_t N = event_offsets[n_events];
     if (pairs.empty()) return MLPF_OK;
     cudaStream_t st = (cudaStream_t)stream;

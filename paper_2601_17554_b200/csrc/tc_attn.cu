@@ -4,48 +4,56 @@
 // n x n weight matrix never leaves the SM.  Keys outside the event or with key_valid == 0 get weight
 // exactly 0 (reading A2); a query with no valid key gets O = 0 (A15).
 //
-// One CTA = one head x two consecutive 128-row query tiles (a, b) of one event, sharing every K / V tile.
-// Key tiles are 64 keys wide and S is DOUBLE-BUFFERED in TMEM, so the tensor pipe computes S_t(j+1) while the
-// softmax warps work on S_t(j): the MMA chain (measured: ~1400 cycles of issue + hand-off latency per tile at
-// hd = 32, because one thread issues at most one tcgen05.mma per ~50 cycles whatever its N) is off the softmax
-// warps' critical path, and the exponentials (MUFU, the binding unit at hd = 32) run back to back.
-//   warps 0-3   softmax warpgroup of query tile a, warps 4-7 of tile b: one query row per thread, the tile's 64
-//               scores in registers:  S -> (mask) -> running max -> exp2 -> bf16 P written back over S's TMEM
-//               columns; then acc = acc * corr + O_t(j-1) in registers (no read-modify-write of O in TMEM).
-//   warp 8      TMA producer: Q_a, Q_b once; then stages of (K, V), each [128 keys x hd] row-major (two key tiles
+// One CTA = one head x NT consecutive 128-row query tiles of one event (NT = 3 at hd <= 32, 2 at hd = 64),
+// sharing every K / V tile.  Key tiles are 64 keys wide and S is DOUBLE-BUFFERED in TMEM, so the tensor pipe
+// computes S_t(j+1) while the softmax warps work on S_t(j): the MMA chain (issue + hand-off latency) is off the
+// softmax warps' critical path.  At hd = 32 the exponentials (MUFU, 16/clk/SM) are the binding unit; one softmax
+// warp's serial chain per tile (TMEM load, max, exp, TMEM store, fold) is about twice its MUFU time, so three
+// warps per SM sub-partition (NT = 3) are what keeps the MUFU pipe busy (measured with -DMLPF_ATT_LOG).
+//   warps 0 .. 4NT-1   softmax warpgroups, one per query tile: one query row per thread, the tile's 64 scores in
+//               registers:  S -> (mask) -> running max -> exp2 -> bf16 P written back over S's TMEM columns;
+//               acc = acc * corr + O_t(j-1) in registers (no read-modify-write of O in TMEM), and only then is
+//               P_t(j) published, so O_t needs a single TMEM buffer.
+//   warp 4NT    TMA producer: Q tiles once; then stages of (K, V), each [128 keys x hd] row-major (two key tiles
 //               per stage).  Q, K, V are column blocks of one row-major [N, 3d] buffer, so an event may start at
 //               any row (TMA needs 16-byte alignment only along the innermost, head-dim, coordinate).
-//   warps 9,10  MMA issuers of tile a / b:  S_t(j) = Q_t K_j^T  (M=128, N=64, K=hd) -> TMEM buffer j&1;
-//               O_t(j) = P_t(j) V_j (A = P read from TMEM, B = V_j as an MN-major operand, K=64, N=hd)
-//               -> TMEM O buffer j&1, fresh each tile.
-//   warp 11     idle (it only makes warpgroup 2 complete for setmaxnreg).
-// TMEM columns: S_t[b] at (2t+b) 64 (P_t[b] aliases its first 32 columns); O_t[b] at 256 + (2t+b) hd.
+//   warps 4NT+1 .. 4NT+NT   MMA issuers, one per query tile:  S_t(j) = Q_t K_j^T  (M=128, N=64, K=hd) -> S buffer
+//               j&1;  O_t(j) = P_t(j) V_j (A = P read from TMEM, B = V_j as an MN-major operand, K=64, N=hd).
+//               All 32 lanes run the issue code with warp-uniform operands (one lane elected inside the wrappers).
+// setmaxnreg moves the producer warpgroup's registers to the softmax warpgroups.
+// TMEM columns: S_t[b] at 128 t + 64 b (P_t[b] aliases its first 32 columns); O_t at 128 NT + hd t.
 #include "tc_api.h"
 #include "ptx.cuh"
 
 namespace mlpf {
 
-constexpr int ATT_THREADS = 384;
-constexpr int ATT_WARP_TMA = 8, ATT_WARP_MMA = 9;       // MMA issuers: warp 9 (tile a), warp 10 (tile b)
 constexpr int ATT_BQ = 128, ATT_BK = 64, ATT_SK = 128;  // query tile, key tile, keys per TMA stage
 
 template <int HD>
 struct AttnCfg {
+    static constexpr int NT = HD <= 32 ? 3 : 2;             // query tiles per CTA
+    static constexpr int THREADS = (NT + 1) * 128;
+    static constexpr int WARP_TMA = 4 * NT, WARP_MMA = 4 * NT + 1;
+    static constexpr int SOFTMAX_REGS = NT == 3 ? 152 : 232, PRODUCER_REGS = 40;
     static constexpr int Q_BYTES = ATT_BQ * HD * 2;
     static constexpr int K_BYTES = ATT_SK * HD * 2;
     static constexpr int V_BYTES = ATT_SK * HD * 2;
     static constexpr int STAGE_BYTES = K_BYTES + V_BYTES;
     static constexpr int STAGES = HD == 64 ? 4 : 6;
-    static constexpr int SMEM_BYTES = 2 * Q_BYTES + STAGES * STAGE_BYTES + 1024;
+    static constexpr int SMEM_BYTES = NT * Q_BYTES + STAGES * STAGE_BYTES + 1024;
     static constexpr int SW = HD * 2;                       // swizzle width of Q / K / V rows in bytes
+    static constexpr int O_COL0 = 128 * NT;
+    static_assert(O_COL0 + NT * HD <= 512, "TMEM budget");
 };
+
+int tc_attn_rows_per_cta(int hd) { return (hd <= 32 ? 3 : 2) * ATT_BQ; }
 
 struct AttnParams {
     const int* key_valid;      // [N] or null
     const int* n_valid;        // [E] valid rows per event, or null: events without pad rows skip the key_valid loads
     const int* offsets;        // [E+1]
-    const int2* pairs;         // (event, pair index)
-    int n_pairs, H, d;
+    const int2* items;         // (event, index of the group of NT query tiles)
+    int n_items, H, d;
     bf16* O; bf16* O_lo;
     float scale_log2;          // log2(e) / sqrt(hd)
 #ifdef MLPF_ATT_LOG
@@ -53,15 +61,17 @@ struct AttnParams {
 #endif
 };
 
-// 32 scores of one row (registers r[0..31]) -> running max
+// 32 scores of one row (registers r[0..31]) -> max, as four independent chains (a single chain of 32 dependent
+// FMNMX costs ~200 cycles of latency that nothing else in the warp can hide)
 template <bool FULL>
 __device__ __forceinline__ float max32(const uint32_t* r, uint32_t mask, float mx) {
+    float m[4] = {mx, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
     for (int i = 0; i < 32; ++i) {
         const float v = __uint_as_float(r[i]);
-        mx = fmaxf(mx, FULL ? v : ((mask >> i) & 1u ? v : -INFINITY));
+        m[i & 3] = fmaxf(m[i & 3], FULL ? v : ((mask >> i) & 1u ? v : -INFINITY));
     }
-    return mx;
+    return fmaxf(fmaxf(m[0], m[1]), fmaxf(m[2], m[3]));
 }
 // p = 2^(s c - m c) for 32 scores -> 16 bf16 pairs; their fp32 sums go to two packed accumulators (short chains)
 template <bool FULL>
@@ -87,9 +97,8 @@ __device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c,
 // Returns corr = 2^((m_old - m_new) c) and the row sum of P in rsum.
 template <bool FULL>
 __device__ __forceinline__ float softmax_tile(const uint32_t (&s)[64], uint32_t s_addr, const uint32_t (&mask)[2], float c,
-                                              float& m_run, float& rsum, uint32_t mid_bar = 0) {
-    float mx = max32<FULL>(&s[0], mask[0], -INFINITY);
-    mx = max32<FULL>(&s[32], mask[1], mx);
+                                              float& m_run, float& rsum) {
+    const float mx = fmaxf(max32<FULL>(&s[0], mask[0], -INFINITY), max32<FULL>(&s[32], mask[1], -INFINITY));
     const float m_new = fmaxf(m_run, mx);
     const float m_use = (m_new == -INFINITY) ? 0.0f : m_new;
     const float corr = ptx::fast_exp2((m_run - m_use) * c);      // m_run = -inf -> 0
@@ -101,25 +110,21 @@ __device__ __forceinline__ float softmax_tile(const uint32_t (&s)[64], uint32_t 
         uint32_t pk[16];
         exp32<FULL>(&s[32 * w], mask[w], c, neg_mc, pk, rs);
         ptx::tmem_st16(s_addr + 16 * w, pk);
-        if (w == 0 && mid_bar) {                                 // half-way through this tile (see bar_stagger)
-            __syncwarp();
-            if ((threadIdx.x & 31) == 0) ptx::mbar_arrive(mid_bar);
-        }
     }
     rsum = (rs[0].x + rs[0].y) + (rs[1].x + rs[1].y);
     return corr;
 }
 
 template <int HD>
-__global__ void __launch_bounds__(ATT_THREADS, 1)
+__global__ void __launch_bounds__(AttnCfg<HD>::THREADS, 1)
 k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     using Cfg = AttnCfg<HD>;
-    constexpr int ST = Cfg::STAGES;
+    constexpr int ST = Cfg::STAGES, NT = Cfg::NT;
     extern __shared__ uint8_t smem_raw[];
-    __shared__ uint64_t bars[1 + 2 * ST + 11];
+    __shared__ uint64_t bars[1 + 2 * ST + 5 * NT];
     __shared__ uint32_t tmem_base_slot;
 #ifdef MLPF_ATT_LOG
-    __shared__ long long tlog[4][32][6];
+    __shared__ long long tlog[2 * NT][32][6];
     const bool logging = prm.prof && blockIdx.x == 200;
 #define TLOG(r, j, k) do { if (logging && (j) < 32 && (threadIdx.x & 31) == 0) tlog[r][j][k] = clock64(); } while (0)
 #else
@@ -128,44 +133,39 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
 
     const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
     const int item = blockIdx.x / prm.H, head = blockIdx.x % prm.H;
-    const int2 pr = prm.pairs[item];
-    const int ev0 = prm.offsets[pr.x], ev1 = prm.offsets[pr.x + 1];
-    const int q0a = ev0 + pr.y * 2 * ATT_BQ, q0b = q0a + ATT_BQ;
-    const bool has_b = q0b < ev1;
+    const int2 it = prm.items[item];
+    const int ev0 = prm.offsets[it.x], ev1 = prm.offsets[it.x + 1];
+    const int q0 = ev0 + it.y * NT * ATT_BQ;                         // first query row of this CTA
+    const int nt = min(NT, (ev1 - q0 + ATT_BQ - 1) / ATT_BQ);        // query tiles that hold rows of the event (>= 1)
     const int nkv = (ev1 - ev0 + ATT_BK - 1) / ATT_BK;              // 64-key tiles
-    const int* key_valid = (prm.key_valid && !(prm.n_valid && prm.n_valid[pr.x] == ev1 - ev0)) ? prm.key_valid : nullptr;
     const int nst = (ev1 - ev0 + ATT_SK - 1) / ATT_SK;              // 128-key TMA stages
+    const int* key_valid = (prm.key_valid && !(prm.n_valid && prm.n_valid[it.x] == ev1 - ev0)) ? prm.key_valid : nullptr;
 
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t sQ = smem_base;                                  // Q_a, Q_b
-    const uint32_t sKV = smem_base + 2 * Cfg::Q_BYTES;
+    const uint32_t sQ = smem_base;                                  // Q tiles
+    const uint32_t sKV = smem_base + NT * Cfg::Q_BYTES;
     const uint32_t bar_q = ptx::smem_u32(&bars[0]);
     const uint32_t bar_kv_full = ptx::smem_u32(&bars[1]);
     const uint32_t bar_kv_empty = ptx::smem_u32(&bars[1 + ST]);
-    const uint32_t bar_s = ptx::smem_u32(&bars[1 + 2 * ST]);        // [2t + b]: S_t(j) landed in buffer b = j & 1
-    const uint32_t bar_p = ptx::smem_u32(&bars[1 + 2 * ST + 4]);    // [2t + b]: P_t(j) written over buffer b
-    const uint32_t bar_o = ptx::smem_u32(&bars[1 + 2 * ST + 8]);    // [t]: O_t(j) complete
-    // tile b's softmax starts half a tile period after tile a's, so that one tile's exponentials (MUFU) overlap the
-    // other's max pass, TMEM traffic and barrier latencies instead of both contending for the same unit in lockstep
-    const uint32_t bar_stagger = ptx::smem_u32(&bars[1 + 2 * ST + 10]);
+    const uint32_t bar_s = ptx::smem_u32(&bars[1 + 2 * ST]);             // [2t + b]: S_t(j) landed in buffer b = j & 1
+    const uint32_t bar_p = ptx::smem_u32(&bars[1 + 2 * ST + 2 * NT]);    // [2t + b]: P_t(j) written over buffer b
+    const uint32_t bar_o = ptx::smem_u32(&bars[1 + 2 * ST + 4 * NT]);    // [t]: O_t(j) complete
 
-    if (warp == ATT_WARP_TMA && lane == 0) {
+    if (warp == Cfg::WARP_TMA && lane == 0) {
         ptx::mbar_init(bar_q, 1);
         for (int s = 0; s < ST; ++s) {
             ptx::mbar_init(bar_kv_full + 8 * s, 1);
-            ptx::mbar_init(bar_kv_empty + 8 * s, has_b ? 2 : 1);     // one commit per query tile
+            ptx::mbar_init(bar_kv_empty + 8 * s, nt);                // one commit per active query tile
         }
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < 2 * NT; ++i) {
             ptx::mbar_init(bar_s + 8 * i, 1);
             ptx::mbar_init(bar_p + 8 * i, 4);                        // one arrival per softmax warp
         }
-        ptx::mbar_init(bar_o, 1);
-        ptx::mbar_init(bar_o + 8, 1);
-        ptx::mbar_init(bar_stagger, 4);
+        for (int i = 0; i < NT; ++i) ptx::mbar_init(bar_o + 8 * i, 1);
         ptx::fence_barrier_init();
         ptx::tma_prefetch_desc(&tmQKV);
     }
-    if (warp == ATT_WARP_MMA) {
+    if (warp == Cfg::WARP_MMA) {
         ptx::tmem_alloc(ptx::smem_u32(&tmem_base_slot), 512);
         ptx::tmem_relinquish();
     }
@@ -174,14 +174,13 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     ptx::tc_fence_after();
     const uint32_t tmem_base = tmem_base_slot;
 
-    if (warp >= 8) {
-    ptx::setmaxnreg_dec<40>();
-    if (warp == ATT_WARP_TMA) {
+    if (warp >= 4 * NT) {
+    ptx::setmaxnreg_dec<Cfg::PRODUCER_REGS>();
+    if (warp == Cfg::WARP_TMA) {
         // ------------------------------------------------------------ TMA producer
         if (lane == 0) {
-            ptx::mbar_expect_tx(bar_q, Cfg::Q_BYTES * (has_b ? 2 : 1));
-            ptx::tma_load_2d(sQ, &tmQKV, bar_q, head * HD, q0a);
-            if (has_b) ptx::tma_load_2d(sQ + Cfg::Q_BYTES, &tmQKV, bar_q, head * HD, q0b);
+            ptx::mbar_expect_tx(bar_q, Cfg::Q_BYTES * nt);
+            for (int t = 0; t < nt; ++t) ptx::tma_load_2d(sQ + t * Cfg::Q_BYTES, &tmQKV, bar_q, head * HD, q0 + t * ATT_BQ);
         }
         for (int i = 0; i < nst; ++i) {
             const int s = i % ST;
@@ -195,9 +194,9 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
             }
             __syncwarp();
         }
-    } else if (warp == ATT_WARP_MMA || warp == ATT_WARP_MMA + 1) {
+    } else if (warp - Cfg::WARP_MMA < nt) {
         // ------------------------------------------------------------ MMA issuers (one per query tile)
-        const int t = warp - ATT_WARP_MMA;
+        const int t = warp - Cfg::WARP_MMA;
         constexpr uint32_t idesc_s = ptx::umma_idesc_bf16(128, ATT_BK);
         constexpr uint32_t idesc_o = ptx::umma_idesc_bf16(128, HD) | ptx::UMMA_B_MN_MAJOR;
         constexpr uint32_t HALF = ATT_BK * Cfg::SW;                  // bytes of a 64-key half of a K or V stage
@@ -206,54 +205,50 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
             const uint32_t qb = sQ + t * Cfg::Q_BYTES;
 #pragma unroll
             for (int k = 0; k < HD / 16; ++k)
-                ptx::mma_ss(tmem_base + (2 * t + (j & 1)) * 64, ptx::umma_desc_kmajor(qb + k * 32, Cfg::SW),
+                ptx::mma_ss(tmem_base + 128 * t + 64 * (j & 1), ptx::umma_desc_kmajor(qb + k * 32, Cfg::SW),
                             ptx::umma_desc_kmajor(kb + k * 32, Cfg::SW), idesc_s, k != 0);
             ptx::mma_commit(bar_s + 8 * (2 * t + (j & 1)));
         };
-        auto issue_o = [&](int j) {                 // O_t(j) = P_t(j) V_j -> O buffer j & 1
+        auto issue_o = [&](int j) {                 // O_t(j) = P_t(j) V_j
             const uint32_t vb = sKV + ((j >> 1) % ST) * Cfg::STAGE_BYTES + Cfg::K_BYTES + (j & 1) * HALF;
-            const uint32_t o_col = 256 + (2 * t + (j & 1)) * HD;
 #pragma unroll
             for (int k = 0; k < ATT_BK / 16; ++k)
-                ptx::mma_ts(tmem_base + o_col, tmem_base + (2 * t + (j & 1)) * 64 + k * 8,
+                ptx::mma_ts(tmem_base + Cfg::O_COL0 + HD * t, tmem_base + 128 * t + 64 * (j & 1) + k * 8,
                             ptx::umma_desc_mnmajor(vb + k * 16 * Cfg::SW, Cfg::SW), idesc_o, k != 0);
             ptx::mma_commit(bar_o + 8 * t);
         };
-        if (t == 0 || has_b) {
-            ptx::mbar_wait(bar_q, 0);
-            ptx::mbar_wait(bar_kv_full, 0);
+        ptx::mbar_wait(bar_q, 0);
+        ptx::mbar_wait(bar_kv_full, 0);
+        ptx::tc_fence_after();
+        issue_s(0);                                  // all lanes: one is elected inside the MMA / commit wrappers
+        if (nkv > 1) issue_s(1);
+        for (int j = 0; j < nkv; ++j) {
+            TLOG(NT + t, j, 0);
+            ptx::mbar_wait(bar_p + 8 * (2 * t + (j & 1)), (j >> 1) & 1);     // P_t(j) is in TMEM, O_t(j-1) is folded
             ptx::tc_fence_after();
-            issue_s(0);                             // all lanes: one is elected inside the MMA / commit wrappers
-            if (nkv > 1) issue_s(1);
-            for (int j = 0; j < nkv; ++j) {
-                TLOG(2 + t, j, 0);
-                ptx::mbar_wait(bar_p + 8 * (2 * t + (j & 1)), (j >> 1) & 1);     // P_t(j) is in TMEM
+            TLOG(NT + t, j, 1);
+            issue_o(j);
+            // K and V of stage j >> 1 are no longer needed by this tile after its second half
+            if ((j & 1) || j == nkv - 1) ptx::mma_commit(bar_kv_empty + 8 * ((j >> 1) % ST));
+            TLOG(NT + t, j, 2);
+            if (j + 2 < nkv) {                       // S_t(j+2) reuses S buffer j & 1: in order after P_t(j) V_j
+                const int i2 = (j + 2) >> 1;
+                if (((j + 2) & 1) == 0) ptx::mbar_wait(bar_kv_full + 8 * (i2 % ST), (i2 / ST) & 1);
                 ptx::tc_fence_after();
-                TLOG(2 + t, j, 1);
-                issue_o(j);
-                // K and V of stage j >> 1 are no longer needed by this tile after its second half
-                if ((j & 1) || j == nkv - 1) ptx::mma_commit(bar_kv_empty + 8 * ((j >> 1) % ST));
-                TLOG(2 + t, j, 2);
-                if (j + 2 < nkv) {                   // S_t(j+2) reuses S buffer j & 1: in order after P_t(j) V_j
-                    const int i2 = (j + 2) >> 1;
-                    if (((j + 2) & 1) == 0) ptx::mbar_wait(bar_kv_full + 8 * (i2 % ST), (i2 / ST) & 1);
-                    ptx::tc_fence_after();
-                    TLOG(2 + t, j, 3);
-                    issue_s(j + 2);
-                    TLOG(2 + t, j, 4);
-                }
+                issue_s(j + 2);
+                TLOG(NT + t, j, 3);
             }
         }
     }
     } else {
         // ------------------------------------------------------------ softmax warpgroups
-        ptx::setmaxnreg_inc<232>();
-        const int t = warp >> 2;                       // 0: tile a, 1: tile b
+        ptx::setmaxnreg_inc<Cfg::SOFTMAX_REGS>();
+        const int t = warp >> 2;                       // query tile of this warpgroup
         const int q = warp & 3;                        // TMEM lane quarter this warp may access
-        const int row_in_tile = q * 32 + lane;
-        const int qrow = (t == 0 ? q0a : q0b) + row_in_tile;
-        if (t == 0 || has_b) {
+        const int qrow = q0 + t * ATT_BQ + q * 32 + lane;
+        if (t < nt) {
             const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16);
+            const uint32_t o_addr = lane_addr + Cfg::O_COL0 + HD * t;
             const float c = prm.scale_log2;
             float acc[HD];
 #pragma unroll
@@ -261,8 +256,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
             float m_run = -INFINITY, l_run = 0.0f, corr_prev = 0.0f, rsum_prev = 0.0f;
             // O_t(j) of a finished P V product: issue the TMEM loads ...
             uint32_t o_r[HD];
-            auto fold_load = [&](int j) {
-                const uint32_t o_addr = lane_addr + 256 + (2 * t + (j & 1)) * HD;
+            auto fold_load = [&]() {
 #pragma unroll
                 for (int w = 0; w < HD / 16; ++w) ptx::tmem_ld16(o_addr + w * 16, *reinterpret_cast<uint32_t(*)[16]>(&o_r[w * 16]));
             };
@@ -282,11 +276,10 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
             auto load_s = [&](int j) {
                 ptx::mbar_wait(bar_s + 8 * (2 * t + (j & 1)), (j >> 1) & 1);
                 ptx::tc_fence_after();
-                const uint32_t s_addr = lane_addr + (2 * t + (j & 1)) * 64;
+                const uint32_t s_addr = lane_addr + 128 * t + 64 * (j & 1);
                 ptx::tmem_ld32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
                 ptx::tmem_ld32(s_addr + 32, *reinterpret_cast<uint32_t(*)[32]>(&s[32]));
             };
-            if (t == 1) ptx::mbar_wait(bar_stagger, 0);
             load_s(0);
             ptx::tmem_ld_wait();
             for (int j = 0; j < nkv; ++j) {
@@ -306,39 +299,37 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                 } else {
                     mask[0] = mask[1] = 0xffffffffu;
                 }
-                const uint32_t s_addr = lane_addr + (2 * t + (j & 1)) * 64;
+                const uint32_t s_addr = lane_addr + 128 * t + 64 * (j & 1);
                 if (q == 0) TLOG(t, j, 0);
                 float rsum;
-                const uint32_t mid = (t == 0 && j == 0 && has_b) ? bar_stagger : 0u;
-                const float corr = full ? softmax_tile<true>(s, s_addr, mask, c, m_run, rsum, mid)
-                                        : softmax_tile<false>(s, s_addr, mask, c, m_run, rsum, mid);
-                // O_t(j-1) was issued about a softmax period ago: this wait does not stall, but it must come BEFORE
-                // P_t(j) is published -- afterwards O_t(j) could complete too and the barrier would be two phases
-                // ahead of this waiter (parity aliasing)
+                const float corr = full ? softmax_tile<true>(s, s_addr, mask, c, m_run, rsum)
+                                        : softmax_tile<false>(s, s_addr, mask, c, m_run, rsum);
                 if (q == 0) TLOG(t, j, 1);
-                if (j > 0) {
+                // S_t(j+1) was issued after O_t(j-1) and the tensor pipe completes in order: once S_t(j+1) has landed,
+                // O_t(j-1) is complete too.  Only the last tile has to wait on bar_o for it.
+                if (j + 1 < nkv) {
+                    load_s(j + 1);                        // double-buffered: usually long complete
+                } else if (j > 0) {
                     ptx::mbar_wait(bar_o + 8 * t, (j - 1) & 1);
                     ptx::tc_fence_after();
-                    fold_load(j - 1);
                 }
+                if (j > 0) fold_load();
                 if (q == 0) TLOG(t, j, 2);
-                if (j + 1 < nkv) load_s(j + 1);
-                if (q == 0) TLOG(t, j, 3);         // S_t(j+1) is double-buffered: usually long complete
-                ptx::tmem_st_wait();                      // the loads above fly while the P stores drain
+                ptx::tmem_ld_wait();
+                if (j > 0) fold(corr_prev, rsum_prev);    // O_t is free again ...
+                if (q == 0) TLOG(t, j, 3);
+                ptx::tmem_st_wait();
                 ptx::tc_fence_before();
                 __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(bar_p + 8 * (2 * t + (j & 1)));      // P_t(j) is in TMEM
+                if (lane == 0) ptx::mbar_arrive(bar_p + 8 * (2 * t + (j & 1)));      // ... so P_t(j) V_j may overwrite it
                 if (q == 0) TLOG(t, j, 4);
-                ptx::tmem_ld_wait();
-                if (j > 0) fold(corr_prev, rsum_prev);
-                if (q == 0) TLOG(t, j, 5);
                 corr_prev = corr;
                 rsum_prev = rsum;
             }
             // last tile's P V
             ptx::mbar_wait(bar_o + 8 * t, (nkv - 1) & 1);
             ptx::tc_fence_after();
-            fold_load(nkv - 1);
+            fold_load();
             ptx::tmem_ld_wait();
             fold(corr_prev, rsum_prev);
             if (qrow < ev1) {
@@ -365,15 +356,14 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     }
     ptx::tc_fence_before();
     __syncthreads();
-    if (warp == ATT_WARP_MMA) ptx::tmem_dealloc(tmem_base, 512);
+    if (warp == Cfg::WARP_MMA) ptx::tmem_dealloc(tmem_base, 512);
 #ifdef MLPF_ATT_LOG
-    if (logging) for (int i = threadIdx.x; i < 4 * 32 * 6; i += ATT_THREADS) prm.prof[i] = (&tlog[0][0][0])[i];
+    if (logging) for (int i = threadIdx.x; i < 2 * NT * 32 * 6; i += Cfg::THREADS) prm.prof[i] = (&tlog[0][0][0])[i];
 #endif
 }
 
 template <int HD>
-static int tc_attn_launch_hd(TcContext* c, const bf16* QKV, int64_t N, const AttnParams& prm,
-                             cudaStream_t st) {
+static int tc_attn_launch_hd(TcContext* c, const bf16* QKV, int64_t N, AttnParams prm, cudaStream_t st) {
     using Cfg = AttnCfg<HD>;
     CUtensorMap tmQKV;
     if (tc_tensor_map(c, &tmQKV, QKV, 3 * prm.d, N, 3 * prm.d, HD, ATT_SK)) return -1;
@@ -384,32 +374,34 @@ static int tc_attn_launch_hd(TcContext* c, const bf16* QKV, int64_t N, const Att
         if (e != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return -1; }
         attr_set = true;
     }
-    kern<<<prm.n_pairs * prm.H, ATT_THREADS, Cfg::SMEM_BYTES, st>>>(tmQKV, prm);
 #ifdef MLPF_ATT_LOG
-    {   // rows 0,1: softmax warp 0 of tile a / b; rows 2,3: MMA issuers; one line per key tile
-        long long h[768];
+    static long long* pbuf = nullptr;
+    constexpr int NLOG = 2 * Cfg::NT * 32 * 6;
+    if (!pbuf) cudaMalloc(&pbuf, NLOG * 8);
+    cudaMemsetAsync(pbuf, 0, NLOG * 8, st);
+    prm.prof = pbuf;
+#endif
+    kern<<<prm.n_items * prm.H, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(tmQKV, prm);
+#ifdef MLPF_ATT_LOG
+    {   // rows 0..NT-1: softmax warp 0 of each tile; rows NT..2NT-1: MMA issuers; one line per key tile
+        long long h[NLOG];
         cudaMemcpy(h, prm.prof, sizeof h, cudaMemcpyDeviceToHost);
         FILE* f = fopen("gpurun_out/att_log.txt", "w");
-        if (f) { for (int r = 0; r < 4; ++r) for (int j = 0; j < 32; ++j) { fprintf(f, "%d %d", r, j); for (int k = 0; k < 6; ++k) fprintf(f, " %lld", h[(r * 32 + j) * 6 + k]); fprintf(f, "\n"); } fclose(f); }
+        if (f) { for (int r = 0; r < 2 * Cfg::NT; ++r) for (int j = 0; j < 32; ++j) { fprintf(f, "%d %d", r, j); for (int k = 0; k < 6; ++k) fprintf(f, " %lld", h[(r * 32 + j) * 6 + k]); fprintf(f, "\n"); } fclose(f); }
     }
 #endif
     return 0;
 }
 
+// items: (event, group index) pairs, one per CTA-row-group of tc_attn_rows_per_cta(hd) query rows
 int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const int* key_valid, const int* n_valid,
-                          const int* offsets, const int2* pairs, int n_pairs, int d, int H, bf16* O, bf16* O_lo,
+                          const int* offsets, const int2* items, int n_items, int d, int H, bf16* O, bf16* O_lo,
                           cudaStream_t st) {
     const int hd = d / H;
     AttnParams prm;
-    prm.key_valid = key_valid; prm.n_valid = n_valid; prm.offsets = offsets; prm.pairs = pairs; prm.n_pairs = n_pairs; prm.H = H; prm.d = d;
-    prm.O = O; prm.O_lo = O_lo;
+    prm.key_valid = key_valid; prm.n_valid = n_valid; prm.offsets = offsets; prm.items = items; prm.n_items = n_items;
+    prm.H = H; prm.d = d; prm.O = O; prm.O_lo = O_lo;
     prm.scale_log2 = 1.4426950408889634f / sqrtf((float)hd);
-#ifdef MLPF_ATT_LOG
-    static long long* pbuf = nullptr;
-    if (!pbuf) cudaMalloc(&pbuf, 768 * 8);
-    cudaMemsetAsync(pbuf, 0, 768 * 8, st);
-    prm.prof = pbuf;
-#endif
     switch (hd) {
         case 16: return tc_attn_launch_hd<16>(c, QKV, N, prm, st);
         case 32: return tc_attn_launch_hd<32>(c, QKV, N, prm, st);
