@@ -73,6 +73,28 @@ __device__ __forceinline__ float max32(const uint32_t* r, uint32_t mask, float m
     }
     return fmaxf(fmaxf(m[0], m[1]), fmaxf(m[2], m[3]));
 }
+// 2^x for a pair, x <= 0, on the FMA / ALU pipes instead of the MUFU (Cody-Waite split + degree-3 polynomial):
+//   x = n + f, n = round(x) taken from the mantissa of x + 1.5 * 2^23, f in [-0.5, 0.5];
+//   2^f ~ 1 + f (c1 + f (c2 + f c3))  (max relative error 1.0e-4, 40x below the bf16 rounding of P);
+//   2^n goes into the exponent field with one integer multiply-add.
+// The MUFU does 16 ex2 per clock and SM and is the binding unit of this kernel at hd = 32 (one ex2 per 128 tensor
+// FLOPs); every ATT_POLY_EVERY-th pair takes this path so that MUFU and FMA pipes finish together.
+__device__ __forceinline__ float2 exp2_poly2(float2 x) {
+    const float2 magic = make_float2(12582912.0f, 12582912.0f);
+    x.x = fmaxf(x.x, -126.0f); x.y = fmaxf(x.y, -126.0f);
+    const float2 xr = ptx::fadd2(x, magic);                                          // low mantissa bits = round(x)
+    const float2 f = ptx::fadd2(x, ptx::fadd2(make_float2(12582912.0f, 12582912.0f), make_float2(-xr.x, -xr.y)));
+    float2 p = ptx::ffma2(f, make_float2(0.0550089306f, 0.0550089306f), make_float2(0.2422109596f, 0.2422109596f));
+    p = ptx::ffma2(p, f, make_float2(0.6932829272f, 0.6932829272f));
+    p = ptx::ffma2(p, f, make_float2(1.0f, 1.0f));
+    return make_float2(__int_as_float(__float_as_int(p.x) + (__float_as_int(xr.x) << 23)),
+                       __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
+}
+#ifndef ATT_POLY_EVERY
+#define ATT_POLY_EVERY 0     // measured on cfg3 (hd = 32): 0 -> 0.893 ms, 4 -> 0.928, 3 -> 0.900, 2 -> 1.03: the kernel is
+#endif                       // issue / latency bound before it is MUFU bound, so the polynomial path stays off
+
+
 // p = 2^(s c - m c) for 32 scores -> 16 bf16 pairs; their fp32 sums go to two packed accumulators (short chains)
 template <bool FULL>
 __device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c, float neg_mc, uint32_t (&pk)[16],
@@ -81,7 +103,9 @@ __device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c,
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
         const float2 x = ptx::ffma2(make_float2(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1])), c2, m2);
-        float2 p = make_float2(ptx::fast_exp2(x.x), ptx::fast_exp2(x.y));
+        float2 p;
+        if (ATT_POLY_EVERY > 0 && (i % (ATT_POLY_EVERY > 0 ? ATT_POLY_EVERY : 1)) == ATT_POLY_EVERY - 1) p = exp2_poly2(x);
+        else p = make_float2(ptx::fast_exp2(x.x), ptx::fast_exp2(x.y));
         if (!FULL) {
             p.x = (mask >> (2 * i)) & 1u ? p.x : 0.0f;
             p.y = (mask >> (2 * i + 1)) & 1u ? p.y : 0.0f;
@@ -308,20 +332,28 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                 // S_t(j+1) was issued after O_t(j-1) and the tensor pipe completes in order: once S_t(j+1) has landed,
                 // O_t(j-1) is complete too.  Only the last tile has to wait on bar_o for it.
                 if (j + 1 < nkv) {
-                    load_s(j + 1);                        // double-buffered: usually long complete
+                    ptx::mbar_wait(bar_s + 8 * (2 * t + ((j + 1) & 1)), ((j + 1) >> 1) & 1);   // usually long complete
                 } else if (j > 0) {
                     ptx::mbar_wait(bar_o + 8 * t, (j - 1) & 1);
-                    ptx::tc_fence_after();
                 }
-                if (j > 0) fold_load();
+                ptx::tc_fence_after();
+                if (j > 0) {                              // O_t is free again after this fold ...
+                    fold_load();
+                    ptx::tmem_ld_wait();
+                    fold(corr_prev, rsum_prev);
+                }
                 if (q == 0) TLOG(t, j, 2);
-                ptx::tmem_ld_wait();
-                if (j > 0) fold(corr_prev, rsum_prev);    // O_t is free again ...
+                if (j + 1 < nkv) {                        // next tile's scores: in flight while the P stores drain
+                    const uint32_t s_next = lane_addr + 128 * t + 64 * ((j + 1) & 1);
+                    ptx::tmem_ld32(s_next, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
+                    ptx::tmem_ld32(s_next + 32, *reinterpret_cast<uint32_t(*)[32]>(&s[32]));
+                }
                 if (q == 0) TLOG(t, j, 3);
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(bar_p + 8 * (2 * t + (j & 1)));      // ... so P_t(j) V_j may overwrite it
+                ptx::tmem_ld_wait();
                 if (q == 0) TLOG(t, j, 4);
                 corr_prev = corr;
                 rsum_prev = rsum;
