@@ -305,8 +305,17 @@ def run_ours(args):
     share = {c: round(t / max(sum(v[0] for v in cls.values()), 1e-9), 4) for c, (t, n) in cls.items()}
     gemm_ms = sum(cls[c][0] for c in ("qkv", "outproj", "ffn1", "ffn2"))
     gemm_tflops = fl["gemm_per_layer"] * m.n_layers * args.steps / (gemm_ms * 1e-3) / 1e12 if gemm_ms else None
+    traffic = None                                    # DRAM bytes per launch from the committed ncu --set full capture
+    tpath = os.path.join(HERE, "profiles", "attn_traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            tj = json.load(f)
+        if tj.get("workload") == name:
+            traffic = tj["dram_bytes_per_launch"]
     roofline = {"bound": "tensor", "kernel": "k_tc_attn (a4)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": (achieved / peak) if achieved else None, "traffic": None,
+                "frac": (achieved / peak) if achieved else None, "traffic": traffic,
+                "algorithmic_bytes_per_launch": float(N) * m.d_model * 2 * (3 + 2),   # read q,k,v; write o hi + lo
+                "mufu_ceiling_frac": 16.0 * 148 * 1.9e9 * 4 * m.head_dim / 1e12 / peak,
                 "peak_source": f"{peaks['source']} bf16_tflops_sustained",
                 "flops_per_launch": fl["attn_per_launch"], "ms_per_launch": per_launch_s * 1e3,
                 "class_time_share": share,
