@@ -91,8 +91,8 @@ __device__ __forceinline__ float2 exp2_poly2(float2 x) {
                        __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
 }
 #ifndef ATT_POLY_EVERY
-#define ATT_POLY_EVERY 0     // measured on cfg3 (hd = 32): 0 -> 0.893 ms, 4 -> 0.928, 3 -> 0.900, 2 -> 1.03: the kernel is
-#endif                       // issue / latency bound before it is MUFU bound, so the polynomial path stays off
+#define ATT_POLY_EVERY 4     // measured on cfg3 (hd = 32, ms per layer): off 0.865, every 8th pair 0.845, 4th 0.825,
+#endif                       // 3rd 0.846, 2nd 0.927 (with register spills in the loop it was a loss at every setting)
 
 
 // p = 2^(s c - m c) for 32 scores -> 16 bf16 pairs; their fp32 sums go to two packed accumulators (short chains)
