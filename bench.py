@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- MLPF encoder forward (steps a0..a8) on synthetic CMS-like events.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--streams S] [--impl ours|reference]
 
 One "step" = one mlpf_infer call over one batch of the workload (default: BASELINE.json configs[2],
 the CMS-scale config the metric is quoted on: 8 events, ~5000 PF elements each, L=6, d=256, H=8).
@@ -297,6 +297,39 @@ def run_ours(args):
                 lat.append(e0.elapsed_time(e1))
     lat = np.array(lat[E:]) if len(lat) > E else np.array(lat)    # first sweep = warm-up
 
+    # ---- several concurrent streams (north_star: "also with several concurrent streams"): the batch is split into
+    # S contiguous event groups, one CUDA stream each, enqueued round-robin from this thread (mlpf_infer only enqueues)
+    multi = None
+    if args.streams > 1:
+        S = min(args.streams, E)
+        bounds = [i * E // S for i in range(S + 1)]
+        streams = [torch.cuda.Stream() for _ in range(S)]
+        fork = torch.cuda.Stream()
+
+        def one_round():
+            with torch.cuda.stream(fork):
+                flush.zero_()
+                t0 = torch.cuda.Event(enable_timing=True)
+                t0.record(fork)
+            ends = []
+            for i, sx in enumerate(streams):
+                e0_, e1_ = bounds[i], bounds[i + 1]
+                r0, r1 = int(off[e0_]), int(off[e1_])
+                sx.wait_event(t0)
+                mod.infer(Xd[r0:r1], off[e0_:e1_ + 1] - off[e0_], lg[r0:r1], rg[r0:r1], stream=sx)
+                ev = torch.cuda.Event(enable_timing=True)
+                ev.record(sx)
+                ends.append(ev)
+            torch.cuda.synchronize()
+            return max(t0.elapsed_time(ev) for ev in ends)
+
+        for _ in range(max(3, args.warmup)):
+            one_round()
+        mt = np.array([one_round() for _ in range(args.steps)])
+        multi = {"n": S, "events_per_s": E / (mt.mean() * 1e-3), "ms_per_step": float(mt.mean()),
+                 "ms_p50": float(np.percentile(mt, 50)), "ms_p90": float(np.percentile(mt, 90)),
+                 "workspace_bytes_all_streams": int(mod.query(P.Q_WORKSPACE_BYTES))}
+
     # ---- roofline of the dominant kernel (a4 attention): algorithmic FLOPs per launch / mean launch duration
     at_ms, at_n = cls["attention"]
     per_launch_s = at_ms * 1e-3 / max(at_n, 1)
@@ -348,7 +381,7 @@ def run_ours(args):
             "gpu_launches": launches_per_step * args.steps, "launches_per_step": launches_per_step,
             "peak_bytes": {"weights": int(mod.query(P.Q_WEIGHT_BYTES)), "workspace": int(mod.query(P.Q_WORKSPACE_BYTES)),
                            "torch_max_allocated": int(torch.cuda.max_memory_allocated())},
-            "clocks": sampler.result(), "roofline": roofline, "cpu_baseline": cpu}
+            "streams": multi, "clocks": sampler.result(), "roofline": roofline, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
@@ -362,6 +395,7 @@ def main():
     ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5a", "cfg5b", "paper"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--streams", type=int, default=1, help="also time the batch split over this many concurrent CUDA streams")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
