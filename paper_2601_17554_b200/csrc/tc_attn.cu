@@ -117,17 +117,26 @@ __device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c,
 }
 
 // One 64-key tile of one query row, scores already in registers s[0..63]:
-// running max -> P = 2^(S c - m c) as bf16, written over S's first 32 TMEM columns at s_addr.
-// Returns corr = 2^((m_old - m_new) c) and the row sum of P in rsum.
+// P = 2^((S - m_ref) c) as bf16, written over S's first 32 TMEM columns at s_addr, row sum of P in rsum.
+// m_ref is a STALE reference maximum (lazy rescaling): it only moves when some row of the warp has a tile maximum
+// more than ATT_RESCALE_LOG2 (in log2 units) above it, so P <= 2^8 and neither bf16 P nor the fp32 sums lose
+// precision, while the accumulated O (in TMEM) has to be rescaled only a few times per row instead of every tile.
+// Returns corr = 2^((m_ref_old - m_ref_new) c); `rescale` (warp-uniform) says whether m_ref moved.
+constexpr float ATT_RESCALE_LOG2 = 8.0f;
 template <bool FULL>
 __device__ __forceinline__ float softmax_tile(const uint32_t (&s)[64], uint32_t s_addr, const uint32_t (&mask)[2], float c,
-                                              float& m_run, float& rsum) {
+                                              float& m_ref, float& rsum, bool& rescale) {
     const float mx = fmaxf(max32<FULL>(&s[0], mask[0], -INFINITY), max32<FULL>(&s[32], mask[1], -INFINITY));
-    const float m_new = fmaxf(m_run, mx);
-    const float m_use = (m_new == -INFINITY) ? 0.0f : m_new;
-    const float corr = ptx::fast_exp2((m_run - m_use) * c);      // m_run = -inf -> 0
-    const float neg_mc = -m_use * c;
-    m_run = m_new;
+    const float m_new = fmaxf(m_ref, mx);
+    // m_ref = -inf and a finite tile maximum: the difference is +inf and votes yes; all keys masked so far: nan -> no
+    rescale = __any_sync(0xffffffffu, (m_new - m_ref) * c > ATT_RESCALE_LOG2);
+    float corr = 1.0f;
+    if (rescale) {
+        const float m_use = (m_new == -INFINITY) ? 0.0f : m_new;
+        corr = ptx::fast_exp2((m_ref - m_use) * c);              // m_ref = -inf -> 0
+        m_ref = m_new;
+    }
+    const float neg_mc = (m_ref == -INFINITY) ? 0.0f : -m_ref * c;
     float2 rs[2] = {make_float2(0.0f, 0.0f), make_float2(0.0f, 0.0f)};
 #pragma unroll
     for (int w = 0; w < 2; ++w) {
@@ -233,12 +242,12 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                             ptx::umma_desc_kmajor(kb + k * 32, Cfg::SW), idesc_s, k != 0);
             ptx::mma_commit(bar_s + 8 * (2 * t + (j & 1)));
         };
-        auto issue_o = [&](int j) {                 // O_t(j) = P_t(j) V_j
+        auto issue_o = [&](int j) {                 // O_t += P_t(j) V_j (accumulated in TMEM over all key tiles)
             const uint32_t vb = sKV + ((j >> 1) % ST) * Cfg::STAGE_BYTES + Cfg::K_BYTES + (j & 1) * HALF;
 #pragma unroll
             for (int k = 0; k < ATT_BK / 16; ++k)
                 ptx::mma_ts(tmem_base + Cfg::O_COL0 + HD * t, tmem_base + 128 * t + 64 * (j & 1) + k * 8,
-                            ptx::umma_desc_mnmajor(vb + k * 16 * Cfg::SW, Cfg::SW), idesc_o, k != 0);
+                            ptx::umma_desc_mnmajor(vb + k * 16 * Cfg::SW, Cfg::SW), idesc_o, (j | k) != 0);
             ptx::mma_commit(bar_o + 8 * t);
         };
         ptx::mbar_wait(bar_q, 0);
@@ -274,26 +283,26 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
             const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16);
             const uint32_t o_addr = lane_addr + Cfg::O_COL0 + HD * t;
             const float c = prm.scale_log2;
-            float acc[HD];
+            float m_ref = -INFINITY, l_run = 0.0f;
+            // O_t *= corr in TMEM (all 32 lanes of the warp, rows that did not move have corr = 1): only when the
+            // warp's reference maximum moved, which happens a few times per row (lazy rescaling)
+            auto rescale_o = [&](float corr) {
+                const float2 c2 = make_float2(corr, corr);
 #pragma unroll
-            for (int i = 0; i < HD; ++i) acc[i] = 0.0f;
-            float m_run = -INFINITY, l_run = 0.0f, corr_prev = 0.0f, rsum_prev = 0.0f;
-            // O_t(j) of a finished P V product: issue the TMEM loads ...
-            uint32_t o_r[HD];
-            auto fold_load = [&]() {
+                for (int c0 = 0; c0 < HD; c0 += 32) {
+                    constexpr int CH = HD < 32 ? HD : 32;
+                    uint32_t r[CH];
 #pragma unroll
-                for (int w = 0; w < HD / 16; ++w) ptx::tmem_ld16(o_addr + w * 16, *reinterpret_cast<uint32_t(*)[16]>(&o_r[w * 16]));
-            };
-            // ... and (after tcgen05.wait::ld) fold them in: acc = acc * corr + O_t(j), l = l * corr + rowsum(P_t(j))
-            auto fold = [&](float corr_j, float rsum_j) {
-                const float2 c2 = make_float2(corr_j, corr_j);
+                    for (int w = 0; w < CH / 16; ++w) ptx::tmem_ld16(o_addr + c0 + w * 16, *reinterpret_cast<uint32_t(*)[16]>(&r[w * 16]));
+                    ptx::tmem_ld_wait();
 #pragma unroll
-                for (int i = 0; i < HD / 2; ++i) {
-                    const float2 a2 = ptx::ffma2(make_float2(acc[2 * i], acc[2 * i + 1]), c2,
-                                                 make_float2(__uint_as_float(o_r[2 * i]), __uint_as_float(o_r[2 * i + 1])));
-                    acc[2 * i] = a2.x; acc[2 * i + 1] = a2.y;
+                    for (int i = 0; i < CH / 2; ++i) {
+                        const float2 v = ptx::fmul2(make_float2(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1])), c2);
+                        r[2 * i] = __float_as_uint(v.x); r[2 * i + 1] = __float_as_uint(v.y);
+                    }
+#pragma unroll
+                    for (int w = 0; w < CH / 16; ++w) ptx::tmem_st16(o_addr + c0 + w * 16, *reinterpret_cast<uint32_t(*)[16]>(&r[w * 16]));
                 }
-                l_run = fmaf(l_run, corr_j, rsum_j);
             };
             // scores of the current tile live in registers; the next tile's are loaded while this one is finished
             uint32_t s[64];
@@ -326,22 +335,20 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                 const uint32_t s_addr = lane_addr + 128 * t + 64 * (j & 1);
                 if (q == 0) TLOG(t, j, 0);
                 float rsum;
-                const float corr = full ? softmax_tile<true>(s, s_addr, mask, c, m_run, rsum)
-                                        : softmax_tile<false>(s, s_addr, mask, c, m_run, rsum);
+                bool rescale;
+                const float corr = full ? softmax_tile<true>(s, s_addr, mask, c, m_ref, rsum, rescale)
+                                        : softmax_tile<false>(s, s_addr, mask, c, m_ref, rsum, rescale);
+                l_run = fmaf(l_run, corr, rsum);
                 if (q == 0) TLOG(t, j, 1);
-                // S_t(j+1) was issued after O_t(j-1) and the tensor pipe completes in order: once S_t(j+1) has landed,
-                // O_t(j-1) is complete too.  Only the last tile has to wait on bar_o for it.
+                // S_t(j+1) was issued after P_t(j-1) V_(j-1) and the tensor pipe completes in order: once S_t(j+1) has
+                // landed, O_t holds all products up to j-1.  Only the last tile has to wait on bar_o for that.
                 if (j + 1 < nkv) {
                     ptx::mbar_wait(bar_s + 8 * (2 * t + ((j + 1) & 1)), ((j + 1) >> 1) & 1);   // usually long complete
                 } else if (j > 0) {
                     ptx::mbar_wait(bar_o + 8 * t, (j - 1) & 1);
                 }
                 ptx::tc_fence_after();
-                if (j > 0) {                              // O_t is free again after this fold ...
-                    fold_load();
-                    ptx::tmem_ld_wait();
-                    fold(corr_prev, rsum_prev);
-                }
+                if (rescale && j > 0) rescale_o(corr);    // before P_t(j) is published: no MMA is writing O_t now
                 if (q == 0) TLOG(t, j, 2);
                 if (j + 1 < nkv) {                        // next tile's scores: in flight while the P stores drain
                     const uint32_t s_next = lane_addr + 128 * t + 64 * ((j + 1) & 1);
@@ -352,24 +359,23 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
                 __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(bar_p + 8 * (2 * t + (j & 1)));      // ... so P_t(j) V_j may overwrite it
+                if (lane == 0) ptx::mbar_arrive(bar_p + 8 * (2 * t + (j & 1)));      // P_t(j) (and the rescaled O_t) are in TMEM
                 ptx::tmem_ld_wait();
                 if (q == 0) TLOG(t, j, 4);
-                corr_prev = corr;
-                rsum_prev = rsum;
             }
-            // last tile's P V
+            // all products are in: O_t -> registers, normalise, store
             ptx::mbar_wait(bar_o + 8 * t, (nkv - 1) & 1);
             ptx::tc_fence_after();
-            fold_load();
+            uint32_t o_r[HD];
+#pragma unroll
+            for (int w = 0; w < HD / 16; ++w) ptx::tmem_ld16(o_addr + w * 16, *reinterpret_cast<uint32_t(*)[16]>(&o_r[w * 16]));
             ptx::tmem_ld_wait();
-            fold(corr_prev, rsum_prev);
             if (qrow < ev1) {
                 const float inv = l_run > 0.0f ? 1.0f / l_run : 0.0f;
                 uint32_t hi[HD / 2], lo[HD / 2];
 #pragma unroll
                 for (int i = 0; i < HD / 2; ++i) {
-                    const float y0 = acc[2 * i] * inv, y1 = acc[2 * i + 1] * inv;
+                    const float y0 = __uint_as_float(o_r[2 * i]) * inv, y1 = __uint_as_float(o_r[2 * i + 1]) * inv;
                     __nv_bfloat162 h2 = __floats2bfloat162_rn(y0, y1);
                     hi[i] = *reinterpret_cast<uint32_t*>(&h2);
                     __nv_bfloat162 l2 = __floats2bfloat162_rn(y0 - __low2float(h2), y1 - __high2float(h2));
