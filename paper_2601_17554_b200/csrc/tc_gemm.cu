@@ -61,6 +61,7 @@ int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, 
 
 // ------------------------------------------------------------------------------------------------ kernel
 constexpr int GEMM_BM = 128, GEMM_BK = 64;
+constexpr int GEMM_STG_BYTES = 4096;                           // per epilogue warp (see stg_f32 / stg_b16)
 constexpr int GEMM_THREADS = 576;                              // TMA, MMA, 4 x 4 epilogue warps
 
 template <int BLOCK_N, int STAGES, bool SPLIT>
@@ -68,7 +69,7 @@ struct GemmCfg {
     static constexpr int A_BYTES = GEMM_BM * GEMM_BK * 2;            // 16 KB per A term
     static constexpr int B_BYTES = BLOCK_N * GEMM_BK * 2;
     static constexpr int STAGE_BYTES = A_BYTES * (SPLIT ? 2 : 1) + B_BYTES;
-    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024;   // + slack for 1024 B alignment
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 16 * GEMM_STG_BYTES + 1024;   // ring + staging + alignment slack
     static constexpr int TMEM_COLS = 2 * BLOCK_N < 32 ? 32 : 2 * BLOCK_N;   // two accumulator buffers (power of 2)
 };
 
@@ -92,10 +93,45 @@ __device__ __forceinline__ float2 gelu2(float2 x) {
     return ptx::fadd2(make_float2(fmaxf(x.x, 0.0f), fmaxf(x.y, 0.0f)), h);
 }
 
-// epilogue of one 16-column chunk held in registers (thread = one row); bias_s = this chunk's bias in shared memory
+// ---- per-warp staging tile (4 KB of shared memory): the epilogue thread owns one ROW of the accumulator, so direct
+// global stores touch 32 different 128-byte lines per instruction (measured: ~1.6 TB/s for the whole GPU whatever
+// the output type).  Results (and the fp32 residual on the way in) go through this tile instead, so that every
+// global access of a warp covers whole 64- or 128-byte row segments.  Layouts, 16-byte pieces XOR-swizzled so that
+// both the row-wise (thread = row) and the coalesced (4 or 8 lanes per row) accesses are bank-conflict free:
+//   fp32: [32 rows][8 pieces of 4 floats]   piece p of row r at  r * 128 + ((p ^ (r & 7)) << 4)
+//   bf16: [32 rows][4 pieces of 8 bf16], hi at +0 and lo at +2048:  r * 64 + ((p ^ ((r >> 1) & 3)) << 4)
+__device__ __forceinline__ uint8_t* stg_f32(uint8_t* stg, int r, int p) { return stg + r * 128 + ((p ^ (r & 7)) << 4); }
+__device__ __forceinline__ uint8_t* stg_b16(uint8_t* stg, int r, int p) { return stg + r * 64 + ((p ^ ((r >> 1) & 3)) << 4); }
+
+// coalesced copy between the staging tile and global rows: local row rr lives at global row __shfl(row, rr) (< 0: skip)
+template <bool LOAD>
+__device__ __forceinline__ void stg_copy_f32(uint8_t* stg, float* g, int64_t ld, int col0, int row, int lane) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {                       // 4 rows x 128 B per instruction
+        const int rr = 4 * i + (lane >> 3), p = lane & 7;
+        const int grow = __shfl_sync(0xffffffffu, row, rr);
+        if (grow >= 0) {
+            float4* gp = reinterpret_cast<float4*>(g + (int64_t)grow * ld + col0) + p;
+            float4* sp = reinterpret_cast<float4*>(stg_f32(stg, rr, p));
+            if (LOAD) *sp = *gp; else *gp = *sp;
+        }
+    }
+}
+__device__ __forceinline__ void stg_flush_b16(uint8_t* stg, bf16* g, int64_t ld, int col0, int row, int lane) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {                       // 8 rows x 64 B per instruction
+        const int rr = 8 * i + (lane >> 2), p = lane & 3;
+        const int grow = __shfl_sync(0xffffffffu, row, rr);
+        if (grow >= 0)
+            *(reinterpret_cast<uint4*>(g + (int64_t)grow * ld + col0) + p) = *reinterpret_cast<uint4*>(stg_b16(stg, rr, p));
+    }
+}
+
+// epilogue of one 16-column chunk held in registers (thread = lane = one row); bias_s = this chunk's bias in shared
+// memory; cc = 0 / 1: which half of the 32-column staging group; results are left in the staging tile
 template <int ACT>
-__device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[16], const Epi& ep, const float* bias_s, int row,
-                                                    int n_base, bool row_ok) {
+__device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[16], const Epi& ep, const float* bias_s, uint8_t* stg,
+                                                    int lane, int cc) {
     float2 v[8];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
@@ -109,22 +145,18 @@ __device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[16], c
         if (ACT == ACT_GELU) v[j] = gelu2(v[j]);
         if (ACT == ACT_RELU) v[j] = make_float2(fmaxf(v[j].x, 0.0f), fmaxf(v[j].y, 0.0f));
     }
-    if (!row_ok) return;
-    if (ep.residual) {
-        const float4* rp = reinterpret_cast<const float4*>(ep.residual + (int64_t)row * ep.ld_res + n_base);
+    if (ep.out_f32) {                                   // fp32 result, optionally + fp32 residual staged in the same place
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const float4 r = rp[j];
-            v[2 * j] = ptx::fadd2(v[2 * j], make_float2(r.x, r.y));
-            v[2 * j + 1] = ptx::fadd2(v[2 * j + 1], make_float2(r.z, r.w));
+            float4* sp = reinterpret_cast<float4*>(stg_f32(stg, lane, 4 * cc + j));
+            if (ep.residual) {
+                const float4 r = *sp;
+                v[2 * j] = ptx::fadd2(v[2 * j], make_float2(r.x, r.y));
+                v[2 * j + 1] = ptx::fadd2(v[2 * j + 1], make_float2(r.z, r.w));
+            }
+            *sp = make_float4(v[2 * j].x, v[2 * j].y, v[2 * j + 1].x, v[2 * j + 1].y);
         }
-    }
-    if (ep.out_f32) {
-        float4* op = reinterpret_cast<float4*>(ep.out_f32 + (int64_t)row * ep.ld_f32 + n_base);
-#pragma unroll
-        for (int j = 0; j < 4; ++j) op[j] = make_float4(v[2 * j].x, v[2 * j].y, v[2 * j + 1].x, v[2 * j + 1].y);
-    }
-    if (ep.out_act) {
+    } else {                                            // bf16 result as hi (+ lo = T(v - hi))
         uint32_t hi[8], lo[8];
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
@@ -137,13 +169,11 @@ __device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[16], c
                 lo[j] = *reinterpret_cast<uint32_t*>(&l2);
             }
         }
-        uint4* op = reinterpret_cast<uint4*>((bf16*)ep.out_act + (int64_t)row * ep.ld_act + n_base);
 #pragma unroll
-        for (int j = 0; j < 2; ++j) op[j] = make_uint4(hi[4 * j], hi[4 * j + 1], hi[4 * j + 2], hi[4 * j + 3]);
-        if (ep.out_act_lo) {
-            uint4* lp = reinterpret_cast<uint4*>((bf16*)ep.out_act_lo + (int64_t)row * ep.ld_act + n_base);
-#pragma unroll
-            for (int j = 0; j < 2; ++j) lp[j] = make_uint4(lo[4 * j], lo[4 * j + 1], lo[4 * j + 2], lo[4 * j + 3]);
+        for (int j = 0; j < 2; ++j) {
+            *reinterpret_cast<uint4*>(stg_b16(stg, lane, 2 * cc + j)) = make_uint4(hi[4 * j], hi[4 * j + 1], hi[4 * j + 2], hi[4 * j + 3]);
+            if (ep.out_act_lo)
+                *reinterpret_cast<uint4*>(stg_b16(stg + 2048, lane, 2 * cc + j)) = make_uint4(lo[4 * j], lo[4 * j + 1], lo[4 * j + 2], lo[4 * j + 3]);
         }
     }
 }
@@ -247,6 +277,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         const int hcol = (ew >> 3) * (BLOCK_N / 2);
         const int q = warp & 3;                                   // TMEM lane quarter this warp may access
         const int tid = ((ew >> 3) * 4 + (ew & 3)) * 32 + lane;   // 0..255 among the threads serving buffer e
+        uint8_t* stg = smem_raw + (smem_base - ptx::smem_u32(smem_raw)) + STAGES * Cfg::STAGE_BYTES + ew * GEMM_STG_BYTES;
         int it = 0;
         for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
             const int m0 = (tile / n_tiles_n) * GEMM_BM, n0 = (tile % n_tiles_n) * BLOCK_N;
@@ -271,16 +302,28 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             ptx::mbar_wait(bar_acc_full + 8 * e, (it >> 1) & 1);
             ptx::tc_fence_after();
             const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + e * BLOCK_N + hcol;
+            const int srow = write_ok ? row : -1;                 // destination row of this lane's accumulator row
             uint32_t ra[16], rb[16];
             ptx::tmem_ld16(t_addr, ra);
 #pragma unroll
-            for (int c = 0; c < BLOCK_N / 2; c += 32) {           // two 16-column chunks per iteration, next load in flight
+            for (int c = 0; c < BLOCK_N / 2; c += 32) {           // one 32-column staging group per iteration
+                const int col0 = n0 + hcol + c;
+                if (ep.residual) stg_copy_f32<true>(stg, const_cast<float*>(ep.residual), ep.ld_res, col0, srow, lane);
                 ptx::tmem_ld_wait();
                 ptx::tmem_ld16(t_addr + c + 16, rb);
-                gemm_epilogue_chunk<ACT>(ra, ep, ep.bias ? &bias_s[e][hcol + c] : nullptr, row, n0 + hcol + c, write_ok);
+                __syncwarp();
+                gemm_epilogue_chunk<ACT>(ra, ep, ep.bias ? &bias_s[e][hcol + c] : nullptr, stg, lane, 0);
                 ptx::tmem_ld_wait();
                 if (c + 32 < BLOCK_N / 2) ptx::tmem_ld16(t_addr + c + 32, ra);
-                gemm_epilogue_chunk<ACT>(rb, ep, ep.bias ? &bias_s[e][hcol + c + 16] : nullptr, row, n0 + hcol + c + 16, write_ok);
+                gemm_epilogue_chunk<ACT>(rb, ep, ep.bias ? &bias_s[e][hcol + c + 16] : nullptr, stg, lane, 1);
+                __syncwarp();
+                if (ep.out_f32) {
+                    stg_copy_f32<false>(stg, ep.out_f32, ep.ld_f32, col0, srow, lane);
+                } else {
+                    stg_flush_b16(stg, (bf16*)ep.out_act, ep.ld_act, col0, srow, lane);
+                    if (ep.out_act_lo) stg_flush_b16(stg + 2048, (bf16*)ep.out_act_lo, ep.ld_act, col0, srow, lane);
+                }
+                __syncwarp();
             }
             ptx::tc_fence_before();
             __syncwarp();
@@ -328,14 +371,17 @@ static int tc_gemm_launch_cfg(TcContext* c, const bf16* A, const bf16* A_lo, con
 
 int tc_gemm_launch(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W, int M, int N, int K,
                           const Epi& ep, cudaStream_t st) {
+    if (ep.out_f32 ? (ep.out_act != nullptr) : (ep.out_act == nullptr || ep.residual != nullptr)) {
+        snprintf(c->err, sizeof c->err, "tc_gemm: the epilogue writes either fp32 (+ residual) or bf16 hi (+ lo)"); return -1;
+    }
     if (N % 64 || K % 64) { snprintf(c->err, sizeof c->err, "tc_gemm: N=%d, K=%d must be multiples of 64", N, K); return -1; }
     const int w_rows = ep.group_offsets ? ep.n_groups * N : N;
     if (N % 128 == 0) {
-        return A_lo ? tc_gemm_launch_cfg<128, 4, true>(c, A, A_lo, W, M, N, K, w_rows, ep, st)
-                    : tc_gemm_launch_cfg<128, 6, false>(c, A, nullptr, W, M, N, K, w_rows, ep, st);
+        return A_lo ? tc_gemm_launch_cfg<128, 3, true>(c, A, A_lo, W, M, N, K, w_rows, ep, st)
+                    : tc_gemm_launch_cfg<128, 4, false>(c, A, nullptr, W, M, N, K, w_rows, ep, st);
     }
-    return A_lo ? tc_gemm_launch_cfg<64, 5, true>(c, A, A_lo, W, M, N, K, w_rows, ep, st)
-                : tc_gemm_launch_cfg<64, 8, false>(c, A, nullptr, W, M, N, K, w_rows, ep, st);
+    return A_lo ? tc_gemm_launch_cfg<64, 3, true>(c, A, A_lo, W, M, N, K, w_rows, ep, st)
+                : tc_gemm_launch_cfg<64, 5, false>(c, A, nullptr, W, M, N, K, w_rows, ep, st);
 }
 
 }  // namespace mlpf
