@@ -117,7 +117,7 @@ __global__ void __launch_bounds__(256)
 k_embed_l1(const float* __restrict__ X, int N, int F, int d, const float* __restrict__ W1t,
            const float* __restrict__ b1, int act, const int* __restrict__ sorted_row,
            T* __restrict__ h1, T* __restrict__ h1_lo, float* __restrict__ h) {
-    __shared__ float xs[EMB_ROWS][65];
+    __shared__ __align__(16) float xs[EMB_ROWS][64];        // rows are read as broadcast 128-bit loads (no padding needed)
     __shared__ int list[5][EMB_ROWS];
     __shared__ int cnt[5];
     const int row0 = blockIdx.x * EMB_ROWS;
@@ -151,8 +151,13 @@ k_embed_l1(const float* __restrict__ X, int N, int F, int d, const float* __rest
             for (int p = 0; p < c; ++p) {
                 const int r = list[t][p];
                 float acc = bj;
+                const float4* xr = reinterpret_cast<const float4*>(xs[r]);
 #pragma unroll
-                for (int k = 0; k < 64; ++k) acc = fmaf(w[k], xs[r][k], acc);
+                for (int k = 0; k < 16; ++k) {          // one LDS.128 per four FMAs (the scalar form was LDS-bound)
+                    const float4 x4 = xr[k];
+                    acc = fmaf(w[4 * k], x4.x, acc); acc = fmaf(w[4 * k + 1], x4.y, acc);
+                    acc = fmaf(w[4 * k + 2], x4.z, acc); acc = fmaf(w[4 * k + 3], x4.w, acc);
+                }
                 int slot = sorted_row[row0 + r];
                 const float a = apply_act(acc, act);
                 const T hi = from_f32<T>(a);
@@ -377,6 +382,62 @@ k_heads_l2(const T* __restrict__ hidden, const T* __restrict__ hidden_lo, int N,
     }
 }
 
+// a8 output layer, bf16 path: the same computation with 128-bit loads (lane = 8 consecutive hidden units per 256-wide
+// chunk, d <= 512, at most 5 head blocks): all of the row's hidden vectors (hi + lo) are requested up front (one
+// round trip to HBM), then each is reused by all outputs of its block.
+template <int NCH>
+__global__ void __launch_bounds__(256)
+k_heads_l2_vec(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden_lo, int N, int d, int ld_hidden, int n_blk,
+               const float* __restrict__ W2, const float* __restrict__ b2, const int* __restrict__ valid, HeadsOut ho,
+               float* __restrict__ out_logits, float* __restrict__ out_regress) {
+    const int row = blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (row >= N) return;
+    const bool ok = valid[row] != 0;
+    uint4 hraw[5][NCH], lraw[5][NCH];
+#pragma unroll
+    for (int b = 0; b < 5; ++b)
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch) {
+            const int c = ch * 256 + lane * 8;
+            hraw[b][ch] = make_uint4(0, 0, 0, 0); lraw[b][ch] = make_uint4(0, 0, 0, 0);
+            if (ok && b < n_blk && c < d) {
+                const int64_t off = (int64_t)row * ld_hidden + b * d + c;
+                hraw[b][ch] = *reinterpret_cast<const uint4*>(hidden + off);
+                if (hidden_lo) lraw[b][ch] = *reinterpret_cast<const uint4*>(hidden_lo + off);
+            }
+        }
+    for (int o = 0; o < ho.n_out; ++o) {
+        float a = 0.0f;
+        if (ok) {
+            const int b = ho.blk[o];
+#pragma unroll
+            for (int ch = 0; ch < NCH; ++ch) {
+                const int c = ch * 256 + lane * 8;
+                if (c < d) {
+                    uint4 h4 = hraw[0][ch], l4 = lraw[0][ch];
+#pragma unroll
+                    for (int bb = 1; bb < 5; ++bb) if (b == bb) { h4 = hraw[bb][ch]; l4 = lraw[bb][ch]; }
+                    const uint32_t hw[4] = {h4.x, h4.y, h4.z, h4.w}, lw[4] = {l4.x, l4.y, l4.z, l4.w};
+                    const float4* wp = reinterpret_cast<const float4*>(W2 + (int64_t)o * d + c);
+                    const float4 w0 = __ldg(wp), w1 = __ldg(wp + 1);
+                    const float wv[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        a = fmaf(__uint_as_float(hw[i] << 16) + __uint_as_float(lw[i] << 16), wv[2 * i], a);
+                        a = fmaf(__uint_as_float(hw[i] & 0xffff0000u) + __uint_as_float(lw[i] & 0xffff0000u), wv[2 * i + 1], a);
+                    }
+                }
+            }
+            a = warp_sum(a) + b2[o];
+        }
+        if (lane == 0) {
+            if (o < ho.n_cls) out_logits[(int64_t)row * ho.n_cls + o] = a;
+            else out_regress[(int64_t)row * ho.n_reg + (o - ho.n_cls)] = a;
+        }
+    }
+}
+
 // fp32 <- T conversion for the debug taps
 template <typename T>
 __global__ void k_to_f32(const T* __restrict__ src, float* __restrict__ dst, int64_t n) {
@@ -453,6 +514,11 @@ void launch_heads_l2(bool fp32, const void* hidden, const void* hidden_lo, int N
                      float* out_regress, cudaStream_t st) {
     dim3 grid((N + 7) / 8);
     if (fp32) k_heads_l2<float><<<grid, 256, 0, st>>>((const float*)hidden, (const float*)hidden_lo, N, d, ld_hidden, W2, b2, valid, ho, out_logits, out_regress);
+    else if (d <= 512 && d % 8 == 0 && ld_hidden % 8 == 0 && ld_hidden / d <= 5) {
+        const int n_blk = ld_hidden / d;
+        if (d <= 256) k_heads_l2_vec<1><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress);
+        else k_heads_l2_vec<2><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress);
+    }
     else k_heads_l2<bf16><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, W2, b2, valid, ho, out_logits, out_regress);
 }
 
