@@ -40,10 +40,12 @@ struct AttnCfg {
     static constexpr int V_BYTES = ATT_SK * HD * 2;
     static constexpr int STAGE_BYTES = K_BYTES + V_BYTES;
     static constexpr int STAGES = HD == 64 ? 4 : 6;
-    static constexpr int SMEM_BYTES = NT * Q_BYTES + STAGES * STAGE_BYTES + 1024;
+    static constexpr int ONES_BYTES = 1024;                 // bf16 1.0: B operand of the row-sum MMA (any layout reads ones)
+    static constexpr int OW = HD + 8;                       // TMEM columns per query tile: O (hd) + row sums (8 equal columns)
+    static constexpr int SMEM_BYTES = NT * Q_BYTES + STAGES * STAGE_BYTES + ONES_BYTES + 1024;
     static constexpr int SW = HD * 2;                       // swizzle width of Q / K / V rows in bytes
     static constexpr int O_COL0 = 128 * NT;
-    static_assert(O_COL0 + NT * HD <= 512, "TMEM budget");
+    static_assert(O_COL0 + NT * OW <= 512, "TMEM budget");
 };
 
 int tc_attn_rows_per_cta(int hd) { return (hd <= 32 ? 3 : 2) * ATT_BQ; }
@@ -95,10 +97,9 @@ __device__ __forceinline__ float2 exp2_poly2(float2 x) {
 #endif                       // 3rd 0.846, 2nd 0.927 (with register spills in the loop it was a loss at every setting)
 
 
-// p = 2^(s c - m c) for 32 scores -> 16 bf16 pairs; their fp32 sums go to two packed accumulators (short chains)
+// p = 2^(s c - m c) for 32 scores -> 16 bf16 pairs (the row sums come from the tensor pipe: P x 1)
 template <bool FULL>
-__device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c, float neg_mc, uint32_t (&pk)[16],
-                                      float2 (&rs)[2]) {
+__device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c, float neg_mc, uint32_t (&pk)[16]) {
     const float2 c2 = make_float2(c, c), m2 = make_float2(neg_mc, neg_mc);
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
@@ -110,14 +111,13 @@ __device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c,
             p.x = (mask >> (2 * i)) & 1u ? p.x : 0.0f;
             p.y = (mask >> (2 * i + 1)) & 1u ? p.y : 0.0f;
         }
-        rs[i & 1] = ptx::fadd2(rs[i & 1], p);
         __nv_bfloat162 b2 = __floats2bfloat162_rn(p.x, p.y);
         pk[i] = *reinterpret_cast<uint32_t*>(&b2);
     }
 }
 
 // One 64-key tile of one query row, scores already in registers s[0..63]:
-// P = 2^((S - m_ref) c) as bf16, written over S's first 32 TMEM columns at s_addr, row sum of P in rsum.
+// P = 2^((S - m_ref) c) as bf16, written over S's first 32 TMEM columns at s_addr.
 // m_ref is a STALE reference maximum (lazy rescaling): it only moves when some row of the warp has a tile maximum
 // more than ATT_RESCALE_LOG2 (in log2 units) above it, so P <= 2^8 and neither bf16 P nor the fp32 sums lose
 // precision, while the accumulated O (in TMEM) has to be rescaled only a few times per row instead of every tile.
@@ -125,7 +125,7 @@ __device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c,
 constexpr float ATT_RESCALE_LOG2 = 8.0f;
 template <bool FULL>
 __device__ __forceinline__ float softmax_tile(const uint32_t (&s)[64], uint32_t s_addr, const uint32_t (&mask)[2], float c,
-                                              float& m_ref, float& rsum, bool& rescale) {
+                                              float& m_ref, bool& rescale) {
     const float mx = fmaxf(max32<FULL>(&s[0], mask[0], -INFINITY), max32<FULL>(&s[32], mask[1], -INFINITY));
     const float m_new = fmaxf(m_ref, mx);
     // m_ref = -inf and a finite tile maximum: the difference is +inf and votes yes; all keys masked so far: nan -> no
@@ -137,14 +137,12 @@ __device__ __forceinline__ float softmax_tile(const uint32_t (&s)[64], uint32_t 
         m_ref = m_new;
     }
     const float neg_mc = (m_ref == -INFINITY) ? 0.0f : -m_ref * c;
-    float2 rs[2] = {make_float2(0.0f, 0.0f), make_float2(0.0f, 0.0f)};
 #pragma unroll
     for (int w = 0; w < 2; ++w) {
         uint32_t pk[16];
-        exp32<FULL>(&s[32 * w], mask[w], c, neg_mc, pk, rs);
+        exp32<FULL>(&s[32 * w], mask[w], c, neg_mc, pk);
         ptx::tmem_st16(s_addr + 16 * w, pk);
     }
-    rsum = (rs[0].x + rs[0].y) + (rs[1].x + rs[1].y);
     return corr;
 }
 
@@ -177,6 +175,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t sQ = smem_base;                                  // Q tiles
     const uint32_t sKV = smem_base + NT * Cfg::Q_BYTES;
+    const uint32_t sOnes = sKV + ST * Cfg::STAGE_BYTES;
     const uint32_t bar_q = ptx::smem_u32(&bars[0]);
     const uint32_t bar_kv_full = ptx::smem_u32(&bars[1]);
     const uint32_t bar_kv_empty = ptx::smem_u32(&bars[1 + ST]);
@@ -201,6 +200,11 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     if (warp == Cfg::WARP_MMA) {
         ptx::tmem_alloc(ptx::smem_u32(&tmem_base_slot), 512);
         ptx::tmem_relinquish();
+    }
+    if (warp < 4 * NT) {
+        for (int i = threadIdx.x; i < Cfg::ONES_BYTES / 4; i += 4 * NT * 32)
+            asm volatile("st.shared.b32 [%0], %1;" ::"r"(sOnes + 4 * i), "r"(0x3f803f80u) : "memory");
+        ptx::fence_proxy_async();                                    // generic-proxy writes -> visible to the MMA
     }
     ptx::tc_fence_before();
     __syncthreads();
@@ -232,6 +236,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
         const int t = warp - Cfg::WARP_MMA;
         constexpr uint32_t idesc_s = ptx::umma_idesc_bf16(128, ATT_BK);
         constexpr uint32_t idesc_o = ptx::umma_idesc_bf16(128, HD) | ptx::UMMA_B_MN_MAJOR;
+        constexpr uint32_t idesc_l = ptx::umma_idesc_bf16(128, 8);
         constexpr uint32_t HALF = ATT_BK * Cfg::SW;                  // bytes of a 64-key half of a K or V stage
         auto issue_s = [&](int j) {                 // S_t(j) = Q_t K_j^T -> S buffer j & 1
             const uint32_t kb = sKV + ((j >> 1) % ST) * Cfg::STAGE_BYTES + (j & 1) * HALF;
@@ -246,8 +251,13 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
             const uint32_t vb = sKV + ((j >> 1) % ST) * Cfg::STAGE_BYTES + Cfg::K_BYTES + (j & 1) * HALF;
 #pragma unroll
             for (int k = 0; k < ATT_BK / 16; ++k)
-                ptx::mma_ts(tmem_base + Cfg::O_COL0 + HD * t, tmem_base + 128 * t + 64 * (j & 1) + k * 8,
+                ptx::mma_ts(tmem_base + Cfg::O_COL0 + Cfg::OW * t, tmem_base + 128 * t + 64 * (j & 1) + k * 8,
                             ptx::umma_desc_mnmajor(vb + k * 16 * Cfg::SW, Cfg::SW), idesc_o, (j | k) != 0);
+            const uint64_t ones = ptx::umma_desc_kmajor(sOnes, 128);      // row sums l_t += P_t(j) 1 next to O_t
+#pragma unroll
+            for (int k = 0; k < ATT_BK / 16; ++k)
+                ptx::mma_ts(tmem_base + Cfg::O_COL0 + Cfg::OW * t + HD, tmem_base + 128 * t + 64 * (j & 1) + k * 8, ones, idesc_l,
+                            (j | k) != 0);
             ptx::mma_commit(bar_o + 8 * t);
         };
         ptx::mbar_wait(bar_q, 0);
@@ -281,13 +291,15 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
         const int qrow = q0 + t * ATT_BQ + q * 32 + lane;
         if (t < nt) {
             const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16);
-            const uint32_t o_addr = lane_addr + Cfg::O_COL0 + HD * t;
+            const uint32_t o_addr = lane_addr + Cfg::O_COL0 + Cfg::OW * t;
             const float c = prm.scale_log2;
-            float m_ref = -INFINITY, l_run = 0.0f;
+            float m_ref = -INFINITY;
             // O_t *= corr in TMEM (all 32 lanes of the warp, rows that did not move have corr = 1): only when the
             // warp's reference maximum moved, which happens a few times per row (lazy rescaling)
             auto rescale_o = [&](float corr) {
                 const float2 c2 = make_float2(corr, corr);
+                uint32_t lsum;
+                ptx::tmem_ld1(o_addr + HD, lsum);                 // the row sum (column hd; columns hd+1.. are copies)
 #pragma unroll
                 for (int c0 = 0; c0 < HD; c0 += 32) {
                     constexpr int CH = HD < 32 ? HD : 32;
@@ -302,6 +314,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                     }
 #pragma unroll
                     for (int w = 0; w < CH / 16; ++w) ptx::tmem_st16(o_addr + c0 + w * 16, *reinterpret_cast<uint32_t(*)[16]>(&r[w * 16]));
+                    if (c0 == 0) ptx::tmem_st1(o_addr + HD, __float_as_uint(__uint_as_float(lsum) * corr));
                 }
             };
             // scores of the current tile live in registers; the next tile's are loaded while this one is finished
@@ -334,11 +347,9 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                 }
                 const uint32_t s_addr = lane_addr + 128 * t + 64 * (j & 1);
                 if (q == 0) TLOG(t, j, 0);
-                float rsum;
                 bool rescale;
-                const float corr = full ? softmax_tile<true>(s, s_addr, mask, c, m_ref, rsum, rescale)
-                                        : softmax_tile<false>(s, s_addr, mask, c, m_ref, rsum, rescale);
-                l_run = fmaf(l_run, corr, rsum);
+                const float corr = full ? softmax_tile<true>(s, s_addr, mask, c, m_ref, rescale)
+                                        : softmax_tile<false>(s, s_addr, mask, c, m_ref, rescale);
                 if (q == 0) TLOG(t, j, 1);
                 // S_t(j+1) was issued after P_t(j-1) V_(j-1) and the tensor pipe completes in order: once S_t(j+1) has
                 // landed, O_t holds all products up to j-1.  Only the last tile has to wait on bar_o for that.
@@ -369,8 +380,11 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
             uint32_t o_r[HD];
 #pragma unroll
             for (int w = 0; w < HD / 16; ++w) ptx::tmem_ld16(o_addr + w * 16, *reinterpret_cast<uint32_t(*)[16]>(&o_r[w * 16]));
+            uint32_t lsum;
+            ptx::tmem_ld1(o_addr + HD, lsum);
             ptx::tmem_ld_wait();
             if (qrow < ev1) {
+                const float l_run = __uint_as_float(lsum);
                 const float inv = l_run > 0.0f ? 1.0f / l_run : 0.0f;
                 uint32_t hi[HD / 2], lo[HD / 2];
 #pragma unroll
