@@ -54,6 +54,7 @@ struct Workspace {
     int64_t g_elems = 0;
     // schedule (a0)
     int *offsets = nullptr, *work = nullptr, *pairs = nullptr;
+    uint32_t* valid_bits = nullptr;   // one bit per row (a0), the attention kernel's key mask
     int *valid = nullptr, *row_event = nullptr, *row_pos = nullptr, *n_valid = nullptr;
     int *block_counts = nullptr, *block_base = nullptr, *type_offsets = nullptr;
     int *sorted_row = nullptr, *type_perm = nullptr;
@@ -200,7 +201,7 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
 }
 
 static void ws_free(Workspace* w) {
-    void* ptrs[] = {w->h, w->u, w->qkv, w->o, w->g, w->u_lo, w->o_lo, w->g_lo, w->offsets, w->work, w->pairs, w->valid, w->row_event,
+    void* ptrs[] = {w->h, w->u, w->qkv, w->o, w->g, w->u_lo, w->o_lo, w->g_lo, w->offsets, w->work, w->pairs, w->valid, w->valid_bits, w->row_event,
                     w->row_pos, w->n_valid, w->block_counts, w->block_base, w->type_offsets, w->sorted_row, w->type_perm};
     for (void* p : ptrs) if (p) cudaFree(p);
 }
@@ -272,7 +273,7 @@ template <typename P> static cudaError_t dmalloc(P** p, int64_t bytes, Workspace
 static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t n_tiles, bool fp32) {
     const int64_t d = h->d;
     if (N > w->cap_rows || fp32 != w->fp32) {
-        void* ptrs[] = {w->h, w->u, w->qkv, w->o, w->g, w->u_lo, w->o_lo, w->g_lo, w->valid, w->row_event, w->row_pos, w->block_counts,
+        void* ptrs[] = {w->h, w->u, w->qkv, w->o, w->g, w->u_lo, w->o_lo, w->g_lo, w->valid, w->valid_bits, w->row_event, w->row_pos, w->block_counts,
                         w->block_base, w->sorted_row, w->type_perm, w->type_offsets};
         for (void* p : ptrs) if (p) cudaFree(p);   // cudaFree waits for work in flight
         // keep the event-indexed arrays' accounting: recompute bytes from scratch
@@ -292,7 +293,7 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
             dmalloc((char**)&w->o, cap * d * es, w) || dmalloc((char**)&w->g, w->g_elems * es, w) ||
             dmalloc((char**)&w->u_lo, cap * d * es, w) || dmalloc((char**)&w->o_lo, cap * d * es, w) ||
             dmalloc((char**)&w->g_lo, w->g_elems * es, w) ||
-            dmalloc(&w->valid, cap * 4, w) || dmalloc(&w->row_event, cap * 4, w) || dmalloc(&w->row_pos, cap * 4, w) ||
+            dmalloc(&w->valid, cap * 4, w) || dmalloc(&w->valid_bits, (cap / 32 + 40) * 4, w) || dmalloc(&w->row_event, cap * 4, w) || dmalloc(&w->row_pos, cap * 4, w) ||
             dmalloc(&w->block_counts, nb * 5 * 4, w) || dmalloc(&w->block_base, nb * 5 * 4, w) ||
             dmalloc(&w->sorted_row, cap * 4, w) || dmalloc(&w->type_perm, m_ub * 4, w) ||
             dmalloc(&w->type_offsets, 8 * 4, w)) {
@@ -302,6 +303,7 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
         }
         // the activation buffers feed TMA loads whose boxes may overrun valid rows: start from zeros so
         // that never-written tails hold finite values
+        cudaMemset(w->valid_bits, 0, (cap / 32 + 40) * 4);
         cudaMemset(w->u, 0, cap * d * es); cudaMemset(w->qkv, 0, cap * 3 * d * es);
         cudaMemset(w->o, 0, cap * d * es);
         cudaMemset(w->g, 0, w->g_elems * es);
@@ -374,7 +376,7 @@ static int run_layernorm(mlpf_handle* h, bool fp32, const float* x, int N, const
 static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspace* w, cudaStream_t st) {
     if (w->n_tiles == 0) return MLPF_OK;
     if (tc && !fp32) {
-        int rc = tc_attn_launch(&h->tc, (const bf16*)w->qkv, w->N, w->valid, w->n_valid, w->offsets,
+        int rc = tc_attn_launch(&h->tc, (const bf16*)w->qkv, w->N, w->valid_bits, w->n_valid, w->offsets,
                                 (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, (bf16*)w->o,
                                 split ? (bf16*)w->o_lo : nullptr, st);
         if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", h->tc.err);
@@ -421,7 +423,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     ProfScope ps(h, w, st, MLPF_KC_SCHED);
     CUDA_TRY(cudaMemsetAsync(w->n_valid, 0, (size_t)E * 4, st));
     CUDA_TRY(cudaMemsetAsync(w->type_perm, 0xff, (size_t)w->m_ub * 4, st));
-    h->last_launches += launch_schedule(X, N, h->F, w->offsets, E, w->block_counts, w->block_base, w->valid, w->row_event,
+    h->last_launches += launch_schedule(X, N, h->F, w->offsets, E, w->block_counts, w->block_base, w->valid, w->valid_bits, w->row_event,
                                         w->row_pos, w->n_valid, w->type_offsets, w->sorted_row, w->type_perm, st) - 1;
     LAUNCH_CHECK(h);
     }
@@ -703,14 +705,20 @@ extern "C" int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_va
     if (pairs.empty()) return MLPF_OK;
     cudaStream_t st = (cudaStream_t)stream;
     int *d_off = nullptr, *d_pairs = nullptr;
+    uint32_t* d_bits = nullptr;
+    if (key_valid) {
+        CUDA_TRY(cudaMalloc(&d_bits, (size_t)(N / 32 + 8) * 4));
+        CUDA_TRY(cudaMemsetAsync(d_bits, 0, (size_t)(N / 32 + 8) * 4, st));
+        launch_pack_valid_bits(key_valid, (int)N, d_bits, st);
+    }
     CUDA_TRY(cudaMalloc(&d_off, (size_t)(n_events + 1) * 4));
     CUDA_TRY(cudaMalloc(&d_pairs, pairs.size() * 4));
     CUDA_TRY(cudaMemcpyAsync(d_off, event_offsets, (size_t)(n_events + 1) * 4, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(d_pairs, pairs.data(), pairs.size() * 4, cudaMemcpyHostToDevice, st));
-    int rc = tc_attn_launch(&ctx, (const bf16*)QKV, N, key_valid, nullptr, d_off, (const int2*)d_pairs,
+    int rc = tc_attn_launch(&ctx, (const bf16*)QKV, N, d_bits, nullptr, d_off, (const int2*)d_pairs,
                             (int)(pairs.size() / 2), d_model, n_heads, (bf16*)O, (bf16*)nullptr, st);
     cudaError_t e = cudaStreamSynchronize(st);
-    cudaFree(d_off); cudaFree(d_pairs);
+    cudaFree(d_off); cudaFree(d_pairs); cudaFree(d_bits);
     if (rc) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", ctx.err);
     if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tcgen05 attention failed: %s", cudaGetErrorString(e));
     return MLPF_OK;

@@ -15,7 +15,7 @@ struct HeadsOut {
 
 // a0 device half: 3 launches.  Returns the number of kernels launched.
 int launch_schedule(const float* X, int N, int F, const int* offsets, int E, int* block_counts, int* block_base,
-                    int* valid, int* row_event, int* row_pos, int* n_valid, int* type_offsets, int* sorted_row,
+                    int* valid, uint32_t* valid_bits, int* row_event, int* row_pos, int* n_valid, int* type_offsets, int* sorted_row,
                     int* type_perm, cudaStream_t st);
 void launch_embed_l1(bool fp32, const float* X, int N, int F, int d, const float* W1t, const float* b1, int act,
                      const int* sorted_row, void* h1, void* h1_lo, float* h, cudaStream_t st);
@@ -29,6 +29,8 @@ void launch_attn_simple(bool fp32, int hd, const void* QKV, const int* key_valid
 void launch_heads_l2(bool fp32, const void* hidden, const void* hidden_lo, int N, int d, int ld_hidden,
                      const float* W2, const float* b2, const int* valid, const HeadsOut& ho, float* out_logits,
                      float* out_regress, cudaStream_t st);
+// bits[i / 32] bit (i % 32) = valid[i] != 0; `bits` holds (N + 31) / 32 words (+ 3 zero words for the attention kernel)
+void launch_pack_valid_bits(const int* valid, int N, uint32_t* bits, cudaStream_t st);
 void launch_to_f32(bool fp32, const void* src, float* dst, int64_t n, cudaStream_t st);
 
 }  // namespace mlpf

@@ -21,8 +21,8 @@ __device__ __forceinline__ int element_type(const float* __restrict__ X, int64_t
 // per 1024-row block: histogram of types 0..4; also valid[], row_event[], row_pos[], n_valid[e] (atomic)
 __global__ void __launch_bounds__(SCHED_BLOCK)
 k_sched_count(const float* __restrict__ X, int N, int F, const int* __restrict__ offsets, int E,
-              int* __restrict__ block_counts, int* __restrict__ valid, int* __restrict__ row_event,
-              int* __restrict__ row_pos, int* __restrict__ n_valid) {
+              int* __restrict__ block_counts, int* __restrict__ valid, uint32_t* __restrict__ valid_bits,
+              int* __restrict__ row_event, int* __restrict__ row_pos, int* __restrict__ n_valid) {
     __shared__ int hist[5];
     if (threadIdx.x < 5) hist[threadIdx.x] = 0;
     __syncthreads();
@@ -40,6 +40,10 @@ k_sched_count(const float* __restrict__ X, int N, int F, const int* __restrict__
         row_event[i] = lo;
         row_pos[i] = i - offsets[lo];
         if (t != 0) atomicAdd(&n_valid[lo], 1);
+    }
+    {   // one bit per row, 32 rows per word (rows >= N: 0): the attention kernel's key mask
+        const unsigned vb = __ballot_sync(0xffffffffu, t > 0);
+        if ((threadIdx.x & 31) == 0) valid_bits[i >> 5] = vb;
     }
 #pragma unroll
     for (int ty = 0; ty < 5; ++ty) {
@@ -438,6 +442,16 @@ k_heads_l2_vec(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden_
     }
 }
 
+// int 0/1 per row -> one bit per row (kernel-level attention entry; the model path gets the bits from k_sched_count)
+__global__ void k_pack_valid_bits(const int* __restrict__ valid, int N, uint32_t* __restrict__ bits) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned vb = __ballot_sync(0xffffffffu, i < N && valid[i] != 0);
+    if ((threadIdx.x & 31) == 0) bits[i >> 5] = vb;
+}
+void launch_pack_valid_bits(const int* valid, int N, uint32_t* bits, cudaStream_t st) {
+    k_pack_valid_bits<<<(N + 255) / 256, 256, 0, st>>>(valid, N, bits);
+}
+
 // fp32 <- T conversion for the debug taps
 template <typename T>
 __global__ void k_to_f32(const T* __restrict__ src, float* __restrict__ dst, int64_t n) {
@@ -447,10 +461,10 @@ __global__ void k_to_f32(const T* __restrict__ src, float* __restrict__ dst, int
 
 // ------------------------------------------------------------------------------------------------ launchers
 int launch_schedule(const float* X, int N, int F, const int* offsets, int E, int* block_counts, int* block_base,
-                    int* valid, int* row_event, int* row_pos, int* n_valid, int* type_offsets, int* sorted_row,
+                    int* valid, uint32_t* valid_bits, int* row_event, int* row_pos, int* n_valid, int* type_offsets, int* sorted_row,
                     int* type_perm, cudaStream_t st) {
     const int nb = (N + SCHED_BLOCK - 1) / SCHED_BLOCK;
-    k_sched_count<<<nb, SCHED_BLOCK, 0, st>>>(X, N, F, offsets, E, block_counts, valid, row_event, row_pos, n_valid);
+    k_sched_count<<<nb, SCHED_BLOCK, 0, st>>>(X, N, F, offsets, E, block_counts, valid, valid_bits, row_event, row_pos, n_valid);
     k_sched_scan<<<1, 32, 0, st>>>(block_counts, nb, block_base, type_offsets);
     k_sched_scatter<<<nb, SCHED_BLOCK, 0, st>>>(X, N, F, block_base, type_offsets, sorted_row, type_perm);
     return 3;

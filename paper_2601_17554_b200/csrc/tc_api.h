@@ -43,9 +43,10 @@ int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, 
 int tc_gemm_launch(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W, int M, int N, int K,
                    const Epi& ep, cudaStream_t st);
 // QKV [N, 3d] row-major bf16 (q | k | v).  items = (event, group) per CTA row group of tc_attn_rows_per_cta(hd)
-// query rows; n_valid [E] (valid rows per event) may be null.
+// query rows; valid_bits: one bit per row (32 rows per word, 3 readable words past the last row's), null = all rows
+// valid; n_valid [E] (valid rows per event) may be null.
 int tc_attn_rows_per_cta(int hd);
-int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const int* key_valid, const int* n_valid,
+int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const uint32_t* valid_bits, const int* n_valid,
                    const int* offsets, const int2* items, int n_items, int d, int H, bf16* O, bf16* O_lo,
                    cudaStream_t st);
 

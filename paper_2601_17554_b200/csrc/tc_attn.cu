@@ -51,7 +51,7 @@ struct AttnCfg {
 int tc_attn_rows_per_cta(int hd) { return (hd <= 32 ? 3 : 2) * ATT_BQ; }
 
 struct AttnParams {
-    const int* key_valid;      // [N] or null
+    const uint32_t* valid_bits; // one bit per row, 32 rows per word (3 readable words past the last row's), or null
     const int* n_valid;        // [E] valid rows per event, or null: events without pad rows skip the key_valid loads
     const int* offsets;        // [E+1]
     const int2* items;         // (event, index of the group of NT query tiles)
@@ -170,7 +170,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     const int nt = min(NT, (ev1 - q0 + ATT_BQ - 1) / ATT_BQ);        // query tiles that hold rows of the event (>= 1)
     const int nkv = (ev1 - ev0 + ATT_BK - 1) / ATT_BK;              // 64-key tiles
     const int nst = (ev1 - ev0 + ATT_SK - 1) / ATT_SK;              // 128-key TMA stages
-    const int* key_valid = (prm.key_valid && !(prm.n_valid && prm.n_valid[it.x] == ev1 - ev0)) ? prm.key_valid : nullptr;
+    const uint32_t* valid_bits = (prm.valid_bits && !(prm.n_valid && prm.n_valid[it.x] == ev1 - ev0)) ? prm.valid_bits : nullptr;
 
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t sQ = smem_base;                                  // Q tiles
@@ -329,17 +329,19 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
             load_s(0);
             ptx::tmem_ld_wait();
             for (int j = 0; j < nkv; ++j) {
-                // key mask of this tile: 2 x 32 bits, computed redundantly per warp (no cross-warp sync)
+                // key mask of this tile: 64 bits = (in the event) & (valid row), from the schedule's bit array
                 const int k0 = ev0 + j * ATT_BK;
                 uint32_t mask[2];
                 bool full = k0 + ATT_BK <= ev1;
-                if (!full || key_valid) {
-#pragma unroll
-                    for (int w = 0; w < 2; ++w) {
-                        const int key = k0 + w * 32 + lane;
-                        bool ok = key < ev1;
-                        if (ok && key_valid) ok = key_valid[key] != 0;
-                        mask[w] = __ballot_sync(0xffffffffu, ok);
+                if (!full || valid_bits) {
+                    const int left = min(ev1 - k0, ATT_BK);                     // 1 .. 64 keys of the event in this tile
+                    mask[0] = left >= 32 ? 0xffffffffu : (1u << left) - 1u;
+                    mask[1] = left >= 64 ? 0xffffffffu : (left <= 32 ? 0u : (1u << (left - 32)) - 1u);
+                    if (valid_bits) {
+                        const uint32_t* wp = valid_bits + (k0 >> 5);            // warp-uniform loads
+                        const uint32_t w0 = __ldg(wp), w1 = __ldg(wp + 1), w2 = __ldg(wp + 2);
+                        mask[0] &= __funnelshift_r(w0, w1, k0 & 31);
+                        mask[1] &= __funnelshift_r(w1, w2, k0 & 31);
                     }
                     full = (mask[0] & mask[1]) == 0xffffffffu;
                 } else {
@@ -446,12 +448,12 @@ static int tc_attn_launch_hd(TcContext* c, const bf16* QKV, int64_t N, AttnParam
 }
 
 // items: (event, group index) pairs, one per CTA-row-group of tc_attn_rows_per_cta(hd) query rows
-int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const int* key_valid, const int* n_valid,
+int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const uint32_t* valid_bits, const int* n_valid,
                           const int* offsets, const int2* items, int n_items, int d, int H, bf16* O, bf16* O_lo,
                           cudaStream_t st) {
     const int hd = d / H;
     AttnParams prm;
-    prm.key_valid = key_valid; prm.n_valid = n_valid; prm.offsets = offsets; prm.items = items; prm.n_items = n_items;
+    prm.valid_bits = valid_bits; prm.n_valid = n_valid; prm.offsets = offsets; prm.items = items; prm.n_items = n_items;
     prm.H = H; prm.d = d; prm.O = O; prm.O_lo = O_lo;
     prm.scale_log2 = 1.4426950408889634f / sqrtf((float)hd);
     switch (hd) {
