@@ -11,17 +11,18 @@
 // warp's serial chain per tile (TMEM load, max, exp, TMEM store, fold) is about twice its MUFU time, so three
 // warps per SM sub-partition (NT = 3) are what keeps the MUFU pipe busy (measured with -DMLPF_ATT_LOG).
 //   warps 0 .. 4NT-1   softmax warpgroups, one per query tile: one query row per thread, the tile's 64 scores in
-//               registers:  S -> (mask) -> running max -> exp2 -> bf16 P written back over S's TMEM columns;
-//               acc = acc * corr + O_t(j-1) in registers (no read-modify-write of O in TMEM), and only then is
-//               P_t(j) published, so O_t needs a single TMEM buffer.
+//               registers:  S -> (mask) -> max -> P = 2^((S - m_ref) c) as bf16 written back over S's TMEM columns.
+//               m_ref is a stale reference maximum (lazy rescaling): O_t and the row sums accumulate in TMEM over
+//               all key tiles and are rescaled in place only when m_ref moves (a few times per row).
 //   warp 4NT    TMA producer: Q tiles once; then stages of (K, V), each [128 keys x hd] row-major (two key tiles
 //               per stage).  Q, K, V are column blocks of one row-major [N, 3d] buffer, so an event may start at
 //               any row (TMA needs 16-byte alignment only along the innermost, head-dim, coordinate).
 //   warps 4NT+1 .. 4NT+NT   MMA issuers, one per query tile:  S_t(j) = Q_t K_j^T  (M=128, N=64, K=hd) -> S buffer
-//               j&1;  O_t(j) = P_t(j) V_j (A = P read from TMEM, B = V_j as an MN-major operand, K=64, N=hd).
+//               j&1;  O_t += P_t(j) V_j (A = P read from TMEM, B = V_j as an MN-major operand, K=64, N=hd) and
+//               l_t += P_t(j) 1 (N = 8, a tile of ones as B): the softmax denominators.
 //               All 32 lanes run the issue code with warp-uniform operands (one lane elected inside the wrappers).
 // setmaxnreg moves the producer warpgroup's registers to the softmax warpgroups.
-// TMEM columns: S_t[b] at 128 t + 64 b (P_t[b] aliases its first 32 columns); O_t at 128 NT + hd t.
+// TMEM columns: S_t[b] at 128 t + 64 b (P_t[b] aliases its first 32 columns); O_t | l_t at 128 NT + (hd + 8) t.
 #include "tc_api.h"
 #include "ptx.cuh"
 
