@@ -94,7 +94,8 @@ def test_fp32_debug_path(name, events):
 
 
 # ------------------------------------------------------------------------------------------- bf16 path
-BF16_CASES = [("cfg1", None), ("cfg2", None), ("cfg3", [0, 3]), ("cfg4", [2, 17]), ("cfg5b", [31])]
+# "paper" = the paper's own block shape: d_model 256, 16 heads x 16, ReLU, 3 blocks
+BF16_CASES = [("cfg1", None), ("cfg2", None), ("cfg3", [0, 3]), ("cfg4", [2, 17]), ("cfg5b", [31]), ("paper", [1])]
 
 
 @pytest.mark.parametrize("kernels", [P.KERNELS_TC, P.KERNELS_SIMPLE])
