@@ -25,6 +25,7 @@
 // TMEM columns: S_t[b] at 128 t + 64 b (P_t[b] aliases its first 32 columns); O_t | l_t at 128 NT + (hd + 8) t.
 #include "tc_api.h"
 #include "ptx.cuh"
+#include <type_traits>
 
 namespace mlpf {
 
@@ -329,12 +330,13 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
             };
             load_s(0);
             ptx::tmem_ld_wait();
-            for (int j = 0; j < nkv; ++j) {
-                // key mask of this tile: 64 bits = (in the event) & (valid row), from the schedule's bit array
-                const int k0 = ev0 + j * ATT_BK;
-                uint32_t mask[2];
-                bool full = k0 + ATT_BK <= ev1;
-                if (!full || valid_bits) {
+            // one key tile; MASKED is a compile-time tag so that the loop over full tiles of pad-free events contains no
+            // masking code at all (with both variants inside one loop body the unmasked path ran 9 % slower: measured)
+            auto tile = [&](int j, auto masked_tag) {
+                constexpr bool MASKED = decltype(masked_tag)::value;
+                uint32_t mask[2] = {0xffffffffu, 0xffffffffu};
+                if (MASKED) {   // 64 bits = (key inside the event) & (valid row), from the schedule's bit array
+                    const int k0 = ev0 + j * ATT_BK;
                     const int left = min(ev1 - k0, ATT_BK);                     // 1 .. 64 keys of the event in this tile
                     mask[0] = left >= 32 ? 0xffffffffu : (1u << left) - 1u;
                     mask[1] = left >= 64 ? 0xffffffffu : (left <= 32 ? 0u : (1u << (left - 32)) - 1u);
@@ -344,15 +346,11 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                         mask[0] &= __funnelshift_r(w0, w1, k0 & 31);
                         mask[1] &= __funnelshift_r(w1, w2, k0 & 31);
                     }
-                    full = (mask[0] & mask[1]) == 0xffffffffu;
-                } else {
-                    mask[0] = mask[1] = 0xffffffffu;
                 }
                 const uint32_t s_addr = lane_addr + 128 * t + 64 * (j & 1);
                 if (q == 0) TLOG(t, j, 0);
                 bool rescale;
-                const float corr = full ? softmax_tile<true>(s, s_addr, mask, c, m_ref, rescale)
-                                        : softmax_tile<false>(s, s_addr, mask, c, m_ref, rescale);
+                const float corr = softmax_tile<!MASKED>(s, s_addr, mask, c, m_ref, rescale);
                 if (q == 0) TLOG(t, j, 1);
                 // S_t(j+1) was issued after P_t(j-1) V_(j-1) and the tensor pipe completes in order: once S_t(j+1) has
                 // landed, O_t holds all products up to j-1.  Only the last tile has to wait on bar_o for that.
@@ -376,7 +374,13 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                 if (lane == 0) ptx::mbar_arrive(bar_p + 8 * (2 * t + (j & 1)));      // P_t(j) (and the rescaled O_t) are in TMEM
                 ptx::tmem_ld_wait();
                 if (q == 0) TLOG(t, j, 4);
+            };
+            int j = 0;
+            if (!valid_bits) {                            // pad-free event: every tile but a ragged last one is full
+                const int n_full = (ev1 - ev0) / ATT_BK;
+                for (; j < n_full; ++j) tile(j, std::false_type{});
             }
+            for (; j < nkv; ++j) tile(j, std::true_type{});
             // all products are in: O_t -> registers, normalise, store
             ptx::mbar_wait(bar_o + 8 * t, (nkv - 1) & 1);
             ptx::tc_fence_after();
