@@ -94,6 +94,9 @@ __device__ __forceinline__ float2 exp2_poly2(float2 x) {
     return make_float2(__int_as_float(__float_as_int(p.x) + (__float_as_int(xr.x) << 23)),
                        __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
 }
+#ifndef ATT_POLY_POS
+#define ATT_POLY_POS 0       // which pair of each group of ATT_POLY_EVERY (0 measured 1-2 % faster than the last)
+#endif
 #ifndef ATT_POLY_EVERY
 #define ATT_POLY_EVERY 4     // measured on cfg3 (hd = 32, ms per layer): off 0.865, every 8th pair 0.845, 4th 0.825,
 #endif                       // 3rd 0.846, 2nd 0.927 (with register spills in the loop it was a loss at every setting)
@@ -107,7 +110,7 @@ __device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c,
     for (int i = 0; i < 16; ++i) {
         const float2 x = ptx::ffma2(make_float2(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1])), c2, m2);
         float2 p;
-        if (ATT_POLY_EVERY > 0 && (i % (ATT_POLY_EVERY > 0 ? ATT_POLY_EVERY : 1)) == ATT_POLY_EVERY - 1) p = exp2_poly2(x);
+        if (ATT_POLY_EVERY > 0 && (i % (ATT_POLY_EVERY > 0 ? ATT_POLY_EVERY : 1)) == ATT_POLY_POS) p = exp2_poly2(x);
         else p = make_float2(ptx::fast_exp2(x.x), ptx::fast_exp2(x.y));
         if (!FULL) {
             p.x = (mask >> (2 * i)) & 1u ? p.x : 0.0f;
