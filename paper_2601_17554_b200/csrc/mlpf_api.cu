@@ -501,8 +501,9 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         int rc = run_layernorm(h, fp32, w->h, N, PV + h->lnfg, PV + h->lnfb, u, lo(MLPF_SPLIT_UF, w->u_lo), st);
         if (rc) return rc;
     } else {
-        // no final LN: u = T(h).  (identity affine with the row kept: done by a cast kernel)
-        return set_err(MLPF_E_ARG, "final_ln = 0 is not supported yet");
+        ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);           // no final LN: u = T(h) (+ lo)
+        launch_cast_rows(fp32, w->h, (int64_t)N * d, u, lo(MLPF_SPLIT_UF, w->u_lo), st);
+        LAUNCH_CHECK(h);
     }
     {
         Epi ep;

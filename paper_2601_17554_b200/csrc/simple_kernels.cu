@@ -452,6 +452,22 @@ void launch_pack_valid_bits(const int* valid, int N, uint32_t* bits, cudaStream_
     k_pack_valid_bits<<<(N + 255) / 256, 256, 0, st>>>(valid, N, bits);
 }
 
+// final_ln = 0 (reading A7 off): the heads read the residual stream itself, u = T(h) (+ u_lo = T(h - u))
+template <typename T>
+__global__ void k_cast_rows(const float* __restrict__ h, int64_t n, T* __restrict__ u, T* __restrict__ u_lo) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float v = h[i];
+    const T hi = from_f32<T>(v);
+    u[i] = hi;
+    if (u_lo) u_lo[i] = from_f32<T>(v - to_f32<T>(hi));
+}
+void launch_cast_rows(bool fp32, const float* h, int64_t n, void* u, void* u_lo, cudaStream_t st) {
+    const unsigned grid = (unsigned)((n + 255) / 256);
+    if (fp32) k_cast_rows<float><<<grid, 256, 0, st>>>(h, n, (float*)u, (float*)u_lo);
+    else k_cast_rows<bf16><<<grid, 256, 0, st>>>(h, n, (bf16*)u, (bf16*)u_lo);
+}
+
 // fp32 <- T conversion for the debug taps
 template <typename T>
 __global__ void k_to_f32(const T* __restrict__ src, float* __restrict__ dst, int64_t n) {

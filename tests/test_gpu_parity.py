@@ -277,3 +277,16 @@ def test_largest_event_properties():
     Xp = np.concatenate([Xs, X])
     lg3, rg3 = [t.cpu().numpy() for t in mod.infer(torch.from_numpy(Xp).cuda(), np.array([0, 77, 77 + N], np.int32))]
     assert np.array_equal(lg3[77:], lg) and np.array_equal(rg3[77:], rg)
+
+
+@pytest.mark.parametrize("precision,tol", [(P.PREC_FP32_DEBUG, TOL_FP32), (P.PREC_BF16, TOL_BF16)])
+def test_without_final_layernorm(precision, tol):
+    """Header flag final_ln = 0 (reading A7): the heads read the residual stream itself."""
+    from dataclasses import replace
+    m = replace(synth.model_cfg("cfg1"), final_ln=False)
+    W = synth.make_weights(m, seed=7)
+    X, off = synth.make_events((70, 130, 9), seed=4, pad_frac=0.1)
+    _, lg, rg = gpu_forward(W, m, X, off, precision=precision)
+    Wq = oracle.quantize_weights(W) if precision == P.PREC_BF16 else W
+    lr, rr = oracle.forward(X, off, Wq, m)
+    check(lg, rg, np.arange(X.shape[0]), lr, rr, X, tol, argmax=False)
