@@ -354,7 +354,14 @@ def run_ours(args):
                 "class_time_share": share,
                 "class_ms_per_step": {c: round(t / args.steps, 4) for c, (t, n) in cls.items()},
                 "gemm_tflops": gemm_tflops, "gemm_frac": (gemm_tflops / peak) if gemm_tflops else None,
-                "whole_step_tflops": fl["total"] * args.steps / (total_ms * 1e-3) / 1e12}
+                "whole_step_tflops": fl["total"] * args.steps / (total_ms * 1e-3) / 1e12,
+                # HBM-bound glue kernels: algorithmic bytes / class time, against the measured copy peak
+                "glue_gbs": {"hbm_peak": peaks["hbm_gbs"],
+                             "layernorm": (N * m.d_model * ((m.n_layers * (4 + 2) + (m.n_layers + 1) * (4 + 4)))) * args.steps
+                                          / max(cls["layernorm"][0], 1e-9) / 1e6,
+                             "embed_l1": N * (m.n_feat * 4 + m.d_model * 4) * args.steps / max(cls["embed_l1"][0], 1e-9) / 1e6,
+                             "heads_l2": N * ((1 + len(m.reg_dims)) * m.d_model * 4 + 56) * args.steps
+                                         / max(cls["heads_l2"][0], 1e-9) / 1e6}}
 
     # ---- CPU oracle on a bounded sample (rank 0, N = 1 only)
     cpu = None

@@ -205,6 +205,63 @@ k_layernorm(const float* __restrict__ h, int N, const float* __restrict__ gamma,
     }
 }
 
+// a2, vectorised: lane owns PER = D / 32 CONTIGUOUS columns (D in {64, 128, 256, 512}), 128-bit loads of h / gamma /
+// beta and 64/128-bit stores of the bf16 outputs; same arithmetic (fp32 statistics, two passes over registers).
+template <int D>
+__global__ void __launch_bounds__(256)
+k_layernorm_vec(const float* __restrict__ h, int N, const float* __restrict__ gamma, const float* __restrict__ beta,
+                float eps, bf16* __restrict__ u, bf16* __restrict__ u_lo) {
+    constexpr int PER = D / 32, V = PER < 4 ? PER : 4;            // floats per vector load
+    const int row = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (row >= N) return;
+    const float* hp = h + (int64_t)row * D + lane * PER;
+    float v[PER], g[PER], b[PER];
+#pragma unroll
+    for (int i = 0; i < PER; i += V) {
+        if (V == 4) {
+            *reinterpret_cast<float4*>(&v[i]) = *reinterpret_cast<const float4*>(hp + i);
+            *reinterpret_cast<float4*>(&g[i]) = __ldg(reinterpret_cast<const float4*>(gamma + lane * PER + i));
+            *reinterpret_cast<float4*>(&b[i]) = __ldg(reinterpret_cast<const float4*>(beta + lane * PER + i));
+        } else {
+            *reinterpret_cast<float2*>(&v[i]) = *reinterpret_cast<const float2*>(hp + i);
+            *reinterpret_cast<float2*>(&g[i]) = __ldg(reinterpret_cast<const float2*>(gamma + lane * PER + i));
+            *reinterpret_cast<float2*>(&b[i]) = __ldg(reinterpret_cast<const float2*>(beta + lane * PER + i));
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) s += v[i];
+    const float mean = warp_sum(s) * (1.0f / D);
+    float q = 0.f;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) { const float c = v[i] - mean; q = fmaf(c, c, q); }
+    const float rstd = rsqrtf(warp_sum(q) * (1.0f / D) + eps);
+    uint32_t hi[PER / 2], lo[PER / 2];
+#pragma unroll
+    for (int i = 0; i < PER / 2; ++i) {
+        const float y0 = (v[2 * i] - mean) * rstd * g[2 * i] + b[2 * i];
+        const float y1 = (v[2 * i + 1] - mean) * rstd * g[2 * i + 1] + b[2 * i + 1];
+        __nv_bfloat162 h2 = __floats2bfloat162_rn(y0, y1);
+        hi[i] = *reinterpret_cast<uint32_t*>(&h2);
+        __nv_bfloat162 l2 = __floats2bfloat162_rn(y0 - __low2float(h2), y1 - __high2float(h2));
+        lo[i] = *reinterpret_cast<uint32_t*>(&l2);
+    }
+    const int64_t o = (int64_t)row * D + lane * PER;
+    auto store = [&](bf16* dst, const uint32_t (&w)[PER / 2]) {
+        if (PER >= 8) {
+#pragma unroll
+            for (int i = 0; i < PER / 8; ++i)
+                reinterpret_cast<uint4*>(dst + o)[i] = make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
+        } else if (PER == 4) {
+            *reinterpret_cast<uint2*>(dst + o) = make_uint2(w[0], w[1]);
+        } else {
+            *reinterpret_cast<uint32_t*>(dst + o) = w[0];
+        }
+    };
+    store(u, hi);
+    if (u_lo) store(u_lo, lo);
+}
+
 // ------------------------------------------------------------------------------------------------
 // CUDA-core GEMM  C = A[M,K] W[N,K]^T with the shared epilogue (fp32 debug path / debugging aid).
 // 64x64 tile, BK = 16, 256 threads x (4x4) outputs, fp32 accumulate.  K % 16 == 0, N % 64 == 0.
@@ -511,6 +568,15 @@ static int layernorm_d(int d, const float* x, int N, const float* g, const float
 }
 int launch_layernorm(bool fp32, int d, const float* x, int N, const float* g, const float* b, float eps, void* u,
                      void* u_lo, cudaStream_t st) {
+    if (!fp32) {
+        dim3 grid((N + 7) / 8);
+        switch (d) {
+            case 64:  k_layernorm_vec<64><<<grid, 256, 0, st>>>(x, N, g, b, eps, (bf16*)u, (bf16*)u_lo); return 0;
+            case 128: k_layernorm_vec<128><<<grid, 256, 0, st>>>(x, N, g, b, eps, (bf16*)u, (bf16*)u_lo); return 0;
+            case 256: k_layernorm_vec<256><<<grid, 256, 0, st>>>(x, N, g, b, eps, (bf16*)u, (bf16*)u_lo); return 0;
+            case 512: k_layernorm_vec<512><<<grid, 256, 0, st>>>(x, N, g, b, eps, (bf16*)u, (bf16*)u_lo); return 0;
+        }
+    }
     return fp32 ? layernorm_d<float>(d, x, N, g, b, eps, (float*)u, (float*)u_lo, st)
                 : layernorm_d<bf16>(d, x, N, g, b, eps, (bf16*)u, (bf16*)u_lo, st);
 }
