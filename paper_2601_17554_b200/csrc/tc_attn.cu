@@ -226,7 +226,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
         }
         for (int i = 0; i < nst; ++i) {
             const int s = i % ST;
-            ptx::mbar_wait(bar_kv_empty + 8 * s, ((i / ST) & 1) ^ 1);
+            ptx::mbar_wait_long(bar_kv_empty + 8 * s, ((i / ST) & 1) ^ 1);
             if (lane == 0) {
                 const uint32_t st = sKV + s * Cfg::STAGE_BYTES;
                 const int k0 = ev0 + i * ATT_SK;
@@ -272,7 +272,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
         if (nkv > 1) issue_s(1);
         for (int j = 0; j < nkv; ++j) {
             TLOG(NT + t, j, 0);
-            ptx::mbar_wait(bar_p + 8 * (2 * t + (j & 1)), (j >> 1) & 1);     // P_t(j) is in TMEM, O_t(j-1) is folded
+            ptx::mbar_wait_long(bar_p + 8 * (2 * t + (j & 1)), (j >> 1) & 1);     // P_t(j) is in TMEM
             ptx::tc_fence_after();
             TLOG(NT + t, j, 1);
             issue_o(j);
