@@ -1,4 +1,4 @@
-// simple_kernels.cuh -- CUDA-core kernels of libmlpf.so.
+// simple_kernels.cu -- CUDA-core kernels of libmlpf.so.
 //  * the integer schedule (step a0), the embedding's first layer (a1), LayerNorm (a2) and the heads'
 //    output layer (a8) are used by every path;
 //  * the tiled FFMA GEMM and the one-thread-per-query attention are the fp32 debug path
