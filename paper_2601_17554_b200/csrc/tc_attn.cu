@@ -103,14 +103,14 @@ __device__ __forceinline__ float2 exp2_poly2(float2 x) {
 
 
 // p = 2^(s c - m c) for 32 scores -> 16 bf16 pairs (the row sums come from the tensor pipe: P x 1)
-template <bool FULL>
+template <bool FULL, bool POLY>
 __device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c, float neg_mc, uint32_t (&pk)[16]) {
     const float2 c2 = make_float2(c, c), m2 = make_float2(neg_mc, neg_mc);
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
         const float2 x = ptx::ffma2(make_float2(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1])), c2, m2);
         float2 p;
-        if (ATT_POLY_EVERY > 0 && (i % (ATT_POLY_EVERY > 0 ? ATT_POLY_EVERY : 1)) == ATT_POLY_POS) p = exp2_poly2(x);
+        if (POLY && ATT_POLY_EVERY > 0 && (i % (ATT_POLY_EVERY > 0 ? ATT_POLY_EVERY : 1)) == ATT_POLY_POS) p = exp2_poly2(x);
         else p = make_float2(ptx::fast_exp2(x.x), ptx::fast_exp2(x.y));
         if (!FULL) {
             p.x = (mask >> (2 * i)) & 1u ? p.x : 0.0f;
@@ -128,7 +128,7 @@ __device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c,
 // precision, while the accumulated O (in TMEM) has to be rescaled only a few times per row instead of every tile.
 // Returns corr = 2^((m_ref_old - m_ref_new) c); `rescale` (warp-uniform) says whether m_ref moved.
 constexpr float ATT_RESCALE_LOG2 = 8.0f;
-template <bool FULL>
+template <bool FULL, bool POLY = true>
 __device__ __forceinline__ float softmax_tile(const uint32_t (&s)[64], uint32_t s_addr, const uint32_t (&mask)[2], float c,
                                               float& m_ref, bool& rescale) {
     const float mx = fmaxf(max32<FULL>(&s[0], mask[0], -INFINITY), max32<FULL>(&s[32], mask[1], -INFINITY));
@@ -145,10 +145,22 @@ __device__ __forceinline__ float softmax_tile(const uint32_t (&s)[64], uint32_t 
 #pragma unroll
     for (int w = 0; w < 2; ++w) {
         uint32_t pk[16];
-        exp32<FULL>(&s[32 * w], mask[w], c, neg_mc, pk);
+        exp32<FULL, POLY>(&s[32 * w], mask[w], c, neg_mc, pk);
         ptx::tmem_st16(s_addr + 16 * w, pk);
     }
     return corr;
+}
+
+// Masked tile, hd = 64 variant: the scores of keys outside the event / of pad rows become -inf ONCE, so the max pass
+// ignores them and 2^(-inf) gives the exact weight 0 on the MUFU (no polynomial path: it clamps its argument).  Two
+// selects per score less than softmax_tile<false>.  Only instantiated at hd = 64: inside the hd <= 32 kernels the same
+// code changed ptxas' schedule of the unmasked loop for the worse (cfg3 3 % slower: measured), there the padded
+// configs matter less than the pad-free headline.
+__device__ __forceinline__ float softmax_tile_mask_once(uint32_t (&s)[64], uint32_t s_addr, const uint32_t (&mask)[2], float c,
+                                                        float& m_ref, bool& rescale) {
+#pragma unroll
+    for (int i = 0; i < 64; ++i) s[i] = (mask[i >> 5] >> (i & 31)) & 1u ? s[i] : 0xff800000u;
+    return softmax_tile<true, false>(s, s_addr, mask, c, m_ref, rescale);
 }
 
 template <int HD>
@@ -353,7 +365,9 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                 const uint32_t s_addr = lane_addr + 128 * t + 64 * (j & 1);
                 if (q == 0) TLOG(t, j, 0);
                 bool rescale;
-                const float corr = softmax_tile<!MASKED>(s, s_addr, mask, c, m_ref, rescale);
+                float corr;
+                if (MASKED && HD == 64) corr = softmax_tile_mask_once(s, s_addr, mask, c, m_ref, rescale);
+                else corr = softmax_tile<!MASKED>(s, s_addr, mask, c, m_ref, rescale);
                 if (q == 0) TLOG(t, j, 1);
                 // S_t(j+1) was issued after P_t(j-1) V_(j-1) and the tensor pipe completes in order: once S_t(j+1) has
                 // landed, O_t holds all products up to j-1.  Only the last tile has to wait on bar_o for that.
