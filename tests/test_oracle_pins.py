@@ -366,3 +366,76 @@ def test_round_bf16_is_rne():
     import torch
     tt = torch.tensor(np.random.default_rng(0).standard_normal(4096).astype(np.float32))
     np.testing.assert_array_equal(oracle.round_bf16(tt.numpy()), tt.to(torch.bfloat16).to(torch.float32).numpy())
+
+
+# ------------------------------------------------------------------ candidate building (NEXT-2; Eq. 2)
+def _cand_inputs(lens=(7, 0, 12, 5), seed=11, pad_frac=0.2, n_classes=9):
+    X, off = synth.make_events(lens, seed=seed, pad_frac=pad_frac)
+    rng = np.random.default_rng(seed + 1)
+    N = int(off[-1])
+    logits = rng.standard_normal((N, n_classes)).astype(np.float32)
+    regress = (0.5 * rng.standard_normal((N, 5))).astype(np.float32)
+    return X, off, logits, regress
+
+
+def test_candidates_invert_eq2_and_recover_phi():
+    """Closed form: feed pT' = log(pT_t / pT_in), E' = log(E_t / E_in) (Eq. 2) and (sin, cos) of a known phi in
+    all four quadrants; decoding must give back pT_t, E_t and phi."""
+    X, off, logits, _ = _cand_inputs(lens=(40, 24), pad_frac=0.0)
+    N = int(off[-1])
+    rng = np.random.default_rng(5)
+    pt_t = np.exp(rng.standard_normal(N)); e_t = pt_t * np.cosh(rng.uniform(-3, 3, N))
+    phi = rng.uniform(-math.pi, math.pi, N)
+    phi[:4] = [0.25 * math.pi, 0.75 * math.pi, -0.75 * math.pi, -0.25 * math.pi]
+    eta = rng.uniform(-5, 5, N)
+    reg = np.stack([np.log(pt_t / X[:, 1].astype(np.float64)), eta, np.sin(phi), np.cos(phi),
+                    np.log(e_t / X[:, 4].astype(np.float64))], axis=1)
+    logits[:, 0] = -10.0                                   # every element yields a candidate
+    c = oracle.build_candidates(X, off, logits, reg)
+    assert c["cand_offsets"].tolist() == [0, 40, 64]
+    assert np.array_equal(c["cand_elem"], np.arange(N))
+    assert np.allclose(c["cand_p4"][:, 0], pt_t, rtol=1e-12)
+    assert np.allclose(c["cand_p4"][:, 1], eta, rtol=0, atol=0)
+    assert np.allclose(c["cand_p4"][:, 2], phi, rtol=0, atol=1e-12)
+    assert np.allclose(c["cand_p4"][:, 3], e_t, rtol=1e-12)
+
+
+def test_candidates_loop_restatement_and_offset_invariants():
+    """Brute force, element by element, with math.* scalars; pad rows and class-0 rows are dropped, order is the
+    element order, offsets are per event (empty event included)."""
+    X, off, logits, reg = _cand_inputs()
+    logits[3, :] = 1.0                                     # an exact tie: lowest class (0) wins -> dropped
+    c = oracle.build_candidates(X, off, logits, reg)
+    exp_off, elem, pid, p4 = [0], [], [], []
+    for e in range(len(off) - 1):
+        for i in range(int(off[e]), int(off[e + 1])):
+            best = 0
+            for k in range(1, logits.shape[1]):
+                if logits[i, k] > logits[i, best]:
+                    best = k
+            if int(X[i, 0]) != 0 and best != 0:
+                elem.append(i); pid.append(best)
+                p4.append((float(X[i, 1]) * math.exp(float(reg[i, 0])), float(reg[i, 1]),
+                           math.atan2(float(reg[i, 2]), float(reg[i, 3])), float(X[i, 4]) * math.exp(float(reg[i, 4]))))
+        exp_off.append(len(elem))
+    assert c["cand_offsets"].tolist() == exp_off
+    assert c["cand_elem"].tolist() == elem and c["cand_pid"].tolist() == pid
+    assert 3 not in elem
+    assert np.allclose(c["cand_p4"], np.asarray(p4).reshape(-1, 4), rtol=1e-14, atol=0)
+    # invariants: every candidate's element lies inside its event, strictly increasing inside an event
+    for e in range(len(off) - 1):
+        seg = c["cand_elem"][c["cand_offsets"][e]:c["cand_offsets"][e + 1]]
+        assert np.all((seg >= off[e]) & (seg < off[e + 1])) and np.all(np.diff(seg) > 0)
+    assert c["cand_offsets"][2] == c["cand_offsets"][1]    # the empty event
+
+
+def test_candidates_packing_invariance():
+    """An event decoded alone gives the same candidates as the same event packed after others (indices shifted)."""
+    X, off, logits, reg = _cand_inputs()
+    c = oracle.build_candidates(X, off, logits, reg)
+    a, b = int(off[2]), int(off[3])
+    c1 = oracle.build_candidates(X[a:b], np.array([0, b - a]), logits[a:b], reg[a:b])
+    s, t = c["cand_offsets"][2], c["cand_offsets"][3]
+    assert np.array_equal(c1["cand_elem"] + a, c["cand_elem"][s:t])
+    assert np.array_equal(c1["cand_pid"], c["cand_pid"][s:t])
+    assert np.array_equal(c1["cand_p4"], c["cand_p4"][s:t])
