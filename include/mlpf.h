@@ -98,6 +98,30 @@ void mlpf_destroy(mlpf_handle* h);
 /* Thread-local text of the last error raised on this thread ("" if none). */
 const char* mlpf_last_error(void);
 
+/* ---- candidate building (the step after the forward pass; "builds the particle candidates") -------
+ * From the per-element outputs of mlpf_infer to the per-event list of particle candidates:
+ *   PID_i = argmax_c logits[i,c] (multiclass PID head, L130/L156; ties -> lowest class);
+ *   element i yields a candidate iff its type (feature 0) != 0 and PID_i != 0 (class 0 = "no particle": reading A22,
+ *   the library's single 9-class head has no separate binary head, reading A11);
+ *   pT = x_i[1] exp(pT'), E = x_i[4] exp(E') (Eq. 2 inverted, L137-L139; x_i[1], x_i[4] = the element's own pT, E),
+ *   eta = raw output, phi = atan2(sin phi, cos phi) (L126).
+ * Candidates keep the element order (stable compaction) and are grouped per event:
+ *   cand_offsets [n_events+1] int32: event e owns candidates cand_offsets[e] .. cand_offsets[e+1]-1;
+ *   cand_elem [M] int32 global row of the element, cand_pid [M] int32, cand_p4 [M,4] fp32 (pT, eta, phi, E),
+ *   M = cand_offsets[n_events] <= N; entries beyond M are not written.
+ * All pointers are DEVICE pointers except event_offsets (HOST, read before return, same rules as mlpf_infer).
+ * regress is [N,5] = (pT', eta, sin phi, cos phi, E'); logits [N,n_classes], n_classes 1..64; elements [N,n_feat],
+ * n_feat >= 5.  cand_elem / cand_pid / cand_p4 need capacity N (cand_p4 16-byte aligned); scratch is caller-owned
+ * device memory, 256-byte aligned, of at least mlpf_candidates_scratch_bytes(N, n_events) bytes, and may be reused
+ * by the next call on the same stream.  Only enqueues on `stream` (three kernels); no allocation, no sync.
+ * Integer outputs are bit-exact vs the oracle on the same fp32 logits; pT, E, phi are fp32 expf / atan2f.
+ * n_events == 0: success, nothing written.  N == 0: cand_offsets is all zeros.  Errors as for mlpf_infer. */
+int64_t mlpf_candidates_scratch_bytes(int64_t n_elements, int32_t n_events);   /* < 0 on error */
+int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* event_offsets, int32_t n_events,
+                          const float* logits, int32_t n_classes, const float* regress, void* scratch,
+                          int64_t scratch_bytes, int32_t* cand_offsets, int32_t* cand_elem, int32_t* cand_pid,
+                          float* cand_p4, void* stream);
+
 /* ---- options -------------------------------------------------------------------------------------- */
 #define MLPF_OPT_PRECISION   1   /* MLPF_PREC_BF16 (default) | MLPF_PREC_FP32_DEBUG                    */
 #define MLPF_OPT_TILE_Q      2   /* query-tile rows of the attention work list: 64 | 128 (default 128) */

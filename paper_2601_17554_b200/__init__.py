@@ -28,7 +28,7 @@ KERNEL_CLASSES = ["sched", "embed_l1", "embed_l2", "layernorm", "qkv", "attentio
 
 EXPORTS = ["mlpf_create", "mlpf_infer", "mlpf_infer_host", "mlpf_destroy", "mlpf_last_error", "mlpf_set_option",
            "mlpf_query", "mlpf_debug_get_schedule", "mlpf_debug_get_tensor", "mlpf_debug_get_profile", "mlpf_tc_gemm_bf16",
-           "mlpf_tc_attention_bf16"]
+           "mlpf_tc_attention_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates"]
 
 _lib = None
 
@@ -67,6 +67,10 @@ def lib():
     L.mlpf_tc_gemm_bf16.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp]
     L.mlpf_tc_attention_bf16.restype = C.c_int
     L.mlpf_tc_attention_bf16.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
+    L.mlpf_candidates_scratch_bytes.restype = i64
+    L.mlpf_candidates_scratch_bytes.argtypes = [i64, i32]
+    L.mlpf_build_candidates.restype = C.c_int
+    L.mlpf_build_candidates.argtypes = [vp, i32, vp, i32, vp, i32, vp, vp, i64, vp, vp, vp, vp, vp]
     _lib = L
     return L
 
@@ -192,4 +196,33 @@ def tc_attention_bf16(QKV, key_valid, event_offsets, d_model, n_heads, stream=No
     _check(lib().mlpf_tc_attention_bf16(C.c_void_p(QKV.data_ptr()), kv,
                                         off.ctypes.data_as(C.c_void_p), len(off) - 1, d_model, n_heads,
                                         C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+    return out
+
+
+def build_candidates(elements, event_offsets, logits, regress, scratch=None, stream=None):
+    """Per-event particle candidates from mlpf_infer's outputs (include/mlpf.h "candidate building").
+    CUDA tensors in; returns dict(cand_offsets [E+1] int32, cand_elem [N] int32, cand_pid [N] int32,
+    cand_p4 [N,4] float32 = (pT, eta, phi, E)), all CUDA, enqueued on `stream`; the first cand_offsets[-1]
+    entries of the last three are the candidates."""
+    import torch
+    off = np.ascontiguousarray(event_offsets, dtype=np.int32)
+    E = len(off) - 1
+    N = int(off[-1]) if E >= 0 else 0
+    dev = elements.device
+    for t in (elements, logits, regress):
+        assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+    assert regress.shape[1] == 5
+    need = _check(lib().mlpf_candidates_scratch_bytes(N, max(E, 0)))
+    if scratch is None:
+        scratch = torch.empty(need, dtype=torch.uint8, device=dev)
+    out = dict(cand_offsets=torch.empty(E + 1, dtype=torch.int32, device=dev),
+               cand_elem=torch.empty(N, dtype=torch.int32, device=dev),
+               cand_pid=torch.empty(N, dtype=torch.int32, device=dev),
+               cand_p4=torch.empty((N, 4), dtype=torch.float32, device=dev))
+    _check(lib().mlpf_build_candidates(C.c_void_p(elements.data_ptr()), elements.shape[1], off.ctypes.data_as(C.c_void_p), E,
+                                       C.c_void_p(logits.data_ptr()), logits.shape[1], C.c_void_p(regress.data_ptr()),
+                                       C.c_void_p(scratch.data_ptr()), scratch.numel(),
+                                       C.c_void_p(out["cand_offsets"].data_ptr()), C.c_void_p(out["cand_elem"].data_ptr()),
+                                       C.c_void_p(out["cand_pid"].data_ptr()), C.c_void_p(out["cand_p4"].data_ptr()),
+                                       _stream_ptr(stream)))
     return out

@@ -5,6 +5,7 @@
 #include "common.cuh"
 #include "simple_api.h"
 #include "tc_api.h"
+#include "cand_api.h"
 
 #include <algorithm>
 #include <cstdarg>
@@ -584,6 +585,36 @@ extern "C" int mlpf_infer_host(mlpf_handle* h, const float* elements_host, const
     CUDA_TRY(cudaMemcpyAsync(out_logits_host, sb.lg, (size_t)N * h->C * 4, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaMemcpyAsync(out_regress_host, sb.rg, (size_t)N * h->R * 4, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
+    return MLPF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ candidate building
+extern "C" int64_t mlpf_candidates_scratch_bytes(int64_t n_elements, int32_t n_events) {
+    if (n_elements < 0 || n_events < 0) return set_err(MLPF_E_ARG, "negative size");
+    return cand_scratch_bytes(n_elements, n_events);
+}
+
+extern "C" int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* event_offsets, int32_t n_events,
+                                     const float* logits, int32_t n_classes, const float* regress, void* scratch,
+                                     int64_t scratch_bytes, int32_t* cand_offsets, int32_t* cand_elem, int32_t* cand_pid,
+                                     float* cand_p4, void* stream) {
+    if (n_events < 0) return set_err(MLPF_E_OFFSETS, "n_events < 0");
+    if (n_events == 0) return MLPF_OK;
+    if (!event_offsets) return set_err(MLPF_E_NULL, "event_offsets is NULL");
+    if (event_offsets[0] != 0) return set_err(MLPF_E_OFFSETS, "event_offsets[0] != 0");
+    for (int e = 0; e < n_events; ++e)
+        if (event_offsets[e + 1] < event_offsets[e]) return set_err(MLPF_E_OFFSETS, "event_offsets decreasing at %d", e);
+    const int64_t N = event_offsets[n_events];
+    if (n_feat < 5 || n_classes < 1 || n_classes > 64) return set_err(MLPF_E_ARG, "n_feat = %d (>= 5), n_classes = %d (1..64)", n_feat, n_classes);
+    if (!scratch || !cand_offsets) return set_err(MLPF_E_NULL, "scratch / cand_offsets NULL");
+    if (N > 0 && (!elements || !logits || !regress || !cand_elem || !cand_pid || !cand_p4)) return set_err(MLPF_E_NULL, "inputs / outputs NULL");
+    if (scratch_bytes < cand_scratch_bytes(N, n_events))
+        return set_err(MLPF_E_ARG, "scratch_bytes %lld < %lld", (long long)scratch_bytes, (long long)cand_scratch_bytes(N, n_events));
+    if (((uintptr_t)cand_p4 & 15) || ((uintptr_t)scratch & 255)) return set_err(MLPF_E_ARG, "cand_p4 must be 16-byte, scratch 256-byte aligned");
+    cudaError_t e = launch_build_candidates(elements, n_feat, event_offsets, n_events, logits, n_classes, regress, scratch,
+                                            cand_offsets, cand_elem, cand_pid, cand_p4, (cudaStream_t)stream);
+    if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "candidate kernels: %s", cudaGetErrorString(e));
+    g_err.clear();
     return MLPF_OK;
 }
 

@@ -71,3 +71,17 @@ def test_no_cpu_fallback_without_a_device(L):
         pytest.skip("a GPU is present")
     with pytest.raises(P.MlpfError, match="no CUDA device"):
         P.Mlpf(synth.make_weights("cfg1"), synth.model_cfg("cfg1"))
+
+
+def test_build_candidates_rejects_bad_arguments_before_touching_the_device(L):
+    off = (C.c_int32 * 3)(0, 4, 2)
+    assert L.mlpf_build_candidates(None, 55, off, 2, None, 9, None, None, 0, None, None, None, None, None) == -3
+    assert "decreasing" in L.mlpf_last_error().decode()
+    off = (C.c_int32 * 2)(1, 4)
+    assert L.mlpf_build_candidates(None, 55, off, 1, None, 9, None, None, 0, None, None, None, None, None) == -3
+    off = (C.c_int32 * 2)(0, 4)
+    assert L.mlpf_build_candidates(None, 4, off, 1, None, 9, None, None, 0, None, None, None, None, None) == -6
+    assert L.mlpf_build_candidates(None, 55, off, 1, None, 9, None, None, 0, None, None, None, None, None) == -1
+    assert L.mlpf_build_candidates(None, 55, None, 0, None, 9, None, None, 0, None, None, None, None, None) == 0
+    assert L.mlpf_candidates_scratch_bytes(1000, 4) >= 1000 + 5 * 4 + 2 * 4 * 4
+    assert L.mlpf_candidates_scratch_bytes(-1, 0) < 0
