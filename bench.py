@@ -297,6 +297,27 @@ def run_ours(args):
                 lat.append(e0.elapsed_time(e1))
     lat = np.array(lat[E:]) if len(lat) > E else np.array(lat)    # first sweep = warm-up
 
+    # ---- candidate building (the step after the forward pass): mlpf_build_candidates on this batch's
+    # own outputs, L2 flushed before each call; HBM / launch-latency bound, reported against the copy peak
+    cand_ms = []
+    scratch = torch.empty(int(P.lib().mlpf_candidates_scratch_bytes(N, E)), dtype=torch.uint8, device="cuda")
+    with torch.cuda.stream(st):
+        mod.infer(Xd, off, lg, rg, stream=st)
+        for i in range(13):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st)
+            cand = P.build_candidates(Xd, off, lg, rg, scratch=scratch, stream=st)
+            e1.record(st)
+            e1.synchronize()
+            if i >= 3:
+                cand_ms.append(e0.elapsed_time(e1))
+    n_cand = int(cand["cand_offsets"][-1])
+    cand_bytes = N * (4 * mod.n_classes + 4 + 20 + 8 + 2) + n_cand * 24     # logits, type, regress, pT/E in, code; outputs
+    candidates = {"ms_p50": float(np.percentile(cand_ms, 50)), "launches": 2, "candidates": n_cand, "elements": N,
+                  "algorithmic_bytes": int(cand_bytes), "gbs": cand_bytes / (np.percentile(cand_ms, 50) * 1e-3) / 1e9,
+                  "hbm_peak_gbs": peaks["hbm_gbs"]}
+
     # ---- several concurrent streams (north_star: "also with several concurrent streams"): the batch is split into
     # S contiguous event groups, one CUDA stream each, enqueued round-robin from this thread (mlpf_infer only enqueues)
     multi = None
@@ -388,7 +409,7 @@ def run_ours(args):
             "gpu_launches": launches_per_step * args.steps, "launches_per_step": launches_per_step,
             "peak_bytes": {"weights": int(mod.query(P.Q_WEIGHT_BYTES)), "workspace": int(mod.query(P.Q_WORKSPACE_BYTES)),
                            "torch_max_allocated": int(torch.cuda.max_memory_allocated())},
-            "streams": multi, "clocks": sampler.result(), "roofline": roofline, "cpu_baseline": cpu}
+            "streams": multi, "candidates": candidates, "clocks": sampler.result(), "roofline": roofline, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -113,7 +113,7 @@ const char* mlpf_last_error(void);
  * regress is [N,5] = (pT', eta, sin phi, cos phi, E'); logits [N,n_classes], n_classes 1..64; elements [N,n_feat],
  * n_feat >= 5.  cand_elem / cand_pid / cand_p4 need capacity N (cand_p4 16-byte aligned); scratch is caller-owned
  * device memory, 256-byte aligned, of at least mlpf_candidates_scratch_bytes(N, n_events) bytes, and may be reused
- * by the next call on the same stream.  Only enqueues on `stream` (three kernels); no allocation, no sync.
+ * by the next call on the same stream.  Only enqueues on `stream` (two kernels); no allocation, no sync.
  * Integer outputs are bit-exact vs the oracle on the same fp32 logits; pT, E, phi are fp32 expf / atan2f.
  * n_events == 0: success, nothing written.  N == 0: cand_offsets is all zeros.  Errors as for mlpf_infer. */
 int64_t mlpf_candidates_scratch_bytes(int64_t n_elements, int32_t n_events);   /* < 0 on error */

@@ -3,8 +3,8 @@
 //   PID = argmax of the logits (L130/L156; ties -> lowest class), kept iff type != 0 and PID != 0 (reading A22),
 //   pT = pT_in exp(pT'), E = E_in exp(E')  (Eq. 2 inverted, L137-L139),  phi = atan2(sin phi, cos phi)  (L126),
 //   candidates in element order, grouped per event by integer offsets (bit-exact vs the oracle).
-// HBM / launch-latency bound (~90 algorithmic bytes per element): three small kernels, a stable stream
-// compaction = per-block counts, one-block scan, per-block scatter.  Blocks of CAND_BLOCK rows; the grid covers
+// HBM / launch-latency bound (~90 algorithmic bytes per element): two small kernels, a stable stream
+// compaction = per-block counts, then per-block prefix + scatter.  Blocks of CAND_BLOCK rows; the grid covers
 // rows 0..N INCLUSIVE (row N is a virtual, never-kept row) so that every event offset, offsets[E] = N and the
 // offsets of trailing empty events included, falls inside exactly one block, which writes that cand_offsets entry.
 #include "cand_api.h"
@@ -40,60 +40,33 @@ k_cand_count(const float* __restrict__ X, int F, const float* __restrict__ logit
     if (threadIdx.x == 0) block_counts[blockIdx.x] = cnt;
 }
 
-// exclusive scan of block_counts[nb] -> block_base[nb] (one block; nb is small: N / 256 + 1)
-__global__ void __launch_bounds__(1024)
-k_cand_scan(const int* __restrict__ block_counts, int nb, int* __restrict__ block_base) {
-    __shared__ int s_warp[32];
-    __shared__ int s_carry;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) s_carry = 0;
-    __syncthreads();
-    for (int b0 = 0; b0 < nb; b0 += 1024) {
-        const int b = b0 + threadIdx.x;
-        const int v = b < nb ? block_counts[b] : 0;
-        int inc = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
-        if (lane == 31) s_warp[warp] = inc;
-        __syncthreads();
-        if (warp == 0) {
-            int w = s_warp[lane];
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, w, o); if (lane >= o) w += t; }
-            s_warp[lane] = w;                              // inclusive over warps
-        }
-        __syncthreads();
-        const int carry = s_carry;
-        const int excl = carry + (warp ? s_warp[warp - 1] : 0) + inc - v;
-        if (b < nb) block_base[b] = excl;
-        __syncthreads();
-        if (threadIdx.x == 1023) s_carry = carry + s_warp[31];
-        __syncthreads();
-    }
-}
-
-// stable scatter of the kept rows + the cand_offsets entries of the event boundaries inside this block
+// stable scatter of the kept rows + the cand_offsets entries of the event boundaries inside this block; the block's
+// base = sum of the counts of the blocks before it (at most N / 256 L2-resident ints: cheaper than a scan launch)
 __global__ void __launch_bounds__(CAND_BLOCK)
 k_cand_emit(const float* __restrict__ X, int F, const float* __restrict__ regress, int64_t N,
-            const int* __restrict__ offsets, int E, const uint8_t* __restrict__ code, const int* __restrict__ block_base,
+            const int* __restrict__ offsets, int E, const uint8_t* __restrict__ code, const int* __restrict__ block_counts,
             int* __restrict__ cand_offsets, int* __restrict__ cand_elem, int* __restrict__ cand_pid,
             float4* __restrict__ cand_p4) {
     __shared__ float s_rg[CAND_BLOCK * 5];
     __shared__ int s_rank[CAND_BLOCK];                     // exclusive rank of each row inside the block
-    __shared__ int s_warp[CAND_BLOCK / 32];
+    __shared__ int s_warp[CAND_BLOCK / 32], s_base[CAND_BLOCK / 32];
     const int64_t row0 = (int64_t)blockIdx.x * CAND_BLOCK, i = row0 + threadIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int part = 0;
+    for (int b = threadIdx.x; b < (int)blockIdx.x; b += CAND_BLOCK) part += block_counts[b];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+    if (lane == 0) s_base[warp] = part;
     cand_stage_rows(regress, row0, N, 5, s_rg);
     const int pid = i < N ? code[i] : 0;
     const unsigned m = __ballot_sync(0xffffffffu, pid != 0);
     if (lane == 0) s_warp[warp] = __popc(m);
     __syncthreads();
-    int before = 0;
+    int before = 0, base = 0;
 #pragma unroll
-    for (int w = 0; w < CAND_BLOCK / 32; ++w) before += w < warp ? s_warp[w] : 0;
+    for (int w = 0; w < CAND_BLOCK / 32; ++w) { before += w < warp ? s_warp[w] : 0; base += s_base[w]; }
     const int local = before + __popc(m & ((1u << lane) - 1u));
     s_rank[threadIdx.x] = local;
-    const int base = block_base[blockIdx.x];
     if (pid != 0) {
         const float* r = s_rg + threadIdx.x * 5;
         const float pt_in = __ldg(X + i * F + 1), e_in = __ldg(X + i * F + 4);
@@ -115,7 +88,7 @@ k_cand_emit(const float* __restrict__ X, int F, const float* __restrict__ regres
 
 int64_t cand_scratch_bytes(int64_t N, int64_t E) {
     const int64_t nb = N / CAND_BLOCK + 1;
-    return ((N + 255) / 256 * 256) + ((E + 1) * 4 + 255) / 256 * 256 + 2 * ((nb * 4 + 255) / 256 * 256);
+    return ((N + 255) / 256 * 256) + ((E + 1) * 4 + 255) / 256 * 256 + (nb * 4 + 255) / 256 * 256;
 }
 
 cudaError_t launch_build_candidates(const float* X, int F, const int32_t* offsets_host, int E, const float* logits, int C,
@@ -126,14 +99,12 @@ cudaError_t launch_build_candidates(const float* X, int F, const int32_t* offset
     uint8_t* p = (uint8_t*)scratch;
     uint8_t* code = p;                     p += (N + 255) / 256 * 256;
     int* offsets = (int*)p;                p += ((int64_t)(E + 1) * 4 + 255) / 256 * 256;
-    int* block_counts = (int*)p;           p += ((int64_t)nb * 4 + 255) / 256 * 256;
-    int* block_base = (int*)p;
+    int* block_counts = (int*)p;
     // pageable -> device async copies are staged by the runtime before returning: the caller may free offsets_host
     cudaError_t e = cudaMemcpyAsync(offsets, offsets_host, (size_t)(E + 1) * 4, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return e;
     k_cand_count<<<nb, CAND_BLOCK, (size_t)CAND_BLOCK * C * 4, st>>>(X, F, logits, C, N, code, block_counts);
-    k_cand_scan<<<1, 1024, 0, st>>>(block_counts, nb, block_base);
-    k_cand_emit<<<nb, CAND_BLOCK, 0, st>>>(X, F, regress, N, offsets, E, code, block_base, cand_offsets, cand_elem,
+    k_cand_emit<<<nb, CAND_BLOCK, 0, st>>>(X, F, regress, N, offsets, E, code, block_counts, cand_offsets, cand_elem,
                                            cand_pid, reinterpret_cast<float4*>(cand_p4));
     return cudaGetLastError();
 }
