@@ -101,7 +101,7 @@ const char* mlpf_last_error(void);
 /* ---- candidate building (the step after the forward pass; "builds the particle candidates") -------
  * From the per-element outputs of mlpf_infer to the per-event list of particle candidates:
  *   PID_i = argmax_c logits[i,c] (multiclass PID head, L130/L156; ties -> lowest class);
- *   element i yields a candidate iff its type (feature 0) != 0 and PID_i != 0 (class 0 = "no particle": reading A22,
+ *   element i yields a candidate iff its type (feature 0) != 0 and PID_i != 0 (class 0 = "no particle": reading A23,
  *   the library's single 9-class head has no separate binary head, reading A11);
  *   pT = x_i[1] exp(pT'), E = x_i[4] exp(E') (Eq. 2 inverted, L137-L139; x_i[1], x_i[4] = the element's own pT, E),
  *   eta = raw output, phi = atan2(sin phi, cos phi) (L126).

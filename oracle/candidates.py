@@ -11,7 +11,7 @@ list of particle candidates that the experiment software consumes (PAPER.md L222
   and E_primary = x[4] of the element itself (DESIGN.md input recipe).  eta is the raw output;
   phi = atan2(sin phi, cos phi) ("parameterized through sin phi and cos phi to preserve the
   quadrant information", L126).
-* Selection (reading A22): the library's 9-class head has no separate binary head
+* Selection (reading A23): the library's 9-class head has no separate binary head
   (reading A11), so class 0 is "no particle": element i yields a candidate iff it is not a pad row
   (type != 0, reading A2) and its PID != 0.
 * Output: candidates in element order (stable), grouped per event by integer offsets.

@@ -1,6 +1,6 @@
 // candidates.cu -- candidate building: the step right after the encoder,
 // turning per-element outputs into the per-event particle list the experiment software consumes.
-//   PID = argmax of the logits (L130/L156; ties -> lowest class), kept iff type != 0 and PID != 0 (reading A22),
+//   PID = argmax of the logits (L130/L156; ties -> lowest class), kept iff type != 0 and PID != 0 (reading A23),
 //   pT = pT_in exp(pT'), E = E_in exp(E')  (Eq. 2 inverted, L137-L139),  phi = atan2(sin phi, cos phi)  (L126),
 //   candidates in element order, grouped per event by integer offsets (bit-exact vs the oracle).
 // HBM / launch-latency bound (~90 algorithmic bytes per element): two small kernels, a stable stream
