@@ -27,7 +27,7 @@ k_sched_count(const float* __restrict__ X, int N, int F, const int* __restrict__
     if (threadIdx.x < 5) hist[threadIdx.x] = 0;
     __syncthreads();
     int i = blockIdx.x * SCHED_BLOCK + threadIdx.x;
-    int t = -1;
+    int t = -1, ev = -1;
     if (i < N) {
         t = element_type(X, i, F);
         valid[i] = (t != 0);
@@ -39,11 +39,15 @@ k_sched_count(const float* __restrict__ X, int N, int F, const int* __restrict__
         }
         row_event[i] = lo;
         row_pos[i] = i - offsets[lo];
-        if (t != 0) atomicAdd(&n_valid[lo], 1);
+        ev = lo;
     }
     {   // one bit per row, 32 rows per word (rows >= N: 0): the attention kernel's key mask
         const unsigned vb = __ballot_sync(0xffffffffu, t > 0);
         if ((threadIdx.x & 31) == 0) valid_bits[i >> 5] = vb;
+        // n_valid: one atomic per (warp, event) instead of one per row (49 k same-address atomics took 30 us on cfg3)
+        const unsigned grp = __match_any_sync(0xffffffffu, ev);
+        const int cnt = __popc(grp & vb);
+        if (ev >= 0 && cnt && (int)(threadIdx.x & 31) == __ffs(grp) - 1) atomicAdd(&n_valid[ev], cnt);
     }
 #pragma unroll
     for (int ty = 0; ty < 5; ++ty) {
@@ -152,21 +156,34 @@ k_embed_l1(const float* __restrict__ X, int N, int F, int d, const float* __rest
 #pragma unroll
             for (int k = 0; k < 64; ++k) w[k] = wp[(int64_t)k * d];
             const float bj = b1[(t - 1) * d + j];
-            for (int p = 0; p < c; ++p) {
-                const int r = list[t][p];
-                float acc = bj;
-                const float4* xr = reinterpret_cast<const float4*>(xs[r]);
+            for (int p = 0; p < c; p += 4) {            // four rows per pass: four independent FMA chains
+                int r[4];
+                float acc[4];
+                const float4* xr[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    r[q] = list[t][min(p + q, c - 1)];
+                    acc[q] = bj;
+                    xr[q] = reinterpret_cast<const float4*>(xs[r[q]]);
+                }
 #pragma unroll
                 for (int k = 0; k < 16; ++k) {          // one LDS.128 per four FMAs (the scalar form was LDS-bound)
-                    const float4 x4 = xr[k];
-                    acc = fmaf(w[4 * k], x4.x, acc); acc = fmaf(w[4 * k + 1], x4.y, acc);
-                    acc = fmaf(w[4 * k + 2], x4.z, acc); acc = fmaf(w[4 * k + 3], x4.w, acc);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const float4 x4 = xr[q][k];
+                        acc[q] = fmaf(w[4 * k], x4.x, acc[q]); acc[q] = fmaf(w[4 * k + 1], x4.y, acc[q]);
+                        acc[q] = fmaf(w[4 * k + 2], x4.z, acc[q]); acc[q] = fmaf(w[4 * k + 3], x4.w, acc[q]);
+                    }
                 }
-                int slot = sorted_row[row0 + r];
-                const float a = apply_act(acc, act);
-                const T hi = from_f32<T>(a);
-                h1[(int64_t)slot * d + j] = hi;
-                if (h1_lo) h1_lo[(int64_t)slot * d + j] = from_f32<T>(a - to_f32<T>(hi));
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    if (p + q >= c) break;
+                    const int slot = sorted_row[row0 + r[q]];
+                    const float a = apply_act(acc[q], act);
+                    const T hi = from_f32<T>(a);
+                    h1[(int64_t)slot * d + j] = hi;
+                    if (h1_lo) h1_lo[(int64_t)slot * d + j] = from_f32<T>(a - to_f32<T>(hi));
+                }
             }
         }
     }
@@ -499,6 +516,94 @@ k_heads_l2_vec(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden_
     }
 }
 
+// a8 output layer, bf16 path, at most 16 outputs: as k_heads_l2_vec, but every hidden vector is unpacked (hi + lo) once,
+// the head block of an output is chosen by a warp-uniform switch over statically indexed registers (no per-output
+// select chains), and the 16 per-lane partial sums are reduced together by a halving butterfly (16 shuffles instead
+// of 5 per output; the additions happen in the same order as warp_sum's, so the results are bit-identical to
+// k_heads_l2_vec's).  After the butterfly lane 2o holds output o.
+template <int HALF>
+__device__ __forceinline__ void heads_fold(float (&acc)[16], int lane) {
+    constexpr int BIT = HALF * 2;
+    const bool up = (lane & BIT) != 0;
+#pragma unroll
+    for (int j = 0; j < HALF; ++j) {
+        const float mine = up ? acc[j + HALF] : acc[j];
+        const float other = up ? acc[j] : acc[j + HALF];
+        acc[j] = mine + __shfl_xor_sync(0xffffffffu, other, BIT);
+    }
+}
+__device__ __forceinline__ float heads_dot8(const float (&h)[8], const float4& w0, const float4& w1, float a) {
+    a = fmaf(h[0], w0.x, a); a = fmaf(h[1], w0.y, a); a = fmaf(h[2], w0.z, a); a = fmaf(h[3], w0.w, a);
+    a = fmaf(h[4], w1.x, a); a = fmaf(h[5], w1.y, a); a = fmaf(h[6], w1.z, a); a = fmaf(h[7], w1.w, a);
+    return a;
+}
+template <int NCH>
+__global__ void __launch_bounds__(256)
+k_heads_l2_fold(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden_lo, int N, int d, int ld_hidden, int n_blk,
+                const float* __restrict__ W2, const float* __restrict__ b2, const int* __restrict__ valid, HeadsOut ho,
+                float* __restrict__ out_logits, float* __restrict__ out_regress) {
+    const int row = blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (row >= N) return;
+    const bool ok = valid[row] != 0;                          // warp-uniform
+    float acc[16];
+#pragma unroll
+    for (int o = 0; o < 16; ++o) acc[o] = 0.0f;
+    if (ok) {
+        float hv[5][NCH][8];
+#pragma unroll
+        for (int b = 0; b < 5; ++b)
+#pragma unroll
+            for (int ch = 0; ch < NCH; ++ch) {
+                const int c = ch * 256 + lane * 8;
+                uint4 h4 = make_uint4(0, 0, 0, 0), l4 = make_uint4(0, 0, 0, 0);
+                if (b < n_blk && c < d) {
+                    const int64_t off = (int64_t)row * ld_hidden + b * d + c;
+                    h4 = *reinterpret_cast<const uint4*>(hidden + off);
+                    if (hidden_lo) l4 = *reinterpret_cast<const uint4*>(hidden_lo + off);
+                }
+                const uint32_t hw[4] = {h4.x, h4.y, h4.z, h4.w}, lw[4] = {l4.x, l4.y, l4.z, l4.w};
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    hv[b][ch][2 * i] = __uint_as_float(hw[i] << 16) + __uint_as_float(lw[i] << 16);
+                    hv[b][ch][2 * i + 1] = __uint_as_float(hw[i] & 0xffff0000u) + __uint_as_float(lw[i] & 0xffff0000u);
+                }
+            }
+#pragma unroll
+        for (int o = 0; o < 16; ++o) {
+            if (o < ho.n_out) {
+                const int b = ho.blk[o];
+#pragma unroll
+                for (int ch = 0; ch < NCH; ++ch) {
+                    const int c = ch * 256 + lane * 8;
+                    if (c < d) {
+                        const float4* wp = reinterpret_cast<const float4*>(W2 + (int64_t)o * d + c);
+                        const float4 w0 = __ldg(wp), w1 = __ldg(wp + 1);
+                        switch (b) {
+                            case 0: acc[o] = heads_dot8(hv[0][ch], w0, w1, acc[o]); break;
+                            case 1: acc[o] = heads_dot8(hv[1][ch], w0, w1, acc[o]); break;
+                            case 2: acc[o] = heads_dot8(hv[2][ch], w0, w1, acc[o]); break;
+                            case 3: acc[o] = heads_dot8(hv[3][ch], w0, w1, acc[o]); break;
+                            default: acc[o] = heads_dot8(hv[4][ch], w0, w1, acc[o]); break;
+                        }
+                    }
+                }
+            }
+        }
+        heads_fold<8>(acc, lane);
+        heads_fold<4>(acc, lane);
+        heads_fold<2>(acc, lane);
+        heads_fold<1>(acc, lane);
+        acc[0] += __shfl_xor_sync(0xffffffffu, acc[0], 1);
+    }
+    const int o = lane >> 1;
+    if ((lane & 1) == 0 && o < ho.n_out) {
+        const float a = ok ? acc[0] + b2[o] : 0.0f;
+        if (o < ho.n_cls) out_logits[(int64_t)row * ho.n_cls + o] = a;
+        else out_regress[(int64_t)row * ho.n_reg + (o - ho.n_cls)] = a;
+    }
+}
+
 // int 0/1 per row -> one bit per row (kernel-level attention entry; the model path gets the bits from k_sched_count)
 __global__ void k_pack_valid_bits(const int* __restrict__ valid, int N, uint32_t* __restrict__ bits) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -612,7 +717,11 @@ void launch_heads_l2(bool fp32, const void* hidden, const void* hidden_lo, int N
     if (fp32) k_heads_l2<float><<<grid, 256, 0, st>>>((const float*)hidden, (const float*)hidden_lo, N, d, ld_hidden, W2, b2, valid, ho, out_logits, out_regress);
     else if (d <= 512 && d % 8 == 0 && ld_hidden % 8 == 0 && ld_hidden / d <= 5) {
         const int n_blk = ld_hidden / d;
-        if (d <= 256) k_heads_l2_vec<1><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress);
+        if (ho.n_out <= 16) {
+            if (d <= 256) k_heads_l2_fold<1><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress);
+            else k_heads_l2_fold<2><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress);
+        }
+        else if (d <= 256) k_heads_l2_vec<1><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress);
         else k_heads_l2_vec<2><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress);
     }
     else k_heads_l2<bf16><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, W2, b2, valid, ho, out_logits, out_regress);
