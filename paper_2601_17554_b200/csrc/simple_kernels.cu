@@ -120,8 +120,12 @@ k_sched_scatter(const float* __restrict__ X, int N, int F, const int* __restrict
 // W1t is [T][64][d] (k-major, zero padded to 64 features) so loads are coalesced over the d outputs.
 // ------------------------------------------------------------------------------------------------
 
+// 128 threads, each owning TWO output columns (j and j + d/2) with both weight columns in registers: every broadcast
+// LDS.128 of a row's features feeds 8 FMAs instead of 4 (the one-column form was bound by shared-memory operand
+// bandwidth: a 128-bit broadcast load costs 4 LSU cycles), two rows per pass for independent FMA chains.
+constexpr int EMB_THREADS = 128;
 template <typename T>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(EMB_THREADS, 3)
 k_embed_l1(const float* __restrict__ X, int N, int F, int d, const float* __restrict__ W1t,
            const float* __restrict__ b1, int act, const int* __restrict__ sorted_row,
            T* __restrict__ h1, T* __restrict__ h1_lo, float* __restrict__ h) {
@@ -131,7 +135,7 @@ k_embed_l1(const float* __restrict__ X, int N, int F, int d, const float* __rest
     const int row0 = blockIdx.x * EMB_ROWS;
     const int rows = min(EMB_ROWS, N - row0);
     if (threadIdx.x < 5) cnt[threadIdx.x] = 0;
-    for (int idx = threadIdx.x; idx < EMB_ROWS * 64; idx += 256) {
+    for (int idx = threadIdx.x; idx < EMB_ROWS * 64; idx += EMB_THREADS) {
         int r = idx >> 6, k = idx & 63;
         xs[r][k] = (r < rows && k < F) ? X[(int64_t)(row0 + r) * F + k] : 0.0f;
     }
@@ -145,44 +149,48 @@ k_embed_l1(const float* __restrict__ X, int N, int F, int d, const float* __rest
     // pad rows -> zero residual-stream rows
     for (int p = 0; p < cnt[0]; ++p) {
         int r = list[0][p];
-        for (int j = threadIdx.x; j < d; j += 256) h[(int64_t)(row0 + r) * d + j] = 0.0f;
+        for (int j = threadIdx.x; j < d; j += EMB_THREADS) h[(int64_t)(row0 + r) * d + j] = 0.0f;
     }
+    const int dh = d >> 1;
     for (int t = 1; t <= 4; ++t) {
         const int c = cnt[t];
         if (c == 0) continue;
-        for (int j = threadIdx.x; j < d; j += 256) {
-            float w[64];
+        for (int j = threadIdx.x; j < dh; j += EMB_THREADS) {
+            float wa[64], wb[64];
             const float* wp = W1t + ((int64_t)(t - 1) * 64) * d + j;
 #pragma unroll
-            for (int k = 0; k < 64; ++k) w[k] = wp[(int64_t)k * d];
-            const float bj = b1[(t - 1) * d + j];
-            for (int p = 0; p < c; p += 4) {            // four rows per pass: four independent FMA chains
-                int r[4];
-                float acc[4];
-                const float4* xr[4];
+            for (int k = 0; k < 64; ++k) { wa[k] = wp[(int64_t)k * d]; wb[k] = wp[(int64_t)k * d + dh]; }
+            const float bja = b1[(t - 1) * d + j], bjb = b1[(t - 1) * d + j + dh];
+            for (int p = 0; p < c; p += 2) {
+                const int r0 = list[t][p], r1 = list[t][min(p + 1, c - 1)];
+                float a0 = bja, a1 = bja, c0 = bjb, c1 = bjb;
+                const float4* x0 = reinterpret_cast<const float4*>(xs[r0]);
+                const float4* x1 = reinterpret_cast<const float4*>(xs[r1]);
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    r[q] = list[t][min(p + q, c - 1)];
-                    acc[q] = bj;
-                    xr[q] = reinterpret_cast<const float4*>(xs[r[q]]);
+                for (int k = 0; k < 16; ++k) {
+                    const float4 u = x0[k], v = x1[k];
+                    a0 = fmaf(wa[4 * k], u.x, a0); a0 = fmaf(wa[4 * k + 1], u.y, a0);
+                    a0 = fmaf(wa[4 * k + 2], u.z, a0); a0 = fmaf(wa[4 * k + 3], u.w, a0);
+                    c0 = fmaf(wb[4 * k], u.x, c0); c0 = fmaf(wb[4 * k + 1], u.y, c0);
+                    c0 = fmaf(wb[4 * k + 2], u.z, c0); c0 = fmaf(wb[4 * k + 3], u.w, c0);
+                    a1 = fmaf(wa[4 * k], v.x, a1); a1 = fmaf(wa[4 * k + 1], v.y, a1);
+                    a1 = fmaf(wa[4 * k + 2], v.z, a1); a1 = fmaf(wa[4 * k + 3], v.w, a1);
+                    c1 = fmaf(wb[4 * k], v.x, c1); c1 = fmaf(wb[4 * k + 1], v.y, c1);
+                    c1 = fmaf(wb[4 * k + 2], v.z, c1); c1 = fmaf(wb[4 * k + 3], v.w, c1);
                 }
+                const float acc[2][2] = {{a0, c0}, {a1, c1}};
+                const int rr[2] = {r0, r1};
 #pragma unroll
-                for (int k = 0; k < 16; ++k) {          // one LDS.128 per four FMAs (the scalar form was LDS-bound)
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const float4 x4 = xr[q][k];
-                        acc[q] = fmaf(w[4 * k], x4.x, acc[q]); acc[q] = fmaf(w[4 * k + 1], x4.y, acc[q]);
-                        acc[q] = fmaf(w[4 * k + 2], x4.z, acc[q]); acc[q] = fmaf(w[4 * k + 3], x4.w, acc[q]);
-                    }
-                }
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
+                for (int q = 0; q < 2; ++q) {
                     if (p + q >= c) break;
-                    const int slot = sorted_row[row0 + r[q]];
-                    const float a = apply_act(acc[q], act);
-                    const T hi = from_f32<T>(a);
-                    h1[(int64_t)slot * d + j] = hi;
-                    if (h1_lo) h1_lo[(int64_t)slot * d + j] = from_f32<T>(a - to_f32<T>(hi));
+                    const int64_t slot = sorted_row[row0 + rr[q]];
+#pragma unroll
+                    for (int hcol = 0; hcol < 2; ++hcol) {
+                        const float a = apply_act(acc[q][hcol], act);
+                        const T hi = from_f32<T>(a);
+                        h1[slot * d + j + hcol * dh] = hi;
+                        if (h1_lo) h1_lo[slot * d + j + hcol * dh] = from_f32<T>(a - to_f32<T>(hi));
+                    }
                 }
             }
         }
@@ -651,8 +659,8 @@ int launch_schedule(const float* X, int N, int F, const int* offsets, int E, int
 void launch_embed_l1(bool fp32, const float* X, int N, int F, int d, const float* W1t, const float* b1, int act,
                      const int* sorted_row, void* h1, void* h1_lo, float* h, cudaStream_t st) {
     dim3 grid((N + EMB_ROWS - 1) / EMB_ROWS);
-    if (fp32) k_embed_l1<float><<<grid, 256, 0, st>>>(X, N, F, d, W1t, b1, act, sorted_row, (float*)h1, (float*)h1_lo, h);
-    else k_embed_l1<bf16><<<grid, 256, 0, st>>>(X, N, F, d, W1t, b1, act, sorted_row, (bf16*)h1, (bf16*)h1_lo, h);
+    if (fp32) k_embed_l1<float><<<grid, EMB_THREADS, 0, st>>>(X, N, F, d, W1t, b1, act, sorted_row, (float*)h1, (float*)h1_lo, h);
+    else k_embed_l1<bf16><<<grid, EMB_THREADS, 0, st>>>(X, N, F, d, W1t, b1, act, sorted_row, (bf16*)h1, (bf16*)h1_lo, h);
 }
 
 template <typename T>
