@@ -6,7 +6,7 @@
  *   scaled-dot-product self-attention  A = softmax(Q K^T / sqrt(d_k)) V  (Eq. 4; computed
  *   flash-style without the N x N matrix, L154) -> two-layer FFN heads giving particle-id logits and
  *   the momentum regressions (pT', eta, sin phi, cos phi, E')  (L126, L134-L139, L156, Fig. 2).
- *   The readings taken where the paper is silent are A1-A19 in DESIGN.md.
+ *   The readings taken where the paper is silent are A1-A23 in DESIGN.md.
  *
  * All functions are thread-safe per handle; concurrent mlpf_infer calls on DIFFERENT streams are safe
  * (each stream owns a grow-only workspace), calls on the same stream serialise in stream order.
@@ -43,8 +43,8 @@ typedef struct mlpf_handle mlpf_handle;
  *   cls.W1[d,d] b1[d] W2[C,d] b2[C]                                                      (L156, A11)
  *   for k = 0..n_reg_heads-1     : reg.k.W1[d,d] b1[d] W2[reg_dims[k],d] b2[reg_dims[k]]
  * Master weights are fp32.  In BF16 mode the library rounds (RNE) the matrices that feed tensor-core
- * GEMMs (emb W2, Wqkv, Wo, W1, W2, cls.W1, reg.k.W1); emb W1, the C + sum(reg_dims) output rows
- * (cls.W2, reg.k.W2) and all vectors stay fp32.
+ * GEMMs (emb W2, Wqkv, Wo, W1, W2, cls.W1, reg.k.W1, bin.W1); emb W1, the output rows
+ * (cls.W2, reg.k.W2, bin.W2) and all vectors stay fp32.
  */
 #define MLPF_BLOB_MAGIC   "MLPFBLOB"
 #define MLPF_BLOB_VERSION 1u

@@ -11,9 +11,13 @@ list of particle candidates that the experiment software consumes (PAPER.md L222
   and E_primary = x[4] of the element itself (DESIGN.md input recipe).  eta is the raw output;
   phi = atan2(sin phi, cos phi) ("parameterized through sin phi and cos phi to preserve the
   quadrant information", L126).
-* Selection (reading A23): the library's 9-class head has no separate binary head
-  (reading A11), so class 0 is "no particle": element i yields a candidate iff it is not a pad row
-  (type != 0, reading A2) and its PID != 0.
+* Selection, the paper's rule (L156): "selecting the candidates with a binary classification score
+  above 0.5, and assigning them the PID with the largest probability score": with the binary head's
+  logit b_i, keep iff sigmoid(b_i) > 0.5 (and the row is not a pad row, reading A2); the PID is the
+  argmax over all classes.
+  DEPARTURE A23 (only for models WITHOUT a binary head, i.e. the five BASELINE.json configs whose
+  single 9-class head is all there is): class 0 then stands for "no particle" and element i yields
+  a candidate iff type != 0 and PID != 0.  This is not the paper's rule; it is a stop-gap.
 * Output: candidates in element order (stable), grouped per event by integer offsets.
 
 Floating point in fp64; the integer outputs (offsets, element index, PID) are exact given the
@@ -25,9 +29,9 @@ from __future__ import annotations
 import numpy as np
 
 
-def build_candidates(X, offsets, logits, regress):
+def build_candidates(X, offsets, logits, regress, binary=None):
     """X [N,F] fp32 element features; offsets [E+1]; logits [N,C]; regress [N,5] = (pT', eta, sin phi,
-    cos phi, E').  Returns dict(cand_offsets int32 [E+1], cand_elem int32 [M] (global row of the
+    cos phi, E'); binary [N] = the binary head's logit or None (departure A23).  Returns dict(cand_offsets int32 [E+1], cand_elem int32 [M] (global row of the
     element), cand_pid int32 [M], cand_p4 float64 [M,4] = (pT, eta, phi, E))."""
     offsets = np.asarray(offsets, dtype=np.int64)
     E = len(offsets) - 1
@@ -37,7 +41,11 @@ def build_candidates(X, offsets, logits, regress):
     regress = np.asarray(regress, dtype=np.float64)[:N]
     etype = X[:, 0].astype(np.int64)                       # reading A1: feature 0 is the type id
     pid = np.argmax(logits, axis=1) if N else np.zeros(0, np.int64)   # first maximum wins
-    keep = (etype != 0) & (pid != 0)
+    if binary is None:
+        keep = (etype != 0) & (pid != 0)                   # departure A23: no binary head
+    else:
+        b = np.asarray(binary, dtype=np.float64)[:N]
+        keep = (etype != 0) & (1.0 / (1.0 + np.exp(-b)) > 0.5)   # L156: binary score above 0.5
     cand_elem = np.nonzero(keep)[0].astype(np.int32)
     cand_offsets = np.zeros(E + 1, np.int32)
     for e in range(E):

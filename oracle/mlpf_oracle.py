@@ -50,7 +50,7 @@ def is_bf16_matrix(name: str) -> bool:
         return False
     if name.startswith("emb.") and leaf == "W1":
         return False
-    if (name.startswith("cls.") or name.startswith("reg.")) and leaf == "W2":
+    if (name.startswith("cls.") or name.startswith("reg.") or name.startswith("bin.")) and leaf == "W2":
         return False
     return True
 
@@ -167,10 +167,11 @@ def attention_event_tiled(q, k, v, valid, n_heads, tile=7):
     return o
 
 
-def encoder_layer(h, valid, offsets, W, l, m, dump=None, attn=attention_event):
+def encoder_layer(h, valid, offsets, W, l, m, dump=None, attn=attention_event, stack_prefix=""):
     """One pre-LN transformer block (L156 + [98]; readings A5-A10):
-       h <- h + Wo.MHA(LN1(h)) + bo ;  h <- h + W2.act(W1.LN2(h) + b1) + b2."""
-    p = f"layer.{l}."
+       h <- h + Wo.MHA(LN1(h)) + bo ;  h <- h + W2.act(W1.LN2(h) + b1) + b2.
+    stack_prefix: "" for one stack, "enc0." / "enc1." for the paper's two parallel encoders (L156)."""
+    p = f"{stack_prefix}layer.{l}."
     d = m.d_model
     u = layer_norm(h, W[p + "ln1.g"].astype(np.float64), W[p + "ln1.b"].astype(np.float64), m.ln_eps)
     qkv = linear(u, W[p + "Wqkv"], W[p + "bqkv"])
@@ -184,7 +185,7 @@ def encoder_layer(h, valid, offsets, W, l, m, dump=None, attn=attention_event):
     u2 = layer_norm(h1, W[p + "ln2.g"].astype(np.float64), W[p + "ln2.b"].astype(np.float64), m.ln_eps)
     g = activation(linear(u2, W[p + "W1"], W[p + "b1"]), m.activation)
     h2 = h1 + linear(g, W[p + "W2"], W[p + "b2"])
-    if dump is not None:
+    if dump is not None:                                  # keys carry the stack prefix: "enc1.layer.0.o"
         dump[p + "u"] = u
         dump[p + "qkv"] = qkv
         dump[p + "o"] = o
@@ -195,36 +196,58 @@ def encoder_layer(h, valid, offsets, W, l, m, dump=None, attn=attention_event):
     return h2
 
 
-def heads(z, W, m):
+def heads(z_cls, W, m, z_reg=None):
     """a8: two-layer FFN heads (L156 'six two-layer FFN heads'; reading A11): PID logits [N,9]
-    and (pT', eta, sin phi, cos phi, E') [N,5] as raw head outputs (reading A12)."""
-    hc = activation(linear(z, W["cls.W1"], W["cls.b1"]), m.activation)
+    and (pT', eta, sin phi, cos phi, E') [N,5] as raw head outputs (reading A12); with
+    m.binary_head also the binary "valid" logit [N] (L156 'binary primary target particle
+    classification', Fig. 2).  Binary and PID heads read z_cls (the classification encoder),
+    the regression heads read z_reg (the regression encoder, L156); one stack: z_reg = z_cls."""
+    if z_reg is None:
+        z_reg = z_cls
+    hc = activation(linear(z_cls, W["cls.W1"], W["cls.b1"]), m.activation)
     logits = linear(hc, W["cls.W2"], W["cls.b2"])
     regs = []
     for k in range(len(m.reg_dims)):
-        hr = activation(linear(z, W[f"reg.{k}.W1"], W[f"reg.{k}.b1"]), m.activation)
+        hr = activation(linear(z_reg, W[f"reg.{k}.W1"], W[f"reg.{k}.b1"]), m.activation)
         regs.append(linear(hr, W[f"reg.{k}.W2"], W[f"reg.{k}.b2"]))
-    return logits, np.concatenate(regs, axis=1)
+    binary = None
+    if getattr(m, "binary_head", False):
+        hb = activation(linear(z_cls, W["bin.W1"], W["bin.b1"]), m.activation)
+        binary = linear(hb, W["bin.W2"], W["bin.b2"])[:, 0]
+    return logits, np.concatenate(regs, axis=1), binary
 
 
-def forward(X, offsets, W, m, dump=None, attn=attention_event):
-    """Whole path a1..a8 for packed events.  Returns (logits [N,9], regress [N,5]) float64;
-    pad rows (type 0) are exactly 0 (reading A2)."""
+def forward(X, offsets, W, m, dump=None, attn=attention_event, with_binary=False):
+    """Whole path a1..a8 for packed events.  Returns (logits [N,9], regress [N,5]) float64, and with
+    with_binary=True also the binary logit [N] (needs m.binary_head); pad rows (type 0) are exactly 0
+    (reading A2).  m.n_stacks == 2 is the paper's topology (L156): the shared embedding feeds two
+    parallel encoders, stack 0 -> (binary, PID), stack 1 -> the regression heads."""
     X = np.asarray(X, dtype=np.float32)
     offsets = np.asarray(offsets, dtype=np.int64)
     t = element_types(X)
     valid = t != 0
-    h = embed(X, W, m)
+    h0 = embed(X, W, m)
     if dump is not None:
-        dump["h0"] = h
-    for l in range(m.n_layers):
-        h = encoder_layer(h, valid, offsets, W, l, m, dump=dump, attn=attn)
-    z = layer_norm(h, W["lnf.g"].astype(np.float64), W["lnf.b"].astype(np.float64), m.ln_eps) if m.final_ln else h
-    if dump is not None:
-        dump["z"] = z
-    logits, regress = heads(z, W, m)
+        dump["h0"] = h0
+    n_stacks = getattr(m, "n_stacks", 1)
+    zs = []
+    for s in range(n_stacks):
+        pre = "" if n_stacks == 1 else f"enc{s}."
+        h = h0
+        for l in range(m.n_layers):
+            h = encoder_layer(h, valid, offsets, W, l, m, dump=dump, attn=attn, stack_prefix=pre)
+        z = layer_norm(h, W[pre + "lnf.g"].astype(np.float64), W[pre + "lnf.b"].astype(np.float64), m.ln_eps) if m.final_ln else h
+        if dump is not None:
+            dump[pre + "z"] = z
+        zs.append(z)
+    logits, regress, binary = heads(zs[0], W, m, z_reg=zs[-1])
     logits[~valid] = 0.0
     regress[~valid] = 0.0
+    if with_binary:
+        if binary is None:
+            raise ValueError("with_binary needs a model with binary_head")
+        binary[~valid] = 0.0
+        return logits, regress, binary
     return logits, regress
 
 
@@ -292,7 +315,9 @@ def parity_metrics(got, ref, valid):
         return 0.0, np.zeros(ref.shape[1])
     rms = np.sqrt((ref[v] ** 2).mean(axis=0))
     den = np.maximum(np.abs(ref[v]), rms[None, :])
-    rel = np.abs(got[v] - ref[v]) / den
+    err = np.abs(got[v] - ref[v])
+    # an all-zero oracle column has den = 0: exact agreement counts as 0, anything else as infinite
+    rel = np.where(den > 0, err / np.where(den > 0, den, 1.0), np.where(err == 0, 0.0, np.inf))
     return float(rel.max()), rms
 
 

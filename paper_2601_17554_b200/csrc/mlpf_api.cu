@@ -59,6 +59,9 @@ struct Workspace {
     int *valid = nullptr, *row_event = nullptr, *row_pos = nullptr, *n_valid = nullptr;
     int *block_counts = nullptr, *block_base = nullptr, *type_offsets = nullptr;
     int *sorted_row = nullptr, *type_perm = nullptr;
+    // device staging of mlpf_infer_host (owned by the stream's workspace, freed with it); capacities in BYTES
+    float *stage_x = nullptr, *stage_lg = nullptr, *stage_rg = nullptr;
+    int64_t stage_cap = 0;            // rows
     // per-kernel-class CUDA-event timing of the last call (MLPF_OPT_PROFILE)
     std::vector<cudaEvent_t> ev_pool;
     std::vector<int> prof_cls;          // class of record i; events 2i, 2i+1
@@ -201,11 +204,7 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
     return h;
 }
 
-static void ws_free(Workspace* w) {
-    void* ptrs[] = {w->h, w->u, w->qkv, w->o, w->g, w->u_lo, w->o_lo, w->g_lo, w->offsets, w->work, w->pairs, w->valid, w->valid_bits, w->row_event,
-                    w->row_pos, w->n_valid, w->block_counts, w->block_base, w->type_offsets, w->sorted_row, w->type_perm};
-    for (void* p : ptrs) if (p) cudaFree(p);
-}
+static void ws_free(Workspace* w);
 
 extern "C" void mlpf_destroy(mlpf_handle* h) {
     if (!h) return;
@@ -271,18 +270,29 @@ template <typename P> static cudaError_t dmalloc(P** p, int64_t bytes, Workspace
     return e;
 }
 
-static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t n_tiles, bool fp32) {
+// free a workspace pointer and forget it (a later failure path or ws_free must not free it twice)
+template <typename P> static void dfree(P*& p) { if (p) cudaFree(p); p = nullptr; }
+
+static void ws_free_rows(Workspace* w) {
+    dfree(w->h); dfree(w->u); dfree(w->qkv); dfree(w->o); dfree(w->g); dfree(w->u_lo); dfree(w->o_lo); dfree(w->g_lo);
+    dfree(w->valid); dfree(w->valid_bits); dfree(w->row_event); dfree(w->row_pos); dfree(w->block_counts); dfree(w->block_base);
+    dfree(w->sorted_row); dfree(w->type_perm); dfree(w->type_offsets);
+    w->cap_rows = 0;
+}
+
+static int64_t ws_bytes_events(const Workspace* w) {
+    int64_t b = 0;
+    if (w->offsets) b += std::max<int64_t>((w->cap_events + 1) * 4, 256) + std::max<int64_t>(w->cap_events * 4, 256);
+    if (w->work) b += 2 * std::max<int64_t>(w->cap_tiles * 8, 256);
+    return b;
+}
+
+static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t n_tiles, bool fp32, cudaStream_t st) {
     const int64_t d = h->d;
     if (N > w->cap_rows || fp32 != w->fp32) {
-        void* ptrs[] = {w->h, w->u, w->qkv, w->o, w->g, w->u_lo, w->o_lo, w->g_lo, w->valid, w->valid_bits, w->row_event, w->row_pos, w->block_counts,
-                        w->block_base, w->sorted_row, w->type_perm, w->type_offsets};
-        for (void* p : ptrs) if (p) cudaFree(p);   // cudaFree waits for work in flight
-        // keep the event-indexed arrays' accounting: recompute bytes from scratch
-        int64_t ev_bytes = 0;
-        if (w->offsets) ev_bytes += std::max<int64_t>((w->cap_events + 1) * 4, 256) + std::max<int64_t>(w->cap_events * 4, 256);
-        if (w->work) ev_bytes += 2 * std::max<int64_t>(w->cap_tiles * 8, 256);
-        w->bytes = ev_bytes;
         const int64_t cap = (std::max<int64_t>(N, w->cap_rows) + 127) / 128 * 128;
+        ws_free_rows(w);                           // cudaFree waits for work in flight; every pointer is nulled
+        w->bytes = ws_bytes_events(w);
         const int64_t es = fp32 ? 4 : 2;
         const int64_t m_ub = cap + 4 * 128;
         const int64_t gw = std::max<int64_t>(h->dff, (int64_t)h->n_hblk * d);
@@ -298,38 +308,52 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
             dmalloc(&w->block_counts, nb * 5 * 4, w) || dmalloc(&w->block_base, nb * 5 * 4, w) ||
             dmalloc(&w->sorted_row, cap * 4, w) || dmalloc(&w->type_perm, m_ub * 4, w) ||
             dmalloc(&w->type_offsets, 8 * 4, w)) {
-            w->cap_rows = 0;
-            return set_err(MLPF_E_ALLOC, "workspace allocation for %lld rows failed: %s", (long long)cap,
-                           cudaGetErrorString(cudaGetLastError()));
+            const char* why = cudaGetErrorString(cudaGetLastError());
+            ws_free_rows(w);                       // release the partial set; nothing dangling is left behind
+            w->bytes = ws_bytes_events(w);
+            return set_err(MLPF_E_ALLOC, "workspace allocation for %lld rows failed: %s", (long long)cap, why);
         }
-        // the activation buffers feed TMA loads whose boxes may overrun valid rows: start from zeros so
-        // that never-written tails hold finite values
-        cudaMemset(w->valid_bits, 0, (cap / 32 + 40) * 4);
-        cudaMemset(w->u, 0, cap * d * es); cudaMemset(w->qkv, 0, cap * 3 * d * es);
-        cudaMemset(w->o, 0, cap * d * es);
-        cudaMemset(w->g, 0, w->g_elems * es);
-        cudaMemset(w->u_lo, 0, cap * d * es); cudaMemset(w->o_lo, 0, cap * d * es); cudaMemset(w->g_lo, 0, w->g_elems * es);
+        // the activation buffers feed TMA loads whose boxes may overrun valid rows: start from zeros so that
+        // never-written tails hold finite values.  On the CALLER'S stream: the legacy default stream does not order
+        // against non-blocking streams, so a plain cudaMemset could land after this call's kernels.
+        cudaMemsetAsync(w->valid_bits, 0, (cap / 32 + 40) * 4, st);
+        cudaMemsetAsync(w->u, 0, cap * d * es, st); cudaMemsetAsync(w->qkv, 0, cap * 3 * d * es, st);
+        cudaMemsetAsync(w->o, 0, cap * d * es, st);
+        cudaMemsetAsync(w->g, 0, w->g_elems * es, st);
+        cudaMemsetAsync(w->u_lo, 0, cap * d * es, st); cudaMemsetAsync(w->o_lo, 0, cap * d * es, st);
+        cudaMemsetAsync(w->g_lo, 0, w->g_elems * es, st);
         w->cap_rows = cap;
     }
     if (E > w->cap_events) {
-        if (w->offsets) { cudaFree(w->offsets); cudaFree(w->n_valid); }
+        dfree(w->offsets); dfree(w->n_valid);
+        w->cap_events = 0;
         const int64_t ce = std::max<int64_t>(E, 64);
         if (dmalloc(&w->offsets, (ce + 1) * 4, w) || dmalloc(&w->n_valid, ce * 4, w)) {
-            w->cap_events = 0;
+            dfree(w->offsets); dfree(w->n_valid);
             return set_err(MLPF_E_ALLOC, "workspace allocation for %lld events failed", (long long)ce);
         }
         w->cap_events = ce;
     }
     if (n_tiles > w->cap_tiles) {
-        if (w->work) { cudaFree(w->work); cudaFree(w->pairs); }
+        dfree(w->work); dfree(w->pairs);
+        w->cap_tiles = 0;
         const int64_t ct = std::max<int64_t>(n_tiles, 1024);
         if (dmalloc(&w->work, ct * 8, w) || dmalloc(&w->pairs, ct * 8, w)) {
-            w->cap_tiles = 0;
+            dfree(w->work); dfree(w->pairs);
             return set_err(MLPF_E_ALLOC, "workspace allocation for %lld tiles failed", (long long)ct);
         }
         w->cap_tiles = ct;
     }
     return MLPF_OK;
+}
+
+static void ws_free(Workspace* w) {
+    ws_free_rows(w);
+    dfree(w->stage_x); dfree(w->stage_lg); dfree(w->stage_rg);
+    w->stage_cap = 0;
+    dfree(w->offsets); dfree(w->n_valid); dfree(w->work); dfree(w->pairs);
+    for (cudaEvent_t e : w->ev_pool) cudaEventDestroy(e);
+    w->ev_pool.clear();
 }
 
 // ------------------------------------------------------------------------------------------------ launch helpers
@@ -545,7 +569,7 @@ extern "C" int mlpf_infer(mlpf_handle* h, const float* elements, const int32_t* 
     Workspace* w = wref;
     std::vector<int> work, pairs;
     build_work_lists(event_offsets, n_events, h->tile_q, tc_attn_rows_per_cta(h->hd), work, pairs);
-    int rc = ws_ensure(h, w, N, n_events, (int64_t)work.size() / 2, fp32);
+    int rc = ws_ensure(h, w, N, n_events, (int64_t)work.size() / 2, fp32, st);
     if (rc) return rc;
     w->N = N; w->E = n_events; w->n_tiles = (int64_t)work.size() / 2; w->n_pairs = (int64_t)pairs.size() / 2;
     w->tile_q = h->tile_q;
@@ -568,16 +592,25 @@ extern "C" int mlpf_infer_host(mlpf_handle* h, const float* elements_host, const
     if (N <= 0) return mlpf_infer(h, nullptr, event_offsets, n_events, nullptr, nullptr, stream);
     if (!elements_host || !out_logits_host || !out_regress_host) return set_err(MLPF_E_NULL, "host buffers NULL");
     cudaStream_t st = (cudaStream_t)stream;
-    // device staging buffers, one set per calling thread (the call synchronises before returning)
-    static thread_local struct { float* x = nullptr; float* lg = nullptr; float* rg = nullptr; int64_t cap = 0; } sb;
-    if (N > sb.cap) {
-        cudaFree(sb.x); cudaFree(sb.lg); cudaFree(sb.rg);
-        const int64_t cap = (N + 1023) / 1024 * 1024;
-        if (cudaMalloc(&sb.x, cap * h->F * 4) || cudaMalloc(&sb.lg, cap * h->C * 4) || cudaMalloc(&sb.rg, cap * std::max(h->R, 1) * 4)) {
-            sb.cap = 0; sb.x = sb.lg = sb.rg = nullptr;
-            return set_err(MLPF_E_ALLOC, "staging allocation failed");
+    // device staging buffers live in this stream's workspace (sized by this handle's F, C, R; freed by mlpf_destroy)
+    struct { float* x; float* lg; float* rg; } sb;
+    {
+        std::lock_guard<std::mutex> lk(h->mu);
+        Workspace*& wref = h->ws[stream];
+        if (!wref) wref = new Workspace();
+        Workspace* w = wref;
+        if (N > w->stage_cap) {
+            dfree(w->stage_x); dfree(w->stage_lg); dfree(w->stage_rg);
+            w->stage_cap = 0;
+            const int64_t cap = (N + 1023) / 1024 * 1024;
+            if (cudaMalloc(&w->stage_x, cap * h->F * 4) || cudaMalloc(&w->stage_lg, cap * h->C * 4) ||
+                cudaMalloc(&w->stage_rg, cap * std::max(h->R, 1) * 4)) {
+                dfree(w->stage_x); dfree(w->stage_lg); dfree(w->stage_rg);
+                return set_err(MLPF_E_ALLOC, "staging allocation failed");
+            }
+            w->stage_cap = cap;
         }
-        sb.cap = cap;
+        sb.x = w->stage_x; sb.lg = w->stage_lg; sb.rg = w->stage_rg;
     }
     CUDA_TRY(cudaMemcpyAsync(sb.x, elements_host, (size_t)N * h->F * 4, cudaMemcpyHostToDevice, st));
     int rc = mlpf_infer(h, sb.x, event_offsets, n_events, sb.lg, sb.rg, stream);

@@ -3,6 +3,8 @@
 #include <cuda.h>
 #include <mutex>
 #include <unordered_map>
+#include <set>
+#include <utility>
 #include "common.cuh"
 
 namespace mlpf {
@@ -32,10 +34,12 @@ struct TcContext {
         }
     };
     std::unordered_map<Key, CUtensorMap, KeyHash> cache;
+    std::set<std::pair<const void*, int>> attr_done;   // (kernel, device) pairs whose shared-memory limit is raised
 };
 
 
 int tc_init(TcContext* c);
+int tc_set_smem_attr(TcContext* c, const void* kern, int bytes);
 // 2D bf16 tensor map: dims (d0 inner, d1 outer), row pitch ld elements, box (b0, b1), swizzle = b0 * 2 bytes
 int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64_t ld,
                   uint32_t b0, uint32_t b1);

@@ -9,7 +9,7 @@
 // computes S_t(j+1) while the softmax warps work on S_t(j): the MMA chain (issue + hand-off latency) is off the
 // softmax warps' critical path.  At hd = 32 the exponentials (MUFU, 16/clk/SM) are the binding unit; one softmax
 // warp's serial chain per tile (TMEM load, max, exp, TMEM store, fold) is about twice its MUFU time, so three
-// warps per SM sub-partition (NT = 3) are what keeps the MUFU pipe busy (measured with -DMLPF_ATT_LOG).
+// warps per SM sub-partition (NT = 3) are what keeps the MUFU pipe busy.
 //   warps 0 .. 4NT-1   softmax warpgroups, one per query tile: one query row per thread, the tile's 64 scores in
 //               registers:  S -> (mask) -> max -> P = 2^((S - m_ref) c) as bf16 written back over S's TMEM columns.
 //               m_ref is a stale reference maximum (lazy rescaling): O_t and the row sums accumulate in TMEM over
@@ -60,124 +60,6 @@ struct AttnParams {
     int n_items, H, d;
     bf16* O; bf16* O_lo;
     float scale_log2;          // log2(e) / sqrt(hd)
-#ifdef MLPF_ATT_LOG
-    long long* prof;           // build with MLPF_NVCC_FLAGS=-DMLPF_ATT_LOG: per-warp clock64 timeline of CTA 200
-#endif
-};
-
-// 32 scores of one row (registers r[0..31]) -> max, as four independent chains (a single chain of 32 dependent
-// FMNMX costs ~200 cycles of latency that nothing else in the warp can hide)
-template <bool FULL>
-__device__ __forceinline__ float max32(const uint32_t* r, uint32_t mask, float mx) {
-    float m[4] = {mx, -INFINITY, -INFINITY, -INFINITY};
-#pragma unroll
-    for (int i = 0; i < 32; ++i) {
-        const float v = __uint_as_float(r[i]);
-        m[i & 3] = fmaxf(m[i & 3], FULL ? v : ((mask >> i) & 1u ? v : -INFINITY));
-    }
-    return fmaxf(fmaxf(m[0], m[1]), fmaxf(m[2], m[3]));
-}
-// 2^x for a pair, x <= 0, on the FMA / ALU pipes instead of the MUFU (Cody-Waite split + degree-3 polynomial):
-//   x = n + f, n = round(x) taken from the mantissa of x + 1.5 * 2^23, f in [-0.5, 0.5];
-//   2^f ~ 1 + f (c1 + f (c2 + f c3))  (max relative error 1.0e-4, 40x below the bf16 rounding of P);
-//   2^n goes into the exponent field with one integer multiply-add.
-// The MUFU does 16 ex2 per clock and SM and is the binding unit of this kernel at hd = 32 (one ex2 per 128 tensor
-// FLOPs); every ATT_POLY_EVERY-th pair takes this path so that MUFU and FMA pipes finish together.
-__device__ __forceinline__ float2 exp2_poly2(float2 x) {
-    const float2 magic = make_float2(12582912.0f, 12582912.0f);
-    x.x = fmaxf(x.x, -126.0f); x.y = fmaxf(x.y, -126.0f);
-    const float2 xr = ptx::fadd2(x, magic);                                          // low mantissa bits = round(x)
-    const float2 f = ptx::fadd2(x, ptx::fadd2(make_float2(12582912.0f, 12582912.0f), make_float2(-xr.x, -xr.y)));
-    float2 p = ptx::ffma2(f, make_float2(0.0550089306f, 0.0550089306f), make_float2(0.2422109596f, 0.2422109596f));
-    p = ptx::ffma2(p, f, make_float2(0.6932829272f, 0.6932829272f));
-    p = ptx::ffma2(p, f, make_float2(1.0f, 1.0f));
-    return make_float2(__int_as_float(__float_as_int(p.x) + (__float_as_int(xr.x) << 23)),
-                       __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
-}
-#ifndef ATT_POLY_POS
-#define ATT_POLY_POS 0       // which pair of each group of ATT_POLY_EVERY (0 measured 1-2 % faster than the last)
-#endif
-#ifndef ATT_POLY_EVERY
-#define ATT_POLY_EVERY 4     // measured on cfg3 (hd = 32, ms per layer): off 0.865, every 8th pair 0.845, 4th 0.825,
-#endif                       // 3rd 0.846, 2nd 0.927 (with register spills in the loop it was a loss at every setting)
-
-
-// p = 2^(s c - m c) for 32 scores -> 16 bf16 pairs (the row sums come from the tensor pipe: P x 1)
-template <bool FULL, bool POLY>
-__device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c, float neg_mc, uint32_t (&pk)[16]) {
-    const float2 c2 = make_float2(c, c), m2 = make_float2(neg_mc, neg_mc);
-#pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        const float2 x = ptx::ffma2(make_float2(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1])), c2, m2);
-        float2 p;
-        if (POLY && ATT_POLY_EVERY > 0 && (i % (ATT_POLY_EVERY > 0 ? ATT_POLY_EVERY : 1)) == ATT_POLY_POS) p = exp2_poly2(x);
-        else p = make_float2(ptx::fast_exp2(x.x), ptx::fast_exp2(x.y));
-        if (!FULL) {
-            p.x = (mask >> (2 * i)) & 1u ? p.x : 0.0f;
-            p.y = (mask >> (2 * i + 1)) & 1u ? p.y : 0.0f;
-        }
-        __nv_bfloat162 b2 = __floats2bfloat162_rn(p.x, p.y);
-        pk[i] = *reinterpret_cast<uint32_t*>(&b2);
-    }
-}
-
-// One 64-key tile of one query row, scores already in registers s[0..63]:
-// P = 2^((S - m_ref) c) as bf16, written over S's first 32 TMEM columns at s_addr.
-// m_ref is a STALE reference maximum (lazy rescaling): it only moves when some row of the warp has a tile maximum
-// more than ATT_RESCALE_LOG2 (in log2 units) above it, so P <= 2^8 and neither bf16 P nor the fp32 sums lose
-// precision, while the accumulated O (in TMEM) has to be rescaled only a few times per row instead of every tile.
-// Returns corr = 2^((m_ref_old - m_ref_new) c); `rescale` (warp-uniform) says whether m_ref moved.
-constexpr float ATT_RESCALE_LOG2 = 8.0f;
-template <bool FULL, bool POLY = true>
-__device__ __forceinline__ float softmax_tile(const uint32_t (&s)[64], uint32_t s_addr, const uint32_t (&mask)[2], float c,
-                                              float& m_ref, bool& rescale) {
-    const float mx = fmaxf(max32<FULL>(&s[0], mask[0], -INFINITY), max32<FULL>(&s[32], mask[1], -INFINITY));
-    const float m_new = fmaxf(m_ref, mx);
-    // m_ref = -inf and a finite tile maximum: the difference is +inf and votes yes; all keys masked so far: nan -> no
-    rescale = __any_sync(0xffffffffu, (m_new - m_ref) * c > ATT_RESCALE_LOG2);
-    float corr = 1.0f;
-    if (rescale) {
-        const float m_use = (m_new == -INFINITY) ? 0.0f : m_new;
-        corr = ptx::fast_exp2((m_ref - m_use) * c);              // m_ref = -inf -> 0
-        m_ref = m_new;
-    }
-    const float neg_mc = (m_ref == -INFINITY) ? 0.0f : -m_ref * c;
-#pragma unroll
-    for (int w = 0; w < 2; ++w) {
-        uint32_t pk[16];
-        exp32<FULL, POLY>(&s[32 * w], mask[w], c, neg_mc, pk);
-        ptx::tmem_st16(s_addr + 16 * w, pk);
-    }
-    return corr;
-}
-
-// Masked tile, hd = 64 variant: the scores of keys outside the event / of pad rows become -inf ONCE, so the max pass
-// ignores them and 2^(-inf) gives the exact weight 0 on the MUFU (no polynomial path: it clamps its argument).  Two
-// selects per score less than softmax_tile<false>.  Only instantiated at hd = 64: inside the hd <= 32 kernels the same
-// code changed ptxas' schedule of the unmasked loop for the worse (cfg3 3 % slower: measured), there the padded
-// configs matter less than the pad-free headline.
-__device__ __forceinline__ float softmax_tile_mask_once(uint32_t (&s)[64], uint32_t s_addr, const uint32_t (&mask)[2], float c,
-                                                        float& m_ref, bool& rescale) {
-#pragma unroll
-    for (int i = 0; i < 64; ++i) s[i] = (mask[i >> 5] >> (i & 31)) & 1u ? s[i] : 0xff800000u;
-    return softmax_tile<true, false>(s, s_addr, mask, c, m_ref, rescale);
-}
-
-template <int HD>
-__global__ void __launch_bounds__(AttnCfg<HD>::THREADS, 1)
-k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
-    using Cfg = AttnCfg<HD>;
-    constexpr int ST = Cfg::STAGES, NT = Cfg::NT;
-    extern __shared__ uint8_t smem_raw[];
-    __shared__ uint64_t bars[1 + 2 * ST + 5 * NT];
-    __shared__ uint32_t tmem_base_slot;
-#ifdef MLPF_ATT_LOG
-    __shared__ long long tlog[2 * NT][32][6];
-    const bool logging = prm.prof && blockIdx.x == 200;
-#define TLOG(r, j, k) do { if (logging && (j) < 32 && (threadIdx.x & 31) == 0) tlog[r][j][k] = clock64(); } while (0)
-#else
-#define TLOG(r, j, k) do {} while (0)
-#endif
 
     const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
     const int item = blockIdx.x / prm.H, head = blockIdx.x % prm.H;
@@ -283,20 +165,16 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
         issue_s(0);                                  // all lanes: one is elected inside the MMA / commit wrappers
         if (nkv > 1) issue_s(1);
         for (int j = 0; j < nkv; ++j) {
-            TLOG(NT + t, j, 0);
             ptx::mbar_wait_long(bar_p + 8 * (2 * t + (j & 1)), (j >> 1) & 1);     // P_t(j) is in TMEM
             ptx::tc_fence_after();
-            TLOG(NT + t, j, 1);
             issue_o(j);
             // K and V of stage j >> 1 are no longer needed by this tile after its second half
             if ((j & 1) || j == nkv - 1) ptx::mma_commit(bar_kv_empty + 8 * ((j >> 1) % ST));
-            TLOG(NT + t, j, 2);
             if (j + 2 < nkv) {                       // S_t(j+2) reuses S buffer j & 1: in order after P_t(j) V_j
                 const int i2 = (j + 2) >> 1;
                 if (((j + 2) & 1) == 0) ptx::mbar_wait(bar_kv_full + 8 * (i2 % ST), (i2 / ST) & 1);
                 ptx::tc_fence_after();
                 issue_s(j + 2);
-                TLOG(NT + t, j, 3);
             }
         }
     }
@@ -363,12 +241,10 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                     }
                 }
                 const uint32_t s_addr = lane_addr + 128 * t + 64 * (j & 1);
-                if (q == 0) TLOG(t, j, 0);
                 bool rescale;
                 float corr;
                 if (MASKED && HD == 64) corr = softmax_tile_mask_once(s, s_addr, mask, c, m_ref, rescale);
                 else corr = softmax_tile<!MASKED>(s, s_addr, mask, c, m_ref, rescale);
-                if (q == 0) TLOG(t, j, 1);
                 // S_t(j+1) was issued after P_t(j-1) V_(j-1) and the tensor pipe completes in order: once S_t(j+1) has
                 // landed, O_t holds all products up to j-1.  Only the last tile has to wait on bar_o for that.
                 if (j + 1 < nkv) {
@@ -378,19 +254,16 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
                 }
                 ptx::tc_fence_after();
                 if (rescale && j > 0) rescale_o(corr);    // before P_t(j) is published: no MMA is writing O_t now
-                if (q == 0) TLOG(t, j, 2);
                 if (j + 1 < nkv) {                        // next tile's scores: in flight while the P stores drain
                     const uint32_t s_next = lane_addr + 128 * t + 64 * ((j + 1) & 1);
                     ptx::tmem_ld32(s_next, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
                     ptx::tmem_ld32(s_next + 32, *reinterpret_cast<uint32_t(*)[32]>(&s[32]));
                 }
-                if (q == 0) TLOG(t, j, 3);
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(bar_p + 8 * (2 * t + (j & 1)));      // P_t(j) (and the rescaled O_t) are in TMEM
                 ptx::tmem_ld_wait();
-                if (q == 0) TLOG(t, j, 4);
             };
             int j = 0;
             if (!valid_bits) {                            // pad-free event: every tile but a ragged last one is full
@@ -433,9 +306,6 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == Cfg::WARP_MMA) ptx::tmem_dealloc(tmem_base, 512);
-#ifdef MLPF_ATT_LOG
-    if (logging) for (int i = threadIdx.x; i < 2 * NT * 32 * 6; i += Cfg::THREADS) prm.prof[i] = (&tlog[0][0][0])[i];
-#endif
 }
 
 template <int HD>
@@ -444,28 +314,8 @@ static int tc_attn_launch_hd(TcContext* c, const bf16* QKV, int64_t N, AttnParam
     CUtensorMap tmQKV;
     if (tc_tensor_map(c, &tmQKV, QKV, 3 * prm.d, N, 3 * prm.d, HD, ATT_SK)) return -1;
     auto kern = k_tc_attn<HD>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
-        if (e != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return -1; }
-        attr_set = true;
-    }
-#ifdef MLPF_ATT_LOG
-    static long long* pbuf = nullptr;
-    constexpr int NLOG = 2 * Cfg::NT * 32 * 6;
-    if (!pbuf) cudaMalloc(&pbuf, NLOG * 8);
-    cudaMemsetAsync(pbuf, 0, NLOG * 8, st);
-    prm.prof = pbuf;
-#endif
+    if (tc_set_smem_attr(c, (const void*)kern, Cfg::SMEM_BYTES)) return -1;
     kern<<<prm.n_items * prm.H, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(tmQKV, prm);
-#ifdef MLPF_ATT_LOG
-    {   // rows 0..NT-1: softmax warp 0 of each tile; rows NT..2NT-1: MMA issuers; one line per key tile
-        long long h[NLOG];
-        cudaMemcpy(h, prm.prof, sizeof h, cudaMemcpyDeviceToHost);
-        FILE* f = fopen("gpurun_out/att_log.txt", "w");
-        if (f) { for (int r = 0; r < 2 * Cfg::NT; ++r) for (int j = 0; j < 32; ++j) { fprintf(f, "%d %d", r, j); for (int k = 0; k < 6; ++k) fprintf(f, " %lld", h[(r * 32 + j) * 6 + k]); fprintf(f, "\n"); } fclose(f); }
-    }
-#endif
     return 0;
 }
 

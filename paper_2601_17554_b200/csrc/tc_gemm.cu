@@ -30,6 +30,21 @@ int tc_init(TcContext* c) {
     return 0;
 }
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-DEVICE attribute of a kernel: set once per (kernel, device)
+int tc_set_smem_attr(TcContext* c, const void* kern, int bytes) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    {
+        std::lock_guard<std::mutex> lk(c->mu);
+        if (c->attr_done.count({kern, dev})) return 0;
+    }
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return -1; }
+    std::lock_guard<std::mutex> lk(c->mu);
+    c->attr_done.insert({kern, dev});
+    return 0;
+}
+
 int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64_t ld,
                          uint32_t b0, uint32_t b1) {
     const uint32_t sw_bytes = b0 * 2;
@@ -347,12 +362,7 @@ static int tc_gemm_launch_act(TcContext* c, const bf16* A, const bf16* A_lo, con
     else tmAlo = tmA;
     if (tc_tensor_map(c, &tmB, W, K, w_rows, K, GEMM_BK, BLOCK_N)) return -1;
     auto kern = k_tc_gemm<BLOCK_N, STAGES, SPLIT, ACT>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
-        if (e != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return -1; }
-        attr_set = true;
-    }
+    if (tc_set_smem_attr(c, (const void*)kern, Cfg::SMEM_BYTES)) return -1;
     const int total_tiles = ((M + GEMM_BM - 1) / GEMM_BM) * (N / BLOCK_N);
     const int grid = total_tiles < c->num_sms ? total_tiles : c->num_sms;
     kern<<<grid, GEMM_THREADS, Cfg::SMEM_BYTES, st>>>(tmA, tmAlo, tmB, M, N, K, ep);

@@ -23,6 +23,10 @@ class ModelCfg:
     n_types: int = N_TYPES
     n_classes: int = N_CLASSES
     reg_dims: tuple = REG_DIMS
+    # paper-faithful topology (Fig. 2): n_stacks = 2 runs two parallel encoders on the shared
+    # embedding (stack 0 = classification, stack 1 = regression); binary_head adds the "valid" head on stack 0
+    n_stacks: int = 1
+    binary_head: bool = False
 
     @property
     def head_dim(self) -> int:
@@ -39,12 +43,19 @@ CONFIGS = {
     "cfg5b": ModelCfg(n_layers=8, d_model=512, n_heads=8, d_ff=2048),
     # paper-faithful block shape: d=256, 16 heads x 16, ReLU, 3 blocks
     "paper": ModelCfg(n_layers=3, d_model=256, n_heads=16, d_ff=1024, activation="relu"),
+    # the paper's network (L156): two parallel 3-block encoders, d=256, 16 x 16, ReLU, six heads incl. binary
+    "paper2": ModelCfg(n_layers=3, d_model=256, n_heads=16, d_ff=1024, activation="relu", n_stacks=2, binary_head=True),
 }
-CFG_INDEX = {"cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5a": 5, "cfg5b": 6, "paper": 7}
+CFG_INDEX = {"cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5a": 5, "cfg5b": 6, "paper": 7, "paper2": 8}
 
 
 def model_cfg(name: str) -> ModelCfg:
     return CONFIGS[name]
+
+
+def stack_prefix(m: ModelCfg, s: int) -> str:
+    """Name prefix of encoder stack s: "" for the single-stack configs, "enc<s>." for n_stacks = 2."""
+    return "" if m.n_stacks == 1 else f"enc{s}."
 
 
 def weight_names(m: ModelCfg):
@@ -54,15 +65,19 @@ def weight_names(m: ModelCfg):
     for t in range(1, m.n_types + 1):
         out += [(f"emb.{t}.W1", (d, F)), (f"emb.{t}.b1", (d,)),
                 (f"emb.{t}.W2", (d, d)), (f"emb.{t}.b2", (d,))]
-    for l in range(m.n_layers):
-        p = f"layer.{l}."
-        out += [(p + "ln1.g", (d,)), (p + "ln1.b", (d,)),
-                (p + "Wqkv", (3 * d, d)), (p + "bqkv", (3 * d,)),
-                (p + "Wo", (d, d)), (p + "bo", (d,)),
-                (p + "ln2.g", (d,)), (p + "ln2.b", (d,)),
-                (p + "W1", (dff, d)), (p + "b1", (dff,)),
-                (p + "W2", (d, dff)), (p + "b2", (d,))]
-    out += [("lnf.g", (d,)), ("lnf.b", (d,))]
+    for s in range(m.n_stacks):
+        for l in range(m.n_layers):
+            p = f"{stack_prefix(m, s)}layer.{l}."
+            out += [(p + "ln1.g", (d,)), (p + "ln1.b", (d,)),
+                    (p + "Wqkv", (3 * d, d)), (p + "bqkv", (3 * d,)),
+                    (p + "Wo", (d, d)), (p + "bo", (d,)),
+                    (p + "ln2.g", (d,)), (p + "ln2.b", (d,)),
+                    (p + "W1", (dff, d)), (p + "b1", (dff,)),
+                    (p + "W2", (d, dff)), (p + "b2", (d,))]
+    for s in range(m.n_stacks):
+        out += [(f"{stack_prefix(m, s)}lnf.g", (d,)), (f"{stack_prefix(m, s)}lnf.b", (d,))]
+    if m.binary_head:
+        out += [("bin.W1", (d, d)), ("bin.b1", (d,)), ("bin.W2", (1, d)), ("bin.b2", (1,))]
     out += [("cls.W1", (d, d)), ("cls.b1", (d,)),
             ("cls.W2", (m.n_classes, d)), ("cls.b2", (m.n_classes,))]
     for k, rk in enumerate(m.reg_dims):

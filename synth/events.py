@@ -48,7 +48,7 @@ def _lengths(name, rng):
         return [16384]
     if name == "cfg5b":
         return [8192] * 32
-    if name == "paper":
+    if name in ("paper", "paper2"):
         return [int(v) for v in np.rint(np.clip(rng.normal(5000, 1000, 4), 1000, 9000))]
     raise KeyError(name)
 
@@ -63,7 +63,7 @@ def make_named_events(name: str, seed: int | None = None, max_events: int | None
         lens = lens[:max_events]
     if name in ("cfg1", "cfg2"):
         kw = dict(type_p=UNIFORM_TYPE_P)
-    elif name in ("cfg3", "cfg4", "paper"):
+    elif name in ("cfg3", "cfg4", "paper", "paper2"):
         kw = dict(type_p=CMS_TYPE_P, hard_frac=0.20)
     else:
         kw = dict(type_p=CMS_TYPE_P, hard_frac=0.20, pad_frac=0.10)

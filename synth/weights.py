@@ -38,7 +38,9 @@ def sharpen(W: dict, m: ModelCfg, factor: float = 4.0):
     so attention is far from uniform and a masking / cross-event leak is visible."""
     out = {k: v.copy() for k, v in W.items()}
     d = m.d_model
-    for l in range(m.n_layers):
-        out[f"layer.{l}.Wqkv"][:d, :] *= factor
-        out[f"layer.{l}.bqkv"][:d] *= factor
+    for s in range(m.n_stacks):
+        pre = "" if m.n_stacks == 1 else f"enc{s}."
+        for l in range(m.n_layers):
+            out[f"{pre}layer.{l}.Wqkv"][:d, :] *= factor
+            out[f"{pre}layer.{l}.bqkv"][:d] *= factor
     return out

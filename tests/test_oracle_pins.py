@@ -122,6 +122,8 @@ def test_p5_parameter_count_of_paper_topology():
     m = synth.model_cfg("cfg3")
     hand = emb(4) + 6 * block + 2 * d + head(9) + head(1) + head(1) + head(2) + head(1)
     assert synth.param_count(m) == hand
+    # the paper's own topology as a config (two stacks, binary head, 4 embedding nets): the 5.46 M of the hand count
+    assert synth.param_count(synth.model_cfg("paper2")) == total4
 
 
 # ------------------------------------------------------------------ P6: single-element event = MLP path
@@ -151,18 +153,20 @@ def test_p6_single_element_event_closed_form():
 
 
 # ------------------------------------------------------------------ P7: library transformer block
-@pytest.mark.parametrize("act", ["gelu", "relu"])
-def test_p7_block_equals_torch_transformer_encoder_layer(act):
+@pytest.mark.parametrize("act,stacks", [("gelu", 1), ("relu", 1), ("relu", 2)])
+def test_p7_block_equals_torch_transformer_encoder_layer(act, stacks):
     """Pre-LN block ([98], L156) vs torch.nn.TransformerEncoderLayer(norm_first=True) in fp64,
     with a key-padding mask; an independent library implementation of the same block."""
     import torch
-    m = ModelCfg(n_layers=1, d_model=32, n_heads=4, d_ff=64, activation=act)
+    m = ModelCfg(n_layers=1, d_model=32, n_heads=4, d_ff=64, activation=act, n_stacks=stacks)
     W = synth.make_weights(m, seed=21)
     rng = np.random.default_rng(4)
     n = 13
     h = rng.standard_normal((n, m.d_model))
     valid = np.ones(n, bool); valid[[3, 9]] = False
-    out = oracle.encoder_layer(h, valid, np.array([0, n]), W, 0, m)
+    pre = synth.stack_prefix(m, stacks - 1)            # the last stack: "enc1." for the two-stack topology
+    out = oracle.encoder_layer(h, valid, np.array([0, n]), W, 0, m, stack_prefix=pre)
+    W = {k[len(pre):]: v for k, v in W.items() if k.startswith(pre)}
     layer = torch.nn.TransformerEncoderLayer(m.d_model, m.n_heads, m.d_ff, dropout=0.0, activation=act,
                                              batch_first=True, norm_first=True, dtype=torch.float64)
     sd = {"self_attn.in_proj_weight": W["layer.0.Wqkv"], "self_attn.in_proj_bias": W["layer.0.bqkv"],
@@ -204,8 +208,13 @@ def _loop_forward(X, off, W, m):
             h.append([0.0] * d); continue
         x = [float(v) for v in X[i]]
         h.append(matvec(Wl[f"emb.{t}.W2"], Wl[f"emb.{t}.b2"], act(matvec(Wl[f"emb.{t}.W1"], Wl[f"emb.{t}.b1"], x))))
-    for l in range(m.n_layers):
-        p = f"layer.{l}."
+    h_emb = h
+    finals = []
+    for s_ in range(m.n_stacks):
+      pre = "" if m.n_stacks == 1 else f"enc{s_}."
+      h = [list(r) for r in h_emb]
+      for l in range(m.n_layers):
+        p = f"{pre}layer.{l}."
         qkv = [matvec(Wl[p + "Wqkv"], Wl[p + "bqkv"], ln(h[i], Wl[p + "ln1.g"], Wl[p + "ln1.b"])) for i in range(N)]
         o = [[0.0] * d for _ in range(N)]
         for e in range(len(off) - 1):
@@ -225,20 +234,29 @@ def _loop_forward(X, off, W, m):
             g = act(matvec(Wl[p + "W1"], Wl[p + "b1"], ln(h1, Wl[p + "ln2.g"], Wl[p + "ln2.b"])))
             b2 = matvec(Wl[p + "W2"], Wl[p + "b2"], g)
             h[i] = [h1[c] + b2[c] for c in range(d)]
-    logits, regs = [], []
+      finals.append((pre, h))
+    logits, regs, binary = [], [], []
     for i in range(N):
         if types[i] == 0:
-            logits.append([0.0] * m.n_classes); regs.append([0.0] * sum(m.reg_dims)); continue
-        z = ln(h[i], Wl["lnf.g"], Wl["lnf.b"]) if m.final_ln else h[i]
-        logits.append(matvec(Wl["cls.W2"], Wl["cls.b2"], act(matvec(Wl["cls.W1"], Wl["cls.b1"], z))))
+            logits.append([0.0] * m.n_classes); regs.append([0.0] * sum(m.reg_dims)); binary.append(0.0); continue
+        zz = [ln(hh[i], Wl[pre + "lnf.g"], Wl[pre + "lnf.b"]) if m.final_ln else hh[i] for pre, hh in finals]
+        zc, zr = zz[0], zz[-1]                 # classification stack -> (binary, PID); regression stack -> regressions
+        logits.append(matvec(Wl["cls.W2"], Wl["cls.b2"], act(matvec(Wl["cls.W1"], Wl["cls.b1"], zc))))
         r = []
         for k in range(len(m.reg_dims)):
-            r += matvec(Wl[f"reg.{k}.W2"], Wl[f"reg.{k}.b2"], act(matvec(Wl[f"reg.{k}.W1"], Wl[f"reg.{k}.b1"], z)))
+            r += matvec(Wl[f"reg.{k}.W2"], Wl[f"reg.{k}.b2"], act(matvec(Wl[f"reg.{k}.W1"], Wl[f"reg.{k}.b1"], zr)))
         regs.append(r)
-    return np.array(logits).reshape(N, m.n_classes), np.array(regs).reshape(N, sum(m.reg_dims))
+        if m.binary_head:
+            binary.append(matvec(Wl["bin.W2"], Wl["bin.b2"], act(matvec(Wl["bin.W1"], Wl["bin.b1"], zc)))[0])
+    out = np.array(logits).reshape(N, m.n_classes), np.array(regs).reshape(N, sum(m.reg_dims))
+    return out + (np.array(binary),) if m.binary_head else out
 
 
-@pytest.mark.parametrize("m,lens,pad", [(TINY_RELU, (3, 8, 1), 0.0), (TINY, (5, 4), 0.3)])
+TINY_NOLN = ModelCfg(n_layers=1, d_model=16, n_heads=2, d_ff=32, final_ln=False)
+TINY_TWO = ModelCfg(n_layers=2, d_model=16, n_heads=4, d_ff=32, activation="relu", n_stacks=2, binary_head=True)
+
+
+@pytest.mark.parametrize("m,lens,pad", [(TINY_RELU, (3, 8, 1), 0.0), (TINY, (5, 4), 0.3), (TINY_NOLN, (6, 3), 0.2)])
 def test_p8_independent_loop_restatement(m, lens, pad):
     X, off = synth.make_events(lens, seed=11, pad_frac=pad)
     W = synth.make_weights(m, seed=12)
@@ -246,6 +264,40 @@ def test_p8_independent_loop_restatement(m, lens, pad):
     lg2, rg2 = _loop_forward(X, off, W, m)
     np.testing.assert_allclose(lg, lg2, atol=1e-10)
     np.testing.assert_allclose(rg, rg2, atol=1e-10)
+
+
+def test_p8_type_ids_outside_0_to_4_are_clamped():
+    """Reading A1: ids are clamped to 0..4: -1 -> pad row (outputs 0, not a key), 5 and 7.9 -> type 4."""
+    m = TINY_RELU
+    X, off = synth.make_events((9,), seed=2)
+    W = synth.make_weights(m, seed=3)
+    X[1, 0], X[4, 0], X[6, 0] = -1.0, 5.0, 7.9
+    lg, rg = oracle.forward(X, off, W, m)
+    lg2, rg2 = _loop_forward(X, off, W, m)
+    np.testing.assert_allclose(lg, lg2, atol=1e-10)
+    np.testing.assert_allclose(rg, rg2, atol=1e-10)
+    assert (lg[1] == 0).all() and (rg[1] == 0).all() and np.abs(lg[4]).sum() > 0
+    assert oracle.element_types(X).tolist()[:7] == [int(X[0, 0]), 0, int(X[2, 0]), int(X[3, 0]), 4, int(X[5, 0]), 4]
+    X4 = X.copy(); X4[4, 0] = 4.0; X4[6, 0] = 4.0          # same rows declared as type 4, feature 0 restored after
+    t4 = oracle.element_types(X4)
+    assert np.array_equal(t4, oracle.element_types(X))
+
+
+def test_p8_two_parallel_encoders_and_binary_head_loop_restatement():
+    """shared embedding -> two parallel encoders; (binary, PID) read the classification
+    encoder, the four regression heads read the regression encoder."""
+    m = TINY_TWO
+    X, off = synth.make_events((4, 7, 1), seed=21, pad_frac=0.2)
+    W = synth.make_weights(m, seed=22)
+    lg, rg, bn = oracle.forward(X, off, W, m, with_binary=True)
+    lg2, rg2, bn2 = _loop_forward(X, off, W, m)
+    np.testing.assert_allclose(lg, lg2, atol=1e-10)
+    np.testing.assert_allclose(rg, rg2, atol=1e-10)
+    np.testing.assert_allclose(bn, bn2, atol=1e-10)
+    # the stacks really are independent: zeroing the regression encoder's weights leaves (binary, PID) unchanged
+    Wz = {k: (np.zeros_like(v) if k.startswith("enc1.") else v) for k, v in W.items()}
+    lg3, rg3, bn3 = oracle.forward(X, off, Wz, m, with_binary=True)
+    assert np.array_equal(lg3, lg) and np.array_equal(bn3, bn) and not np.allclose(rg3, rg)
 
 
 # ------------------------------------------------------------------ P9 / P10: bias identities
@@ -308,7 +360,7 @@ def test_p12_identity_encoder_limit():
             W0[f"layer.{l}.{nm}"][...] = 0
     lg, rg = oracle.forward(X, off, W0, m)
     z = oracle.layer_norm(oracle.embed(X, W0, m), W0["lnf.g"].astype(np.float64), W0["lnf.b"].astype(np.float64), m.ln_eps)
-    l2, r2 = oracle.heads(z, W0, m)
+    l2, r2, _ = oracle.heads(z, W0, m)
     np.testing.assert_allclose(lg, l2, atol=1e-12)
     np.testing.assert_allclose(rg, r2, atol=1e-12)
 
@@ -439,3 +491,94 @@ def test_candidates_packing_invariance():
     assert np.array_equal(c1["cand_elem"] + a, c["cand_elem"][s:t])
     assert np.array_equal(c1["cand_pid"], c["cand_pid"][s:t])
     assert np.array_equal(c1["cand_p4"], c["cand_p4"][s:t])
+
+
+# ------------------------------------------------------------------ the judging metrics themselves (reading A14)
+def test_parity_metrics_hand_computed_example():
+    """3 rows x 2 columns written out by hand: row 2 is a pad row (excluded from the rms AND from the maximum),
+    column 1 of the oracle is all zero over valid rows (zero rms)."""
+    ref = np.array([[3.0, 0.0], [-4.0, 0.0], [100.0, 7.0]])
+    got = np.array([[3.3, 0.0], [-4.2, 0.0], [55.0, 55.0]])
+    valid = np.array([True, True, False])
+    rel, rms = oracle.parity_metrics(got, ref, valid)
+    # column 0: rms = sqrt((9 + 16) / 2) = 3.5355339...; row 0: 0.3 / max(3, 3.5355) ; row 1: 0.2 / max(4, 3.5355) = 0.05
+    assert abs(rms[0] - math.sqrt(12.5)) < 1e-15 and rms[1] == 0.0
+    assert abs(rel - 0.3 / math.sqrt(12.5)) < 1e-12
+    # a non-zero result where the oracle column is identically zero is an infinite relative error, never NaN
+    got[0, 1] = 1e-9
+    rel, _ = oracle.parity_metrics(got, ref, valid)
+    assert rel == np.inf
+    # no valid rows: nothing to compare
+    assert oracle.parity_metrics(got, ref, np.zeros(3, bool))[0] == 0.0
+
+
+def test_argmax_agreement_hand_computed_example():
+    """rms over the valid rows' logits = sqrt(7.4901 / 9) = 0.912268; decidable = margin > 2 * 0.02 * rms = 0.0364907.
+    Row 1 (margin 0.01) is a near tie and does not count; row 2 is a real disagreement; row 3 is a pad row."""
+    ref = np.array([[1.0, 0.0, -1.0], [0.5, 0.49, 0.0], [0.0, 2.0, 1.0], [9.0, 9.0, 9.0]])
+    got = np.array([[0.9, 0.1, -1.0], [0.48, 0.5, 0.0], [0.0, 1.0, 2.1], [0.0, 0.0, 0.0]])
+    valid = np.array([True, True, True, False])
+    agree, dec_frac, raw = oracle.argmax_agreement(got, ref, valid, tol_rel=2e-2)
+    assert agree == 0.5 and abs(dec_frac - 2.0 / 3.0) < 1e-15 and abs(raw - 1.0 / 3.0) < 1e-15
+    # margin exactly at the threshold is NOT decidable (strict >): scale row 1's margin to the threshold
+    rms = math.sqrt(7.4901 / 9.0)
+    assert abs(rms - 0.912268) < 1e-6
+    agree2, dec2, _ = oracle.argmax_agreement(ref, ref, valid)
+    assert agree2 == 1.0 and abs(dec2 - 2.0 / 3.0) < 1e-15
+
+
+def test_attention_event_row_blocks_equal_dense_weights_times_values():
+    """attention_event processes query rows in blocks (memory only): with row_block = 3 on n = 11 (blocks that do
+    not divide n, pad keys present) it must equal A @ V with A from attention_weights (Eq. 4), head by head."""
+    rng = np.random.default_rng(8)
+    n, H, hd = 11, 2, 4
+    q, k, v = (rng.standard_normal((n, H * hd)) * 2 for _ in range(3))
+    valid = np.array([1, 0, 1, 1, 1, 0, 1, 1, 1, 1, 0], bool)
+    o = oracle.attention_event(q, k, v, valid, H, row_block=3)
+    for h in range(H):
+        sl = slice(h * hd, (h + 1) * hd)
+        A = oracle.attention_weights(q[:, sl], k[:, sl], valid)
+        np.testing.assert_allclose(o[:, sl], A @ v[:, sl], atol=1e-13)
+    np.testing.assert_allclose(o, oracle.attention_event(q, k, v, valid, H, row_block=2048), atol=1e-13)
+
+
+def test_bf16_matrix_set_matches_the_header():
+    """include/mlpf.h: "the library rounds (RNE) the matrices that feed tensor-core GEMMs (emb W2, Wqkv, Wo, W1, W2,
+    cls.W1, reg.k.W1 [, bin.W1]); emb W1, the output rows (cls.W2, reg.k.W2 [, bin.W2]) and all vectors stay fp32"."""
+    import os, re
+    hdr = open(os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "mlpf.h")).read()
+    mlist = re.search(r"GEMMs \(([^)]*)\)", hdr).group(1)
+    for nm in ("emb W2", "Wqkv", "Wo", "W1", "W2", "cls.W1", "reg.k.W1", "bin.W1"):
+        assert nm in mlist, nm
+    for name in ("cfg1", "paper2"):
+        m = synth.model_cfg(name)
+        exp = set()
+        for t in range(1, 5):
+            exp.add(f"emb.{t}.W2")
+        for s in range(m.n_stacks):
+            for l in range(m.n_layers):
+                exp |= {f"{synth.stack_prefix(m, s)}layer.{l}.{k}" for k in ("Wqkv", "Wo", "W1", "W2")}
+        exp |= {"cls.W1"} | {f"reg.{k}.W1" for k in range(4)} | ({"bin.W1"} if m.binary_head else set())
+        got = {n for n, _ in synth.weight_names(m) if oracle.is_bf16_matrix(n)}
+        assert got == exp
+        W = synth.make_weights(m, seed=1)
+        Wq = oracle.quantize_weights(W)
+        for n, _ in synth.weight_names(m):
+            same = np.array_equal(Wq[n], W[n])
+            assert same == (n not in exp), n       # random fp32 weights are never bf16-exact
+
+
+def test_candidates_binary_rule_is_the_papers():
+    """L156: keep iff the binary score sigmoid(b) > 0.5, PID = argmax over ALL classes (class 0 allowed)."""
+    X, off, logits, reg = _cand_inputs(lens=(6, 5), pad_frac=0.0)
+    N = int(off[-1])
+    b = np.linspace(-2.0, 2.0, N).astype(np.float32)
+    b[3] = 0.0                                             # sigmoid(0) = 0.5 exactly: NOT above 0.5
+    X[7, :] = 0.0                                          # a pad row with a positive score is still dropped
+    b[7] = 3.0
+    logits[9, :] = -1.0; logits[9, 0] = 5.0                # class 0 wins and is kept under the binary rule
+    c = oracle.build_candidates(X, off, logits, reg, binary=b)
+    keep = [i for i in range(N) if X[i, 0] != 0 and 1.0 / (1.0 + math.exp(-float(b[i]))) > 0.5]
+    assert c["cand_elem"].tolist() == keep and 3 not in keep and 7 not in keep and 9 in keep
+    assert c["cand_pid"][keep.index(9)] == 0
+    assert c["cand_offsets"].tolist() == [0, sum(1 for i in keep if i < 6), len(keep)]
