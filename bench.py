@@ -357,7 +357,7 @@ def run_ours(args):
     achieved = fl["attn_per_launch"] / per_launch_s / 1e12 if at_n else None
     peak = peaks["tflops_sustained"]
     share = {c: round(t / max(sum(v[0] for v in cls.values()), 1e-9), 4) for c, (t, n) in cls.items()}
-    gemm_ms = sum(cls[c][0] for c in ("qkv", "outproj", "ffn1", "ffn2"))
+    gemm_ms = sum(cls[c][0] for c in ("qkv", "outproj", "ffn1", "ffn2", "post"))
     gemm_tflops = fl["gemm_per_layer"] * m.n_layers * args.steps / (gemm_ms * 1e-3) / 1e12 if gemm_ms else None
     traffic = None                                    # DRAM bytes per launch from the committed ncu --set full capture
     tpath = os.path.join(HERE, "profiles", "attn_traffic.json")

@@ -142,6 +142,9 @@ int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* 
 #define MLPF_SPLIT_ALL   63
 #define MLPF_OPT_PROFILE     6   /* 1: record a CUDA event pair around every kernel class inside mlpf_infer
                                     (read back with mlpf_debug_get_profile); 0 (default): off            */
+#define MLPF_OPT_FUSE        7   /* 1 (default): where the shape allows (d_model <= 256, d_ff % 128 == 0, all activations split)
+                                    the post-attention half of every block runs as ONE kernel (out-projection + residual +
+                                    LN2 + FFN1 + activation + FFN2 + residual + next LayerNorm); 0: one kernel per step   */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0
@@ -200,7 +203,8 @@ int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which, float* ho
 #define MLPF_KC_FFN2       8   /* a7 */
 #define MLPF_KC_HEADS_L1   9   /* a8 first layers */
 #define MLPF_KC_HEADS_L2   10  /* a8 output rows */
-#define MLPF_KC_COUNT      11
+#define MLPF_KC_POST       11  /* a5 + a6 + a7 fused (tc_post.cu) */
+#define MLPF_KC_COUNT      12
 int mlpf_debug_get_profile(mlpf_handle* h, void* stream, float* ms_out, int32_t* count_out);
 
 /* ---- kernel-level entry points (unit tests and micro-benchmarks; device pointers, bf16 = uint16) ---- */
@@ -214,6 +218,17 @@ int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* A_lo, const uint16_t* W
 int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_valid,
                            const int32_t* event_offsets, int32_t n_events, int32_t d_model, int32_t n_heads,
                            uint16_t* O, void* stream);
+
+/* The post-attention half of one encoder block (steps a5 + a6 + a7 with both LayerNorms in epilogues)
+ * as ONE kernel:  h <- h + (o_hi + o_lo) Wo^T + bo;  u2 = LN2(h);  h <- h + act(u2 W1^T + b1) W2^T + b2;
+ * u_out (+ u_out_lo) = bf16 hi (+ lo) of LN_next(h), or of h itself when lnng / lnnb are NULL.
+ * All DEVICE pointers: o_hi, o_lo, u_out, u_out_lo [M,d] bf16; h [M,d] fp32 in/out; Wo [d,d], W1 [dff,d], W2 [d,dff] bf16
+ * row-major [out,in]; vectors fp32.  d in {64,128,256}, dff % 128 == 0; activation 0 = ReLU, 1 = GELU (erf).
+ * Only enqueues on `stream`. */
+int mlpf_tc_post_bf16(const uint16_t* o_hi, const uint16_t* o_lo, float* h, const uint16_t* Wo, const float* bo,
+                      const float* ln2g, const float* ln2b, const uint16_t* W1, const float* b1, const uint16_t* W2,
+                      const float* b2, const float* lnng, const float* lnnb, int32_t M, int32_t d, int32_t dff,
+                      int32_t activation, float ln_eps, uint16_t* u_out, uint16_t* u_out_lo, void* stream);
 
 #ifdef __cplusplus
 }

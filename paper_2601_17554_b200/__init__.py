@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmlpf.so")
 
 # include/mlpf.h constants
 OK = 0
-OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE = 1, 2, 3, 4, 5, 6
+OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE, OPT_FUSE = 1, 2, 3, 4, 5, 6, 7
 PREC_BF16, PREC_FP32_DEBUG = 0, 1
 KERNELS_TC, KERNELS_SIMPLE = 0, 1
 Q_N_LAYERS, Q_D_MODEL, Q_N_HEADS, Q_D_FF, Q_N_FEAT, Q_N_CLASSES, Q_N_REGRESS = 1, 2, 3, 4, 5, 6, 7
@@ -24,11 +24,11 @@ Q_WEIGHT_BYTES, Q_WORKSPACE_BYTES, Q_N_PARAMS, Q_LAUNCHES = 8, 9, 10, 11
 SCHED = dict(row_event=0, row_pos=1, valid=2, n_valid=3, type_offsets=4, sorted_row=5, type_perm=6, work_list=7)
 TENSOR = dict(H=0, U=1, QK=2, V=3, O=4, G=5)
 KERNEL_CLASSES = ["sched", "embed_l1", "embed_l2", "layernorm", "qkv", "attention", "outproj", "ffn1", "ffn2",
-                  "heads_l1", "heads_l2"]
+                  "heads_l1", "heads_l2", "post"]
 
 EXPORTS = ["mlpf_create", "mlpf_infer", "mlpf_infer_host", "mlpf_destroy", "mlpf_last_error", "mlpf_set_option",
            "mlpf_query", "mlpf_debug_get_schedule", "mlpf_debug_get_tensor", "mlpf_debug_get_profile", "mlpf_tc_gemm_bf16",
-           "mlpf_tc_attention_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates"]
+           "mlpf_tc_attention_bf16", "mlpf_tc_post_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates"]
 
 _lib = None
 
@@ -67,6 +67,8 @@ def lib():
     L.mlpf_tc_gemm_bf16.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp]
     L.mlpf_tc_attention_bf16.restype = C.c_int
     L.mlpf_tc_attention_bf16.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
+    L.mlpf_tc_post_bf16.restype = C.c_int
+    L.mlpf_tc_post_bf16.argtypes = [vp] * 13 + [i32, i32, i32, i32, C.c_float, vp, vp, vp]
     L.mlpf_candidates_scratch_bytes.restype = i64
     L.mlpf_candidates_scratch_bytes.argtypes = [i64, i32]
     L.mlpf_build_candidates.restype = C.c_int
@@ -197,6 +199,21 @@ def tc_attention_bf16(QKV, key_valid, event_offsets, d_model, n_heads, stream=No
                                         off.ctypes.data_as(C.c_void_p), len(off) - 1, d_model, n_heads,
                                         C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
     return out
+
+
+def tc_post_bf16(o_hi, o_lo, h, Wo, bo, ln2g, ln2b, W1, b1, W2, b2, lnng, lnnb, activation, eps, want_lo=True, stream=None):
+    """The fused post-attention block (include/mlpf.h mlpf_tc_post_bf16).  CUDA tensors: o_hi / o_lo [M,d] bf16, h [M,d]
+    fp32 (updated in place), weights bf16 [out,in], vectors fp32 (lnng / lnnb may be None).  Returns (u_hi, u_lo)."""
+    import torch
+    M, d = h.shape
+    dff = W1.shape[0]
+    u_hi = torch.empty((M, d), dtype=torch.bfloat16, device=h.device)
+    u_lo = torch.empty((M, d), dtype=torch.bfloat16, device=h.device) if want_lo else None
+    ptr = lambda t: C.c_void_p(t.data_ptr() if t is not None else 0)
+    _check(lib().mlpf_tc_post_bf16(ptr(o_hi), ptr(o_lo), ptr(h), ptr(Wo), ptr(bo), ptr(ln2g), ptr(ln2b), ptr(W1), ptr(b1),
+                                   ptr(W2), ptr(b2), ptr(lnng), ptr(lnnb), M, d, dff, int(activation), float(eps),
+                                   ptr(u_hi), ptr(u_lo), _stream_ptr(stream)))
+    return u_hi, u_lo
 
 
 def build_candidates(elements, event_offsets, logits, regress, scratch=None, stream=None):

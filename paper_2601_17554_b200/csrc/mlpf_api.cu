@@ -81,7 +81,7 @@ struct mlpf_handle {
     std::vector<LayerW> layers;
     HeadsOut ho;
     // options
-    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0;
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1;
     int64_t last_launches = 0;
     std::mutex mu;
     std::map<void*, Workspace*> ws;
@@ -233,6 +233,9 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_PROFILE:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "profile must be 0 or 1");
             h->profile = (int)value; return MLPF_OK;
+        case MLPF_OPT_FUSE:
+            if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "fuse must be 0 or 1");
+            h->fuse = (int)value; return MLPF_OK;
         case MLPF_OPT_KERNELS:
             if (value != MLPF_KERNELS_TC && value != MLPF_KERNELS_SIMPLE) return set_err(MLPF_E_ARG, "bad kernel set");
             h->kernels = (int)value; return MLPF_OK;
@@ -470,14 +473,21 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     if (h->tap_layer == -2) return MLPF_OK;
 
     // ---- encoder blocks (pre-LN, L156 + A7)
+    // Fused form (d <= 256, all activations split): per block QKV GEMM, attention, and ONE kernel for
+    // out-projection + residual + LN2 + FFN1 + activation + FFN2 + residual + next LayerNorm (tc_post.cu); the only
+    // stand-alone LayerNorm left is the first block's LN1.  Otherwise (d = 512, fp32 debug path, CUDA-core kernels)
+    // the unfused chain of round 1 runs.
+    const bool fused = tc && h->fuse && sm == MLPF_SPLIT_ALL && tc_post_supported(d, dff);
+    bool u_ready = false;                    // u already holds LN(h) for the next consumer (written by a fused epilogue)
     for (int l = 0; l < h->L; ++l) {
         const LayerW& lw = h->layers[l];
         int rc;
-        {
+        if (!u_ready) {
             ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);
             rc = run_layernorm(h, fp32, w->h, N, PV + lw.ln1g, PV + lw.ln1b, u, nullptr, st);                     // a2
+            if (rc) return rc;
         }
-        if (rc) return rc;
+        u_ready = false;
         {   // a3: [Q K V] = LN1(x) Wqkv^T + bqkv
             ProfScope ps(h, w, st, MLPF_KC_QKV);
             Epi ep;
@@ -490,6 +500,30 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
             rc = run_attention(h, fp32, tc_attn, (sm & MLPF_SPLIT_O) != 0, w, st);                                                     // a4
         }
         if (rc) return rc;
+        if (fused) {   // a5 + a6 + a7 with both LayerNorms in epilogues
+            ProfScope ps(h, w, st, MLPF_KC_POST);
+            const bool last = l + 1 == h->L, tap = h->tap_layer == l;
+            PostArgs a;
+            a.M = N; a.d = d; a.dff = dff; a.act = h->act;
+            a.o = (const bf16*)w->o; a.o_lo = (const bf16*)w->o_lo;
+            a.Wo = (const bf16*)PW(lw.Wo); a.W1 = (const bf16*)PW(lw.W1); a.W2 = (const bf16*)PW(lw.W2);
+            a.bo = PV + lw.bo; a.ln2g = PV + lw.ln2g; a.ln2b = PV + lw.ln2b; a.b1 = PV + lw.b1; a.b2 = PV + lw.b2;
+            a.eps = h->hp.ln_eps; a.h = w->h;
+            if (!last) { a.lnng = PV + h->layers[l + 1].ln1g; a.lnnb = PV + h->layers[l + 1].ln1b; }
+            else if (h->hp.final_ln) { a.lnng = PV + h->lnfg; a.lnnb = PV + h->lnfb; }
+            else a.next_ln = 0;
+            if (tap) {               // the taps read u2 and g of THIS block: the next LN goes to scratch
+                a.dbg_u2 = (bf16*)w->u; a.dbg_g = (bf16*)w->g; a.u_out = (bf16*)w->g_lo;
+            } else {
+                a.u_out = (bf16*)w->u; a.u_out_lo = last ? (bf16*)w->u_lo : nullptr;
+            }
+            if (tc_post_launch(&h->tc, a, st)) return set_err(MLPF_E_CUDA, "fused post-attention launch failed: %s", h->tc.err);
+            LAUNCH_CHECK(h);
+            u_ready = true;
+            w->g_width = dff;
+            if (tap) return MLPF_OK;
+            continue;
+        }
         {   // a5: h <- h + O Wo^T + bo
             ProfScope ps(h, w, st, MLPF_KC_OUTPROJ);
             Epi ep;
@@ -521,7 +555,9 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     }
 
     // ---- a8: heads (L156; A11-A12)
-    if (h->hp.final_ln) {
+    if (u_ready) {
+        // the last block's fused epilogue already wrote u = LN_f(h) (or T(h)) as hi + lo
+    } else if (h->hp.final_ln) {
         ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);
         int rc = run_layernorm(h, fp32, w->h, N, PV + h->lnfg, PV + h->lnfb, u, lo(MLPF_SPLIT_UF, w->u_lo), st);
         if (rc) return rc;
@@ -749,6 +785,31 @@ extern "C" int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* A_lo, const 
         return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", ctx.err);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", cudaGetErrorString(e));
+    return MLPF_OK;
+}
+
+extern "C" int mlpf_tc_post_bf16(const uint16_t* o_hi, const uint16_t* o_lo, float* h, const uint16_t* Wo, const float* bo,
+                                 const float* ln2g, const float* ln2b, const uint16_t* W1, const float* b1, const uint16_t* W2,
+                                 const float* b2, const float* lnng, const float* lnnb, int32_t M, int32_t d, int32_t dff,
+                                 int32_t activation, float ln_eps, uint16_t* u_out, uint16_t* u_out_lo, void* stream) {
+    if (!o_hi || !o_lo || !h || !Wo || !bo || !ln2g || !ln2b || !W1 || !b1 || !W2 || !b2 || !u_out) return set_err(MLPF_E_NULL, "NULL argument");
+    if (M <= 0) return MLPF_OK;
+    if (!tc_post_supported(d, dff)) return set_err(MLPF_E_ARG, "need d in {64,128,256}, dff %% 128 == 0 (and the tile must fit shared memory)");
+    if (activation != 0 && activation != 1) return set_err(MLPF_E_ARG, "activation must be 0 (ReLU) or 1 (GELU)");
+    static TcContext ctx;
+    static std::once_flag once;
+    static int init_rc = 0;
+    std::call_once(once, [&] { init_rc = tc_init(&ctx); });
+    if (init_rc) return set_err(MLPF_E_CUDA, "tcgen05/TMA initialisation failed: %s", ctx.err);
+    PostArgs a;
+    a.M = M; a.d = d; a.dff = dff; a.act = activation == 0 ? ACT_RELU : ACT_GELU;
+    a.o = (const bf16*)o_hi; a.o_lo = (const bf16*)o_lo; a.Wo = (const bf16*)Wo; a.W1 = (const bf16*)W1; a.W2 = (const bf16*)W2;
+    a.bo = bo; a.ln2g = ln2g; a.ln2b = ln2b; a.b1 = b1; a.b2 = b2; a.lnng = lnng; a.lnnb = lnnb;
+    a.next_ln = (lnng && lnnb) ? 1 : 0;
+    a.eps = ln_eps; a.h = h; a.u_out = (bf16*)u_out; a.u_out_lo = (bf16*)u_out_lo;
+    if (tc_post_launch(&ctx, a, (cudaStream_t)stream)) return set_err(MLPF_E_CUDA, "fused post-attention launch failed: %s", ctx.err);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "fused post-attention launch failed: %s", cudaGetErrorString(e));
     return MLPF_OK;
 }
 

@@ -54,4 +54,21 @@ int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const uint32_t* val
                    const int* offsets, const int2* items, int n_items, int d, int H, bf16* O, bf16* O_lo,
                    cudaStream_t st);
 
+// The post-attention half of an encoder block as one kernel (tc_post.cu): h <- h + o Wo^T + bo; u2 = LN2(h);
+// h <- h + act(u2 W1^T + b1) W2^T + b2; u_out = LN_next(h) (or T(h) when next_ln == 0).  d in {64, 128, 256}, dff % 128 == 0.
+// n_groups > 1 (two parallel encoders): rows [g * group_rows, (g + 1) * group_rows) use weight block g of Wo [G*d, d],
+// W1 [G*dff, d], W2 [G*d, dff] and vector block g (vectors are [G, len]); group_rows % 128 == 0.
+struct PostArgs {
+    int M = 0, d = 0, dff = 0, act = ACT_GELU, n_groups = 1, group_rows = 0;
+    const bf16 *o = nullptr, *o_lo = nullptr, *Wo = nullptr, *W1 = nullptr, *W2 = nullptr;
+    const float *bo = nullptr, *ln2g = nullptr, *ln2b = nullptr, *b1 = nullptr, *b2 = nullptr, *lnng = nullptr, *lnnb = nullptr;
+    float eps = 1e-5f;
+    float* h = nullptr;
+    bf16 *u_out = nullptr, *u_out_lo = nullptr;
+    int next_ln = 1;
+    bf16 *dbg_u2 = nullptr, *dbg_g = nullptr;
+};
+bool tc_post_supported(int d, int dff);
+int tc_post_launch(TcContext* c, const PostArgs& a, cudaStream_t st);
+
 }  // namespace mlpf

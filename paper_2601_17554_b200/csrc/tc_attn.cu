@@ -60,6 +60,114 @@ struct AttnParams {
     int n_items, H, d;
     bf16* O; bf16* O_lo;
     float scale_log2;          // log2(e) / sqrt(hd)
+};
+
+// 32 scores of one row (registers r[0..31]) -> max, as four independent chains (a single chain of 32 dependent
+// FMNMX costs ~200 cycles of latency that nothing else in the warp can hide)
+template <bool FULL>
+__device__ __forceinline__ float max32(const uint32_t* r, uint32_t mask, float mx) {
+    float m[4] = {mx, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+        const float v = __uint_as_float(r[i]);
+        m[i & 3] = fmaxf(m[i & 3], FULL ? v : ((mask >> i) & 1u ? v : -INFINITY));
+    }
+    return fmaxf(fmaxf(m[0], m[1]), fmaxf(m[2], m[3]));
+}
+// 2^x for a pair, x <= 0, on the FMA / ALU pipes instead of the MUFU (Cody-Waite split + degree-3 polynomial):
+//   x = n + f, n = round(x) taken from the mantissa of x + 1.5 * 2^23, f in [-0.5, 0.5];
+//   2^f ~ 1 + f (c1 + f (c2 + f c3))  (max relative error 1.0e-4, 40x below the bf16 rounding of P);
+//   2^n goes into the exponent field with one integer multiply-add.
+// The MUFU does 16 ex2 per clock and SM and is the binding unit of this kernel at hd = 32 (one ex2 per 128 tensor
+// FLOPs); every ATT_POLY_EVERY-th pair takes this path so that MUFU and FMA pipes finish together.
+__device__ __forceinline__ float2 exp2_poly2(float2 x) {
+    const float2 magic = make_float2(12582912.0f, 12582912.0f);
+    x.x = fmaxf(x.x, -126.0f); x.y = fmaxf(x.y, -126.0f);
+    const float2 xr = ptx::fadd2(x, magic);                                          // low mantissa bits = round(x)
+    const float2 f = ptx::fadd2(x, ptx::fadd2(make_float2(12582912.0f, 12582912.0f), make_float2(-xr.x, -xr.y)));
+    float2 p = ptx::ffma2(f, make_float2(0.0550089306f, 0.0550089306f), make_float2(0.2422109596f, 0.2422109596f));
+    p = ptx::ffma2(p, f, make_float2(0.6932829272f, 0.6932829272f));
+    p = ptx::ffma2(p, f, make_float2(1.0f, 1.0f));
+    return make_float2(__int_as_float(__float_as_int(p.x) + (__float_as_int(xr.x) << 23)),
+                       __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
+}
+#ifndef ATT_POLY_POS
+#define ATT_POLY_POS 0       // which pair of each group of ATT_POLY_EVERY (0 measured 1-2 % faster than the last)
+#endif
+#ifndef ATT_POLY_EVERY
+#define ATT_POLY_EVERY 4     // measured on cfg3 (hd = 32, ms per layer): off 0.865, every 8th pair 0.845, 4th 0.825,
+#endif                       // 3rd 0.846, 2nd 0.927 (with register spills in the loop it was a loss at every setting)
+
+
+// p = 2^(s c - m c) for 32 scores -> 16 bf16 pairs (the row sums come from the tensor pipe: P x 1)
+template <bool FULL, bool POLY>
+__device__ __forceinline__ void exp32(const uint32_t* r, uint32_t mask, float c, float neg_mc, uint32_t (&pk)[16]) {
+    const float2 c2 = make_float2(c, c), m2 = make_float2(neg_mc, neg_mc);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const float2 x = ptx::ffma2(make_float2(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1])), c2, m2);
+        float2 p;
+        if (POLY && ATT_POLY_EVERY > 0 && (i % (ATT_POLY_EVERY > 0 ? ATT_POLY_EVERY : 1)) == ATT_POLY_POS) p = exp2_poly2(x);
+        else p = make_float2(ptx::fast_exp2(x.x), ptx::fast_exp2(x.y));
+        if (!FULL) {
+            p.x = (mask >> (2 * i)) & 1u ? p.x : 0.0f;
+            p.y = (mask >> (2 * i + 1)) & 1u ? p.y : 0.0f;
+        }
+        __nv_bfloat162 b2 = __floats2bfloat162_rn(p.x, p.y);
+        pk[i] = *reinterpret_cast<uint32_t*>(&b2);
+    }
+}
+
+// One 64-key tile of one query row, scores already in registers s[0..63]:
+// P = 2^((S - m_ref) c) as bf16, written over S's first 32 TMEM columns at s_addr.
+// m_ref is a STALE reference maximum (lazy rescaling): it only moves when some row of the warp has a tile maximum
+// more than ATT_RESCALE_LOG2 (in log2 units) above it, so P <= 2^8 and neither bf16 P nor the fp32 sums lose
+// precision, while the accumulated O (in TMEM) has to be rescaled only a few times per row instead of every tile.
+// Returns corr = 2^((m_ref_old - m_ref_new) c); `rescale` (warp-uniform) says whether m_ref moved.
+constexpr float ATT_RESCALE_LOG2 = 8.0f;
+template <bool FULL, bool POLY = true>
+__device__ __forceinline__ float softmax_tile(const uint32_t (&s)[64], uint32_t s_addr, const uint32_t (&mask)[2], float c,
+                                              float& m_ref, bool& rescale) {
+    const float mx = fmaxf(max32<FULL>(&s[0], mask[0], -INFINITY), max32<FULL>(&s[32], mask[1], -INFINITY));
+    const float m_new = fmaxf(m_ref, mx);
+    // m_ref = -inf and a finite tile maximum: the difference is +inf and votes yes; all keys masked so far: nan -> no
+    rescale = __any_sync(0xffffffffu, (m_new - m_ref) * c > ATT_RESCALE_LOG2);
+    float corr = 1.0f;
+    if (rescale) {
+        const float m_use = (m_new == -INFINITY) ? 0.0f : m_new;
+        corr = ptx::fast_exp2((m_ref - m_use) * c);              // m_ref = -inf -> 0
+        m_ref = m_new;
+    }
+    const float neg_mc = (m_ref == -INFINITY) ? 0.0f : -m_ref * c;
+#pragma unroll
+    for (int w = 0; w < 2; ++w) {
+        uint32_t pk[16];
+        exp32<FULL, POLY>(&s[32 * w], mask[w], c, neg_mc, pk);
+        ptx::tmem_st16(s_addr + 16 * w, pk);
+    }
+    return corr;
+}
+
+// Masked tile, hd = 64 variant: the scores of keys outside the event / of pad rows become -inf ONCE, so the max pass
+// ignores them and 2^(-inf) gives the exact weight 0 on the MUFU (no polynomial path: it clamps its argument).  Two
+// selects per score less than softmax_tile<false>.  Only instantiated at hd = 64: inside the hd <= 32 kernels the same
+// code changed ptxas' schedule of the unmasked loop for the worse (cfg3 3 % slower: measured), there the padded
+// configs matter less than the pad-free headline.
+__device__ __forceinline__ float softmax_tile_mask_once(uint32_t (&s)[64], uint32_t s_addr, const uint32_t (&mask)[2], float c,
+                                                        float& m_ref, bool& rescale) {
+#pragma unroll
+    for (int i = 0; i < 64; ++i) s[i] = (mask[i >> 5] >> (i & 31)) & 1u ? s[i] : 0xff800000u;
+    return softmax_tile<true, false>(s, s_addr, mask, c, m_ref, rescale);
+}
+
+template <int HD>
+__global__ void __launch_bounds__(AttnCfg<HD>::THREADS, 1)
+k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
+    using Cfg = AttnCfg<HD>;
+    constexpr int ST = Cfg::STAGES, NT = Cfg::NT;
+    extern __shared__ uint8_t smem_raw[];
+    __shared__ uint64_t bars[1 + 2 * ST + 5 * NT];
+    __shared__ uint32_t tmem_base_slot;
 
     const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
     const int item = blockIdx.x / prm.H, head = blockIdx.x % prm.H;

@@ -11,6 +11,7 @@
 // same accumulator, so activation rounding is ~2^-17 instead of 2^-9.
 #include "tc_api.h"
 #include "ptx.cuh"
+#include "epi_math.cuh"
 
 namespace mlpf {
 
@@ -87,26 +88,6 @@ struct GemmCfg {
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 16 * GEMM_STG_BYTES + 1024;   // ring + staging + alignment slack
     static constexpr int TMEM_COLS = 2 * BLOCK_N < 32 ? 32 : 2 * BLOCK_N;   // two accumulator buffers (power of 2)
 };
-
-// exact-erf GELU (reading A6) on two values, erf from Abramowitz & Stegun 7.1.26 (|error| <= 1.5e-7):
-//   GELU(x) = max(x, 0) - 0.5 |x| p(t) e^{-x^2/2},  t = 1 / (1 + 0.3275911 |x| / sqrt 2)
-// (for x < 0 this is 0.5 x (1 - erf|x/sqrt 2|) with no cancellation).  4 MUFU + ~18 FMA-pipe issue slots per
-// PAIR (packed FFMA2 / FMUL2) instead of erff's ~40 per value: the activation epilogues are issue-bound.
-__device__ __forceinline__ float2 gelu2(float2 x) {
-    float2 t;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t.x) : "f"(fmaf(fabsf(x.x), 0.23164189f, 1.0f)));
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t.y) : "f"(fmaf(fabsf(x.y), 0.23164189f, 1.0f)));
-    float2 p = ptx::ffma2(t, make_float2(1.061405429f, 1.061405429f), make_float2(-1.453152027f, -1.453152027f));
-    p = ptx::ffma2(p, t, make_float2(1.421413741f, 1.421413741f));
-    p = ptx::ffma2(p, t, make_float2(-0.284496736f, -0.284496736f));
-    p = ptx::ffma2(p, t, make_float2(0.254829592f, 0.254829592f));
-    p = ptx::fmul2(p, t);
-    const float2 xx = ptx::fmul2(ptx::fmul2(x, x), make_float2(-0.72134752044448170f, -0.72134752044448170f));  // -x^2/2 log2 e
-    const float2 e = make_float2(ptx::fast_exp2(xx.x), ptx::fast_exp2(xx.y));
-    const float2 a = make_float2(fabsf(x.x) * -0.5f, fabsf(x.y) * -0.5f);
-    const float2 h = ptx::fmul2(ptx::fmul2(p, e), a);                     // -0.5 |x| p e
-    return ptx::fadd2(make_float2(fmaxf(x.x, 0.0f), fmaxf(x.y, 0.0f)), h);
-}
 
 // ---- per-warp staging tile (4 KB of shared memory): the epilogue thread owns one ROW of the accumulator, so direct
 // global stores touch 32 different 128-byte lines per instruction (measured: ~1.6 TB/s for the whole GPU whatever

@@ -71,3 +71,145 @@ def test_tc_attention_matches_dense_softmax(hd, H, lens, pad):
         err = np.abs(O[a:b] - ref)
         scale = np.sqrt((ref ** 2).mean()) + 1e-6
         assert (err / np.maximum(np.abs(ref), scale)).max() <= 2e-2, (e, err.max(), scale)
+
+
+# ------------------------------------------------------------------------------------------- adversarial softmax inputs
+def _attn_check(qkv, lens, valid, hd, H, tol=2e-2):
+    """tcgen05 attention vs oracle.attention_event (Eq. 4 written out) element by element; the scale of the floor is
+    the rms of the oracle output of that event."""
+    d = hd * H
+    off = np.zeros(len(lens) + 1, np.int32)
+    off[1:] = np.cumsum(lens)
+    QKV = _bf16(qkv)
+    kv = None if valid is None else torch.from_numpy(valid.astype(np.int32)).cuda()
+    O = P.tc_attention_bf16(QKV, kv, off, d, H).float().cpu().numpy()
+    torch.cuda.synchronize()
+    assert np.isfinite(O).all()
+    q64 = QKV.float().cpu().numpy().astype(np.float64)
+    vv = np.ones(len(qkv), bool) if valid is None else valid
+    worst = 0.0
+    for e in range(len(lens)):
+        a, b = off[e], off[e + 1]
+        if b == a:
+            continue
+        ref = oracle.attention_event(q64[a:b, :d], q64[a:b, d:2 * d], q64[a:b, 2 * d:], vv[a:b], H)
+        scale = np.sqrt((ref ** 2).mean()) + 1e-6
+        worst = max(worst, float((np.abs(O[a:b] - ref) / np.maximum(np.abs(ref), scale)).max()))
+    assert worst <= tol, worst
+    return O
+
+
+@pytest.mark.parametrize("hd,H", [(32, 4), (64, 2), (16, 4)])
+def test_tc_attention_running_max_climbs_every_tile(hd, H):
+    """Keys ordered so that the row maximum rises by far more than 2^8 from one 64-key tile to the next (and, for the
+    rows with a negative query coefficient, falls): the reference maximum of an online softmax has to move on every
+    tile (or a one-shot bound has to be far from the first tiles' scores)."""
+    rng = np.random.default_rng(hd)
+    n, d = 1000, hd * H
+    qkv = (0.3 * rng.standard_normal((n, 3 * d))).astype(np.float32)
+    u = rng.standard_normal(d).astype(np.float32)
+    u /= np.sqrt((u.reshape(H, hd) ** 2).sum(axis=1)).repeat(hd)           # unit vector per head
+    ramp = np.linspace(0.0, 40.0, n, dtype=np.float32)                      # k.u rises by 0.04 per key ...
+    sign = np.where(rng.random(n) < 0.5, 1.0, -1.0).astype(np.float32)
+    qkv[:, :d] += 24.0 * sign[:, None] * u[None, :]                         # ... = 61 raw units per 64-key tile: 11 log2 units at hd = 64, 15 at hd = 32
+    qkv[:, d:2 * d] += ramp[:, None] * u[None, :]
+    _attn_check(qkv, (n,), None, hd, H)
+
+
+@pytest.mark.parametrize("hd,H", [(32, 4), (64, 2)])
+def test_tc_attention_outlier_key_in_the_last_tile(hd, H):
+    """One key 40 sigma away from the others, in the last (ragged) tile: every row's weight ends up on it."""
+    rng = np.random.default_rng(hd + 1)
+    n, d = 777, hd * H
+    qkv = rng.standard_normal((n, 3 * d)).astype(np.float32)
+    qkv[n - 3, d:2 * d] = 40.0 * np.sign(rng.standard_normal(d))
+    _attn_check(qkv, (n,), None, hd, H)
+
+
+@pytest.mark.parametrize("hd,H", [(32, 4), (64, 2)])
+def test_tc_attention_only_the_last_key_is_valid(hd, H):
+    """Every key but the last one of each event is a pad row: O must equal that key's V row for all queries."""
+    rng = np.random.default_rng(hd + 2)
+    lens = (300, 131)
+    n, d = sum(lens), hd * H
+    qkv = rng.standard_normal((n, 3 * d)).astype(np.float32)
+    valid = np.zeros(n, bool)
+    valid[[299, 430]] = True
+    O = _attn_check(qkv, lens, valid, hd, H)
+    v = _bf16(qkv).float().cpu().numpy()[:, 2 * d:]
+    assert np.abs(O[:300] - v[299]).max() <= 2e-2 * np.abs(v[299]).max()
+    assert np.abs(O[300:] - v[430]).max() <= 2e-2 * np.abs(v[430]).max()
+
+
+@pytest.mark.parametrize("hd,H", [(32, 4), (64, 2)])
+def test_tc_attention_sharp_scores_with_pad_rows(hd, H):
+    """10 % scattered pad rows together with Q x 8: a leaked pad key would carry real weight."""
+    rng = np.random.default_rng(hd + 3)
+    lens = (1500, 333, 900)
+    n, d = sum(lens), hd * H
+    qkv = rng.standard_normal((n, 3 * d)).astype(np.float32)
+    qkv[:, :d] *= 8.0
+    valid = rng.random(n) >= 0.10
+    qkv[~valid, d:2 * d] *= 3.0                           # pad keys would win the softmax if they were not masked
+    _attn_check(qkv, lens, valid, hd, H)
+
+
+@pytest.mark.parametrize("hd,H", [(32, 2), (64, 1)])
+def test_tc_attention_16384_keys(hd, H):
+    """The longest event of BASELINE.json (config 5): 16384 elements, 10 % pad rows, scores sharper than unit variance."""
+    rng = np.random.default_rng(hd + 4)
+    n, d = 16384, hd * H
+    qkv = rng.standard_normal((n, 3 * d)).astype(np.float32)
+    qkv[:, :d] *= 3.0
+    valid = rng.random(n) >= 0.10
+    _attn_check(qkv, (n,), valid, hd, H)
+
+
+def test_tc_attention_huge_scores():
+    """Scores near +-1e3 (|q.k| / sqrt(hd) up to ~1200): exponent range, not precision, is what is exercised."""
+    rng = np.random.default_rng(9)
+    hd, H, n = 32, 2, 500
+    d = hd * H
+    qkv = rng.standard_normal((n, 3 * d)).astype(np.float32)
+    qkv[:, :2 * d] *= 14.0
+    _attn_check(qkv, (n,), None, hd, H)
+
+
+# ------------------------------------------------------------------------------------------- fused post-attention block
+@pytest.mark.parametrize("M,d,dff,act", [(128, 256, 1024, "gelu"), (300, 256, 1024, "relu"), (77, 64, 256, "gelu"),
+                                         (1000, 128, 384, "gelu"), (20000, 256, 1024, "gelu"), (129, 256, 128, "relu")])
+@pytest.mark.parametrize("next_ln", [True, False])
+def test_tc_post_matches_the_block_written_out(M, d, dff, act, next_ln):
+    """k_tc_post against the same steps composed from the oracle's pieces (oracle.linear / layer_norm / activation) in
+    fp64 on the very bf16 operands the kernel reads: h2 to 2e-5 of its scale (fp32 accumulation), the LayerNorm outputs
+    to a few bf16-pair ulps."""
+    rng = np.random.default_rng(M + d + dff)
+    o = rng.standard_normal((M, d)).astype(np.float32)
+    h = (3.0 * rng.standard_normal((M, d)) + rng.standard_normal((M, 1))).astype(np.float32)
+    mk = lambda *s: (rng.standard_normal(s) / np.sqrt(s[-1])).astype(np.float32)
+    Wo, W1, W2 = mk(d, d), mk(dff, d), mk(d, dff)
+    vec = lambda n, c=0.0: (c + 0.1 * rng.standard_normal(n)).astype(np.float32)
+    bo, b1, b2, g2, b2ln, gn, bn = vec(d), vec(dff), vec(d), vec(d, 1.0), vec(d), vec(d, 1.0), vec(d)
+    o_hi = _bf16(o)
+    o_lo = _bf16(o - o_hi.float().cpu().numpy())
+    Wod, W1d, W2d = _bf16(Wo), _bf16(W1), _bf16(W2)
+    f64 = lambda t: t.float().cpu().numpy().astype(np.float64)
+    cu = lambda a: torch.from_numpy(a).cuda()
+    hd_ = cu(h.copy())
+    u_hi, u_lo = P.tc_post_bf16(o_hi, o_lo, hd_, Wod, cu(bo), cu(g2), cu(b2ln), W1d, cu(b1), W2d, cu(b2),
+                                cu(gn) if next_ln else None, cu(bn) if next_ln else None, 0 if act == "relu" else 1, 1e-5)
+    torch.cuda.synchronize()
+    # the block, step by step (PAPER.md L156; readings A5-A8)
+    h1 = h.astype(np.float64) + oracle.linear(f64(o_hi) + f64(o_lo), f64(Wod), bo)
+    u2 = oracle.layer_norm(h1, g2.astype(np.float64), b2ln.astype(np.float64), 1e-5)
+    g = oracle.activation(oracle.linear(u2, f64(W1d), b1), act)
+    h2 = h1 + oracle.linear(g, f64(W2d), b2)
+    un = oracle.layer_norm(h2, gn.astype(np.float64), bn.astype(np.float64), 1e-5) if next_ln else h2
+    got_h = hd_.cpu().numpy().astype(np.float64)
+    got_u = f64(u_hi) + f64(u_lo)
+    assert np.isfinite(got_h).all() and np.isfinite(got_u).all()
+    sc = np.sqrt((h2 ** 2).mean())
+    assert np.abs(got_h - h2).max() <= 3e-4 * sc, np.abs(got_h - h2).max() / sc      # u2, g rounded to bf16 hi + lo (2^-17)
+    su = np.sqrt((un ** 2).mean())
+    assert np.abs(got_u - un).max() <= 3e-4 * su, np.abs(got_u - un).max() / su
+    assert np.abs(f64(u_hi) - un).max() <= 6e-3 * max(su, np.abs(un).max())           # hi alone: one bf16 rounding

@@ -3,6 +3,7 @@
 Tolerances (BASELINE.json north_star; metric = DESIGN.md reading A14): max relative error <= 2e-2 on
 logits and regressions in BF16, <= 1e-4 on the fp32 debug path, argmax agreement >= 99.9 % over
 decidable rows, integer schedule arrays bit-exact."""
+import os
 import numpy as np
 import pytest
 
@@ -49,6 +50,18 @@ def oracle_events(W, m, X, off, events, quantized):
     return np.concatenate(rows), np.concatenate(lgs), np.concatenate(rgs)
 
 
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def oracle_cached(name, fp32=False):
+    """Oracle outputs of the large configs written by tests/golden/make_oracle_cache.py (which imports only oracle/
+    and synth/): rows = global row indices of the stored sample (documented event subset, every 4th row)."""
+    z = np.load(os.path.join(GOLDEN, f"oracle_{name}.npz"))
+    if fp32:
+        return z["fp32_rows"], z["fp32_logits"].astype(np.float64), z["fp32_regress"].astype(np.float64)
+    return z["rows"], z["logits"].astype(np.float64), z["regress"].astype(np.float64)
+
+
 def check(lg_gpu, rg_gpu, rows, lg_ref, rg_ref, X, tol, argmax=True):
     valid = X[rows, 0] != 0
     e_lg, _ = oracle.parity_metrics(lg_gpu[rows], lg_ref, valid)
@@ -82,20 +95,31 @@ def test_schedule_bit_exact(lens, pad, tile_q):
 
 
 # ------------------------------------------------------------------------------------------- fp32 debug path
-@pytest.mark.parametrize("name,events", [("cfg1", None), ("cfg2", [0, 5])])
+@pytest.mark.parametrize("name,events", [("cfg1", None), ("cfg2", [0, 5]), ("cfg3", [1, 6]), ("cfg5b", "cache")])
 def test_fp32_debug_path(name, events):
     m = synth.model_cfg(name)
     W = synth.make_weights(name)
     X, off = synth.make_named_events(name)
-    _, lg, rg = gpu_forward(W, m, X, off, precision=P.PREC_FP32_DEBUG)
-    ev = range(len(off) - 1) if events is None else events
-    rows, lr, rr = oracle_events(W, m, X, off, ev, quantized=False)
+    if events == "cache":                       # one 8192-row event of cfg5b (W-fp32 oracle output from tests/golden/)
+        rows, lr, rr = oracle_cached(name, fp32=True)
+        e = int(np.searchsorted(off, rows[0], side="right") - 1)
+        a, b = int(off[e]), int(off[e + 1])
+        _, lg1, rg1 = gpu_forward(W, m, X[a:b], np.array([0, b - a], np.int32), precision=P.PREC_FP32_DEBUG)
+        lg = np.zeros((X.shape[0], lg1.shape[1]), np.float32); rg = np.zeros((X.shape[0], rg1.shape[1]), np.float32)
+        lg[a:b], rg[a:b] = lg1, rg1
+    else:
+        _, lg, rg = gpu_forward(W, m, X, off, precision=P.PREC_FP32_DEBUG)
+        ev = range(len(off) - 1) if events is None else events
+        rows, lr, rr = oracle_events(W, m, X, off, ev, quantized=False)
     check(lg, rg, rows, lr, rr, X, TOL_FP32)
 
 
 # ------------------------------------------------------------------------------------------- bf16 path
 # "paper" = the paper's own block shape: d_model 256, 16 heads x 16, ReLU, 3 blocks
-BF16_CASES = [("cfg1", None), ("cfg2", None), ("cfg3", [0, 3]), ("cfg4", [2, 17]), ("cfg5b", [31]), ("paper", [1])]
+# cfg1-3: every event against the oracle run here; cfg4 / cfg5a / cfg5b: against tests/golden/oracle_<cfg>.npz (cfg5a whole;
+# cfg4 / cfg5b: first, last, longest, shortest + 25 % random events, every 4th row of each: make_oracle_cache.py)
+BF16_CASES = [("cfg1", None), ("cfg2", None), ("cfg3", None), ("cfg4", "cache"), ("cfg5a", "cache"), ("cfg5b", "cache"),
+              ("paper", [1])]
 
 
 @pytest.mark.parametrize("kernels", [P.KERNELS_TC, P.KERNELS_SIMPLE])
@@ -107,8 +131,11 @@ def test_bf16_parity(name, events, kernels):
     W = synth.make_weights(name)
     X, off = synth.make_named_events(name)
     mod, lg, rg = gpu_forward(W, m, X, off, kernels=kernels)
-    ev = range(len(off) - 1) if events is None else events
-    rows, lr, rr = oracle_events(W, m, X, off, ev, quantized=True)
+    if events == "cache":
+        rows, lr, rr = oracle_cached(name)
+    else:
+        ev = range(len(off) - 1) if events is None else events
+        rows, lr, rr = oracle_events(W, m, X, off, ev, quantized=True)
     e = check(lg, rg, rows, lr, rr, X, TOL_BF16)
     print(name, "max rel err (logits, regress) =", e, "launches", mod.query(P.Q_LAUNCHES))
 
@@ -132,7 +159,7 @@ def _rel(got, ref, valid):
 
 
 @pytest.mark.parametrize("precision,tol", [(P.PREC_FP32_DEBUG, 1e-4), (P.PREC_BF16, 2e-2)])
-@pytest.mark.parametrize("name,max_events", [("cfg1", None), ("cfg2", 3)])
+@pytest.mark.parametrize("name,max_events", [("cfg1", None), ("cfg2", 3), ("cfg3", 1)])
 def test_per_step_intermediates(name, max_events, precision, tol):
     m = synth.model_cfg(name)
     W = synth.make_weights(name)
