@@ -67,6 +67,7 @@ struct Workspace {
     std::vector<int> prof_cls;          // class of record i; events 2i, 2i+1
     // last call
     int64_t N = 0, E = 0, n_tiles = 0, n_pairs = 0, m_ub = 0, g_width = 0;
+    bool h_tiled = false;             // layout of h after the last call: tiled between fused blocks (tc_post.cu)
     int tile_q = 128;
 };
 
@@ -447,6 +448,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
 
     // ---- a0 (device half)
     w->prof_cls.clear();
+    w->h_tiled = false;
     {
     ProfScope ps(h, w, st, MLPF_KC_SCHED);
     CUDA_TRY(cudaMemsetAsync(w->n_valid, 0, (size_t)E * 4, st));
@@ -509,6 +511,8 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
             a.Wo = (const bf16*)PW(lw.Wo); a.W1 = (const bf16*)PW(lw.W1); a.W2 = (const bf16*)PW(lw.W2);
             a.bo = PV + lw.bo; a.ln2g = PV + lw.ln2g; a.ln2b = PV + lw.ln2b; a.b1 = PV + lw.b1; a.b2 = PV + lw.b2;
             a.eps = h->hp.ln_eps; a.h = w->h;
+            a.h_in_tiled = w->h_tiled ? 1 : 0; a.h_out_tiled = 1;      // tiled between fused blocks (tc_post.cu h_off)
+            w->h_tiled = true;
             if (!last) { a.lnng = PV + h->layers[l + 1].ln1g; a.lnnb = PV + h->layers[l + 1].ln1b; }
             else if (h->hp.final_ln) { a.lnng = PV + h->lnfg; a.lnnb = PV + h->lnfb; }
             else a.next_ln = 0;
@@ -737,6 +741,15 @@ extern "C" int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which
     switch (which) {
         case MLPF_TENSOR_H: {
             if (N * d > capacity) return set_err(MLPF_E_ARG, "capacity too small");
+            if (w->h_tiled) {                         // the fused blocks keep h in their tiled layout: un-tile for the tap
+                float* tmp = nullptr;
+                CUDA_TRY(cudaMalloc(&tmp, (size_t)N * d * 4));
+                launch_untile_h(w->h, tmp, N, (int)d, 0);
+                cudaError_t e = cudaMemcpy(host_out, tmp, (size_t)N * d * 4, cudaMemcpyDeviceToHost);
+                cudaFree(tmp);
+                if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tap copy failed: %s", cudaGetErrorString(e));
+                return N * d;
+            }
             CUDA_TRY(cudaMemcpy(host_out, w->h, (size_t)N * d * 4, cudaMemcpyDeviceToHost));
             return N * d;
         }

@@ -32,6 +32,7 @@ void launch_heads_l2(bool fp32, const void* hidden, const void* hidden_lo, int N
 // bits[i / 32] bit (i % 32) = valid[i] != 0; `bits` holds (N + 31) / 32 words (+ 3 zero words for the attention kernel)
 void launch_pack_valid_bits(const int* valid, int N, uint32_t* bits, cudaStream_t st);
 void launch_cast_rows(bool fp32, const float* h, int64_t n, void* u, void* u_lo, cudaStream_t st);
+void launch_untile_h(const float* h_tiled, float* out, int64_t N, int d, cudaStream_t st);
 void launch_to_f32(bool fp32, const void* src, float* dst, int64_t n, cudaStream_t st);
 
 }  // namespace mlpf

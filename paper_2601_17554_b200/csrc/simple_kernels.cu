@@ -645,6 +645,17 @@ __global__ void k_to_f32(const T* __restrict__ src, float* __restrict__ dst, int
     if (i < n) dst[i] = to_f32<T>(src[i]);
 }
 
+// debug tap: the fused blocks' tiled residual-stream layout (tc_post.cu h_off) -> row-major
+__global__ void k_untile_h(const float* __restrict__ ht, float* __restrict__ out, int64_t N, int d) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N * d) return;
+    const int64_t row = i / d; const int col = (int)(i % d);
+    out[i] = ht[(row / 128) * (128 * (int64_t)d) + (col >> 2) * 512 + (row % 128) * 4 + (col & 3)];
+}
+void launch_untile_h(const float* ht, float* out, int64_t N, int d, cudaStream_t st) {
+    k_untile_h<<<(unsigned)((N * d + 255) / 256), 256, 0, st>>>(ht, out, N, d);
+}
+
 // ------------------------------------------------------------------------------------------------ launchers
 int launch_schedule(const float* X, int N, int F, const int* offsets, int E, int* block_counts, int* block_base,
                     int* valid, uint32_t* valid_bits, int* row_event, int* row_pos, int* n_valid, int* type_offsets, int* sorted_row,

@@ -64,6 +64,7 @@ struct PostArgs {
     const float *bo = nullptr, *ln2g = nullptr, *ln2b = nullptr, *b1 = nullptr, *b2 = nullptr, *lnng = nullptr, *lnnb = nullptr;
     float eps = 1e-5f;
     float* h = nullptr;
+    int h_in_tiled = 0, h_out_tiled = 0;     // residual-stream layout in / out (tc_post.cu h_off); capacity: whole 128-row tiles
     bf16 *u_out = nullptr, *u_out_lo = nullptr;
     int next_ln = 1;
     bf16 *dbg_u2 = nullptr, *dbg_g = nullptr;

@@ -48,10 +48,26 @@ struct PostParams {
     const float *bo, *ln2g, *ln2b, *b1, *b2, *lnng, *lnnb;   // per group: D, D, D, dff, D, D, D floats
     float eps;
     float* h;                       // [M, D] fp32 residual stream, updated in place
+    int h_in_tiled, h_out_tiled;    // layout of h on the way in / out: 0 = row-major, 1 = tiled (see h_off)
     bf16* u_out; bf16* u_out_lo;    // [M, D] next LayerNorm output (lo may be null)
     int next_ln;                    // 0: u_out = T(h2) (final_ln = 0)
     bf16* dbg_u2; bf16* dbg_g;      // debug taps (null in production): u2 [M, D], g [M, dff] (hi terms)
 };
+
+// The epilogue thread owns one ROW of the tile, so 16-byte accesses to a row-major [M, D] matrix touch 32 different
+// 128-byte lines per warp instruction (one L1TEX wavefront each: measured 11 k cycles per 128 x 256 fp32 tile, with
+// the tensor pipe idle).  The residual stream is private to the library's kernels, so between fused blocks it lives in
+// a TILED layout in which those accesses are contiguous: element (row, col) of 128-row tile t = row / 128 is at
+//   t * 128 * D + (col / 4) * 512 + (row % 128) * 4 + col % 4        (floats)
+// i.e. for each group of 4 columns the 128 rows of the tile are adjacent: a warp's LDG.128 / STG.128 covers 512
+// contiguous bytes.  The block reads either layout and writes either layout (first block: row-major in, tiled out);
+// a tiled buffer holds whole 128-row tiles.
+// Both layouts as (base, stride): the float4 holding columns 4 k .. 4 k + 3 of row r of tile t is at base + k * stride.
+template <int D>
+__device__ __forceinline__ void h_addr(bool tiled, int tile, int r, int64_t& base, int& stride) {
+    base = tiled ? (int64_t)tile * (POST_BM * D) + r * 4 : ((int64_t)tile * POST_BM + r) * D;
+    stride = tiled ? POST_BM * 4 : 4;
+}
 
 template <int N> __device__ __forceinline__ void tmem_ld_n(uint32_t addr, uint32_t (&r)[N]);
 template <> __device__ __forceinline__ void tmem_ld_n<32>(uint32_t addr, uint32_t (&r)[32]) { ptx::tmem_ld32(addr, r); }
@@ -59,6 +75,11 @@ template <> __device__ __forceinline__ void tmem_ld_n<16>(uint32_t addr, uint32_
 template <int N> __device__ __forceinline__ void tmem_st_n(uint32_t addr, const uint32_t (&r)[N]) {
 #pragma unroll
     for (int i = 0; i < N / 16; ++i) ptx::tmem_st16(addr + 16 * i, *reinterpret_cast<const uint32_t(*)[16]>(&r[16 * i]));
+}
+
+__device__ __forceinline__ void st_global_v8(void* ptr, const uint32_t* v) {
+    asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(ptr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]),
+                 "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]) : "memory");
 }
 
 // (n, mean, M2) of a set merged with (nb, mb, m2b) of another (Chan et al.): exact pairwise update
@@ -282,19 +303,26 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
             // ---------------- epilogue of the output projection: h1 = h + acc + bo -> acc (TMEM); u2 = LN2(h1) -> A operand
             ptx::mbar_wait(bar_acc_full, it & 1);
             ptx::tc_fence_after();
-            float* const hrow = p.h + (int64_t)row * D;
             float sn = 0.f, smean = 0.f, sm2 = 0.f;
+            // rows past M (last tile) read the last valid row instead (their results are never stored): the loads need
+            // no predicate or branch, so all of a piece's loads are in flight together
+            const int r_ld = min(r, p.M - 1 - m0);
+            int64_t hin_base, hout_base; int hin_stride, hout_stride;
+            h_addr<D>(p.h_in_tiled != 0, tile, r_ld, hin_base, hin_stride);
+            h_addr<D>(p.h_out_tiled != 0, tile, r, hout_base, hout_stride);
 #pragma unroll
             for (int c0 = cg * CW; c0 < (cg + 1) * CW; c0 += PIECE) {
                 uint32_t a[PIECE];
                 tmem_ld_n<PIECE>(lane_addr + c0, a);
+                float4 hv[PIECE / 4];
+#pragma unroll
+                for (int i = 0; i < PIECE / 4; ++i)
+                    hv[i] = *reinterpret_cast<const float4*>(p.h + hin_base + (int64_t)(c0 / 4 + i) * hin_stride);
                 float v[PIECE];
 #pragma unroll
                 for (int i = 0; i < PIECE / 4; ++i) {
-                    float4 hv = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (row_ok) hv = *reinterpret_cast<const float4*>(hrow + c0 + 4 * i);
                     const float4 bb = *reinterpret_cast<const float4*>(v_bo + c0 + 4 * i);
-                    v[4 * i] = hv.x + bb.x; v[4 * i + 1] = hv.y + bb.y; v[4 * i + 2] = hv.z + bb.z; v[4 * i + 3] = hv.w + bb.w;
+                    v[4 * i] = hv[i].x + bb.x; v[4 * i + 1] = hv[i].y + bb.y; v[4 * i + 2] = hv[i].z + bb.z; v[4 * i + 3] = hv[i].w + bb.w;
                 }
                 ptx::tmem_ld_wait();
 #pragma unroll
@@ -383,7 +411,11 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
                     const float4 bb = *reinterpret_cast<const float4*>(v_b2 + c0 + 4 * i);
                     v[4 * i] = __uint_as_float(a[4 * i]) + bb.x; v[4 * i + 1] = __uint_as_float(a[4 * i + 1]) + bb.y;
                     v[4 * i + 2] = __uint_as_float(a[4 * i + 2]) + bb.z; v[4 * i + 3] = __uint_as_float(a[4 * i + 3]) + bb.w;
-                    if (row_ok) *reinterpret_cast<float4*>(hrow + c0 + 4 * i) = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+                }
+                if (row_ok) {
+#pragma unroll
+                    for (int i = 0; i < PIECE / 4; ++i)
+                        *reinterpret_cast<float4*>(p.h + hout_base + (int64_t)(c0 / 4 + i) * hout_stride) = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
                 }
                 stats_piece<PIECE>(v, sn, smean, sm2);
             }
@@ -394,22 +426,21 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
                 uint32_t a[PIECE];
                 tmem_ld_n<PIECE>(lane_addr + c0, a);
                 ptx::tmem_ld_wait();
+                uint32_t hi[PIECE / 2], lo[PIECE / 2];
 #pragma unroll
-                for (int j = 0; j < PIECE / 8; ++j) {
-                    uint32_t hi[4], lo[4];
+                for (int i = 0; i < PIECE / 2; ++i) {
+                    const int col = c0 + 2 * i;
+                    const float2 b2v = *reinterpret_cast<const float2*>(v_b2 + col);
+                    const float2 gg = *reinterpret_cast<const float2*>(v_gn + col), bb = *reinterpret_cast<const float2*>(v_bn + col);
+                    const float2 y = make_float2((__uint_as_float(a[2 * i]) + b2v.x - mu) * rstd * gg.x + bb.x,
+                                                 (__uint_as_float(a[2 * i + 1]) + b2v.y - mu) * rstd * gg.y + bb.y);
+                    split_bf16x2(y, hi[i], lo[i]);
+                }
+                if (row_ok) {                             // 32-byte stores: a full sector per lane
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const int col = c0 + 8 * j + 2 * i;
-                        const float2 b2v = *reinterpret_cast<const float2*>(v_b2 + col);
-                        const float2 gg = *reinterpret_cast<const float2*>(v_gn + col), bb = *reinterpret_cast<const float2*>(v_bn + col);
-                        const float2 y = make_float2((__uint_as_float(a[8 * j + 2 * i]) + b2v.x - mu) * rstd * gg.x + bb.x,
-                                                     (__uint_as_float(a[8 * j + 2 * i + 1]) + b2v.y - mu) * rstd * gg.y + bb.y);
-                        split_bf16x2(y, hi[i], lo[i]);
-                    }
-                    if (row_ok) {
-                        *reinterpret_cast<uint4*>(p.u_out + (int64_t)row * D + c0 + 8 * j) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-                        if (p.u_out_lo)
-                            *reinterpret_cast<uint4*>(p.u_out_lo + (int64_t)row * D + c0 + 8 * j) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+                    for (int j = 0; j < PIECE / 16; ++j) {
+                        st_global_v8(p.u_out + (int64_t)row * D + c0 + 16 * j, &hi[8 * j]);
+                        if (p.u_out_lo) st_global_v8(p.u_out_lo + (int64_t)row * D + c0 + 16 * j, &lo[8 * j]);
                     }
                 }
             }
@@ -447,7 +478,7 @@ static int tc_post_launch_t(TcContext* c, const PostArgs& a, cudaStream_t st) {
     PostParams p;
     p.M = a.M; p.dff = a.dff; p.group_rows = a.group_rows > 0 ? a.group_rows : 0x7fffff80;
     p.bo = a.bo; p.ln2g = a.ln2g; p.ln2b = a.ln2b; p.b1 = a.b1; p.b2 = a.b2; p.lnng = a.lnng; p.lnnb = a.lnnb;
-    p.eps = a.eps; p.h = a.h; p.u_out = a.u_out; p.u_out_lo = a.u_out_lo; p.next_ln = a.next_ln;
+    p.eps = a.eps; p.h = a.h; p.h_in_tiled = a.h_in_tiled; p.h_out_tiled = a.h_out_tiled; p.u_out = a.u_out; p.u_out_lo = a.u_out_lo; p.next_ln = a.next_ln;
     p.dbg_u2 = a.dbg_u2; p.dbg_g = a.dbg_g;
     const int n_tiles = (a.M + POST_BM - 1) / POST_BM;
     const int grid = n_tiles < c->num_sms ? n_tiles : c->num_sms;
