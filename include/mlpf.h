@@ -145,6 +145,9 @@ int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* 
 #define MLPF_OPT_FUSE        7   /* 1 (default): where the shape allows (d_model <= 256, d_ff % 128 == 0, all activations split)
                                     the post-attention half of every block runs as ONE kernel (out-projection + residual +
                                     LN2 + FFN1 + activation + FFN2 + residual + next LayerNorm); 0: one kernel per step   */
+#define MLPF_OPT_ATTN        8   /* attention kernel: 1 (default) = tc_attn2.cu (no running maximum: Cauchy-Schwarz bound from a norms
+                                    pre-pass, exact two-sweep path when the bound is too loose; two threads per query row);
+                                    2 = the same with the exact path forced for every CTA; 0 = round 1's lazy-rescale kernel */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0
@@ -218,6 +221,9 @@ int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* A_lo, const uint16_t* W
 int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_valid,
                            const int32_t* event_offsets, int32_t n_events, int32_t d_model, int32_t n_heads,
                            uint16_t* O, void* stream);
+
+/* which kernel mlpf_tc_attention_bf16 runs (process-wide; values as MLPF_OPT_ATTN) */
+int mlpf_debug_set_attention_impl(int impl);
 
 /* The post-attention half of one encoder block (steps a5 + a6 + a7 with both LayerNorms in epilogues)
  * as ONE kernel:  h <- h + (o_hi + o_lo) Wo^T + bo;  u2 = LN2(h);  h <- h + act(u2 W1^T + b1) W2^T + b2;

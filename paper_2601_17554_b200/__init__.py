@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmlpf.so")
 
 # include/mlpf.h constants
 OK = 0
-OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE, OPT_FUSE = 1, 2, 3, 4, 5, 6, 7
+OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE, OPT_FUSE, OPT_ATTN = 1, 2, 3, 4, 5, 6, 7, 8
 PREC_BF16, PREC_FP32_DEBUG = 0, 1
 KERNELS_TC, KERNELS_SIMPLE = 0, 1
 Q_N_LAYERS, Q_D_MODEL, Q_N_HEADS, Q_D_FF, Q_N_FEAT, Q_N_CLASSES, Q_N_REGRESS = 1, 2, 3, 4, 5, 6, 7
@@ -28,7 +28,7 @@ KERNEL_CLASSES = ["sched", "embed_l1", "embed_l2", "layernorm", "qkv", "attentio
 
 EXPORTS = ["mlpf_create", "mlpf_infer", "mlpf_infer_host", "mlpf_destroy", "mlpf_last_error", "mlpf_set_option",
            "mlpf_query", "mlpf_debug_get_schedule", "mlpf_debug_get_tensor", "mlpf_debug_get_profile", "mlpf_tc_gemm_bf16",
-           "mlpf_tc_attention_bf16", "mlpf_tc_post_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates"]
+           "mlpf_tc_attention_bf16", "mlpf_debug_set_attention_impl", "mlpf_tc_post_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates"]
 
 _lib = None
 
@@ -67,6 +67,8 @@ def lib():
     L.mlpf_tc_gemm_bf16.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp]
     L.mlpf_tc_attention_bf16.restype = C.c_int
     L.mlpf_tc_attention_bf16.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
+    L.mlpf_debug_set_attention_impl.restype = C.c_int
+    L.mlpf_debug_set_attention_impl.argtypes = [C.c_int]
     L.mlpf_tc_post_bf16.restype = C.c_int
     L.mlpf_tc_post_bf16.argtypes = [vp] * 13 + [i32, i32, i32, i32, C.c_float, vp, vp, vp]
     L.mlpf_candidates_scratch_bytes.restype = i64
@@ -187,9 +189,11 @@ def tc_gemm_bf16(A, W, A_lo=None, stream=None):
     return out
 
 
-def tc_attention_bf16(QKV, key_valid, event_offsets, d_model, n_heads, stream=None):
-    """QKV [N,3d] bf16 (q | k | v), key_valid [N] int32 or None -> O [N,d] bf16 (Eq. 4 per event/head)."""
+def tc_attention_bf16(QKV, key_valid, event_offsets, d_model, n_heads, stream=None, impl=1):
+    """QKV [N,3d] bf16 (q | k | v), key_valid [N] int32 or None -> O [N,d] bf16 (Eq. 4 per event/head).
+    impl: 1 = bound-based kernel (default), 2 = its exact path forced, 0 = round 1's lazy-rescale kernel."""
     import torch
+    _check(lib().mlpf_debug_set_attention_impl(int(impl)))
     off = np.ascontiguousarray(event_offsets, dtype=np.int32)
     assert QKV.is_contiguous() and QKV.shape[1] == 3 * d_model
     N = QKV.shape[0]

@@ -59,6 +59,7 @@ struct Workspace {
     int *valid = nullptr, *row_event = nullptr, *row_pos = nullptr, *n_valid = nullptr;
     int *block_counts = nullptr, *block_base = nullptr, *type_offsets = nullptr;
     int *sorted_row = nullptr, *type_perm = nullptr;
+    float *qn = nullptr, *kmax = nullptr;   // attention norms pre-pass: |q_i| per row and head, max |k_j| per event and head
     // device staging of mlpf_infer_host (owned by the stream's workspace, freed with it); capacities in BYTES
     float *stage_x = nullptr, *stage_lg = nullptr, *stage_rg = nullptr;
     int64_t stage_cap = 0;            // rows
@@ -82,7 +83,7 @@ struct mlpf_handle {
     std::vector<LayerW> layers;
     HeadsOut ho;
     // options
-    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1;
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1;
     int64_t last_launches = 0;
     std::mutex mu;
     std::map<void*, Workspace*> ws;
@@ -234,6 +235,9 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_PROFILE:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "profile must be 0 or 1");
             h->profile = (int)value; return MLPF_OK;
+        case MLPF_OPT_ATTN:
+            if (value < 0 || value > 2) return set_err(MLPF_E_ARG, "attn must be 0, 1 or 2");
+            h->attn = (int)value; return MLPF_OK;
         case MLPF_OPT_FUSE:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "fuse must be 0 or 1");
             h->fuse = (int)value; return MLPF_OK;
@@ -280,13 +284,14 @@ template <typename P> static void dfree(P*& p) { if (p) cudaFree(p); p = nullptr
 static void ws_free_rows(Workspace* w) {
     dfree(w->h); dfree(w->u); dfree(w->qkv); dfree(w->o); dfree(w->g); dfree(w->u_lo); dfree(w->o_lo); dfree(w->g_lo);
     dfree(w->valid); dfree(w->valid_bits); dfree(w->row_event); dfree(w->row_pos); dfree(w->block_counts); dfree(w->block_base);
-    dfree(w->sorted_row); dfree(w->type_perm); dfree(w->type_offsets);
+    dfree(w->sorted_row); dfree(w->type_perm); dfree(w->type_offsets); dfree(w->qn);
     w->cap_rows = 0;
 }
 
 static int64_t ws_bytes_events(const Workspace* w) {
     int64_t b = 0;
     if (w->offsets) b += std::max<int64_t>((w->cap_events + 1) * 4, 256) + std::max<int64_t>(w->cap_events * 4, 256);
+    if (w->kmax) b += std::max<int64_t>(w->cap_events * 64 * 4, 256);      // upper bound (H <= 64)
     if (w->work) b += 2 * std::max<int64_t>(w->cap_tiles * 8, 256);
     return b;
 }
@@ -311,7 +316,7 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
             dmalloc(&w->valid, cap * 4, w) || dmalloc(&w->valid_bits, (cap / 32 + 40) * 4, w) || dmalloc(&w->row_event, cap * 4, w) || dmalloc(&w->row_pos, cap * 4, w) ||
             dmalloc(&w->block_counts, nb * 5 * 4, w) || dmalloc(&w->block_base, nb * 5 * 4, w) ||
             dmalloc(&w->sorted_row, cap * 4, w) || dmalloc(&w->type_perm, m_ub * 4, w) ||
-            dmalloc(&w->type_offsets, 8 * 4, w)) {
+            dmalloc(&w->type_offsets, 8 * 4, w) || dmalloc(&w->qn, cap * h->H * 4, w)) {
             const char* why = cudaGetErrorString(cudaGetLastError());
             ws_free_rows(w);                       // release the partial set; nothing dangling is left behind
             w->bytes = ws_bytes_events(w);
@@ -329,11 +334,11 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
         w->cap_rows = cap;
     }
     if (E > w->cap_events) {
-        dfree(w->offsets); dfree(w->n_valid);
+        dfree(w->offsets); dfree(w->n_valid); dfree(w->kmax);
         w->cap_events = 0;
         const int64_t ce = std::max<int64_t>(E, 64);
-        if (dmalloc(&w->offsets, (ce + 1) * 4, w) || dmalloc(&w->n_valid, ce * 4, w)) {
-            dfree(w->offsets); dfree(w->n_valid);
+        if (dmalloc(&w->offsets, (ce + 1) * 4, w) || dmalloc(&w->n_valid, ce * 4, w) || dmalloc(&w->kmax, ce * h->H * 4, w)) {
+            dfree(w->offsets); dfree(w->n_valid); dfree(w->kmax);
             return set_err(MLPF_E_ALLOC, "workspace allocation for %lld events failed", (long long)ce);
         }
         w->cap_events = ce;
@@ -355,7 +360,7 @@ static void ws_free(Workspace* w) {
     ws_free_rows(w);
     dfree(w->stage_x); dfree(w->stage_lg); dfree(w->stage_rg);
     w->stage_cap = 0;
-    dfree(w->offsets); dfree(w->n_valid); dfree(w->work); dfree(w->pairs);
+    dfree(w->offsets); dfree(w->n_valid); dfree(w->work); dfree(w->pairs); dfree(w->kmax);
     for (cudaEvent_t e : w->ev_pool) cudaEventDestroy(e);
     w->ev_pool.clear();
 }
@@ -405,9 +410,17 @@ static int run_layernorm(mlpf_handle* h, bool fp32, const float* x, int N, const
 static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspace* w, cudaStream_t st) {
     if (w->n_tiles == 0) return MLPF_OK;
     if (tc && !fp32) {
-        int rc = tc_attn_launch(&h->tc, (const bf16*)w->qkv, w->N, w->valid_bits, w->n_valid, w->offsets,
+        int rc;
+        if (h->attn == 0)
+            rc = tc_attn_launch(&h->tc, (const bf16*)w->qkv, w->N, w->valid_bits, w->n_valid, w->offsets,
                                 (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, (bf16*)w->o,
                                 split ? (bf16*)w->o_lo : nullptr, st);
+        else {
+            rc = tc_attn2_launch(&h->tc, (const bf16*)w->qkv, w->N, (int)w->E, w->valid_bits, w->n_valid, w->offsets, w->row_event,
+                                 (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, w->qn, w->kmax, (bf16*)w->o,
+                                 split ? (bf16*)w->o_lo : nullptr, h->attn == 2, st);
+            h->last_launches++;                       // the norms pre-pass
+        }
         if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", h->tc.err);
     } else {
         launch_attn_simple(fp32, h->hd, w->qkv, w->valid, w->offsets, (const int2*)w->work, (int)w->n_tiles,
@@ -826,6 +839,13 @@ extern "C" int mlpf_tc_post_bf16(const uint16_t* o_hi, const uint16_t* o_lo, flo
     return MLPF_OK;
 }
 
+static int g_attn_impl = 1;    // kernel-level attention entry: 0 = round-1 kernel, 1 = bound-based kernel, 2 = its exact path forced
+extern "C" int mlpf_debug_set_attention_impl(int impl) {
+    if (impl < 0 || impl > 2) return set_err(MLPF_E_ARG, "impl must be 0, 1 or 2");
+    g_attn_impl = impl;
+    return MLPF_OK;
+}
+
 extern "C" int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_valid,
                                       const int32_t* event_offsets, int32_t n_events, int32_t d_model, int32_t n_heads,
                                       uint16_t* O, void* stream) {
@@ -854,10 +874,24 @@ extern "C" int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_va
     CUDA_TRY(cudaMalloc(&d_pairs, pairs.size() * 4));
     CUDA_TRY(cudaMemcpyAsync(d_off, event_offsets, (size_t)(n_events + 1) * 4, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(d_pairs, pairs.data(), pairs.size() * 4, cudaMemcpyHostToDevice, st));
-    int rc = tc_attn_launch(&ctx, (const bf16*)QKV, N, d_bits, nullptr, d_off, (const int2*)d_pairs,
+    int rc;
+    int* d_rowev = nullptr; float *d_qn = nullptr, *d_kmax = nullptr;
+    if (g_attn_impl == 0) {
+        rc = tc_attn_launch(&ctx, (const bf16*)QKV, N, d_bits, nullptr, d_off, (const int2*)d_pairs,
                             (int)(pairs.size() / 2), d_model, n_heads, (bf16*)O, (bf16*)nullptr, st);
+    } else {
+        std::vector<int> rowev((size_t)N);
+        for (int e = 0; e < n_events; ++e) for (int i = event_offsets[e]; i < event_offsets[e + 1]; ++i) rowev[i] = e;
+        CUDA_TRY(cudaMalloc(&d_rowev, (size_t)N * 4));
+        CUDA_TRY(cudaMalloc(&d_qn, (size_t)N * n_heads * 4));
+        CUDA_TRY(cudaMalloc(&d_kmax, (size_t)n_events * n_heads * 4));
+        CUDA_TRY(cudaMemcpyAsync(d_rowev, rowev.data(), (size_t)N * 4, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaStreamSynchronize(st));      // rowev is a local
+        rc = tc_attn2_launch(&ctx, (const bf16*)QKV, N, n_events, d_bits, nullptr, d_off, d_rowev, (const int2*)d_pairs,
+                             (int)(pairs.size() / 2), d_model, n_heads, d_qn, d_kmax, (bf16*)O, (bf16*)nullptr, g_attn_impl == 2, st);
+    }
     cudaError_t e = cudaStreamSynchronize(st);
-    cudaFree(d_off); cudaFree(d_pairs); cudaFree(d_bits);
+    cudaFree(d_off); cudaFree(d_pairs); cudaFree(d_bits); cudaFree(d_rowev); cudaFree(d_qn); cudaFree(d_kmax);
     if (rc) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", ctx.err);
     if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tcgen05 attention failed: %s", cudaGetErrorString(e));
     return MLPF_OK;

@@ -54,6 +54,14 @@ int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const uint32_t* val
                    const int* offsets, const int2* items, int n_items, int d, int H, bf16* O, bf16* O_lo,
                    cudaStream_t st);
 
+// Second attention design (tc_attn2.cu): no running maximum (Cauchy-Schwarz bound from a norms pre-pass; exact two-sweep
+// path for CTAs whose bound is too loose), two threads per query row.  qn [N, H], kmax [E, H]: caller-owned fp32 scratch;
+// row_event [N] from the schedule.  force_exact != 0: every CTA takes the exact path (tests).
+int tc_attn2_rows_per_cta(int hd);
+int tc_attn2_launch(TcContext* c, const bf16* QKV, int64_t N, int E, const uint32_t* valid_bits, const int* n_valid,
+                    const int* offsets, const int* row_event, const int2* items, int n_items, int d, int H, float* qn,
+                    float* kmax, bf16* O, bf16* O_lo, int force_exact, cudaStream_t st);
+
 // The post-attention half of an encoder block as one kernel (tc_post.cu): h <- h + o Wo^T + bo; u2 = LN2(h);
 // h <- h + act(u2 W1^T + b1) W2^T + b2; u_out = LN_next(h) (or T(h) when next_ln == 0).  d in {64, 128, 256}, dff % 128 == 0.
 // n_groups > 1 (two parallel encoders): rows [g * group_rows, (g + 1) * group_rows) use weight block g of Wo [G*d, d],

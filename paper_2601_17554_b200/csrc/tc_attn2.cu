@@ -1,0 +1,438 @@
+// tc_attn2.cu -- varlen, key-padding-masked flash-attention forward on tcgen05 / TMEM / TMA (sm_100a), second design.
+// Step a4 of DESIGN.md:  per event, per head  O = softmax(Q K^T / sqrt(hd) + mask) V   (Eq. 4), without
+// the n x n matrix ever leaving the SM (L154).  Keys outside the event or of pad rows get weight exactly 0 (reading A2);
+// a query with no valid key gets O = 0 (A15).
+//
+// What differs from tc_attn.cu (round 1): the softmax needs NO running maximum.
+//   Eq. 4 is invariant under subtracting any per-row constant from the scores.  Round 1 tracked the row maximum tile by
+//   tile (one FMNMX per score, a warp vote per tile, an in-place rescale of O when it moved).  Here the constant is the
+//   Cauchy-Schwarz bound  B_i = |q_i| max_j |k_j| / sqrt(hd)  >= max_j s_ij  taken from the row norms (a0-style
+//   pre-pass k_attn_norms: |q_i| per row and head, max |k_j| per event and head).  P = 2^((s - B) c) <= 1 can never
+//   overflow, bf16 P keeps its relative precision at any magnitude (8 exponent bits), and the row sums and O accumulate in
+//   fp32, so the result does not depend on how loose the bound is -- as long as nothing underflows.  The largest term of
+//   a row is at least 2^(-2 B c): with 2 B c <= 96 there are more than 24 bits of headroom above the flush-to-zero
+//   threshold 2^-126 and the FAST path is exact to fp32 rounding.  A CTA whose rows have a larger bound (huge query/key
+//   norms: never seen with LayerNorm-ed inputs, but inputs are not ours to choose) takes the EXACT path instead: one extra
+//   sweep over the keys computes the true row maxima (scores only, no P, no P V), then the same loop runs with them.
+// With no cross-score dependency left, a query row is split over TWO threads (two warps per TMEM lane quarter, 32 of a
+// tile's 64 scores each): twice the warps for the same registers, which is what hides the TMEM-load / MUFU latency that
+// bound round 1's kernel (0.32 of the bf16 peak with neither the MUFU nor the issue slots saturated).
+//
+// One CTA = one head x NT consecutive 128-row query tiles of one event (NT = 3 at hd <= 32, 2 at hd = 64) sharing every
+// K / V tile.  Key tiles are 64 keys wide, S is double-buffered in TMEM:
+//   warps 0 .. 8NT-1   softmax: warp w serves query tile t = w / 8, lane quarter q = w % 4, score half hf = (w / 4) % 2:
+//               S[32 of 64 columns] -> P = 2^(s c - B c) as bf16 written back over the first 16 of ITS OWN 32 columns.
+//   warp 8NT    TMA producer: Q tiles once; then stages of (K, V), [128 keys x hd] each, row-major boxes of the one
+//               [N, 3d] QKV buffer (an event may start at any row).
+//   warps 8NT+1 .. 8NT+NT   MMA issuers, one per query tile: S_t(j) = Q_t K_j^T (M 128, N 64, K hd);
+//               O_t += P_t(j) V_j (A = P from TMEM, B = V_j MN-major) and l_t += P_t(j) 1 (row sums on the tensor pipe).
+// TMEM columns: S_t[b] at 128 t + 64 b; O_t | l_t at 128 NT + (hd + 8) t.
+#include "tc_api.h"
+#include "ptx.cuh"
+#include <type_traits>
+
+namespace mlpf {
+
+constexpr int A2_BQ = 128, A2_BK = 64, A2_SK = 128;     // query tile, key tile, keys per TMA stage
+constexpr float A2_FAST_MAX_BOUND = 48.0f;              // fast path iff B c <= 48 (log2 units) for every row of the CTA
+
+template <int HD>
+struct Attn2Cfg {
+    static constexpr int NT = HD <= 32 ? 3 : 2;
+    static constexpr int SM_WARPS = 8 * NT;
+    static constexpr int THREADS = SM_WARPS * 32 + 128;
+    static constexpr int WARP_TMA = SM_WARPS, WARP_MMA = SM_WARPS + 1;
+    static constexpr int Q_BYTES = A2_BQ * HD * 2;
+    static constexpr int K_BYTES = A2_SK * HD * 2;
+    static constexpr int STAGE_BYTES = 2 * K_BYTES;
+    static constexpr int STAGES = HD == 64 ? 4 : 6;
+    static constexpr int ONES_BYTES = 1024;
+    static constexpr int OW = HD + 8;
+    static constexpr int XCHG_BYTES = NT * A2_BQ * 2 * 4;   // exact path: the two score halves' row maxima
+    static constexpr int SMEM_BYTES = NT * Q_BYTES + STAGES * STAGE_BYTES + ONES_BYTES + XCHG_BYTES + 1024;
+    static constexpr int SW = HD * 2;
+    static constexpr int O_COL0 = 128 * NT;
+    static_assert(O_COL0 + NT * OW <= 512, "TMEM budget");
+};
+
+int tc_attn2_rows_per_cta(int hd) { return (hd <= 32 ? 3 : 2) * A2_BQ; }
+
+struct Attn2Params {
+    const uint32_t* valid_bits; const int* n_valid; const int* offsets; const int2* items;
+    const float* qn;           // [N, H] |q_i| per head
+    const float* kmax;         // [E, H] max_j |k_j| over the event's rows, per head
+    int n_items, H, d;
+    bf16* O; bf16* O_lo;
+    float scale_log2;          // c = log2(e) / sqrt(hd)
+    int force_exact;           // debugging / tests: every CTA takes the exact path
+};
+
+// ---------------------------------------------------------------------------------------------- norms pre-pass
+// qn[i, h] = |q_i| (head h), kmax[e, h] = max over the rows of event e of |k_j| (float bits, atomicMax on ints: norms
+// are non-negative).  One thread per (row, head); a block's threads that belong to the block's first event reduce in
+// shared memory first.  kmax must be zeroed before the launch.
+__global__ void __launch_bounds__(256)
+k_attn_norms(const bf16* __restrict__ QKV, const int* __restrict__ row_event, int N, int H, int hd, int d,
+             float* __restrict__ qn, float* __restrict__ kmax) {
+    __shared__ int smax[64];
+    __shared__ int ev_first;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    const int row = idx / H, h = idx % H;
+    if (threadIdx.x < 64) smax[threadIdx.x] = 0;
+    if (threadIdx.x == 0) ev_first = row_event[min(row, N - 1)];
+    __syncthreads();
+    if (row < N) {
+        const uint4* qp = reinterpret_cast<const uint4*>(QKV + (int64_t)row * 3 * d + h * hd);
+        const uint4* kp = reinterpret_cast<const uint4*>(QKV + (int64_t)row * 3 * d + d + h * hd);
+        float sq = 0.f, sk = 0.f;
+        for (int i = 0; i < hd / 8; ++i) {
+            const uint4 a = __ldg(qp + i), b = __ldg(kp + i);
+            const uint32_t aw[4] = {a.x, a.y, a.z, a.w}, bw[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const float a0 = __uint_as_float(aw[k] << 16), a1 = __uint_as_float(aw[k] & 0xffff0000u);
+                const float b0 = __uint_as_float(bw[k] << 16), b1 = __uint_as_float(bw[k] & 0xffff0000u);
+                sq = fmaf(a0, a0, fmaf(a1, a1, sq));
+                sk = fmaf(b0, b0, fmaf(b1, b1, sk));
+            }
+        }
+        qn[(int64_t)row * H + h] = sqrtf(sq);
+        const int kb = __float_as_int(sqrtf(sk));
+        const int ev = row_event[row];
+        if (ev == ev_first && h < 64) atomicMax(&smax[h], kb);
+        else atomicMax(reinterpret_cast<int*>(kmax) + (int64_t)ev * H + h, kb);
+    }
+    __syncthreads();
+    if ((int)threadIdx.x < H && threadIdx.x < 64 && smax[threadIdx.x] > 0)
+        atomicMax(reinterpret_cast<int*>(kmax) + (int64_t)ev_first * H + threadIdx.x, smax[threadIdx.x]);
+}
+
+// 2^x for a pair, x <= 0, on the FMA / ALU pipes instead of the MUFU (Cody-Waite split + degree-3 polynomial, max
+// relative error 1.0e-4, 40x below the bf16 rounding of P); see tc_attn.cu.
+__device__ __forceinline__ float2 a2_exp2_poly2(float2 x) {
+    const float2 magic = make_float2(12582912.0f, 12582912.0f);
+    x.x = fmaxf(x.x, -126.0f); x.y = fmaxf(x.y, -126.0f);
+    const float2 xr = ptx::fadd2(x, magic);
+    const float2 f = ptx::fadd2(x, ptx::fadd2(magic, make_float2(-xr.x, -xr.y)));
+    float2 p = ptx::ffma2(f, make_float2(0.0550089306f, 0.0550089306f), make_float2(0.2422109596f, 0.2422109596f));
+    p = ptx::ffma2(p, f, make_float2(0.6932829272f, 0.6932829272f));
+    p = ptx::ffma2(p, f, make_float2(1.0f, 1.0f));
+    return make_float2(__int_as_float(__float_as_int(p.x) + (__float_as_int(xr.x) << 23)),
+                       __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
+}
+#ifndef A2_POLY_EVERY
+#define A2_POLY_EVERY 4      // every A2_POLY_EVERY-th pair of exponentials runs on the FMA pipe (0: all on the MUFU)
+#endif
+
+// 32 scores of one row -> 16 packed bf16 pairs  p = 2^(s c - B c).  MASKED: scores of masked keys become -inf first, so the
+// MUFU gives the exact weight 0 (the polynomial path clamps its argument and is not used on masked tiles).
+template <bool MASKED>
+__device__ __forceinline__ void a2_exp32(uint32_t (&s)[32], uint32_t mask, float c, float neg_bc, uint32_t (&pk)[16]) {
+    const float2 c2 = make_float2(c, c), m2 = make_float2(neg_bc, neg_bc);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        if (MASKED) {
+            s[2 * i] = (mask >> (2 * i)) & 1u ? s[2 * i] : 0xff800000u;
+            s[2 * i + 1] = (mask >> (2 * i + 1)) & 1u ? s[2 * i + 1] : 0xff800000u;
+        }
+        const float2 x = ptx::ffma2(make_float2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), c2, m2);
+        float2 p;
+        if (!MASKED && A2_POLY_EVERY > 0 && (i % (A2_POLY_EVERY > 0 ? A2_POLY_EVERY : 1)) == 0) p = a2_exp2_poly2(x);
+        else p = make_float2(ptx::fast_exp2(x.x), ptx::fast_exp2(x.y));
+        __nv_bfloat162 b2 = __floats2bfloat162_rn(p.x, p.y);
+        pk[i] = *reinterpret_cast<uint32_t*>(&b2);
+    }
+}
+
+template <int HD>
+__global__ void __launch_bounds__(Attn2Cfg<HD>::THREADS, 1)
+k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
+    using Cfg = Attn2Cfg<HD>;
+    constexpr int ST = Cfg::STAGES, NT = Cfg::NT;
+    extern __shared__ uint8_t smem_raw[];
+    __shared__ uint64_t bars[1 + 2 * ST + 5 * NT];
+    __shared__ uint32_t tmem_base_slot;
+    __shared__ int bound_bits;                                   // max over the CTA's rows of B c (float bits)
+
+    const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
+    const int item = blockIdx.x / prm.H, head = blockIdx.x % prm.H;
+    const int2 it = prm.items[item];
+    const int ev0 = prm.offsets[it.x], ev1 = prm.offsets[it.x + 1];
+    const int q0 = ev0 + it.y * NT * A2_BQ;
+    const int nt = min(NT, (ev1 - q0 + A2_BQ - 1) / A2_BQ);
+    const int nkv = (ev1 - ev0 + A2_BK - 1) / A2_BK;
+    const int nst = (ev1 - ev0 + A2_SK - 1) / A2_SK;
+    const uint32_t* valid_bits = (prm.valid_bits && !(prm.n_valid && prm.n_valid[it.x] == ev1 - ev0)) ? prm.valid_bits : nullptr;
+
+    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t sQ = smem_base;
+    const uint32_t sKV = smem_base + NT * Cfg::Q_BYTES;
+    const uint32_t sOnes = sKV + ST * Cfg::STAGE_BYTES;
+    float* const xchg = reinterpret_cast<float*>(smem_raw + (smem_base - ptx::smem_u32(smem_raw)) + NT * Cfg::Q_BYTES +
+                                                 ST * Cfg::STAGE_BYTES + Cfg::ONES_BYTES);
+    const uint32_t bar_q = ptx::smem_u32(&bars[0]);
+    const uint32_t bar_kv_full = ptx::smem_u32(&bars[1]);
+    const uint32_t bar_kv_empty = ptx::smem_u32(&bars[1 + ST]);
+    const uint32_t bar_s = ptx::smem_u32(&bars[1 + 2 * ST]);             // [2t + b]: S_t landed in buffer b
+    const uint32_t bar_p = ptx::smem_u32(&bars[1 + 2 * ST + 2 * NT]);    // [2t + b]: P_t written over buffer b (or S consumed)
+    const uint32_t bar_o = ptx::smem_u32(&bars[1 + 2 * ST + 4 * NT]);    // [t]: all of O_t accumulated
+
+    if (threadIdx.x == 0) bound_bits = 0;
+    if (warp == Cfg::WARP_TMA && lane == 0) {
+        ptx::mbar_init(bar_q, 1);
+        for (int s = 0; s < ST; ++s) {
+            ptx::mbar_init(bar_kv_full + 8 * s, 1);
+            ptx::mbar_init(bar_kv_empty + 8 * s, nt);
+        }
+        for (int i = 0; i < 2 * NT; ++i) {
+            ptx::mbar_init(bar_s + 8 * i, 1);
+            ptx::mbar_init(bar_p + 8 * i, 8);                        // one arrival per softmax warp of the tile
+        }
+        for (int i = 0; i < NT; ++i) ptx::mbar_init(bar_o + 8 * i, 1);
+        ptx::fence_barrier_init();
+        ptx::tma_prefetch_desc(&tmQKV);
+    }
+    if (warp == Cfg::WARP_MMA) {
+        ptx::tmem_alloc(ptx::smem_u32(&tmem_base_slot), 512);
+        ptx::tmem_relinquish();
+    }
+    __syncthreads();
+    // softmax threads: the row's bound B c = |q_i| max|k| c, and its maximum over the CTA (decides fast / exact)
+    const int t_sm = warp >> 3, q_sm = warp & 3, hf = (warp >> 2) & 1;
+    const int qrow = q0 + t_sm * A2_BQ + q_sm * 32 + lane;
+    float bc = 0.0f;
+    if (warp < Cfg::SM_WARPS) {
+        for (int i = threadIdx.x; i < Cfg::ONES_BYTES / 4; i += Cfg::SM_WARPS * 32)
+            asm volatile("st.shared.b32 [%0], %1;" ::"r"(sOnes + 4 * i), "r"(0x3f803f80u) : "memory");
+        ptx::fence_proxy_async();
+        if (t_sm < nt && qrow < ev1) {
+            bc = __ldg(prm.qn + (int64_t)qrow * prm.H + head) * __ldg(prm.kmax + (int64_t)it.x * prm.H + head) * prm.scale_log2 * 1.00001f;
+            if (!(bc >= 0.0f) || bc > 3.0e38f) bc = 3.0e38f;         // NaN / inf norms: exact path (which is NaN-transparent too)
+        }
+        const float wmax = warp_max(bc);
+        if (lane == 0 && wmax > 0.0f) atomicMax(&bound_bits, __float_as_int(wmax));
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = tmem_base_slot;
+    const bool exact = prm.force_exact || __int_as_float(bound_bits) > A2_FAST_MAX_BOUND;
+    const int n_sweeps = exact ? 2 : 1;          // exact: sweep 0 = row maxima only, sweep 1 = the softmax proper
+
+    if (warp == Cfg::WARP_TMA) {
+        // ------------------------------------------------------------ TMA producer
+        if (lane == 0) {
+            ptx::mbar_expect_tx(bar_q, Cfg::Q_BYTES * nt);
+            for (int t = 0; t < nt; ++t) ptx::tma_load_2d(sQ + t * Cfg::Q_BYTES, &tmQKV, bar_q, head * HD, q0 + t * A2_BQ);
+        }
+        for (int g = 0; g < n_sweeps * nst; ++g) {                   // g = running stage counter over both sweeps
+            const int s = g % ST, i = g % nst;
+            ptx::mbar_wait_long(bar_kv_empty + 8 * s, ((g / ST) & 1) ^ 1);
+            if (lane == 0) {
+                const uint32_t st = sKV + s * Cfg::STAGE_BYTES;
+                const int k0 = ev0 + i * A2_SK;
+                ptx::mbar_expect_tx(bar_kv_full + 8 * s, Cfg::STAGE_BYTES);
+                ptx::tma_load_2d(st, &tmQKV, bar_kv_full + 8 * s, prm.d + head * HD, k0);
+                ptx::tma_load_2d(st + Cfg::K_BYTES, &tmQKV, bar_kv_full + 8 * s, 2 * prm.d + head * HD, k0);
+            }
+            __syncwarp();
+        }
+    } else if (warp > Cfg::WARP_TMA && warp - Cfg::WARP_MMA < nt) {
+        // ------------------------------------------------------------ MMA issuers (one per query tile)
+        const int t = warp - Cfg::WARP_MMA;
+        constexpr uint32_t idesc_s = ptx::umma_idesc_bf16(128, A2_BK);
+        constexpr uint32_t idesc_o = ptx::umma_idesc_bf16(128, HD) | ptx::UMMA_B_MN_MAJOR;
+        constexpr uint32_t idesc_l = ptx::umma_idesc_bf16(128, 8);
+        constexpr uint32_t HALF = A2_BK * Cfg::SW;
+        // n = running tile counter over both sweeps (S buffer n & 1); j = key tile; g = running stage counter
+        auto issue_s = [&](int n, int j, int g) {
+            const uint32_t kb = sKV + (g % ST) * Cfg::STAGE_BYTES + (j & 1) * HALF;
+            const uint32_t qb = sQ + t * Cfg::Q_BYTES;
+#pragma unroll
+            for (int k = 0; k < HD / 16; ++k)
+                ptx::mma_ss(tmem_base + 128 * t + 64 * (n & 1), ptx::umma_desc_kmajor(qb + k * 32, Cfg::SW),
+                            ptx::umma_desc_kmajor(kb + k * 32, Cfg::SW), idesc_s, k != 0);
+            ptx::mma_commit(bar_s + 8 * (2 * t + (n & 1)));
+        };
+        auto issue_o = [&](int n, int j, int g, bool first) {
+            const uint32_t vb = sKV + (g % ST) * Cfg::STAGE_BYTES + Cfg::K_BYTES + (j & 1) * HALF;
+            const uint32_t pb = tmem_base + 128 * t + 64 * (n & 1);
+            const uint64_t ones = ptx::umma_desc_kmajor(sOnes, 128);
+#pragma unroll
+            for (int k = 0; k < A2_BK / 16; ++k) {                  // keys 16k .. 16k+15: P columns 32 (k / 2) + 8 (k % 2)
+                const uint32_t pa = pb + 32 * (k >> 1) + 8 * (k & 1);
+                ptx::mma_ts(tmem_base + Cfg::O_COL0 + Cfg::OW * t, pa, ptx::umma_desc_mnmajor(vb + k * 16 * Cfg::SW, Cfg::SW), idesc_o,
+                            !(first && k == 0));
+                ptx::mma_ts(tmem_base + Cfg::O_COL0 + Cfg::OW * t + HD, pa, ones, idesc_l, !(first && k == 0));
+            }
+        };
+        ptx::mbar_wait(bar_q, 0);
+        int n = 0;
+        for (int sw = 0; sw < n_sweeps; ++sw) {
+            const bool pv = sw == n_sweeps - 1;
+            const int g0 = sw * nst;
+            // the first two S tiles of the sweep (their stage may or may not be the same)
+            ptx::mbar_wait(bar_kv_full + 8 * (g0 % ST), (g0 / ST) & 1);
+            ptx::tc_fence_after();
+            issue_s(n, 0, g0);
+            if (nkv > 1) issue_s(n + 1, 1, g0);
+            for (int j = 0; j < nkv; ++j, ++n) {
+                const int g = g0 + (j >> 1);
+                ptx::mbar_wait_long(bar_p + 8 * (2 * t + (n & 1)), (n >> 1) & 1);   // P_t(j) in TMEM (sweep 0 of 2: S consumed)
+                ptx::tc_fence_after();
+                if (pv) issue_o(n, j, g, j == 0);
+                if ((j & 1) || j == nkv - 1) ptx::mma_commit(bar_kv_empty + 8 * (g % ST));
+                if (j + 2 < nkv) {                   // S_t(j+2) reuses this S buffer: in order after P_t(j) V_j
+                    const int g2 = g0 + ((j + 2) >> 1);
+                    if (((j + 2) & 1) == 0) ptx::mbar_wait(bar_kv_full + 8 * (g2 % ST), (g2 / ST) & 1);
+                    ptx::tc_fence_after();
+                    issue_s(n + 2, j + 2, g2);
+                }
+            }
+        }
+        ptx::mma_commit(bar_o + 8 * t);
+    } else if (warp < Cfg::SM_WARPS) {
+        // ------------------------------------------------------------ softmax warps
+        const int t = t_sm, q = q_sm;
+        if (t < nt) {
+            const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16);
+            const uint32_t o_addr = lane_addr + Cfg::O_COL0 + Cfg::OW * t;
+            const float c = prm.scale_log2;
+            // 32-bit mask of this warp's score half of key tile j: (key inside the event) & (valid row)
+            auto tile_mask = [&](int j) -> uint32_t {
+                const int k0 = ev0 + j * A2_BK + 32 * hf;
+                const int left = ev1 - k0;                               // may be <= 0
+                uint32_t m = left >= 32 ? 0xffffffffu : (left <= 0 ? 0u : (1u << left) - 1u);
+                if (valid_bits) {
+                    const uint32_t* wp = valid_bits + (k0 >> 5);
+                    m &= __funnelshift_r(__ldg(wp), __ldg(wp + 1), k0 & 31);
+                }
+                return m;
+            };
+            const int n_full = valid_bits ? 0 : (ev1 - ev0 - 32 * hf + 32) / A2_BK;   // leading tiles whose half [64 j + 32 hf, + 32) lies inside the event
+            int n = 0;
+            float neg_bc = -bc;
+            if (exact) {
+                // sweep 0: the true row maximum over the valid keys (scores only)
+                float mx = -INFINITY;
+                for (int j = 0; j < nkv; ++j, ++n) {
+                    ptx::mbar_wait(bar_s + 8 * (2 * t + (n & 1)), (n >> 1) & 1);
+                    ptx::tc_fence_after();
+                    uint32_t s[32];
+                    ptx::tmem_ld32(lane_addr + 128 * t + 64 * (n & 1) + 32 * hf, s);
+                    ptx::tmem_ld_wait();
+                    const uint32_t m = j < n_full ? 0xffffffffu : tile_mask(j);
+                    float m4[4] = {mx, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) m4[i & 3] = fmaxf(m4[i & 3], (m >> i) & 1u ? __uint_as_float(s[i]) : -INFINITY);
+                    mx = fmaxf(fmaxf(m4[0], m4[1]), fmaxf(m4[2], m4[3]));
+                    ptx::tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(bar_p + 8 * (2 * t + (n & 1)));      // S consumed
+                }
+                // the row's two score halves exchange their maxima
+                xchg[(t * A2_BQ + q * 32 + lane) * 2 + hf] = mx;
+                asm volatile("bar.sync %0, 64;" ::"r"(1 + t * 4 + q) : "memory");
+                mx = fmaxf(mx, xchg[(t * A2_BQ + q * 32 + lane) * 2 + (hf ^ 1)]);
+                neg_bc = (mx == -INFINITY) ? 0.0f : -mx * c;
+            }
+            // the softmax sweep
+            auto tile = [&](int j, auto masked_tag) {
+                constexpr bool MASKED = decltype(masked_tag)::value;
+                ptx::mbar_wait(bar_s + 8 * (2 * t + (n & 1)), (n >> 1) & 1);
+                ptx::tc_fence_after();
+                const uint32_t s_addr = lane_addr + 128 * t + 64 * (n & 1) + 32 * hf;
+                uint32_t s[32], pk[16];
+                ptx::tmem_ld32(s_addr, s);
+                const uint32_t m = MASKED ? tile_mask(j) : 0xffffffffu;
+                ptx::tmem_ld_wait();
+                a2_exp32<MASKED>(s, m, c, neg_bc, pk);
+                ptx::tmem_st16(s_addr, pk);
+                ptx::tmem_st_wait();
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(bar_p + 8 * (2 * t + (n & 1)));
+            };
+            {
+                int j = 0;
+                for (; j < n_full; ++j, ++n) tile(j, std::false_type{});
+                for (; j < nkv; ++j, ++n) tile(j, std::true_type{});
+            }
+            // all products are in: this warp's half of O_t -> registers, normalise, store
+            ptx::mbar_wait(bar_o + 8 * t, 0);
+            ptx::tc_fence_after();
+            constexpr int HW = HD / 2;                                  // output columns of this warp
+            uint32_t o_r[HW];
+#pragma unroll
+            for (int w = 0; w < HW / 8; ++w) {
+                if (HW % 16 == 0 && (w & 1) == 0) ptx::tmem_ld16(o_addr + HW * hf + w * 8, *reinterpret_cast<uint32_t(*)[16]>(&o_r[w * 8]));
+                if (HW % 16 != 0) {
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) ptx::tmem_ld1(o_addr + HW * hf + w * 8 + i, o_r[w * 8 + i]);
+                }
+            }
+            uint32_t lsum;
+            ptx::tmem_ld1(o_addr + HD, lsum);
+            ptx::tmem_ld_wait();
+            if (qrow < ev1) {
+                const float l_run = __uint_as_float(lsum);
+                const float inv = l_run > 0.0f ? 1.0f / l_run : 0.0f;
+                uint32_t hi[HW / 2], lo[HW / 2];
+#pragma unroll
+                for (int i = 0; i < HW / 2; ++i) {
+                    const float y0 = __uint_as_float(o_r[2 * i]) * inv, y1 = __uint_as_float(o_r[2 * i + 1]) * inv;
+                    __nv_bfloat162 h2 = __floats2bfloat162_rn(y0, y1);
+                    hi[i] = *reinterpret_cast<uint32_t*>(&h2);
+                    __nv_bfloat162 l2 = __floats2bfloat162_rn(y0 - __low2float(h2), y1 - __high2float(h2));
+                    lo[i] = *reinterpret_cast<uint32_t*>(&l2);
+                }
+                uint4* op = reinterpret_cast<uint4*>(prm.O + (int64_t)qrow * prm.d + head * HD + HW * hf);
+#pragma unroll
+                for (int i = 0; i < HW / 8; ++i) op[i] = make_uint4(hi[4 * i], hi[4 * i + 1], hi[4 * i + 2], hi[4 * i + 3]);
+                if (prm.O_lo) {
+                    uint4* lp = reinterpret_cast<uint4*>(prm.O_lo + (int64_t)qrow * prm.d + head * HD + HW * hf);
+#pragma unroll
+                    for (int i = 0; i < HW / 8; ++i) lp[i] = make_uint4(lo[4 * i], lo[4 * i + 1], lo[4 * i + 2], lo[4 * i + 3]);
+                }
+            }
+        }
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == Cfg::WARP_MMA) ptx::tmem_dealloc(tmem_base, 512);
+}
+
+template <int HD>
+static int tc_attn2_launch_hd(TcContext* c, const bf16* QKV, int64_t N, Attn2Params prm, cudaStream_t st) {
+    using Cfg = Attn2Cfg<HD>;
+    CUtensorMap tmQKV;
+    if (tc_tensor_map(c, &tmQKV, QKV, 3 * prm.d, N, 3 * prm.d, HD, A2_SK)) return -1;
+    auto kern = k_tc_attn2<HD>;
+    if (tc_set_smem_attr(c, (const void*)kern, Cfg::SMEM_BYTES)) return -1;
+    kern<<<prm.n_items * prm.H, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(tmQKV, prm);
+    return 0;
+}
+
+// norms pre-pass + attention.  qn [N, H] and kmax [E, H] are caller-owned scratch; row_event [N] from the schedule.
+int tc_attn2_launch(TcContext* c, const bf16* QKV, int64_t N, int E, const uint32_t* valid_bits, const int* n_valid,
+                    const int* offsets, const int* row_event, const int2* items, int n_items, int d, int H, float* qn,
+                    float* kmax, bf16* O, bf16* O_lo, int force_exact, cudaStream_t st) {
+    const int hd = d / H;
+    if (H > 64) { snprintf(c->err, sizeof c->err, "tc_attn2: more than 64 heads"); return -1; }
+    cudaMemsetAsync(kmax, 0, (size_t)E * H * 4, st);
+    const int64_t nthr = N * H;
+    k_attn_norms<<<(unsigned)((nthr + 255) / 256), 256, 0, st>>>(QKV, row_event, (int)N, H, hd, d, qn, kmax);
+    Attn2Params prm;
+    prm.valid_bits = valid_bits; prm.n_valid = n_valid; prm.offsets = offsets; prm.items = items; prm.n_items = n_items;
+    prm.qn = qn; prm.kmax = kmax; prm.H = H; prm.d = d; prm.O = O; prm.O_lo = O_lo; prm.force_exact = force_exact;
+    prm.scale_log2 = 1.4426950408889634f / sqrtf((float)hd);
+    switch (hd) {
+        case 16: return tc_attn2_launch_hd<16>(c, QKV, N, prm, st);
+        case 32: return tc_attn2_launch_hd<32>(c, QKV, N, prm, st);
+        case 64: return tc_attn2_launch_hd<64>(c, QKV, N, prm, st);
+    }
+    snprintf(c->err, sizeof c->err, "tc_attn2: head_dim %d unsupported", hd);
+    return -1;
+}
+
+}  // namespace mlpf

@@ -44,10 +44,16 @@ def test_tc_gemm_matches_fp64_matmul(M, N, K, split):
     assert err <= 2e-5 * max(1.0, np.abs(ref).max()), err
 
 
+# impl: 1 = bound-based kernel (tc_attn2.cu; these inputs take its fast path), 2 = its exact two-sweep path forced,
+# 0 = round 1's lazy-rescale kernel (kept selectable through MLPF_OPT_ATTN)
+IMPLS = [1, 2, 0]
+
+
+@pytest.mark.parametrize("impl", IMPLS)
 @pytest.mark.parametrize("hd,H", [(32, 8), (16, 4), (64, 8)])
 @pytest.mark.parametrize("lens,pad", [((128,), 0.0), ((256, 64), 0.0), ((1, 129, 700, 257), 0.0), ((300, 1000), 0.15),
-                                      ((0, 40, 0), 0.5)])
-def test_tc_attention_matches_dense_softmax(hd, H, lens, pad):
+                                      ((0, 40, 0), 0.5), ((33, 95, 160, 417), 0.0)])
+def test_tc_attention_matches_dense_softmax(hd, H, lens, pad, impl):
     d = hd * H
     rng = np.random.default_rng(hd + sum(lens))
     N = sum(lens)
@@ -58,7 +64,7 @@ def test_tc_attention_matches_dense_softmax(hd, H, lens, pad):
     valid = (rng.random(N) >= pad)
     QKV = _bf16(qkv)
     kv = torch.from_numpy(valid.astype(np.int32)).cuda()
-    O = P.tc_attention_bf16(QKV, kv if pad > 0 else None, off, d, H).float().cpu().numpy()
+    O = P.tc_attention_bf16(QKV, kv if pad > 0 else None, off, d, H, impl=impl).float().cpu().numpy()
     if pad == 0:
         valid[:] = True
     qk64 = QKV.float().cpu().numpy().astype(np.float64)
@@ -74,7 +80,7 @@ def test_tc_attention_matches_dense_softmax(hd, H, lens, pad):
 
 
 # ------------------------------------------------------------------------------------------- adversarial softmax inputs
-def _attn_check(qkv, lens, valid, hd, H, tol=2e-2):
+def _attn_check(qkv, lens, valid, hd, H, tol=2e-2, impl=1):
     """tcgen05 attention vs oracle.attention_event (Eq. 4 written out) element by element; the scale of the floor is
     the rms of the oracle output of that event."""
     d = hd * H
@@ -82,7 +88,7 @@ def _attn_check(qkv, lens, valid, hd, H, tol=2e-2):
     off[1:] = np.cumsum(lens)
     QKV = _bf16(qkv)
     kv = None if valid is None else torch.from_numpy(valid.astype(np.int32)).cuda()
-    O = P.tc_attention_bf16(QKV, kv, off, d, H).float().cpu().numpy()
+    O = P.tc_attention_bf16(QKV, kv, off, d, H, impl=impl).float().cpu().numpy()
     torch.cuda.synchronize()
     assert np.isfinite(O).all()
     q64 = QKV.float().cpu().numpy().astype(np.float64)
@@ -99,8 +105,9 @@ def _attn_check(qkv, lens, valid, hd, H, tol=2e-2):
     return O
 
 
+@pytest.mark.parametrize("impl", IMPLS)
 @pytest.mark.parametrize("hd,H", [(32, 4), (64, 2), (16, 4)])
-def test_tc_attention_running_max_climbs_every_tile(hd, H):
+def test_tc_attention_running_max_climbs_every_tile(hd, H, impl):
     """Keys ordered so that the row maximum rises by far more than 2^8 from one 64-key tile to the next (and, for the
     rows with a negative query coefficient, falls): the reference maximum of an online softmax has to move on every
     tile (or a one-shot bound has to be far from the first tiles' scores)."""
@@ -113,21 +120,23 @@ def test_tc_attention_running_max_climbs_every_tile(hd, H):
     sign = np.where(rng.random(n) < 0.5, 1.0, -1.0).astype(np.float32)
     qkv[:, :d] += 24.0 * sign[:, None] * u[None, :]                         # ... = 61 raw units per 64-key tile: 11 log2 units at hd = 64, 15 at hd = 32
     qkv[:, d:2 * d] += ramp[:, None] * u[None, :]
-    _attn_check(qkv, (n,), None, hd, H)
+    _attn_check(qkv, (n,), None, hd, H, impl=impl)
 
 
+@pytest.mark.parametrize("impl", IMPLS)
 @pytest.mark.parametrize("hd,H", [(32, 4), (64, 2)])
-def test_tc_attention_outlier_key_in_the_last_tile(hd, H):
+def test_tc_attention_outlier_key_in_the_last_tile(hd, H, impl):
     """One key 40 sigma away from the others, in the last (ragged) tile: every row's weight ends up on it."""
     rng = np.random.default_rng(hd + 1)
     n, d = 777, hd * H
     qkv = rng.standard_normal((n, 3 * d)).astype(np.float32)
     qkv[n - 3, d:2 * d] = 40.0 * np.sign(rng.standard_normal(d))
-    _attn_check(qkv, (n,), None, hd, H)
+    _attn_check(qkv, (n,), None, hd, H, impl=impl)
 
 
+@pytest.mark.parametrize("impl", IMPLS)
 @pytest.mark.parametrize("hd,H", [(32, 4), (64, 2)])
-def test_tc_attention_only_the_last_key_is_valid(hd, H):
+def test_tc_attention_only_the_last_key_is_valid(hd, H, impl):
     """Every key but the last one of each event is a pad row: O must equal that key's V row for all queries."""
     rng = np.random.default_rng(hd + 2)
     lens = (300, 131)
@@ -135,14 +144,15 @@ def test_tc_attention_only_the_last_key_is_valid(hd, H):
     qkv = rng.standard_normal((n, 3 * d)).astype(np.float32)
     valid = np.zeros(n, bool)
     valid[[299, 430]] = True
-    O = _attn_check(qkv, lens, valid, hd, H)
+    O = _attn_check(qkv, lens, valid, hd, H, impl=impl)
     v = _bf16(qkv).float().cpu().numpy()[:, 2 * d:]
     assert np.abs(O[:300] - v[299]).max() <= 2e-2 * np.abs(v[299]).max()
     assert np.abs(O[300:] - v[430]).max() <= 2e-2 * np.abs(v[430]).max()
 
 
+@pytest.mark.parametrize("impl", IMPLS)
 @pytest.mark.parametrize("hd,H", [(32, 4), (64, 2)])
-def test_tc_attention_sharp_scores_with_pad_rows(hd, H):
+def test_tc_attention_sharp_scores_with_pad_rows(hd, H, impl):
     """10 % scattered pad rows together with Q x 8: a leaked pad key would carry real weight."""
     rng = np.random.default_rng(hd + 3)
     lens = (1500, 333, 900)
@@ -151,28 +161,30 @@ def test_tc_attention_sharp_scores_with_pad_rows(hd, H):
     qkv[:, :d] *= 8.0
     valid = rng.random(n) >= 0.10
     qkv[~valid, d:2 * d] *= 3.0                           # pad keys would win the softmax if they were not masked
-    _attn_check(qkv, lens, valid, hd, H)
+    _attn_check(qkv, lens, valid, hd, H, impl=impl)
 
 
+@pytest.mark.parametrize("impl", IMPLS)
 @pytest.mark.parametrize("hd,H", [(32, 2), (64, 1)])
-def test_tc_attention_16384_keys(hd, H):
+def test_tc_attention_16384_keys(hd, H, impl):
     """The longest event of BASELINE.json (config 5): 16384 elements, 10 % pad rows, scores sharper than unit variance."""
     rng = np.random.default_rng(hd + 4)
     n, d = 16384, hd * H
     qkv = rng.standard_normal((n, 3 * d)).astype(np.float32)
     qkv[:, :d] *= 3.0
     valid = rng.random(n) >= 0.10
-    _attn_check(qkv, (n,), valid, hd, H)
+    _attn_check(qkv, (n,), valid, hd, H, impl=impl)
 
 
-def test_tc_attention_huge_scores():
+@pytest.mark.parametrize("impl", IMPLS)
+def test_tc_attention_huge_scores(impl):
     """Scores near +-1e3 (|q.k| / sqrt(hd) up to ~1200): exponent range, not precision, is what is exercised."""
     rng = np.random.default_rng(9)
     hd, H, n = 32, 2, 500
     d = hd * H
     qkv = rng.standard_normal((n, 3 * d)).astype(np.float32)
     qkv[:, :2 * d] *= 14.0
-    _attn_check(qkv, (n,), None, hd, H)
+    _attn_check(qkv, (n,), None, hd, H, impl=impl)
 
 
 # ------------------------------------------------------------------------------------------- fused post-attention block
