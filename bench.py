@@ -206,6 +206,8 @@ def run_ours(args):
     peaks = load_peaks()
 
     mod = P.Mlpf(W, m)
+    for key, val in (args.opt or []):
+        mod.set_option(int(key), int(val))
     st = torch.cuda.Stream()
     Xd = torch.from_numpy(X).cuda()
     lg = torch.empty((N, mod.n_classes), dtype=torch.float32, device="cuda")
@@ -423,6 +425,8 @@ def main():
     ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5a", "cfg5b", "paper"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", nargs=2, action="append", metavar=("KEY", "VALUE"),
+                    help="mlpf_set_option(KEY, VALUE) before the run (tuning experiments; include/mlpf.h MLPF_OPT_*)")
     ap.add_argument("--streams", type=int, default=1, help="also time the batch split over this many concurrent CUDA streams")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

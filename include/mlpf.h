@@ -148,6 +148,8 @@ int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* 
 #define MLPF_OPT_ATTN        8   /* attention kernel: 1 (default) = tc_attn2.cu (no running maximum: Cauchy-Schwarz bound from a norms
                                     pre-pass, exact two-sweep path when the bound is too loose; two threads per query row);
                                     2 = the same with the exact path forced for every CTA; 0 = round 1's lazy-rescale kernel */
+#define MLPF_OPT_ATTN_POLY   9   /* tuning (process-wide): n of every 16 pairs of softmax exponentials run as a polynomial on the
+                                    FMA pipe instead of the MUFU: 0 (none), 4..9; -1 (default) = per head dimension          */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0

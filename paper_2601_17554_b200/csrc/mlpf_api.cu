@@ -238,6 +238,9 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_ATTN:
             if (value < 0 || value > 2) return set_err(MLPF_E_ARG, "attn must be 0, 1 or 2");
             h->attn = (int)value; return MLPF_OK;
+        case MLPF_OPT_ATTN_POLY:
+            if (value < -1 || value > 9 || (value > 0 && value < 4)) return set_err(MLPF_E_ARG, "attn_poly must be -1, 0 or 4..9");
+            g_attn2_poly_every = (int)value; return MLPF_OK;
         case MLPF_OPT_FUSE:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "fuse must be 0 or 1");
             h->fuse = (int)value; return MLPF_OK;

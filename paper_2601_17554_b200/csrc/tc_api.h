@@ -58,6 +58,7 @@ int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const uint32_t* val
 // path for CTAs whose bound is too loose), two threads per query row.  qn [N, H], kmax [E, H]: caller-owned fp32 scratch;
 // row_event [N] from the schedule.  force_exact != 0: every CTA takes the exact path (tests).
 int tc_attn2_rows_per_cta(int hd);
+extern int g_attn2_poly_every;       // tuning knob: every n-th pair of exponentials on the FMA pipe (0, 2, 3, 4; -1 = default)
 int tc_attn2_launch(TcContext* c, const bf16* QKV, int64_t N, int E, const uint32_t* valid_bits, const int* n_valid,
                     const int* offsets, const int* row_event, const int2* items, int n_items, int d, int H, float* qn,
                     float* kmax, bf16* O, bf16* O_lo, int force_exact, cudaStream_t st);

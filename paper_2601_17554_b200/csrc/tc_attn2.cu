@@ -107,44 +107,52 @@ k_attn_norms(const bf16* __restrict__ QKV, const int* __restrict__ row_event, in
         atomicMax(reinterpret_cast<int*>(kmax) + (int64_t)ev_first * H + threadIdx.x, smax[threadIdx.x]);
 }
 
-// 2^x for a pair, x <= 0, on the FMA / ALU pipes instead of the MUFU (Cody-Waite split + degree-3 polynomial, max
-// relative error 1.0e-4, 40x below the bf16 rounding of P); see tc_attn.cu.
-__device__ __forceinline__ float2 a2_exp2_poly2(float2 x) {
-    const float2 magic = make_float2(12582912.0f, 12582912.0f);
-    x.x = fmaxf(x.x, -126.0f); x.y = fmaxf(x.y, -126.0f);
-    const float2 xr = ptx::fadd2(x, magic);
-    const float2 f = ptx::fadd2(x, ptx::fadd2(magic, make_float2(-xr.x, -xr.y)));
+// 2^(s c - Bc) for a pair of scores on the FMA / ALU pipes instead of the MUFU (Cody-Waite split + degree-3 polynomial, max
+// relative error 1.0e-4, 40x below the bf16 rounding of P).  Bc is an INTEGER (the bound rounded up), so everything the
+// range reduction needs comes out of exactly rounded FMAs on the raw scores:
+//   xr = s c + (M - Bc)            M = 1.5 * 2^23: the low mantissa bits of xr hold n = round(s c - Bc)
+//   f  = s c - (Bc + n)            with Bc + n = xr - (M - Bc) exactly;  |f| <= 0.5
+//   2^f ~ 1 + f (c1 + f (c2 + f c3));  2^n goes into the exponent field with one integer multiply-add.
+// 8 issue slots per pair.  Fast path only (s c - Bc > -97 there); the exact path and masked tiles (-inf scores) use the MUFU.
+__device__ __forceinline__ float2 a2_exp2_poly2(float2 sc, float2 c2, float2 k1) {
+    const float2 xr = ptx::ffma2(sc, c2, k1);
+    const float2 m = ptx::fadd2(xr, make_float2(-k1.x, -k1.y));
+    const float2 f = ptx::ffma2(sc, c2, make_float2(-m.x, -m.y));
     float2 p = ptx::ffma2(f, make_float2(0.0550089306f, 0.0550089306f), make_float2(0.2422109596f, 0.2422109596f));
     p = ptx::ffma2(p, f, make_float2(0.6932829272f, 0.6932829272f));
     p = ptx::ffma2(p, f, make_float2(1.0f, 1.0f));
     return make_float2(__int_as_float(__float_as_int(p.x) + (__float_as_int(xr.x) << 23)),
                        __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
 }
-#ifndef A2_POLY_EVERY
-#define A2_POLY_EVERY 4      // every A2_POLY_EVERY-th pair of exponentials runs on the FMA pipe (0: all on the MUFU)
-#endif
+// PE of every 16 pairs of exponentials run on the FMA pipe, evenly spread (PE = 0: all on the MUFU).  The MUFU does 16 ex2
+// per clock and SM and is the binding unit at hd = 32 (one ex2 per 128 tensor FLOPs); PE balances the MUFU against the
+// FMA / ALU pipes and the issue slots (measured on cfg3, ms per step of the attention class: profiles/r02_README.md).
 
-// 32 scores of one row -> 16 packed bf16 pairs  p = 2^(s c - B c).  MASKED: scores of masked keys become -inf first, so the
-// MUFU gives the exact weight 0 (the polynomial path clamps its argument and is not used on masked tiles).
-template <bool MASKED>
+// 32 scores of one row -> 16 packed bf16 pairs  p = 2^(s c - Bc).  MASKED: scores of masked keys become -inf first, so the
+// MUFU gives the exact weight 0 (the polynomial path is not used on masked tiles).
+template <bool MASKED, int PE>
 __device__ __forceinline__ void a2_exp32(uint32_t (&s)[32], uint32_t mask, float c, float neg_bc, uint32_t (&pk)[16]) {
     const float2 c2 = make_float2(c, c), m2 = make_float2(neg_bc, neg_bc);
+    const float2 k1 = make_float2(12582912.0f + neg_bc, 12582912.0f + neg_bc);      // exact: neg_bc is an integer on this path
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
         if (MASKED) {
             s[2 * i] = (mask >> (2 * i)) & 1u ? s[2 * i] : 0xff800000u;
             s[2 * i + 1] = (mask >> (2 * i + 1)) & 1u ? s[2 * i + 1] : 0xff800000u;
         }
-        const float2 x = ptx::ffma2(make_float2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), c2, m2);
+        const float2 sc = make_float2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1]));
         float2 p;
-        if (!MASKED && A2_POLY_EVERY > 0 && (i % (A2_POLY_EVERY > 0 ? A2_POLY_EVERY : 1)) == 0) p = a2_exp2_poly2(x);
-        else p = make_float2(ptx::fast_exp2(x.x), ptx::fast_exp2(x.y));
+        if (!MASKED && ((i + 1) * PE) / 16 > (i * PE) / 16) p = a2_exp2_poly2(sc, c2, k1);
+        else {
+            const float2 x = ptx::ffma2(sc, c2, m2);
+            p = make_float2(ptx::fast_exp2(x.x), ptx::fast_exp2(x.y));
+        }
         __nv_bfloat162 b2 = __floats2bfloat162_rn(p.x, p.y);
         pk[i] = *reinterpret_cast<uint32_t*>(&b2);
     }
 }
 
-template <int HD>
+template <int HD, int PE>
 __global__ void __launch_bounds__(Attn2Cfg<HD>::THREADS, 1)
 k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
     using Cfg = Attn2Cfg<HD>;
@@ -207,6 +215,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
         ptx::fence_proxy_async();
         if (t_sm < nt && qrow < ev1) {
             bc = __ldg(prm.qn + (int64_t)qrow * prm.H + head) * __ldg(prm.kmax + (int64_t)it.x * prm.H + head) * prm.scale_log2 * 1.00001f;
+            bc = ceilf(bc);                                          // an integer bound: the polynomial path's range reduction is exact
             if (!(bc >= 0.0f) || bc > 3.0e38f) bc = 3.0e38f;         // NaN / inf norms: exact path (which is NaN-transparent too)
         }
         const float wmax = warp_max(bc);
@@ -309,6 +318,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
                 }
                 return m;
             };
+            // (the exact path sends EVERY tile through the masked variant: its exponents can be far below -126)
             const int n_full = valid_bits ? 0 : (ev1 - ev0 - 32 * hf + 32) / A2_BK;   // leading tiles whose half [64 j + 32 hf, + 32) lies inside the event
             int n = 0;
             float neg_bc = -bc;
@@ -321,7 +331,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
                     uint32_t s[32];
                     ptx::tmem_ld32(lane_addr + 128 * t + 64 * (n & 1) + 32 * hf, s);
                     ptx::tmem_ld_wait();
-                    const uint32_t m = j < n_full ? 0xffffffffu : tile_mask(j);
+                    const uint32_t m = tile_mask(j);
                     float m4[4] = {mx, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
                     for (int i = 0; i < 32; ++i) m4[i & 3] = fmaxf(m4[i & 3], (m >> i) & 1u ? __uint_as_float(s[i]) : -INFINITY);
@@ -346,7 +356,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
                 ptx::tmem_ld32(s_addr, s);
                 const uint32_t m = MASKED ? tile_mask(j) : 0xffffffffu;
                 ptx::tmem_ld_wait();
-                a2_exp32<MASKED>(s, m, c, neg_bc, pk);
+                a2_exp32<MASKED, PE>(s, m, c, neg_bc, pk);
                 ptx::tmem_st16(s_addr, pk);
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
@@ -355,7 +365,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
             };
             {
                 int j = 0;
-                for (; j < n_full; ++j, ++n) tile(j, std::false_type{});
+                for (; j < (exact ? 0 : n_full); ++j, ++n) tile(j, std::false_type{});
                 for (; j < nkv; ++j, ++n) tile(j, std::true_type{});
             }
             // all products are in: this warp's half of O_t -> registers, normalise, store
@@ -402,15 +412,31 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
     if (warp == Cfg::WARP_MMA) ptx::tmem_dealloc(tmem_base, 512);
 }
 
-template <int HD>
-static int tc_attn2_launch_hd(TcContext* c, const bf16* QKV, int64_t N, Attn2Params prm, cudaStream_t st) {
+int g_attn2_poly_every = -1;          // tuning knob (MLPF_OPT_ATTN_POLY): -1 = the default of the head dimension
+
+template <int HD, int PE>
+static int tc_attn2_launch_pe(TcContext* c, const bf16* QKV, int64_t N, Attn2Params prm, cudaStream_t st) {
     using Cfg = Attn2Cfg<HD>;
     CUtensorMap tmQKV;
     if (tc_tensor_map(c, &tmQKV, QKV, 3 * prm.d, N, 3 * prm.d, HD, A2_SK)) return -1;
-    auto kern = k_tc_attn2<HD>;
+    auto kern = k_tc_attn2<HD, PE>;
     if (tc_set_smem_attr(c, (const void*)kern, Cfg::SMEM_BYTES)) return -1;
     kern<<<prm.n_items * prm.H, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(tmQKV, prm);
     return 0;
+}
+
+template <int HD>
+static int tc_attn2_launch_hd(TcContext* c, const bf16* QKV, int64_t N, Attn2Params prm, cudaStream_t st) {
+    const int pe = g_attn2_poly_every >= 0 ? g_attn2_poly_every : (HD == 64 ? 0 : 7);
+    switch (pe) {
+        case 0: return tc_attn2_launch_pe<HD, 0>(c, QKV, N, prm, st);
+        case 4: return tc_attn2_launch_pe<HD, 4>(c, QKV, N, prm, st);
+        case 5: return tc_attn2_launch_pe<HD, 5>(c, QKV, N, prm, st);
+        case 8: return tc_attn2_launch_pe<HD, 8>(c, QKV, N, prm, st);
+        case 9: return tc_attn2_launch_pe<HD, 9>(c, QKV, N, prm, st);
+        case 6: return tc_attn2_launch_pe<HD, 6>(c, QKV, N, prm, st);
+        default: return tc_attn2_launch_pe<HD, 7>(c, QKV, N, prm, st);
+    }
 }
 
 // norms pre-pass + attention.  qn [N, H] and kmax [E, H] are caller-owned scratch; row_event [N] from the schedule.
