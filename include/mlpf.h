@@ -37,9 +37,11 @@ typedef struct mlpf_handle mlpf_handle;
 /* ---- weight blob (little-endian) -------------------------------------------------------------------
  * 256-byte header, then fp32 tensors, row-major [out,in] (y = x W^T + b), in this order:
  *   for type t = 1..n_types      : emb.t.W1[d,F] b1[d] W2[d,d] b2[d]                     (L156, A3-A4)
- *   for layer l = 0..n_layers-1  : ln1.g[d] ln1.b[d] Wqkv[3d,d] bqkv[3d] Wo[d,d] bo[d]
+ *   for stack s = 0..n_stacks-1, for layer l = 0..n_layers-1 :
+ *                                  ln1.g[d] ln1.b[d] Wqkv[3d,d] bqkv[3d] Wo[d,d] bo[d]
  *                                  ln2.g[d] ln2.b[d] W1[dff,d] b1[dff] W2[d,dff] b2[d]   (L148-L156)
- *   lnf.g[d] lnf.b[d]                                                                    (A7)
+ *   for stack s                  : lnf.g[d] lnf.b[d]                                     (A7)
+ *   if binary_head               : bin.W1[d,d] b1[d] W2[1,d] b2[1]                       (L156, Fig. 2)
  *   cls.W1[d,d] b1[d] W2[C,d] b2[C]                                                      (L156, A11)
  *   for k = 0..n_reg_heads-1     : reg.k.W1[d,d] b1[d] W2[reg_dims[k],d] b2[reg_dims[k]]
  * Master weights are fp32.  In BF16 mode the library rounds (RNE) the matrices that feed tensor-core
@@ -47,7 +49,7 @@ typedef struct mlpf_handle mlpf_handle;
  * (cls.W2, reg.k.W2, bin.W2) and all vectors stay fp32.
  */
 #define MLPF_BLOB_MAGIC   "MLPFBLOB"
-#define MLPF_BLOB_VERSION 1u
+#define MLPF_BLOB_VERSION 2u  /* version 1 blobs (one stack, no binary head; the two new header fields are padding) still load */
 #define MLPF_HEADER_BYTES 256
 #define MLPF_MAX_REG_HEADS 4
 
@@ -66,6 +68,9 @@ typedef struct mlpf_blob_header {
     uint32_t activation;     /* 0 = ReLU (L156), 1 = GELU exact-erf form (A6) */
     uint32_t final_ln;       /* 0/1 (A7) */
     float    ln_eps;         /* 1e-5 (A8) */
+    uint32_t n_stacks;       /* version 2: 1 = one encoder; 2 = the paper's two parallel encoders on the shared embedding
+                                (L156): stack 0 = classification, stack 1 = regression */
+    uint32_t binary_head;    /* version 2: 1 = a binary "valid" head on stack 0 (L156, Fig. 2) */
     /* zero padding up to MLPF_HEADER_BYTES */
 } mlpf_blob_header;
 
@@ -93,6 +98,13 @@ int mlpf_infer(mlpf_handle* h, const float* elements, const int32_t* event_offse
 int mlpf_infer_host(mlpf_handle* h, const float* elements_host, const int32_t* event_offsets,
                     int32_t n_events, float* out_logits_host, float* out_regress_host, void* stream);
 
+/* mlpf_infer_ex: mlpf_infer plus the binary head's logit, out_binary DEVICE [N] fp32 (pad rows 0), for models with a binary
+ * head (MLPF_Q_BINARY_HEAD); out_binary may be NULL.  With n_stacks = 2 the binary and PID heads read the classification
+ * encoder and the regression heads read the regression encoder (L156); both encoders run as ONE grouped batch (every
+ * kernel launch covers both stacks). */
+int mlpf_infer_ex(mlpf_handle* h, const float* elements, const int32_t* event_offsets, int32_t n_events,
+                  float* out_logits, float* out_regress, float* out_binary, void* stream);
+
 void mlpf_destroy(mlpf_handle* h);
 
 /* Thread-local text of the last error raised on this thread ("" if none). */
@@ -101,8 +113,9 @@ const char* mlpf_last_error(void);
 /* ---- candidate building (the step after the forward pass; "builds the particle candidates") -------
  * From the per-element outputs of mlpf_infer to the per-event list of particle candidates:
  *   PID_i = argmax_c logits[i,c] (multiclass PID head, L130/L156; ties -> lowest class);
- *   element i yields a candidate iff its type (feature 0) != 0 and PID_i != 0 (class 0 = "no particle": reading A23,
- *   the library's single 9-class head has no separate binary head, reading A11);
+ *   element i yields a candidate iff its type (feature 0, clamped to 0..4) != 0 and PID_i != 0 (class 0 = "no particle":
+ *   DEPARTURE A23 from the paper's rule, for models whose single PID head is all there is; models with a binary head use
+ *   mlpf_build_candidates_ex, which implements the paper's rule);
  *   pT = x_i[1] exp(pT'), E = x_i[4] exp(E') (Eq. 2 inverted, L137-L139; x_i[1], x_i[4] = the element's own pT, E),
  *   eta = raw output, phi = atan2(sin phi, cos phi) (L126).
  * Candidates keep the element order (stable compaction) and are grouped per event:
@@ -117,6 +130,14 @@ const char* mlpf_last_error(void);
  * Integer outputs are bit-exact vs the oracle on the same fp32 logits; pT, E, phi are fp32 expf / atan2f.
  * n_events == 0: success, nothing written.  N == 0: cand_offsets is all zeros.  Errors as for mlpf_infer. */
 int64_t mlpf_candidates_scratch_bytes(int64_t n_elements, int32_t n_events);   /* < 0 on error */
+/* mlpf_build_candidates_ex: the same with the paper's selection rule (L156): `binary` DEVICE [N] fp32 = the binary head's
+ * logit; an element yields a candidate iff it is not a pad row and sigmoid(binary) > 0.5 (i.e. binary > 0), its PID is
+ * the argmax over ALL classes.  binary == NULL: the class-0 rule above (departure A23).  n_regress must be 5;
+ * n_classes <= 48. */
+int mlpf_build_candidates_ex(const float* elements, int32_t n_feat, const int32_t* event_offsets, int32_t n_events,
+                             const float* logits, int32_t n_classes, const float* regress, int32_t n_regress,
+                             const float* binary, void* scratch, int64_t scratch_bytes, int32_t* cand_offsets,
+                             int32_t* cand_elem, int32_t* cand_pid, float* cand_p4, void* stream);
 int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* event_offsets, int32_t n_events,
                           const float* logits, int32_t n_classes, const float* regress, void* scratch,
                           int64_t scratch_bytes, int32_t* cand_offsets, int32_t* cand_elem, int32_t* cand_pid,
@@ -168,6 +189,8 @@ int mlpf_set_option(mlpf_handle* h, int key, int64_t value);
 #define MLPF_Q_WORKSPACE_BYTES 9   /* device bytes held by all per-stream workspaces (linear in N)      */
 #define MLPF_Q_N_PARAMS        10
 #define MLPF_Q_LAUNCHES        11  /* kernels launched by the last mlpf_infer on this handle             */
+#define MLPF_Q_N_STACKS        12
+#define MLPF_Q_BINARY_HEAD     13
 int64_t mlpf_query(const mlpf_handle* h, int key);   /* < 0 on error */
 
 /* ---- debug taps (tests only; these synchronise `stream`) ------------------------------------------- */

@@ -39,13 +39,15 @@ def build_candidates(X, offsets, logits, regress, binary=None):
     X = np.asarray(X)[:N]
     logits = np.asarray(logits)[:N]
     regress = np.asarray(regress, dtype=np.float64)[:N]
-    etype = X[:, 0].astype(np.int64)                       # reading A1: feature 0 is the type id
+    etype = np.clip(X[:, 0].astype(np.int64), 0, 4)       # reading A1: feature 0 is the type id, clamped to 0..4 as in the forward pass
     pid = np.argmax(logits, axis=1) if N else np.zeros(0, np.int64)   # first maximum wins
     if binary is None:
         keep = (etype != 0) & (pid != 0)                   # departure A23: no binary head
     else:
         b = np.asarray(binary, dtype=np.float64)[:N]
-        keep = (etype != 0) & (1.0 / (1.0 + np.exp(-b)) > 0.5)   # L156: binary score above 0.5
+        # L156: binary score above 0.5.  The score is sigmoid(b); sigmoid is strictly increasing with sigmoid(0) = 1/2, so
+        # "score > 0.5" is exactly "b > 0" (evaluating 1 / (1 + exp(-b)) in floating point would round tiny b > 0 to 0.5)
+        keep = (etype != 0) & (b > 0.0)
     cand_elem = np.nonzero(keep)[0].astype(np.int32)
     cand_offsets = np.zeros(E + 1, np.int32)
     for e in range(E):

@@ -20,13 +20,13 @@ OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE, O
 PREC_BF16, PREC_FP32_DEBUG = 0, 1
 KERNELS_TC, KERNELS_SIMPLE = 0, 1
 Q_N_LAYERS, Q_D_MODEL, Q_N_HEADS, Q_D_FF, Q_N_FEAT, Q_N_CLASSES, Q_N_REGRESS = 1, 2, 3, 4, 5, 6, 7
-Q_WEIGHT_BYTES, Q_WORKSPACE_BYTES, Q_N_PARAMS, Q_LAUNCHES = 8, 9, 10, 11
+Q_WEIGHT_BYTES, Q_WORKSPACE_BYTES, Q_N_PARAMS, Q_LAUNCHES, Q_N_STACKS, Q_BINARY_HEAD = 8, 9, 10, 11, 12, 13
 SCHED = dict(row_event=0, row_pos=1, valid=2, n_valid=3, type_offsets=4, sorted_row=5, type_perm=6, work_list=7)
 TENSOR = dict(H=0, U=1, QK=2, V=3, O=4, G=5)
 KERNEL_CLASSES = ["sched", "embed_l1", "embed_l2", "layernorm", "qkv", "attention", "outproj", "ffn1", "ffn2",
                   "heads_l1", "heads_l2", "post"]
 
-EXPORTS = ["mlpf_create", "mlpf_infer", "mlpf_infer_host", "mlpf_destroy", "mlpf_last_error", "mlpf_set_option",
+EXPORTS = ["mlpf_create", "mlpf_infer", "mlpf_infer_ex", "mlpf_build_candidates_ex", "mlpf_infer_host", "mlpf_destroy", "mlpf_last_error", "mlpf_set_option",
            "mlpf_query", "mlpf_debug_get_schedule", "mlpf_debug_get_tensor", "mlpf_debug_get_profile", "mlpf_tc_gemm_bf16",
            "mlpf_tc_attention_bf16", "mlpf_debug_set_attention_impl", "mlpf_tc_post_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates"]
 
@@ -47,6 +47,10 @@ def lib():
     L.mlpf_create.argtypes = [vp, C.c_size_t]
     L.mlpf_infer.restype = C.c_int
     L.mlpf_infer.argtypes = [vp, vp, vp, i32, vp, vp, vp]
+    L.mlpf_infer_ex.restype = C.c_int
+    L.mlpf_infer_ex.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp]
+    L.mlpf_build_candidates_ex.restype = C.c_int
+    L.mlpf_build_candidates_ex.argtypes = [vp, i32, vp, i32, vp, i32, vp, i32, vp, vp, i64, vp, vp, vp, vp, vp]
     L.mlpf_infer_host.restype = C.c_int
     L.mlpf_infer_host.argtypes = [vp, vp, vp, i32, vp, vp, vp]
     L.mlpf_destroy.restype = None
@@ -112,6 +116,7 @@ class Mlpf:
         self.n_regress = int(self.query(Q_N_REGRESS))
         self.n_feat = int(self.query(Q_N_FEAT))
         self.d_model = int(self.query(Q_D_MODEL))
+        self.binary_head = bool(self.query(Q_BINARY_HEAD))
 
     def close(self):
         if self._h is not None:
@@ -130,13 +135,26 @@ class Mlpf:
     def query(self, key):
         return _check(lib().mlpf_query(self._h, key))
 
-    def infer(self, elements, event_offsets, out_logits=None, out_regress=None, stream=None):
+    def infer(self, elements, event_offsets, out_logits=None, out_regress=None, stream=None, out_binary=None, with_binary=False):
         """elements: CUDA float32 tensor [N, n_feat]; event_offsets: host int32 array [E+1].
-        Returns (logits [N,C], regress [N,R]) CUDA float32 tensors (enqueued on `stream`)."""
+        Returns (logits [N,C], regress [N,R]) CUDA float32 tensors (enqueued on `stream`); with with_binary=True (models with
+        a binary head) also the binary head's logit [N]."""
         import torch
         assert elements.is_cuda and elements.dtype == torch.float32 and elements.is_contiguous()
         off = np.ascontiguousarray(event_offsets, dtype=np.int32)
         N = elements.shape[0]
+        assert len(off) >= 1 and int(off[-1]) == N, "event_offsets[-1] must equal the number of element rows"
+        if with_binary or out_binary is not None:
+            if out_logits is None:
+                out_logits = torch.empty((N, self.n_classes), dtype=torch.float32, device=elements.device)
+            if out_regress is None:
+                out_regress = torch.empty((N, self.n_regress), dtype=torch.float32, device=elements.device)
+            if out_binary is None:
+                out_binary = torch.empty((N,), dtype=torch.float32, device=elements.device)
+            _check(lib().mlpf_infer_ex(self._h, C.c_void_p(elements.data_ptr()), off.ctypes.data_as(C.c_void_p), len(off) - 1,
+                                       C.c_void_p(out_logits.data_ptr()), C.c_void_p(out_regress.data_ptr()),
+                                       C.c_void_p(out_binary.data_ptr()), _stream_ptr(stream)))
+            return out_logits, out_regress, out_binary
         if out_logits is None:
             out_logits = torch.empty((N, self.n_classes), dtype=torch.float32, device=elements.device)
         if out_regress is None:
@@ -220,7 +238,7 @@ def tc_post_bf16(o_hi, o_lo, h, Wo, bo, ln2g, ln2b, W1, b1, W2, b2, lnng, lnnb, 
     return u_hi, u_lo
 
 
-def build_candidates(elements, event_offsets, logits, regress, scratch=None, stream=None):
+def build_candidates(elements, event_offsets, logits, regress, scratch=None, stream=None, binary=None):
     """Per-event particle candidates from mlpf_infer's outputs (include/mlpf.h "candidate building").
     CUDA tensors in; returns dict(cand_offsets [E+1] int32, cand_elem [N] int32, cand_pid [N] int32,
     cand_p4 [N,4] float32 = (pT, eta, phi, E)), all CUDA, enqueued on `stream`; the first cand_offsets[-1]
@@ -240,8 +258,9 @@ def build_candidates(elements, event_offsets, logits, regress, scratch=None, str
                cand_elem=torch.empty(N, dtype=torch.int32, device=dev),
                cand_pid=torch.empty(N, dtype=torch.int32, device=dev),
                cand_p4=torch.empty((N, 4), dtype=torch.float32, device=dev))
-    _check(lib().mlpf_build_candidates(C.c_void_p(elements.data_ptr()), elements.shape[1], off.ctypes.data_as(C.c_void_p), E,
-                                       C.c_void_p(logits.data_ptr()), logits.shape[1], C.c_void_p(regress.data_ptr()),
+    _check(lib().mlpf_build_candidates_ex(C.c_void_p(elements.data_ptr()), elements.shape[1], off.ctypes.data_as(C.c_void_p), E,
+                                       C.c_void_p(logits.data_ptr()), logits.shape[1], C.c_void_p(regress.data_ptr()), regress.shape[1],
+                                       C.c_void_p(binary.data_ptr() if binary is not None else 0),
                                        C.c_void_p(scratch.data_ptr()), scratch.numel(),
                                        C.c_void_p(out["cand_offsets"].data_ptr()), C.c_void_p(out["cand_elem"].data_ptr()),
                                        C.c_void_p(out["cand_pid"].data_ptr()), C.c_void_p(out["cand_p4"].data_ptr()),

@@ -7,7 +7,7 @@ namespace mlpf {
 int64_t cand_scratch_bytes(int64_t N, int64_t E);
 // 2 kernels + one small H2D copy on `st`; returns the launch status
 cudaError_t launch_build_candidates(const float* X, int F, const int32_t* offsets_host, int E, const float* logits, int C,
-                                    const float* regress, void* scratch, int32_t* cand_offsets, int32_t* cand_elem,
+                                    const float* regress, const float* binary, void* scratch, int32_t* cand_offsets, int32_t* cand_elem,
                                     int32_t* cand_pid, float* cand_p4, cudaStream_t st);
 
 }  // namespace mlpf

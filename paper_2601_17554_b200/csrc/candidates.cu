@@ -1,6 +1,8 @@
 // candidates.cu -- candidate building: the step right after the encoder,
 // turning per-element outputs into the per-event particle list the experiment software consumes.
-//   PID = argmax of the logits (L130/L156; ties -> lowest class), kept iff type != 0 and PID != 0 (reading A23),
+//   PID = argmax of the logits (L130/L156; ties -> lowest class); an element yields a candidate iff it is not a pad row and
+//   its binary score is above 0.5, i.e. the binary head's logit b > 0 (the paper's rule, L156); for models without a
+//   binary head (binary == NULL): iff PID != 0 (departure A23),
 //   pT = pT_in exp(pT'), E = E_in exp(E')  (Eq. 2 inverted, L137-L139),  phi = atan2(sin phi, cos phi)  (L126),
 //   candidates in element order, grouped per event by integer offsets (bit-exact vs the oracle).
 // HBM / launch-latency bound (~90 algorithmic bytes per element): two small kernels, a stable stream
@@ -20,23 +22,28 @@ __device__ __forceinline__ void cand_stage_rows(const float* __restrict__ g, int
     for (int64_t i = threadIdx.x; i < n; i += CAND_BLOCK) s[i] = __ldg(src + i);
 }
 
-// code[i] = PID if element i yields a candidate, else 0; block_counts[b] = candidates in block b
+// code[i] = PID + 1 if element i yields a candidate, else 0; block_counts[b] = candidates in block b
 __global__ void __launch_bounds__(CAND_BLOCK)
-k_cand_count(const float* __restrict__ X, int F, const float* __restrict__ logits, int C, int64_t N,
-             uint8_t* __restrict__ code, int* __restrict__ block_counts) {
+k_cand_count(const float* __restrict__ X, int F, const float* __restrict__ logits, int C, const float* __restrict__ binary,
+             int64_t N, uint8_t* __restrict__ code, int* __restrict__ block_counts) {
     extern __shared__ float s_lg[];                        // [CAND_BLOCK, C]
     const int64_t row0 = (int64_t)blockIdx.x * CAND_BLOCK, i = row0 + threadIdx.x;
     cand_stage_rows(logits, row0, N, C, s_lg);
     __syncthreads();
-    int pid = 0;
+    int kept = 0;
     if (i < N) {
         const float* l = s_lg + threadIdx.x * C;           // stride C: conflict-free for odd C, 2-way at worst otherwise
         float best = l[0];
+        int pid = 0;
         for (int k = 1; k < C; ++k) { const float v = l[k]; if (v > best) { best = v; pid = k; } }
-        if ((int)__ldg(X + i * F) == 0) pid = 0;           // pad row (reading A2)
-        code[i] = (uint8_t)pid;
+        const float x0 = __ldg(X + i * F);
+        const bool pad = !(x0 >= 1.0f);                     // type id clamped to 0..4 as in a0 (reading A1/A2): < 1 or NaN -> pad row
+        // sigmoid(b) > 0.5  <=>  b > 0 (L156); without a binary head: class 0 = "no particle" (departure A23)
+        const bool keep = !pad && (binary ? __ldg(binary + i) > 0.0f : pid != 0);
+        kept = keep ? pid + 1 : 0;
+        code[i] = (uint8_t)kept;
     }
-    const int cnt = __syncthreads_count(pid != 0);
+    const int cnt = __syncthreads_count(kept != 0);
     if (threadIdx.x == 0) block_counts[blockIdx.x] = cnt;
 }
 
@@ -58,8 +65,9 @@ k_cand_emit(const float* __restrict__ X, int F, const float* __restrict__ regres
     for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
     if (lane == 0) s_base[warp] = part;
     cand_stage_rows(regress, row0, N, 5, s_rg);
-    const int pid = i < N ? code[i] : 0;
-    const unsigned m = __ballot_sync(0xffffffffu, pid != 0);
+    const int kept = i < N ? code[i] : 0;
+    const int pid = kept - 1;
+    const unsigned m = __ballot_sync(0xffffffffu, kept != 0);
     if (lane == 0) s_warp[warp] = __popc(m);
     __syncthreads();
     int before = 0, base = 0;
@@ -67,7 +75,7 @@ k_cand_emit(const float* __restrict__ X, int F, const float* __restrict__ regres
     for (int w = 0; w < CAND_BLOCK / 32; ++w) { before += w < warp ? s_warp[w] : 0; base += s_base[w]; }
     const int local = before + __popc(m & ((1u << lane) - 1u));
     s_rank[threadIdx.x] = local;
-    if (pid != 0) {
+    if (kept != 0) {
         const float* r = s_rg + threadIdx.x * 5;
         const float pt_in = __ldg(X + i * F + 1), e_in = __ldg(X + i * F + 4);
         const int c = base + local;
@@ -92,7 +100,7 @@ int64_t cand_scratch_bytes(int64_t N, int64_t E) {
 }
 
 cudaError_t launch_build_candidates(const float* X, int F, const int32_t* offsets_host, int E, const float* logits, int C,
-                                    const float* regress, void* scratch, int32_t* cand_offsets, int32_t* cand_elem,
+                                    const float* regress, const float* binary, void* scratch, int32_t* cand_offsets, int32_t* cand_elem,
                                     int32_t* cand_pid, float* cand_p4, cudaStream_t st) {
     const int64_t N = offsets_host[E];
     const int nb = (int)(N / CAND_BLOCK + 1);
@@ -103,7 +111,7 @@ cudaError_t launch_build_candidates(const float* X, int F, const int32_t* offset
     // pageable -> device async copies are staged by the runtime before returning: the caller may free offsets_host
     cudaError_t e = cudaMemcpyAsync(offsets, offsets_host, (size_t)(E + 1) * 4, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return e;
-    k_cand_count<<<nb, CAND_BLOCK, (size_t)CAND_BLOCK * C * 4, st>>>(X, F, logits, C, N, code, block_counts);
+    k_cand_count<<<nb, CAND_BLOCK, (size_t)CAND_BLOCK * C * 4, st>>>(X, F, logits, C, binary, N, code, block_counts);
     k_cand_emit<<<nb, CAND_BLOCK, 0, st>>>(X, F, regress, N, offsets, E, code, block_counts, cand_offsets, cand_elem,
                                            cand_pid, reinterpret_cast<float4*>(cand_p4));
     return cudaGetLastError();

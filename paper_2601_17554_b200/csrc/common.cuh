@@ -41,6 +41,9 @@ struct Epi {
     const int* row_perm = nullptr;
     const int* group_offsets = nullptr;
     int n_groups = 0;
+    // Uniform groups (two parallel encoders): group_rows > 0 (a multiple of 128) -> the M-tile starting at
+    // m0 uses weight / bias block m0 / group_rows of a weight matrix [G * N, K] and a bias [G * N].
+    int group_rows = 0;
 };
 
 __device__ __forceinline__ float warp_sum(float v) {

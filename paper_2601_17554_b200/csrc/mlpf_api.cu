@@ -64,17 +64,24 @@ struct Workspace {
     float *stage_x = nullptr, *stage_lg = nullptr, *stage_rg = nullptr;
     int64_t stage_cap = 0;            // rows
     // per-kernel-class CUDA-event timing of the last call (MLPF_OPT_PROFILE)
+    std::vector<int> host_work, host_pairs;   // host copies of the work lists of the last call
     std::vector<cudaEvent_t> ev_pool;
     std::vector<int> prof_cls;          // class of record i; events 2i, 2i+1
     // last call
     int64_t N = 0, E = 0, n_tiles = 0, n_pairs = 0, m_ub = 0, g_width = 0;
     bool h_tiled = false;             // layout of h after the last call: tiled between fused blocks (tc_post.cu)
+    // two-stack models: both encoders run as one batch over Mtot = (S - 1) Npad + N rows and Ev = S (E + 1) virtual events
+    int64_t Npad = 0, Mtot = 0, Ev = 0, n_tiles_real = 0;
     int tile_q = 128;
 };
 
 struct mlpf_handle {
     mlpf_blob_header hp;
     int d, H, hd, dff, F, C, R, n_out, L, n_hblk;
+    int S = 1;                        // encoder stacks (2 = the paper's parallel classification / regression encoders, L156)
+    int n_bin = 0;                    // 1: binary "valid" head (L156, Fig. 2)
+    int n_hblk0 = 0;                  // head blocks that read stack 0 (binary + PID); the rest read the last stack
+    int device = 0;
     int act;
     int64_t n_params = 0, n_packed = 0;
     float* P32 = nullptr;             // packed parameters, fp32
@@ -104,14 +111,16 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
     mlpf_blob_header hp;
     memcpy(&hp, blob, sizeof hp);
     if (memcmp(hp.magic, MLPF_BLOB_MAGIC, 8) != 0) { set_err(MLPF_E_BLOB, "bad magic"); return nullptr; }
-    if (hp.version != MLPF_BLOB_VERSION) { set_err(MLPF_E_BLOB, "unsupported version %u", hp.version); return nullptr; }
+    if (hp.version != 1u && hp.version != MLPF_BLOB_VERSION) { set_err(MLPF_E_BLOB, "unsupported version %u", hp.version); return nullptr; }
+    if (hp.version == 1u) { hp.n_stacks = 1; hp.binary_head = 0; }           // version 1: those header bytes are padding
     const int d = hp.d_model, H = hp.n_heads, dff = hp.d_ff, F = hp.n_feat, C = hp.n_classes, L = hp.n_layers;
     const int T = hp.n_types, K = hp.n_reg_heads;
-    if (L < 1 || L > 64 || d < 64 || d > 512 || d % 64 || H < 1 || d % H || dff < 64 || dff % 64 || dff > 4096 ||
+    const int S = hp.n_stacks == 0 ? 1 : (int)hp.n_stacks, NB = (int)hp.binary_head;
+    if (L < 1 || L > 64 || d < 64 || d > 512 || d % 64 || H < 1 || H > 64 || d % H || dff < 64 || dff % 64 || dff > 4096 ||
         F < 1 || F > 64 || T != 4 || C < 1 || C > 16 || K < 0 || K > MLPF_MAX_REG_HEADS || hp.activation > 1 ||
-        hp.final_ln > 1 || !(hp.ln_eps > 0.0f)) {
-        set_err(MLPF_E_BLOB, "unsupported hyper-parameters (L=%d d=%d H=%d dff=%d F=%d T=%d C=%d K=%d)", L, d, H,
-                dff, F, T, C, K);
+        hp.final_ln > 1 || !(hp.ln_eps > 0.0f) || S < 1 || S > 2 || NB < 0 || NB > 1) {
+        set_err(MLPF_E_BLOB, "unsupported hyper-parameters (L=%d d=%d H=%d dff=%d F=%d T=%d C=%d K=%d stacks=%d binary=%d)", L, d, H,
+                dff, F, T, C, K, S, NB);
         return nullptr;
     }
     const int hd = d / H;
@@ -121,12 +130,14 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
         if (hp.reg_dims[k] < 1 || hp.reg_dims[k] > 8) { set_err(MLPF_E_BLOB, "bad reg_dims"); return nullptr; }
         R += hp.reg_dims[k];
     }
-    if (C + R > MAX_OUT) { set_err(MLPF_E_BLOB, "too many outputs"); return nullptr; }
+    if (NB + C + R > MAX_OUT || NB + 1 + K > MAX_HBLK) { set_err(MLPF_E_BLOB, "too many outputs / heads"); return nullptr; }
     // ---- expected size
+    const int64_t layer_sz = 2 * d + 3LL * d * d + 3 * d + (int64_t)d * d + d + 2 * d + (int64_t)dff * d + dff + (int64_t)d * dff + d;
     int64_t np = 0;
     np += (int64_t)T * ((int64_t)d * F + d + (int64_t)d * d + d);
-    np += (int64_t)L * (2 * d + 3LL * d * d + 3 * d + (int64_t)d * d + d + 2 * d + (int64_t)dff * d + dff + (int64_t)d * dff + d);
-    np += 2 * d;
+    np += (int64_t)S * L * layer_sz;
+    np += (int64_t)S * 2 * d;
+    if (NB) np += (int64_t)d * d + d + d + 1;
     np += (int64_t)d * d + d + (int64_t)C * d + C;
     for (int k = 0; k < K; ++k) np += (int64_t)d * d + d + (int64_t)hp.reg_dims[k] * d + hp.reg_dims[k];
     if (blob_bytes != (size_t)(MLPF_HEADER_BYTES + np * 4)) {
@@ -140,11 +151,14 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
     }
     mlpf_handle* h = new (std::nothrow) mlpf_handle();
     if (!h) { set_err(MLPF_E_ALLOC, "host allocation failed"); return nullptr; }
+    cudaGetDevice(&h->device);
     h->hp = hp; h->d = d; h->H = H; h->hd = hd; h->dff = dff; h->F = F; h->C = C; h->R = R; h->L = L;
-    h->n_out = C + R; h->n_hblk = 1 + K; h->n_params = np;
+    h->S = S; h->n_bin = NB; h->n_out = NB + C + R; h->n_hblk = NB + 1 + K; h->n_hblk0 = NB + 1; h->n_params = np;
     h->act = hp.activation == 0 ? ACT_RELU : ACT_GELU;
 
-    // ---- repack into the layouts the kernels want
+    // ---- repack into the layouts the kernels want.  Blob order: embeddings; per stack, per layer, 12 tensors; per stack
+    // the final LN; heads.  Packed order: per layer and tensor kind the S stacks' copies are ADJACENT, so that a grouped
+    // launch addresses stack g's weights as row block g of one [S * out, in] matrix and its vectors as row g of [S, len].
     const float* src = (const float*)((const char*)blob + MLPF_HEADER_BYTES);
     std::vector<float> P;
     auto reserve = [&](int64_t n) { int64_t off = (int64_t)P.size(); P.resize(off + ((n + 63) / 64) * 64, 0.0f); return off; };
@@ -161,23 +175,34 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
         memcpy(&P[h->embW2 + (int64_t)t * d * d], src + s, (size_t)d * d * 4); s += (int64_t)d * d;
         memcpy(&P[h->embB2 + (int64_t)t * d], src + s, d * 4); s += d;
     }
-    auto take = [&](int64_t n) { int64_t off = reserve(n); memcpy(&P[off], src + s, (size_t)n * 4); s += n; return off; };
+    const int64_t enc0 = s;                               // blob offset of stack 0, layer 0
+    // one tensor of every stack, stacks adjacent: blob offset of stack st = first + st * stride
+    auto take_stacked = [&](int64_t first, int64_t stride, int64_t n) {
+        const int64_t off = reserve(n * S);               // every tensor size here is a multiple of 64: no gaps between stacks
+        for (int st = 0; st < S; ++st) memcpy(&P[off + st * n], src + first + st * stride, (size_t)n * 4);
+        return off;
+    };
     h->layers.resize(L);
+    const int64_t stack_stride = (int64_t)L * layer_sz;
     for (int l = 0; l < L; ++l) {
         LayerW& w = h->layers[l];
-        w.ln1g = take(d); w.ln1b = take(d); w.Wqkv = take(3LL * d * d); w.bqkv = take(3 * d);
-        w.Wo = take((int64_t)d * d); w.bo = take(d); w.ln2g = take(d); w.ln2b = take(d);
-        w.W1 = take((int64_t)dff * d); w.b1 = take(dff); w.W2 = take((int64_t)d * dff); w.b2 = take(d);
+        int64_t o = enc0 + (int64_t)l * layer_sz;
+        auto nx = [&](int64_t n) { const int64_t off = take_stacked(o, stack_stride, n); o += n; return off; };
+        w.ln1g = nx(d); w.ln1b = nx(d); w.Wqkv = nx(3LL * d * d); w.bqkv = nx(3 * d);
+        w.Wo = nx((int64_t)d * d); w.bo = nx(d); w.ln2g = nx(d); w.ln2b = nx(d);
+        w.W1 = nx((int64_t)dff * d); w.b1 = nx(dff); w.W2 = nx((int64_t)d * dff); w.b2 = nx(d);
     }
-    h->lnfg = take(d); h->lnfb = take(d);
+    s = enc0 + (int64_t)S * stack_stride;
+    h->lnfg = take_stacked(s, 2 * d, d); h->lnfb = take_stacked(s + d, 2 * d, d);
+    s += (int64_t)S * 2 * d;
     h->headW1 = reserve((int64_t)h->n_hblk * d * d);
     h->headB1 = reserve((int64_t)h->n_hblk * d);
     h->headW2 = reserve((int64_t)h->n_out * d);
     h->headB2 = reserve(h->n_out);
-    h->ho.n_out = h->n_out; h->ho.n_cls = C; h->ho.n_reg = R;
+    h->ho.n_out = h->n_out; h->ho.n_bin = NB; h->ho.n_cls = C; h->ho.n_reg = R;
     int o = 0;
-    for (int b = 0; b < h->n_hblk; ++b) {
-        int rk = (b == 0) ? C : (int)hp.reg_dims[b - 1];
+    for (int b = 0; b < h->n_hblk; ++b) {                 // blocks: [binary] PID reg.0 .. reg.K-1 (blob order)
+        int rk = (b < NB) ? 1 : (b == NB ? C : (int)hp.reg_dims[b - NB - 1]);
         memcpy(&P[h->headW1 + (int64_t)b * d * d], src + s, (size_t)d * d * 4); s += (int64_t)d * d;
         memcpy(&P[h->headB1 + (int64_t)b * d], src + s, d * 4); s += d;
         memcpy(&P[h->headW2 + (int64_t)o * d], src + s, (size_t)rk * d * 4); s += (int64_t)rk * d;
@@ -264,6 +289,8 @@ extern "C" int64_t mlpf_query(const mlpf_handle* h, int key) {
         case MLPF_Q_WEIGHT_BYTES: return h->n_packed * 6;
         case MLPF_Q_N_PARAMS: return h->n_params;
         case MLPF_Q_LAUNCHES: return h->last_launches;
+        case MLPF_Q_N_STACKS: return h->S;
+        case MLPF_Q_BINARY_HEAD: return h->n_bin;
         case MLPF_Q_WORKSPACE_BYTES: {
             int64_t b = 0;
             std::lock_guard<std::mutex> lk(const_cast<mlpf_handle*>(h)->mu);
@@ -301,8 +328,9 @@ static int64_t ws_bytes_events(const Workspace* w) {
 
 static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t n_tiles, bool fp32, cudaStream_t st) {
     const int64_t d = h->d;
-    if (N > w->cap_rows || fp32 != w->fp32) {
-        const int64_t cap = (std::max<int64_t>(N, w->cap_rows) + 127) / 128 * 128;
+    if (((N + 127) / 128 * 128) * h->S > w->cap_rows || fp32 != w->fp32) {
+        // rows: S stacks of N rounded up to 128 each (two-stack models run both encoders as one batch)
+        const int64_t cap = std::max<int64_t>(((N + 127) / 128 * 128) * h->S, w->cap_rows);
         ws_free_rows(w);                           // cudaFree waits for work in flight; every pointer is nulled
         w->bytes = ws_bytes_events(w);
         const int64_t es = fp32 ? 4 : 2;
@@ -329,6 +357,8 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
         // never-written tails hold finite values.  On the CALLER'S stream: the legacy default stream does not order
         // against non-blocking streams, so a plain cudaMemset could land after this call's kernels.
         cudaMemsetAsync(w->valid_bits, 0, (cap / 32 + 40) * 4, st);
+        cudaMemsetAsync(w->h, 0, cap * d * 4, st);
+        cudaMemsetAsync(w->valid, 0, cap * 4, st); cudaMemsetAsync(w->row_event, 0, cap * 4, st);
         cudaMemsetAsync(w->u, 0, cap * d * es, st); cudaMemsetAsync(w->qkv, 0, cap * 3 * d * es, st);
         cudaMemsetAsync(w->o, 0, cap * d * es, st);
         cudaMemsetAsync(w->g, 0, w->g_elems * es, st);
@@ -415,11 +445,11 @@ static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspa
     if (tc && !fp32) {
         int rc;
         if (h->attn == 0)
-            rc = tc_attn_launch(&h->tc, (const bf16*)w->qkv, w->N, w->valid_bits, w->n_valid, w->offsets,
+            rc = tc_attn_launch(&h->tc, (const bf16*)w->qkv, w->Mtot, w->valid_bits, w->n_valid, w->offsets,
                                 (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, (bf16*)w->o,
                                 split ? (bf16*)w->o_lo : nullptr, st);
         else {
-            rc = tc_attn2_launch(&h->tc, (const bf16*)w->qkv, w->N, (int)w->E, w->valid_bits, w->n_valid, w->offsets, w->row_event,
+            rc = tc_attn2_launch(&h->tc, (const bf16*)w->qkv, w->Mtot, (int)w->Ev, w->valid_bits, w->n_valid, w->offsets, w->row_event,
                                  (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, w->qn, w->kmax, (bf16*)w->o,
                                  split ? (bf16*)w->o_lo : nullptr, h->attn == 2, st);
             h->last_launches++;                       // the norms pre-pass
@@ -449,8 +479,11 @@ static void build_work_lists(const int32_t* off, int E, int tile_q, int rows_per
     }
 }
 
-static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, float* out_logits, float* out_regress, cudaStream_t st) {
+static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, float* out_logits, float* out_regress,
+                      float* out_binary, cudaStream_t st) {
     const int N = (int)w->N, E = (int)w->E, d = h->d, dff = h->dff;
+    const int S = h->S, Npad = (int)w->Npad, M = (int)w->Mtot;          // M rows cover all stacks (S = 1: M = N)
+    const int grp_rows = S > 1 ? Npad : 0;
     const bool tc_req = !fp32 && h->kernels == MLPF_KERNELS_TC;
     const bool tc = tc_req, tc_attn = tc_req;
     const int64_t es = fp32 ? 4 : 2;
@@ -489,6 +522,21 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         if (rc) return rc;
     }
     if (h->tap_layer == -2) return MLPF_OK;
+    for (int g1 = 1; g1 < S; ++g1) {       // the shared embedding feeds every encoder stack (L156): stack g1's rows + schedule
+        ProfScope ps(h, w, st, MLPF_KC_SCHED);
+        launch_sched_replicate(N, Npad, E, g1, d, w->offsets, w->n_valid, w->row_event, w->valid, w->valid_bits, w->h, st);
+        LAUNCH_CHECK(h);
+    }
+    // stand-alone LayerNorm of every stack's rows with that stack's gamma / beta (vectors are stacked [S, d])
+    auto layernorm_stacks = [&](int64_t g_off, int64_t b_off, void* out, void* out_lo) -> int {
+        for (int g1 = 0; g1 < S; ++g1) {
+            const int64_t r0 = (int64_t)g1 * Npad;
+            int rc = run_layernorm(h, fp32, w->h + r0 * d, N, PV + g_off + g1 * d, PV + b_off + g1 * d, (char*)out + r0 * d * es,
+                                   out_lo ? (char*)out_lo + r0 * d * es : nullptr, st);
+            if (rc) return rc;
+        }
+        return MLPF_OK;
+    };
 
     // ---- encoder blocks (pre-LN, L156 + A7)
     // Fused form (d <= 256, all activations split): per block QKV GEMM, attention, and ONE kernel for
@@ -502,15 +550,15 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         int rc;
         if (!u_ready) {
             ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);
-            rc = run_layernorm(h, fp32, w->h, N, PV + lw.ln1g, PV + lw.ln1b, u, nullptr, st);                     // a2
+            rc = layernorm_stacks(lw.ln1g, lw.ln1b, u, nullptr);                                                // a2
             if (rc) return rc;
         }
         u_ready = false;
         {   // a3: [Q K V] = LN1(x) Wqkv^T + bqkv
             ProfScope ps(h, w, st, MLPF_KC_QKV);
             Epi ep;
-            ep.bias = PV + lw.bqkv; ep.out_act = w->qkv; ep.ld_act = 3 * d;
-            rc = run_gemm(h, fp32, tc, u, nullptr, PW(lw.Wqkv), N, 3 * d, d, ep, st);
+            ep.bias = PV + lw.bqkv; ep.out_act = w->qkv; ep.ld_act = 3 * d; ep.group_rows = grp_rows; ep.n_groups = S;
+            rc = run_gemm(h, fp32, tc, u, nullptr, PW(lw.Wqkv), M, 3 * d, d, ep, st);
             if (rc) return rc;
         }
         {
@@ -522,7 +570,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
             ProfScope ps(h, w, st, MLPF_KC_POST);
             const bool last = l + 1 == h->L, tap = h->tap_layer == l;
             PostArgs a;
-            a.M = N; a.d = d; a.dff = dff; a.act = h->act;
+            a.M = M; a.d = d; a.dff = dff; a.act = h->act; a.n_groups = S; a.group_rows = grp_rows;
             a.o = (const bf16*)w->o; a.o_lo = (const bf16*)w->o_lo;
             a.Wo = (const bf16*)PW(lw.Wo); a.W1 = (const bf16*)PW(lw.W1); a.W2 = (const bf16*)PW(lw.W2);
             a.bo = PV + lw.bo; a.ln2g = PV + lw.ln2g; a.ln2b = PV + lw.ln2b; a.b1 = PV + lw.b1; a.b2 = PV + lw.b2;
@@ -548,26 +596,29 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
             ProfScope ps(h, w, st, MLPF_KC_OUTPROJ);
             Epi ep;
             ep.bias = PV + lw.bo; ep.residual = w->h; ep.ld_res = d; ep.out_f32 = w->h; ep.ld_f32 = d;
-            rc = run_gemm(h, fp32, tc, w->o, lo(MLPF_SPLIT_O, w->o_lo), PW(lw.Wo), N, d, d, ep, st);
+            ep.group_rows = grp_rows; ep.n_groups = S;
+            rc = run_gemm(h, fp32, tc, w->o, lo(MLPF_SPLIT_O, w->o_lo), PW(lw.Wo), M, d, d, ep, st);
             if (rc) return rc;
         }
         {
             ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);
-            rc = run_layernorm(h, fp32, w->h, N, PV + lw.ln2g, PV + lw.ln2b, u, lo(MLPF_SPLIT_U2, w->u_lo), st);
+            rc = layernorm_stacks(lw.ln2g, lw.ln2b, u, lo(MLPF_SPLIT_U2, w->u_lo));
         }
         if (rc) return rc;
         {   // a6: g = act(LN2(h) W1^T + b1)
             ProfScope ps(h, w, st, MLPF_KC_FFN1);
             Epi ep;
             ep.bias = PV + lw.b1; ep.act = h->act; ep.out_act = g; ep.out_act_lo = lo(MLPF_SPLIT_G, w->g_lo); ep.ld_act = dff;
-            rc = run_gemm(h, fp32, tc, u, lo(MLPF_SPLIT_U2, w->u_lo), PW(lw.W1), N, dff, d, ep, st);
+            ep.group_rows = grp_rows; ep.n_groups = S;
+            rc = run_gemm(h, fp32, tc, u, lo(MLPF_SPLIT_U2, w->u_lo), PW(lw.W1), M, dff, d, ep, st);
             if (rc) return rc;
         }
         {   // a7: h <- h + g W2^T + b2
             ProfScope ps(h, w, st, MLPF_KC_FFN2);
             Epi ep;
             ep.bias = PV + lw.b2; ep.residual = w->h; ep.ld_res = d; ep.out_f32 = w->h; ep.ld_f32 = d;
-            rc = run_gemm(h, fp32, tc, g, lo(MLPF_SPLIT_G, w->g_lo), PW(lw.W2), N, d, dff, ep, st);
+            ep.group_rows = grp_rows; ep.n_groups = S;
+            rc = run_gemm(h, fp32, tc, g, lo(MLPF_SPLIT_G, w->g_lo), PW(lw.W2), M, d, dff, ep, st);
             if (rc) return rc;
         }
         w->g_width = dff;
@@ -579,33 +630,45 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         // the last block's fused epilogue already wrote u = LN_f(h) (or T(h)) as hi + lo
     } else if (h->hp.final_ln) {
         ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);
-        int rc = run_layernorm(h, fp32, w->h, N, PV + h->lnfg, PV + h->lnfb, u, lo(MLPF_SPLIT_UF, w->u_lo), st);
+        int rc = layernorm_stacks(h->lnfg, h->lnfb, u, lo(MLPF_SPLIT_UF, w->u_lo));
         if (rc) return rc;
     } else {
         ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);           // no final LN: u = T(h) (+ lo)
-        launch_cast_rows(fp32, w->h, (int64_t)N * d, u, lo(MLPF_SPLIT_UF, w->u_lo), st);
+        launch_cast_rows(fp32, w->h, (int64_t)M * d, u, lo(MLPF_SPLIT_UF, w->u_lo), st);
         LAUNCH_CHECK(h);
     }
     {
-        Epi ep;
+        // first layers of all heads: hidden block b = act(z W1[b]^T + b1[b]); the binary and PID blocks read the classification
+        // stack's z (rows 0 .. N-1), the regression blocks the regression stack's (rows (S-1) Npad ..), L156
         const int hw = h->n_hblk * d;
-        ep.bias = PV + h->headB1; ep.act = h->act; ep.out_act = g; ep.out_act_lo = lo(MLPF_SPLIT_HEAD, w->g_lo); ep.ld_act = hw;
-        int rc;
+        int rc = MLPF_OK;
         {
             ProfScope ps(h, w, st, MLPF_KC_HEADS_L1);
-            rc = run_gemm(h, fp32, tc, u, lo(MLPF_SPLIT_UF, w->u_lo), PW(h->headW1), N, hw, d, ep, st);
+            const int nb0 = S > 1 ? h->n_hblk0 : h->n_hblk;
+            for (int part = 0; part < (S > 1 ? 2 : 1) && rc == MLPF_OK; ++part) {
+                const int b0 = part == 0 ? 0 : nb0, nb = part == 0 ? nb0 : h->n_hblk - nb0;
+                if (nb == 0) continue;
+                const int64_t r0 = part == 0 ? 0 : (int64_t)(S - 1) * Npad;
+                Epi ep;
+                ep.bias = PV + h->headB1 + (int64_t)b0 * d; ep.act = h->act; ep.ld_act = hw;
+                ep.out_act = (char*)g + (int64_t)b0 * d * es;
+                ep.out_act_lo = lo(MLPF_SPLIT_HEAD, w->g_lo) ? (char*)w->g_lo + (int64_t)b0 * d * es : nullptr;
+                rc = run_gemm(h, fp32, tc, (char*)u + r0 * d * es, lo(MLPF_SPLIT_UF, w->u_lo) ? (char*)w->u_lo + r0 * d * es : nullptr,
+                              PW(h->headW1 + (int64_t)b0 * d * d), N, nb * d, d, ep, st);
+            }
         }
         if (rc) return rc;
         w->g_width = hw;
         ProfScope ps(h, w, st, MLPF_KC_HEADS_L2);
-        launch_heads_l2(fp32, g, lo(MLPF_SPLIT_HEAD, w->g_lo), N, d, hw, PV + h->headW2, PV + h->headB2, w->valid, h->ho, out_logits, out_regress, st);
+        launch_heads_l2(fp32, g, lo(MLPF_SPLIT_HEAD, w->g_lo), N, d, hw, PV + h->headW2, PV + h->headB2, w->valid, h->ho, out_logits,
+                        out_regress, out_binary, st);
         LAUNCH_CHECK(h);
     }
     return MLPF_OK;
 }
 
-extern "C" int mlpf_infer(mlpf_handle* h, const float* elements, const int32_t* event_offsets, int32_t n_events,
-                          float* out_logits, float* out_regress, void* stream) {
+extern "C" int mlpf_infer_ex(mlpf_handle* h, const float* elements, const int32_t* event_offsets, int32_t n_events,
+                             float* out_logits, float* out_regress, float* out_binary, void* stream) {
     if (!h) return set_err(MLPF_E_NULL, "handle is NULL");
     if (n_events < 0) return set_err(MLPF_E_OFFSETS, "n_events < 0");
     if (n_events == 0) return MLPF_OK;
@@ -616,28 +679,48 @@ extern "C" int mlpf_infer(mlpf_handle* h, const float* elements, const int32_t* 
     const int64_t N = event_offsets[n_events];
     if (N == 0) return MLPF_OK;
     if (!elements || !out_logits || !out_regress) return set_err(MLPF_E_NULL, "elements / outputs NULL");
+    if (out_binary && !h->n_bin) return set_err(MLPF_E_ARG, "out_binary given but the model has no binary head");
     cudaStream_t st = (cudaStream_t)stream;
+    const int S = h->S;
+    if ((int64_t)S * ((N + 127) / 128 * 128) > 0x7fffff00LL) return set_err(MLPF_E_ARG, "too many rows");
 
     std::unique_lock<std::mutex> lk(h->mu);
     const bool fp32 = h->precision == MLPF_PREC_FP32_DEBUG;
     Workspace*& wref = h->ws[stream];
     if (!wref) wref = new Workspace();
     Workspace* w = wref;
-    std::vector<int> work, pairs;
+    std::vector<int>& work = w->host_work; std::vector<int>& pairs = w->host_pairs;
     build_work_lists(event_offsets, n_events, h->tile_q, tc_attn_rows_per_cta(h->hd), work, pairs);
-    int rc = ws_ensure(h, w, N, n_events, (int64_t)work.size() / 2, fp32, st);
+    const int64_t n_tiles_real = (int64_t)work.size() / 2;
+    if (S > 1) {                           // the second encoder's events are the virtual events (E + 1) + e
+        const size_t nw = work.size(), npz = pairs.size();
+        for (int g1 = 1; g1 < S; ++g1) {
+            for (size_t i = 0; i < nw; i += 2) { work.push_back(work[i] + g1 * (n_events + 1)); work.push_back(work[i + 1]); }
+            for (size_t i = 0; i < npz; i += 2) { pairs.push_back(pairs[i] + g1 * (n_events + 1)); pairs.push_back(pairs[i + 1]); }
+        }
+    }
+    const int64_t Ev = S > 1 ? (int64_t)S * (n_events + 1) : n_events;
+    int rc = ws_ensure(h, w, N, Ev, (int64_t)work.size() / 2, fp32, st);
     if (rc) return rc;
     w->N = N; w->E = n_events; w->n_tiles = (int64_t)work.size() / 2; w->n_pairs = (int64_t)pairs.size() / 2;
+    w->n_tiles_real = n_tiles_real;
+    w->Npad = (N + 127) / 128 * 128; w->Mtot = (int64_t)(S - 1) * w->Npad + N; w->Ev = Ev;
     w->tile_q = h->tile_q;
     w->m_ub = (N + 127) / 128 * 128 + 4 * 128;
     h->last_launches = 0;
-    // pageable -> device async copies are staged by the runtime before returning: the caller may free
+    // pageable -> device async copies are staged by the runtime before returning: the caller may free event_offsets;
+    // the work lists live in the workspace (the copies may still be reading them after this call returns on other paths)
     CUDA_TRY(cudaMemcpyAsync(w->offsets, event_offsets, (size_t)(n_events + 1) * 4, cudaMemcpyHostToDevice, st));
     if (!work.empty()) CUDA_TRY(cudaMemcpyAsync(w->work, work.data(), work.size() * 4, cudaMemcpyHostToDevice, st));
     if (!pairs.empty()) CUDA_TRY(cudaMemcpyAsync(w->pairs, pairs.data(), pairs.size() * 4, cudaMemcpyHostToDevice, st));
-    rc = infer_impl(h, fp32, w, elements, out_logits, out_regress, st);
+    rc = infer_impl(h, fp32, w, elements, out_logits, out_regress, out_binary, st);
     if (rc == MLPF_OK) g_err.clear();
     return rc;
+}
+
+extern "C" int mlpf_infer(mlpf_handle* h, const float* elements, const int32_t* event_offsets, int32_t n_events,
+                          float* out_logits, float* out_regress, void* stream) {
+    return mlpf_infer_ex(h, elements, event_offsets, n_events, out_logits, out_regress, nullptr, stream);
 }
 
 extern "C" int mlpf_infer_host(mlpf_handle* h, const float* elements_host, const int32_t* event_offsets,
@@ -683,10 +766,10 @@ extern "C" int64_t mlpf_candidates_scratch_bytes(int64_t n_elements, int32_t n_e
     return cand_scratch_bytes(n_elements, n_events);
 }
 
-extern "C" int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* event_offsets, int32_t n_events,
-                                     const float* logits, int32_t n_classes, const float* regress, void* scratch,
-                                     int64_t scratch_bytes, int32_t* cand_offsets, int32_t* cand_elem, int32_t* cand_pid,
-                                     float* cand_p4, void* stream) {
+extern "C" int mlpf_build_candidates_ex(const float* elements, int32_t n_feat, const int32_t* event_offsets, int32_t n_events,
+                                        const float* logits, int32_t n_classes, const float* regress, int32_t n_regress,
+                                        const float* binary, void* scratch, int64_t scratch_bytes, int32_t* cand_offsets,
+                                        int32_t* cand_elem, int32_t* cand_pid, float* cand_p4, void* stream) {
     if (n_events < 0) return set_err(MLPF_E_OFFSETS, "n_events < 0");
     if (n_events == 0) return MLPF_OK;
     if (!event_offsets) return set_err(MLPF_E_NULL, "event_offsets is NULL");
@@ -694,17 +777,26 @@ extern "C" int mlpf_build_candidates(const float* elements, int32_t n_feat, cons
     for (int e = 0; e < n_events; ++e)
         if (event_offsets[e + 1] < event_offsets[e]) return set_err(MLPF_E_OFFSETS, "event_offsets decreasing at %d", e);
     const int64_t N = event_offsets[n_events];
-    if (n_feat < 5 || n_classes < 1 || n_classes > 64) return set_err(MLPF_E_ARG, "n_feat = %d (>= 5), n_classes = %d (1..64)", n_feat, n_classes);
+    if (n_feat < 5 || n_classes < 1 || n_classes > 48) return set_err(MLPF_E_ARG, "n_feat = %d (>= 5), n_classes = %d (1..48)", n_feat, n_classes);
+    if (n_regress != 5) return set_err(MLPF_E_ARG, "n_regress = %d: the decode needs (pT', eta, sin phi, cos phi, E')", n_regress);
     if (!scratch || !cand_offsets) return set_err(MLPF_E_NULL, "scratch / cand_offsets NULL");
     if (N > 0 && (!elements || !logits || !regress || !cand_elem || !cand_pid || !cand_p4)) return set_err(MLPF_E_NULL, "inputs / outputs NULL");
     if (scratch_bytes < cand_scratch_bytes(N, n_events))
         return set_err(MLPF_E_ARG, "scratch_bytes %lld < %lld", (long long)scratch_bytes, (long long)cand_scratch_bytes(N, n_events));
     if (((uintptr_t)cand_p4 & 15) || ((uintptr_t)scratch & 255)) return set_err(MLPF_E_ARG, "cand_p4 must be 16-byte, scratch 256-byte aligned");
-    cudaError_t e = launch_build_candidates(elements, n_feat, event_offsets, n_events, logits, n_classes, regress, scratch,
+    cudaError_t e = launch_build_candidates(elements, n_feat, event_offsets, n_events, logits, n_classes, regress, binary, scratch,
                                             cand_offsets, cand_elem, cand_pid, cand_p4, (cudaStream_t)stream);
     if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "candidate kernels: %s", cudaGetErrorString(e));
     g_err.clear();
     return MLPF_OK;
+}
+
+extern "C" int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* event_offsets, int32_t n_events,
+                                     const float* logits, int32_t n_classes, const float* regress, void* scratch,
+                                     int64_t scratch_bytes, int32_t* cand_offsets, int32_t* cand_elem, int32_t* cand_pid,
+                                     float* cand_p4, void* stream) {
+    return mlpf_build_candidates_ex(elements, n_feat, event_offsets, n_events, logits, n_classes, regress, 5, nullptr, scratch,
+                                    scratch_bytes, cand_offsets, cand_elem, cand_pid, cand_p4, stream);
 }
 
 // ------------------------------------------------------------------------------------------------ debug taps
@@ -727,7 +819,7 @@ extern "C" int64_t mlpf_debug_get_schedule(mlpf_handle* h, void* stream, int whi
         case MLPF_SCHED_TYPE_PERM:
             CUDA_TRY(cudaMemcpy(toff, w->type_offsets, 6 * 4, cudaMemcpyDeviceToHost));
             src = w->type_perm; n = toff[5]; break;
-        case MLPF_SCHED_WORK_LIST: src = w->work; n = w->n_tiles * 2; break;
+        case MLPF_SCHED_WORK_LIST: src = w->work; n = w->n_tiles_real * 2; break;
         default: return set_err(MLPF_E_ARG, "unknown schedule array %d", which);
     }
     if (n > capacity) return set_err(MLPF_E_ARG, "capacity %lld < %lld", (long long)capacity, (long long)n);

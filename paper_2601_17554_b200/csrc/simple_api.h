@@ -8,8 +8,9 @@ namespace mlpf {
 constexpr int SCHED_BLOCK = 1024;
 constexpr int EMB_ROWS = 64;
 constexpr int MAX_OUT = 24;
+constexpr int MAX_HBLK = 6;        // head blocks: [binary] + PID + up to 4 regression heads (L156: "six two-layer FFN heads")
 struct HeadsOut {
-    int n_out; int n_cls; int n_reg;
+    int n_out; int n_bin; int n_cls; int n_reg;     // outputs in this order: binary (0 | 1), class logits, regressions
     int blk[MAX_OUT];
 };
 
@@ -28,7 +29,9 @@ void launch_attn_simple(bool fp32, int hd, const void* QKV, const int* key_valid
                         void* O_lo, cudaStream_t st);
 void launch_heads_l2(bool fp32, const void* hidden, const void* hidden_lo, int N, int d, int ld_hidden,
                      const float* W2, const float* b2, const int* valid, const HeadsOut& ho, float* out_logits,
-                     float* out_regress, cudaStream_t st);
+                     float* out_regress, float* out_binary, cudaStream_t st);
+void launch_sched_replicate(int N, int N_pad, int E, int g, int d, int* offsets, int* n_valid, int* row_event, int* valid,
+                            uint32_t* valid_bits, float* h, cudaStream_t st);
 // bits[i / 32] bit (i % 32) = valid[i] != 0; `bits` holds (N + 31) / 32 words (+ 3 zero words for the attention kernel)
 void launch_pack_valid_bits(const int* valid, int N, uint32_t* bits, cudaStream_t st);
 void launch_cast_rows(bool fp32, const float* h, int64_t n, void* u, void* u_lo, cudaStream_t st);

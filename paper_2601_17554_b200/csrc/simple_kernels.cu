@@ -303,7 +303,7 @@ k_gemm_simple(const T* __restrict__ A, const T* __restrict__ A_lo, const T* __re
         if (m0 >= ep.group_offsets[ep.n_groups + 1]) return;
         while (g < ep.n_groups && m0 >= ep.group_offsets[g + 1]) ++g;
         w_row0 = (int64_t)(g - 1) * N;
-    }
+    } else if (ep.group_rows > 0) w_row0 = (int64_t)(m0 / ep.group_rows) * N;
     const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
     float acc[4][4] = {};
     const int lr = threadIdx.x >> 2, lk = (threadIdx.x & 3) * 4;   // 64 rows x 16 k, 4 k per thread
@@ -438,11 +438,19 @@ k_attn_simple(const T* __restrict__ QKV, const int* __restrict__ key_valid, cons
 // hidden block blk[o].  Outputs 0..C-1 -> logits, C.. -> regress.
 // ------------------------------------------------------------------------------------------------
 
+// output o of a row: [binary (n_bin = 0 | 1)] [class logits (n_cls)] [regressions (n_reg)]  (L156 / Fig. 2)
+__device__ __forceinline__ void heads_store(const HeadsOut& ho, int row, int o, float a, float* __restrict__ out_logits,
+                                            float* __restrict__ out_regress, float* __restrict__ out_binary) {
+    if (o < ho.n_bin) { if (out_binary) out_binary[row] = a; }
+    else if (o < ho.n_bin + ho.n_cls) out_logits[(int64_t)row * ho.n_cls + (o - ho.n_bin)] = a;
+    else out_regress[(int64_t)row * ho.n_reg + (o - ho.n_bin - ho.n_cls)] = a;
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256)
 k_heads_l2(const T* __restrict__ hidden, const T* __restrict__ hidden_lo, int N, int d, int ld_hidden, const float* __restrict__ W2,
            const float* __restrict__ b2, const int* __restrict__ valid, HeadsOut ho,
-           float* __restrict__ out_logits, float* __restrict__ out_regress) {
+           float* __restrict__ out_logits, float* __restrict__ out_regress, float* __restrict__ out_binary) {
     int row = blockIdx.x * 8 + (threadIdx.x >> 5);
     int lane = threadIdx.x & 31;
     if (row >= N) return;
@@ -461,10 +469,7 @@ k_heads_l2(const T* __restrict__ hidden, const T* __restrict__ hidden_lo, int N,
             }
             a = warp_sum(a) + b2[o];
         }
-        if (lane == 0) {
-            if (o < ho.n_cls) out_logits[(int64_t)row * ho.n_cls + o] = a;
-            else out_regress[(int64_t)row * ho.n_reg + (o - ho.n_cls)] = a;
-        }
+        if (lane == 0) heads_store(ho, row, o, a, out_logits, out_regress, out_binary);
     }
 }
 
@@ -475,14 +480,14 @@ template <int NCH>
 __global__ void __launch_bounds__(256)
 k_heads_l2_vec(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden_lo, int N, int d, int ld_hidden, int n_blk,
                const float* __restrict__ W2, const float* __restrict__ b2, const int* __restrict__ valid, HeadsOut ho,
-               float* __restrict__ out_logits, float* __restrict__ out_regress) {
+               float* __restrict__ out_logits, float* __restrict__ out_regress, float* __restrict__ out_binary) {
     const int row = blockIdx.x * 8 + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     if (row >= N) return;
     const bool ok = valid[row] != 0;
-    uint4 hraw[5][NCH], lraw[5][NCH];
+    uint4 hraw[MAX_HBLK][NCH], lraw[MAX_HBLK][NCH];
 #pragma unroll
-    for (int b = 0; b < 5; ++b)
+    for (int b = 0; b < MAX_HBLK; ++b)
 #pragma unroll
         for (int ch = 0; ch < NCH; ++ch) {
             const int c = ch * 256 + lane * 8;
@@ -503,7 +508,7 @@ k_heads_l2_vec(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden_
                 if (c < d) {
                     uint4 h4 = hraw[0][ch], l4 = lraw[0][ch];
 #pragma unroll
-                    for (int bb = 1; bb < 5; ++bb) if (b == bb) { h4 = hraw[bb][ch]; l4 = lraw[bb][ch]; }
+                    for (int bb = 1; bb < MAX_HBLK; ++bb) if (b == bb) { h4 = hraw[bb][ch]; l4 = lraw[bb][ch]; }
                     const uint32_t hw[4] = {h4.x, h4.y, h4.z, h4.w}, lw[4] = {l4.x, l4.y, l4.z, l4.w};
                     const float4* wp = reinterpret_cast<const float4*>(W2 + (int64_t)o * d + c);
                     const float4 w0 = __ldg(wp), w1 = __ldg(wp + 1);
@@ -517,10 +522,7 @@ k_heads_l2_vec(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden_
             }
             a = warp_sum(a) + b2[o];
         }
-        if (lane == 0) {
-            if (o < ho.n_cls) out_logits[(int64_t)row * ho.n_cls + o] = a;
-            else out_regress[(int64_t)row * ho.n_reg + (o - ho.n_cls)] = a;
-        }
+        if (lane == 0) heads_store(ho, row, o, a, out_logits, out_regress, out_binary);
     }
 }
 
@@ -549,7 +551,7 @@ template <int NCH>
 __global__ void __launch_bounds__(256)
 k_heads_l2_fold(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden_lo, int N, int d, int ld_hidden, int n_blk,
                 const float* __restrict__ W2, const float* __restrict__ b2, const int* __restrict__ valid, HeadsOut ho,
-                float* __restrict__ out_logits, float* __restrict__ out_regress) {
+                float* __restrict__ out_logits, float* __restrict__ out_regress, float* __restrict__ out_binary) {
     const int row = blockIdx.x * 8 + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     if (row >= N) return;
@@ -558,9 +560,9 @@ k_heads_l2_fold(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden
 #pragma unroll
     for (int o = 0; o < 16; ++o) acc[o] = 0.0f;
     if (ok) {
-        float hv[5][NCH][8];
+        float hv[MAX_HBLK][NCH][8];
 #pragma unroll
-        for (int b = 0; b < 5; ++b)
+        for (int b = 0; b < MAX_HBLK; ++b)
 #pragma unroll
             for (int ch = 0; ch < NCH; ++ch) {
                 const int c = ch * 256 + lane * 8;
@@ -592,7 +594,8 @@ k_heads_l2_fold(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden
                             case 1: acc[o] = heads_dot8(hv[1][ch], w0, w1, acc[o]); break;
                             case 2: acc[o] = heads_dot8(hv[2][ch], w0, w1, acc[o]); break;
                             case 3: acc[o] = heads_dot8(hv[3][ch], w0, w1, acc[o]); break;
-                            default: acc[o] = heads_dot8(hv[4][ch], w0, w1, acc[o]); break;
+                            case 4: acc[o] = heads_dot8(hv[4][ch], w0, w1, acc[o]); break;
+                            default: acc[o] = heads_dot8(hv[5][ch], w0, w1, acc[o]); break;
                         }
                     }
                 }
@@ -607,8 +610,7 @@ k_heads_l2_fold(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden
     const int o = lane >> 1;
     if ((lane & 1) == 0 && o < ho.n_out) {
         const float a = ok ? acc[0] + b2[o] : 0.0f;
-        if (o < ho.n_cls) out_logits[(int64_t)row * ho.n_cls + o] = a;
-        else out_regress[(int64_t)row * ho.n_reg + (o - ho.n_cls)] = a;
+        heads_store(ho, row, o, a, out_logits, out_regress, out_binary);
     }
 }
 
@@ -654,6 +656,30 @@ __global__ void k_untile_h(const float* __restrict__ ht, float* __restrict__ out
 }
 void launch_untile_h(const float* ht, float* out, int64_t N, int d, cudaStream_t st) {
     k_untile_h<<<(unsigned)((N * d + 255) / 256), 256, 0, st>>>(ht, out, N, d);
+}
+
+// Two parallel encoders run as ONE batch over 2 N_pad rows: stack g owns rows [g N_pad, g N_pad + N)
+// (N_pad = N rounded up to 128) and the virtual events g (E + 1) .. g (E + 1) + E - 1; virtual event g (E + 1) + E is the
+// gap [g N_pad + N, (g + 1) N_pad), which no work item touches.  This kernel copies the schedule arrays the per-row
+// kernels read (and the embedded residual stream) from stack 0's rows to stack g's (g >= 1).
+__global__ void k_sched_replicate(int N, int N_pad, int E, int g, int d, int* __restrict__ offsets, int* __restrict__ n_valid,
+                                  int* __restrict__ row_event, int* __restrict__ valid, uint32_t* __restrict__ valid_bits,
+                                  float* __restrict__ h) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t base = (int64_t)g * N_pad;
+    const int Ev = E + 1;
+    if (i < N) { row_event[base + i] = row_event[i] + g * Ev; valid[base + i] = valid[i]; }
+    if (i < N_pad - N) { row_event[base - N_pad + N + i] = (g - 1) * Ev + E; valid[base - N_pad + N + i] = 0; }   // the gap before this stack
+    if (i < N_pad / 32) valid_bits[base / 32 + i] = (i * 32 < N) ? valid_bits[i] : 0u;
+    if (i < E) n_valid[g * Ev + i] = n_valid[i];
+    if (i <= E) offsets[g * Ev + i] = (int)base + offsets[i];
+    if (i == 0) { offsets[(g + 1) * Ev] = (int)base + N_pad; n_valid[g * Ev + E] = 0; n_valid[(g - 1) * Ev + E] = 0; }
+    if (i < (int64_t)N * d / 4) reinterpret_cast<float4*>(h + base * d)[i] = reinterpret_cast<const float4*>(h)[i];
+}
+void launch_sched_replicate(int N, int N_pad, int E, int g, int d, int* offsets, int* n_valid, int* row_event, int* valid,
+                            uint32_t* valid_bits, float* h, cudaStream_t st) {
+    const int64_t n = (int64_t)N * d / 4;
+    k_sched_replicate<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(N, N_pad, E, g, d, offsets, n_valid, row_event, valid, valid_bits, h);
 }
 
 // ------------------------------------------------------------------------------------------------ launchers
@@ -731,19 +757,19 @@ void launch_attn_simple(bool fp32, int hd, const void* QKV, const int* key_valid
 
 void launch_heads_l2(bool fp32, const void* hidden, const void* hidden_lo, int N, int d, int ld_hidden,
                      const float* W2, const float* b2, const int* valid, const HeadsOut& ho, float* out_logits,
-                     float* out_regress, cudaStream_t st) {
+                     float* out_regress, float* out_binary, cudaStream_t st) {
     dim3 grid((N + 7) / 8);
-    if (fp32) k_heads_l2<float><<<grid, 256, 0, st>>>((const float*)hidden, (const float*)hidden_lo, N, d, ld_hidden, W2, b2, valid, ho, out_logits, out_regress);
-    else if (d <= 512 && d % 8 == 0 && ld_hidden % 8 == 0 && ld_hidden / d <= 5) {
+    if (fp32) k_heads_l2<float><<<grid, 256, 0, st>>>((const float*)hidden, (const float*)hidden_lo, N, d, ld_hidden, W2, b2, valid, ho, out_logits, out_regress, out_binary);
+    else if (d <= 512 && d % 8 == 0 && ld_hidden % 8 == 0 && ld_hidden / d <= MAX_HBLK) {
         const int n_blk = ld_hidden / d;
         if (ho.n_out <= 16) {
-            if (d <= 256) k_heads_l2_fold<1><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress);
-            else k_heads_l2_fold<2><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress);
+            if (d <= 256) k_heads_l2_fold<1><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress, out_binary);
+            else k_heads_l2_fold<2><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress, out_binary);
         }
-        else if (d <= 256) k_heads_l2_vec<1><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress);
-        else k_heads_l2_vec<2><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress);
+        else if (d <= 256) k_heads_l2_vec<1><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress, out_binary);
+        else k_heads_l2_vec<2><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress, out_binary);
     }
-    else k_heads_l2<bf16><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, W2, b2, valid, ho, out_logits, out_regress);
+    else k_heads_l2<bf16><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, W2, b2, valid, ho, out_logits, out_regress, out_binary);
 }
 
 void launch_to_f32(bool fp32, const void* src, float* dst, int64_t n, cudaStream_t st) {

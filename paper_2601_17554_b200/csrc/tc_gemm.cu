@@ -223,7 +223,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 int g = 1;
                 while (g < ep.n_groups && m0 >= ep.group_offsets[g + 1]) ++g;
                 w_row0 = (g - 1) * N;
-            }
+            } else if (ep.group_rows > 0) w_row0 = (m0 / ep.group_rows) * N;   // one weight block per encoder stack
             for (int kb = 0; kb < num_kb; ++kb, ++kbg) {
                 const uint32_t s = kbg % STAGES;
                 ptx::mbar_wait(bar_empty + 8 * s, ((kbg / STAGES) & 1) ^ 1);
@@ -284,7 +284,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 int g = 1;
                 while (g < ep.n_groups && m0 >= ep.group_offsets[g + 1]) ++g;
                 w_row0 = (g - 1) * N;
-            }
+            } else if (ep.group_rows > 0) w_row0 = (m0 / ep.group_rows) * N;
             // this tile's bias -> shared memory (read back as broadcast 128-bit loads)
             asm volatile("bar.sync %0, 256;" ::"r"(1 + e) : "memory");          // everyone is done with the last tile's
             if (ep.bias)
@@ -366,7 +366,7 @@ int tc_gemm_launch(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W,
         snprintf(c->err, sizeof c->err, "tc_gemm: the epilogue writes either fp32 (+ residual) or bf16 hi (+ lo)"); return -1;
     }
     if (N % 64 || K % 64) { snprintf(c->err, sizeof c->err, "tc_gemm: N=%d, K=%d must be multiples of 64", N, K); return -1; }
-    const int w_rows = ep.group_offsets ? ep.n_groups * N : N;
+    const int w_rows = (ep.group_offsets || ep.group_rows > 0) ? ep.n_groups * N : N;
     if (N % 128 == 0) {
         return A_lo ? tc_gemm_launch_cfg<128, 3, true>(c, A, A_lo, W, M, N, K, w_rows, ep, st)
                     : tc_gemm_launch_cfg<128, 4, false>(c, A, nullptr, W, M, N, K, w_rows, ep, st);

@@ -36,7 +36,11 @@ def test_header_struct_matches_blob_writer():
     assert len(blob) == 256 + 4 * synth.param_count(m)
     assert blob[:8] == b"MLPFBLOB"
     f = struct.unpack_from("<9I", blob, 8)
-    assert f == (1, m.n_layers, m.d_model, m.n_heads, m.d_ff, 55, 4, 9, 4)
+    assert f == (2, m.n_layers, m.d_model, m.n_heads, m.d_ff, 55, 4, 9, 4)
+    assert struct.unpack_from("<2I", blob, 72) == (1, 0)                       # n_stacks, binary_head
+    m2 = synth.model_cfg("paper2")
+    blob2 = P.pack_blob(synth.make_weights("paper2"), m2)
+    assert len(blob2) == 256 + 4 * synth.param_count(m2) and struct.unpack_from("<2I", blob2, 72) == (2, 1)
     assert struct.unpack_from("<4I", blob, 44) == (1, 1, 2, 1)
     assert struct.unpack_from("<2If", blob, 60)[:2] == (1, 1)
 
@@ -83,5 +87,8 @@ def test_build_candidates_rejects_bad_arguments_before_touching_the_device(L):
     assert L.mlpf_build_candidates(None, 4, off, 1, None, 9, None, None, 0, None, None, None, None, None) == -6
     assert L.mlpf_build_candidates(None, 55, off, 1, None, 9, None, None, 0, None, None, None, None, None) == -1
     assert L.mlpf_build_candidates(None, 55, None, 0, None, 9, None, None, 0, None, None, None, None, None) == 0
+    off = (C.c_int32 * 2)(0, 4)
+    assert L.mlpf_build_candidates_ex(None, 55, off, 1, None, 9, None, 4, None, None, 0, None, None, None, None, None) == -6   # n_regress
+    assert L.mlpf_build_candidates_ex(None, 55, off, 1, None, 49, None, 5, None, None, 0, None, None, None, None, None) == -6  # n_classes
     assert L.mlpf_candidates_scratch_bytes(1000, 4) >= 1000 + 5 * 4 + 2 * 4 * 4
     assert L.mlpf_candidates_scratch_bytes(-1, 0) < 0

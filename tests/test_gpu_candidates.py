@@ -20,10 +20,11 @@ def _need_gpu():
     assert P.lib() is not None
 
 
-def _compare(X, off, logits, regress):
-    c = P.build_candidates(torch.from_numpy(X).cuda(), off, torch.from_numpy(logits).cuda(), torch.from_numpy(regress).cuda())
+def _compare(X, off, logits, regress, binary=None):
+    c = P.build_candidates(torch.from_numpy(X).cuda(), off, torch.from_numpy(logits).cuda(), torch.from_numpy(regress).cuda(),
+                           binary=None if binary is None else torch.from_numpy(binary).cuda())
     torch.cuda.synchronize()
-    ref = oracle.build_candidates(X, off, logits, regress)
+    ref = oracle.build_candidates(X, off, logits, regress, binary=binary)
     got_off = c["cand_offsets"].cpu().numpy()
     assert np.array_equal(got_off, ref["cand_offsets"])
     M = int(got_off[-1]) if len(got_off) else 0
@@ -112,3 +113,21 @@ def test_candidates_deterministic_and_scratch_reuse():
     for k in a:
         n = M if k != "cand_offsets" else 3
         assert torch.equal(a[k][:n], b[k][:n])
+
+
+@pytest.mark.parametrize("lens,pad", [((64, 192), 0.0), ((5, 0, 0, 300, 1, 0), 0.2), ((1000, 1500, 777, 2049), 0.1)])
+def test_candidates_binary_rule_matches_oracle(lens, pad):
+    """The paper's selection (L156): binary score > 0.5; PID = argmax over all classes (class 0 can be kept); a type id
+    outside 0..4 is clamped as in the forward pass (-1 -> pad row, 7 -> a real element)."""
+    X, off = synth.make_events(lens, seed=41, pad_frac=pad)
+    N = int(off[-1])
+    logits, regress = _random_outputs(N, 42)
+    rng = np.random.default_rng(43)
+    binary = rng.standard_normal(N).astype(np.float32)
+    binary[::7] = 0.0                                      # sigmoid(0) = 0.5: not above
+    binary[1::11] = 1e-30                                  # tiny positive logit: above
+    if N > 20:
+        X[3, 0], X[5, 0] = -1.0, 7.0
+        binary[3] = binary[5] = 2.0
+    M = _compare(X, off, logits, regress, binary=binary)
+    assert M > 0

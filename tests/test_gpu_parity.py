@@ -317,3 +317,61 @@ def test_without_final_layernorm(precision, tol):
     Wq = oracle.quantize_weights(W) if precision == P.PREC_BF16 else W
     lr, rr = oracle.forward(X, off, Wq, m)
     check(lg, rg, np.arange(X.shape[0]), lr, rr, X, tol, argmax=False)
+
+
+# ------------------------------------------------------------------------------------------- the paper's topology (NEXT-1)
+def _two_stack_check(W, m, X, off, precision, tol, fuse=1):
+    mod = P.Mlpf(W, m)
+    mod.set_option(P.OPT_PRECISION, precision)
+    mod.set_option(P.OPT_FUSE, fuse)
+    lg, rg, bn = [t.cpu().numpy() for t in mod.infer(torch.from_numpy(X).cuda(), off, with_binary=True)]
+    torch.cuda.synchronize()
+    Wq = oracle.quantize_weights(W) if precision == P.PREC_BF16 else W
+    lr, rr, br = oracle.forward(X, off, Wq, m, with_binary=True)
+    valid = X[:, 0] != 0
+    check(lg, rg, np.arange(X.shape[0]), lr, rr, X, tol, argmax=X.shape[0] > 1000)
+    e_b, _ = oracle.parity_metrics(bn[:, None], br[:, None], valid)
+    assert (bn[~valid] == 0).all() and e_b <= tol, e_b
+    return mod, lg, rg, bn
+
+
+TWO_TINY = ModelCfg(n_layers=2, d_model=64, n_heads=4, d_ff=256, activation="relu", n_stacks=2, binary_head=True)
+
+
+@pytest.mark.parametrize("precision,tol", [(P.PREC_FP32_DEBUG, TOL_FP32), (P.PREC_BF16, TOL_BF16)])
+@pytest.mark.parametrize("fuse", [1, 0])
+@pytest.mark.parametrize("lens,pad", [((70, 130, 9), 0.1), ((1,), 0.0), ((0, 300, 0, 129), 0.3), ((128, 256), 0.0)])
+def test_two_stack_small(lens, pad, fuse, precision, tol):
+    """Two parallel encoders + binary head on ragged / padded / empty events; N both a multiple of 128
+    (no gap between the stacks' row blocks) and not."""
+    W = synth.make_weights(TWO_TINY, seed=31)
+    X, off = synth.make_events(lens, seed=32, pad_frac=pad)
+    _two_stack_check(W, TWO_TINY, X, off, precision, tol, fuse)
+
+
+def test_two_stack_paper_topology_bf16_and_candidates():
+    """config `paper2` = the paper's network (two 3-block encoders, d 256, 16 x 16, ReLU, six heads): all 4 events against the
+    oracle, then the paper's decode (binary score > 0.5, L156) of the GPU's own outputs, integers bit-exact."""
+    name = "paper2"
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    X, off = synth.make_named_events(name)
+    mod, lg, rg, bn = _two_stack_check(W, m, X, off, P.PREC_BF16, TOL_BF16)
+    print("paper2 launches per step:", mod.query(P.Q_LAUNCHES))
+    Xd = torch.from_numpy(X).cuda()
+    c = P.build_candidates(Xd, off, torch.from_numpy(lg).cuda(), torch.from_numpy(rg).cuda(), binary=torch.from_numpy(bn).cuda())
+    torch.cuda.synchronize()
+    ref = oracle.build_candidates(X, off, lg, rg, binary=bn)
+    Mc = int(ref["cand_offsets"][-1])
+    assert 0 < Mc < X.shape[0]
+    assert np.array_equal(c["cand_offsets"].cpu().numpy(), ref["cand_offsets"])
+    assert np.array_equal(c["cand_elem"].cpu().numpy()[:Mc], ref["cand_elem"])
+    assert np.array_equal(c["cand_pid"].cpu().numpy()[:Mc], ref["cand_pid"])
+    assert np.allclose(c["cand_p4"].cpu().numpy()[:Mc], ref["cand_p4"], rtol=1e-5, atol=1e-5)
+
+
+def test_two_stack_fp32_debug_one_event():
+    name = "paper2"
+    m = synth.model_cfg(name)
+    X, off = synth.make_named_events(name, max_events=1)
+    _two_stack_check(synth.make_weights(name), m, X, off, P.PREC_FP32_DEBUG, TOL_FP32)
