@@ -257,7 +257,10 @@ def schedule(X, offsets, tile_q: int):
     row_event, row_pos, valid, n_valid per event, the stable by-type row order with each type
     segment padded to a multiple of 128 rows (type_offsets in padded 'sorted' space), and the
     attention work list (event, q_tile) ordered by descending n_e, then ascending event id,
-    then ascending q_tile; events with n_e = 0 contribute no tiles."""
+    then ascending q_tile; events with n_e = 0 contribute no tiles.  Pad-row compaction: the valid rows keep
+    their order and are numbered consecutively (comp_row, -1 for pad rows; comp_type_perm = type_perm through
+    that numbering), so event e owns the compacted rows offsets_c[e] .. offsets_c[e+1]-1 (offsets_c =
+    running sum of n_valid): pad rows take part in nothing (reading A2), the kernels skip them altogether."""
     offsets = np.asarray(offsets, dtype=np.int64)
     E = len(offsets) - 1
     N = int(offsets[-1])
@@ -292,6 +295,16 @@ def schedule(X, offsets, tile_q: int):
     for i in range(N):
         if sorted_row[i] >= 0:
             type_perm[sorted_row[i]] = i
+    comp_row = np.full(N, -1, np.int32)
+    nxt = 0
+    for i in range(N):
+        if t[i] != 0:
+            comp_row[i] = nxt
+            nxt += 1
+    offsets_c = np.zeros(E + 1, np.int32)
+    for e in range(E):
+        offsets_c[e + 1] = offsets_c[e] + n_valid[e]
+    comp_type_perm = np.where(type_perm >= 0, comp_row[np.maximum(type_perm, 0)], -1).astype(np.int32)
     lens = offsets[1:] - offsets[:-1]
     order = sorted(range(E), key=lambda e: (-int(lens[e]), e))
     work = []
@@ -301,7 +314,7 @@ def schedule(X, offsets, tile_q: int):
     work = np.asarray(work, np.int32).reshape(-1, 2)
     return dict(row_event=row_event, row_pos=row_pos, valid=valid, n_valid=n_valid,
                 type_offsets=type_offsets, sorted_row=sorted_row, type_perm=type_perm,
-                work_list=work)
+                comp_row=comp_row, offsets_c=offsets_c, comp_type_perm=comp_type_perm, work_list=work)
 
 
 # ----------------------------------------------------------------------------- error metric (A14)

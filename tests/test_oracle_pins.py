@@ -399,6 +399,16 @@ def test_p13_schedule_bruteforce():
         assert (s["type_perm"][to[ty] + len(rows):to[ty + 1]] == -1).all()
         assert [s["sorted_row"][i] for i in rows] == list(range(to[ty], to[ty] + len(rows)))
     assert all(s["sorted_row"][i] == -1 for i in range(N) if t[i] == 0)
+    # pad-row compaction, brute force: the c-th valid row (global order) is compacted row c; events stay contiguous
+    valid_rows = [i for i in range(N) if t[i] != 0]
+    assert [int(s["comp_row"][i]) for i in valid_rows] == list(range(len(valid_rows)))
+    assert all(s["comp_row"][i] == -1 for i in range(N) if t[i] == 0)
+    for e in range(len(off) - 1):
+        mine = [int(s["comp_row"][i]) for i in range(int(off[e]), int(off[e + 1])) if t[i] != 0]
+        assert mine == list(range(int(s["offsets_c"][e]), int(s["offsets_c"][e + 1])))
+    assert s["offsets_c"][0] == 0 and s["offsets_c"][-1] == len(valid_rows)
+    for slot, row in enumerate(s["type_perm"]):
+        assert s["comp_type_perm"][slot] == (-1 if row < 0 else s["comp_row"][row])
     # work list: longest event first, ties by id, tiles ascending
     lens = [int(off[e + 1] - off[e]) for e in range(len(off) - 1)]
     expect = []
