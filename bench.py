@@ -48,17 +48,23 @@ def workload(name, rank=0):
     return X, off
 
 
-def flop_model(m, off):
-    """Algorithmic FLOPs of one forward pass (linear 2*M*N*K, attention 4*d*sum n_e^2 per layer)."""
+def flop_model(m, off, X=None):
+    """Algorithmic FLOPs of one forward pass (linear 2*M*N*K, attention 4*d*sum n_e^2 per layer).  With X the
+    row counts are those of the VALID rows: pad rows (type 0) take part in nothing (reading A2) and are dropped after a0."""
     n = np.diff(off).astype(np.float64)
+    if X is not None:
+        v = np.concatenate([[0], np.cumsum(X[:, 0] != 0)])
+        n = (v[off[1:]] - v[off[:-1]]).astype(np.float64)
     N, s2 = n.sum(), (n * n).sum()
     d, dff, L, F = m.d_model, m.d_ff, m.n_layers, m.n_feat
     attn_layer = 4.0 * d * s2
     lin_layer = 2.0 * N * (3 * d * d + d * d + 2 * d * dff)
     emb = 2.0 * N * (F * d + d * d)
     heads = 2.0 * N * ((1 + len(m.reg_dims)) * d * d + (m.n_classes + sum(m.reg_dims)) * d)
-    return dict(attn_per_launch=attn_layer, total=L * (attn_layer + lin_layer) + emb + heads,
-                gemm_per_layer=lin_layer)
+    S = getattr(m, "n_stacks", 1)
+    heads += 2.0 * N * (m.d_model * m.d_model + m.d_model) * (1 if getattr(m, "binary_head", False) else 0)
+    return dict(attn_per_launch=S * attn_layer, total=S * L * (attn_layer + lin_layer) + emb + heads,
+                gemm_per_layer=S * lin_layer)
 
 
 class ClockSampler(threading.Thread):
@@ -202,7 +208,7 @@ def run_ours(args):
     W = synth.make_weights(name)
     X, off = workload(name, rank)
     E, N = len(off) - 1, int(off[-1])
-    fl = flop_model(m, off)
+    fl = flop_model(m, off, X)
     peaks = load_peaks()
 
     mod = P.Mlpf(W, m)

@@ -171,6 +171,9 @@ int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* 
                                     2 = the same with the exact path forced for every CTA; 0 = round 1's lazy-rescale kernel */
 #define MLPF_OPT_ATTN_POLY   9   /* tuning (process-wide): n of every 16 pairs of softmax exponentials run as a polynomial on the
                                     FMA pipe instead of the MUFU: 0 (none), 4..9; -1 (default) = per head dimension          */
+#define MLPF_OPT_COMPACT     10  /* 1 (default): pad rows (type 0) are dropped after a0: every later step runs on the compacted rows
+                                    (events stay contiguous, oracle.schedule comp_row / offsets_c), outputs are scattered back;
+                                    0: pad rows stay in place and are masked as keys (round 1's behaviour)                   */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0
@@ -203,6 +206,9 @@ int64_t mlpf_query(const mlpf_handle* h, int key);   /* < 0 on error */
 #define MLPF_SCHED_SORTED_ROW   5   /* [N] row -> sorted slot, -1 for pad    */
 #define MLPF_SCHED_TYPE_PERM    6   /* [type_offsets[5]] slot -> row, -1 filler */
 #define MLPF_SCHED_WORK_LIST    7   /* [n_tiles,2] (event, q_tile)           */
+#define MLPF_SCHED_COMP_ROW     8   /* [N] row -> compacted row, -1 for pad  */
+#define MLPF_SCHED_OFFSETS_C    9   /* [E+1] event offsets in compacted rows */
+#define MLPF_SCHED_COMP_TYPE_PERM 10 /* [type_offsets[5]] slot -> compacted row, -1 filler */
 /* returns the number of int32 written, or a negative error (MLPF_E_ARG if capacity is too small) */
 int64_t mlpf_debug_get_schedule(mlpf_handle* h, void* stream, int which, int32_t* host_out, int64_t capacity);
 

@@ -16,12 +16,13 @@ LIB_PATH = os.path.join(_HERE, "libmlpf.so")
 
 # include/mlpf.h constants
 OK = 0
-OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE, OPT_FUSE, OPT_ATTN, OPT_ATTN_POLY = 1, 2, 3, 4, 5, 6, 7, 8, 9
+OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE, OPT_FUSE, OPT_ATTN, OPT_ATTN_POLY, OPT_COMPACT = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 PREC_BF16, PREC_FP32_DEBUG = 0, 1
 KERNELS_TC, KERNELS_SIMPLE = 0, 1
 Q_N_LAYERS, Q_D_MODEL, Q_N_HEADS, Q_D_FF, Q_N_FEAT, Q_N_CLASSES, Q_N_REGRESS = 1, 2, 3, 4, 5, 6, 7
 Q_WEIGHT_BYTES, Q_WORKSPACE_BYTES, Q_N_PARAMS, Q_LAUNCHES, Q_N_STACKS, Q_BINARY_HEAD = 8, 9, 10, 11, 12, 13
-SCHED = dict(row_event=0, row_pos=1, valid=2, n_valid=3, type_offsets=4, sorted_row=5, type_perm=6, work_list=7)
+SCHED = dict(row_event=0, row_pos=1, valid=2, n_valid=3, type_offsets=4, sorted_row=5, type_perm=6, work_list=7,
+             comp_row=8, offsets_c=9, comp_type_perm=10)
 TENSOR = dict(H=0, U=1, QK=2, V=3, O=4, G=5)
 KERNEL_CLASSES = ["sched", "embed_l1", "embed_l2", "layernorm", "qkv", "attention", "outproj", "ffn1", "ffn2",
                   "heads_l1", "heads_l2", "post"]

@@ -44,6 +44,9 @@ struct Epi {
     // Uniform groups (two parallel encoders): group_rows > 0 (a multiple of 128) -> the M-tile starting at
     // m0 uses weight / bias block m0 / group_rows of a weight matrix [G * N, K] and a bias [G * N].
     int group_rows = 0;
+    // Pad-row compaction: nc_dev (device, may be null) holds the number of meaningful rows (per group when group_rows > 0);
+    // M-tiles that start at or beyond it are skipped (the host only knows the upper bound M).
+    const int* nc_dev = nullptr;
 };
 
 __device__ __forceinline__ float warp_sum(float v) {

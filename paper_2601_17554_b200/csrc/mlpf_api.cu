@@ -59,6 +59,8 @@ struct Workspace {
     int *valid = nullptr, *row_event = nullptr, *row_pos = nullptr, *n_valid = nullptr;
     int *block_counts = nullptr, *block_base = nullptr, *type_offsets = nullptr;
     int *sorted_row = nullptr, *type_perm = nullptr;
+    SchedCompact sc = {};                    // pad-row compaction arrays (a0)
+    bool compact = false;                    // the last call ran on compacted rows
     float *qn = nullptr, *kmax = nullptr;   // attention norms pre-pass: |q_i| per row and head, max |k_j| per event and head
     // device staging of mlpf_infer_host (owned by the stream's workspace, freed with it); capacities in BYTES
     float *stage_x = nullptr, *stage_lg = nullptr, *stage_rg = nullptr;
@@ -90,7 +92,7 @@ struct mlpf_handle {
     std::vector<LayerW> layers;
     HeadsOut ho;
     // options
-    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1;
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1;
     int64_t last_launches = 0;
     std::mutex mu;
     std::map<void*, Workspace*> ws;
@@ -263,6 +265,9 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_ATTN:
             if (value < 0 || value > 2) return set_err(MLPF_E_ARG, "attn must be 0, 1 or 2");
             h->attn = (int)value; return MLPF_OK;
+        case MLPF_OPT_COMPACT:
+            if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "compact must be 0 or 1");
+            h->compact = (int)value; return MLPF_OK;
         case MLPF_OPT_ATTN_POLY:
             if (value < -1 || value > 9 || (value > 0 && value < 4)) return set_err(MLPF_E_ARG, "attn_poly must be -1, 0 or 4..9");
             g_attn2_poly_every = (int)value; return MLPF_OK;
@@ -315,13 +320,15 @@ static void ws_free_rows(Workspace* w) {
     dfree(w->h); dfree(w->u); dfree(w->qkv); dfree(w->o); dfree(w->g); dfree(w->u_lo); dfree(w->o_lo); dfree(w->g_lo);
     dfree(w->valid); dfree(w->valid_bits); dfree(w->row_event); dfree(w->row_pos); dfree(w->block_counts); dfree(w->block_base);
     dfree(w->sorted_row); dfree(w->type_perm); dfree(w->type_offsets); dfree(w->qn);
+    dfree(w->sc.block_vbase); dfree(w->sc.n_comp); dfree(w->sc.vbefore); dfree(w->sc.comp_row); dfree(w->sc.orig_row);
+    dfree(w->sc.row_event_c); dfree(w->sc.comp_type_perm);
     w->cap_rows = 0;
 }
 
 static int64_t ws_bytes_events(const Workspace* w) {
     int64_t b = 0;
     if (w->offsets) b += std::max<int64_t>((w->cap_events + 1) * 4, 256) + std::max<int64_t>(w->cap_events * 4, 256);
-    if (w->kmax) b += std::max<int64_t>(w->cap_events * 64 * 4, 256);      // upper bound (H <= 64)
+    if (w->kmax) b += std::max<int64_t>(w->cap_events * 64 * 4, 256) + std::max<int64_t>((w->cap_events + 1) * 4, 256);   // upper bound (H <= 64)
     if (w->work) b += 2 * std::max<int64_t>(w->cap_tiles * 8, 256);
     return b;
 }
@@ -347,7 +354,10 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
             dmalloc(&w->valid, cap * 4, w) || dmalloc(&w->valid_bits, (cap / 32 + 40) * 4, w) || dmalloc(&w->row_event, cap * 4, w) || dmalloc(&w->row_pos, cap * 4, w) ||
             dmalloc(&w->block_counts, nb * 5 * 4, w) || dmalloc(&w->block_base, nb * 5 * 4, w) ||
             dmalloc(&w->sorted_row, cap * 4, w) || dmalloc(&w->type_perm, m_ub * 4, w) ||
-            dmalloc(&w->type_offsets, 8 * 4, w) || dmalloc(&w->qn, cap * h->H * 4, w)) {
+            dmalloc(&w->type_offsets, 8 * 4, w) || dmalloc(&w->qn, cap * h->H * 4, w) ||
+            dmalloc(&w->sc.block_vbase, nb * 4, w) || dmalloc(&w->sc.n_comp, 4, w) || dmalloc(&w->sc.vbefore, cap * 4, w) ||
+            dmalloc(&w->sc.comp_row, cap * 4, w) || dmalloc(&w->sc.orig_row, cap * 4, w) || dmalloc(&w->sc.row_event_c, cap * 4, w) ||
+            dmalloc(&w->sc.comp_type_perm, m_ub * 4, w)) {
             const char* why = cudaGetErrorString(cudaGetLastError());
             ws_free_rows(w);                       // release the partial set; nothing dangling is left behind
             w->bytes = ws_bytes_events(w);
@@ -359,6 +369,7 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
         cudaMemsetAsync(w->valid_bits, 0, (cap / 32 + 40) * 4, st);
         cudaMemsetAsync(w->h, 0, cap * d * 4, st);
         cudaMemsetAsync(w->valid, 0, cap * 4, st); cudaMemsetAsync(w->row_event, 0, cap * 4, st);
+        cudaMemsetAsync(w->sc.row_event_c, 0, cap * 4, st);
         cudaMemsetAsync(w->u, 0, cap * d * es, st); cudaMemsetAsync(w->qkv, 0, cap * 3 * d * es, st);
         cudaMemsetAsync(w->o, 0, cap * d * es, st);
         cudaMemsetAsync(w->g, 0, w->g_elems * es, st);
@@ -367,11 +378,12 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
         w->cap_rows = cap;
     }
     if (E > w->cap_events) {
-        dfree(w->offsets); dfree(w->n_valid); dfree(w->kmax);
+        dfree(w->offsets); dfree(w->n_valid); dfree(w->kmax); dfree(w->sc.offsets_c);
         w->cap_events = 0;
         const int64_t ce = std::max<int64_t>(E, 64);
-        if (dmalloc(&w->offsets, (ce + 1) * 4, w) || dmalloc(&w->n_valid, ce * 4, w) || dmalloc(&w->kmax, ce * h->H * 4, w)) {
-            dfree(w->offsets); dfree(w->n_valid); dfree(w->kmax);
+        if (dmalloc(&w->offsets, (ce + 1) * 4, w) || dmalloc(&w->n_valid, ce * 4, w) || dmalloc(&w->kmax, ce * h->H * 4, w) ||
+            dmalloc(&w->sc.offsets_c, (ce + 1) * 4, w)) {
+            dfree(w->offsets); dfree(w->n_valid); dfree(w->kmax); dfree(w->sc.offsets_c);
             return set_err(MLPF_E_ALLOC, "workspace allocation for %lld events failed", (long long)ce);
         }
         w->cap_events = ce;
@@ -393,7 +405,7 @@ static void ws_free(Workspace* w) {
     ws_free_rows(w);
     dfree(w->stage_x); dfree(w->stage_lg); dfree(w->stage_rg);
     w->stage_cap = 0;
-    dfree(w->offsets); dfree(w->n_valid); dfree(w->work); dfree(w->pairs); dfree(w->kmax);
+    dfree(w->offsets); dfree(w->n_valid); dfree(w->work); dfree(w->pairs); dfree(w->kmax); dfree(w->sc.offsets_c);
     for (cudaEvent_t e : w->ev_pool) cudaEventDestroy(e);
     w->ev_pool.clear();
 }
@@ -442,21 +454,28 @@ static int run_layernorm(mlpf_handle* h, bool fp32, const float* x, int N, const
 
 static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspace* w, cudaStream_t st) {
     if (w->n_tiles == 0) return MLPF_OK;
+    // compacted rows: every row of an event is a valid key (no mask but the event tail), events are offsets_c
+    const int* offsets = w->compact ? w->sc.offsets_c : w->offsets;
+    const int* row_event = w->compact ? w->sc.row_event_c : w->row_event;
+    const uint32_t* valid_bits = w->compact ? nullptr : w->valid_bits;
+    const int* n_valid = w->compact ? nullptr : w->n_valid;
+    const int* valid = w->compact ? nullptr : w->valid;
     if (tc && !fp32) {
         int rc;
         if (h->attn == 0)
-            rc = tc_attn_launch(&h->tc, (const bf16*)w->qkv, w->Mtot, w->valid_bits, w->n_valid, w->offsets,
+            rc = tc_attn_launch(&h->tc, (const bf16*)w->qkv, w->Mtot, valid_bits, n_valid, offsets,
                                 (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, (bf16*)w->o,
                                 split ? (bf16*)w->o_lo : nullptr, st);
         else {
-            rc = tc_attn2_launch(&h->tc, (const bf16*)w->qkv, w->Mtot, (int)w->Ev, w->valid_bits, w->n_valid, w->offsets, w->row_event,
+            rc = tc_attn2_launch(&h->tc, (const bf16*)w->qkv, w->Mtot, (int)w->Ev, valid_bits, n_valid, offsets, row_event,
                                  (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, w->qn, w->kmax, (bf16*)w->o,
-                                 split ? (bf16*)w->o_lo : nullptr, h->attn == 2, st);
+                                 split ? (bf16*)w->o_lo : nullptr, h->attn == 2, w->compact ? w->sc.n_comp : nullptr,
+                                 h->S > 1 ? (int)w->Npad : 0, st);
             h->last_launches++;                       // the norms pre-pass
         }
         if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", h->tc.err);
     } else {
-        launch_attn_simple(fp32, h->hd, w->qkv, w->valid, w->offsets, (const int2*)w->work, (int)w->n_tiles,
+        launch_attn_simple(fp32, h->hd, w->qkv, valid, offsets, (const int2*)w->work, (int)w->n_tiles,
                            h->H, w->tile_q, h->d, w->o, split ? w->o_lo : nullptr, st);
     }
     LAUNCH_CHECK(h);
@@ -484,6 +503,9 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     const int N = (int)w->N, E = (int)w->E, d = h->d, dff = h->dff;
     const int S = h->S, Npad = (int)w->Npad, M = (int)w->Mtot;          // M rows cover all stacks (S = 1: M = N)
     const int grp_rows = S > 1 ? Npad : 0;
+    const bool compact = h->compact != 0;                                // pad rows dropped from every step after a0 / a1
+    w->compact = compact;
+    const int* nc_dev = compact ? w->sc.n_comp : nullptr;
     const bool tc_req = !fp32 && h->kernels == MLPF_KERNELS_TC;
     const bool tc = tc_req, tc_attn = tc_req;
     const int64_t es = fp32 ? 4 : 2;
@@ -502,29 +524,32 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     ProfScope ps(h, w, st, MLPF_KC_SCHED);
     CUDA_TRY(cudaMemsetAsync(w->n_valid, 0, (size_t)E * 4, st));
     CUDA_TRY(cudaMemsetAsync(w->type_perm, 0xff, (size_t)w->m_ub * 4, st));
+    CUDA_TRY(cudaMemsetAsync(w->sc.comp_type_perm, 0xff, (size_t)w->m_ub * 4, st));
     h->last_launches += launch_schedule(X, N, h->F, w->offsets, E, w->block_counts, w->block_base, w->valid, w->valid_bits, w->row_event,
-                                        w->row_pos, w->n_valid, w->type_offsets, w->sorted_row, w->type_perm, st) - 1;
+                                        w->row_pos, w->n_valid, w->type_offsets, w->sorted_row, w->type_perm, w->sc, st) - 1;
     LAUNCH_CHECK(h);
     }
 
     // ---- a1: per-type embedding (L156; A3-A5)
     {
     ProfScope ps(h, w, st, MLPF_KC_EMBED_L1);
-    launch_embed_l1(fp32, X, N, h->F, d, PV + h->embW1t, PV + h->embB1, h->act, w->sorted_row, g, lo(MLPF_SPLIT_EMB, w->g_lo), w->h, st);
+    launch_embed_l1(fp32, X, N, h->F, d, PV + h->embW1t, PV + h->embB1, h->act, w->sorted_row, g, lo(MLPF_SPLIT_EMB, w->g_lo),
+                    compact ? nullptr : w->h, st);
     LAUNCH_CHECK(h);
     }
     {
         ProfScope ps(h, w, st, MLPF_KC_EMBED_L2);
         Epi ep;
         ep.bias = PV + h->embB2; ep.out_f32 = w->h; ep.ld_f32 = d;
-        ep.row_perm = w->type_perm; ep.group_offsets = w->type_offsets; ep.n_groups = 4;
+        ep.row_perm = compact ? w->sc.comp_type_perm : w->type_perm; ep.group_offsets = w->type_offsets; ep.n_groups = 4;
         int rc = run_gemm(h, fp32, tc, g, lo(MLPF_SPLIT_EMB, w->g_lo), PW(h->embW2), (int)w->m_ub, d, d, ep, st);
         if (rc) return rc;
     }
     if (h->tap_layer == -2) return MLPF_OK;
     for (int g1 = 1; g1 < S; ++g1) {       // the shared embedding feeds every encoder stack (L156): stack g1's rows + schedule
         ProfScope ps(h, w, st, MLPF_KC_SCHED);
-        launch_sched_replicate(N, Npad, E, g1, d, w->offsets, w->n_valid, w->row_event, w->valid, w->valid_bits, w->h, st);
+        launch_sched_replicate(N, Npad, E, g1, d, compact ? w->sc.offsets_c : w->offsets, w->n_valid,
+                               compact ? w->sc.row_event_c : w->row_event, w->valid, w->valid_bits, w->h, st);
         LAUNCH_CHECK(h);
     }
     // stand-alone LayerNorm of every stack's rows with that stack's gamma / beta (vectors are stacked [S, d])
@@ -557,7 +582,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         {   // a3: [Q K V] = LN1(x) Wqkv^T + bqkv
             ProfScope ps(h, w, st, MLPF_KC_QKV);
             Epi ep;
-            ep.bias = PV + lw.bqkv; ep.out_act = w->qkv; ep.ld_act = 3 * d; ep.group_rows = grp_rows; ep.n_groups = S;
+            ep.bias = PV + lw.bqkv; ep.out_act = w->qkv; ep.ld_act = 3 * d; ep.group_rows = grp_rows; ep.n_groups = S; ep.nc_dev = nc_dev;
             rc = run_gemm(h, fp32, tc, u, nullptr, PW(lw.Wqkv), M, 3 * d, d, ep, st);
             if (rc) return rc;
         }
@@ -570,7 +595,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
             ProfScope ps(h, w, st, MLPF_KC_POST);
             const bool last = l + 1 == h->L, tap = h->tap_layer == l;
             PostArgs a;
-            a.M = M; a.d = d; a.dff = dff; a.act = h->act; a.n_groups = S; a.group_rows = grp_rows;
+            a.M = M; a.d = d; a.dff = dff; a.act = h->act; a.n_groups = S; a.group_rows = grp_rows; a.nc_dev = nc_dev;
             a.o = (const bf16*)w->o; a.o_lo = (const bf16*)w->o_lo;
             a.Wo = (const bf16*)PW(lw.Wo); a.W1 = (const bf16*)PW(lw.W1); a.W2 = (const bf16*)PW(lw.W2);
             a.bo = PV + lw.bo; a.ln2g = PV + lw.ln2g; a.ln2b = PV + lw.ln2b; a.b1 = PV + lw.b1; a.b2 = PV + lw.b2;
@@ -596,7 +621,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
             ProfScope ps(h, w, st, MLPF_KC_OUTPROJ);
             Epi ep;
             ep.bias = PV + lw.bo; ep.residual = w->h; ep.ld_res = d; ep.out_f32 = w->h; ep.ld_f32 = d;
-            ep.group_rows = grp_rows; ep.n_groups = S;
+            ep.group_rows = grp_rows; ep.n_groups = S; ep.nc_dev = nc_dev;
             rc = run_gemm(h, fp32, tc, w->o, lo(MLPF_SPLIT_O, w->o_lo), PW(lw.Wo), M, d, d, ep, st);
             if (rc) return rc;
         }
@@ -609,7 +634,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
             ProfScope ps(h, w, st, MLPF_KC_FFN1);
             Epi ep;
             ep.bias = PV + lw.b1; ep.act = h->act; ep.out_act = g; ep.out_act_lo = lo(MLPF_SPLIT_G, w->g_lo); ep.ld_act = dff;
-            ep.group_rows = grp_rows; ep.n_groups = S;
+            ep.group_rows = grp_rows; ep.n_groups = S; ep.nc_dev = nc_dev;
             rc = run_gemm(h, fp32, tc, u, lo(MLPF_SPLIT_U2, w->u_lo), PW(lw.W1), M, dff, d, ep, st);
             if (rc) return rc;
         }
@@ -617,7 +642,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
             ProfScope ps(h, w, st, MLPF_KC_FFN2);
             Epi ep;
             ep.bias = PV + lw.b2; ep.residual = w->h; ep.ld_res = d; ep.out_f32 = w->h; ep.ld_f32 = d;
-            ep.group_rows = grp_rows; ep.n_groups = S;
+            ep.group_rows = grp_rows; ep.n_groups = S; ep.nc_dev = nc_dev;
             rc = run_gemm(h, fp32, tc, g, lo(MLPF_SPLIT_G, w->g_lo), PW(lw.W2), M, d, dff, ep, st);
             if (rc) return rc;
         }
@@ -653,6 +678,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
                 ep.bias = PV + h->headB1 + (int64_t)b0 * d; ep.act = h->act; ep.ld_act = hw;
                 ep.out_act = (char*)g + (int64_t)b0 * d * es;
                 ep.out_act_lo = lo(MLPF_SPLIT_HEAD, w->g_lo) ? (char*)w->g_lo + (int64_t)b0 * d * es : nullptr;
+                ep.nc_dev = nc_dev;
                 rc = run_gemm(h, fp32, tc, (char*)u + r0 * d * es, lo(MLPF_SPLIT_UF, w->u_lo) ? (char*)w->u_lo + r0 * d * es : nullptr,
                               PW(h->headW1 + (int64_t)b0 * d * d), N, nb * d, d, ep, st);
             }
@@ -660,8 +686,8 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         if (rc) return rc;
         w->g_width = hw;
         ProfScope ps(h, w, st, MLPF_KC_HEADS_L2);
-        launch_heads_l2(fp32, g, lo(MLPF_SPLIT_HEAD, w->g_lo), N, d, hw, PV + h->headW2, PV + h->headB2, w->valid, h->ho, out_logits,
-                        out_regress, out_binary, st);
+        launch_heads_l2(fp32, g, lo(MLPF_SPLIT_HEAD, w->g_lo), N, d, hw, PV + h->headW2, PV + h->headB2, w->valid, compact ? w->sc.comp_row : nullptr,
+                        h->ho, out_logits, out_regress, out_binary, st);
         LAUNCH_CHECK(h);
     }
     return MLPF_OK;
@@ -819,6 +845,11 @@ extern "C" int64_t mlpf_debug_get_schedule(mlpf_handle* h, void* stream, int whi
         case MLPF_SCHED_TYPE_PERM:
             CUDA_TRY(cudaMemcpy(toff, w->type_offsets, 6 * 4, cudaMemcpyDeviceToHost));
             src = w->type_perm; n = toff[5]; break;
+        case MLPF_SCHED_COMP_ROW: src = w->sc.comp_row; n = w->N; break;
+        case MLPF_SCHED_OFFSETS_C: src = w->sc.offsets_c; n = w->E + 1; break;
+        case MLPF_SCHED_COMP_TYPE_PERM:
+            CUDA_TRY(cudaMemcpy(toff, w->type_offsets, 6 * 4, cudaMemcpyDeviceToHost));
+            src = w->sc.comp_type_perm; n = toff[5]; break;
         case MLPF_SCHED_WORK_LIST: src = w->work; n = w->n_tiles_real * 2; break;
         default: return set_err(MLPF_E_ARG, "unknown schedule array %d", which);
     }
@@ -827,12 +858,21 @@ extern "C" int64_t mlpf_debug_get_schedule(mlpf_handle* h, void* stream, int whi
     return n;
 }
 
-static int tap_copy(bool fp32, const void* src, int64_t rows, int64_t cols, int64_t ld, float* host_out) {
-    float* tmp = nullptr;
+// rows x cols block (row pitch ld, element type of the activation buffers) -> host fp32 [rows, cols]; comp_row != null:
+// the block's rows are COMPACTED rows, the result is indexed by original row (pad rows 0)
+static int tap_copy(bool fp32, const void* src, int64_t rows, int64_t cols, int64_t ld, const int* comp_row, float* host_out) {
+    float *tmp = nullptr, *tmp2 = nullptr, *tmp3 = nullptr;
     CUDA_TRY(cudaMalloc(&tmp, (size_t)rows * ld * 4));
     launch_to_f32(fp32, src, tmp, (rows - 1) * ld + cols, 0);     // src may be a column block of a wider buffer
-    cudaError_t e = cudaMemcpy2D(host_out, (size_t)cols * 4, tmp, (size_t)ld * 4, (size_t)cols * 4, (size_t)rows, cudaMemcpyDeviceToHost);
-    cudaFree(tmp);
+    const float* res = tmp;
+    cudaError_t e = cudaSuccess;
+    if (comp_row) {
+        if (cudaMalloc(&tmp2, (size_t)rows * cols * 4) != cudaSuccess || cudaMalloc(&tmp3, (size_t)rows * cols * 4) != cudaSuccess) e = cudaErrorMemoryAllocation;
+        if (e == cudaSuccess) e = cudaMemcpy2D(tmp2, (size_t)cols * 4, tmp, (size_t)ld * 4, (size_t)cols * 4, (size_t)rows, cudaMemcpyDeviceToDevice);
+        if (e == cudaSuccess) { launch_uncompact(tmp2, comp_row, tmp3, rows, (int)cols, 0); res = tmp3; ld = cols; }
+    }
+    if (e == cudaSuccess) e = cudaMemcpy2D(host_out, (size_t)cols * 4, res, (size_t)ld * 4, (size_t)cols * 4, (size_t)rows, cudaMemcpyDeviceToHost);
+    cudaFree(tmp); cudaFree(tmp2); cudaFree(tmp3);
     if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tap copy failed: %s", cudaGetErrorString(e));
     return MLPF_OK;
 }
@@ -845,20 +885,21 @@ extern "C" int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which
     Workspace* w = it->second;
     CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
     const int64_t N = w->N, d = h->d;
+    const int* comp_row = w->compact ? w->sc.comp_row : nullptr;
     const void* src = nullptr; int64_t rows = N, cols = d, ld = d;
     switch (which) {
         case MLPF_TENSOR_H: {
             if (N * d > capacity) return set_err(MLPF_E_ARG, "capacity too small");
+            float* tmp = nullptr;
+            const float* hsrc = w->h;
             if (w->h_tiled) {                         // the fused blocks keep h in their tiled layout: un-tile for the tap
-                float* tmp = nullptr;
                 CUDA_TRY(cudaMalloc(&tmp, (size_t)N * d * 4));
                 launch_untile_h(w->h, tmp, N, (int)d, 0);
-                cudaError_t e = cudaMemcpy(host_out, tmp, (size_t)N * d * 4, cudaMemcpyDeviceToHost);
-                cudaFree(tmp);
-                if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tap copy failed: %s", cudaGetErrorString(e));
-                return N * d;
+                hsrc = tmp;
             }
-            CUDA_TRY(cudaMemcpy(host_out, w->h, (size_t)N * d * 4, cudaMemcpyDeviceToHost));
+            int rc = tap_copy(true, hsrc, N, d, d, comp_row, host_out);
+            cudaFree(tmp);
+            if (rc) return rc;
             return N * d;
         }
         case MLPF_TENSOR_U: src = w->u; break;
@@ -869,7 +910,7 @@ extern "C" int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which
         default: return set_err(MLPF_E_ARG, "unknown tensor %d", which);
     }
     if (rows * cols > capacity) return set_err(MLPF_E_ARG, "capacity too small");
-    int rc = tap_copy(w->fp32, src, rows, cols, ld, host_out);
+    int rc = tap_copy(w->fp32, src, rows, cols, ld, comp_row, host_out);
     if (rc) return rc;
     return rows * cols;
 }
@@ -983,7 +1024,7 @@ extern "C" int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_va
         CUDA_TRY(cudaMemcpyAsync(d_rowev, rowev.data(), (size_t)N * 4, cudaMemcpyHostToDevice, st));
         CUDA_TRY(cudaStreamSynchronize(st));      // rowev is a local
         rc = tc_attn2_launch(&ctx, (const bf16*)QKV, N, n_events, d_bits, nullptr, d_off, d_rowev, (const int2*)d_pairs,
-                             (int)(pairs.size() / 2), d_model, n_heads, d_qn, d_kmax, (bf16*)O, (bf16*)nullptr, g_attn_impl == 2, st);
+                             (int)(pairs.size() / 2), d_model, n_heads, d_qn, d_kmax, (bf16*)O, (bf16*)nullptr, g_attn_impl == 2, nullptr, 0, st);
     }
     cudaError_t e = cudaStreamSynchronize(st);
     cudaFree(d_off); cudaFree(d_pairs); cudaFree(d_bits); cudaFree(d_rowev); cudaFree(d_qn); cudaFree(d_kmax);

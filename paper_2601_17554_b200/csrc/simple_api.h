@@ -14,10 +14,19 @@ struct HeadsOut {
     int blk[MAX_OUT];
 };
 
-// a0 device half: 3 launches.  Returns the number of kernels launched.
+// pad-row compaction arrays of a0 (oracle.schedule: comp_row, offsets_c, comp_type_perm), all device pointers
+struct SchedCompact {
+    int *block_vbase, *n_comp;        // [blocks], [1]: valid rows before each 1024-row block, total valid rows
+    int *vbefore, *comp_row;          // [N]
+    int *orig_row, *row_event_c;      // [N] indexed by compacted row
+    int *comp_type_perm;              // [type_offsets[5]]: sorted slot -> compacted row
+    int *offsets_c;                   // [E + 1]
+};
+// a0 device half: 4 launches.  Returns the number of kernels launched.
 int launch_schedule(const float* X, int N, int F, const int* offsets, int E, int* block_counts, int* block_base,
                     int* valid, uint32_t* valid_bits, int* row_event, int* row_pos, int* n_valid, int* type_offsets, int* sorted_row,
-                    int* type_perm, cudaStream_t st);
+                    int* type_perm, const SchedCompact& sc, cudaStream_t st);
+void launch_uncompact(const float* src, const int* comp_row, float* out, int64_t N, int cols, cudaStream_t st);
 void launch_embed_l1(bool fp32, const float* X, int N, int F, int d, const float* W1t, const float* b1, int act,
                      const int* sorted_row, void* h1, void* h1_lo, float* h, cudaStream_t st);
 int launch_layernorm(bool fp32, int d, const float* x, int N, const float* g, const float* b, float eps, void* u,
@@ -28,7 +37,7 @@ void launch_attn_simple(bool fp32, int hd, const void* QKV, const int* key_valid
                         const int* offsets, const int2* work, int n_tiles, int H, int tile_q, int d, void* O,
                         void* O_lo, cudaStream_t st);
 void launch_heads_l2(bool fp32, const void* hidden, const void* hidden_lo, int N, int d, int ld_hidden,
-                     const float* W2, const float* b2, const int* valid, const HeadsOut& ho, float* out_logits,
+                     const float* W2, const float* b2, const int* valid, const int* hid_row, const HeadsOut& ho, float* out_logits,
                      float* out_regress, float* out_binary, cudaStream_t st);
 void launch_sched_replicate(int N, int N_pad, int E, int g, int d, int* offsets, int* n_valid, int* row_event, int* valid,
                             uint32_t* valid_bits, float* h, cudaStream_t st);

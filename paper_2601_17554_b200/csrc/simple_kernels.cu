@@ -58,9 +58,10 @@ k_sched_count(const float* __restrict__ X, int N, int F, const int* __restrict__
     if (threadIdx.x < 5) block_counts[blockIdx.x * 5 + threadIdx.x] = hist[threadIdx.x];
 }
 
-// one block: exclusive scan of the per-block counts per type; segment starts padded to 128 rows
+// one block: exclusive scan of the per-block counts per type; segment starts padded to 128 rows.  Thread 5: the same
+// scan over the valid rows of all types (pad-row compaction): block_vbase[b] = valid rows before block b, n_comp[0] = total
 __global__ void k_sched_scan(const int* __restrict__ block_counts, int nb, int* __restrict__ block_base,
-                             int* __restrict__ type_offsets) {
+                             int* __restrict__ type_offsets, int* __restrict__ block_vbase, int* __restrict__ n_comp) {
     __shared__ int total[5];
     int ty = threadIdx.x;
     if (ty < 5) {
@@ -70,6 +71,13 @@ __global__ void k_sched_scan(const int* __restrict__ block_counts, int nb, int* 
             run += block_counts[b * 5 + ty];
         }
         total[ty] = run;
+    } else if (ty == 5) {
+        int run = 0;
+        for (int b = 0; b < nb; ++b) {
+            block_vbase[b] = run;
+            run += block_counts[b * 5 + 1] + block_counts[b * 5 + 2] + block_counts[b * 5 + 3] + block_counts[b * 5 + 4];
+        }
+        n_comp[0] = run;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -84,10 +92,14 @@ __global__ void k_sched_scan(const int* __restrict__ block_counts, int nb, int* 
 }
 
 // stable counting sort by type: sorted_row[i] = slot, type_perm[slot] = i  (type_perm pre-filled with -1)
+// Pad-row compaction (same pass): vbefore[i] = valid rows before row i; comp_row[i] = that
+// number for a valid row, -1 for a pad row; orig_row / row_event_c = the inverse map and the event of a compacted row;
+// comp_type_perm[slot] = compacted row of the slot's row.
 __global__ void __launch_bounds__(SCHED_BLOCK)
 k_sched_scatter(const float* __restrict__ X, int N, int F, const int* __restrict__ block_base,
-                const int* __restrict__ type_offsets, int* __restrict__ sorted_row,
-                int* __restrict__ type_perm) {
+                const int* __restrict__ type_offsets, const int* __restrict__ block_vbase, const int* __restrict__ row_event,
+                int* __restrict__ sorted_row, int* __restrict__ type_perm, int* __restrict__ vbefore, int* __restrict__ comp_row,
+                int* __restrict__ orig_row, int* __restrict__ row_event_c, int* __restrict__ comp_type_perm) {
     __shared__ int warp_cnt[32][5];
     int i = blockIdx.x * SCHED_BLOCK + threadIdx.x;
     int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -99,17 +111,36 @@ k_sched_scatter(const float* __restrict__ X, int N, int F, const int* __restrict
         if (t == ty) my_rank = __popc(m & ((1u << lane) - 1u));
         if (lane == 0) warp_cnt[w][ty] = __popc(m);
     }
+    const unsigned mv = __ballot_sync(0xffffffffu, t > 0);
+    const int vrank = __popc(mv & ((1u << lane) - 1u));
     __syncthreads();
     if (i < N) {
+        int before_v = 0;
+        for (int ww = 0; ww < w; ++ww) before_v += warp_cnt[ww][1] + warp_cnt[ww][2] + warp_cnt[ww][3] + warp_cnt[ww][4];
+        const int comp = block_vbase[blockIdx.x] + before_v + vrank;
+        vbefore[i] = comp;
+        comp_row[i] = t > 0 ? comp : -1;
         if (t == 0) {
             sorted_row[i] = -1;
         } else {
+            orig_row[comp] = i;
+            row_event_c[comp] = row_event[i];
             int before = 0;
             for (int ww = 0; ww < w; ++ww) before += warp_cnt[ww][t];
             int slot = type_offsets[t] + block_base[blockIdx.x * 5 + t] + before + my_rank;
             sorted_row[i] = slot;
             type_perm[slot] = i;
+            comp_type_perm[slot] = comp;
         }
+    }
+}
+
+// offsets_c[e] = valid rows before the first row of event e (e = 0 .. E; offsets[E] = N)
+__global__ void k_sched_offsets_c(const int* __restrict__ offsets, int E, int N, const int* __restrict__ vbefore,
+                                  const int* __restrict__ n_comp, int* __restrict__ offsets_c) {
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e <= E; e += gridDim.x * blockDim.x) {
+        const int o = offsets[e];
+        offsets_c[e] = o < N ? vbefore[o] : n_comp[0];
     }
 }
 
@@ -147,7 +178,7 @@ k_embed_l1(const float* __restrict__ X, int N, int F, int d, const float* __rest
     }
     __syncthreads();
     // pad rows -> zero residual-stream rows
-    for (int p = 0; p < cnt[0]; ++p) {
+    for (int p = 0; h && p < cnt[0]; ++p) {                  // (h == nullptr: compacted rows, pad rows do not exist there)
         int r = list[0][p];
         for (int j = threadIdx.x; j < d; j += EMB_THREADS) h[(int64_t)(row0 + r) * d + j] = 0.0f;
     }
@@ -449,20 +480,21 @@ __device__ __forceinline__ void heads_store(const HeadsOut& ho, int row, int o, 
 template <typename T>
 __global__ void __launch_bounds__(256)
 k_heads_l2(const T* __restrict__ hidden, const T* __restrict__ hidden_lo, int N, int d, int ld_hidden, const float* __restrict__ W2,
-           const float* __restrict__ b2, const int* __restrict__ valid, HeadsOut ho,
+           const float* __restrict__ b2, const int* __restrict__ valid, const int* __restrict__ hid_row, HeadsOut ho,
            float* __restrict__ out_logits, float* __restrict__ out_regress, float* __restrict__ out_binary) {
     int row = blockIdx.x * 8 + (threadIdx.x >> 5);
     int lane = threadIdx.x & 31;
     if (row >= N) return;
-    const bool ok = valid[row] != 0;
-    const T* hp = hidden + (int64_t)row * ld_hidden;
+    const int hrow = hid_row ? hid_row[row] : (valid[row] != 0 ? row : -1);   // row of `hidden` holding this element (-1: pad row)
+    const bool ok = hrow >= 0;
+    const T* hp = hidden + (int64_t)(ok ? hrow : 0) * ld_hidden;
     for (int o = 0; o < ho.n_out; ++o) {
         float a = 0.0f;
         if (ok) {
             const T* hb = hp + ho.blk[o] * d;
             const float* w = W2 + (int64_t)o * d;
             if (hidden_lo) {
-                const T* lb = hidden_lo + (int64_t)row * ld_hidden + ho.blk[o] * d;
+                const T* lb = hidden_lo + (int64_t)hrow * ld_hidden + ho.blk[o] * d;
                 for (int c = lane; c < d; c += 32) a = fmaf(to_f32<T>(hb[c]) + to_f32<T>(lb[c]), w[c], a);
             } else {
                 for (int c = lane; c < d; c += 32) a = fmaf(to_f32<T>(hb[c]), w[c], a);
@@ -479,12 +511,13 @@ k_heads_l2(const T* __restrict__ hidden, const T* __restrict__ hidden_lo, int N,
 template <int NCH>
 __global__ void __launch_bounds__(256)
 k_heads_l2_vec(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden_lo, int N, int d, int ld_hidden, int n_blk,
-               const float* __restrict__ W2, const float* __restrict__ b2, const int* __restrict__ valid, HeadsOut ho,
+               const float* __restrict__ W2, const float* __restrict__ b2, const int* __restrict__ valid, const int* __restrict__ hid_row, HeadsOut ho,
                float* __restrict__ out_logits, float* __restrict__ out_regress, float* __restrict__ out_binary) {
     const int row = blockIdx.x * 8 + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     if (row >= N) return;
-    const bool ok = valid[row] != 0;
+    const int hrow = hid_row ? hid_row[row] : (valid[row] != 0 ? row : -1);
+    const bool ok = hrow >= 0;
     uint4 hraw[MAX_HBLK][NCH], lraw[MAX_HBLK][NCH];
 #pragma unroll
     for (int b = 0; b < MAX_HBLK; ++b)
@@ -493,7 +526,7 @@ k_heads_l2_vec(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden_
             const int c = ch * 256 + lane * 8;
             hraw[b][ch] = make_uint4(0, 0, 0, 0); lraw[b][ch] = make_uint4(0, 0, 0, 0);
             if (ok && b < n_blk && c < d) {
-                const int64_t off = (int64_t)row * ld_hidden + b * d + c;
+                const int64_t off = (int64_t)hrow * ld_hidden + b * d + c;
                 hraw[b][ch] = *reinterpret_cast<const uint4*>(hidden + off);
                 if (hidden_lo) lraw[b][ch] = *reinterpret_cast<const uint4*>(hidden_lo + off);
             }
@@ -550,12 +583,13 @@ __device__ __forceinline__ float heads_dot8(const float (&h)[8], const float4& w
 template <int NCH>
 __global__ void __launch_bounds__(256)
 k_heads_l2_fold(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden_lo, int N, int d, int ld_hidden, int n_blk,
-                const float* __restrict__ W2, const float* __restrict__ b2, const int* __restrict__ valid, HeadsOut ho,
+                const float* __restrict__ W2, const float* __restrict__ b2, const int* __restrict__ valid, const int* __restrict__ hid_row, HeadsOut ho,
                 float* __restrict__ out_logits, float* __restrict__ out_regress, float* __restrict__ out_binary) {
     const int row = blockIdx.x * 8 + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     if (row >= N) return;
-    const bool ok = valid[row] != 0;                          // warp-uniform
+    const int hrow = hid_row ? hid_row[row] : (valid[row] != 0 ? row : -1);   // warp-uniform
+    const bool ok = hrow >= 0;
     float acc[16];
 #pragma unroll
     for (int o = 0; o < 16; ++o) acc[o] = 0.0f;
@@ -568,7 +602,7 @@ k_heads_l2_fold(const bf16* __restrict__ hidden, const bf16* __restrict__ hidden
                 const int c = ch * 256 + lane * 8;
                 uint4 h4 = make_uint4(0, 0, 0, 0), l4 = make_uint4(0, 0, 0, 0);
                 if (b < n_blk && c < d) {
-                    const int64_t off = (int64_t)row * ld_hidden + b * d + c;
+                    const int64_t off = (int64_t)hrow * ld_hidden + b * d + c;
                     h4 = *reinterpret_cast<const uint4*>(hidden + off);
                     if (hidden_lo) l4 = *reinterpret_cast<const uint4*>(hidden_lo + off);
                 }
@@ -647,6 +681,17 @@ __global__ void k_to_f32(const T* __restrict__ src, float* __restrict__ dst, int
     if (i < n) dst[i] = to_f32<T>(src[i]);
 }
 
+// debug tap: rows of a compacted [Nc, cols] matrix back to their original rows (pad rows -> 0)
+__global__ void k_uncompact(const float* __restrict__ src, const int* __restrict__ comp_row, float* __restrict__ out, int64_t N, int cols) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N * cols) return;
+    const int c = comp_row[i / cols];
+    out[i] = c >= 0 ? src[(int64_t)c * cols + i % cols] : 0.0f;
+}
+void launch_uncompact(const float* src, const int* comp_row, float* out, int64_t N, int cols, cudaStream_t st) {
+    k_uncompact<<<(unsigned)((N * cols + 255) / 256), 256, 0, st>>>(src, comp_row, out, N, cols);
+}
+
 // debug tap: the fused blocks' tiled residual-stream layout (tc_post.cu h_off) -> row-major
 __global__ void k_untile_h(const float* __restrict__ ht, float* __restrict__ out, int64_t N, int d) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -685,12 +730,14 @@ void launch_sched_replicate(int N, int N_pad, int E, int g, int d, int* offsets,
 // ------------------------------------------------------------------------------------------------ launchers
 int launch_schedule(const float* X, int N, int F, const int* offsets, int E, int* block_counts, int* block_base,
                     int* valid, uint32_t* valid_bits, int* row_event, int* row_pos, int* n_valid, int* type_offsets, int* sorted_row,
-                    int* type_perm, cudaStream_t st) {
+                    int* type_perm, const SchedCompact& sc, cudaStream_t st) {
     const int nb = (N + SCHED_BLOCK - 1) / SCHED_BLOCK;
     k_sched_count<<<nb, SCHED_BLOCK, 0, st>>>(X, N, F, offsets, E, block_counts, valid, valid_bits, row_event, row_pos, n_valid);
-    k_sched_scan<<<1, 32, 0, st>>>(block_counts, nb, block_base, type_offsets);
-    k_sched_scatter<<<nb, SCHED_BLOCK, 0, st>>>(X, N, F, block_base, type_offsets, sorted_row, type_perm);
-    return 3;
+    k_sched_scan<<<1, 32, 0, st>>>(block_counts, nb, block_base, type_offsets, sc.block_vbase, sc.n_comp);
+    k_sched_scatter<<<nb, SCHED_BLOCK, 0, st>>>(X, N, F, block_base, type_offsets, sc.block_vbase, row_event, sorted_row, type_perm,
+                                                sc.vbefore, sc.comp_row, sc.orig_row, sc.row_event_c, sc.comp_type_perm);
+    k_sched_offsets_c<<<1, 256, 0, st>>>(offsets, E, N, sc.vbefore, sc.n_comp, sc.offsets_c);
+    return 4;
 }
 
 void launch_embed_l1(bool fp32, const float* X, int N, int F, int d, const float* W1t, const float* b1, int act,
@@ -756,20 +803,20 @@ void launch_attn_simple(bool fp32, int hd, const void* QKV, const int* key_valid
 }
 
 void launch_heads_l2(bool fp32, const void* hidden, const void* hidden_lo, int N, int d, int ld_hidden,
-                     const float* W2, const float* b2, const int* valid, const HeadsOut& ho, float* out_logits,
+                     const float* W2, const float* b2, const int* valid, const int* hid_row, const HeadsOut& ho, float* out_logits,
                      float* out_regress, float* out_binary, cudaStream_t st) {
     dim3 grid((N + 7) / 8);
-    if (fp32) k_heads_l2<float><<<grid, 256, 0, st>>>((const float*)hidden, (const float*)hidden_lo, N, d, ld_hidden, W2, b2, valid, ho, out_logits, out_regress, out_binary);
+    if (fp32) k_heads_l2<float><<<grid, 256, 0, st>>>((const float*)hidden, (const float*)hidden_lo, N, d, ld_hidden, W2, b2, valid, hid_row, ho, out_logits, out_regress, out_binary);
     else if (d <= 512 && d % 8 == 0 && ld_hidden % 8 == 0 && ld_hidden / d <= MAX_HBLK) {
         const int n_blk = ld_hidden / d;
         if (ho.n_out <= 16) {
-            if (d <= 256) k_heads_l2_fold<1><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress, out_binary);
-            else k_heads_l2_fold<2><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress, out_binary);
+            if (d <= 256) k_heads_l2_fold<1><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, hid_row, ho, out_logits, out_regress, out_binary);
+            else k_heads_l2_fold<2><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, hid_row, ho, out_logits, out_regress, out_binary);
         }
-        else if (d <= 256) k_heads_l2_vec<1><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress, out_binary);
-        else k_heads_l2_vec<2><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, ho, out_logits, out_regress, out_binary);
+        else if (d <= 256) k_heads_l2_vec<1><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, hid_row, ho, out_logits, out_regress, out_binary);
+        else k_heads_l2_vec<2><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, n_blk, W2, b2, valid, hid_row, ho, out_logits, out_regress, out_binary);
     }
-    else k_heads_l2<bf16><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, W2, b2, valid, ho, out_logits, out_regress, out_binary);
+    else k_heads_l2<bf16><<<grid, 256, 0, st>>>((const bf16*)hidden, (const bf16*)hidden_lo, N, d, ld_hidden, W2, b2, valid, hid_row, ho, out_logits, out_regress, out_binary);
 }
 
 void launch_to_f32(bool fp32, const void* src, float* dst, int64_t n, cudaStream_t st) {

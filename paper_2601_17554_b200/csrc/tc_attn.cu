@@ -174,6 +174,7 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     const int2 it = prm.items[item];
     const int ev0 = prm.offsets[it.x], ev1 = prm.offsets[it.x + 1];
     const int q0 = ev0 + it.y * NT * ATT_BQ;                         // first query row of this CTA
+    if (q0 >= ev1) return;      // the host sized the work list from the event's row count INCLUDING pad rows (an upper bound)
     const int nt = min(NT, (ev1 - q0 + ATT_BQ - 1) / ATT_BQ);        // query tiles that hold rows of the event (>= 1)
     const int nkv = (ev1 - ev0 + ATT_BK - 1) / ATT_BK;              // 64-key tiles
     const int nst = (ev1 - ev0 + ATT_SK - 1) / ATT_SK;              // 128-key TMA stages

@@ -73,7 +73,7 @@ struct Attn2Params {
 // shared memory first.  kmax must be zeroed before the launch.
 __global__ void __launch_bounds__(256)
 k_attn_norms(const bf16* __restrict__ QKV, const int* __restrict__ row_event, int N, int H, int hd, int d,
-             float* __restrict__ qn, float* __restrict__ kmax) {
+             const int* __restrict__ nc_dev, int group_rows, float* __restrict__ qn, float* __restrict__ kmax) {
     __shared__ int smax[64];
     __shared__ int ev_first;
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
@@ -81,7 +81,10 @@ k_attn_norms(const bf16* __restrict__ QKV, const int* __restrict__ row_event, in
     if (threadIdx.x < 64) smax[threadIdx.x] = 0;
     if (threadIdx.x == 0) ev_first = row_event[min(row, N - 1)];
     __syncthreads();
-    if (row < N) {
+    // pad-row compaction: rows at or beyond the number of meaningful rows (of their stack) hold stale data and stale event
+    // ids: they must not leak into kmax (the bound, and with it the rounding of P, would depend on the buffer's history)
+    const int nc = nc_dev ? __ldg(nc_dev) : 0x7fffffff;
+    if (row < N && (group_rows > 0 ? row % group_rows : row) < nc) {
         const uint4* qp = reinterpret_cast<const uint4*>(QKV + (int64_t)row * 3 * d + h * hd);
         const uint4* kp = reinterpret_cast<const uint4*>(QKV + (int64_t)row * 3 * d + d + h * hd);
         float sq = 0.f, sk = 0.f;
@@ -167,6 +170,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
     const int2 it = prm.items[item];
     const int ev0 = prm.offsets[it.x], ev1 = prm.offsets[it.x + 1];
     const int q0 = ev0 + it.y * NT * A2_BQ;
+    if (q0 >= ev1) return;      // the host sized the work list from the event's row count INCLUDING pad rows (an upper bound)
     const int nt = min(NT, (ev1 - q0 + A2_BQ - 1) / A2_BQ);
     const int nkv = (ev1 - ev0 + A2_BK - 1) / A2_BK;
     const int nst = (ev1 - ev0 + A2_SK - 1) / A2_SK;
@@ -442,12 +446,12 @@ static int tc_attn2_launch_hd(TcContext* c, const bf16* QKV, int64_t N, Attn2Par
 // norms pre-pass + attention.  qn [N, H] and kmax [E, H] are caller-owned scratch; row_event [N] from the schedule.
 int tc_attn2_launch(TcContext* c, const bf16* QKV, int64_t N, int E, const uint32_t* valid_bits, const int* n_valid,
                     const int* offsets, const int* row_event, const int2* items, int n_items, int d, int H, float* qn,
-                    float* kmax, bf16* O, bf16* O_lo, int force_exact, cudaStream_t st) {
+                    float* kmax, bf16* O, bf16* O_lo, int force_exact, const int* nc_dev, int group_rows, cudaStream_t st) {
     const int hd = d / H;
     if (H > 64) { snprintf(c->err, sizeof c->err, "tc_attn2: more than 64 heads"); return -1; }
     cudaMemsetAsync(kmax, 0, (size_t)E * H * 4, st);
     const int64_t nthr = N * H;
-    k_attn_norms<<<(unsigned)((nthr + 255) / 256), 256, 0, st>>>(QKV, row_event, (int)N, H, hd, d, qn, kmax);
+    k_attn_norms<<<(unsigned)((nthr + 255) / 256), 256, 0, st>>>(QKV, row_event, (int)N, H, hd, d, nc_dev, group_rows, qn, kmax);
     Attn2Params prm;
     prm.valid_bits = valid_bits; prm.n_valid = n_valid; prm.offsets = offsets; prm.items = items; prm.n_items = n_items;
     prm.qn = qn; prm.kmax = kmax; prm.H = H; prm.d = d; prm.O = O; prm.O_lo = O_lo; prm.force_exact = force_exact;

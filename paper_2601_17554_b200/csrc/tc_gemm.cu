@@ -188,6 +188,9 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     const int n_tiles_n = N / BLOCK_N;
     const int total_tiles = ((M + GEMM_BM - 1) / GEMM_BM) * n_tiles_n;
     const int m_end = ep.group_offsets ? ep.group_offsets[ep.n_groups + 1] : M;   // grouped: rows beyond the last group
+    const int nc_rows = ep.nc_dev ? __ldg(ep.nc_dev) : 0x7fffffff;
+    // tiles without meaningful rows (all three roles skip the same ones)
+    auto skip_tile = [&](int m0) { return m0 >= m_end || (ep.group_rows > 0 ? m0 % ep.group_rows : m0) >= nc_rows; };
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_full = ptx::smem_u32(&bars[0]);
     const uint32_t bar_empty = ptx::smem_u32(&bars[STAGES]);
@@ -217,7 +220,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         uint32_t kbg = 0;
         for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
             const int m0 = (tile / n_tiles_n) * GEMM_BM, n0 = (tile % n_tiles_n) * BLOCK_N;
-            if (m0 >= m_end) continue;
+            if (skip_tile(m0)) continue;
             int w_row0 = 0;
             if (ep.group_offsets) {                               // grouped GEMM (per-type embedding weights)
                 int g = 1;
@@ -243,7 +246,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         uint32_t kbg = 0;
         int it = 0;
         for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-            if ((tile / n_tiles_n) * GEMM_BM >= m_end) continue;
+            if (skip_tile((tile / n_tiles_n) * GEMM_BM)) continue;
             const int buf = it & 1;
             ptx::mbar_wait(bar_acc_empty + 8 * buf, ((it >> 1) & 1) ^ 1);      // the epilogue drained this buffer
             ptx::tc_fence_after();
@@ -277,7 +280,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         int it = 0;
         for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
             const int m0 = (tile / n_tiles_n) * GEMM_BM, n0 = (tile % n_tiles_n) * BLOCK_N;
-            if (m0 >= m_end) continue;
+            if (skip_tile(m0)) continue;
             if ((it & 1) != e) { ++it; continue; }
             int w_row0 = 0;
             if (ep.group_offsets) {

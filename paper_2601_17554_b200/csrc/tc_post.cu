@@ -45,6 +45,7 @@ struct PostCfg {
 
 struct PostParams {
     int M, dff, group_rows;
+    const int* nc_dev;              // meaningful rows (per group), device, may be null: tiles at or beyond it are skipped
     const float *bo, *ln2g, *ln2b, *b1, *b2, *lnng, *lnnb;   // per group: D, D, D, dff, D, D, D floats
     float eps;
     float* h;                       // [M, D] fp32 residual stream, updated in place
@@ -117,6 +118,8 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
     const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
     const int n_tiles = (p.M + POST_BM - 1) / POST_BM;
     const int NC = p.dff / POST_CH;
+    const int nc_rows = p.nc_dev ? __ldg(p.nc_dev) : 0x7fffffff;
+    auto skip_tile = [&](int tile) { return (tile * POST_BM) % p.group_rows >= nc_rows; };   // all three roles skip the same tiles
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* const smem_gen = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
     const uint32_t sA = smem_base, sRing = sA + Cfg::A_BYTES;
@@ -159,8 +162,10 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
             __syncwarp();
             ++slot_it;
         };
-        int it = 0;
-        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        int it = -1;
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            if (skip_tile(tile)) continue;
+            ++it;
             const int m0 = tile * POST_BM, g = m0 / p.group_rows;
             if (it > 0) ptx::mbar_wait(bar_a_free, (it - 1) & 1);        // the last tile's u2 is no longer read
             if (lane == 0) {
@@ -197,8 +202,10 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
             return sRing + s * POST_SLOT;
         };
         auto free_slot = [&]() { ptx::mma_commit(bar_empty + 8 * (slot_it % NS)); ++slot_it; };
-        int it = 0;
-        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        int it = -1;
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            if (skip_tile(tile)) continue;
+            ++it;
             ptx::mbar_wait(bar_a_full, it & 1);
             if (it > 0) ptx::mbar_wait(bar_acc_free, (it - 1) & 1);      // the last tile's final epilogue drained acc
             ptx::tc_fence_after();
@@ -270,7 +277,7 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
         float* const v_b2 = vec + 3 * D; float* const v_gn = vec + 4 * D; float* const v_bn = vec + 5 * D;
         float* const v_b1 = vec + 6 * D;
         uint32_t ph_s = 0;
-        int it = 0;
+        int it = -1;
         // mean and 1/sigma of the row from the four column groups' partials (each over CW columns)
         auto row_stats = [&](float n, float mean, float m2, float& mu, float& rstd) {
             part[cg * POST_BM + r] = make_float2(mean, m2);
@@ -286,7 +293,9 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
             mu = tm;
             rstd = rsqrtf(t2 * (1.0f / D) + p.eps);
         };
-        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            if (skip_tile(tile)) continue;
+            ++it;
             const int m0 = tile * POST_BM, g = m0 / p.group_rows;
             const int row = m0 + r;
             const bool row_ok = row < p.M;
@@ -476,7 +485,7 @@ static int tc_post_launch_t(TcContext* c, const PostArgs& a, cudaStream_t st) {
     const int smem = Cfg::smem_bytes(a.dff);
     if (tc_set_smem_attr(c, (const void*)kern, 232448 - 1024)) return -1;   // upper bound once per device; dff varies per model
     PostParams p;
-    p.M = a.M; p.dff = a.dff; p.group_rows = a.group_rows > 0 ? a.group_rows : 0x7fffff80;
+    p.M = a.M; p.dff = a.dff; p.group_rows = a.group_rows > 0 ? a.group_rows : 0x7fffff80; p.nc_dev = a.nc_dev;
     p.bo = a.bo; p.ln2g = a.ln2g; p.ln2b = a.ln2b; p.b1 = a.b1; p.b2 = a.b2; p.lnng = a.lnng; p.lnnb = a.lnnb;
     p.eps = a.eps; p.h = a.h; p.h_in_tiled = a.h_in_tiled; p.h_out_tiled = a.h_out_tiled; p.u_out = a.u_out; p.u_out_lo = a.u_out_lo; p.next_ln = a.next_ln;
     p.dbg_u2 = a.dbg_u2; p.dbg_g = a.dbg_g;

@@ -88,7 +88,8 @@ def test_schedule_bit_exact(lens, pad, tile_q):
     mod.set_option(P.OPT_TAP_LAYER, -2)
     mod.infer(torch.from_numpy(X).cuda(), off)
     ref = oracle.schedule(X, off, tile_q)
-    for k in ("row_event", "row_pos", "valid", "n_valid", "type_offsets", "sorted_row", "type_perm", "work_list"):
+    for k in ("row_event", "row_pos", "valid", "n_valid", "type_offsets", "sorted_row", "type_perm", "work_list",
+              "comp_row", "offsets_c", "comp_type_perm"):
         got = mod.schedule(k)
         assert got.dtype == np.int32
         np.testing.assert_array_equal(got, ref[k], err_msg=k)
