@@ -105,6 +105,15 @@ int mlpf_infer_host(mlpf_handle* h, const float* elements_host, const int32_t* e
 int mlpf_infer_ex(mlpf_handle* h, const float* elements, const int32_t* event_offsets, int32_t n_events,
                   float* out_logits, float* out_regress, float* out_binary, void* stream);
 
+/* mlpf_infer_host_async / mlpf_host_sync: the same as mlpf_infer_host without the final synchronisation.  The H2D copy runs
+ * on a copy-in stream of the library, the kernels on `stream`, the D2H copies on a copy-out stream, chained by events; two
+ * device staging slots alternate, so with several calls in flight the copies of one call overlap the kernels of its
+ * neighbours (the paper's "asynchronous ... execution", L232).  The host buffers of a call must stay valid and untouched
+ * until mlpf_host_sync(h, stream) returns (it waits for every call issued on that stream so far). */
+int mlpf_infer_host_async(mlpf_handle* h, const float* elements_host, const int32_t* event_offsets, int32_t n_events,
+                          float* out_logits_host, float* out_regress_host, void* stream);
+int mlpf_host_sync(mlpf_handle* h, void* stream);
+
 void mlpf_destroy(mlpf_handle* h);
 
 /* Thread-local text of the last error raised on this thread ("" if none). */
@@ -174,6 +183,9 @@ int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* 
 #define MLPF_OPT_COMPACT     10  /* 1 (default): pad rows (type 0) are dropped after a0: every later step runs on the compacted rows
                                     (events stay contiguous, oracle.schedule comp_row / offsets_c), outputs are scattered back;
                                     0: pad rows stay in place and are masked as keys (round 1's behaviour)                   */
+#define MLPF_OPT_GRAPH       11  /* 1: a forward pass whose key (pointers, sizes, event_offsets, options) repeats is captured into a
+                                    CUDA graph on its second occurrence and replayed afterwards (one launch per call: the
+                                    one-event-per-call mode of PAPER.md L224); 0 (default): plain launches                   */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0

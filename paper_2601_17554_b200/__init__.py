@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmlpf.so")
 
 # include/mlpf.h constants
 OK = 0
-OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE, OPT_FUSE, OPT_ATTN, OPT_ATTN_POLY, OPT_COMPACT = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
+OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE, OPT_FUSE, OPT_ATTN, OPT_ATTN_POLY, OPT_COMPACT, OPT_GRAPH = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11
 PREC_BF16, PREC_FP32_DEBUG = 0, 1
 KERNELS_TC, KERNELS_SIMPLE = 0, 1
 Q_N_LAYERS, Q_D_MODEL, Q_N_HEADS, Q_D_FF, Q_N_FEAT, Q_N_CLASSES, Q_N_REGRESS = 1, 2, 3, 4, 5, 6, 7
@@ -27,7 +27,8 @@ TENSOR = dict(H=0, U=1, QK=2, V=3, O=4, G=5)
 KERNEL_CLASSES = ["sched", "embed_l1", "embed_l2", "layernorm", "qkv", "attention", "outproj", "ffn1", "ffn2",
                   "heads_l1", "heads_l2", "post"]
 
-EXPORTS = ["mlpf_create", "mlpf_infer", "mlpf_infer_ex", "mlpf_build_candidates_ex", "mlpf_infer_host", "mlpf_destroy", "mlpf_last_error", "mlpf_set_option",
+EXPORTS = ["mlpf_create", "mlpf_infer", "mlpf_infer_ex", "mlpf_build_candidates_ex", "mlpf_infer_host", "mlpf_infer_host_async",
+           "mlpf_host_sync", "mlpf_destroy", "mlpf_last_error", "mlpf_set_option",
            "mlpf_query", "mlpf_debug_get_schedule", "mlpf_debug_get_tensor", "mlpf_debug_get_profile", "mlpf_tc_gemm_bf16",
            "mlpf_tc_attention_bf16", "mlpf_debug_set_attention_impl", "mlpf_tc_post_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates"]
 
@@ -54,6 +55,10 @@ def lib():
     L.mlpf_build_candidates_ex.argtypes = [vp, i32, vp, i32, vp, i32, vp, i32, vp, vp, i64, vp, vp, vp, vp, vp]
     L.mlpf_infer_host.restype = C.c_int
     L.mlpf_infer_host.argtypes = [vp, vp, vp, i32, vp, vp, vp]
+    L.mlpf_infer_host_async.restype = C.c_int
+    L.mlpf_infer_host_async.argtypes = [vp, vp, vp, i32, vp, vp, vp]
+    L.mlpf_host_sync.restype = C.c_int
+    L.mlpf_host_sync.argtypes = [vp, vp]
     L.mlpf_destroy.restype = None
     L.mlpf_destroy.argtypes = [vp]
     L.mlpf_last_error.restype = C.c_char_p
@@ -172,6 +177,17 @@ class Mlpf:
                                      off.ctypes.data_as(C.c_void_p), len(off) - 1,
                                      C.c_void_p(out_logits_host.data_ptr()),
                                      C.c_void_p(out_regress_host.data_ptr()), _stream_ptr(stream)))
+
+    def infer_host_async(self, elements_host, event_offsets, out_logits_host, out_regress_host, stream=None):
+        """As infer_host without the final synchronisation (call host_sync before reading the outputs)."""
+        off = np.ascontiguousarray(event_offsets, dtype=np.int32)
+        _check(lib().mlpf_infer_host_async(self._h, C.c_void_p(elements_host.data_ptr()),
+                                           off.ctypes.data_as(C.c_void_p), len(off) - 1,
+                                           C.c_void_p(out_logits_host.data_ptr()),
+                                           C.c_void_p(out_regress_host.data_ptr()), _stream_ptr(stream)))
+
+    def host_sync(self, stream=None):
+        _check(lib().mlpf_host_sync(self._h, _stream_ptr(stream)))
 
     def schedule(self, which: str, stream=None):
         cap = 1 << 22

@@ -62,9 +62,21 @@ struct Workspace {
     SchedCompact sc = {};                    // pad-row compaction arrays (a0)
     bool compact = false;                    // the last call ran on compacted rows
     float *qn = nullptr, *kmax = nullptr;   // attention norms pre-pass: |q_i| per row and head, max |k_j| per event and head
-    // device staging of mlpf_infer_host (owned by the stream's workspace, freed with it); capacities in BYTES
-    float *stage_x = nullptr, *stage_lg = nullptr, *stage_rg = nullptr;
-    int64_t stage_cap = 0;            // rows
+    // device staging of mlpf_infer_host[_async] (owned by the stream's workspace, freed with it): two slots, so that the
+    // copies of one call overlap the kernels of the next; h2d_st / d2h_st are the library's own copy streams
+    struct HostSlot { float *x = nullptr, *lg = nullptr, *rg = nullptr; int64_t cap = 0; cudaEvent_t h2d = nullptr, comp = nullptr, d2h = nullptr; };
+    HostSlot slot[2];
+    cudaStream_t h2d_st = nullptr, d2h_st = nullptr;
+    uint64_t host_calls = 0;
+    // pinned staging of the host-built lists (offsets, work lists): a ring, each entry guarded by an event, so that
+    // mlpf_infer never copies from pageable memory (which would stage synchronously and cannot be graph-captured)
+    struct ListSlot { int* p = nullptr; int64_t cap = 0; cudaEvent_t done = nullptr; };
+    ListSlot lists[4];
+    uint64_t list_calls = 0;
+    // CUDA graphs of whole forward passes (MLPF_OPT_GRAPH), keyed by everything a replay bakes in
+    struct GraphEntry { std::vector<int32_t> key; cudaGraphExec_t exec = nullptr; int* lists = nullptr; int launches = 0; uint64_t last_use = 0; };
+    std::vector<GraphEntry> graphs;
+    std::vector<std::vector<int32_t>> seen_keys;
     // per-kernel-class CUDA-event timing of the last call (MLPF_OPT_PROFILE)
     std::vector<int> host_work, host_pairs;   // host copies of the work lists of the last call
     std::vector<cudaEvent_t> ev_pool;
@@ -92,7 +104,7 @@ struct mlpf_handle {
     std::vector<LayerW> layers;
     HeadsOut ho;
     // options
-    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1;
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1, graph = 0;
     int64_t last_launches = 0;
     std::mutex mu;
     std::map<void*, Workspace*> ws;
@@ -265,6 +277,9 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_ATTN:
             if (value < 0 || value > 2) return set_err(MLPF_E_ARG, "attn must be 0, 1 or 2");
             h->attn = (int)value; return MLPF_OK;
+        case MLPF_OPT_GRAPH:
+            if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "graph must be 0 or 1");
+            h->graph = (int)value; return MLPF_OK;
         case MLPF_OPT_COMPACT:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "compact must be 0 or 1");
             h->compact = (int)value; return MLPF_OK;
@@ -403,8 +418,16 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
 
 static void ws_free(Workspace* w) {
     ws_free_rows(w);
-    dfree(w->stage_x); dfree(w->stage_lg); dfree(w->stage_rg);
-    w->stage_cap = 0;
+    for (auto& sl : w->slot) {
+        dfree(sl.x); dfree(sl.lg); dfree(sl.rg); sl.cap = 0;
+        if (sl.h2d) cudaEventDestroy(sl.h2d); if (sl.comp) cudaEventDestroy(sl.comp); if (sl.d2h) cudaEventDestroy(sl.d2h);
+        sl.h2d = sl.comp = sl.d2h = nullptr;
+    }
+    if (w->h2d_st) cudaStreamDestroy(w->h2d_st); if (w->d2h_st) cudaStreamDestroy(w->d2h_st);
+    w->h2d_st = w->d2h_st = nullptr;
+    for (auto& ls : w->lists) { if (ls.p) cudaFreeHost(ls.p); if (ls.done) cudaEventDestroy(ls.done); ls.p = nullptr; ls.done = nullptr; ls.cap = 0; }
+    for (auto& g : w->graphs) { if (g.exec) cudaGraphExecDestroy(g.exec); if (g.lists) cudaFreeHost(g.lists); }
+    w->graphs.clear(); w->seen_keys.clear();
     dfree(w->offsets); dfree(w->n_valid); dfree(w->work); dfree(w->pairs); dfree(w->kmax); dfree(w->sc.offsets_c);
     for (cudaEvent_t e : w->ev_pool) cudaEventDestroy(e);
     w->ev_pool.clear();
@@ -734,12 +757,84 @@ extern "C" int mlpf_infer_ex(mlpf_handle* h, const float* elements, const int32_
     w->tile_q = h->tile_q;
     w->m_ub = (N + 127) / 128 * 128 + 4 * 128;
     h->last_launches = 0;
-    // pageable -> device async copies are staged by the runtime before returning: the caller may free event_offsets;
-    // the work lists live in the workspace (the copies may still be reading them after this call returns on other paths)
-    CUDA_TRY(cudaMemcpyAsync(w->offsets, event_offsets, (size_t)(n_events + 1) * 4, cudaMemcpyHostToDevice, st));
-    if (!work.empty()) CUDA_TRY(cudaMemcpyAsync(w->work, work.data(), work.size() * 4, cudaMemcpyHostToDevice, st));
-    if (!pairs.empty()) CUDA_TRY(cudaMemcpyAsync(w->pairs, pairs.data(), pairs.size() * 4, cudaMemcpyHostToDevice, st));
-    rc = infer_impl(h, fp32, w, elements, out_logits, out_regress, out_binary, st);
+    // the host-built lists go through a pinned ring slot (one H2D copy; the caller may free event_offsets on return)
+    const size_t n_off = (size_t)n_events + 1, n_work = work.size(), n_pairs = pairs.size();
+    Workspace::ListSlot& ls = w->lists[w->list_calls++ % 4];
+    if (!ls.done) CUDA_TRY(cudaEventCreateWithFlags(&ls.done, cudaEventDisableTiming));
+    else CUDA_TRY(cudaEventSynchronize(ls.done));                        // the copy that last used this slot has run
+    if ((int64_t)(n_off + n_work + n_pairs) > ls.cap) {
+        if (ls.p) cudaFreeHost(ls.p);
+        ls.p = nullptr; ls.cap = 0;
+        const int64_t cap = (int64_t)(n_off + n_work + n_pairs) * 2 + 1024;
+        if (cudaMallocHost(&ls.p, (size_t)cap * 4) != cudaSuccess) return set_err(MLPF_E_ALLOC, "pinned staging allocation failed");
+        ls.cap = cap;
+    }
+    memcpy(ls.p, event_offsets, n_off * 4);
+    if (n_work) memcpy(ls.p + n_off, work.data(), n_work * 4);
+    if (n_pairs) memcpy(ls.p + n_off + n_work, pairs.data(), n_pairs * 4);
+    auto enqueue = [&](const int* lists) -> int {
+        CUDA_TRY(cudaMemcpyAsync(w->offsets, lists, n_off * 4, cudaMemcpyHostToDevice, st));
+        if (n_work) CUDA_TRY(cudaMemcpyAsync(w->work, lists + n_off, n_work * 4, cudaMemcpyHostToDevice, st));
+        if (n_pairs) CUDA_TRY(cudaMemcpyAsync(w->pairs, lists + n_off + n_work, n_pairs * 4, cudaMemcpyHostToDevice, st));
+        return infer_impl(h, fp32, w, elements, out_logits, out_regress, out_binary, st);
+    };
+    // MLPF_OPT_GRAPH: a call whose key (pointers, sizes, offsets, options) was seen before is captured into a CUDA graph the
+    // second time and replayed from then on: one launch instead of ~25 (the one-event-per-call mode of PAPER.md L224)
+    const bool graph_ok = h->graph && !h->profile && h->tap_layer == -1 && st != nullptr;
+    if (graph_ok) {
+        std::vector<int32_t> key;
+        auto push64 = [&](uint64_t v) { key.push_back((int32_t)(v & 0xffffffffu)); key.push_back((int32_t)(v >> 32)); };
+        push64((uint64_t)(uintptr_t)elements); push64((uint64_t)(uintptr_t)out_logits); push64((uint64_t)(uintptr_t)out_regress);
+        push64((uint64_t)(uintptr_t)out_binary);
+        key.push_back(h->precision); key.push_back(h->kernels); key.push_back(h->split); key.push_back(h->fuse);
+        key.push_back(h->attn); key.push_back(h->compact); key.push_back(h->tile_q); key.push_back(g_attn2_poly_every);
+        key.insert(key.end(), event_offsets, event_offsets + n_off);
+        for (auto& ge : w->graphs)
+            if (ge.key == key) {
+                ge.last_use = w->list_calls;
+                CUDA_TRY(cudaGraphLaunch(ge.exec, st));
+                CUDA_TRY(cudaEventRecord(ls.done, st));
+                h->last_launches = ge.launches;
+                g_err.clear();
+                return MLPF_OK;
+            }
+        bool seen = false;
+        for (auto& k : w->seen_keys) if (k == key) { seen = true; break; }
+        if (seen) {
+            // the graph's copy nodes read the lists from a pinned buffer of their own (its content is a function of the key)
+            Workspace::GraphEntry ge;
+            if (cudaMallocHost(&ge.lists, (n_off + n_work + n_pairs) * 4) != cudaSuccess) return set_err(MLPF_E_ALLOC, "pinned staging allocation failed");
+            memcpy(ge.lists, ls.p, (n_off + n_work + n_pairs) * 4);
+            cudaGraph_t graph = nullptr;
+            cudaError_t ce = cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal);
+            if (ce != cudaSuccess) { cudaFreeHost(ge.lists); return set_err(MLPF_E_CUDA, "graph capture failed: %s", cudaGetErrorString(ce)); }
+            rc = enqueue(ge.lists);
+            ce = cudaStreamEndCapture(st, &graph);
+            if (rc) { if (graph) cudaGraphDestroy(graph); cudaFreeHost(ge.lists); return rc; }
+            if (ce != cudaSuccess) { cudaFreeHost(ge.lists); return set_err(MLPF_E_CUDA, "graph capture failed: %s", cudaGetErrorString(ce)); }
+            ce = cudaGraphInstantiate(&ge.exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (ce != cudaSuccess) { cudaFreeHost(ge.lists); return set_err(MLPF_E_CUDA, "graph instantiation failed: %s", cudaGetErrorString(ce)); }
+            ge.key = key; ge.launches = (int)h->last_launches; ge.last_use = w->list_calls;
+            if (w->graphs.size() >= 64) {                                // evict the least recently used graph
+                size_t v = 0;
+                for (size_t i = 1; i < w->graphs.size(); ++i) if (w->graphs[i].last_use < w->graphs[v].last_use) v = i;
+                cudaStreamSynchronize(st);                               // a replay of the victim may still be in flight
+                cudaGraphExecDestroy(w->graphs[v].exec);
+                cudaFreeHost(w->graphs[v].lists);
+                w->graphs.erase(w->graphs.begin() + v);
+            }
+            w->graphs.push_back(ge);
+            CUDA_TRY(cudaGraphLaunch(ge.exec, st));
+            CUDA_TRY(cudaEventRecord(ls.done, st));
+            g_err.clear();
+            return MLPF_OK;
+        }
+        if (w->seen_keys.size() >= 256) w->seen_keys.clear();
+        w->seen_keys.push_back(key);
+    }
+    rc = enqueue(ls.p);
+    cudaEventRecord(ls.done, st);
     if (rc == MLPF_OK) g_err.clear();
     return rc;
 }
@@ -749,41 +844,80 @@ extern "C" int mlpf_infer(mlpf_handle* h, const float* elements, const int32_t* 
     return mlpf_infer_ex(h, elements, event_offsets, n_events, out_logits, out_regress, nullptr, stream);
 }
 
-extern "C" int mlpf_infer_host(mlpf_handle* h, const float* elements_host, const int32_t* event_offsets,
-                               int32_t n_events, float* out_logits_host, float* out_regress_host, void* stream) {
+// Pipelined end-to-end entry: H2D of the elements on the library's copy-in stream, the forward pass on `stream`, D2H of the
+// outputs on the copy-out stream, chained by events; two staging slots alternate, so the copies of one call overlap the
+// kernels of its neighbours.  Returns after enqueueing; mlpf_host_sync waits for everything issued so far.
+extern "C" int mlpf_infer_host_async(mlpf_handle* h, const float* elements_host, const int32_t* event_offsets,
+                                     int32_t n_events, float* out_logits_host, float* out_regress_host, void* stream) {
     if (!h) return set_err(MLPF_E_NULL, "handle is NULL");
     if (n_events <= 0 || !event_offsets) return mlpf_infer(h, nullptr, event_offsets, n_events, nullptr, nullptr, stream);
     const int64_t N = event_offsets[n_events];
     if (N <= 0) return mlpf_infer(h, nullptr, event_offsets, n_events, nullptr, nullptr, stream);
     if (!elements_host || !out_logits_host || !out_regress_host) return set_err(MLPF_E_NULL, "host buffers NULL");
     cudaStream_t st = (cudaStream_t)stream;
-    // device staging buffers live in this stream's workspace (sized by this handle's F, C, R; freed by mlpf_destroy)
-    struct { float* x; float* lg; float* rg; } sb;
+    Workspace* w;
+    Workspace::HostSlot* sl;
     {
         std::lock_guard<std::mutex> lk(h->mu);
         Workspace*& wref = h->ws[stream];
         if (!wref) wref = new Workspace();
-        Workspace* w = wref;
-        if (N > w->stage_cap) {
-            dfree(w->stage_x); dfree(w->stage_lg); dfree(w->stage_rg);
-            w->stage_cap = 0;
+        w = wref;
+        if (!w->h2d_st) {
+            CUDA_TRY(cudaStreamCreateWithFlags(&w->h2d_st, cudaStreamNonBlocking));
+            CUDA_TRY(cudaStreamCreateWithFlags(&w->d2h_st, cudaStreamNonBlocking));
+        }
+        sl = &w->slot[w->host_calls++ & 1];
+        if (!sl->h2d) {
+            CUDA_TRY(cudaEventCreateWithFlags(&sl->h2d, cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&sl->comp, cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&sl->d2h, cudaEventDisableTiming));
+        }
+        if (N > sl->cap) {
+            cudaEventSynchronize(sl->d2h);
+            dfree(sl->x); dfree(sl->lg); dfree(sl->rg);
+            sl->cap = 0;
             const int64_t cap = (N + 1023) / 1024 * 1024;
-            if (cudaMalloc(&w->stage_x, cap * h->F * 4) || cudaMalloc(&w->stage_lg, cap * h->C * 4) ||
-                cudaMalloc(&w->stage_rg, cap * std::max(h->R, 1) * 4)) {
-                dfree(w->stage_x); dfree(w->stage_lg); dfree(w->stage_rg);
+            if (cudaMalloc(&sl->x, cap * h->F * 4) || cudaMalloc(&sl->lg, cap * h->C * 4) || cudaMalloc(&sl->rg, cap * std::max(h->R, 1) * 4)) {
+                dfree(sl->x); dfree(sl->lg); dfree(sl->rg);
                 return set_err(MLPF_E_ALLOC, "staging allocation failed");
             }
-            w->stage_cap = cap;
+            sl->cap = cap;
         }
-        sb.x = w->stage_x; sb.lg = w->stage_lg; sb.rg = w->stage_rg;
     }
-    CUDA_TRY(cudaMemcpyAsync(sb.x, elements_host, (size_t)N * h->F * 4, cudaMemcpyHostToDevice, st));
-    int rc = mlpf_infer(h, sb.x, event_offsets, n_events, sb.lg, sb.rg, stream);
+    // the slot's previous outputs must have left (d2h) before its input buffer is overwritten and its outputs rewritten
+    CUDA_TRY(cudaStreamWaitEvent(w->h2d_st, sl->d2h, 0));
+    CUDA_TRY(cudaMemcpyAsync(sl->x, elements_host, (size_t)N * h->F * 4, cudaMemcpyHostToDevice, w->h2d_st));
+    CUDA_TRY(cudaEventRecord(sl->h2d, w->h2d_st));
+    CUDA_TRY(cudaStreamWaitEvent(st, sl->h2d, 0));
+    CUDA_TRY(cudaStreamWaitEvent(st, sl->d2h, 0));
+    int rc = mlpf_infer(h, sl->x, event_offsets, n_events, sl->lg, sl->rg, stream);
     if (rc) return rc;
-    CUDA_TRY(cudaMemcpyAsync(out_logits_host, sb.lg, (size_t)N * h->C * 4, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaMemcpyAsync(out_regress_host, sb.rg, (size_t)N * h->R * 4, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
+    CUDA_TRY(cudaEventRecord(sl->comp, st));
+    CUDA_TRY(cudaStreamWaitEvent(w->d2h_st, sl->comp, 0));
+    CUDA_TRY(cudaMemcpyAsync(out_logits_host, sl->lg, (size_t)N * h->C * 4, cudaMemcpyDeviceToHost, w->d2h_st));
+    CUDA_TRY(cudaMemcpyAsync(out_regress_host, sl->rg, (size_t)N * h->R * 4, cudaMemcpyDeviceToHost, w->d2h_st));
+    CUDA_TRY(cudaEventRecord(sl->d2h, w->d2h_st));
     return MLPF_OK;
+}
+
+extern "C" int mlpf_host_sync(mlpf_handle* h, void* stream) {
+    if (!h) return set_err(MLPF_E_NULL, "handle is NULL");
+    Workspace* w = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(h->mu);
+        auto it = h->ws.find(stream);
+        if (it != h->ws.end()) w = it->second;
+    }
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+    if (w && w->d2h_st) { CUDA_TRY(cudaStreamSynchronize(w->d2h_st)); CUDA_TRY(cudaStreamSynchronize(w->h2d_st)); }
+    return MLPF_OK;
+}
+
+extern "C" int mlpf_infer_host(mlpf_handle* h, const float* elements_host, const int32_t* event_offsets,
+                               int32_t n_events, float* out_logits_host, float* out_regress_host, void* stream) {
+    int rc = mlpf_infer_host_async(h, elements_host, event_offsets, n_events, out_logits_host, out_regress_host, stream);
+    if (rc) return rc;
+    return mlpf_host_sync(h, stream);
 }
 
 // ------------------------------------------------------------------------------------------------ candidate building

@@ -376,3 +376,51 @@ def test_two_stack_fp32_debug_one_event():
     m = synth.model_cfg(name)
     X, off = synth.make_named_events(name, max_events=1)
     _two_stack_check(synth.make_weights(name), m, X, off, P.PREC_FP32_DEBUG, TOL_FP32)
+
+
+# ------------------------------------------------------------------------------------------- NEXT-4: latency / pipelined entries
+def test_graph_replay_is_bitwise_identical():
+    """MLPF_OPT_GRAPH: the second call with the same key is captured, later ones replayed; other events in between get
+    graphs of their own; results are bitwise those of plain launches."""
+    name = "cfg2"
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    X, off = synth.make_named_events(name, max_events=4)
+    mod = P.Mlpf(W, m)
+    Xd = torch.from_numpy(X).cuda()
+    st = torch.cuda.Stream()
+    N = X.shape[0]
+    lg = torch.empty((N, 9), device="cuda"); rg = torch.empty((N, 5), device="cuda")
+    ref = [t.clone() for t in mod.infer(Xd, off)]
+    torch.cuda.synchronize()
+    mod.set_option(P.OPT_GRAPH, 1)
+    with torch.cuda.stream(st):
+        for rep in range(4):                               # eager, capture, replay, replay -- per event
+            for e in range(4):
+                a, b = int(off[e]), int(off[e + 1])
+                lg[a:b].zero_(); rg[a:b].zero_()
+                mod.infer(Xd[a:b], np.array([0, b - a], np.int32), lg[a:b], rg[a:b], stream=st)
+            st.synchronize()
+            assert torch.equal(lg, ref[0]) and torch.equal(rg, ref[1]), rep
+    assert mod.query(P.Q_LAUNCHES) > 0
+
+
+def test_pipelined_host_entry_matches_synchronous_calls():
+    name = "cfg2"
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    mod = P.Mlpf(W, m)
+    st = torch.cuda.Stream()
+    batches = []
+    for k in range(5):
+        X, off = synth.make_events((300 + 50 * k, 517, 64 * k + 1), seed=50 + k, pad_frac=0.1)
+        xh = torch.from_numpy(X).pin_memory()
+        N = X.shape[0]
+        batches.append((xh, off, torch.empty((N, 9)).pin_memory(), torch.empty((N, 5)).pin_memory(), X))
+    for xh, off, lh, rh, X in batches:                     # all five in flight, one synchronisation at the end
+        mod.infer_host_async(xh, off, lh, rh, stream=st)
+    mod.host_sync(stream=st)
+    for xh, off, lh, rh, X in batches:
+        lg, rg = mod.infer(torch.from_numpy(X).cuda(), off)
+        torch.cuda.synchronize()
+        assert torch.equal(lh, lg.cpu()) and torch.equal(rh, rg.cpu())
