@@ -390,38 +390,73 @@ def run_ours(args):
                  "ms_p50": float(np.percentile(mt, 50)), "ms_p90": float(np.percentile(mt, 90)),
                  "workspace_bytes_all_streams": int(mod.query(P.Q_WORKSPACE_BYTES))}
 
-    # ---- roofline of the dominant kernel (a4 attention): algorithmic FLOPs per launch / mean launch duration
+    # ---- roofline of the dominant kernel (a4 attention): algorithmic FLOPs per launch / mean launch duration.
+    # The class time includes the norms pre-pass (one small launch per layer); launches = layers.
     at_ms, at_n = cls["attention"]
-    per_launch_s = at_ms * 1e-3 / max(at_n, 1)
-    achieved = fl["attn_per_launch"] / per_launch_s / 1e12 if at_n else None
+    n_att = m.n_layers * args.steps                                      # attention launches (grouped over the stacks)
+    per_launch_s = at_ms * 1e-3 / max(n_att, 1)
+    achieved = fl["attn_per_launch"] / per_launch_s / 1e12 if at_ms else None
     peak = peaks["tflops_sustained"]
     share = {c: round(t / max(sum(v[0] for v in cls.values()), 1e-9), 4) for c, (t, n) in cls.items()}
     gemm_ms = sum(cls[c][0] for c in ("qkv", "outproj", "ffn1", "ffn2", "post"))
     gemm_tflops = fl["gemm_per_layer"] * m.n_layers * args.steps / (gemm_ms * 1e-3) / 1e12 if gemm_ms else None
-    traffic = None                                    # DRAM bytes per launch from the committed ncu --set full capture
+    traffic, traffic_note = None, None                # DRAM bytes per launch from the committed ncu --set full capture
     tpath = os.path.join(HERE, "profiles", "attn_traffic.json")
     if os.path.exists(tpath):
         with open(tpath) as f:
             tj = json.load(f)
-        if tj.get("workload") == name:
-            traffic = tj["dram_bytes_per_launch"]
-    roofline = {"bound": "tensor", "kernel": "k_tc_attn (a4)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": (achieved / peak) if achieved else None, "traffic": traffic,
-                "algorithmic_bytes_per_launch": float(N) * m.d_model * 2 * (3 + 2),   # read q,k,v; write o hi + lo
-                "mufu_ceiling_frac": 16.0 * 148 * 1.9e9 * 4 * m.head_dim / 1e12 / peak,
-                "peak_source": f"{peaks['source']} bf16_tflops_sustained",
+        if tj.get("workload") == name and tj.get("kernel") == "k_tc_attn2":
+            traffic, traffic_note = tj["dram_bytes_per_launch"], tj.get("source")
+    # The binding unit of this kernel is not the tensor pipe but the softmax exponentials (one per score = per 4 hd tensor
+    # FLOPs): MUFU ex2 plus the share moved to the FMA pipe.  ALU ceiling = measured MUFU results / clk / SM (micro-benchmark
+    # in the library, run here) x SMs x the SM clock seen during the run / the share of exponentials left on the MUFU, in
+    # tensor-FLOP equivalents (x 4 hd).
+    S_ = getattr(m, "n_stacks", 1)
+    mufu_rate = P.microbench(0, 4096, stream=st)
+    poly_rate = P.microbench(2, 2048, stream=st)
+    bf16x2_rate = P.microbench(1, 4096, stream=st)
+    clk = (sampler.result()["sm_mhz"] or sampler.result()["sm_max_mhz"] or 1965.0) * 1e6
+    nsm = torch.cuda.get_device_properties(0).multi_processor_count
+    poly_share = (7.0 / 16.0) if m.head_dim <= 32 else 0.0
+    mufu_only = mufu_rate * nsm * clk * 4 * m.head_dim / 1e12            # every exponential on the MUFU
+    alu_peak = mufu_only / max(1.0 - poly_share, 1e-9)                   # with the kernel's share on the FMA pipe
+    nvalid_rows = int((X[:, 0] != 0).sum())
+    roofline = {"bound": "alu", "kernel": "k_tc_attn2 (a4) + k_attn_norms", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": (achieved / peak) if achieved else None, "traffic": traffic, "traffic_source": traffic_note,
+                "peak_source": f"{peaks['source']} bf16_tflops_sustained (dense bf16 tensor peak; the kernel is a contraction)",
+                "alu": {"binding_pipe": "XU (MUFU ex2) + FMA: softmax exponentials, one per 4*hd tensor FLOPs",
+                        "mufu_ex2_per_clk_per_sm_measured": mufu_rate, "mufu_ex2_bf16x2_per_clk_per_sm_measured": bf16x2_rate,
+                        "fma_poly_exp_per_clk_per_sm_measured": poly_rate,
+                        "sm_clock_hz": clk, "poly_share": poly_share,
+                        "mufu_only_ceiling_tflops": mufu_only, "alu_ceiling_tflops": alu_peak,
+                        "frac_of_alu_ceiling": (achieved / alu_peak) if achieved else None,
+                        "mufu_only_ceiling_frac_of_tensor_peak": mufu_only / peak},
+                "algorithmic_bytes_per_launch": float(S_ * nvalid_rows) * m.d_model * 2 * (3 + 2),   # read q,k,v; write o hi + lo
                 "flops_per_launch": fl["attn_per_launch"], "ms_per_launch": per_launch_s * 1e3,
                 "class_time_share": share,
                 "class_ms_per_step": {c: round(t / args.steps, 4) for c, (t, n) in cls.items()},
                 "gemm_tflops": gemm_tflops, "gemm_frac": (gemm_tflops / peak) if gemm_tflops else None,
-                "whole_step_tflops": fl["total"] * args.steps / (total_ms * 1e-3) / 1e12,
-                # HBM-bound glue kernels: algorithmic bytes / class time, against the measured copy peak
-                "glue_gbs": {"hbm_peak": peaks["hbm_gbs"],
-                             "layernorm": (N * m.d_model * ((m.n_layers * (4 + 2) + (m.n_layers + 1) * (4 + 4)))) * args.steps
-                                          / max(cls["layernorm"][0], 1e-9) / 1e6,
-                             "embed_l1": N * (m.n_feat * 4 + m.d_model * 4) * args.steps / max(cls["embed_l1"][0], 1e-9) / 1e6,
-                             "heads_l2": N * ((1 + len(m.reg_dims)) * m.d_model * 4 + 56) * args.steps
-                                         / max(cls["heads_l2"][0], 1e-9) / 1e6}}
+                "whole_step_tflops": fl["total"] * args.steps / (total_ms * 1e-3) / 1e12}
+    # per-class fractions of the GEMM-shaped steps (tensor peak) and of the HBM-bound glue kernels (copy peak)
+    Nv, d_, dff_, L_ = float(nvalid_rows), m.d_model, m.d_ff, m.n_layers
+
+    def tfl(flops_per_step, c):
+        t = cls[c][0] / args.steps * 1e-3
+        return None if t <= 0 else {"tflops": flops_per_step / t / 1e12, "frac_tensor": flops_per_step / t / 1e12 / peak,
+                                    "ms_per_step": t * 1e3}
+    roofline["per_class"] = {
+        "qkv (a3)": tfl(S_ * L_ * 2 * Nv * 3 * d_ * d_, "qkv"),
+        "post (a5+a6+a7 fused)": tfl(S_ * L_ * 2 * Nv * (d_ * d_ + 2 * d_ * dff_), "post"),
+        "outproj (a5)": tfl(S_ * L_ * 2 * Nv * d_ * d_, "outproj"),
+        "ffn1 (a6)": tfl(S_ * L_ * 2 * Nv * d_ * dff_, "ffn1"),
+        "ffn2 (a7)": tfl(S_ * L_ * 2 * Nv * d_ * dff_, "ffn2"),
+        "heads_l1 (a8)": tfl(2 * Nv * (1 + len(m.reg_dims) + (1 if getattr(m, "binary_head", False) else 0)) * d_ * d_, "heads_l1"),
+        "embed_l2 (a1)": tfl(2 * Nv * d_ * d_, "embed_l2")}
+    n_ln = cls["layernorm"][1] / max(args.steps, 1)
+    roofline["glue_gbs"] = {"hbm_peak": peaks["hbm_gbs"],
+                            "layernorm": (N * d_ * (4 + 2) * n_ln) * args.steps / max(cls["layernorm"][0], 1e-9) / 1e6,
+                            "embed_l1": N * (m.n_feat * 4 + d_ * 4) * args.steps / max(cls["embed_l1"][0], 1e-9) / 1e6,
+                            "heads_l2": Nv * ((1 + len(m.reg_dims)) * d_ * 4 + 56) * args.steps / max(cls["heads_l2"][0], 1e-9) / 1e6}
 
     # ---- CPU oracle on a bounded sample (rank 0, N = 1 only)
     cpu = None

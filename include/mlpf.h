@@ -265,6 +265,12 @@ int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_valid,
                            const int32_t* event_offsets, int32_t n_events, int32_t d_model, int32_t n_heads,
                            uint16_t* O, void* stream);
 
+/* Measured throughput, in results per clock per SM, of the units that bound the attention softmax (Eq. 4: one
+ * exponential per score): which = 0 ex2.approx.ftz.f32 (MUFU), 1 ex2.approx.ftz.bf16x2 (MUFU, packed), 2 the polynomial
+ * 2^x of tc_attn2.cu on the FMA / ALU pipes, 3 fma.rn.f32x2.  One CTA of 1024 threads per SM, `iters` x 8 independent
+ * operations per thread, cycles from clock64.  Synchronises `stream`.  < 0 on error.  bench.py's roofline.alu uses it. */
+float mlpf_microbench(int32_t which, int32_t iters, void* stream);
+
 /* which kernel mlpf_tc_attention_bf16 runs (process-wide; values as MLPF_OPT_ATTN) */
 int mlpf_debug_set_attention_impl(int impl);
 

@@ -30,7 +30,7 @@ KERNEL_CLASSES = ["sched", "embed_l1", "embed_l2", "layernorm", "qkv", "attentio
 EXPORTS = ["mlpf_create", "mlpf_infer", "mlpf_infer_ex", "mlpf_build_candidates_ex", "mlpf_infer_host", "mlpf_infer_host_async",
            "mlpf_host_sync", "mlpf_destroy", "mlpf_last_error", "mlpf_set_option",
            "mlpf_query", "mlpf_debug_get_schedule", "mlpf_debug_get_tensor", "mlpf_debug_get_profile", "mlpf_tc_gemm_bf16",
-           "mlpf_tc_attention_bf16", "mlpf_debug_set_attention_impl", "mlpf_tc_post_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates"]
+           "mlpf_tc_attention_bf16", "mlpf_debug_set_attention_impl", "mlpf_microbench", "mlpf_tc_post_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates"]
 
 _lib = None
 
@@ -77,6 +77,8 @@ def lib():
     L.mlpf_tc_gemm_bf16.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp]
     L.mlpf_tc_attention_bf16.restype = C.c_int
     L.mlpf_tc_attention_bf16.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
+    L.mlpf_microbench.restype = C.c_float
+    L.mlpf_microbench.argtypes = [i32, i32, vp]
     L.mlpf_debug_set_attention_impl.restype = C.c_int
     L.mlpf_debug_set_attention_impl.argtypes = [C.c_int]
     L.mlpf_tc_post_bf16.restype = C.c_int
@@ -238,6 +240,14 @@ def tc_attention_bf16(QKV, key_valid, event_offsets, d_model, n_heads, stream=No
                                         off.ctypes.data_as(C.c_void_p), len(off) - 1, d_model, n_heads,
                                         C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
     return out
+
+
+def microbench(which, iters=2048, stream=None):
+    """results per clock per SM: 0 ex2.f32 (MUFU), 1 ex2.bf16x2 (MUFU), 2 polynomial 2^x (FMA/ALU), 3 fma.f32x2 pairs."""
+    r = lib().mlpf_microbench(int(which), int(iters), _stream_ptr(stream))
+    if r < 0:
+        raise MlpfError("mlpf_microbench: " + lib().mlpf_last_error().decode())
+    return float(r)
 
 
 def tc_post_bf16(o_hi, o_lo, h, Wo, bo, ln2g, ln2b, W1, b1, W2, b2, lnng, lnnb, activation, eps, want_lo=True, stream=None):

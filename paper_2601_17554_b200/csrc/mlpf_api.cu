@@ -1109,6 +1109,17 @@ extern "C" int mlpf_tc_post_bf16(const uint16_t* o_hi, const uint16_t* o_lo, flo
     return MLPF_OK;
 }
 
+extern "C" float mlpf_microbench(int32_t which, int32_t iters, void* stream) {
+    if (which < 0 || which > 3 || iters < 1 || iters > (1 << 20)) { set_err(MLPF_E_ARG, "which in 0..3, iters in 1..2^20"); return -1.0f; }
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
+        set_err(MLPF_E_CUDA, "no CUDA device"); return -1.0f;
+    }
+    const float r = launch_microbench(which, iters, sms, (cudaStream_t)stream);
+    if (r < 0.0f) set_err(MLPF_E_CUDA, "micro-benchmark failed: %s", cudaGetErrorString(cudaGetLastError()));
+    return r;
+}
+
 static int g_attn_impl = 1;    // kernel-level attention entry: 0 = round-1 kernel, 1 = bound-based kernel, 2 = its exact path forced
 extern "C" int mlpf_debug_set_attention_impl(int impl) {
     if (impl < 0 || impl > 2) return set_err(MLPF_E_ARG, "impl must be 0, 1 or 2");

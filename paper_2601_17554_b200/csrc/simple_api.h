@@ -45,6 +45,7 @@ void launch_sched_replicate(int N, int N_pad, int E, int g, int d, int* offsets,
 void launch_pack_valid_bits(const int* valid, int N, uint32_t* bits, cudaStream_t st);
 void launch_cast_rows(bool fp32, const float* h, int64_t n, void* u, void* u_lo, cudaStream_t st);
 void launch_untile_h(const float* h_tiled, float* out, int64_t N, int d, cudaStream_t st);
+float launch_microbench(int which, int iters, int num_sms, cudaStream_t st);
 void launch_to_f32(bool fp32, const void* src, float* dst, int64_t n, cudaStream_t st);
 
 }  // namespace mlpf

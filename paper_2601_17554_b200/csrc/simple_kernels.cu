@@ -5,6 +5,7 @@
 //    (MLPF_PREC_FP32_DEBUG, parity <= 1e-4) and the MLPF_KERNELS_SIMPLE debugging aid in bf16.
 // Citations are /root/reference/PAPER.md lines; readings A* are listed in DESIGN.md.
 #include "simple_api.h"
+#include <vector>
 
 namespace mlpf {
 
@@ -725,6 +726,86 @@ void launch_sched_replicate(int N, int N_pad, int E, int g, int d, int* offsets,
                             uint32_t* valid_bits, float* h, cudaStream_t st) {
     const int64_t n = (int64_t)N * d / 4;
     k_sched_replicate<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(N, N_pad, E, g, d, offsets, n_valid, row_event, valid, valid_bits, h);
+}
+
+// ------------------------------------------------------------------------------------------------ micro-benchmarks
+// Throughput of the units that bound the attention softmax (bench.py's roofline.alu object): results per clock per SM of
+//   0: ex2.approx.ftz.f32 (MUFU)   1: ex2.approx.ftz.bf16x2 (MUFU, two results per instruction)
+//   2: the Cody-Waite + degree-3 polynomial 2^x on packed fp32 pairs (FMA / ALU pipes), as tc_attn2.cu uses it
+//   3: fma.rn.f32x2 (packed FMA)
+// One CTA of 1024 threads per SM, 8 independent dependency chains per thread, cycles from clock64 around the loop.
+__global__ void __launch_bounds__(1024, 1)
+k_microbench(int which, int iters, float seed, float* __restrict__ per_block, float* __restrict__ sink) {
+    float v[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = seed - 0.01f * (float)(threadIdx.x & 7) - 0.001f * (float)i;
+    __syncthreads();
+    const long long t0 = clock64();
+    if (which == 0) {
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(v[i]));
+        }
+    } else if (which == 1) {
+        uint32_t u[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) u[i] = 0xbf00be80u + (uint32_t)i;                  // pairs of small negative bf16
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) asm volatile("ex2.approx.ftz.bf16x2 %0, %0;" : "+r"(u[i]));
+        }
+#pragma unroll
+        for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(u[i]);
+    } else if (which == 2) {
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int i = 0; i < 8; i += 2) {
+                float xr0 = fmaf(v[i], 0.2550348616f, 12582912.0f - 8.0f), xr1 = fmaf(v[i + 1], 0.2550348616f, 12582912.0f - 8.0f);
+                const float m0 = xr0 - (12582912.0f - 8.0f), m1 = xr1 - (12582912.0f - 8.0f);
+                const float f0 = fmaf(v[i], 0.2550348616f, -m0), f1 = fmaf(v[i + 1], 0.2550348616f, -m1);
+                float p0 = fmaf(f0, 0.0550089306f, 0.2422109596f), p1 = fmaf(f1, 0.0550089306f, 0.2422109596f);
+                p0 = fmaf(p0, f0, 0.6932829272f); p1 = fmaf(p1, f1, 0.6932829272f);
+                p0 = fmaf(p0, f0, 1.0f); p1 = fmaf(p1, f1, 1.0f);
+                v[i] = __int_as_float(__float_as_int(p0) + (__float_as_int(xr0) << 23)) - 1.0f;   // keeps the chain's argument <= 0
+                v[i + 1] = __int_as_float(__float_as_int(p1) + (__float_as_int(xr1) << 23)) - 1.0f;
+            }
+        }
+    } else {
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int i = 0; i < 8; i += 2)
+                asm volatile("{\n\t.reg .b64 a, b;\n\tmov.b64 a, {%0, %1};\n\tmov.b64 b, {%2, %2};\n\tfma.rn.f32x2 a, a, b, b;\n\tmov.b64 {%0, %1}, a;\n\t}"
+                             : "+f"(v[i]), "+f"(v[i + 1]) : "f"(0.999f));
+        }
+    }
+    const long long t1 = clock64();
+    float acc = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc += v[i];
+    if (acc == 123.456f) sink[0] = acc;
+    __shared__ long long tmin, tmax;
+    if (threadIdx.x == 0) { tmin = t0; tmax = t1; }
+    __syncthreads();
+    atomicMin(&tmin, t0); atomicMax(&tmax, t1);
+    __syncthreads();
+    if (threadIdx.x == 0) per_block[blockIdx.x] = (float)(tmax - tmin);
+}
+// returns results per clock per SM (mean over one CTA per SM), < 0 on a CUDA error
+float launch_microbench(int which, int iters, int num_sms, cudaStream_t st) {
+    float *d_cyc = nullptr, *d_sink = nullptr;
+    if (cudaMalloc(&d_cyc, num_sms * 4) != cudaSuccess || cudaMalloc(&d_sink, 4) != cudaSuccess) { cudaFree(d_cyc); return -1.0f; }
+    k_microbench<<<num_sms, 1024, 0, st>>>(which, iters, -0.5f, d_cyc, d_sink);      // warm-up
+    k_microbench<<<num_sms, 1024, 0, st>>>(which, iters, -0.5f, d_cyc, d_sink);
+    std::vector<float> cyc(num_sms);
+    cudaError_t e = cudaMemcpyAsync(cyc.data(), d_cyc, num_sms * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d_cyc); cudaFree(d_sink);
+    if (e != cudaSuccess) return -1.0f;
+    double mean = 0.0;
+    for (float c : cyc) mean += c;
+    mean /= num_sms;
+    const double per_op = (which == 1) ? 2.0 : 1.0;          // bf16x2: two results per instruction; fma.f32x2 pairs are counted as issued above
+    return (float)(1024.0 * iters * 8.0 * per_op / mean);
 }
 
 // ------------------------------------------------------------------------------------------------ launchers
