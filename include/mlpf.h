@@ -186,6 +186,8 @@ int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* 
 #define MLPF_OPT_GRAPH       11  /* 1: a forward pass whose key (pointers, sizes, event_offsets, options) repeats is captured into a
                                     CUDA graph on its second occurrence and replayed afterwards (one launch per call: the
                                     one-event-per-call mode of PAPER.md L224); 0 (default): plain launches                   */
+#define MLPF_OPT_TAIL_SPLIT  12  /* 1 (default): the attention CTAs of a mostly empty last wave are split into single-query-tile
+                                    CTAs (shorter tail); 0: every CTA takes up to NT query tiles                              */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0

@@ -104,7 +104,7 @@ struct mlpf_handle {
     std::vector<LayerW> layers;
     HeadsOut ho;
     // options
-    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1, graph = 0;
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1, graph = 0, tail_split = 1;
     int64_t last_launches = 0;
     std::mutex mu;
     std::map<void*, Workspace*> ws;
@@ -277,6 +277,9 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_ATTN:
             if (value < 0 || value > 2) return set_err(MLPF_E_ARG, "attn must be 0, 1 or 2");
             h->attn = (int)value; return MLPF_OK;
+        case MLPF_OPT_TAIL_SPLIT:
+            if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "tail_split must be 0 or 1");
+            h->tail_split = (int)value; return MLPF_OK;
         case MLPF_OPT_GRAPH:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "graph must be 0 or 1");
             h->graph = (int)value; return MLPF_OK;
@@ -505,20 +508,40 @@ static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspa
     return MLPF_OK;
 }
 
-// host half of a0: the attention work list (event, q_tile), longest event first, ties by event id, then
-// q_tile ascending; `pairs` = the same order with two consecutive q-tiles of one event per entry.
-static void build_work_lists(const int32_t* off, int E, int tile_q, int rows_per_item, std::vector<int>& work, std::vector<int>& pairs) {
+// host half of a0: the attention work list (event, q_tile), longest event first, ties by event id, then q_tile ascending
+// (bit-exact vs oracle.schedule); `items` = the tensor-core kernels' CTAs in the same order: (event, first query tile |
+// tiles << 24) with nt_max consecutive 128-row query tiles of one event per item.
+static void build_work_lists(const int32_t* off, int E, int tile_q, int nt_max, std::vector<int>& work, std::vector<int>& items) {
     std::vector<int> order(E);
     for (int e = 0; e < E; ++e) order[e] = e;
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return (off[a + 1] - off[a]) > (off[b + 1] - off[b]); });
-    work.clear(); pairs.clear();
+    work.clear(); items.clear();
     for (int e : order) {
         int n = off[e + 1] - off[e];
         int nt = (n + tile_q - 1) / tile_q;
         for (int q = 0; q < nt; ++q) { work.push_back(e); work.push_back(q); }
-        int np128 = (n + rows_per_item - 1) / rows_per_item;
-        for (int p = 0; p < np128; ++p) { pairs.push_back(e); pairs.push_back(p); }
+        int n128 = (n + 127) / 128;
+        for (int t0 = 0; t0 < n128; t0 += nt_max) { items.push_back(e); items.push_back(t0 | (std::min(nt_max, n128 - t0) << 24)); }
     }
+}
+
+// The attention grid is items x heads CTAs, one per SM at a time, all of similar length within an event: when the last wave
+// is mostly empty, the whole GPU waits for a handful of full-length CTAs.  The items of that last partial wave (the tail of
+// the list = the shortest events) are split into single-tile items, which run about twice as fast each (the softmax
+// exponentials, not the K / V sweep, bound a CTA), so the tail is shorter and fills more SMs.
+static void split_tail_items(std::vector<int>& items, int H, int num_sms) {
+    const int64_t ctas = (int64_t)(items.size() / 2) * H;
+    if (ctas <= num_sms) return;
+    const int64_t rem = ctas % num_sms;
+    if (rem == 0 || rem * 4 > (int64_t)num_sms * 3) return;            // last wave more than 3/4 full: leave it
+    int k = (int)((rem + H - 1) / H);                                  // items in the partial wave
+    std::vector<int> tail;
+    while (k-- > 0 && !items.empty()) {
+        const int y = items.back(); items.pop_back();
+        const int e = items.back(); items.pop_back();
+        for (int t = (y >> 24) - 1; t >= 0; --t) { tail.push_back((y & 0xffffff) + t | (1 << 24)); tail.push_back(e); }
+    }
+    while (!tail.empty()) { items.push_back(tail.back()); tail.pop_back(); items.push_back(tail.back()); tail.pop_back(); }
 }
 
 static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, float* out_logits, float* out_regress,
@@ -739,7 +762,7 @@ extern "C" int mlpf_infer_ex(mlpf_handle* h, const float* elements, const int32_
     if (!wref) wref = new Workspace();
     Workspace* w = wref;
     std::vector<int>& work = w->host_work; std::vector<int>& pairs = w->host_pairs;
-    build_work_lists(event_offsets, n_events, h->tile_q, tc_attn_rows_per_cta(h->hd), work, pairs);
+    build_work_lists(event_offsets, n_events, h->tile_q, tc_attn_rows_per_cta(h->hd) / 128, work, pairs);
     const int64_t n_tiles_real = (int64_t)work.size() / 2;
     if (S > 1) {                           // the second encoder's events are the virtual events (E + 1) + e
         const size_t nw = work.size(), npz = pairs.size();
@@ -748,6 +771,7 @@ extern "C" int mlpf_infer_ex(mlpf_handle* h, const float* elements, const int32_
             for (size_t i = 0; i < npz; i += 2) { pairs.push_back(pairs[i] + g1 * (n_events + 1)); pairs.push_back(pairs[i + 1]); }
         }
     }
+    if (h->tail_split) split_tail_items(pairs, h->H, h->tc.num_sms);
     const int64_t Ev = S > 1 ? (int64_t)S * (n_events + 1) : n_events;
     int rc = ws_ensure(h, w, N, Ev, (int64_t)work.size() / 2, fp32, st);
     if (rc) return rc;
@@ -1140,7 +1164,7 @@ extern "C" int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_va
     std::call_once(once, [&] { init_rc = tc_init(&ctx); });
     if (init_rc) return set_err(MLPF_E_CUDA, "tcgen05/TMA initialisation failed: %s", ctx.err);
     std::vector<int> work, pairs;
-    build_work_lists(event_offsets, n_events, 128, tc_attn_rows_per_cta(hd), work, pairs);
+    build_work_lists(event_offsets, n_events, 128, tc_attn_rows_per_cta(hd) / 128, work, pairs);
     const int64_t N = event_offsets[n_events];
     if (pairs.empty()) return MLPF_OK;
     cudaStream_t st = (cudaStream_t)stream;

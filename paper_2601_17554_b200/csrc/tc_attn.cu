@@ -173,9 +173,9 @@ k_tc_attn(const __grid_constant__ CUtensorMap tmQKV, AttnParams prm) {
     const int item = blockIdx.x / prm.H, head = blockIdx.x % prm.H;
     const int2 it = prm.items[item];
     const int ev0 = prm.offsets[it.x], ev1 = prm.offsets[it.x + 1];
-    const int q0 = ev0 + it.y * NT * ATT_BQ;                         // first query row of this CTA
+    const int q0 = ev0 + (it.y & 0xffffff) * ATT_BQ;                 // item = (event, first query tile | tiles << 24)
     if (q0 >= ev1) return;      // the host sized the work list from the event's row count INCLUDING pad rows (an upper bound)
-    const int nt = min(NT, (ev1 - q0 + ATT_BQ - 1) / ATT_BQ);        // query tiles that hold rows of the event (>= 1)
+    const int nt = min(min(NT, it.y >> 24), (ev1 - q0 + ATT_BQ - 1) / ATT_BQ);   // query tiles of this CTA that hold rows of the event (>= 1)
     const int nkv = (ev1 - ev0 + ATT_BK - 1) / ATT_BK;              // 64-key tiles
     const int nst = (ev1 - ev0 + ATT_SK - 1) / ATT_SK;              // 128-key TMA stages
     const uint32_t* valid_bits = (prm.valid_bits && !(prm.n_valid && prm.n_valid[it.x] == ev1 - ev0)) ? prm.valid_bits : nullptr;

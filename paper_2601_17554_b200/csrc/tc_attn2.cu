@@ -169,9 +169,9 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
     const int item = blockIdx.x / prm.H, head = blockIdx.x % prm.H;
     const int2 it = prm.items[item];
     const int ev0 = prm.offsets[it.x], ev1 = prm.offsets[it.x + 1];
-    const int q0 = ev0 + it.y * NT * A2_BQ;
+    const int q0 = ev0 + (it.y & 0xffffff) * A2_BQ;               // item = (event, first query tile | tiles << 24)
     if (q0 >= ev1) return;      // the host sized the work list from the event's row count INCLUDING pad rows (an upper bound)
-    const int nt = min(NT, (ev1 - q0 + A2_BQ - 1) / A2_BQ);
+    const int nt = min(min(NT, it.y >> 24), (ev1 - q0 + A2_BQ - 1) / A2_BQ);
     const int nkv = (ev1 - ev0 + A2_BK - 1) / A2_BK;
     const int nst = (ev1 - ev0 + A2_SK - 1) / A2_SK;
     const uint32_t* valid_bits = (prm.valid_bits && !(prm.n_valid && prm.n_valid[it.x] == ev1 - ev0)) ? prm.valid_bits : nullptr;
