@@ -188,6 +188,9 @@ int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* 
                                     one-event-per-call mode of PAPER.md L224); 0 (default): plain launches                   */
 #define MLPF_OPT_TAIL_SPLIT  12  /* 1 (default): the attention CTAs of a mostly empty last wave are split into single-query-tile
                                     CTAs (shorter tail); 0: every CTA takes up to NT query tiles                              */
+#define MLPF_OPT_FP8         13  /* NEXT-3 (PAPER.md L232 / L238 "quantization"): 1 = the QKV projection runs with e4m3 operands
+                                    (tcgen05 kind::f8f6f4; one scale per weight matrix, a fixed scale of 16 for the LayerNorm
+                                    output, fp32 accumulate); 0 (default): BF16.  The measured drift is in DESIGN.md.          */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0
@@ -260,6 +263,9 @@ int mlpf_debug_get_profile(mlpf_handle* h, void* stream, float* ms_out, int32_t*
  * via the tcgen05 GEMM.  K % 64 == 0, N % 64 == 0.  Step a3/a5/a6/a7's contraction (L148-L156), no epilogue. */
 int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* A_lo, const uint16_t* W, float* C, int32_t M, int32_t N,
                       int32_t K, void* stream);
+/* C[M,N] (fp32) = out_scale * A[M,K] W[N,K]^T with e4m3 operands (one byte per element, row-major) via the tcgen05
+ * kind::f8f6f4 GEMM.  K % 128 == 0, N % 128 == 0. */
+int mlpf_tc_gemm_fp8(const uint8_t* A, const uint8_t* W, float* C, int32_t M, int32_t N, int32_t K, float out_scale, void* stream);
 /* O[N,d] (bf16) = per-event multi-head softmax(Q K^T / sqrt(hd)) V (Eq. 4) via the tcgen05 flash kernel.
  * QKV [N,3d] bf16 row-major (q | k | v), key_valid [N] int32 0/1 (NULL = all valid),
  * event_offsets HOST int32 [n_events+1]; events may start at any row. */

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmlpf.so")
 
 # include/mlpf.h constants
 OK = 0
-OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE, OPT_FUSE, OPT_ATTN, OPT_ATTN_POLY, OPT_COMPACT, OPT_GRAPH, OPT_TAIL_SPLIT = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12
+OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE, OPT_FUSE, OPT_ATTN, OPT_ATTN_POLY, OPT_COMPACT, OPT_GRAPH, OPT_TAIL_SPLIT, OPT_FP8 = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13
 PREC_BF16, PREC_FP32_DEBUG = 0, 1
 KERNELS_TC, KERNELS_SIMPLE = 0, 1
 Q_N_LAYERS, Q_D_MODEL, Q_N_HEADS, Q_D_FF, Q_N_FEAT, Q_N_CLASSES, Q_N_REGRESS = 1, 2, 3, 4, 5, 6, 7
@@ -30,7 +30,7 @@ KERNEL_CLASSES = ["sched", "embed_l1", "embed_l2", "layernorm", "qkv", "attentio
 EXPORTS = ["mlpf_create", "mlpf_infer", "mlpf_infer_ex", "mlpf_build_candidates_ex", "mlpf_infer_host", "mlpf_infer_host_async",
            "mlpf_host_sync", "mlpf_destroy", "mlpf_last_error", "mlpf_set_option",
            "mlpf_query", "mlpf_debug_get_schedule", "mlpf_debug_get_tensor", "mlpf_debug_get_profile", "mlpf_tc_gemm_bf16",
-           "mlpf_tc_attention_bf16", "mlpf_debug_set_attention_impl", "mlpf_microbench", "mlpf_tc_post_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates"]
+           "mlpf_tc_attention_bf16", "mlpf_debug_set_attention_impl", "mlpf_microbench", "mlpf_tc_gemm_fp8", "mlpf_tc_post_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates"]
 
 _lib = None
 
@@ -77,6 +77,8 @@ def lib():
     L.mlpf_tc_gemm_bf16.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp]
     L.mlpf_tc_attention_bf16.restype = C.c_int
     L.mlpf_tc_attention_bf16.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
+    L.mlpf_tc_gemm_fp8.restype = C.c_int
+    L.mlpf_tc_gemm_fp8.argtypes = [vp, vp, vp, i32, i32, i32, C.c_float, vp]
     L.mlpf_microbench.restype = C.c_float
     L.mlpf_microbench.argtypes = [i32, i32, vp]
     L.mlpf_debug_set_attention_impl.restype = C.c_int
@@ -239,6 +241,17 @@ def tc_attention_bf16(QKV, key_valid, event_offsets, d_model, n_heads, stream=No
     _check(lib().mlpf_tc_attention_bf16(C.c_void_p(QKV.data_ptr()), kv,
                                         off.ctypes.data_as(C.c_void_p), len(off) - 1, d_model, n_heads,
                                         C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+    return out
+
+
+def tc_gemm_fp8(A8, W8, out_scale=1.0, stream=None):
+    """A8 [M,K], W8 [N,K] CUDA tensors of dtype float8_e4m3fn -> fp32 [M,N] = out_scale * A W^T via the tcgen05 f8f6f4 GEMM."""
+    import torch
+    M, K = A8.shape
+    N = W8.shape[0]
+    out = torch.empty((M, N), dtype=torch.float32, device=A8.device)
+    _check(lib().mlpf_tc_gemm_fp8(C.c_void_p(A8.data_ptr()), C.c_void_p(W8.data_ptr()), C.c_void_p(out.data_ptr()),
+                                  M, N, K, float(out_scale), _stream_ptr(stream)))
     return out
 
 

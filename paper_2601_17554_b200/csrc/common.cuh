@@ -47,6 +47,8 @@ struct Epi {
     // Pad-row compaction: nc_dev (device, may be null) holds the number of meaningful rows (per group when group_rows > 0);
     // M-tiles that start at or beyond it are skipped (the host only knows the upper bound M).
     const int* nc_dev = nullptr;
+    // FP8 operands (NEXT-3): the accumulator is multiplied by out_scale = 1 / (scale_A scale_W) before the bias
+    float out_scale = 1.0f;
 };
 
 __device__ __forceinline__ float warp_sum(float v) {

@@ -8,6 +8,7 @@
 #include "cand_api.h"
 
 #include <algorithm>
+#include <cuda_fp8.h>
 #include <cstdarg>
 #include <cstdio>
 #include <type_traits>
@@ -61,6 +62,7 @@ struct Workspace {
     int *sorted_row = nullptr, *type_perm = nullptr;
     SchedCompact sc = {};                    // pad-row compaction arrays (a0)
     bool compact = false;                    // the last call ran on compacted rows
+    uint8_t* u8 = nullptr;                   // e4m3 copy of the LayerNorm output feeding the QKV projection (MLPF_OPT_FP8)
     float *qn = nullptr, *kmax = nullptr;   // attention norms pre-pass: |q_i| per row and head, max |k_j| per event and head
     // device staging of mlpf_infer_host[_async] (owned by the stream's workspace, freed with it): two slots, so that the
     // copies of one call overlap the kernels of the next; h2d_st / d2h_st are the library's own copy streams
@@ -100,11 +102,13 @@ struct mlpf_handle {
     int64_t n_params = 0, n_packed = 0;
     float* P32 = nullptr;             // packed parameters, fp32
     bf16* P16 = nullptr;              // same offsets, RNE-rounded to bf16
+    uint8_t* W8 = nullptr;            // e4m3 copies of the QKV projection matrices (NEXT-3), layer l at l * S * 3d * d bytes
+    std::vector<float> w8_scale;      // per layer: W8 = e4m3(W * w8_scale)
     int64_t embW1t, embB1, embW2, embB2, lnfg, lnfb, headW1, headB1, headW2, headB2;
     std::vector<LayerW> layers;
     HeadsOut ho;
     // options
-    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1, graph = 0, tail_split = 1;
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1, graph = 0, tail_split = 1, fp8 = 0;
     int64_t last_launches = 0;
     std::mutex mu;
     std::map<void*, Workspace*> ws;
@@ -237,6 +241,23 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
         set_err(MLPF_E_CUDA, "weight upload failed: %s", cudaGetErrorString(cudaGetLastError()));
         cudaFree(h->P32); cudaFree(h->P16); delete h; return nullptr;
     }
+    {   // e4m3 copies of Wqkv with one scale per layer (max |W| -> 448, the largest e4m3 value)
+        const int64_t per = (int64_t)S * 3 * d * d;
+        std::vector<uint8_t> W8((size_t)(per * L));
+        h->w8_scale.resize(L);
+        for (int l = 0; l < L; ++l) {
+            const float* wq = &P[h->layers[l].Wqkv];
+            float amax = 0.0f;
+            for (int64_t i = 0; i < per; ++i) amax = std::max(amax, fabsf(wq[i]));
+            const float sc = amax > 0.0f ? 448.0f / amax : 1.0f;
+            h->w8_scale[l] = sc;
+            for (int64_t i = 0; i < per; ++i) W8[(size_t)(l * per + i)] = (uint8_t)__nv_cvt_float_to_fp8(wq[i] * sc, __NV_SATFINITE, __NV_E4M3);
+        }
+        if (cudaMalloc(&h->W8, W8.size()) != cudaSuccess || cudaMemcpy(h->W8, W8.data(), W8.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+            set_err(MLPF_E_ALLOC, "FP8 weight upload failed");
+            cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W8); delete h; return nullptr;
+        }
+    }
     if (tc_init(&h->tc) != 0) {
         set_err(MLPF_E_CUDA, "tcgen05/TMA initialisation failed: %s", h->tc.err);
         cudaFree(h->P32); cudaFree(h->P16); delete h; return nullptr;
@@ -251,7 +272,7 @@ extern "C" void mlpf_destroy(mlpf_handle* h) {
     if (!h) return;
     cudaDeviceSynchronize();
     for (auto& kv : h->ws) { ws_free(kv.second); delete kv.second; }
-    cudaFree(h->P32); cudaFree(h->P16);
+    cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W8);
     delete h;
 }
 
@@ -277,6 +298,10 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_ATTN:
             if (value < 0 || value > 2) return set_err(MLPF_E_ARG, "attn must be 0, 1 or 2");
             h->attn = (int)value; return MLPF_OK;
+        case MLPF_OPT_FP8:
+            if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "fp8 must be 0 or 1");
+            if (value && h->d % 128) return set_err(MLPF_E_ARG, "FP8 operands need d_model %% 128 == 0");
+            h->fp8 = (int)value; return MLPF_OK;
         case MLPF_OPT_TAIL_SPLIT:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "tail_split must be 0 or 1");
             h->tail_split = (int)value; return MLPF_OK;
@@ -309,7 +334,7 @@ extern "C" int64_t mlpf_query(const mlpf_handle* h, int key) {
         case MLPF_Q_N_FEAT: return h->F;
         case MLPF_Q_N_CLASSES: return h->C;
         case MLPF_Q_N_REGRESS: return h->R;
-        case MLPF_Q_WEIGHT_BYTES: return h->n_packed * 6;
+        case MLPF_Q_WEIGHT_BYTES: return h->n_packed * 6 + (int64_t)h->L * h->S * 3 * h->d * h->d;
         case MLPF_Q_N_PARAMS: return h->n_params;
         case MLPF_Q_LAUNCHES: return h->last_launches;
         case MLPF_Q_N_STACKS: return h->S;
@@ -337,7 +362,7 @@ template <typename P> static void dfree(P*& p) { if (p) cudaFree(p); p = nullptr
 static void ws_free_rows(Workspace* w) {
     dfree(w->h); dfree(w->u); dfree(w->qkv); dfree(w->o); dfree(w->g); dfree(w->u_lo); dfree(w->o_lo); dfree(w->g_lo);
     dfree(w->valid); dfree(w->valid_bits); dfree(w->row_event); dfree(w->row_pos); dfree(w->block_counts); dfree(w->block_base);
-    dfree(w->sorted_row); dfree(w->type_perm); dfree(w->type_offsets); dfree(w->qn);
+    dfree(w->sorted_row); dfree(w->type_perm); dfree(w->type_offsets); dfree(w->qn); dfree(w->u8);
     dfree(w->sc.block_vbase); dfree(w->sc.n_comp); dfree(w->sc.vbefore); dfree(w->sc.comp_row); dfree(w->sc.orig_row);
     dfree(w->sc.row_event_c); dfree(w->sc.comp_type_perm);
     w->cap_rows = 0;
@@ -375,7 +400,7 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
             dmalloc(&w->type_offsets, 8 * 4, w) || dmalloc(&w->qn, cap * h->H * 4, w) ||
             dmalloc(&w->sc.block_vbase, nb * 4, w) || dmalloc(&w->sc.n_comp, 4, w) || dmalloc(&w->sc.vbefore, cap * 4, w) ||
             dmalloc(&w->sc.comp_row, cap * 4, w) || dmalloc(&w->sc.orig_row, cap * 4, w) || dmalloc(&w->sc.row_event_c, cap * 4, w) ||
-            dmalloc(&w->sc.comp_type_perm, m_ub * 4, w)) {
+            dmalloc(&w->sc.comp_type_perm, m_ub * 4, w) || dmalloc(&w->u8, cap * d, w)) {
             const char* why = cudaGetErrorString(cudaGetLastError());
             ws_free_rows(w);                       // release the partial set; nothing dangling is left behind
             w->bytes = ws_bytes_events(w);
@@ -388,6 +413,7 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
         cudaMemsetAsync(w->h, 0, cap * d * 4, st);
         cudaMemsetAsync(w->valid, 0, cap * 4, st); cudaMemsetAsync(w->row_event, 0, cap * 4, st);
         cudaMemsetAsync(w->sc.row_event_c, 0, cap * 4, st);
+        cudaMemsetAsync(w->u8, 0, cap * d, st);
         cudaMemsetAsync(w->u, 0, cap * d * es, st); cudaMemsetAsync(w->qkv, 0, cap * 3 * d * es, st);
         cudaMemsetAsync(w->o, 0, cap * d * es, st);
         cudaMemsetAsync(w->g, 0, w->g_elems * es, st);
@@ -470,9 +496,11 @@ static int run_gemm(mlpf_handle* h, bool fp32, bool tc, const void* A, const voi
     return MLPF_OK;
 }
 
+constexpr float U8_SCALE = 16.0f;     // LayerNorm outputs are O(1): e4m3(16 y) keeps |y| < 28 and 3 mantissa bits down to 2^-10
+
 static int run_layernorm(mlpf_handle* h, bool fp32, const float* x, int N, const float* g, const float* b, void* u, void* u_lo,
-                         cudaStream_t st) {
-    if (launch_layernorm(fp32, h->d, x, N, g, b, h->hp.ln_eps, u, u_lo, st))
+                         cudaStream_t st, uint8_t* u8 = nullptr) {
+    if (launch_layernorm(fp32, h->d, x, N, g, b, h->hp.ln_eps, u, u_lo, st, u8, U8_SCALE))
         return set_err(MLPF_E_ARG, "d_model %d unsupported by LayerNorm", h->d);
     LAUNCH_CHECK(h);
     return MLPF_OK;
@@ -599,11 +627,12 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         LAUNCH_CHECK(h);
     }
     // stand-alone LayerNorm of every stack's rows with that stack's gamma / beta (vectors are stacked [S, d])
-    auto layernorm_stacks = [&](int64_t g_off, int64_t b_off, void* out, void* out_lo) -> int {
+    const bool fp8 = tc && h->fp8 && d % 128 == 0;       // QKV projection with e4m3 operands (NEXT-3)
+    auto layernorm_stacks = [&](int64_t g_off, int64_t b_off, void* out, void* out_lo, bool want_u8 = false) -> int {
         for (int g1 = 0; g1 < S; ++g1) {
             const int64_t r0 = (int64_t)g1 * Npad;
             int rc = run_layernorm(h, fp32, w->h + r0 * d, N, PV + g_off + g1 * d, PV + b_off + g1 * d, (char*)out + r0 * d * es,
-                                   out_lo ? (char*)out_lo + r0 * d * es : nullptr, st);
+                                   out_lo ? (char*)out_lo + r0 * d * es : nullptr, st, want_u8 ? w->u8 + r0 * d : nullptr);
             if (rc) return rc;
         }
         return MLPF_OK;
@@ -621,7 +650,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         int rc;
         if (!u_ready) {
             ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);
-            rc = layernorm_stacks(lw.ln1g, lw.ln1b, u, nullptr);                                                // a2
+            rc = layernorm_stacks(lw.ln1g, lw.ln1b, u, nullptr, fp8);                                           // a2
             if (rc) return rc;
         }
         u_ready = false;
@@ -629,7 +658,14 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
             ProfScope ps(h, w, st, MLPF_KC_QKV);
             Epi ep;
             ep.bias = PV + lw.bqkv; ep.out_act = w->qkv; ep.ld_act = 3 * d; ep.group_rows = grp_rows; ep.n_groups = S; ep.nc_dev = nc_dev;
-            rc = run_gemm(h, fp32, tc, u, nullptr, PW(lw.Wqkv), M, 3 * d, d, ep, st);
+            if (fp8) {
+                ep.out_scale = 1.0f / (U8_SCALE * h->w8_scale[l]);
+                if (tc_gemm_fp8_launch(&h->tc, w->u8, h->W8 + (int64_t)l * S * 3 * d * d, M, 3 * d, d, ep, st))
+                    return set_err(MLPF_E_CUDA, "FP8 GEMM launch failed: %s", h->tc.err);
+                LAUNCH_CHECK(h);
+                rc = MLPF_OK;
+            } else
+                rc = run_gemm(h, fp32, tc, u, nullptr, PW(lw.Wqkv), M, 3 * d, d, ep, st);
             if (rc) return rc;
         }
         {
@@ -655,6 +691,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
                 a.dbg_u2 = (bf16*)w->u; a.dbg_g = (bf16*)w->g; a.u_out = (bf16*)w->g_lo;
             } else {
                 a.u_out = (bf16*)w->u; a.u_out_lo = last ? (bf16*)w->u_lo : nullptr;
+                if (fp8 && !last) { a.u_out_f8 = w->u8; a.f8_scale = U8_SCALE; }
             }
             if (tc_post_launch(&h->tc, a, st)) return set_err(MLPF_E_CUDA, "fused post-attention launch failed: %s", h->tc.err);
             LAUNCH_CHECK(h);
@@ -1105,6 +1142,22 @@ extern "C" int mlpf_tc_gemm_bf16(const uint16_t* A, const uint16_t* A_lo, const 
         return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", ctx.err);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", cudaGetErrorString(e));
+    return MLPF_OK;
+}
+
+extern "C" int mlpf_tc_gemm_fp8(const uint8_t* A, const uint8_t* W, float* C, int32_t M, int32_t N, int32_t K, float out_scale, void* stream) {
+    if (!A || !W || !C) return set_err(MLPF_E_NULL, "NULL argument");
+    if (M <= 0 || N <= 0 || K <= 0 || N % 128 || K % 128) return set_err(MLPF_E_ARG, "need M > 0, N %% 128 == 0, K %% 128 == 0");
+    static TcContext ctx;
+    static std::once_flag once;
+    static int init_rc = 0;
+    std::call_once(once, [&] { init_rc = tc_init(&ctx); });
+    if (init_rc) return set_err(MLPF_E_CUDA, "tcgen05/TMA initialisation failed: %s", ctx.err);
+    Epi ep;
+    ep.out_f32 = C; ep.ld_f32 = N; ep.out_scale = out_scale;
+    if (tc_gemm_fp8_launch(&ctx, A, W, M, N, K, ep, (cudaStream_t)stream)) return set_err(MLPF_E_CUDA, "FP8 GEMM launch failed: %s", ctx.err);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "FP8 GEMM launch failed: %s", cudaGetErrorString(e));
     return MLPF_OK;
 }
 

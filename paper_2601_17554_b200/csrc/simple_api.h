@@ -30,7 +30,7 @@ void launch_uncompact(const float* src, const int* comp_row, float* out, int64_t
 void launch_embed_l1(bool fp32, const float* X, int N, int F, int d, const float* W1t, const float* b1, int act,
                      const int* sorted_row, void* h1, void* h1_lo, float* h, cudaStream_t st);
 int launch_layernorm(bool fp32, int d, const float* x, int N, const float* g, const float* b, float eps, void* u,
-                     void* u_lo, cudaStream_t st);
+                     void* u_lo, cudaStream_t st, uint8_t* u8 = nullptr, float u8_scale = 1.0f);
 void launch_gemm_simple(bool fp32, const void* A, const void* A_lo, const void* W, int M, int N, int K, const Epi& ep,
                         cudaStream_t st);
 void launch_attn_simple(bool fp32, int hd, const void* QKV, const int* key_valid,

@@ -6,6 +6,7 @@
 // Citations are /root/reference/PAPER.md lines; readings A* are listed in DESIGN.md.
 #include "simple_api.h"
 #include <vector>
+#include <cuda_fp8.h>
 
 namespace mlpf {
 
@@ -267,7 +268,7 @@ k_layernorm(const float* __restrict__ h, int N, const float* __restrict__ gamma,
 template <int D>
 __global__ void __launch_bounds__(256)
 k_layernorm_vec(const float* __restrict__ h, int N, const float* __restrict__ gamma, const float* __restrict__ beta,
-                float eps, bf16* __restrict__ u, bf16* __restrict__ u_lo) {
+                float eps, bf16* __restrict__ u, bf16* __restrict__ u_lo, uint8_t* __restrict__ u8, float u8_scale) {
     constexpr int PER = D / 32, V = PER < 4 ? PER : 4;            // floats per vector load
     const int row = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (row >= N) return;
@@ -294,10 +295,12 @@ k_layernorm_vec(const float* __restrict__ h, int N, const float* __restrict__ ga
     for (int i = 0; i < PER; ++i) { const float c = v[i] - mean; q = fmaf(c, c, q); }
     const float rstd = rsqrtf(warp_sum(q) * (1.0f / D) + eps);
     uint32_t hi[PER / 2], lo[PER / 2];
+    uint16_t q8[PER / 2];
 #pragma unroll
     for (int i = 0; i < PER / 2; ++i) {
         const float y0 = (v[2 * i] - mean) * rstd * g[2 * i] + b[2 * i];
         const float y1 = (v[2 * i + 1] - mean) * rstd * g[2 * i + 1] + b[2 * i + 1];
+        q8[i] = (uint16_t)__nv_cvt_float2_to_fp8x2(make_float2(y0 * u8_scale, y1 * u8_scale), __NV_SATFINITE, __NV_E4M3);
         __nv_bfloat162 h2 = __floats2bfloat162_rn(y0, y1);
         hi[i] = *reinterpret_cast<uint32_t*>(&h2);
         __nv_bfloat162 l2 = __floats2bfloat162_rn(y0 - __low2float(h2), y1 - __high2float(h2));
@@ -317,6 +320,10 @@ k_layernorm_vec(const float* __restrict__ h, int N, const float* __restrict__ ga
     };
     store(u, hi);
     if (u_lo) store(u_lo, lo);
+    if (u8) {                                                     // e4m3 copy (NEXT-3: FP8 operands of the QKV projection)
+#pragma unroll
+        for (int i = 0; i < PER / 2; ++i) reinterpret_cast<uint16_t*>(u8 + (int64_t)row * D + lane * PER)[i] = q8[i];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -845,14 +852,14 @@ static int layernorm_d(int d, const float* x, int N, const float* g, const float
     return 0;
 }
 int launch_layernorm(bool fp32, int d, const float* x, int N, const float* g, const float* b, float eps, void* u,
-                     void* u_lo, cudaStream_t st) {
+                     void* u_lo, cudaStream_t st, uint8_t* u8, float u8_scale) {
     if (!fp32) {
         dim3 grid((N + 7) / 8);
         switch (d) {
-            case 64:  k_layernorm_vec<64><<<grid, 256, 0, st>>>(x, N, g, b, eps, (bf16*)u, (bf16*)u_lo); return 0;
-            case 128: k_layernorm_vec<128><<<grid, 256, 0, st>>>(x, N, g, b, eps, (bf16*)u, (bf16*)u_lo); return 0;
-            case 256: k_layernorm_vec<256><<<grid, 256, 0, st>>>(x, N, g, b, eps, (bf16*)u, (bf16*)u_lo); return 0;
-            case 512: k_layernorm_vec<512><<<grid, 256, 0, st>>>(x, N, g, b, eps, (bf16*)u, (bf16*)u_lo); return 0;
+            case 64:  k_layernorm_vec<64><<<grid, 256, 0, st>>>(x, N, g, b, eps, (bf16*)u, (bf16*)u_lo, u8, u8_scale); return 0;
+            case 128: k_layernorm_vec<128><<<grid, 256, 0, st>>>(x, N, g, b, eps, (bf16*)u, (bf16*)u_lo, u8, u8_scale); return 0;
+            case 256: k_layernorm_vec<256><<<grid, 256, 0, st>>>(x, N, g, b, eps, (bf16*)u, (bf16*)u_lo, u8, u8_scale); return 0;
+            case 512: k_layernorm_vec<512><<<grid, 256, 0, st>>>(x, N, g, b, eps, (bf16*)u, (bf16*)u_lo, u8, u8_scale); return 0;
         }
     }
     return fp32 ? layernorm_d<float>(d, x, N, g, b, eps, (float*)u, (float*)u_lo, st)

@@ -42,7 +42,8 @@ int tc_init(TcContext* c);
 int tc_set_smem_attr(TcContext* c, const void* kern, int bytes);
 // 2D bf16 tensor map: dims (d0 inner, d1 outer), row pitch ld elements, box (b0, b1), swizzle = b0 * 2 bytes
 int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64_t ld,
-                  uint32_t b0, uint32_t b1);
+                  uint32_t b0, uint32_t b1, int elem_bytes = 2);
+int tc_gemm_fp8_launch(TcContext* c, const uint8_t* A, const uint8_t* W, int M, int N, int K, const Epi& ep, cudaStream_t st);
 // C = (A + A_lo) W^T with the shared epilogue; A_lo == nullptr -> plain bf16 A.  N % 64 == 0, K % 64 == 0.
 int tc_gemm_launch(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W, int M, int N, int K,
                    const Epi& ep, cudaStream_t st);
@@ -76,6 +77,7 @@ struct PostArgs {
     float* h = nullptr;
     int h_in_tiled = 0, h_out_tiled = 0;     // residual-stream layout in / out (tc_post.cu h_off); capacity: whole 128-row tiles
     bf16 *u_out = nullptr, *u_out_lo = nullptr;
+    uint8_t* u_out_f8 = nullptr; float f8_scale = 1.0f;     // optional e4m3 copy of u_out * f8_scale
     int next_ln = 1;
     bf16 *dbg_u2 = nullptr, *dbg_g = nullptr;
 };

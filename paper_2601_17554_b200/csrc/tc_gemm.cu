@@ -47,9 +47,9 @@ int tc_set_smem_attr(TcContext* c, const void* kern, int bytes) {
 }
 
 int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64_t ld,
-                         uint32_t b0, uint32_t b1) {
-    const uint32_t sw_bytes = b0 * 2;
-    TcContext::Key key{ptr, d0, d1, ld, b0, b1, sw_bytes};
+                         uint32_t b0, uint32_t b1, int elem_bytes) {
+    const uint32_t sw_bytes = b0 * elem_bytes;
+    TcContext::Key key{ptr, d0, d1, ld, b0, b1, sw_bytes + 1024u * (uint32_t)elem_bytes};
     std::lock_guard<std::mutex> lk(c->mu);
     auto it = c->cache.find(key);
     if (it != c->cache.end()) { *out = it->second; return 0; }
@@ -57,11 +57,11 @@ int tc_tensor_map(TcContext* c, CUtensorMap* out, const void* ptr, uint64_t d0, 
                           : sw_bytes == 64  ? CU_TENSOR_MAP_SWIZZLE_64B
                           : sw_bytes == 32  ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_NONE;
     cuuint64_t dims[2] = {d0, d1};
-    cuuint64_t strides[1] = {ld * 2};
+    cuuint64_t strides[1] = {ld * (uint64_t)elem_bytes};
     cuuint32_t box[2] = {b0, b1};
     cuuint32_t estr[2] = {1, 1};
     alignas(64) CUtensorMap tm;
-    CUresult r = c->encode(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
+    CUresult r = c->encode(&tm, elem_bytes == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
                            CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
@@ -133,8 +133,9 @@ __device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[16], c
     for (int j = 0; j < 4; ++j) {
         float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
         if (bias_s) b = *reinterpret_cast<const float4*>(bias_s + 4 * j);       // broadcast LDS.128
-        v[2 * j] = ptx::fadd2(make_float2(__uint_as_float(acc[4 * j]), __uint_as_float(acc[4 * j + 1])), make_float2(b.x, b.y));
-        v[2 * j + 1] = ptx::fadd2(make_float2(__uint_as_float(acc[4 * j + 2]), __uint_as_float(acc[4 * j + 3])), make_float2(b.z, b.w));
+        const float2 sc = make_float2(ep.out_scale, ep.out_scale);
+        v[2 * j] = ptx::ffma2(make_float2(__uint_as_float(acc[4 * j]), __uint_as_float(acc[4 * j + 1])), sc, make_float2(b.x, b.y));
+        v[2 * j + 1] = ptx::ffma2(make_float2(__uint_as_float(acc[4 * j + 2]), __uint_as_float(acc[4 * j + 3])), sc, make_float2(b.z, b.w));
     }
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
@@ -174,7 +175,9 @@ __device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[16], c
     }
 }
 
-template <int BLOCK_N, int STAGES, bool SPLIT, int ACT>
+// FP8: A and W are e4m3 (one byte per element, 128 elements per 128-byte swizzled row, K = 32 per MMA): the byte
+// arithmetic of the stage ring is that of bf16 with K counted in units of 128 bytes; the epilogue rescales (ep.out_scale).
+template <int BLOCK_N, int STAGES, bool SPLIT, int ACT, bool FP8 = false>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmA_lo,
           const __grid_constant__ CUtensorMap tmB, int M, int N, int K, Epi ep) {
@@ -213,7 +216,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem_base = tmem_base_slot;
-    const int num_kb = K / GEMM_BK;
+    const int num_kb = K / (FP8 ? 2 * GEMM_BK : GEMM_BK);
 
     if (warp == 0) {
         // ---------------- TMA producer: the stage ring runs on across tiles
@@ -233,16 +236,17 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 if (lane == 0) {
                     const uint32_t st = smem_base + s * Cfg::STAGE_BYTES;
                     ptx::mbar_expect_tx(bar_full + 8 * s, Cfg::STAGE_BYTES);
-                    ptx::tma_load_2d(st, &tmA, bar_full + 8 * s, kb * GEMM_BK, m0);
-                    if (SPLIT) ptx::tma_load_2d(st + Cfg::A_BYTES, &tmA_lo, bar_full + 8 * s, kb * GEMM_BK, m0);
-                    ptx::tma_load_2d(st + Cfg::A_BYTES * (SPLIT ? 2 : 1), &tmB, bar_full + 8 * s, kb * GEMM_BK, w_row0 + n0);
+                    constexpr int KE = FP8 ? 2 * GEMM_BK : GEMM_BK;           // elements of K per stage (128 bytes per row)
+                    ptx::tma_load_2d(st, &tmA, bar_full + 8 * s, kb * KE, m0);
+                    if (SPLIT) ptx::tma_load_2d(st + Cfg::A_BYTES, &tmA_lo, bar_full + 8 * s, kb * KE, m0);
+                    ptx::tma_load_2d(st + Cfg::A_BYTES * (SPLIT ? 2 : 1), &tmB, bar_full + 8 * s, kb * KE, w_row0 + n0);
                 }
                 __syncwarp();
             }
         }
     } else if (warp == 1) {
         // ---------------- MMA issuer (all lanes, warp-uniform operands; one lane elected inside the wrappers)
-        constexpr uint32_t idesc = ptx::umma_idesc_bf16(GEMM_BM, BLOCK_N);
+        constexpr uint32_t idesc = FP8 ? ptx::umma_idesc_e4m3(GEMM_BM, BLOCK_N) : ptx::umma_idesc_bf16(GEMM_BM, BLOCK_N);
         uint32_t kbg = 0;
         int it = 0;
         for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
@@ -260,7 +264,8 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 #pragma unroll
                 for (int k = 0; k < GEMM_BK / 16; ++k) {
                     const uint64_t bd = ptx::umma_desc_kmajor(b_addr + k * 32, 128);
-                    ptx::mma_ss(d_tmem, ptx::umma_desc_kmajor(a_addr + k * 32, 128), bd, idesc, (kb | k) != 0);
+                    if (FP8) ptx::mma_ss_f8(d_tmem, ptx::umma_desc_kmajor(a_addr + k * 32, 128), bd, idesc, (kb | k) != 0);
+                    else ptx::mma_ss(d_tmem, ptx::umma_desc_kmajor(a_addr + k * 32, 128), bd, idesc, (kb | k) != 0);
                     if (SPLIT) ptx::mma_ss(d_tmem, ptx::umma_desc_kmajor(a_addr + Cfg::A_BYTES + k * 32, 128), bd, idesc, 1);
                 }
                 ptx::mma_commit(bar_empty + 8 * s);               // frees the stage when these MMAs retire
@@ -336,16 +341,17 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 }
 
 // ------------------------------------------------------------------------------------------------ launch
-template <int BLOCK_N, int STAGES, bool SPLIT, int ACT>
+template <int BLOCK_N, int STAGES, bool SPLIT, int ACT, bool FP8 = false>
 static int tc_gemm_launch_act(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W, int M, int N, int K,
                               int w_rows, const Epi& ep, cudaStream_t st) {
     using Cfg = GemmCfg<BLOCK_N, STAGES, SPLIT>;
     CUtensorMap tmA, tmAlo, tmB;
-    if (tc_tensor_map(c, &tmA, A, K, M, K, GEMM_BK, GEMM_BM)) return -1;
-    if (SPLIT) { if (tc_tensor_map(c, &tmAlo, A_lo, K, M, K, GEMM_BK, GEMM_BM)) return -1; }
+    constexpr int EB = FP8 ? 1 : 2, KE = FP8 ? 2 * GEMM_BK : GEMM_BK;
+    if (tc_tensor_map(c, &tmA, A, K, M, K, KE, GEMM_BM, EB)) return -1;
+    if (SPLIT) { if (tc_tensor_map(c, &tmAlo, A_lo, K, M, K, KE, GEMM_BM, EB)) return -1; }
     else tmAlo = tmA;
-    if (tc_tensor_map(c, &tmB, W, K, w_rows, K, GEMM_BK, BLOCK_N)) return -1;
-    auto kern = k_tc_gemm<BLOCK_N, STAGES, SPLIT, ACT>;
+    if (tc_tensor_map(c, &tmB, W, K, w_rows, K, KE, BLOCK_N, EB)) return -1;
+    auto kern = k_tc_gemm<BLOCK_N, STAGES, SPLIT, ACT, FP8>;
     if (tc_set_smem_attr(c, (const void*)kern, Cfg::SMEM_BYTES)) return -1;
     const int total_tiles = ((M + GEMM_BM - 1) / GEMM_BM) * (N / BLOCK_N);
     const int grid = total_tiles < c->num_sms ? total_tiles : c->num_sms;
@@ -376,6 +382,17 @@ int tc_gemm_launch(TcContext* c, const bf16* A, const bf16* A_lo, const bf16* W,
     }
     return A_lo ? tc_gemm_launch_cfg<64, 3, true>(c, A, A_lo, W, M, N, K, w_rows, ep, st)
                 : tc_gemm_launch_cfg<64, 5, false>(c, A, nullptr, W, M, N, K, w_rows, ep, st);
+}
+
+// C = (A W^T) out_scale + bias ...: A [M, K] and W [N, K] are e4m3 bytes (kind::f8f6f4), K % 128 == 0, N % 128 == 0;
+// no activation, no split (the QKV projection, NEXT-3).
+int tc_gemm_fp8_launch(TcContext* c, const uint8_t* A, const uint8_t* W, int M, int N, int K, const Epi& ep, cudaStream_t st) {
+    if (N % 128 || K % 128 || ep.act != ACT_NONE) { snprintf(c->err, sizeof c->err, "tc_gemm_fp8: N=%d, K=%d must be multiples of 128, no activation", N, K); return -1; }
+    if (ep.out_f32 ? (ep.out_act != nullptr) : (ep.out_act == nullptr || ep.residual != nullptr)) {
+        snprintf(c->err, sizeof c->err, "tc_gemm_fp8: the epilogue writes either fp32 (+ residual) or bf16 hi (+ lo)"); return -1;
+    }
+    const int w_rows = (ep.group_offsets || ep.group_rows > 0) ? ep.n_groups * N : N;
+    return tc_gemm_launch_act<128, 4, false, ACT_NONE, true>(c, (const bf16*)A, nullptr, (const bf16*)W, M, N, K, w_rows, ep, st);
 }
 
 }  // namespace mlpf

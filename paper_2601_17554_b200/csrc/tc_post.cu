@@ -25,6 +25,7 @@
 #include "tc_api.h"
 #include "ptx.cuh"
 #include "epi_math.cuh"
+#include <cuda_fp8.h>
 
 namespace mlpf {
 
@@ -51,6 +52,7 @@ struct PostParams {
     float* h;                       // [M, D] fp32 residual stream, updated in place
     int h_in_tiled, h_out_tiled;    // layout of h on the way in / out: 0 = row-major, 1 = tiled (see h_off)
     bf16* u_out; bf16* u_out_lo;    // [M, D] next LayerNorm output (lo may be null)
+    uint8_t* u_out_f8; float f8_scale;   // optional e4m3 copy of it times f8_scale (FP8 operands of the next QKV projection)
     int next_ln;                    // 0: u_out = T(h2) (final_ln = 0)
     bf16* dbg_u2; bf16* dbg_g;      // debug taps (null in production): u2 [M, D], g [M, dff] (hi terms)
 };
@@ -435,7 +437,7 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
                 uint32_t a[PIECE];
                 tmem_ld_n<PIECE>(lane_addr + c0, a);
                 ptx::tmem_ld_wait();
-                uint32_t hi[PIECE / 2], lo[PIECE / 2];
+                uint32_t hi[PIECE / 2], lo[PIECE / 2], f8[PIECE / 4];
 #pragma unroll
                 for (int i = 0; i < PIECE / 2; ++i) {
                     const int col = c0 + 2 * i;
@@ -444,6 +446,15 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
                     const float2 y = make_float2((__uint_as_float(a[2 * i]) + b2v.x - mu) * rstd * gg.x + bb.x,
                                                  (__uint_as_float(a[2 * i + 1]) + b2v.y - mu) * rstd * gg.y + bb.y);
                     split_bf16x2(y, hi[i], lo[i]);
+                    if (p.u_out_f8) {                       // (lo[] is free to carry the e4m3 pairs when there is no lo output)
+                        const uint32_t q = __nv_cvt_float2_to_fp8x2(make_float2(y.x * p.f8_scale, y.y * p.f8_scale), __NV_SATFINITE, __NV_E4M3);
+                        if (i & 1) f8[i >> 1] |= q << 16; else f8[i >> 1] = q;
+                    }
+                }
+                if (row_ok && p.u_out_f8) {
+#pragma unroll
+                    for (int j = 0; j < PIECE / 16; ++j)
+                        *reinterpret_cast<uint4*>(p.u_out_f8 + (int64_t)row * D + c0 + 16 * j) = make_uint4(f8[4 * j], f8[4 * j + 1], f8[4 * j + 2], f8[4 * j + 3]);
                 }
                 if (row_ok) {                             // 32-byte stores: a full sector per lane
 #pragma unroll
@@ -488,7 +499,7 @@ static int tc_post_launch_t(TcContext* c, const PostArgs& a, cudaStream_t st) {
     p.M = a.M; p.dff = a.dff; p.group_rows = a.group_rows > 0 ? a.group_rows : 0x7fffff80; p.nc_dev = a.nc_dev;
     p.bo = a.bo; p.ln2g = a.ln2g; p.ln2b = a.ln2b; p.b1 = a.b1; p.b2 = a.b2; p.lnng = a.lnng; p.lnnb = a.lnnb;
     p.eps = a.eps; p.h = a.h; p.h_in_tiled = a.h_in_tiled; p.h_out_tiled = a.h_out_tiled; p.u_out = a.u_out; p.u_out_lo = a.u_out_lo; p.next_ln = a.next_ln;
-    p.dbg_u2 = a.dbg_u2; p.dbg_g = a.dbg_g;
+    p.dbg_u2 = a.dbg_u2; p.dbg_g = a.dbg_g; p.u_out_f8 = a.u_out_f8; p.f8_scale = a.f8_scale;
     const int n_tiles = (a.M + POST_BM - 1) / POST_BM;
     const int grid = n_tiles < c->num_sms ? n_tiles : c->num_sms;
     kern<<<grid, POST_THREADS, smem, st>>>(tmO, tmOlo, tmWo, tmW1, tmW2, p);

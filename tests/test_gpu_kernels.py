@@ -225,3 +225,16 @@ def test_tc_post_matches_the_block_written_out(M, d, dff, act, next_ln):
     su = np.sqrt((un ** 2).mean())
     assert np.abs(got_u - un).max() <= 3e-4 * su, np.abs(got_u - un).max() / su
     assert np.abs(f64(u_hi) - un).max() <= 6e-3 * max(su, np.abs(un).max())           # hi alone: one bf16 rounding
+
+
+# ------------------------------------------------------------------------------------------- FP8 operands (NEXT-3)
+@pytest.mark.parametrize("M,N,K", [(128, 128, 128), (300, 768, 256), (1000, 1536, 512), (4097, 256, 128)])
+def test_tc_gemm_fp8_matches_fp64_matmul_of_the_e4m3_values(M, N, K):
+    """kind::f8f6f4 multiplies e4m3 values exactly and accumulates in fp32: against numpy fp64 on the dequantised operands."""
+    rng = np.random.default_rng(M + N + K)
+    A = torch.from_numpy(rng.standard_normal((M, K)).astype(np.float32) * 4).cuda().to(torch.float8_e4m3fn)
+    W = torch.from_numpy((rng.standard_normal((N, K)) * 30).astype(np.float32)).cuda().to(torch.float8_e4m3fn)
+    got = P.tc_gemm_fp8(A, W, out_scale=0.125).cpu().numpy()
+    torch.cuda.synchronize()
+    ref = 0.125 * oracle.linear(A.float().cpu().numpy().astype(np.float64), W.float().cpu().numpy().astype(np.float64), np.zeros(N))
+    assert np.abs(got - ref).max() <= 2e-5 * np.abs(ref).max()

@@ -424,3 +424,27 @@ def test_pipelined_host_entry_matches_synchronous_calls():
         lg, rg = mod.infer(torch.from_numpy(X).cuda(), off)
         torch.cuda.synchronize()
         assert torch.equal(lh, lg.cpu()) and torch.equal(rh, rg.cpu())
+
+
+# ------------------------------------------------------------------------------------------- NEXT-3: FP8 operands
+@pytest.mark.parametrize("name,max_events", [("cfg2", 4), ("cfg3", 2), ("paper2", 1)])
+def test_fp8_qkv_projection_drift(name, max_events):
+    """MLPF_OPT_FP8 = 1: the QKV projection with e4m3 operands.  Not a parity claim: the drift against the (unchanged)
+    fp64 / W-bf16 oracle is MEASURED, printed, and only bounded loosely (it is recorded in DESIGN.md; BF16 stays the default)."""
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    X, off = synth.make_named_events(name, max_events=max_events)
+    mod = P.Mlpf(W, m)
+    Xd = torch.from_numpy(X).cuda()
+    lg0, rg0 = [t.cpu().numpy() for t in mod.infer(Xd, off)]
+    mod.set_option(P.OPT_FP8, 1)
+    lg8, rg8 = [t.cpu().numpy() for t in mod.infer(Xd, off)]
+    torch.cuda.synchronize()
+    assert np.isfinite(lg8).all() and np.isfinite(rg8).all() and not np.array_equal(lg8, lg0)
+    lr, rr = oracle.forward(X, off, oracle.quantize_weights(W), m)
+    valid = X[:, 0] != 0
+    e_bf16 = max(oracle.parity_metrics(lg0, lr, valid)[0], oracle.parity_metrics(rg0, rr, valid)[0])
+    e_fp8 = max(oracle.parity_metrics(lg8, lr, valid)[0], oracle.parity_metrics(rg8, rr, valid)[0])
+    agree = oracle.argmax_agreement(lg8, lr, valid)
+    print(f"FP8 drift {name}: max rel err bf16 {e_bf16:.2e} -> fp8-qkv {e_fp8:.2e}; argmax agreement (decidable, frac, raw) {agree}")
+    assert e_bf16 <= TOL_BF16 and e_fp8 <= 0.25
