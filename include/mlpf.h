@@ -179,7 +179,7 @@ int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* 
                                     pre-pass, exact two-sweep path when the bound is too loose; two threads per query row);
                                     2 = the same with the exact path forced for every CTA; 0 = round 1's lazy-rescale kernel */
 #define MLPF_OPT_ATTN_POLY   9   /* tuning (process-wide): n of every 16 pairs of softmax exponentials run as a polynomial on the
-                                    FMA pipe instead of the MUFU: 0 (none), 4..9; -1 (default) = per head dimension          */
+                                    FMA pipe instead of the MUFU: 0 (none), 4, 7, 8; -1 (default) = 7 at hd <= 32, 0 at hd = 64 */
 #define MLPF_OPT_COMPACT     10  /* 1 (default): pad rows (type 0) are dropped after a0: every later step runs on the compacted rows
                                     (events stay contiguous, oracle.schedule comp_row / offsets_c), outputs are scattered back;
                                     0: pad rows stay in place and are masked as keys (round 1's behaviour)                   */

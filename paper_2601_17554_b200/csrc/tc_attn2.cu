@@ -435,10 +435,7 @@ static int tc_attn2_launch_hd(TcContext* c, const bf16* QKV, int64_t N, Attn2Par
     switch (pe) {
         case 0: return tc_attn2_launch_pe<HD, 0>(c, QKV, N, prm, st);
         case 4: return tc_attn2_launch_pe<HD, 4>(c, QKV, N, prm, st);
-        case 5: return tc_attn2_launch_pe<HD, 5>(c, QKV, N, prm, st);
         case 8: return tc_attn2_launch_pe<HD, 8>(c, QKV, N, prm, st);
-        case 9: return tc_attn2_launch_pe<HD, 9>(c, QKV, N, prm, st);
-        case 6: return tc_attn2_launch_pe<HD, 6>(c, QKV, N, prm, st);
         default: return tc_attn2_launch_pe<HD, 7>(c, QKV, N, prm, st);
     }
 }
