@@ -102,6 +102,7 @@ struct mlpf_handle {
     int64_t n_params = 0, n_packed = 0;
     float* P32 = nullptr;             // packed parameters, fp32
     bf16* P16 = nullptr;              // same offsets, RNE-rounded to bf16
+    bf16* W2p = nullptr;              // heads' output rows packed for tc_heads.cu: [chunk][hi | lo][16][chunk columns] bf16
     uint8_t* W8 = nullptr;            // e4m3 copies of the QKV projection matrices (NEXT-3), layer l at l * S * 3d * d bytes
     std::vector<float> w8_scale;      // per layer: W8 = e4m3(W * w8_scale)
     int64_t embW1t, embB1, embW2, embB2, lnfg, lnfb, headW1, headB1, headW2, headB2;
@@ -241,6 +242,30 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
         set_err(MLPF_E_CUDA, "weight upload failed: %s", cudaGetErrorString(cudaGetLastError()));
         cudaFree(h->P32); cudaFree(h->P16); delete h; return nullptr;
     }
+    if (tc_heads_supported(d, h->n_hblk)) {   // the output rows as bf16 hi + lo, 16-row tiles per chunk of hidden columns
+        const int CH = tc_heads_chunk(d), CPB = d / CH;
+        std::vector<uint16_t> W2p((size_t)h->n_hblk * CPB * 2 * 16 * CH, 0);
+        int o0 = 0;
+        for (int b = 0; b < h->n_hblk; ++b) {
+            int rk = 0;
+            for (int o = 0; o < h->n_out; ++o) if (h->ho.blk[o] == b) ++rk;
+            for (int c = 0; c < CPB; ++c)
+                for (int j = 0; j < rk; ++j)
+                    for (int k = 0; k < CH; ++k) {
+                        const float w = P[h->headW2 + (int64_t)(o0 + j) * d + c * CH + k];
+                        const uint16_t hi = f32_to_bf16_rne(w);
+                        uint32_t hb = (uint32_t)hi << 16; float hf; memcpy(&hf, &hb, 4);
+                        const size_t base = ((size_t)(b * CPB + c) * 2) * 16 * CH;
+                        W2p[base + (size_t)j * CH + k] = hi;
+                        W2p[base + (size_t)16 * CH + (size_t)j * CH + k] = f32_to_bf16_rne(w - hf);
+                    }
+            o0 += rk;
+        }
+        if (cudaMalloc(&h->W2p, W2p.size() * 2) != cudaSuccess || cudaMemcpy(h->W2p, W2p.data(), W2p.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) {
+            set_err(MLPF_E_ALLOC, "head weight upload failed");
+            cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W2p); delete h; return nullptr;
+        }
+    }
     {   // e4m3 copies of Wqkv with one scale per layer (max |W| -> 448, the largest e4m3 value)
         const int64_t per = (int64_t)S * 3 * d * d;
         std::vector<uint8_t> W8((size_t)(per * L));
@@ -255,7 +280,7 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
         }
         if (cudaMalloc(&h->W8, W8.size()) != cudaSuccess || cudaMemcpy(h->W8, W8.data(), W8.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
             set_err(MLPF_E_ALLOC, "FP8 weight upload failed");
-            cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W8); delete h; return nullptr;
+            cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W8); cudaFree(h->W2p); delete h; return nullptr;
         }
     }
     if (tc_init(&h->tc) != 0) {
@@ -272,7 +297,7 @@ extern "C" void mlpf_destroy(mlpf_handle* h) {
     if (!h) return;
     cudaDeviceSynchronize();
     for (auto& kv : h->ws) { ws_free(kv.second); delete kv.second; }
-    cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W8);
+    cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W8); cudaFree(h->W2p);
     delete h;
 }
 
@@ -643,7 +668,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     // out-projection + residual + LN2 + FFN1 + activation + FFN2 + residual + next LayerNorm (tc_post.cu); the only
     // stand-alone LayerNorm left is the first block's LN1.  Otherwise (d = 512, fp32 debug path, CUDA-core kernels)
     // the unfused chain of round 1 runs.
-    const bool fused = tc && h->fuse && sm == MLPF_SPLIT_ALL && tc_post_supported(d, dff);
+    const bool fused = tc && h->fuse && (sm | MLPF_SPLIT_HEAD | MLPF_SPLIT_EMB) == MLPF_SPLIT_ALL && tc_post_supported(d, dff);   // the fused block carries o, u2, g, u_final as hi + lo
     bool u_ready = false;                    // u already holds LN(h) for the next consumer (written by a fused epilogue)
     for (int l = 0; l < h->L; ++l) {
         const LayerW& lw = h->layers[l];
@@ -750,6 +775,29 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         // stack's z (rows 0 .. N-1), the regression blocks the regression stack's (rows (S-1) Npad ..), L156
         const int hw = h->n_hblk * d;
         int rc = MLPF_OK;
+        if (tc && h->fuse && compact && h->W2p && (sm & MLPF_SPLIT_UF) && tc_heads_supported(d, h->n_hblk)) {
+            // all heads, both layers, one kernel per encoder stack (tc_heads.cu): the hidden layers stay on chip, the
+            // outputs are scattered to the original rows; pad rows are zeroed here
+            ProfScope ps(h, w, st, MLPF_KC_HEADS_L1);
+            CUDA_TRY(cudaMemsetAsync(out_logits, 0, (size_t)N * h->C * 4, st));
+            if (h->R) CUDA_TRY(cudaMemsetAsync(out_regress, 0, (size_t)N * h->R * 4, st));
+            if (out_binary) CUDA_TRY(cudaMemsetAsync(out_binary, 0, (size_t)N * 4, st));
+            const int nb0 = S > 1 ? h->n_hblk0 : h->n_hblk;
+            for (int part = 0; part < (S > 1 ? 2 : 1); ++part) {
+                HeadsArgs a;
+                a.M = N; a.d = d; a.act = h->act; a.n_hblk_total = h->n_hblk;
+                a.blk0 = part == 0 ? 0 : nb0; a.nblk = part == 0 ? nb0 : h->n_hblk - nb0;
+                if (a.nblk == 0) continue;
+                const int64_t r0 = part == 0 ? 0 : (int64_t)(S - 1) * Npad;
+                a.z = (const bf16*)u + r0 * d; a.z_lo = (const bf16*)w->u_lo + r0 * d;
+                a.W1 = (const bf16*)PW(h->headW1); a.W2p = h->W2p; a.b1 = PV + h->headB1; a.b2 = PV + h->headB2;
+                a.orig_row = w->sc.orig_row; a.nc_dev = nc_dev; a.ho = h->ho;
+                a.out_logits = out_logits; a.out_regress = out_regress; a.out_binary = out_binary;
+                if (tc_heads_launch(&h->tc, a, st)) return set_err(MLPF_E_CUDA, "fused heads launch failed: %s", h->tc.err);
+                LAUNCH_CHECK(h);
+            }
+            return MLPF_OK;
+        }
         {
             ProfScope ps(h, w, st, MLPF_KC_HEADS_L1);
             const int nb0 = S > 1 ? h->n_hblk0 : h->n_hblk;

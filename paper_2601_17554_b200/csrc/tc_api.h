@@ -6,6 +6,7 @@
 #include <set>
 #include <utility>
 #include "common.cuh"
+#include "simple_api.h"
 
 namespace mlpf {
 
@@ -83,5 +84,22 @@ struct PostArgs {
 };
 bool tc_post_supported(int d, int dff);
 int tc_post_launch(TcContext* c, const PostArgs& a, cudaStream_t st);
+
+// All heads of step a8 as one kernel (tc_heads.cu): out = act(z W1[b]^T + b1[b]) W2[b]^T + b2[b] per head block b, hidden
+// layers kept on chip.  z, z_lo [M, d] bf16 (compacted rows); W1 [n_hblk_total * d, d] bf16; W2p = the output rows packed
+// per 128-column chunk as [chunk][hi | lo][16 rows][chunk columns] bf16 (tc_heads_chunk(d) columns per chunk; built by
+// mlpf_create); this launch covers blocks blk0 .. blk0 + nblk - 1 (two-stack models: one launch per stack).  Outputs go to
+// the ORIGINAL rows (orig_row, null = identity); the caller zeroes the output buffers first (pad rows).
+struct HeadsArgs {
+    int M = 0, d = 0, act = ACT_GELU, n_hblk_total = 0, blk0 = 0, nblk = 0;
+    const bf16 *z = nullptr, *z_lo = nullptr, *W1 = nullptr, *W2p = nullptr;
+    const float *b1 = nullptr, *b2 = nullptr;
+    const int *orig_row = nullptr, *nc_dev = nullptr;
+    HeadsOut ho = {};
+    float *out_logits = nullptr, *out_regress = nullptr, *out_binary = nullptr;
+};
+bool tc_heads_supported(int d, int n_hblk);
+int tc_heads_chunk(int d);
+int tc_heads_launch(TcContext* c, const HeadsArgs& a, cudaStream_t st);
 
 }  // namespace mlpf
