@@ -191,6 +191,8 @@ int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* 
 #define MLPF_OPT_FP8         13  /* NEXT-3 (PAPER.md L232 / L238 "quantization"): 1 = the QKV projection runs with e4m3 operands
                                     (tcgen05 kind::f8f6f4; one scale per weight matrix, a fixed scale of 16 for the LayerNorm
                                     output, fp32 accumulate); 0 (default): BF16.  The measured drift is in DESIGN.md.          */
+#define MLPF_OPT_EPI_NORMS   14  /* 1 (default): the attention softmax bound's inputs (|q| per row and head, max |k| per event and
+                                    head) come out of the QKV projection's epilogue; 0: a separate pre-pass kernel computes them */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0

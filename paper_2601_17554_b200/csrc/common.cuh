@@ -49,6 +49,12 @@ struct Epi {
     const int* nc_dev = nullptr;
     // FP8 operands (NEXT-3): the accumulator is multiplied by out_scale = 1 / (scale_A scale_W) before the bias
     float out_scale = 1.0f;
+    // QKV projection only (a3 -> a4): the epilogue also emits the attention kernel's softmax bound inputs (tc_attn2.cu):
+    // qn[row, head] = |q_row| per head and kmax[event, head] = max |k_row| (atomicMax on the float bits; zeroed by the
+    // caller), from the fp32 values before the bf16 rounding (the consumer pads the bound by 2^-7).  Columns [0, nd) are
+    // q, [nd, 2 nd) k; heads are nhd columns wide; row_event gives the (compacted) row's event.
+    float* qn = nullptr; float* kmax = nullptr; const int* row_event = nullptr;
+    int nH = 0, nhd = 0, nd = 0;
 };
 
 __device__ __forceinline__ float warp_sum(float v) {

@@ -109,7 +109,7 @@ struct mlpf_handle {
     std::vector<LayerW> layers;
     HeadsOut ho;
     // options
-    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1, graph = 0, tail_split = 1, fp8 = 0;
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1, graph = 0, tail_split = 1, fp8 = 0, epi_norms = 1;
     int64_t last_launches = 0;
     std::mutex mu;
     std::map<void*, Workspace*> ws;
@@ -323,6 +323,9 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_ATTN:
             if (value < 0 || value > 2) return set_err(MLPF_E_ARG, "attn must be 0, 1 or 2");
             h->attn = (int)value; return MLPF_OK;
+        case MLPF_OPT_EPI_NORMS:
+            if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "epi_norms must be 0 or 1");
+            h->epi_norms = (int)value; return MLPF_OK;
         case MLPF_OPT_FP8:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "fp8 must be 0 or 1");
             if (value && h->d % 128) return set_err(MLPF_E_ARG, "FP8 operands need d_model %% 128 == 0");
@@ -531,7 +534,7 @@ static int run_layernorm(mlpf_handle* h, bool fp32, const float* x, int N, const
     return MLPF_OK;
 }
 
-static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspace* w, cudaStream_t st) {
+static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspace* w, cudaStream_t st, bool norms_ready = false) {
     if (w->n_tiles == 0) return MLPF_OK;
     // compacted rows: every row of an event is a valid key (no mask but the event tail), events are offsets_c
     const int* offsets = w->compact ? w->sc.offsets_c : w->offsets;
@@ -549,8 +552,8 @@ static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspa
             rc = tc_attn2_launch(&h->tc, (const bf16*)w->qkv, w->Mtot, (int)w->Ev, valid_bits, n_valid, offsets, row_event,
                                  (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, w->qn, w->kmax, (bf16*)w->o,
                                  split ? (bf16*)w->o_lo : nullptr, h->attn == 2, w->compact ? w->sc.n_comp : nullptr,
-                                 h->S > 1 ? (int)w->Npad : 0, st);
-            h->last_launches++;                       // the norms pre-pass
+                                 h->S > 1 ? (int)w->Npad : 0, st, norms_ready);
+            if (!norms_ready) h->last_launches++;     // the norms pre-pass
         }
         if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", h->tc.err);
     } else {
@@ -653,6 +656,8 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     }
     // stand-alone LayerNorm of every stack's rows with that stack's gamma / beta (vectors are stacked [S, d])
     const bool fp8 = tc && h->fp8 && d % 128 == 0;       // QKV projection with e4m3 operands (NEXT-3)
+    // the QKV epilogue emits the attention norms when a head does not straddle two epilogue warps' column ranges
+    const bool epi_norms = tc && h->attn != 0 && h->epi_norms && (((3 * d) % 128 == 0 ? 64 : 32) % h->hd == 0);
     auto layernorm_stacks = [&](int64_t g_off, int64_t b_off, void* out, void* out_lo, bool want_u8 = false) -> int {
         for (int g1 = 0; g1 < S; ++g1) {
             const int64_t r0 = (int64_t)g1 * Npad;
@@ -683,6 +688,11 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
             ProfScope ps(h, w, st, MLPF_KC_QKV);
             Epi ep;
             ep.bias = PV + lw.bqkv; ep.out_act = w->qkv; ep.ld_act = 3 * d; ep.group_rows = grp_rows; ep.n_groups = S; ep.nc_dev = nc_dev;
+            if (epi_norms) {                        // |q| per row and head, max |k| per event and head for a4's softmax bound
+                CUDA_TRY(cudaMemsetAsync(w->kmax, 0, (size_t)w->Ev * h->H * 4, st));
+                ep.qn = w->qn; ep.kmax = w->kmax; ep.row_event = compact ? w->sc.row_event_c : w->row_event;
+                ep.nH = h->H; ep.nhd = h->hd; ep.nd = d;
+            }
             if (fp8) {
                 ep.out_scale = 1.0f / (U8_SCALE * h->w8_scale[l]);
                 if (tc_gemm_fp8_launch(&h->tc, w->u8, h->W8 + (int64_t)l * S * 3 * d * d, M, 3 * d, d, ep, st))
@@ -695,7 +705,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         }
         {
             ProfScope ps(h, w, st, MLPF_KC_ATTENTION);
-            rc = run_attention(h, fp32, tc_attn, (sm & MLPF_SPLIT_O) != 0, w, st);                                                     // a4
+            rc = run_attention(h, fp32, tc_attn, (sm & MLPF_SPLIT_O) != 0, w, st, epi_norms);                                          // a4
         }
         if (rc) return rc;
         if (fused) {   // a5 + a6 + a7 with both LayerNorms in epilogues
@@ -896,7 +906,7 @@ extern "C" int mlpf_infer_ex(mlpf_handle* h, const float* elements, const int32_
         push64((uint64_t)(uintptr_t)elements); push64((uint64_t)(uintptr_t)out_logits); push64((uint64_t)(uintptr_t)out_regress);
         push64((uint64_t)(uintptr_t)out_binary);
         key.push_back(h->precision); key.push_back(h->kernels); key.push_back(h->split); key.push_back(h->fuse);
-        key.push_back(h->attn); key.push_back(h->compact); key.push_back(h->tile_q); key.push_back(g_attn2_poly_every);
+        key.push_back(h->attn); key.push_back(h->compact); key.push_back(h->epi_norms); key.push_back(h->fp8); key.push_back(h->tail_split); key.push_back(h->tile_q); key.push_back(g_attn2_poly_every);
         key.insert(key.end(), event_offsets, event_offsets + n_off);
         for (auto& ge : w->graphs)
             if (ge.key == key) {

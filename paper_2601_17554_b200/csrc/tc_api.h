@@ -63,7 +63,8 @@ int tc_attn2_rows_per_cta(int hd);
 extern int g_attn2_poly_every;       // tuning knob: every n-th pair of exponentials on the FMA pipe (0, 2, 3, 4; -1 = default)
 int tc_attn2_launch(TcContext* c, const bf16* QKV, int64_t N, int E, const uint32_t* valid_bits, const int* n_valid,
                     const int* offsets, const int* row_event, const int2* items, int n_items, int d, int H, float* qn,
-                    float* kmax, bf16* O, bf16* O_lo, int force_exact, const int* nc_dev, int group_rows, cudaStream_t st);
+                    float* kmax, bf16* O, bf16* O_lo, int force_exact, const int* nc_dev, int group_rows, cudaStream_t st,
+                    bool norms_ready = false);
 
 // The post-attention half of an encoder block as one kernel (tc_post.cu): h <- h + o Wo^T + bo; u2 = LN2(h);
 // h <- h + act(u2 W1^T + b1) W2^T + b2; u_out = LN_next(h) (or T(h) when next_ln == 0).  d in {64, 128, 256}, dff % 128 == 0.

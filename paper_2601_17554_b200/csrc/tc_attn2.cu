@@ -218,7 +218,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
             asm volatile("st.shared.b32 [%0], %1;" ::"r"(sOnes + 4 * i), "r"(0x3f803f80u) : "memory");
         ptx::fence_proxy_async();
         if (t_sm < nt && qrow < ev1) {
-            bc = __ldg(prm.qn + (int64_t)qrow * prm.H + head) * __ldg(prm.kmax + (int64_t)it.x * prm.H + head) * prm.scale_log2 * 1.00001f;
+            bc = __ldg(prm.qn + (int64_t)qrow * prm.H + head) * __ldg(prm.kmax + (int64_t)it.x * prm.H + head) * prm.scale_log2 * 1.008f;   // 2^-7: norms may come from the values before their bf16 rounding
             bc = ceilf(bc);                                          // an integer bound: the polynomial path's range reduction is exact
             if (!(bc >= 0.0f) || bc > 3.0e38f) bc = 3.0e38f;         // NaN / inf norms: exact path (which is NaN-transparent too)
         }
@@ -456,12 +456,15 @@ static int tc_attn2_launch_hd(TcContext* c, const bf16* QKV, int64_t N, Attn2Par
 // norms pre-pass + attention.  qn [N, H] and kmax [E, H] are caller-owned scratch; row_event [N] from the schedule.
 int tc_attn2_launch(TcContext* c, const bf16* QKV, int64_t N, int E, const uint32_t* valid_bits, const int* n_valid,
                     const int* offsets, const int* row_event, const int2* items, int n_items, int d, int H, float* qn,
-                    float* kmax, bf16* O, bf16* O_lo, int force_exact, const int* nc_dev, int group_rows, cudaStream_t st) {
+                    float* kmax, bf16* O, bf16* O_lo, int force_exact, const int* nc_dev, int group_rows, cudaStream_t st,
+                    bool norms_ready) {
     const int hd = d / H;
     if (H > 64) { snprintf(c->err, sizeof c->err, "tc_attn2: more than 64 heads"); return -1; }
-    cudaMemsetAsync(kmax, 0, (size_t)E * H * 4, st);
-    const int64_t nthr = N * H;
-    k_attn_norms<<<(unsigned)((nthr + 255) / 256), 256, 0, st>>>(QKV, row_event, (int)N, H, hd, d, nc_dev, group_rows, qn, kmax);
+    if (!norms_ready) {                      // (the model path gets qn / kmax from the QKV projection's epilogue instead)
+        cudaMemsetAsync(kmax, 0, (size_t)E * H * 4, st);
+        const int64_t nthr = N * H;
+        k_attn_norms<<<(unsigned)((nthr + 255) / 256), 256, 0, st>>>(QKV, row_event, (int)N, H, hd, d, nc_dev, group_rows, qn, kmax);
+    }
     Attn2Params prm;
     prm.valid_bits = valid_bits; prm.n_valid = n_valid; prm.offsets = offsets; prm.items = items; prm.n_items = n_items;
     prm.qn = qn; prm.kmax = kmax; prm.H = H; prm.d = d; prm.O = O; prm.O_lo = O_lo; prm.force_exact = force_exact;

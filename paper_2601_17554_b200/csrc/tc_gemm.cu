@@ -127,7 +127,7 @@ __device__ __forceinline__ void stg_flush_b16(uint8_t* stg, bf16* g, int64_t ld,
 // memory; cc = 0 / 1: which half of the 32-column staging group; results are left in the staging tile
 template <int ACT>
 __device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[16], const Epi& ep, const float* bias_s, uint8_t* stg,
-                                                    int lane, int cc) {
+                                                    int lane, int cc, float* ss = nullptr) {
     float2 v[8];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
@@ -136,6 +136,12 @@ __device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[16], c
         const float2 sc = make_float2(ep.out_scale, ep.out_scale);
         v[2 * j] = ptx::ffma2(make_float2(__uint_as_float(acc[4 * j]), __uint_as_float(acc[4 * j + 1])), sc, make_float2(b.x, b.y));
         v[2 * j + 1] = ptx::ffma2(make_float2(__uint_as_float(acc[4 * j + 2]), __uint_as_float(acc[4 * j + 3])), sc, make_float2(b.z, b.w));
+    }
+    if (ss) {                                           // sum of squares of the chunk (attention norms, QKV projection)
+        float2 q2 = ptx::fmul2(v[0], v[0]);
+#pragma unroll
+        for (int j = 1; j < 8; ++j) q2 = ptx::ffma2(v[j], v[j], q2);
+        *ss += q2.x + q2.y;
     }
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
@@ -309,6 +315,24 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             const int srow = write_ok ? row : -1;                 // destination row of this lane's accumulator row
             uint32_t ra[16], rb[16];
             ptx::tmem_ld16(t_addr, ra);
+            // attention norms (QKV projection): this lane's row, its event, running sum of squares of the current head
+            const bool norms = ep.qn != nullptr && n0 + hcol < 2 * ep.nd;
+            int n_ev = -1;
+            if (norms && row_ok && (ep.group_rows > 0 ? m % ep.group_rows : m) < nc_rows) n_ev = __ldg(ep.row_event + m);
+            float n_ss = 0.0f;
+            auto norm_emit = [&](int col_end) {                   // columns up to col_end (exclusive) close a head
+                if (col_end % ep.nhd) return;
+                const int blk = (col_end - 1) / ep.nd, head = ((col_end - 1) % ep.nd) / ep.nhd;
+                const float nrm = sqrtf(n_ss);
+                n_ss = 0.0f;
+                if (blk == 0) { if (n_ev >= 0) ep.qn[(int64_t)m * ep.nH + head] = nrm; }
+                else {
+                    const unsigned grp = __match_any_sync(0xffffffffu, n_ev);
+                    const unsigned mx = __reduce_max_sync(grp, __float_as_uint(nrm));
+                    if (n_ev >= 0 && (int)(threadIdx.x & 31) == __ffs(grp) - 1)
+                        atomicMax(reinterpret_cast<unsigned*>(ep.kmax) + (int64_t)n_ev * ep.nH + head, mx);
+                }
+            };
 #pragma unroll
             for (int c = 0; c < BLOCK_N / 2; c += 32) {           // one 32-column staging group per iteration
                 const int col0 = n0 + hcol + c;
@@ -316,10 +340,12 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 ptx::tmem_ld_wait();
                 ptx::tmem_ld16(t_addr + c + 16, rb);
                 __syncwarp();
-                gemm_epilogue_chunk<ACT>(ra, ep, ep.bias ? &bias_s[e][hcol + c] : nullptr, stg, lane, 0);
+                gemm_epilogue_chunk<ACT>(ra, ep, ep.bias ? &bias_s[e][hcol + c] : nullptr, stg, lane, 0, norms ? &n_ss : nullptr);
+                if (norms) norm_emit(col0 + 16);
                 ptx::tmem_ld_wait();
                 if (c + 32 < BLOCK_N / 2) ptx::tmem_ld16(t_addr + c + 32, ra);
-                gemm_epilogue_chunk<ACT>(rb, ep, ep.bias ? &bias_s[e][hcol + c + 16] : nullptr, stg, lane, 1);
+                gemm_epilogue_chunk<ACT>(rb, ep, ep.bias ? &bias_s[e][hcol + c + 16] : nullptr, stg, lane, 1, norms ? &n_ss : nullptr);
+                if (norms) norm_emit(col0 + 32);
                 __syncwarp();
                 if (ep.out_f32) {
                     stg_copy_f32<false>(stg, ep.out_f32, ep.ld_f32, col0, srow, lane);
