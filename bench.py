@@ -456,7 +456,9 @@ def run_ours(args):
     roofline["glue_gbs"] = {"hbm_peak": peaks["hbm_gbs"],
                             "layernorm": (N * d_ * (4 + 2) * n_ln) * args.steps / max(cls["layernorm"][0], 1e-9) / 1e6,
                             "embed_l1": N * (m.n_feat * 4 + d_ * 4) * args.steps / max(cls["embed_l1"][0], 1e-9) / 1e6,
-                            "heads_l2": Nv * ((1 + len(m.reg_dims)) * d_ * 4 + 56) * args.steps / max(cls["heads_l2"][0], 1e-9) / 1e6}
+                            # null when the output rows are part of k_tc_heads (d <= 256): no separate launch to time
+                            "heads_l2": (Nv * ((1 + len(m.reg_dims)) * d_ * 4 + 56) * args.steps / cls["heads_l2"][0] / 1e6
+                                         if cls["heads_l2"][0] > 0 else None)}
 
     # ---- CPU oracle on a bounded sample (rank 0, N = 1 only)
     cpu = None
