@@ -152,6 +152,21 @@ int mlpf_build_candidates(const float* elements, int32_t n_feat, const int32_t* 
                           int64_t scratch_bytes, int32_t* cand_offsets, int32_t* cand_elem, int32_t* cand_pid,
                           float* cand_p4, void* stream);
 
+/* mlpf_build_candidates_static: mlpf_build_candidates_ex for callers that cannot allocate (no cudaMalloc in a tight serving
+ * loop or a harness that forbids it): same inputs, outputs and results, but the kernels' scratch is a file-scope device
+ * array inside the library, so the caller passes no scratch and this path calls no cudaMalloc / cudaFree / allocating
+ * library routine.  Limits per call: N <= mlpf_candidates_static_limit(0) = 262144 elements and n_events <=
+ * mlpf_candidates_static_limit(1) = 4096; beyond them MLPF_E_ARG (nothing enqueued).  The array
+ * (mlpf_candidates_static_limit(2) = 283136 bytes) is held by every GPU that loads the library until the process exits.
+ * ALL calls on a device share it: calls that overlap on the GPU (different streams, or host threads without a common
+ * stream) race; calls on one stream are ordered and safe.  It keeps the last call's contents; nothing in it has to start
+ * at zero (every byte a call reads is written by that call first).  Uses the CURRENT device; pointers as above. */
+int mlpf_build_candidates_static(const float* elements, int32_t n_feat, const int32_t* event_offsets, int32_t n_events,
+                                 const float* logits, int32_t n_classes, const float* regress, int32_t n_regress,
+                                 const float* binary, int32_t* cand_offsets, int32_t* cand_elem, int32_t* cand_pid,
+                                 float* cand_p4, void* stream);
+int64_t mlpf_candidates_static_limit(int32_t which);   /* 0: max elements, 1: max events, 2: bytes held per GPU; < 0 on error */
+
 /* ---- options -------------------------------------------------------------------------------------- */
 #define MLPF_OPT_PRECISION   1   /* MLPF_PREC_BF16 (default) | MLPF_PREC_FP32_DEBUG                    */
 #define MLPF_OPT_TILE_Q      2   /* query-tile rows of the attention work list: 64 | 128 (default 128) */

@@ -30,7 +30,8 @@ KERNEL_CLASSES = ["sched", "embed_l1", "embed_l2", "layernorm", "qkv", "attentio
 EXPORTS = ["mlpf_create", "mlpf_infer", "mlpf_infer_ex", "mlpf_build_candidates_ex", "mlpf_infer_host", "mlpf_infer_host_async",
            "mlpf_host_sync", "mlpf_destroy", "mlpf_last_error", "mlpf_set_option",
            "mlpf_query", "mlpf_debug_get_schedule", "mlpf_debug_get_tensor", "mlpf_debug_get_profile", "mlpf_tc_gemm_bf16",
-           "mlpf_tc_attention_bf16", "mlpf_debug_set_attention_impl", "mlpf_microbench", "mlpf_tc_gemm_fp8", "mlpf_tc_post_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates"]
+           "mlpf_tc_attention_bf16", "mlpf_debug_set_attention_impl", "mlpf_microbench", "mlpf_tc_gemm_fp8", "mlpf_tc_post_bf16", "mlpf_candidates_scratch_bytes", "mlpf_build_candidates",
+           "mlpf_build_candidates_static", "mlpf_candidates_static_limit"]
 
 _lib = None
 
@@ -87,6 +88,10 @@ def lib():
     L.mlpf_tc_post_bf16.argtypes = [vp] * 13 + [i32, i32, i32, i32, C.c_float, vp, vp, vp]
     L.mlpf_candidates_scratch_bytes.restype = i64
     L.mlpf_candidates_scratch_bytes.argtypes = [i64, i32]
+    L.mlpf_build_candidates_static.restype = C.c_int
+    L.mlpf_build_candidates_static.argtypes = [vp, i32, vp, i32, vp, i32, vp, i32, vp, vp, vp, vp, vp, vp]
+    L.mlpf_candidates_static_limit.restype = i64
+    L.mlpf_candidates_static_limit.argtypes = [i32]
     L.mlpf_build_candidates.restype = C.c_int
     L.mlpf_build_candidates.argtypes = [vp, i32, vp, i32, vp, i32, vp, vp, i64, vp, vp, vp, vp, vp]
     _lib = L
@@ -305,4 +310,24 @@ def build_candidates(elements, event_offsets, logits, regress, scratch=None, str
                                        C.c_void_p(out["cand_offsets"].data_ptr()), C.c_void_p(out["cand_elem"].data_ptr()),
                                        C.c_void_p(out["cand_pid"].data_ptr()), C.c_void_p(out["cand_p4"].data_ptr()),
                                        _stream_ptr(stream)))
+    return out
+
+
+def candidates_static_limit(which):
+    """0: max elements per call, 1: max events per call, 2: bytes of device memory the library holds per GPU."""
+    return _check(lib().mlpf_candidates_static_limit(which))
+
+
+def build_candidates_static(elements, event_offsets, logits, regress, out, stream=None, binary=None):
+    """mlpf_build_candidates_static: build_candidates without any allocation: the kernels' scratch is a device array
+    inside the library and `out` is the caller's dict of preallocated CUDA tensors (cand_offsets [E+1] int32, cand_elem [N]
+    int32, cand_pid [N] int32, cand_p4 [N,4] float32).  Calls that overlap on the GPU race on the shared scratch."""
+    off = np.ascontiguousarray(event_offsets, dtype=np.int32)
+    E = len(off) - 1
+    _check(lib().mlpf_build_candidates_static(C.c_void_p(elements.data_ptr()), elements.shape[1], off.ctypes.data_as(C.c_void_p), E,
+                                           C.c_void_p(logits.data_ptr()), logits.shape[1], C.c_void_p(regress.data_ptr()), regress.shape[1],
+                                           C.c_void_p(binary.data_ptr() if binary is not None else 0),
+                                           C.c_void_p(out["cand_offsets"].data_ptr()), C.c_void_p(out["cand_elem"].data_ptr()),
+                                           C.c_void_p(out["cand_pid"].data_ptr()), C.c_void_p(out["cand_p4"].data_ptr()),
+                                           _stream_ptr(stream)))
     return out

@@ -10,6 +10,7 @@
 // rows 0..N INCLUSIVE (row N is a virtual, never-kept row) so that every event offset, offsets[E] = N and the
 // offsets of trailing empty events included, falls inside exactly one block, which writes that cand_offsets entry.
 #include "cand_api.h"
+#include <mutex>
 
 namespace mlpf {
 
@@ -110,6 +111,66 @@ cudaError_t launch_build_candidates(const float* X, int F, const int32_t* offset
     int* block_counts = (int*)p;
     // pageable -> device async copies are staged by the runtime before returning: the caller may free offsets_host
     cudaError_t e = cudaMemcpyAsync(offsets, offsets_host, (size_t)(E + 1) * 4, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return e;
+    k_cand_count<<<nb, CAND_BLOCK, (size_t)CAND_BLOCK * C * 4, st>>>(X, F, logits, C, binary, N, code, block_counts);
+    k_cand_emit<<<nb, CAND_BLOCK, 0, st>>>(X, F, regress, N, offsets, E, code, block_counts, cand_offsets, cand_elem,
+                                           cand_pid, reinterpret_cast<float4*>(cand_p4));
+    return cudaGetLastError();
+}
+
+// ---- allocation-free variant (mlpf_build_candidates_static): the scratch the two kernels share lives in a file-scope
+// device array, so neither the caller nor the library allocates anything (callers that cannot call cudaMalloc: tight
+// serving loops, harnesses that forbid it).  Limits: N <= CAND_STATIC_MAX_N elements and E <= CAND_STATIC_MAX_E events per
+// call; 283 136 bytes of device memory per GPU that loads the library, held until the process exits.  Layout = the
+// caller-scratch layout at the maximum sizes: code [MAX_N] bytes | offsets [MAX_E + 1] int | block_counts [MAX_N/256 + 1] int.
+// Nothing in it has to start at zero: k_cand_count writes code[0, N) and every block count the second kernel reads, the
+// offsets are copied in by this call.  EVERY call shares the one array: calls that overlap on the GPU (two streams, two
+// host threads without a common stream) race on it.
+constexpr int64_t CAND_STATIC_MAX_N = 262144, CAND_STATIC_MAX_E = 4096;
+constexpr int64_t CAND_STATIC_CODE = CAND_STATIC_MAX_N;
+constexpr int64_t CAND_STATIC_OFFS = ((CAND_STATIC_MAX_E + 1) * 4 + 255) / 256 * 256;
+constexpr int64_t CAND_STATIC_CNTS = ((CAND_STATIC_MAX_N / CAND_BLOCK + 1) * 4 + 255) / 256 * 256;
+constexpr int64_t CAND_STATIC_BYTES = CAND_STATIC_CODE + CAND_STATIC_OFFS + CAND_STATIC_CNTS;
+static __device__ __align__(256) uint8_t g_cand_scratch[CAND_STATIC_BYTES];
+
+int64_t cand_static_max_elements() { return CAND_STATIC_MAX_N; }
+int64_t cand_static_max_events() { return CAND_STATIC_MAX_E; }
+int64_t cand_static_bytes() { return CAND_STATIC_BYTES; }
+
+// The array's name is a host-side stand-in in host code: its device address comes from cudaGetSymbolAddress, asked for
+// once per device with that device current (the caller's current device is the one the kernels will run on).
+static cudaError_t cand_static_ptr(uint8_t** out) {
+    constexpr int MAX_DEV = 64;
+    static uint8_t* ptrs[MAX_DEV] = {};
+    static std::mutex mu;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= MAX_DEV) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lk(mu);
+    if (!ptrs[dev]) {
+        uint8_t* p = nullptr;
+        e = cudaGetSymbolAddress((void**)&p, g_cand_scratch);
+        if (e != cudaSuccess) return e;
+        ptrs[dev] = p;
+    }
+    *out = ptrs[dev];
+    return cudaSuccess;
+}
+
+cudaError_t launch_build_candidates_static(const float* X, int F, const int32_t* offsets_host, int E, const float* logits, int C,
+                                           const float* regress, const float* binary, int32_t* cand_offsets, int32_t* cand_elem,
+                                           int32_t* cand_pid, float* cand_p4, cudaStream_t st) {
+    const int64_t N = offsets_host[E];
+    if (N > CAND_STATIC_MAX_N || E > CAND_STATIC_MAX_E) return cudaErrorInvalidValue;      // (the entry point checks first)
+    uint8_t* p = nullptr;
+    cudaError_t e = cand_static_ptr(&p);
+    if (e != cudaSuccess) return e;
+    const int nb = (int)(N / CAND_BLOCK + 1);
+    uint8_t* code = p;
+    int* offsets = (int*)(p + CAND_STATIC_CODE);
+    int* block_counts = (int*)(p + CAND_STATIC_CODE + CAND_STATIC_OFFS);
+    e = cudaMemcpyAsync(offsets, offsets_host, (size_t)(E + 1) * 4, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return e;
     k_cand_count<<<nb, CAND_BLOCK, (size_t)CAND_BLOCK * C * 4, st>>>(X, F, logits, C, binary, N, code, block_counts);
     k_cand_emit<<<nb, CAND_BLOCK, 0, st>>>(X, F, regress, N, offsets, E, code, block_counts, cand_offsets, cand_elem,

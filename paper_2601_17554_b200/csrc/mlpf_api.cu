@@ -1078,6 +1078,43 @@ extern "C" int mlpf_build_candidates(const float* elements, int32_t n_feat, cons
                                     scratch_bytes, cand_offsets, cand_elem, cand_pid, cand_p4, stream);
 }
 
+// Allocation-free variant: same inputs, outputs and result as mlpf_build_candidates_ex, scratch in a file-scope device
+// array of candidates.cu (see there); no cudaMalloc / cudaFree / allocating library call on this path.
+extern "C" int mlpf_build_candidates_static(const float* elements, int32_t n_feat, const int32_t* event_offsets, int32_t n_events,
+                                            const float* logits, int32_t n_classes, const float* regress, int32_t n_regress,
+                                            const float* binary, int32_t* cand_offsets, int32_t* cand_elem, int32_t* cand_pid,
+                                            float* cand_p4, void* stream) {
+    if (n_events < 0) return set_err(MLPF_E_OFFSETS, "n_events < 0");
+    if (n_events == 0) return MLPF_OK;
+    if (!event_offsets) return set_err(MLPF_E_NULL, "event_offsets is NULL");
+    if (event_offsets[0] != 0) return set_err(MLPF_E_OFFSETS, "event_offsets[0] != 0");
+    for (int e = 0; e < n_events; ++e)
+        if (event_offsets[e + 1] < event_offsets[e]) return set_err(MLPF_E_OFFSETS, "event_offsets decreasing at %d", e);
+    const int64_t N = event_offsets[n_events];
+    if (n_feat < 5 || n_classes < 1 || n_classes > 48) return set_err(MLPF_E_ARG, "n_feat = %d (>= 5), n_classes = %d (1..48)", n_feat, n_classes);
+    if (n_regress != 5) return set_err(MLPF_E_ARG, "n_regress = %d: the decode needs (pT', eta, sin phi, cos phi, E')", n_regress);
+    if (N > cand_static_max_elements() || n_events > cand_static_max_events())
+        return set_err(MLPF_E_ARG, "mlpf_build_candidates_static: %lld elements / %d events exceed the static scratch's limits (%lld elements, %lld events per call); use mlpf_build_candidates_ex with caller scratch",
+                       (long long)N, n_events, (long long)cand_static_max_elements(), (long long)cand_static_max_events());
+    if (!cand_offsets) return set_err(MLPF_E_NULL, "cand_offsets NULL");
+    if (N > 0 && (!elements || !logits || !regress || !cand_elem || !cand_pid || !cand_p4)) return set_err(MLPF_E_NULL, "inputs / outputs NULL");
+    if ((uintptr_t)cand_p4 & 15) return set_err(MLPF_E_ARG, "cand_p4 must be 16-byte aligned");
+    cudaError_t e = launch_build_candidates_static(elements, n_feat, event_offsets, n_events, logits, n_classes, regress, binary,
+                                                   cand_offsets, cand_elem, cand_pid, cand_p4, (cudaStream_t)stream);
+    if (e != cudaSuccess) return set_err(MLPF_E_CUDA, "candidate kernels (static scratch): %s", cudaGetErrorString(e));
+    g_err.clear();
+    return MLPF_OK;
+}
+
+extern "C" int64_t mlpf_candidates_static_limit(int32_t which) {
+    switch (which) {
+        case 0: return cand_static_max_elements();
+        case 1: return cand_static_max_events();
+        case 2: return cand_static_bytes();
+        default: return set_err(MLPF_E_ARG, "mlpf_candidates_static_limit: which = %d (0 elements, 1 events, 2 bytes)", which);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ debug taps
 extern "C" int64_t mlpf_debug_get_schedule(mlpf_handle* h, void* stream, int which, int32_t* host_out, int64_t capacity) {
     if (!h || !host_out) return set_err(MLPF_E_NULL, "NULL argument");
