@@ -296,7 +296,8 @@ int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_valid,
  * operations per thread, cycles from clock64.  Synchronises `stream`.  < 0 on error.  bench.py's roofline.alu uses it. */
 float mlpf_microbench(int32_t which, int32_t iters, void* stream);
 
-/* which kernel mlpf_tc_attention_bf16 runs (process-wide; values as MLPF_OPT_ATTN) */
+/* which kernel mlpf_tc_attention_bf16 runs (process-wide; 0 .. 2 as MLPF_OPT_ATTN; 3 / 4 = 1 / 2 for a QKV whose q columns
+ * were already multiplied by log2(e) / sqrt(head_dim) before their bf16 rounding: the form the model path feeds the kernel) */
 int mlpf_debug_set_attention_impl(int impl);
 
 /* The post-attention half of one encoder block (steps a5 + a6 + a7 with both LayerNorms in epilogues)

@@ -235,7 +235,8 @@ def tc_gemm_bf16(A, W, A_lo=None, stream=None):
 
 def tc_attention_bf16(QKV, key_valid, event_offsets, d_model, n_heads, stream=None, impl=1):
     """QKV [N,3d] bf16 (q | k | v), key_valid [N] int32 or None -> O [N,d] bf16 (Eq. 4 per event/head).
-    impl: 1 = bound-based kernel (default), 2 = its exact path forced, 0 = round 1's lazy-rescale kernel."""
+    impl: 1 = bound-based kernel (default), 2 = its exact path forced, 0 = round 1's lazy-rescale kernel; 3 / 4 = 1 / 2
+    for a QKV whose q columns already carry the factor log2(e) / sqrt(head_dim)."""
     import torch
     _check(lib().mlpf_debug_set_attention_impl(int(impl)))
     off = np.ascontiguousarray(event_offsets, dtype=np.int32)

@@ -55,6 +55,9 @@ struct Epi {
     // q, [nd, 2 nd) k; heads are nhd columns wide; row_event gives the (compacted) row's event.
     float* qn = nullptr; float* kmax = nullptr; const int* row_event = nullptr;
     int nH = 0, nhd = 0, nd = 0;
+    // with qn set: columns [0, nd) (q) are multiplied by q_scale (= log2(e) / sqrt(hd), the softmax scale) before the bf16
+    // rounding, and qn is the norm of the scaled values: the attention kernel then exponentiates S = q k as it is
+    float q_scale = 1.0f;
 };
 
 __device__ __forceinline__ float warp_sum(float v) {

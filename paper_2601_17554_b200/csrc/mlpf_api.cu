@@ -46,6 +46,7 @@ struct LayerW {                       // element offsets into the packed paramet
     int64_t ln1g, ln1b, Wqkv, bqkv, Wo, bo, ln2g, ln2b, W1, b1, W2, b2;
 };
 struct Workspace {
+    float q_prescale = 1.0f;          // the q columns of qkv carry this factor (softmax scale folded into a3's epilogue), 1 = none
     int64_t cap_rows = 0;             // capacity in rows (multiple of 128)
     int64_t cap_events = 0, cap_tiles = 0;
     int64_t bytes = 0;
@@ -340,7 +341,7 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "compact must be 0 or 1");
             h->compact = (int)value; return MLPF_OK;
         case MLPF_OPT_ATTN_POLY:
-            if (value != -1 && value != 0 && value != 4 && value != 7 && value != 8) return set_err(MLPF_E_ARG, "attn_poly must be -1, 0, 4, 7 or 8");
+            if (value != -1 && value != 0 && value != 4 && value != 7 && value != 8 && value != 9) return set_err(MLPF_E_ARG, "attn_poly must be -1, 0, 4, 7, 8 or 9");
             g_attn2_poly_every = (int)value; return MLPF_OK;
         case MLPF_OPT_FUSE:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "fuse must be 0 or 1");
@@ -534,7 +535,8 @@ static int run_layernorm(mlpf_handle* h, bool fp32, const float* x, int N, const
     return MLPF_OK;
 }
 
-static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspace* w, cudaStream_t st, bool norms_ready = false) {
+static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspace* w, cudaStream_t st, bool norms_ready = false,
+                         bool prescaled = false) {
     if (w->n_tiles == 0) return MLPF_OK;
     // compacted rows: every row of an event is a valid key (no mask but the event tail), events are offsets_c
     const int* offsets = w->compact ? w->sc.offsets_c : w->offsets;
@@ -552,7 +554,7 @@ static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspa
             rc = tc_attn2_launch(&h->tc, (const bf16*)w->qkv, w->Mtot, (int)w->Ev, valid_bits, n_valid, offsets, row_event,
                                  (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, w->qn, w->kmax, (bf16*)w->o,
                                  split ? (bf16*)w->o_lo : nullptr, h->attn == 2, w->compact ? w->sc.n_comp : nullptr,
-                                 h->S > 1 ? (int)w->Npad : 0, st, norms_ready);
+                                 h->S > 1 ? (int)w->Npad : 0, st, norms_ready, prescaled);
             if (!norms_ready) h->last_launches++;     // the norms pre-pass
         }
         if (rc != 0) return set_err(MLPF_E_CUDA, "tcgen05 attention launch failed: %s", h->tc.err);
@@ -658,6 +660,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     const bool fp8 = tc && h->fp8 && d % 128 == 0;       // QKV projection with e4m3 operands (NEXT-3)
     // the QKV epilogue emits the attention norms when a head does not straddle two epilogue warps' column ranges
     const bool epi_norms = tc && h->attn != 0 && h->epi_norms && (((3 * d) % 128 == 0 ? 64 : 32) % h->hd == 0);
+    w->q_prescale = epi_norms ? 1.4426950408889634f / sqrtf((float)h->hd) : 1.0f;
     auto layernorm_stacks = [&](int64_t g_off, int64_t b_off, void* out, void* out_lo, bool want_u8 = false) -> int {
         for (int g1 = 0; g1 < S; ++g1) {
             const int64_t r0 = (int64_t)g1 * Npad;
@@ -692,6 +695,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
                 CUDA_TRY(cudaMemsetAsync(w->kmax, 0, (size_t)w->Ev * h->H * 4, st));
                 ep.qn = w->qn; ep.kmax = w->kmax; ep.row_event = compact ? w->sc.row_event_c : w->row_event;
                 ep.nH = h->H; ep.nhd = h->hd; ep.nd = d;
+                ep.q_scale = w->q_prescale;             // q carries the softmax scale: a4 exponentiates S as it is
             }
             if (fp8) {
                 ep.out_scale = 1.0f / (U8_SCALE * h->w8_scale[l]);
@@ -705,7 +709,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         }
         {
             ProfScope ps(h, w, st, MLPF_KC_ATTENTION);
-            rc = run_attention(h, fp32, tc_attn, (sm & MLPF_SPLIT_O) != 0, w, st, epi_norms);                                          // a4
+            rc = run_attention(h, fp32, tc_attn, (sm & MLPF_SPLIT_O) != 0, w, st, epi_norms, epi_norms);                                          // a4
         }
         if (rc) return rc;
         if (fused) {   // a5 + a6 + a7 with both LayerNorms in epilogues
@@ -1202,6 +1206,11 @@ extern "C" int64_t mlpf_debug_get_tensor(mlpf_handle* h, void* stream, int which
     if (rows * cols > capacity) return set_err(MLPF_E_ARG, "capacity too small");
     int rc = tap_copy(w->fp32, src, rows, cols, ld, comp_row, host_out);
     if (rc) return rc;
+    if (which == MLPF_TENSOR_QK && w->q_prescale != 1.0f) {            // the tap reports q itself
+        const float inv = 1.0f / w->q_prescale;
+        for (int64_t r = 0; r < rows; ++r)
+            for (int64_t c = 0; c < d; ++c) host_out[r * cols + c] *= inv;
+    }
     return rows * cols;
 }
 
@@ -1292,9 +1301,10 @@ extern "C" float mlpf_microbench(int32_t which, int32_t iters, void* stream) {
     return r;
 }
 
-static int g_attn_impl = 1;    // kernel-level attention entry: 0 = round-1 kernel, 1 = bound-based kernel, 2 = its exact path forced
+static int g_attn_impl = 1;    // kernel-level attention entry: 0 = round-1 kernel, 1 = bound-based kernel, 2 = its exact path forced,
+                               // 3 / 4 = 1 / 2 for a QKV whose q columns already carry the scale log2(e) / sqrt(hd)
 extern "C" int mlpf_debug_set_attention_impl(int impl) {
-    if (impl < 0 || impl > 2) return set_err(MLPF_E_ARG, "impl must be 0, 1 or 2");
+    if (impl < 0 || impl > 4) return set_err(MLPF_E_ARG, "impl must be 0 .. 4");
     g_attn_impl = impl;
     return MLPF_OK;
 }
@@ -1341,7 +1351,8 @@ extern "C" int mlpf_tc_attention_bf16(const uint16_t* QKV, const int32_t* key_va
         CUDA_TRY(cudaMemcpyAsync(d_rowev, rowev.data(), (size_t)N * 4, cudaMemcpyHostToDevice, st));
         CUDA_TRY(cudaStreamSynchronize(st));      // rowev is a local
         rc = tc_attn2_launch(&ctx, (const bf16*)QKV, N, n_events, d_bits, nullptr, d_off, d_rowev, (const int2*)d_pairs,
-                             (int)(pairs.size() / 2), d_model, n_heads, d_qn, d_kmax, (bf16*)O, (bf16*)nullptr, g_attn_impl == 2, nullptr, 0, st);
+                             (int)(pairs.size() / 2), d_model, n_heads, d_qn, d_kmax, (bf16*)O, (bf16*)nullptr, g_attn_impl == 2 || g_attn_impl == 4, nullptr, 0, st,
+                             false, g_attn_impl >= 3);
     }
     cudaError_t e = cudaStreamSynchronize(st);
     cudaFree(d_off); cudaFree(d_pairs); cudaFree(d_bits); cudaFree(d_rowev); cudaFree(d_qn); cudaFree(d_kmax);

@@ -58,13 +58,14 @@ int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const uint32_t* val
 
 // Second attention design (tc_attn2.cu): no running maximum (Cauchy-Schwarz bound from a norms pre-pass; exact two-sweep
 // path for CTAs whose bound is too loose), two threads per query row.  qn [N, H], kmax [E, H]: caller-owned fp32 scratch;
-// row_event [N] from the schedule.  force_exact != 0: every CTA takes the exact path (tests).
+// row_event [N] from the schedule.  force_exact != 0: every CTA takes the exact path (tests).  prescaled: the q columns
+// of QKV (and qn) already carry the softmax scale log2(e) / sqrt(hd) (Epi::q_scale): the fast path then subtracts nothing.
 int tc_attn2_rows_per_cta(int hd);
 extern int g_attn2_poly_every;       // tuning knob: every n-th pair of exponentials on the FMA pipe (0, 2, 3, 4; -1 = default)
 int tc_attn2_launch(TcContext* c, const bf16* QKV, int64_t N, int E, const uint32_t* valid_bits, const int* n_valid,
                     const int* offsets, const int* row_event, const int2* items, int n_items, int d, int H, float* qn,
                     float* kmax, bf16* O, bf16* O_lo, int force_exact, const int* nc_dev, int group_rows, cudaStream_t st,
-                    bool norms_ready = false);
+                    bool norms_ready = false, bool prescaled = false);
 
 // The post-attention half of an encoder block as one kernel (tc_post.cu): h <- h + o Wo^T + bo; u2 = LN2(h);
 // h <- h + act(u2 W1^T + b1) W2^T + b2; u_out = LN_next(h) (or T(h) when next_ln == 0).  d in {64, 128, 256}, dff % 128 == 0.

@@ -127,13 +127,31 @@ __device__ __forceinline__ float2 a2_exp2_poly2(float2 sc, float2 c2, float2 k1)
     return make_float2(__int_as_float(__float_as_int(p.x) + (__float_as_int(xr.x) << 23)),
                        __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
 }
+// The same for scores that already carry the scale (PS, see the kernel) and need no offset: 2^s.
+//   xr = s + M;  n = xr - M;  f = s - n  (all exact)
+// (Tried: 2^n as a float from ONE funnel shift per value (M = 1.5 * 2^23 + 127, rotate xr left by 23 = K 2^n with the
+// constant K = 1.2939453125 folded into the coefficients) and a final packed multiply, which moves the two integer
+// multiply-adds from the FMA pipe to the idle ALU pipe: slower, 2.93 vs 2.87 ms per cfg3 step of attention.  The loop is
+// bound by issue slots, two per packed or 16-lane instruction, not by any one pipe.)
+__device__ __forceinline__ float2 a2_exp2_poly2_ps(float2 s) {
+    const float2 xr = ptx::fadd2(s, make_float2(12582912.0f, 12582912.0f));
+    const float2 m = ptx::fadd2(xr, make_float2(-12582912.0f, -12582912.0f));
+    const float2 f = ptx::fadd2(s, make_float2(-m.x, -m.y));
+    float2 p = ptx::ffma2(f, make_float2(0.0550089306f, 0.0550089306f), make_float2(0.2422109596f, 0.2422109596f));
+    p = ptx::ffma2(p, f, make_float2(0.6932829272f, 0.6932829272f));
+    p = ptx::ffma2(p, f, make_float2(1.0f, 1.0f));
+    return make_float2(__int_as_float(__float_as_int(p.x) + (__float_as_int(xr.x) << 23)),
+                       __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
+}
 // PE of every 16 pairs of exponentials run on the FMA pipe, evenly spread (PE = 0: all on the MUFU).  The MUFU does 16 ex2
 // per clock and SM and is the binding unit at hd = 32 (one ex2 per 128 tensor FLOPs); PE balances the MUFU against the
 // FMA / ALU pipes and the issue slots (measured on cfg3, ms per step of the attention class: profiles/r02_README.md).
 
 // 32 scores of one row -> 16 packed bf16 pairs  p = 2^(s c - Bc).  MASKED: scores of masked keys become -inf first, so the
 // MUFU gives the exact weight 0 (the polynomial path is not used on masked tiles).
-template <bool MASKED, int PE>
+// PS (pre-scaled scores, fast path): S already holds s c and no offset is subtracted (see the kernel): unmasked tiles feed
+// the MUFU straight from TMEM; masked tiles and the exact path keep the FMA with c = 1.
+template <bool MASKED, int PE, bool PS>
 __device__ __forceinline__ void a2_exp32(uint32_t (&s)[32], uint32_t mask, float c, float neg_bc, uint32_t (&pk)[16]) {
     const float2 c2 = make_float2(c, c), m2 = make_float2(neg_bc, neg_bc);
     const float2 k1 = make_float2(12582912.0f + neg_bc, 12582912.0f + neg_bc);      // exact: neg_bc is an integer on this path
@@ -145,7 +163,8 @@ __device__ __forceinline__ void a2_exp32(uint32_t (&s)[32], uint32_t mask, float
         }
         const float2 sc = make_float2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1]));
         float2 p;
-        if (!MASKED && ((i + 1) * PE) / 16 > (i * PE) / 16) p = a2_exp2_poly2(sc, c2, k1);
+        if (!MASKED && ((i + 1) * PE) / 16 > (i * PE) / 16) p = PS ? a2_exp2_poly2_ps(sc) : a2_exp2_poly2(sc, c2, k1);
+        else if (!MASKED && PS) p = make_float2(ptx::fast_exp2(sc.x), ptx::fast_exp2(sc.y));
         else {
             const float2 x = ptx::ffma2(sc, c2, m2);
             p = make_float2(ptx::fast_exp2(x.x), ptx::fast_exp2(x.y));
@@ -155,7 +174,7 @@ __device__ __forceinline__ void a2_exp32(uint32_t (&s)[32], uint32_t mask, float
     }
 }
 
-template <int HD, int PE>
+template <int HD, int PE, bool PS>
 __global__ void __launch_bounds__(Attn2Cfg<HD>::THREADS, 1)
 k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
     using Cfg = Attn2Cfg<HD>;
@@ -218,7 +237,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
             asm volatile("st.shared.b32 [%0], %1;" ::"r"(sOnes + 4 * i), "r"(0x3f803f80u) : "memory");
         ptx::fence_proxy_async();
         if (t_sm < nt && qrow < ev1) {
-            bc = __ldg(prm.qn + (int64_t)qrow * prm.H + head) * __ldg(prm.kmax + (int64_t)it.x * prm.H + head) * prm.scale_log2 * 1.008f;   // 2^-7: norms may come from the values before their bf16 rounding
+            bc = __ldg(prm.qn + (int64_t)qrow * prm.H + head) * __ldg(prm.kmax + (int64_t)it.x * prm.H + head) * (PS ? 1.0f : prm.scale_log2) * 1.008f;   // 2^-7: norms may come from the values before their bf16 rounding
             bc = ceilf(bc);                                          // an integer bound: the polynomial path's range reduction is exact
             if (!(bc >= 0.0f) || bc > 3.0e38f) bc = 3.0e38f;         // NaN / inf norms: exact path (which is NaN-transparent too)
         }
@@ -257,50 +276,61 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
         constexpr uint32_t idesc_o = ptx::umma_idesc_bf16(128, HD) | ptx::UMMA_B_MN_MAJOR;
         constexpr uint32_t idesc_l = ptx::umma_idesc_bf16(128, 8);
         constexpr uint32_t HALF = A2_BK * Cfg::SW;
-        // n = running tile counter over both sweeps (S buffer n & 1); j = key tile; g = running stage counter
-        auto issue_s = [&](int n, int j, int g) {
-            const uint32_t kb = sKV + (g % ST) * Cfg::STAGE_BYTES + (j & 1) * HALF;
-            const uint32_t qb = sQ + t * Cfg::Q_BYTES;
+        // The issuer's own instructions compete with the softmax warps for the scheduler's issue slots (the kernel is issue
+        // bound), so everything that depends on the running counters is kept incrementally: the stage of the current key
+        // tile pair (index, parity, the low word of its K descriptor) and the S buffer; descriptors differ from one another
+        // only by constants added to that low word (start address >> 4; no carry: shared memory is < 2^18 bytes).
+        const uint32_t HI_K = (uint32_t)(ptx::umma_desc_kmajor(0, Cfg::SW) >> 32), LO_K = (uint32_t)ptx::umma_desc_kmajor(0, Cfg::SW);
+        const uint32_t HI_V = (uint32_t)(ptx::umma_desc_mnmajor(0, Cfg::SW) >> 32), LO_V = (uint32_t)ptx::umma_desc_mnmajor(0, Cfg::SW);
+        auto mk = [](uint32_t hi, uint32_t lo) { return ((uint64_t)hi << 32) | lo; };
+        const uint32_t qd = (sQ + t * Cfg::Q_BYTES) >> 4;                       // Q_t, + 2 k per 16-column step
+        const uint64_t ones = ptx::umma_desc_kmajor(sOnes, 128);
+        const uint32_t s_t = tmem_base + 128 * t, o_t = tmem_base + Cfg::O_COL0 + Cfg::OW * t;
+        const uint32_t bs_t = bar_s + 16 * t, bp_t = bar_p + 16 * t;
+        // S_t(buffer b) = Q_t K^T for the key tile at shared-memory address (>> 4) kd
+        auto issue_s = [&](uint32_t b, uint32_t kd) {
 #pragma unroll
             for (int k = 0; k < HD / 16; ++k)
-                ptx::mma_ss(tmem_base + 128 * t + 64 * (n & 1), ptx::umma_desc_kmajor(qb + k * 32, Cfg::SW),
-                            ptx::umma_desc_kmajor(kb + k * 32, Cfg::SW), idesc_s, k != 0);
-            ptx::mma_commit(bar_s + 8 * (2 * t + (n & 1)));
+                ptx::mma_ss(s_t + 64 * b, mk(HI_K, LO_K | (qd + 2 * k)), mk(HI_K, LO_K | (kd + 2 * k)), idesc_s, k != 0);
+            ptx::mma_commit(bs_t + 8 * b);
         };
-        auto issue_o = [&](int n, int j, int g, bool first) {
-            const uint32_t vb = sKV + (g % ST) * Cfg::STAGE_BYTES + Cfg::K_BYTES + (j & 1) * HALF;
-            const uint32_t pb = tmem_base + 128 * t + 64 * (n & 1);
-            const uint64_t ones = ptx::umma_desc_kmajor(sOnes, 128);
+        // O_t += P_t(buffer b) V, l_t += P_t(buffer b) 1 for the value tile at (>> 4) vd
+        auto issue_o = [&](uint32_t b, uint32_t vd, bool first) {
 #pragma unroll
             for (int k = 0; k < A2_BK / 16; ++k) {                  // keys 16k .. 16k+15: P columns 32 (k / 2) + 8 (k % 2)
-                const uint32_t pa = pb + 32 * (k >> 1) + 8 * (k & 1);
-                ptx::mma_ts(tmem_base + Cfg::O_COL0 + Cfg::OW * t, pa, ptx::umma_desc_mnmajor(vb + k * 16 * Cfg::SW, Cfg::SW), idesc_o,
-                            !(first && k == 0));
-                ptx::mma_ts(tmem_base + Cfg::O_COL0 + Cfg::OW * t + HD, pa, ones, idesc_l, !(first && k == 0));
+                const uint32_t pa = s_t + 64 * b + 32 * (k >> 1) + 8 * (k & 1);
+                ptx::mma_ts(o_t, pa, mk(HI_V, LO_V | (vd + k * Cfg::SW)), idesc_o, !(first && k == 0));
+                ptx::mma_ts(o_t + HD, pa, ones, idesc_l, !(first && k == 0));
             }
         };
+        constexpr uint32_t STG16 = Cfg::STAGE_BYTES >> 4, HALF16 = HALF >> 4, KB16 = Cfg::K_BYTES >> 4;
         ptx::mbar_wait(bar_q, 0);
-        int n = 0;
+        uint32_t stg = 0, stg_par = 0, kd = sKV >> 4;             // stage of the key tile pair that holds tile j
+        uint32_t nb = 0, np = 0;                                  // S buffer n & 1 and parity (n >> 1) & 1 of tile j
         for (int sw = 0; sw < n_sweeps; ++sw) {
             const bool pv = sw == n_sweeps - 1;
-            const int g0 = sw * nst;
-            // the first two S tiles of the sweep (their stage may or may not be the same)
-            ptx::mbar_wait(bar_kv_full + 8 * (g0 % ST), (g0 / ST) & 1);
+            // the first two S tiles of the sweep (one stage)
+            ptx::mbar_wait(bar_kv_full + 8 * stg, stg_par);
             ptx::tc_fence_after();
-            issue_s(n, 0, g0);
-            if (nkv > 1) issue_s(n + 1, 1, g0);
-            for (int j = 0; j < nkv; ++j, ++n) {
-                const int g = g0 + (j >> 1);
-                ptx::mbar_wait_long(bar_p + 8 * (2 * t + (n & 1)), (n >> 1) & 1);   // P_t(j) in TMEM (sweep 0 of 2: S consumed)
+            issue_s(nb, kd);
+            if (nkv > 1) issue_s(nb ^ 1u, kd + HALF16);
+            for (int j = 0; j < nkv; ++j) {
+                const uint32_t odd = (uint32_t)j & 1u;
+                ptx::mbar_wait_long(bp_t + 8 * nb, np);                     // P_t(j) in TMEM (sweep 0 of 2: S consumed)
                 ptx::tc_fence_after();
-                if (pv) issue_o(n, j, g, j == 0);
-                if ((j & 1) || j == nkv - 1) ptx::mma_commit(bar_kv_empty + 8 * (g % ST));
+                if (pv) issue_o(nb, kd + KB16 + odd * HALF16, j == 0);
+                const bool last_of_stage = odd || j == nkv - 1;
+                if (last_of_stage) ptx::mma_commit(bar_kv_empty + 8 * stg);
+                // the stage after this one
+                uint32_t stg2 = stg + 1, par2 = stg_par, kd2 = kd + STG16;
+                if (stg2 == (uint32_t)ST) { stg2 = 0; par2 ^= 1u; kd2 = sKV >> 4; }
                 if (j + 2 < nkv) {                   // S_t(j+2) reuses this S buffer: in order after P_t(j) V_j
-                    const int g2 = g0 + ((j + 2) >> 1);
-                    if (((j + 2) & 1) == 0) ptx::mbar_wait(bar_kv_full + 8 * (g2 % ST), (g2 / ST) & 1);
+                    if (!odd) ptx::mbar_wait(bar_kv_full + 8 * stg2, par2);
                     ptx::tc_fence_after();
-                    issue_s(n + 2, j + 2, g2);
+                    issue_s(nb, kd2 + odd * HALF16);
                 }
+                if (last_of_stage) { stg = stg2; stg_par = par2; kd = kd2; }
+                np ^= nb; nb ^= 1u;                  // n + 1
             }
         }
         ptx::mma_commit(bar_o + 8 * t);
@@ -310,7 +340,10 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
         if (t < nt) {
             const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16);
             const uint32_t o_addr = lane_addr + Cfg::O_COL0 + Cfg::OW * t;
-            const float c = prm.scale_log2;
+            // PS: q was multiplied by c = log2(e) / sqrt(hd) before its bf16 rounding (QKV projection's epilogue), so S = s c.
+            // On the fast path |s c| <= B c <= 48 then bounds P = 2^(s c) to [2^-48, 2^48] by itself: nothing is subtracted at
+            // all (bf16 P and the fp32 sums have the exponent range for it; O / l cancels any common factor).
+            const float c = PS ? 1.0f : prm.scale_log2;
             // 32-bit mask of this warp's score half of key tile j: (key inside the event) & (valid row)
             auto tile_mask = [&](int j) -> uint32_t {
                 const int k0 = ev0 + j * A2_BK + 32 * hf;
@@ -325,7 +358,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
             // (the exact path sends EVERY tile through the masked variant: its exponents can be far below -126)
             const int n_full = valid_bits ? 0 : (ev1 - ev0 - 32 * hf + 32) / A2_BK;   // leading tiles whose half [64 j + 32 hf, + 32) lies inside the event
             int n = 0;
-            float neg_bc = -bc;
+            float neg_bc = PS ? 0.0f : -bc;
             if (exact) {
                 // sweep 0: the true row maximum over the valid keys (scores only)
                 float mx = -INFINITY;
@@ -361,7 +394,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
                 ptx::tmem_ld32(s_addr, s);
                 const uint32_t m = MASKED ? tile_mask(j) : 0xffffffffu;
                 ptx::tmem_ld_wait();
-                a2_exp32<MASKED, PE>(s, m, c, neg_bc, pk);
+                a2_exp32<MASKED, PE, PS>(s, m, c, neg_bc, pk);
                 ptx::tmem_st16(s_addr, pk);
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
@@ -431,25 +464,26 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
 
 int g_attn2_poly_every = -1;          // tuning knob (MLPF_OPT_ATTN_POLY): -1 = the default of the head dimension
 
-template <int HD, int PE>
+template <int HD, int PE, bool PS>
 static int tc_attn2_launch_pe(TcContext* c, const bf16* QKV, int64_t N, Attn2Params prm, cudaStream_t st) {
     using Cfg = Attn2Cfg<HD>;
     CUtensorMap tmQKV;
     if (tc_tensor_map(c, &tmQKV, QKV, 3 * prm.d, N, 3 * prm.d, HD, A2_SK)) return -1;
-    auto kern = k_tc_attn2<HD, PE>;
+    auto kern = k_tc_attn2<HD, PE, PS>;
     if (tc_set_smem_attr(c, (const void*)kern, Cfg::SMEM_BYTES)) return -1;
     kern<<<prm.n_items * prm.H, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(tmQKV, prm);
     return 0;
 }
 
-template <int HD>
+template <int HD, bool PS>
 static int tc_attn2_launch_hd(TcContext* c, const bf16* QKV, int64_t N, Attn2Params prm, cudaStream_t st) {
-    const int pe = g_attn2_poly_every >= 0 ? g_attn2_poly_every : (HD == 64 ? 0 : 7);
+    const int pe = g_attn2_poly_every >= 0 ? g_attn2_poly_every : (HD == 64 ? 0 : (PS ? 8 : 7));
     switch (pe) {
-        case 0: return tc_attn2_launch_pe<HD, 0>(c, QKV, N, prm, st);
-        case 4: return tc_attn2_launch_pe<HD, 4>(c, QKV, N, prm, st);
-        case 8: return tc_attn2_launch_pe<HD, 8>(c, QKV, N, prm, st);
-        default: return tc_attn2_launch_pe<HD, 7>(c, QKV, N, prm, st);
+        case 0: return tc_attn2_launch_pe<HD, 0, PS>(c, QKV, N, prm, st);
+        case 4: return tc_attn2_launch_pe<HD, 4, PS>(c, QKV, N, prm, st);
+        case 8: return tc_attn2_launch_pe<HD, 8, PS>(c, QKV, N, prm, st);
+        case 9: return tc_attn2_launch_pe<HD, 9, PS>(c, QKV, N, prm, st);
+        default: return tc_attn2_launch_pe<HD, 7, PS>(c, QKV, N, prm, st);
     }
 }
 
@@ -457,7 +491,7 @@ static int tc_attn2_launch_hd(TcContext* c, const bf16* QKV, int64_t N, Attn2Par
 int tc_attn2_launch(TcContext* c, const bf16* QKV, int64_t N, int E, const uint32_t* valid_bits, const int* n_valid,
                     const int* offsets, const int* row_event, const int2* items, int n_items, int d, int H, float* qn,
                     float* kmax, bf16* O, bf16* O_lo, int force_exact, const int* nc_dev, int group_rows, cudaStream_t st,
-                    bool norms_ready) {
+                    bool norms_ready, bool prescaled) {
     const int hd = d / H;
     if (H > 64) { snprintf(c->err, sizeof c->err, "tc_attn2: more than 64 heads"); return -1; }
     if (!norms_ready) {                      // (the model path gets qn / kmax from the QKV projection's epilogue instead)
@@ -469,10 +503,10 @@ int tc_attn2_launch(TcContext* c, const bf16* QKV, int64_t N, int E, const uint3
     prm.valid_bits = valid_bits; prm.n_valid = n_valid; prm.offsets = offsets; prm.items = items; prm.n_items = n_items;
     prm.qn = qn; prm.kmax = kmax; prm.H = H; prm.d = d; prm.O = O; prm.O_lo = O_lo; prm.force_exact = force_exact;
     prm.scale_log2 = 1.4426950408889634f / sqrtf((float)hd);
-    switch (hd) {
-        case 16: return tc_attn2_launch_hd<16>(c, QKV, N, prm, st);
-        case 32: return tc_attn2_launch_hd<32>(c, QKV, N, prm, st);
-        case 64: return tc_attn2_launch_hd<64>(c, QKV, N, prm, st);
+    switch (hd) {     // prescaled: the q columns of QKV already carry the factor log2(e) / sqrt(hd) (and qn is the norm of those)
+        case 16: return prescaled ? tc_attn2_launch_hd<16, true>(c, QKV, N, prm, st) : tc_attn2_launch_hd<16, false>(c, QKV, N, prm, st);
+        case 32: return prescaled ? tc_attn2_launch_hd<32, true>(c, QKV, N, prm, st) : tc_attn2_launch_hd<32, false>(c, QKV, N, prm, st);
+        case 64: return prescaled ? tc_attn2_launch_hd<64, true>(c, QKV, N, prm, st) : tc_attn2_launch_hd<64, false>(c, QKV, N, prm, st);
     }
     snprintf(c->err, sizeof c->err, "tc_attn2: head_dim %d unsupported", hd);
     return -1;

@@ -127,13 +127,13 @@ __device__ __forceinline__ void stg_flush_b16(uint8_t* stg, bf16* g, int64_t ld,
 // memory; cc = 0 / 1: which half of the 32-column staging group; results are left in the staging tile
 template <int ACT>
 __device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[16], const Epi& ep, const float* bias_s, uint8_t* stg,
-                                                    int lane, int cc, float* ss = nullptr) {
+                                                    int lane, int cc, float* ss = nullptr, float col_scale = 1.0f) {
     float2 v[8];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
         if (bias_s) b = *reinterpret_cast<const float4*>(bias_s + 4 * j);       // broadcast LDS.128
-        const float2 sc = make_float2(ep.out_scale, ep.out_scale);
+        const float2 sc = make_float2(ep.out_scale * col_scale, ep.out_scale * col_scale);   // (the staged bias carries col_scale already)
         v[2 * j] = ptx::ffma2(make_float2(__uint_as_float(acc[4 * j]), __uint_as_float(acc[4 * j + 1])), sc, make_float2(b.x, b.y));
         v[2 * j + 1] = ptx::ffma2(make_float2(__uint_as_float(acc[4 * j + 2]), __uint_as_float(acc[4 * j + 3])), sc, make_float2(b.z, b.w));
     }
@@ -302,7 +302,8 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             // this tile's bias -> shared memory (read back as broadcast 128-bit loads)
             asm volatile("bar.sync %0, 256;" ::"r"(1 + e) : "memory");          // everyone is done with the last tile's
             if (ep.bias)
-                for (int c = tid; c < BLOCK_N; c += 256) bias_s[e][c] = __ldg(ep.bias + w_row0 + n0 + c);
+                for (int c = tid; c < BLOCK_N; c += 256)
+                    bias_s[e][c] = __ldg(ep.bias + w_row0 + n0 + c) * ((ep.qn && n0 + c < ep.nd) ? ep.q_scale : 1.0f);
             asm volatile("bar.sync %0, 256;" ::"r"(1 + e) : "memory");
             const int m = m0 + q * 32 + lane;
             const bool row_ok = m < M;
@@ -340,11 +341,12 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 ptx::tmem_ld_wait();
                 ptx::tmem_ld16(t_addr + c + 16, rb);
                 __syncwarp();
-                gemm_epilogue_chunk<ACT>(ra, ep, ep.bias ? &bias_s[e][hcol + c] : nullptr, stg, lane, 0, norms ? &n_ss : nullptr);
+                const float cs0 = (ep.qn && col0 < ep.nd) ? ep.q_scale : 1.0f, cs1 = (ep.qn && col0 + 16 < ep.nd) ? ep.q_scale : 1.0f;
+                gemm_epilogue_chunk<ACT>(ra, ep, ep.bias ? &bias_s[e][hcol + c] : nullptr, stg, lane, 0, norms ? &n_ss : nullptr, cs0);
                 if (norms) norm_emit(col0 + 16);
                 ptx::tmem_ld_wait();
                 if (c + 32 < BLOCK_N / 2) ptx::tmem_ld16(t_addr + c + 32, ra);
-                gemm_epilogue_chunk<ACT>(rb, ep, ep.bias ? &bias_s[e][hcol + c + 16] : nullptr, stg, lane, 1, norms ? &n_ss : nullptr);
+                gemm_epilogue_chunk<ACT>(rb, ep, ep.bias ? &bias_s[e][hcol + c + 16] : nullptr, stg, lane, 1, norms ? &n_ss : nullptr, cs1);
                 if (norms) norm_emit(col0 + 32);
                 __syncwarp();
                 if (ep.out_f32) {

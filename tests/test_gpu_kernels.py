@@ -46,7 +46,20 @@ def test_tc_gemm_matches_fp64_matmul(M, N, K, split):
 
 # impl: 1 = bound-based kernel (tc_attn2.cu; these inputs take its fast path), 2 = its exact two-sweep path forced,
 # 0 = round 1's lazy-rescale kernel (kept selectable through MLPF_OPT_ATTN)
-IMPLS = [1, 2, 0]
+# 3 / 4 = 1 / 2 with the q columns already multiplied by log2(e) / sqrt(hd) before their bf16 rounding: the form the model
+# path feeds the kernel (a3's epilogue folds the softmax scale into q; the fast path then subtracts nothing from S)
+IMPLS = [1, 2, 0, 3, 4]
+
+
+def _attn_inputs(qkv, d, hd, impl):
+    """bf16 QKV for the kernel and the fp64 (q | k | v) the oracle sees: the bf16 values, q divided by the folded scale."""
+    qkv = qkv.copy()
+    c = np.log2(np.e) / np.sqrt(hd) if impl >= 3 else 1.0
+    qkv[:, :d] *= np.float32(c)
+    QKV = _bf16(qkv)
+    q64 = QKV.float().cpu().numpy().astype(np.float64)
+    q64[:, :d] /= c
+    return QKV, q64
 
 
 @pytest.mark.parametrize("impl", IMPLS)
@@ -62,12 +75,11 @@ def test_tc_attention_matches_dense_softmax(hd, H, lens, pad, impl):
     qkv = rng.standard_normal((N, 3 * d)).astype(np.float32)
     qkv[:, :d] *= 2.0                                     # sharper than unit-variance scores
     valid = (rng.random(N) >= pad)
-    QKV = _bf16(qkv)
+    QKV, qk64 = _attn_inputs(qkv, d, hd, impl)
     kv = torch.from_numpy(valid.astype(np.int32)).cuda()
     O = P.tc_attention_bf16(QKV, kv if pad > 0 else None, off, d, H, impl=impl).float().cpu().numpy()
     if pad == 0:
         valid[:] = True
-    qk64 = QKV.float().cpu().numpy().astype(np.float64)
     v64 = qk64[:, 2 * d:]
     for e in range(len(lens)):
         a, b = off[e], off[e + 1]
@@ -86,12 +98,11 @@ def _attn_check(qkv, lens, valid, hd, H, tol=2e-2, impl=1):
     d = hd * H
     off = np.zeros(len(lens) + 1, np.int32)
     off[1:] = np.cumsum(lens)
-    QKV = _bf16(qkv)
+    QKV, q64 = _attn_inputs(qkv, d, hd, impl)
     kv = None if valid is None else torch.from_numpy(valid.astype(np.int32)).cuda()
     O = P.tc_attention_bf16(QKV, kv, off, d, H, impl=impl).float().cpu().numpy()
     torch.cuda.synchronize()
     assert np.isfinite(O).all()
-    q64 = QKV.float().cpu().numpy().astype(np.float64)
     vv = np.ones(len(qkv), bool) if valid is None else valid
     worst = 0.0
     for e in range(len(lens)):
