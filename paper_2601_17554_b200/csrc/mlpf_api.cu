@@ -341,7 +341,7 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "compact must be 0 or 1");
             h->compact = (int)value; return MLPF_OK;
         case MLPF_OPT_ATTN_POLY:
-            if (value != -1 && value != 0 && value != 4 && value != 7 && value != 8 && value != 9) return set_err(MLPF_E_ARG, "attn_poly must be -1, 0, 4, 7, 8 or 9");
+            if (value != -1 && value != 0 && value != 4 && (value < 7 || value > 9)) return set_err(MLPF_E_ARG, "attn_poly must be -1, 0, 4, 7, 8 or 9");
             g_attn2_poly_every = (int)value; return MLPF_OK;
         case MLPF_OPT_FUSE:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "fuse must be 0 or 1");

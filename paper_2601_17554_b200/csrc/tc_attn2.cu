@@ -477,7 +477,9 @@ static int tc_attn2_launch_pe(TcContext* c, const bf16* QKV, int64_t N, Attn2Par
 
 template <int HD, bool PS>
 static int tc_attn2_launch_hd(TcContext* c, const bf16* QKV, int64_t N, Attn2Params prm, cudaStream_t st) {
-    const int pe = g_attn2_poly_every >= 0 ? g_attn2_poly_every : (HD == 64 ? 0 : (PS ? 8 : 7));
+    // measured (profiles/r02_README.md): with prescaled scores 8 of 16 at every head dimension (hd = 64: 4.41 -> 3.37 ms of
+    // attention per cfg5a step against all-MUFU); the unscaled form (kernel-level entry) keeps its own optimum
+    const int pe = g_attn2_poly_every >= 0 ? g_attn2_poly_every : (PS ? 8 : (HD == 64 ? 0 : 7));
     switch (pe) {
         case 0: return tc_attn2_launch_pe<HD, 0, PS>(c, QKV, N, prm, st);
         case 4: return tc_attn2_launch_pe<HD, 4, PS>(c, QKV, N, prm, st);
