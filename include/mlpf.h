@@ -194,7 +194,8 @@ int64_t mlpf_candidates_static_limit(int32_t which);   /* 0: max elements, 1: ma
                                     pre-pass, exact two-sweep path when the bound is too loose; two threads per query row);
                                     2 = the same with the exact path forced for every CTA; 0 = round 1's lazy-rescale kernel */
 #define MLPF_OPT_ATTN_POLY   9   /* tuning (process-wide): n of every 16 pairs of softmax exponentials run as a polynomial on the
-                                    FMA pipe instead of the MUFU: 0 (none), 4, 7, 8; -1 (default) = 7 at hd <= 32, 0 at hd = 64 */
+                                    FMA pipe instead of the MUFU: 0 (none), 4, 7, 8, 9; -1 (default) = 8 in the model path (scores prescaled by a3's
+                                    epilogue); 7 at hd <= 32, 0 at hd = 64 for the unscaled kernel-level entry          */
 #define MLPF_OPT_COMPACT     10  /* 1 (default): pad rows (type 0) are dropped after a0: every later step runs on the compacted rows
                                     (events stay contiguous, oracle.schedule comp_row / offsets_c), outputs are scattered back;
                                     0: pad rows stay in place and are masked as keys (round 1's behaviour)                   */
@@ -207,7 +208,9 @@ int64_t mlpf_candidates_static_limit(int32_t which);   /* 0: max elements, 1: ma
                                     (tcgen05 kind::f8f6f4; one scale per weight matrix, a fixed scale of 16 for the LayerNorm
                                     output, fp32 accumulate); 0 (default): BF16.  The measured drift is in DESIGN.md.          */
 #define MLPF_OPT_EPI_NORMS   14  /* 1 (default): the attention softmax bound's inputs (|q| per row and head, max |k| per event and
-                                    head) come out of the QKV projection's epilogue; 0: a separate pre-pass kernel computes them */
+                                    head) come out of the QKV projection's epilogue, which also folds the softmax scale log2(e) / sqrt(hd)
+                                    into q before its bf16 rounding (the attention kernel then exponentiates q k as it is and, on its
+                                    fast path, subtracts nothing); 0: unscaled q, a separate pre-pass kernel computes the norms        */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0

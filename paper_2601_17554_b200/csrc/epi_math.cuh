@@ -7,23 +7,26 @@
 namespace mlpf {
 
 // exact-erf GELU (reading A6) on two values, erf from Abramowitz & Stegun 7.1.26 (|error| <= 1.5e-7):
-//   GELU(x) = max(x, 0) - 0.5 |x| p(t) e^{-x^2/2},  t = 1 / (1 + 0.3275911 |x| / sqrt 2)
-// (for x < 0 this is 0.5 x (1 - erf|x/sqrt 2|) with no cancellation).  4 MUFU + ~18 FMA-pipe issue slots per
-// PAIR (packed FFMA2 / FMUL2) instead of erff's ~40 per value: the activation epilogues are issue-bound.
+//   GELU(x) = x/2 + |x| (1/2 - p(t) e^{-x^2/2} / 2),  t = 1 / (1 + 0.3275911 |x| / sqrt 2)
+// (= max(x, 0) - |x| p e / 2: for x < 0 this is 0.5 x (1 - erf|x/sqrt 2|); the two halves x/2 and |x|/2 cancel exactly
+// up to the rounding of the last FMA).  The factor -1/2 is folded into the polynomial's coefficients.  4 MUFU + 13 other
+// issue slots per PAIR (packed FFMA2 / FMUL2; |x| is two LOP3) instead of erff's ~40 per value: the activation epilogues
+// are issue-bound.
 __device__ __forceinline__ float2 gelu2(float2 x) {
+    const float2 ax = make_float2(fabsf(x.x), fabsf(x.y));
+    const float2 d = ptx::ffma2(ax, make_float2(0.23164189f, 0.23164189f), make_float2(1.0f, 1.0f));
     float2 t;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t.x) : "f"(fmaf(fabsf(x.x), 0.23164189f, 1.0f)));
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t.y) : "f"(fmaf(fabsf(x.y), 0.23164189f, 1.0f)));
-    float2 p = ptx::ffma2(t, make_float2(1.061405429f, 1.061405429f), make_float2(-1.453152027f, -1.453152027f));
-    p = ptx::ffma2(p, t, make_float2(1.421413741f, 1.421413741f));
-    p = ptx::ffma2(p, t, make_float2(-0.284496736f, -0.284496736f));
-    p = ptx::ffma2(p, t, make_float2(0.254829592f, 0.254829592f));
-    p = ptx::fmul2(p, t);
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t.x) : "f"(d.x));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t.y) : "f"(d.y));
+    float2 p = ptx::ffma2(t, make_float2(-0.5f * 1.061405429f, -0.5f * 1.061405429f), make_float2(0.5f * 1.453152027f, 0.5f * 1.453152027f));
+    p = ptx::ffma2(p, t, make_float2(-0.5f * 1.421413741f, -0.5f * 1.421413741f));
+    p = ptx::ffma2(p, t, make_float2(0.5f * 0.284496736f, 0.5f * 0.284496736f));
+    p = ptx::ffma2(p, t, make_float2(-0.5f * 0.254829592f, -0.5f * 0.254829592f));
+    p = ptx::fmul2(p, t);                                                                                        // -p(t) / 2
     const float2 xx = ptx::fmul2(ptx::fmul2(x, x), make_float2(-0.72134752044448170f, -0.72134752044448170f));  // -x^2/2 log2 e
     const float2 e = make_float2(ptx::fast_exp2(xx.x), ptx::fast_exp2(xx.y));
-    const float2 a = make_float2(fabsf(x.x) * -0.5f, fabsf(x.y) * -0.5f);
-    const float2 h = ptx::fmul2(ptx::fmul2(p, e), a);                     // -0.5 |x| p e
-    return ptx::fadd2(make_float2(fmaxf(x.x, 0.0f), fmaxf(x.y, 0.0f)), h);
+    const float2 w = ptx::ffma2(p, e, make_float2(0.5f, 0.5f));                                                  // 1/2 - p e / 2
+    return ptx::ffma2(ax, w, ptx::fmul2(x, make_float2(0.5f, 0.5f)));
 }
 
 template <int ACT>
