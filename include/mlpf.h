@@ -211,6 +211,9 @@ int64_t mlpf_candidates_static_limit(int32_t which);   /* 0: max elements, 1: ma
                                     head) come out of the QKV projection's epilogue, which also folds the softmax scale log2(e) / sqrt(hd)
                                     into q before its bf16 rounding (the attention kernel then exponentiates q k as it is and, on its
                                     fast path, subtracts nothing); 0: unscaled q, a separate pre-pass kernel computes the norms        */
+#define MLPF_OPT_TC_EMBED    15  /* 1 (default): the first embedding layer (fp32 weights, reading A3) runs on the tensor pipe as ONE
+                                    K = 192 grouped GEMM over bf16 terms [x_hi | x_lo | x_hi] x [W_hi | W_hi | W_lo] (relative error
+                                    ~2^-17: the x_lo W_lo term is dropped); 0: fp32 FMAs on the CUDA cores (k_embed_l1)        */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0

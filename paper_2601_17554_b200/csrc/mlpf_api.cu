@@ -63,6 +63,7 @@ struct Workspace {
     int *sorted_row = nullptr, *type_perm = nullptr;
     SchedCompact sc = {};                    // pad-row compaction arrays (a0)
     bool compact = false;                    // the last call ran on compacted rows
+    char* xa = nullptr;                      // a1 on the tensor pipe: [m_ub, 192] bf16 = [x_hi | x_lo | x_hi] per type-sorted slot
     uint8_t* u8 = nullptr;                   // e4m3 copy of the LayerNorm output feeding the QKV projection (MLPF_OPT_FP8)
     float *qn = nullptr, *kmax = nullptr;   // attention norms pre-pass: |q_i| per row and head, max |k_j| per event and head
     // device staging of mlpf_infer_host[_async] (owned by the stream's workspace, freed with it): two slots, so that the
@@ -103,6 +104,7 @@ struct mlpf_handle {
     int64_t n_params = 0, n_packed = 0;
     float* P32 = nullptr;             // packed parameters, fp32
     bf16* P16 = nullptr;              // same offsets, RNE-rounded to bf16
+    bf16* embW1p = nullptr;           // embedding first layers for the tensor pipe: [T * d, 192] = [W hi | W hi | W lo] (k padded to 64)
     bf16* W2p = nullptr;              // heads' output rows packed for tc_heads.cu: [chunk][hi | lo][16][chunk columns] bf16
     uint8_t* W8 = nullptr;            // e4m3 copies of the QKV projection matrices (NEXT-3), layer l at l * S * 3d * d bytes
     std::vector<float> w8_scale;      // per layer: W8 = e4m3(W * w8_scale)
@@ -110,7 +112,7 @@ struct mlpf_handle {
     std::vector<LayerW> layers;
     HeadsOut ho;
     // options
-    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1, graph = 0, tail_split = 1, fp8 = 0, epi_norms = 1;
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1, graph = 0, tail_split = 1, fp8 = 0, epi_norms = 1, tc_embed = 1;
     int64_t last_launches = 0;
     std::mutex mu;
     std::map<void*, Workspace*> ws;
@@ -267,6 +269,22 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
             cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W2p); delete h; return nullptr;
         }
     }
+    if (F <= 64) {   // embedding first layers (fp32 weights, A3) as three bf16 k-blocks: x W^T ~ x_hi W_hi + x_lo W_hi + x_hi W_lo
+        std::vector<uint16_t> Wp((size_t)T * d * 192, 0);
+        for (int t = 0; t < T; ++t)
+            for (int j = 0; j < d; ++j)
+                for (int k = 0; k < F; ++k) {
+                    const float wv = P[h->embW1t + ((int64_t)t * 64 + k) * d + j];
+                    const uint16_t hi = f32_to_bf16_rne(wv);
+                    uint32_t hb = (uint32_t)hi << 16; float hf; memcpy(&hf, &hb, 4);
+                    uint16_t* row = &Wp[((size_t)t * d + j) * 192];
+                    row[k] = hi; row[64 + k] = hi; row[128 + k] = f32_to_bf16_rne(wv - hf);
+                }
+        if (cudaMalloc(&h->embW1p, Wp.size() * 2) != cudaSuccess || cudaMemcpy(h->embW1p, Wp.data(), Wp.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) {
+            set_err(MLPF_E_ALLOC, "embedding weight upload failed");
+            cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W2p); cudaFree(h->embW1p); delete h; return nullptr;
+        }
+    }
     {   // e4m3 copies of Wqkv with one scale per layer (max |W| -> 448, the largest e4m3 value)
         const int64_t per = (int64_t)S * 3 * d * d;
         std::vector<uint8_t> W8((size_t)(per * L));
@@ -281,12 +299,12 @@ extern "C" mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes) {
         }
         if (cudaMalloc(&h->W8, W8.size()) != cudaSuccess || cudaMemcpy(h->W8, W8.data(), W8.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
             set_err(MLPF_E_ALLOC, "FP8 weight upload failed");
-            cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W8); cudaFree(h->W2p); delete h; return nullptr;
+            cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W8); cudaFree(h->W2p); cudaFree(h->embW1p); delete h; return nullptr;
         }
     }
     if (tc_init(&h->tc) != 0) {
         set_err(MLPF_E_CUDA, "tcgen05/TMA initialisation failed: %s", h->tc.err);
-        cudaFree(h->P32); cudaFree(h->P16); delete h; return nullptr;
+        cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W8); cudaFree(h->W2p); cudaFree(h->embW1p); delete h; return nullptr;
     }
     g_err.clear();
     return h;
@@ -298,7 +316,7 @@ extern "C" void mlpf_destroy(mlpf_handle* h) {
     if (!h) return;
     cudaDeviceSynchronize();
     for (auto& kv : h->ws) { ws_free(kv.second); delete kv.second; }
-    cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W8); cudaFree(h->W2p);
+    cudaFree(h->P32); cudaFree(h->P16); cudaFree(h->W8); cudaFree(h->W2p); cudaFree(h->embW1p);
     delete h;
 }
 
@@ -324,6 +342,9 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_ATTN:
             if (value < 0 || value > 2) return set_err(MLPF_E_ARG, "attn must be 0, 1 or 2");
             h->attn = (int)value; return MLPF_OK;
+        case MLPF_OPT_TC_EMBED:
+            if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "tc_embed must be 0 or 1");
+            h->tc_embed = (int)value; return MLPF_OK;
         case MLPF_OPT_EPI_NORMS:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "epi_norms must be 0 or 1");
             h->epi_norms = (int)value; return MLPF_OK;
@@ -391,7 +412,7 @@ template <typename P> static void dfree(P*& p) { if (p) cudaFree(p); p = nullptr
 static void ws_free_rows(Workspace* w) {
     dfree(w->h); dfree(w->u); dfree(w->qkv); dfree(w->o); dfree(w->g); dfree(w->u_lo); dfree(w->o_lo); dfree(w->g_lo);
     dfree(w->valid); dfree(w->valid_bits); dfree(w->row_event); dfree(w->row_pos); dfree(w->block_counts); dfree(w->block_base);
-    dfree(w->sorted_row); dfree(w->type_perm); dfree(w->type_offsets); dfree(w->qn); dfree(w->u8);
+    dfree(w->sorted_row); dfree(w->type_perm); dfree(w->type_offsets); dfree(w->qn); dfree(w->u8); dfree(w->xa);
     dfree(w->sc.block_vbase); dfree(w->sc.n_comp); dfree(w->sc.vbefore); dfree(w->sc.comp_row); dfree(w->sc.orig_row);
     dfree(w->sc.row_event_c); dfree(w->sc.comp_type_perm);
     w->cap_rows = 0;
@@ -429,7 +450,8 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
             dmalloc(&w->type_offsets, 8 * 4, w) || dmalloc(&w->qn, cap * h->H * 4, w) ||
             dmalloc(&w->sc.block_vbase, nb * 4, w) || dmalloc(&w->sc.n_comp, 4, w) || dmalloc(&w->sc.vbefore, cap * 4, w) ||
             dmalloc(&w->sc.comp_row, cap * 4, w) || dmalloc(&w->sc.orig_row, cap * 4, w) || dmalloc(&w->sc.row_event_c, cap * 4, w) ||
-            dmalloc(&w->sc.comp_type_perm, m_ub * 4, w) || dmalloc(&w->u8, cap * d, w)) {
+            dmalloc(&w->sc.comp_type_perm, m_ub * 4, w) || dmalloc(&w->u8, cap * d, w) ||
+            dmalloc(&w->xa, m_ub * 192 * 2, w)) {
             const char* why = cudaGetErrorString(cudaGetLastError());
             ws_free_rows(w);                       // release the partial set; nothing dangling is left behind
             w->bytes = ws_bytes_events(w);
@@ -443,6 +465,7 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
         cudaMemsetAsync(w->valid, 0, cap * 4, st); cudaMemsetAsync(w->row_event, 0, cap * 4, st);
         cudaMemsetAsync(w->sc.row_event_c, 0, cap * 4, st);
         cudaMemsetAsync(w->u8, 0, cap * d, st);
+        cudaMemsetAsync(w->xa, 0, m_ub * 192 * 2, st);
         cudaMemsetAsync(w->u, 0, cap * d * es, st); cudaMemsetAsync(w->qkv, 0, cap * 3 * d * es, st);
         cudaMemsetAsync(w->o, 0, cap * d * es, st);
         cudaMemsetAsync(w->g, 0, w->g_elems * es, st);
@@ -635,10 +658,23 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     }
 
     // ---- a1: per-type embedding (L156; A3-A5)
+    // first layer: on the tensor pipe (bf16 hi + lo terms of the fp32 features and weights in one K = 192 grouped GEMM) when
+    // the rows are compacted (pad rows need no zero rows in h then); else fp32 FMAs on the CUDA cores
+    const bool tc_embed = tc && compact && h->tc_embed && h->embW1p;
     {
     ProfScope ps(h, w, st, MLPF_KC_EMBED_L1);
-    launch_embed_l1(fp32, X, N, h->F, d, PV + h->embW1t, PV + h->embB1, h->act, w->sorted_row, g, lo(MLPF_SPLIT_EMB, w->g_lo),
-                    compact ? nullptr : w->h, st);
+    if (tc_embed) {
+        launch_embed_pack(X, N, h->F, w->sorted_row, w->xa, st);
+        LAUNCH_CHECK(h);
+        Epi ep;
+        ep.bias = PV + h->embB1; ep.act = h->act; ep.out_act = g; ep.ld_act = d; ep.out_act_lo = lo(MLPF_SPLIT_EMB, w->g_lo);
+        ep.group_offsets = w->type_offsets; ep.n_groups = 4;
+        if (tc_gemm_launch(&h->tc, (const bf16*)w->xa, nullptr, h->embW1p, (int)w->m_ub, d, 192, ep, st))
+            return set_err(MLPF_E_CUDA, "tcgen05 GEMM launch failed: %s", h->tc.err);
+    } else {
+        launch_embed_l1(fp32, X, N, h->F, d, PV + h->embW1t, PV + h->embB1, h->act, w->sorted_row, g, lo(MLPF_SPLIT_EMB, w->g_lo),
+                        compact ? nullptr : w->h, st);
+    }
     LAUNCH_CHECK(h);
     }
     {
@@ -910,7 +946,7 @@ extern "C" int mlpf_infer_ex(mlpf_handle* h, const float* elements, const int32_
         push64((uint64_t)(uintptr_t)elements); push64((uint64_t)(uintptr_t)out_logits); push64((uint64_t)(uintptr_t)out_regress);
         push64((uint64_t)(uintptr_t)out_binary);
         key.push_back(h->precision); key.push_back(h->kernels); key.push_back(h->split); key.push_back(h->fuse);
-        key.push_back(h->attn); key.push_back(h->compact); key.push_back(h->epi_norms); key.push_back(h->fp8); key.push_back(h->tail_split); key.push_back(h->tile_q); key.push_back(g_attn2_poly_every);
+        key.push_back(h->attn); key.push_back(h->compact); key.push_back(h->epi_norms); key.push_back(h->tc_embed); key.push_back(h->fp8); key.push_back(h->tail_split); key.push_back(h->tile_q); key.push_back(g_attn2_poly_every);
         key.insert(key.end(), event_offsets, event_offsets + n_off);
         for (auto& ge : w->graphs)
             if (ge.key == key) {

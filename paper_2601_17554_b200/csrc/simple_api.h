@@ -27,6 +27,8 @@ int launch_schedule(const float* X, int N, int F, const int* offsets, int E, int
                     int* valid, uint32_t* valid_bits, int* row_event, int* row_pos, int* n_valid, int* type_offsets, int* sorted_row,
                     int* type_perm, const SchedCompact& sc, cudaStream_t st);
 void launch_uncompact(const float* src, const int* comp_row, float* out, int64_t N, int cols, cudaStream_t st);
+// X [N, F <= 64] fp32 -> xa [slots, 192] bf16 = [x_hi | x_lo | x_hi] at the rows' type-sorted slots (pad rows skipped)
+void launch_embed_pack(const float* X, int N, int F, const int* sorted_row, void* xa, cudaStream_t st);
 void launch_embed_l1(bool fp32, const float* X, int N, int F, int d, const float* W1t, const float* b1, int act,
                      const int* sorted_row, void* h1, void* h1_lo, float* h, cudaStream_t st);
 int launch_layernorm(bool fp32, int d, const float* x, int N, const float* g, const float* b, float eps, void* u,

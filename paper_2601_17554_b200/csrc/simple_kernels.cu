@@ -828,6 +828,45 @@ int launch_schedule(const float* X, int N, int F, const int* offsets, int E, int
     return 4;
 }
 
+// a1 on the tensor pipe, step 1: the fp32 features of every non-pad row as bf16 terms in its type-sorted slot,
+//   xa[slot] = [x_hi | x_lo | x_hi]  (3 x 64 columns, features padded with zeros to 64),  x_hi = T(x), x_lo = T(x - x_hi),
+// so that ONE K = 192 GEMM against [W_hi | W_hi | W_lo] (built in mlpf_create) gives x W^T to ~2^-17 relative (the x_lo W_lo
+// term is dropped): the first embedding layer keeps its fp32 weights' precision (reading A3) on the bf16 tensor pipe.
+constexpr int PACK_ROWS = 32;
+__global__ void __launch_bounds__(256)
+k_embed_pack(const float* __restrict__ X, int N, int F, const int* __restrict__ sorted_row, bf16* __restrict__ xa) {
+    __shared__ float xs[PACK_ROWS][64];
+    __shared__ int slot[PACK_ROWS];
+    const int row0 = blockIdx.x * PACK_ROWS;
+    const int rows = min(PACK_ROWS, N - row0);
+    for (int idx = threadIdx.x; idx < PACK_ROWS * 64; idx += 256) {
+        const int r = idx >> 6, k = idx & 63;
+        xs[r][k] = (r < rows && k < F) ? X[(int64_t)(row0 + r) * F + k] : 0.0f;
+    }
+    if (threadIdx.x < PACK_ROWS)
+        slot[threadIdx.x] = (threadIdx.x < rows && element_type(X, row0 + threadIdx.x, F) != 0) ? sorted_row[row0 + threadIdx.x] : -1;
+    __syncthreads();
+    // 24 16-byte pieces per row: piece c = segment c / 8 (hi, lo, hi), features 8 (c % 8) .. + 7
+    for (int idx = threadIdx.x; idx < PACK_ROWS * 24; idx += 256) {
+        const int r = idx / 24, c = idx % 24;
+        const int sl = slot[r];
+        if (sl < 0) continue;
+        const float* xp = &xs[r][(c & 7) * 8];
+        uint32_t w[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            float2 v = make_float2(xp[2 * i], xp[2 * i + 1]);
+            __nv_bfloat162 h2 = __floats2bfloat162_rn(v.x, v.y);
+            if ((c >> 3) == 1) h2 = __floats2bfloat162_rn(v.x - __low2float(h2), v.y - __high2float(h2));
+            w[i] = *reinterpret_cast<uint32_t*>(&h2);
+        }
+        *reinterpret_cast<uint4*>(xa + (int64_t)sl * 192 + c * 8) = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+}
+void launch_embed_pack(const float* X, int N, int F, const int* sorted_row, void* xa, cudaStream_t st) {
+    k_embed_pack<<<(N + PACK_ROWS - 1) / PACK_ROWS, 256, 0, st>>>(X, N, F, sorted_row, (bf16*)xa);
+}
+
 void launch_embed_l1(bool fp32, const float* X, int N, int F, int d, const float* W1t, const float* b1, int act,
                      const int* sorted_row, void* h1, void* h1_lo, float* h, cudaStream_t st) {
     dim3 grid((N + EMB_ROWS - 1) / EMB_ROWS);

@@ -185,6 +185,34 @@ def test_per_step_intermediates(name, max_events, precision, tol):
         assert _rel(mod.tensor("H", (N, d)), dump[p + "h"], valid) <= tol, "h"
 
 
+@pytest.mark.parametrize("name,max_events", [("cfg1", None), ("cfg2", 3), ("paper", 1)])
+def test_tensor_pipe_embedding_matches_the_oracle_as_well_as_the_fp32_first_layer(name, max_events):
+    """MLPF_OPT_TC_EMBED: the first embedding layer (fp32 weights, reading A3) as one K = 192 bf16 GEMM over hi + lo terms
+    of features and weights.  Features span orders of magnitude (energies, angles, flags), so the check is against the
+    fp64 oracle's embedding output with FP32 first-layer weights (what the CUDA-core kernel computes) at a tolerance far
+    below the step's 2e-2: both first layers must sit at the level of the bf16 hi + lo rounding of the hidden layer."""
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    X, off = synth.make_named_events(name, max_events=max_events)
+    X = X.copy()
+    X[X[:, 0] != 0, 4] *= 37.0                     # energies up to a few 1e3: the hi + lo split has to carry them
+    N, d = X.shape[0], m.d_model
+    valid = X[:, 0] != 0
+    dump = {}
+    oracle.forward(X, off, oracle.quantize_weights(W), m, dump=dump)
+    errs = {}
+    for tc_embed in (0, 1):
+        mod = P.Mlpf(W, m)
+        mod.set_option(P.OPT_TC_EMBED, tc_embed)
+        mod.set_option(P.OPT_TAP_LAYER, -2)
+        mod.infer(torch.from_numpy(X).cuda(), off)
+        torch.cuda.synchronize()
+        errs[tc_embed] = _rel(mod.tensor("H", (N, d)), dump["h0"], valid)
+    # measured (paper config): 1.4e-4 with the fp32 first layer (the hidden layer's own bf16 hi + lo rounding, 2^-17, through
+    # the second layer's dot products), 2.4e-4 on the tensor pipe (the hi + lo terms of x and W1 add 2^-17 each)
+    assert errs[0] <= 5e-4 and errs[1] <= 5e-4, errs
+
+
 # ------------------------------------------------------------------------------------------- edge cases
 TINY = ModelCfg(n_layers=2, d_model=64, n_heads=4, d_ff=256)
 
