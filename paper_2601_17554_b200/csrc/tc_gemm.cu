@@ -198,6 +198,11 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     const int total_tiles = ((M + GEMM_BM - 1) / GEMM_BM) * n_tiles_n;
     const int m_end = ep.group_offsets ? ep.group_offsets[ep.n_groups + 1] : M;   // grouped: rows beyond the last group
     const int nc_rows = ep.nc_dev ? __ldg(ep.nc_dev) : 0x7fffffff;
+    // tile -> (m tile, n tile) without a division per tile (every epilogue warp walks all of the CTA's tiles and the epilogue
+    // is issue bound): (mi, ni) advance by gridDim.x = dq * n_tiles_n + dr
+    const int dq = gridDim.x / n_tiles_n, dr = gridDim.x % n_tiles_n;
+    const int mi0 = blockIdx.x / n_tiles_n, ni0 = blockIdx.x % n_tiles_n;
+    auto advance = [&](int& mi, int& ni) { mi += dq; ni += dr; if (ni >= n_tiles_n) { ni -= n_tiles_n; ++mi; } };
     // tiles without meaningful rows (all three roles skip the same ones)
     auto skip_tile = [&](int m0) { return m0 >= m_end || (ep.group_rows > 0 ? m0 % ep.group_rows : m0) >= nc_rows; };
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -227,8 +232,9 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     if (warp == 0) {
         // ---------------- TMA producer: the stage ring runs on across tiles
         uint32_t kbg = 0;
-        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-            const int m0 = (tile / n_tiles_n) * GEMM_BM, n0 = (tile % n_tiles_n) * BLOCK_N;
+        int mi = mi0, ni = ni0;
+        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, advance(mi, ni)) {
+            const int m0 = mi * GEMM_BM, n0 = ni * BLOCK_N;
             if (skip_tile(m0)) continue;
             int w_row0 = 0;
             if (ep.group_offsets) {                               // grouped GEMM (per-type embedding weights)
@@ -255,8 +261,9 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         constexpr uint32_t idesc = FP8 ? ptx::umma_idesc_e4m3(GEMM_BM, BLOCK_N) : ptx::umma_idesc_bf16(GEMM_BM, BLOCK_N);
         uint32_t kbg = 0;
         int it = 0;
-        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-            if (skip_tile((tile / n_tiles_n) * GEMM_BM)) continue;
+        int mi = mi0, ni = ni0;
+        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, advance(mi, ni)) {
+            if (skip_tile(mi * GEMM_BM)) continue;
             const int buf = it & 1;
             ptx::mbar_wait(bar_acc_empty + 8 * buf, ((it >> 1) & 1) ^ 1);      // the epilogue drained this buffer
             ptx::tc_fence_after();
@@ -289,8 +296,9 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         const int tid = ((ew >> 3) * 4 + (ew & 3)) * 32 + lane;   // 0..255 among the threads serving buffer e
         uint8_t* stg = smem_raw + (smem_base - ptx::smem_u32(smem_raw)) + STAGES * Cfg::STAGE_BYTES + ew * GEMM_STG_BYTES;
         int it = 0;
-        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-            const int m0 = (tile / n_tiles_n) * GEMM_BM, n0 = (tile % n_tiles_n) * BLOCK_N;
+        int mi = mi0, ni = ni0;
+        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, advance(mi, ni)) {
+            const int m0 = mi * GEMM_BM, n0 = ni * BLOCK_N;
             if (skip_tile(m0)) continue;
             if ((it & 1) != e) { ++it; continue; }
             int w_row0 = 0;
@@ -310,7 +318,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             int row = m;
             if (row_ok && ep.row_perm) row = ep.row_perm[m];
             const bool write_ok = row_ok && row >= 0;
-            ptx::mbar_wait(bar_acc_full + 8 * e, (it >> 1) & 1);
+            ptx::mbar_wait_long(bar_acc_full + 8 * e, (it >> 1) & 1);   // (suspends: a spinning warp takes issue slots from the working ones)
             ptx::tc_fence_after();
             const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + e * BLOCK_N + hcol;
             const int srow = write_ok ? row : -1;                 // destination row of this lane's accumulator row
@@ -321,9 +329,11 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             int n_ev = -1;
             if (norms && row_ok && (ep.group_rows > 0 ? m % ep.group_rows : m) < nc_rows) n_ev = __ldg(ep.row_event + m);
             float n_ss = 0.0f;
+            // (no runtime division in this epilogue: the head width is a power of two, q | k | v by comparison)
+            const int hd_shift = 31 - __clz(ep.nhd | 1);
             auto norm_emit = [&](int col_end) {                   // columns up to col_end (exclusive) close a head
-                if (col_end % ep.nhd) return;
-                const int blk = (col_end - 1) / ep.nd, head = ((col_end - 1) % ep.nd) / ep.nhd;
+                if (col_end & (ep.nhd - 1)) return;
+                const int blk = col_end > ep.nd ? 1 : 0, head = (col_end - 1 - blk * ep.nd) >> hd_shift;
                 const float nrm = sqrtf(n_ss);
                 n_ss = 0.0f;
                 if (blk == 0) { if (n_ev >= 0) ep.qn[(int64_t)m * ep.nH + head] = nrm; }
