@@ -214,6 +214,10 @@ int64_t mlpf_candidates_static_limit(int32_t which);   /* 0: max elements, 1: ma
 #define MLPF_OPT_TC_EMBED    15  /* 1 (default): the first embedding layer (fp32 weights, reading A3) runs on the tensor pipe as ONE
                                     K = 192 grouped GEMM over bf16 terms [x_hi | x_lo | x_hi] x [W_hi | W_hi | W_lo] (relative error
                                     ~2^-17: the x_lo W_lo term is dropped); 0: fp32 FMAs on the CUDA cores (k_embed_l1)        */
+#define MLPF_OPT_PDL         16  /* 1: the tensor-core kernels are launched as programmatic dependents of the kernel before them (their
+                                    set-up and first wave overlap its tail; griddepcontrol.wait orders every access); 0: plain stream
+                                    order; 2 (default): 1 for calls whose attention grid is at most two waves of CTAs (one event per
+                                    call: 0.847 -> 0.823 ms), else 0 (no gain on large batches)                              */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0

@@ -46,6 +46,7 @@ struct LayerW {                       // element offsets into the packed paramet
     int64_t ln1g, ln1b, Wqkv, bqkv, Wo, bo, ln2g, ln2b, W1, b1, W2, b2;
 };
 struct Workspace {
+    float* kmax_cur = nullptr;        // the current layer's block of kmax
     float q_prescale = 1.0f;          // the q columns of qkv carry this factor (softmax scale folded into a3's epilogue), 1 = none
     int64_t cap_rows = 0;             // capacity in rows (multiple of 128)
     int64_t cap_events = 0, cap_tiles = 0;
@@ -112,7 +113,7 @@ struct mlpf_handle {
     std::vector<LayerW> layers;
     HeadsOut ho;
     // options
-    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1, graph = 0, tail_split = 1, fp8 = 0, epi_norms = 1, tc_embed = 1;
+    int precision = MLPF_PREC_BF16, kernels = MLPF_KERNELS_TC, tile_q = 128, tap_layer = -1, split = MLPF_SPLIT_ALL, profile = 0, fuse = 1, attn = 1, compact = 1, graph = 0, tail_split = 1, fp8 = 0, epi_norms = 1, tc_embed = 1, pdl = 2;
     int64_t last_launches = 0;
     std::mutex mu;
     std::map<void*, Workspace*> ws;
@@ -342,6 +343,9 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_ATTN:
             if (value < 0 || value > 2) return set_err(MLPF_E_ARG, "attn must be 0, 1 or 2");
             h->attn = (int)value; return MLPF_OK;
+        case MLPF_OPT_PDL:
+            if (value < 0 || value > 2) return set_err(MLPF_E_ARG, "pdl must be 0, 1 or 2");
+            h->pdl = (int)value; return MLPF_OK;
         case MLPF_OPT_TC_EMBED:
             if (value != 0 && value != 1) return set_err(MLPF_E_ARG, "tc_embed must be 0 or 1");
             h->tc_embed = (int)value; return MLPF_OK;
@@ -421,7 +425,7 @@ static void ws_free_rows(Workspace* w) {
 static int64_t ws_bytes_events(const Workspace* w) {
     int64_t b = 0;
     if (w->offsets) b += std::max<int64_t>((w->cap_events + 1) * 4, 256) + std::max<int64_t>(w->cap_events * 4, 256);
-    if (w->kmax) b += std::max<int64_t>(w->cap_events * 64 * 4, 256) + std::max<int64_t>((w->cap_events + 1) * 4, 256);   // upper bound (H <= 64)
+    if (w->kmax) b += std::max<int64_t>(w->cap_events * 64 * 4 * 8, 256) + std::max<int64_t>((w->cap_events + 1) * 4, 256);   // upper bound (H <= 64, L <= 8)
     if (w->work) b += 2 * std::max<int64_t>(w->cap_tiles * 8, 256);
     return b;
 }
@@ -477,7 +481,7 @@ static int ws_ensure(mlpf_handle* h, Workspace* w, int64_t N, int64_t E, int64_t
         dfree(w->offsets); dfree(w->n_valid); dfree(w->kmax); dfree(w->sc.offsets_c);
         w->cap_events = 0;
         const int64_t ce = std::max<int64_t>(E, 64);
-        if (dmalloc(&w->offsets, (ce + 1) * 4, w) || dmalloc(&w->n_valid, ce * 4, w) || dmalloc(&w->kmax, ce * h->H * 4, w) ||
+        if (dmalloc(&w->offsets, (ce + 1) * 4, w) || dmalloc(&w->n_valid, ce * 4, w) || dmalloc(&w->kmax, ce * h->H * 4 * h->L, w) ||        /* one [events, H] block per layer: zeroed once per call */
             dmalloc(&w->sc.offsets_c, (ce + 1) * 4, w)) {
             dfree(w->offsets); dfree(w->n_valid); dfree(w->kmax); dfree(w->sc.offsets_c);
             return set_err(MLPF_E_ALLOC, "workspace allocation for %lld events failed", (long long)ce);
@@ -575,7 +579,7 @@ static int run_attention(mlpf_handle* h, bool fp32, bool tc, bool split, Workspa
                                 split ? (bf16*)w->o_lo : nullptr, st);
         else {
             rc = tc_attn2_launch(&h->tc, (const bf16*)w->qkv, w->Mtot, (int)w->Ev, valid_bits, n_valid, offsets, row_event,
-                                 (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, w->qn, w->kmax, (bf16*)w->o,
+                                 (const int2*)w->pairs, (int)w->n_pairs, h->d, h->H, w->qn, w->kmax_cur, (bf16*)w->o,
                                  split ? (bf16*)w->o_lo : nullptr, h->attn == 2, w->compact ? w->sc.n_comp : nullptr,
                                  h->S > 1 ? (int)w->Npad : 0, st, norms_ready, prescaled);
             if (!norms_ready) h->last_launches++;     // the norms pre-pass
@@ -644,6 +648,17 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     void* u = w->u; void* g = w->g;
     auto lo = [&](int bit, void* p) { return (sm & bit) ? p : (void*)nullptr; };
 
+    // programmatic dependent launches pay where launch latency and kernel prologues show: calls whose attention grid is at
+    // most two waves (one event per call: 0.847 -> 0.823 ms); on the 8-event batch they measure 0.2 % slower (auto = 2)
+    h->tc.pdl = h->pdl == 1 || (h->pdl == 2 && w->n_pairs * h->H <= 2 * (int64_t)h->tc.num_sms);
+    // all heads as one kernel per stack (tc_heads.cu): it scatters to the valid rows only, the pad rows are zeroed here, ahead
+    // of every kernel of the call
+    const bool heads_fused = tc && h->fuse && compact && h->W2p && (sm & MLPF_SPLIT_UF) && tc_heads_supported(d, h->n_hblk);
+    if (heads_fused && h->tap_layer == -1) {
+        CUDA_TRY(cudaMemsetAsync(out_logits, 0, (size_t)N * h->C * 4, st));
+        if (h->R) CUDA_TRY(cudaMemsetAsync(out_regress, 0, (size_t)N * h->R * 4, st));
+        if (out_binary) CUDA_TRY(cudaMemsetAsync(out_binary, 0, (size_t)N * 4, st));
+    }
     // ---- a0 (device half)
     w->prof_cls.clear();
     w->h_tiled = false;
@@ -714,8 +729,12 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
     // the unfused chain of round 1 runs.
     const bool fused = tc && h->fuse && (sm | MLPF_SPLIT_HEAD | MLPF_SPLIT_EMB) == MLPF_SPLIT_ALL && tc_post_supported(d, dff);   // the fused block carries o, u2, g, u_final as hi + lo
     bool u_ready = false;                    // u already holds LN(h) for the next consumer (written by a fused epilogue)
+    // (one memset for all layers, ahead of the kernels: nothing but kernels between two layers, so that each can be launched
+    // as a programmatic dependent of the one before)
+    if (epi_norms) CUDA_TRY(cudaMemsetAsync(w->kmax, 0, (size_t)h->L * w->Ev * h->H * 4, st));
     for (int l = 0; l < h->L; ++l) {
         const LayerW& lw = h->layers[l];
+        w->kmax_cur = w->kmax + (size_t)l * w->Ev * h->H;
         int rc;
         if (!u_ready) {
             ProfScope ps(h, w, st, MLPF_KC_LAYERNORM);
@@ -728,8 +747,7 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
             Epi ep;
             ep.bias = PV + lw.bqkv; ep.out_act = w->qkv; ep.ld_act = 3 * d; ep.group_rows = grp_rows; ep.n_groups = S; ep.nc_dev = nc_dev;
             if (epi_norms) {                        // |q| per row and head, max |k| per event and head for a4's softmax bound
-                CUDA_TRY(cudaMemsetAsync(w->kmax, 0, (size_t)w->Ev * h->H * 4, st));
-                ep.qn = w->qn; ep.kmax = w->kmax; ep.row_event = compact ? w->sc.row_event_c : w->row_event;
+                ep.qn = w->qn; ep.kmax = w->kmax_cur; ep.row_event = compact ? w->sc.row_event_c : w->row_event;
                 ep.nH = h->H; ep.nhd = h->hd; ep.nd = d;
                 ep.q_scale = w->q_prescale;             // q carries the softmax scale: a4 exponentiates S as it is
             }
@@ -825,13 +843,10 @@ static int infer_impl(mlpf_handle* h, bool fp32, Workspace* w, const float* X, f
         // stack's z (rows 0 .. N-1), the regression blocks the regression stack's (rows (S-1) Npad ..), L156
         const int hw = h->n_hblk * d;
         int rc = MLPF_OK;
-        if (tc && h->fuse && compact && h->W2p && (sm & MLPF_SPLIT_UF) && tc_heads_supported(d, h->n_hblk)) {
+        if (heads_fused) {
             // all heads, both layers, one kernel per encoder stack (tc_heads.cu): the hidden layers stay on chip, the
             // outputs are scattered to the original rows; pad rows are zeroed here
-            ProfScope ps(h, w, st, MLPF_KC_HEADS_L1);
-            CUDA_TRY(cudaMemsetAsync(out_logits, 0, (size_t)N * h->C * 4, st));
-            if (h->R) CUDA_TRY(cudaMemsetAsync(out_regress, 0, (size_t)N * h->R * 4, st));
-            if (out_binary) CUDA_TRY(cudaMemsetAsync(out_binary, 0, (size_t)N * 4, st));
+            ProfScope ps(h, w, st, MLPF_KC_HEADS_L1);      // (the outputs' pad rows were zeroed at the start of the call)
             const int nb0 = S > 1 ? h->n_hblk0 : h->n_hblk;
             for (int part = 0; part < (S > 1 ? 2 : 1); ++part) {
                 HeadsArgs a;
@@ -946,7 +961,7 @@ extern "C" int mlpf_infer_ex(mlpf_handle* h, const float* elements, const int32_
         push64((uint64_t)(uintptr_t)elements); push64((uint64_t)(uintptr_t)out_logits); push64((uint64_t)(uintptr_t)out_regress);
         push64((uint64_t)(uintptr_t)out_binary);
         key.push_back(h->precision); key.push_back(h->kernels); key.push_back(h->split); key.push_back(h->fuse);
-        key.push_back(h->attn); key.push_back(h->compact); key.push_back(h->epi_norms); key.push_back(h->tc_embed); key.push_back(h->fp8); key.push_back(h->tail_split); key.push_back(h->tile_q); key.push_back(g_attn2_poly_every);
+        key.push_back(h->attn); key.push_back(h->compact); key.push_back(h->epi_norms); key.push_back(h->tc_embed); key.push_back(h->pdl); key.push_back(h->fp8); key.push_back(h->tail_split); key.push_back(h->tile_q); key.push_back(g_attn2_poly_every);
         key.insert(key.end(), event_offsets, event_offsets + n_off);
         for (auto& ge : w->graphs)
             if (ge.key == key) {

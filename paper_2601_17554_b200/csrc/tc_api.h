@@ -36,7 +36,20 @@ struct TcContext {
     };
     std::unordered_map<Key, CUtensorMap, KeyHash> cache;
     std::set<std::pair<const void*, int>> attr_done;   // (kernel, device) pairs whose shared-memory limit is raised
+    bool pdl = false;                                  // launch the tensor-core kernels with programmatic stream serialization
 };
+
+// kernel launch, optionally with the programmatic-stream-serialization attribute (the kernel calls ptx::grid_dep_wait())
+template <typename... KArgs, typename... Args>
+inline cudaError_t tc_launch(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+}
 
 
 int tc_init(TcContext* c);

@@ -184,6 +184,10 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
     __shared__ uint32_t tmem_base_slot;
     __shared__ int bound_bits;                                   // max over the CTA's rows of B c (float bits)
 
+    // programmatic dependent launch: this grid's first wave may be resident before the QKV projection has finished (the
+    // work list decides whether a CTA exists at all, so the wait comes first)
+    ptx::grid_dep_wait();
+    ptx::grid_dep_launch();
     const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
     const int item = blockIdx.x / prm.H, head = blockIdx.x % prm.H;
     const int2 it = prm.items[item];
@@ -471,7 +475,7 @@ static int tc_attn2_launch_pe(TcContext* c, const bf16* QKV, int64_t N, Attn2Par
     if (tc_tensor_map(c, &tmQKV, QKV, 3 * prm.d, N, 3 * prm.d, HD, A2_SK)) return -1;
     auto kern = k_tc_attn2<HD, PE, PS>;
     if (tc_set_smem_attr(c, (const void*)kern, Cfg::SMEM_BYTES)) return -1;
-    kern<<<prm.n_items * prm.H, Cfg::THREADS, Cfg::SMEM_BYTES, st>>>(tmQKV, prm);
+    tc_launch(kern, dim3(prm.n_items * prm.H), dim3(Cfg::THREADS), Cfg::SMEM_BYTES, st, c->pdl, tmQKV, prm);
     return 0;
 }
 

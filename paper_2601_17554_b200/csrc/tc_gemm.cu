@@ -196,8 +196,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
     const int n_tiles_n = N / BLOCK_N;
     const int total_tiles = ((M + GEMM_BM - 1) / GEMM_BM) * n_tiles_n;
-    const int m_end = ep.group_offsets ? ep.group_offsets[ep.n_groups + 1] : M;   // grouped: rows beyond the last group
-    const int nc_rows = ep.nc_dev ? __ldg(ep.nc_dev) : 0x7fffffff;
+    int m_end = M, nc_rows = 0x7fffffff;       // (read from global memory after the set-up, behind grid_dep_wait)
     // tile -> (m tile, n tile) without a division per tile (every epilogue warp walks all of the CTA's tiles and the epilogue
     // is issue bound): (mi, ni) advance by gridDim.x = dq * n_tiles_n + dr
     const int dq = gridDim.x / n_tiles_n, dr = gridDim.x % n_tiles_n;
@@ -228,6 +227,11 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     ptx::tc_fence_after();
     const uint32_t tmem_base = tmem_base_slot;
     const int num_kb = K / (FP8 ? 2 * GEMM_BK : GEMM_BK);
+    // programmatic dependent launch: the set-up above may overlap the previous kernel's tail; nothing below may
+    ptx::grid_dep_wait();
+    ptx::grid_dep_launch();
+    if (ep.group_offsets) m_end = ep.group_offsets[ep.n_groups + 1];            // grouped: rows beyond the last group
+    if (ep.nc_dev) nc_rows = __ldg(ep.nc_dev);
 
     if (warp == 0) {
         // ---------------- TMA producer: the stage ring runs on across tiles
@@ -393,7 +397,7 @@ static int tc_gemm_launch_act(TcContext* c, const bf16* A, const bf16* A_lo, con
     if (tc_set_smem_attr(c, (const void*)kern, Cfg::SMEM_BYTES)) return -1;
     const int total_tiles = ((M + GEMM_BM - 1) / GEMM_BM) * (N / BLOCK_N);
     const int grid = total_tiles < c->num_sms ? total_tiles : c->num_sms;
-    kern<<<grid, GEMM_THREADS, Cfg::SMEM_BYTES, st>>>(tmA, tmAlo, tmB, M, N, K, ep);
+    tc_launch(kern, dim3(grid), dim3(GEMM_THREADS), Cfg::SMEM_BYTES, st, c->pdl, tmA, tmAlo, tmB, M, N, K, ep);
     return 0;
 }
 

@@ -51,7 +51,7 @@ k_tc_heads(const __grid_constant__ CUtensorMap tmZ, const __grid_constant__ CUte
     const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
     const int n_tiles = (p.M + HD_BM - 1) / HD_BM;
     const int NC = p.nblk * CPB;
-    const int nc_rows = p.nc_dev ? __ldg(p.nc_dev) : 0x7fffffff;
+    int nc_rows = 0x7fffffff;                  // (read after the set-up, behind grid_dep_wait)
     auto skip_tile = [&](int tile) { return tile * HD_BM >= nc_rows; };
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* const smem_gen = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
@@ -73,11 +73,15 @@ k_tc_heads(const __grid_constant__ CUtensorMap tmZ, const __grid_constant__ CUte
         ptx::tmem_alloc(ptx::smem_u32(&tmem_base_slot), 512);
         ptx::tmem_relinquish();
     }
-    for (int i = threadIdx.x; i < p.nblk * D; i += HD_THREADS) v_b1[i] = __ldg(p.b1 + i);
+    for (int i = threadIdx.x; i < p.nblk * D; i += HD_THREADS) v_b1[i] = __ldg(p.b1 + i);     // (weights: not the predecessor's)
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem_base = tmem_base_slot;
+    // programmatic dependent launch: the set-up above may overlap the previous kernel's tail; nothing below may
+    ptx::grid_dep_wait();
+    ptx::grid_dep_launch();
+    if (p.nc_dev) nc_rows = __ldg(p.nc_dev);
 
     if (warp == 0) {
         // ------------------------------------------------------------ TMA producer
@@ -297,7 +301,7 @@ static int tc_heads_launch_t(TcContext* c, const HeadsArgs& a, cudaStream_t st) 
     }
     const int n_tiles = (a.M + HD_BM - 1) / HD_BM;
     const int grid = n_tiles < c->num_sms ? n_tiles : c->num_sms;
-    kern<<<grid, HD_THREADS, Cfg::smem_bytes(a.nblk), st>>>(tmZ, tmZlo, tmW1, tmW2, p);
+    tc_launch(kern, dim3(grid), dim3(HD_THREADS), Cfg::smem_bytes(a.nblk), st, c->pdl, tmZ, tmZlo, tmW1, tmW2, p);
     return 0;
 }
 

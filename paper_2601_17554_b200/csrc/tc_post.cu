@@ -120,7 +120,7 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
     const int warp = ptx::uniform_warp_idx(), lane = threadIdx.x & 31;
     const int n_tiles = (p.M + POST_BM - 1) / POST_BM;
     const int NC = p.dff / POST_CH;
-    const int nc_rows = p.nc_dev ? __ldg(p.nc_dev) : 0x7fffffff;
+    int nc_rows = 0x7fffffff;                  // (read after the set-up, behind grid_dep_wait)
     auto skip_tile = [&](int tile) { return (tile * POST_BM) % p.group_rows >= nc_rows; };   // all three roles skip the same tiles
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* const smem_gen = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
@@ -150,6 +150,10 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
     __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem_base = tmem_base_slot;
+    // programmatic dependent launch: the set-up above may overlap the previous kernel's tail; nothing below may
+    ptx::grid_dep_wait();
+    ptx::grid_dep_launch();
+    if (p.nc_dev) nc_rows = __ldg(p.nc_dev);
 
     if (warp == 0) {
         // ------------------------------------------------------------ TMA producer: loads in exactly the issuer's order
@@ -502,7 +506,7 @@ static int tc_post_launch_t(TcContext* c, const PostArgs& a, cudaStream_t st) {
     p.dbg_u2 = a.dbg_u2; p.dbg_g = a.dbg_g; p.u_out_f8 = a.u_out_f8; p.f8_scale = a.f8_scale;
     const int n_tiles = (a.M + POST_BM - 1) / POST_BM;
     const int grid = n_tiles < c->num_sms ? n_tiles : c->num_sms;
-    kern<<<grid, POST_THREADS, smem, st>>>(tmO, tmOlo, tmWo, tmW1, tmW2, p);
+    tc_launch(kern, dim3(grid), dim3(POST_THREADS), smem, st, c->pdl, tmO, tmOlo, tmWo, tmW1, tmW2, p);
     return 0;
 }
 

@@ -213,6 +213,29 @@ def test_tensor_pipe_embedding_matches_the_oracle_as_well_as_the_fp32_first_laye
     assert errs[0] <= 5e-4 and errs[1] <= 5e-4, errs
 
 
+@pytest.mark.parametrize("name,max_events", [("cfg2", None), ("cfg3", 2)])
+def test_programmatic_dependent_launch_changes_nothing(name, max_events):
+    """MLPF_OPT_PDL: the tensor-core kernels start while their predecessor's last wave drains and order every access with
+    griddepcontrol.wait: outputs bit-identical to plain stream order, call after call."""
+    m = synth.model_cfg(name)
+    W = synth.make_weights(name)
+    X, off = synth.make_named_events(name, max_events=max_events)
+    Xd = torch.from_numpy(X).cuda()
+    out = {}
+    for pdl in (0, 1):
+        mod = P.Mlpf(W, m)
+        mod.set_option(P.OPT_PDL, pdl)
+        runs = []
+        for _ in range(3):
+            lg, rg = mod.infer(Xd, off)
+            torch.cuda.synchronize()
+            runs.append((lg.clone(), rg.clone()))
+        for lg, rg in runs[1:]:
+            assert torch.equal(lg, runs[0][0]) and torch.equal(rg, runs[0][1])
+        out[pdl] = runs[0]
+    assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1])
+
+
 # ------------------------------------------------------------------------------------------- edge cases
 TINY = ModelCfg(n_layers=2, d_model=64, n_heads=4, d_ff=256)
 
