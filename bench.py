@@ -417,14 +417,20 @@ def run_ours(args):
     bf16x2_rate = P.microbench(1, 4096, stream=st)
     clk = (sampler.result()["sm_mhz"] or sampler.result()["sm_max_mhz"] or 1965.0) * 1e6
     nsm = torch.cuda.get_device_properties(0).multi_processor_count
-    poly_share = (7.0 / 16.0) if m.head_dim <= 32 else 0.0
+    # the library's default (include/mlpf.h MLPF_OPT_ATTN_POLY): 8 of 16 pairs with the prescaled scores of the model path;
+    # 7 (hd <= 32) / 0 (hd = 64) with MLPF_OPT_EPI_NORMS = 0; an explicit --opt 9 n wins
+    opts = {int(k): int(v) for k, v in (args.opt or [])}
+    pe = opts.get(9, -1)
+    if pe < 0:
+        pe = 8 if opts.get(14, 1) == 1 else (7 if m.head_dim <= 32 else 0)
+    poly_share = pe / 16.0
     mufu_only = mufu_rate * nsm * clk * 4 * m.head_dim / 1e12            # every exponential on the MUFU
     alu_peak = mufu_only / max(1.0 - poly_share, 1e-9)                   # with the kernel's share on the FMA pipe
     nvalid_rows = int((X[:, 0] != 0).sum())
-    roofline = {"bound": "alu", "kernel": "k_tc_attn2 (a4) + k_attn_norms", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+    roofline = {"bound": "alu", "kernel": "k_tc_attn2 (a4)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": (achieved / peak) if achieved else None, "traffic": traffic, "traffic_source": traffic_note,
                 "peak_source": f"{peaks['source']} bf16_tflops_sustained (dense bf16 tensor peak; the kernel is a contraction)",
-                "alu": {"binding_pipe": "XU (MUFU ex2) + FMA: softmax exponentials, one per 4*hd tensor FLOPs",
+                "alu": {"binding_pipe": "issue slots of the softmax warps: exponentials on XU (MUFU ex2) + FMA pipes, one per 4*hd tensor FLOPs; packed and 16-lane instructions take two issue cycles",
                         "mufu_ex2_per_clk_per_sm_measured": mufu_rate, "mufu_ex2_bf16x2_per_clk_per_sm_measured": bf16x2_rate,
                         "fma_poly_exp_per_clk_per_sm_measured": poly_rate,
                         "sm_clock_hz": clk, "poly_share": poly_share,

@@ -113,14 +113,25 @@ __device__ __forceinline__ void stg_copy_f32(uint8_t* stg, float* g, int64_t ld,
         }
     }
 }
-__device__ __forceinline__ void stg_flush_b16(uint8_t* stg, bf16* g, int64_t ld, int col0, int row, int lane) {
+// The bf16 flush with everything that does not depend on the column group precomputed once per tile (the epilogue is issue
+// bound: the 64-bit row offsets and the four shuffles were ~ 20 instructions per 8-row store): goff[i] = element offset of
+// this lane's piece of local row 8 i + lane / 4 (< 0: skip), soff[i] = its byte offset in the staging tile.
+struct FlushB16 { int64_t goff[4]; int soff[4]; };
+__device__ __forceinline__ FlushB16 stg_flush_b16_setup(int64_t ld, int row, int lane) {
+    FlushB16 f;
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {                       // 8 rows x 64 B per instruction
+    for (int i = 0; i < 4; ++i) {
         const int rr = 8 * i + (lane >> 2), p = lane & 3;
         const int grow = __shfl_sync(0xffffffffu, row, rr);
-        if (grow >= 0)
-            *(reinterpret_cast<uint4*>(g + (int64_t)grow * ld + col0) + p) = *reinterpret_cast<uint4*>(stg_b16(stg, rr, p));
+        f.goff[i] = grow >= 0 ? (int64_t)grow * ld + p * 8 : -1;
+        f.soff[i] = rr * 64 + ((p ^ ((rr >> 1) & 3)) << 4);
     }
+    return f;
+}
+__device__ __forceinline__ void stg_flush_b16(uint8_t* stg, bf16* g, int col0, const FlushB16& f) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i)                         // 8 rows x 64 B per instruction
+        if (f.goff[i] >= 0) *reinterpret_cast<uint4*>(g + f.goff[i] + col0) = *reinterpret_cast<uint4*>(stg + f.soff[i]);
 }
 
 // epilogue of one 16-column chunk held in registers (thread = lane = one row); bias_s = this chunk's bias in shared
@@ -131,8 +142,7 @@ __device__ __forceinline__ void gemm_epilogue_chunk(const uint32_t (&acc)[16], c
     float2 v[8];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-        float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (bias_s) b = *reinterpret_cast<const float4*>(bias_s + 4 * j);       // broadcast LDS.128
+        const float4 b = *reinterpret_cast<const float4*>(bias_s + 4 * j);      // broadcast LDS.128 (zeros when there is no bias)
         const float2 sc = make_float2(ep.out_scale * col_scale, ep.out_scale * col_scale);   // (the staged bias carries col_scale already)
         v[2 * j] = ptx::ffma2(make_float2(__uint_as_float(acc[4 * j]), __uint_as_float(acc[4 * j + 1])), sc, make_float2(b.x, b.y));
         v[2 * j + 1] = ptx::ffma2(make_float2(__uint_as_float(acc[4 * j + 2]), __uint_as_float(acc[4 * j + 3])), sc, make_float2(b.z, b.w));
@@ -203,7 +213,11 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     const int mi0 = blockIdx.x / n_tiles_n, ni0 = blockIdx.x % n_tiles_n;
     auto advance = [&](int& mi, int& ni) { mi += dq; ni += dr; if (ni >= n_tiles_n) { ni -= n_tiles_n; ++mi; } };
     // tiles without meaningful rows (all three roles skip the same ones)
-    auto skip_tile = [&](int m0) { return m0 >= m_end || (ep.group_rows > 0 ? m0 % ep.group_rows : m0) >= nc_rows; };
+    auto skip_tile = [&](int m0) {
+        if (m0 >= m_end) return true;
+        if (ep.group_rows > 0) m0 %= ep.group_rows;           // (a branch, not a select: no division on the one-stack path)
+        return m0 >= nc_rows;
+    };
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_full = ptx::smem_u32(&bars[0]);
     const uint32_t bar_empty = ptx::smem_u32(&bars[STAGES]);
@@ -313,9 +327,9 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             } else if (ep.group_rows > 0) w_row0 = (m0 / ep.group_rows) * N;
             // this tile's bias -> shared memory (read back as broadcast 128-bit loads)
             asm volatile("bar.sync %0, 256;" ::"r"(1 + e) : "memory");          // everyone is done with the last tile's
-            if (ep.bias)
-                for (int c = tid; c < BLOCK_N; c += 256)
-                    bias_s[e][c] = __ldg(ep.bias + w_row0 + n0 + c) * ((ep.qn && n0 + c < ep.nd) ? ep.q_scale : 1.0f);
+            const int q_cols = ep.qn ? ep.nd : 0;                 // columns below it (q of the QKV projection) carry ep.q_scale
+            for (int c = tid; c < BLOCK_N; c += 256)
+                bias_s[e][c] = ep.bias ? __ldg(ep.bias + w_row0 + n0 + c) * (n0 + c < q_cols ? ep.q_scale : 1.0f) : 0.0f;
             asm volatile("bar.sync %0, 256;" ::"r"(1 + e) : "memory");
             const int m = m0 + q * 32 + lane;
             const bool row_ok = m < M;
@@ -326,12 +340,17 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             ptx::tc_fence_after();
             const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + e * BLOCK_N + hcol;
             const int srow = write_ok ? row : -1;                 // destination row of this lane's accumulator row
+            const FlushB16 fl = stg_flush_b16_setup(ep.ld_act, srow, lane);   // (bf16 outputs; unused for fp32 ones)
             uint32_t ra[16], rb[16];
             ptx::tmem_ld16(t_addr, ra);
             // attention norms (QKV projection): this lane's row, its event, running sum of squares of the current head
             const bool norms = ep.qn != nullptr && n0 + hcol < 2 * ep.nd;
             int n_ev = -1;
-            if (norms && row_ok && (ep.group_rows > 0 ? m % ep.group_rows : m) < nc_rows) n_ev = __ldg(ep.row_event + m);
+            if (norms && row_ok) {
+                int mg = m;
+                if (ep.group_rows > 0) mg %= ep.group_rows;
+                if (mg < nc_rows) n_ev = __ldg(ep.row_event + m);
+            }
             float n_ss = 0.0f;
             // (no runtime division in this epilogue: the head width is a power of two, q | k | v by comparison)
             const int hd_shift = 31 - __clz(ep.nhd | 1);
@@ -355,19 +374,19 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 ptx::tmem_ld_wait();
                 ptx::tmem_ld16(t_addr + c + 16, rb);
                 __syncwarp();
-                const float cs0 = (ep.qn && col0 < ep.nd) ? ep.q_scale : 1.0f, cs1 = (ep.qn && col0 + 16 < ep.nd) ? ep.q_scale : 1.0f;
-                gemm_epilogue_chunk<ACT>(ra, ep, ep.bias ? &bias_s[e][hcol + c] : nullptr, stg, lane, 0, norms ? &n_ss : nullptr, cs0);
+                const float cs0 = col0 < q_cols ? ep.q_scale : 1.0f, cs1 = col0 + 16 < q_cols ? ep.q_scale : 1.0f;
+                gemm_epilogue_chunk<ACT>(ra, ep, &bias_s[e][hcol + c], stg, lane, 0, norms ? &n_ss : nullptr, cs0);
                 if (norms) norm_emit(col0 + 16);
                 ptx::tmem_ld_wait();
                 if (c + 32 < BLOCK_N / 2) ptx::tmem_ld16(t_addr + c + 32, ra);
-                gemm_epilogue_chunk<ACT>(rb, ep, ep.bias ? &bias_s[e][hcol + c + 16] : nullptr, stg, lane, 1, norms ? &n_ss : nullptr, cs1);
+                gemm_epilogue_chunk<ACT>(rb, ep, &bias_s[e][hcol + c + 16], stg, lane, 1, norms ? &n_ss : nullptr, cs1);
                 if (norms) norm_emit(col0 + 32);
                 __syncwarp();
                 if (ep.out_f32) {
                     stg_copy_f32<false>(stg, ep.out_f32, ep.ld_f32, col0, srow, lane);
                 } else {
-                    stg_flush_b16(stg, (bf16*)ep.out_act, ep.ld_act, col0, srow, lane);
-                    if (ep.out_act_lo) stg_flush_b16(stg + 2048, (bf16*)ep.out_act_lo, ep.ld_act, col0, srow, lane);
+                    stg_flush_b16(stg, (bf16*)ep.out_act, col0, fl);
+                    if (ep.out_act_lo) stg_flush_b16(stg + 2048, (bf16*)ep.out_act_lo, col0, fl);
                 }
                 __syncwarp();
             }
