@@ -225,7 +225,16 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
         }
         for (int i = 0; i < NT; ++i) ptx::mbar_init(bar_o + 8 * i, 1);
         ptx::fence_barrier_init();
-        ptx::tma_prefetch_desc(&tmQKV);
+        // Q and the first ring of K / V stages go out at once: they do not depend on the fast / exact decision below, whose
+        // global loads (row norms) would otherwise sit in front of the first TMA in every CTA's prologue
+        ptx::mbar_expect_tx(bar_q, Cfg::Q_BYTES * nt);
+        for (int t = 0; t < nt; ++t) ptx::tma_load_2d(sQ + t * Cfg::Q_BYTES, &tmQKV, bar_q, head * HD, q0 + t * A2_BQ);
+        for (int g = 0; g < min(ST, nst); ++g) {
+            const uint32_t st = sKV + g * Cfg::STAGE_BYTES;
+            ptx::mbar_expect_tx(bar_kv_full + 8 * g, Cfg::STAGE_BYTES);
+            ptx::tma_load_2d(st, &tmQKV, bar_kv_full + 8 * g, prm.d + head * HD, ev0 + g * A2_SK);
+            ptx::tma_load_2d(st + Cfg::K_BYTES, &tmQKV, bar_kv_full + 8 * g, 2 * prm.d + head * HD, ev0 + g * A2_SK);
+        }
     }
     if (warp == Cfg::WARP_MMA) {
         ptx::tmem_alloc(ptx::smem_u32(&tmem_base_slot), 512);
@@ -257,11 +266,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
 
     if (warp == Cfg::WARP_TMA) {
         // ------------------------------------------------------------ TMA producer
-        if (lane == 0) {
-            ptx::mbar_expect_tx(bar_q, Cfg::Q_BYTES * nt);
-            for (int t = 0; t < nt; ++t) ptx::tma_load_2d(sQ + t * Cfg::Q_BYTES, &tmQKV, bar_q, head * HD, q0 + t * A2_BQ);
-        }
-        for (int g = 0; g < n_sweeps * nst; ++g) {                   // g = running stage counter over both sweeps
+        for (int g = min(ST, nst); g < n_sweeps * nst; ++g) {        // g = running stage counter over both sweeps (the first ring is under way)
             const int s = g % ST, i = g % nst;
             ptx::mbar_wait_long(bar_kv_empty + 8 * s, ((g / ST) & 1) ^ 1);
             if (lane == 0) {
