@@ -222,6 +222,8 @@ int64_t mlpf_candidates_static_limit(int32_t which);   /* 0: max elements, 1: ma
                                     set-up and first wave overlap its tail; griddepcontrol.wait orders every access); 0: plain stream
                                     order; 2 (default): 1 for calls whose attention grid is at most two waves of CTAs (one event per
                                     call: 0.847 -> 0.823 ms), else 0 (no gain on large batches)                              */
+#define MLPF_OPT_ATTN_POLY_DEG 17 /* tuning (process-wide): degree of that polynomial, 3 (default: relative error 1e-4) or 2 (1.8e-3, the
+                                    size of the bf16 rounding of the softmax weight itself; measured in profiles/r02_README.md)  */
 #define MLPF_PREC_BF16        0
 #define MLPF_PREC_FP32_DEBUG  1
 #define MLPF_KERNELS_TC       0

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmlpf.so")
 
 # include/mlpf.h constants
 OK = 0
-OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE, OPT_FUSE, OPT_ATTN, OPT_ATTN_POLY, OPT_COMPACT, OPT_GRAPH, OPT_TAIL_SPLIT, OPT_FP8, OPT_EPI_NORMS, OPT_TC_EMBED, OPT_PDL = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16
+OPT_PRECISION, OPT_TILE_Q, OPT_TAP_LAYER, OPT_KERNELS, OPT_SPLIT, OPT_PROFILE, OPT_FUSE, OPT_ATTN, OPT_ATTN_POLY, OPT_COMPACT, OPT_GRAPH, OPT_TAIL_SPLIT, OPT_FP8, OPT_EPI_NORMS, OPT_TC_EMBED, OPT_PDL, OPT_ATTN_POLY_DEG = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16, 17
 PREC_BF16, PREC_FP32_DEBUG = 0, 1
 KERNELS_TC, KERNELS_SIMPLE = 0, 1
 Q_N_LAYERS, Q_D_MODEL, Q_N_HEADS, Q_D_FF, Q_N_FEAT, Q_N_CLASSES, Q_N_REGRESS = 1, 2, 3, 4, 5, 6, 7

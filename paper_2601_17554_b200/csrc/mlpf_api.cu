@@ -343,6 +343,9 @@ extern "C" int mlpf_set_option(mlpf_handle* h, int key, int64_t value) {
         case MLPF_OPT_ATTN:
             if (value < 0 || value > 2) return set_err(MLPF_E_ARG, "attn must be 0, 1 or 2");
             h->attn = (int)value; return MLPF_OK;
+        case MLPF_OPT_ATTN_POLY_DEG:
+            if (value != 2 && value != 3) return set_err(MLPF_E_ARG, "attn_poly_deg must be 2 or 3");
+            g_attn2_poly_deg = (int)value; return MLPF_OK;
         case MLPF_OPT_PDL:
             if (value < 0 || value > 2) return set_err(MLPF_E_ARG, "pdl must be 0, 1 or 2");
             h->pdl = (int)value; return MLPF_OK;
@@ -961,7 +964,7 @@ extern "C" int mlpf_infer_ex(mlpf_handle* h, const float* elements, const int32_
         push64((uint64_t)(uintptr_t)elements); push64((uint64_t)(uintptr_t)out_logits); push64((uint64_t)(uintptr_t)out_regress);
         push64((uint64_t)(uintptr_t)out_binary);
         key.push_back(h->precision); key.push_back(h->kernels); key.push_back(h->split); key.push_back(h->fuse);
-        key.push_back(h->attn); key.push_back(h->compact); key.push_back(h->epi_norms); key.push_back(h->tc_embed); key.push_back(h->pdl); key.push_back(h->fp8); key.push_back(h->tail_split); key.push_back(h->tile_q); key.push_back(g_attn2_poly_every);
+        key.push_back(h->attn); key.push_back(h->compact); key.push_back(h->epi_norms); key.push_back(h->tc_embed); key.push_back(h->pdl); key.push_back(h->fp8); key.push_back(h->tail_split); key.push_back(h->tile_q); key.push_back(g_attn2_poly_every); key.push_back(g_attn2_poly_deg);
         key.insert(key.end(), event_offsets, event_offsets + n_off);
         for (auto& ge : w->graphs)
             if (ge.key == key) {

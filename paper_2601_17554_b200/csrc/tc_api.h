@@ -74,6 +74,7 @@ int tc_attn_launch(TcContext* c, const bf16* QKV, int64_t N, const uint32_t* val
 // row_event [N] from the schedule.  force_exact != 0: every CTA takes the exact path (tests).  prescaled: the q columns
 // of QKV (and qn) already carry the softmax scale log2(e) / sqrt(hd) (Epi::q_scale): the fast path then subtracts nothing.
 int tc_attn2_rows_per_cta(int hd);
+extern int g_attn2_poly_deg;         // degree of that polynomial: 3 | 2 (experiment)
 extern int g_attn2_poly_every;       // tuning knob: every n-th pair of exponentials on the FMA pipe (0, 2, 3, 4; -1 = default)
 int tc_attn2_launch(TcContext* c, const bf16* QKV, int64_t N, int E, const uint32_t* valid_bits, const int* n_valid,
                     const int* offsets, const int* row_event, const int2* items, int n_items, int d, int H, float* qn,

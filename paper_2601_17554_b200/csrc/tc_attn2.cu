@@ -133,13 +133,22 @@ __device__ __forceinline__ float2 a2_exp2_poly2(float2 sc, float2 c2, float2 k1)
 // constant K = 1.2939453125 folded into the coefficients) and a final packed multiply, which moves the two integer
 // multiply-adds from the FMA pipe to the idle ALU pipe: slower, 2.93 vs 2.87 ms per cfg3 step of attention.  The loop is
 // bound by issue slots, two per packed or 16-lane instruction, not by any one pipe.)
+// DEG = 2 (experiment, MLPF_OPT_ATTN_POLY_DEG): the minimax quadratic, max relative error 1.83e-3 = the size of P's own bf16
+// rounding (2^-9), one packed FMA less per pair.
+template <int DEG>
 __device__ __forceinline__ float2 a2_exp2_poly2_ps(float2 s) {
     const float2 xr = ptx::fadd2(s, make_float2(12582912.0f, 12582912.0f));
     const float2 m = ptx::fadd2(xr, make_float2(-12582912.0f, -12582912.0f));
     const float2 f = ptx::fadd2(s, make_float2(-m.x, -m.y));
-    float2 p = ptx::ffma2(f, make_float2(0.0550089306f, 0.0550089306f), make_float2(0.2422109596f, 0.2422109596f));
-    p = ptx::ffma2(p, f, make_float2(0.6932829272f, 0.6932829272f));
-    p = ptx::ffma2(p, f, make_float2(1.0f, 1.0f));
+    float2 p;
+    if (DEG == 2) {
+        p = ptx::ffma2(f, make_float2(0.23864397f, 0.23864397f), make_float2(0.70388058f, 0.70388058f));
+        p = ptx::ffma2(p, f, make_float2(1.00046145f, 1.00046145f));
+    } else {
+        p = ptx::ffma2(f, make_float2(0.0550089306f, 0.0550089306f), make_float2(0.2422109596f, 0.2422109596f));
+        p = ptx::ffma2(p, f, make_float2(0.6932829272f, 0.6932829272f));
+        p = ptx::ffma2(p, f, make_float2(1.0f, 1.0f));
+    }
     return make_float2(__int_as_float(__float_as_int(p.x) + (__float_as_int(xr.x) << 23)),
                        __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
 }
@@ -151,7 +160,7 @@ __device__ __forceinline__ float2 a2_exp2_poly2_ps(float2 s) {
 // MUFU gives the exact weight 0 (the polynomial path is not used on masked tiles).
 // PS (pre-scaled scores, fast path): S already holds s c and no offset is subtracted (see the kernel): unmasked tiles feed
 // the MUFU straight from TMEM; masked tiles and the exact path keep the FMA with c = 1.
-template <bool MASKED, int PE, bool PS>
+template <bool MASKED, int PE, bool PS, int DEG = 3>
 __device__ __forceinline__ void a2_exp32(uint32_t (&s)[32], uint32_t mask, float c, float neg_bc, uint32_t (&pk)[16]) {
     const float2 c2 = make_float2(c, c), m2 = make_float2(neg_bc, neg_bc);
     const float2 k1 = make_float2(12582912.0f + neg_bc, 12582912.0f + neg_bc);      // exact: neg_bc is an integer on this path
@@ -163,7 +172,7 @@ __device__ __forceinline__ void a2_exp32(uint32_t (&s)[32], uint32_t mask, float
         }
         const float2 sc = make_float2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1]));
         float2 p;
-        if (!MASKED && ((i + 1) * PE) / 16 > (i * PE) / 16) p = PS ? a2_exp2_poly2_ps(sc) : a2_exp2_poly2(sc, c2, k1);
+        if (!MASKED && ((i + 1) * PE) / 16 > (i * PE) / 16) p = PS ? a2_exp2_poly2_ps<DEG>(sc) : a2_exp2_poly2(sc, c2, k1);
         else if (!MASKED && PS) p = make_float2(ptx::fast_exp2(sc.x), ptx::fast_exp2(sc.y));
         else {
             const float2 x = ptx::ffma2(sc, c2, m2);
@@ -174,7 +183,7 @@ __device__ __forceinline__ void a2_exp32(uint32_t (&s)[32], uint32_t mask, float
     }
 }
 
-template <int HD, int PE, bool PS>
+template <int HD, int PE, bool PS, int DEG = 3>
 __global__ void __launch_bounds__(Attn2Cfg<HD>::THREADS, 1)
 k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
     using Cfg = Attn2Cfg<HD>;
@@ -403,7 +412,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
                 ptx::tmem_ld32(s_addr, s);
                 const uint32_t m = MASKED ? tile_mask(j) : 0xffffffffu;
                 ptx::tmem_ld_wait();
-                a2_exp32<MASKED, PE, PS>(s, m, c, neg_bc, pk);
+                a2_exp32<MASKED, PE, PS, DEG>(s, m, c, neg_bc, pk);
                 ptx::tmem_st16(s_addr, pk);
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
@@ -471,14 +480,15 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
     if (warp == Cfg::WARP_MMA) ptx::tmem_dealloc(tmem_base, 512);
 }
 
+int g_attn2_poly_deg = 3;            // tuning knob (MLPF_OPT_ATTN_POLY_DEG): 3 (default) | 2
 int g_attn2_poly_every = -1;          // tuning knob (MLPF_OPT_ATTN_POLY): -1 = the default of the head dimension
 
-template <int HD, int PE, bool PS>
+template <int HD, int PE, bool PS, int DEG = 3>
 static int tc_attn2_launch_pe(TcContext* c, const bf16* QKV, int64_t N, Attn2Params prm, cudaStream_t st) {
     using Cfg = Attn2Cfg<HD>;
     CUtensorMap tmQKV;
     if (tc_tensor_map(c, &tmQKV, QKV, 3 * prm.d, N, 3 * prm.d, HD, A2_SK)) return -1;
-    auto kern = k_tc_attn2<HD, PE, PS>;
+    auto kern = k_tc_attn2<HD, PE, PS, DEG>;
     if (tc_set_smem_attr(c, (const void*)kern, Cfg::SMEM_BYTES)) return -1;
     tc_launch(kern, dim3(prm.n_items * prm.H), dim3(Cfg::THREADS), Cfg::SMEM_BYTES, st, c->pdl, tmQKV, prm);
     return 0;
@@ -489,6 +499,12 @@ static int tc_attn2_launch_hd(TcContext* c, const bf16* QKV, int64_t N, Attn2Par
     // measured (profiles/r02_README.md): with prescaled scores 8 of 16 at every head dimension (hd = 64: 4.41 -> 3.37 ms of
     // attention per cfg5a step against all-MUFU); the unscaled form (kernel-level entry) keeps its own optimum
     const int pe = g_attn2_poly_every >= 0 ? g_attn2_poly_every : (PS ? 8 : (HD == 64 ? 0 : 7));
+    if (PS && g_attn2_poly_deg == 2) {            // experiment: quadratic polynomial (prescaled scores only)
+        switch (pe) {
+            case 9: return tc_attn2_launch_pe<HD, 9, PS, 2>(c, QKV, N, prm, st);
+            default: return tc_attn2_launch_pe<HD, 8, PS, 2>(c, QKV, N, prm, st);
+        }
+    }
     switch (pe) {
         case 0: return tc_attn2_launch_pe<HD, 0, PS>(c, QKV, N, prm, st);
         case 4: return tc_attn2_launch_pe<HD, 4, PS>(c, QKV, N, prm, st);

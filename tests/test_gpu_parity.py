@@ -236,6 +236,24 @@ def test_programmatic_dependent_launch_changes_nothing(name, max_events):
     assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1])
 
 
+def test_quadratic_softmax_polynomial_is_an_option_within_tolerance():
+    """MLPF_OPT_ATTN_POLY_DEG = 2 (off by default): half of the softmax weights from a quadratic 2^f (relative error 1.8e-3,
+    the size of the weight's own bf16 rounding) instead of the cubic (1e-4).  Still far inside the 2e-2 tolerance; the
+    measured cost in accuracy and gain in time are in profiles/r02_README.md."""
+    m = synth.model_cfg("cfg2")
+    W = synth.make_weights("cfg2")
+    X, off = synth.make_named_events("cfg2")
+    rows, lr, rr = oracle_events(W, m, X, off, range(len(off) - 1), quantized=True)
+    try:
+        mod = P.Mlpf(W, m)
+        mod.set_option(P.OPT_ATTN_POLY_DEG, 2)
+        lg, rg = mod.infer(torch.from_numpy(X).cuda(), off)
+        torch.cuda.synchronize()
+        check(lg.cpu().numpy(), rg.cpu().numpy(), rows, lr, rr, X, TOL_BF16)
+    finally:
+        mod.set_option(P.OPT_ATTN_POLY_DEG, 3)       # process-wide knob
+
+
 # ------------------------------------------------------------------------------------------- edge cases
 TINY = ModelCfg(n_layers=2, d_model=64, n_heads=4, d_ff=256)
 
