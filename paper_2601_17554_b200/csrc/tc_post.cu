@@ -283,7 +283,7 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
         float* const v_b2 = vec + 3 * D; float* const v_gn = vec + 4 * D; float* const v_bn = vec + 5 * D;
         float* const v_b1 = vec + 6 * D;
         uint32_t ph_s = 0;
-        int it = -1;
+        int it = -1, g_staged = -1;
         // mean and 1/sigma of the row from the four column groups' partials (each over CW columns)
         auto row_stats = [&](float n, float mean, float m2, float& mu, float& rstd) {
             part[cg * POST_BM + r] = make_float2(mean, m2);
@@ -305,19 +305,20 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
             const int m0 = tile * POST_BM, g = m0 / p.group_rows;
             const int row = m0 + r;
             const bool row_ok = row < p.M;
-            // this tile's vectors (per group) -> shared memory
-            asm volatile("bar.sync 1, 512;" ::: "memory");
-            for (int i = et; i < D; i += 512) {
-                v_bo[i] = __ldg(p.bo + g * D + i); v_g2[i] = __ldg(p.ln2g + g * D + i); v_b2ln[i] = __ldg(p.ln2b + g * D + i);
-                v_b2[i] = __ldg(p.b2 + g * D + i);
-                v_gn[i] = p.next_ln ? __ldg(p.lnng + g * D + i) : 1.0f; v_bn[i] = p.next_ln ? __ldg(p.lnnb + g * D + i) : 0.0f;
+            // this tile's vectors (per group) -> shared memory; they change only where the group (encoder stack) does
+            if (g != g_staged) {
+                asm volatile("bar.sync 1, 512;" ::: "memory");
+                for (int i = et; i < D; i += 512) {
+                    v_bo[i] = __ldg(p.bo + g * D + i); v_g2[i] = __ldg(p.ln2g + g * D + i); v_b2ln[i] = __ldg(p.ln2b + g * D + i);
+                    v_b2[i] = __ldg(p.b2 + g * D + i);
+                    v_gn[i] = p.next_ln ? __ldg(p.lnng + g * D + i) : 1.0f; v_bn[i] = p.next_ln ? __ldg(p.lnnb + g * D + i) : 0.0f;
+                }
+                for (int i = et; i < p.dff; i += 512) v_b1[i] = __ldg(p.b1 + g * p.dff + i);
+                asm volatile("bar.sync 1, 512;" ::: "memory");
+                g_staged = g;
             }
-            for (int i = et; i < p.dff; i += 512) v_b1[i] = __ldg(p.b1 + g * p.dff + i);
-            asm volatile("bar.sync 1, 512;" ::: "memory");
 
             // ---------------- epilogue of the output projection: h1 = h + acc + bo -> acc (TMEM); u2 = LN2(h1) -> A operand
-            ptx::mbar_wait(bar_acc_full, it & 1);
-            ptx::tc_fence_after();
             float sn = 0.f, smean = 0.f, sm2 = 0.f;
             // rows past M (last tile) read the last valid row instead (their results are never stored): the loads need
             // no predicate or branch, so all of a piece's loads are in flight together
@@ -325,6 +326,13 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
             int64_t hin_base, hout_base; int hin_stride, hout_stride;
             h_addr<D>(p.h_in_tiled != 0, tile, r_ld, hin_base, hin_stride);
             h_addr<D>(p.h_out_tiled != 0, tile, r, hout_base, hout_stride);
+            // the residual rows of the first piece are fetched while the output projection's MMAs still run
+            float4 hv0[PIECE / 4];
+#pragma unroll
+            for (int i = 0; i < PIECE / 4; ++i)
+                hv0[i] = *reinterpret_cast<const float4*>(p.h + hin_base + (int64_t)(cg * CW / 4 + i) * hin_stride);
+            ptx::mbar_wait(bar_acc_full, it & 1);
+            ptx::tc_fence_after();
 #pragma unroll
             for (int c0 = cg * CW; c0 < (cg + 1) * CW; c0 += PIECE) {
                 uint32_t a[PIECE];
@@ -332,7 +340,7 @@ k_tc_post(const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUten
                 float4 hv[PIECE / 4];
 #pragma unroll
                 for (int i = 0; i < PIECE / 4; ++i)
-                    hv[i] = *reinterpret_cast<const float4*>(p.h + hin_base + (int64_t)(c0 / 4 + i) * hin_stride);
+                    hv[i] = c0 == cg * CW ? hv0[i] : *reinterpret_cast<const float4*>(p.h + hin_base + (int64_t)(c0 / 4 + i) * hin_stride);
                 float v[PIECE];
 #pragma unroll
                 for (int i = 0; i < PIECE / 4; ++i) {
