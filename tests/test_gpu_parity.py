@@ -254,6 +254,48 @@ def test_quadratic_softmax_polynomial_is_an_option_within_tolerance():
         mod.set_option(P.OPT_ATTN_POLY_DEG, 3)       # process-wide knob
 
 
+# ------------------------------------------------------------------------------------------- random shapes
+@pytest.mark.parametrize("seed", [101, 102, 103, 104])
+def test_random_models_and_ragged_batches_against_the_oracle(seed):
+    """Seeded random draws of everything the blob header can express at d_model <= 256 (1-3 layers, head widths 16 / 32 /
+    64, d_ff 128..1024, GELU / ReLU, with and without the final LayerNorm, one or two stacks, binary head) on ragged batches
+    (empty events, lengths around the 64 / 128 tile edges, pad rows): the tensor-core path within 2e-2 and the fp32 debug
+    path within 1e-4 of the oracle (reading A14), pad rows exactly 0.  A sweep of 150 such cases measured <= 9.2e-3 / 2.1e-5."""
+    rng = np.random.default_rng(seed)
+    for case in range(6):
+        d, H = [(64, 4), (128, 8), (256, 8), (256, 16), (128, 2), (64, 1), (256, 4)][rng.integers(0, 7)]
+        stacks = int(rng.integers(1, 3))
+        m = ModelCfg(n_layers=int(rng.integers(1, 4)), d_model=d, n_heads=H, d_ff=int(rng.choice([128, 256, 512, 1024])),
+                     activation=str(rng.choice(["gelu", "relu"])), final_ln=bool(rng.integers(0, 2)), n_stacks=stacks,
+                     binary_head=bool(stacks == 2 and rng.integers(0, 2)))
+        E = int(rng.integers(1, 20))
+        kind = rng.integers(0, 3)
+        if kind == 0:
+            lens = rng.integers(0, 40, E)
+        elif kind == 1:
+            lens = np.where(rng.random(E) < 0.3, 0, rng.integers(1, 400, E))
+        else:
+            lens = rng.choice([1, 63, 64, 65, 127, 128, 129, 255, 256, 257, 383, 384, 385], E)
+        W = synth.make_weights(m, seed=int(rng.integers(1, 1 << 30)))
+        X, off = synth.make_events([int(x) for x in lens], seed=int(rng.integers(1, 1 << 30)), pad_frac=float(rng.choice([0.0, 0.1, 0.5])))
+        valid = X[:, 0] != 0
+        if valid.sum() < 2:
+            continue
+        Xd = torch.from_numpy(X).cuda()
+        for precision, tol, Wo in ((P.PREC_BF16, TOL_BF16, oracle.quantize_weights(W)), (P.PREC_FP32_DEBUG, TOL_FP32, W)):
+            mod = P.Mlpf(W, m)
+            mod.set_option(P.OPT_PRECISION, precision)
+            got = mod.infer(Xd, off, with_binary=True) if m.binary_head else mod.infer(Xd, off)
+            torch.cuda.synchronize()
+            ref = oracle.forward(X, off, Wo, m, with_binary=True) if m.binary_head else oracle.forward(X, off, Wo, m)
+            for g, r in zip(got, ref):
+                g = g.cpu().numpy().reshape(X.shape[0], -1)
+                r = np.asarray(r).reshape(X.shape[0], -1)
+                assert np.isfinite(g).all() and (g[~valid] == 0).all(), (seed, case)
+                err, _ = oracle.parity_metrics(g, r, valid)
+                assert err <= tol, (seed, case, precision, err, m, [int(x) for x in lens])
+
+
 # ------------------------------------------------------------------------------------------- edge cases
 TINY = ModelCfg(n_layers=2, d_model=64, n_heads=4, d_ff=256)
 
