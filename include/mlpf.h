@@ -81,10 +81,11 @@ mlpf_handle* mlpf_create(const void* blob, size_t blob_bytes);
 /* mlpf_infer: one forward pass (steps a0..a8 of DESIGN.md) over n_events packed events.
  *   elements      DEVICE, [N, n_feat] row-major fp32, N = event_offsets[n_events]; feature 0 is the
  *                 element type id as a float (0 = pad row, 1 track, 2 ECAL, 3 HCAL, 4 HF; A1-A2).
- *                 PRECONDITION: the features of non-pad rows are finite.  Events do not see each other's VALUES, but a
- *                 128-row K / V tile at the end of an event runs into the next event's first rows; their keys get weight
- *                 exactly 0, and 0 x NaN = NaN in the tensor core: a NaN / Inf row of event B would poison the tail of
- *                 event A.  Pad rows may hold anything (they are dropped before the first GEMM).
+ *                 NaN / Inf features of a non-pad row give undefined outputs for THAT event and no other (never a crash):
+ *                 every step but attention is row-local, and the attention kernel zeroes, in shared memory, the rows of
+ *                 the next event that an event's last K / V tile overlaps (their keys have weight exactly 0, but
+ *                 0 x NaN = NaN in the tensor core).  Round 1's attention kernel (MLPF_OPT_ATTN = 0) does not: with it,
+ *                 finite features are a precondition.  Pad rows may hold anything (dropped before the first GEMM).
  *   event_offsets HOST, n_events+1 int32, [0] = 0, non-decreasing; read before return (caller may free).
  *   out_logits    DEVICE, [N, n_classes] fp32.   out_regress  DEVICE, [N, sum(reg_dims)] fp32
  *                 = raw head outputs (pT', eta, sin phi, cos phi, E'), no inverse transform (A12).

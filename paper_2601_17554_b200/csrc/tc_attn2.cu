@@ -189,7 +189,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
     using Cfg = Attn2Cfg<HD>;
     constexpr int ST = Cfg::STAGES, NT = Cfg::NT;
     extern __shared__ uint8_t smem_raw[];
-    __shared__ uint64_t bars[1 + 2 * ST + 5 * NT];
+    __shared__ uint64_t bars[2 + 2 * ST + 5 * NT];
     __shared__ uint32_t tmem_base_slot;
     __shared__ int bound_bits;                                   // max over the CTA's rows of B c (float bits)
 
@@ -220,6 +220,12 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
     const uint32_t bar_s = ptx::smem_u32(&bars[1 + 2 * ST]);             // [2t + b]: S_t landed in buffer b
     const uint32_t bar_p = ptx::smem_u32(&bars[1 + 2 * ST + 2 * NT]);    // [2t + b]: P_t written over buffer b (or S consumed)
     const uint32_t bar_o = ptx::smem_u32(&bars[1 + 2 * ST + 4 * NT]);    // [t]: all of O_t accumulated
+    const uint32_t bar_vc = ptx::smem_u32(&bars[1 + 2 * ST + 5 * NT]);   // the last V stage's foreign rows are zeroed
+    // The last 128-row K / V stage of an event runs into the NEXT event's first rows.  Their keys get weight exactly 0 (masked
+    // tile), but 0 x NaN = NaN in the P V product: a non-finite row of the next event would poison this event's accumulators.
+    // The producer warp therefore zeroes those V rows in shared memory before the issuers may read the stage (once per CTA).
+    const int last_rows = (ev1 - ev0) - (nst - 1) * A2_SK;                 // keys of this event in its last stage: 1 .. 128
+    const bool v_clean = last_rows < A2_SK;
 
     if (threadIdx.x == 0) bound_bits = 0;
     if (warp == Cfg::WARP_TMA && lane == 0) {
@@ -233,6 +239,7 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
             ptx::mbar_init(bar_p + 8 * i, 8);                        // one arrival per softmax warp of the tile
         }
         for (int i = 0; i < NT; ++i) ptx::mbar_init(bar_o + 8 * i, 1);
+        ptx::mbar_init(bar_vc, 1);
         ptx::fence_barrier_init();
         // Q and the first ring of K / V stages go out at once: they do not depend on the fast / exact decision below, whose
         // global loads (row norms) would otherwise sit in front of the first TMA in every CTA's prologue
@@ -287,6 +294,16 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
             }
             __syncwarp();
         }
+        if (v_clean) {                           // the softmax sweep's last stage has landed: zero V rows last_rows .. 127
+            const int g = n_sweeps * nst - 1, s = g % ST;
+            ptx::mbar_wait_long(bar_kv_full + 8 * s, (g / ST) & 1);
+            const uint32_t vt = sKV + s * Cfg::STAGE_BYTES + Cfg::K_BYTES + last_rows * Cfg::SW;   // (a row's swizzled chunks stay inside the row)
+            for (int i = lane; i < (A2_SK - last_rows) * Cfg::SW / 16; i += 32)
+                asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(vt + 16 * i), "r"(0) : "memory");
+            ptx::fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(bar_vc);
+        }
     } else if (warp > Cfg::WARP_TMA && warp - Cfg::WARP_MMA < nt) {
         // ------------------------------------------------------------ MMA issuers (one per query tile)
         const int t = warp - Cfg::WARP_MMA;
@@ -336,6 +353,10 @@ k_tc_attn2(const __grid_constant__ CUtensorMap tmQKV, Attn2Params prm) {
                 const uint32_t odd = (uint32_t)j & 1u;
                 ptx::mbar_wait_long(bp_t + 8 * nb, np);                     // P_t(j) in TMEM (sweep 0 of 2: S consumed)
                 ptx::tc_fence_after();
+                if (pv && v_clean && (j >> 1) == nst - 1 && (!odd || j == 0)) {      // first tile of the last stage
+                    ptx::mbar_wait_long(bar_vc, 0);
+                    ptx::tc_fence_after();
+                }
                 if (pv) issue_o(nb, kd + KB16 + odd * HALF16, j == 0);
                 const bool last_of_stage = odd || j == nkv - 1;
                 if (last_of_stage) ptx::mma_commit(bar_kv_empty + 8 * stg);

@@ -18,6 +18,7 @@ import paper_2601_17554_b200 as P
 
 TOL_BF16 = 2e-2
 TOL_FP32 = 1e-4
+TINY_FOR_NAN = ModelCfg(n_layers=2, d_model=64, n_heads=2, d_ff=256)
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -252,6 +253,34 @@ def test_quadratic_softmax_polynomial_is_an_option_within_tolerance():
         check(lg.cpu().numpy(), rg.cpu().numpy(), rows, lr, rr, X, TOL_BF16)
     finally:
         mod.set_option(P.OPT_ATTN_POLY_DEG, 3)       # process-wide knob
+
+
+def test_non_finite_features_stay_inside_their_event():
+    """include/mlpf.h: NaN / Inf features give undefined outputs for THAT event only.  The 128-row K / V tile at the end of
+    event A runs into event B's first rows: their keys get weight exactly 0, and the v values are made finite by a3's
+    epilogue so that 0 x v cannot poison A's accumulators."""
+    m = TINY_FOR_NAN
+    W = synth.make_weights(m, seed=11)
+    X, off = synth.make_events((300, 257, 190), seed=12)
+    X = X.copy()
+    b0 = int(off[1])
+    X[b0, 3] = np.nan                         # first rows of event B: NaN, +Inf, -Inf features (types stay valid)
+    X[b0 + 1, 5] = np.inf
+    X[b0 + 2, 7] = -np.inf
+    for precision, tol, Wo in ((P.PREC_BF16, TOL_BF16, oracle.quantize_weights(W)), (P.PREC_FP32_DEBUG, TOL_FP32, W)):
+        mod = P.Mlpf(W, m)
+        mod.set_option(P.OPT_PRECISION, precision)
+        lg, rg = mod.infer(torch.from_numpy(X).cuda(), off)
+        torch.cuda.synchronize()
+        lg = lg.cpu().numpy(); rg = rg.cpu().numpy()
+        for e in (0, 2):                      # the events before and after the poisoned one
+            a, b = int(off[e]), int(off[e + 1])
+            lr, rr = oracle.forward(X[a:b], np.array([0, b - a], np.int32), Wo, m)
+            valid = X[a:b, 0] != 0
+            assert np.isfinite(lg[a:b]).all() and np.isfinite(rg[a:b]).all(), (precision, e)
+            e_lg, _ = oracle.parity_metrics(lg[a:b], lr, valid)
+            e_rg, _ = oracle.parity_metrics(rg[a:b], rr, valid)
+            assert e_lg <= tol and e_rg <= tol, (precision, e, e_lg, e_rg)
 
 
 # ------------------------------------------------------------------------------------------- random shapes
