@@ -283,6 +283,49 @@ def test_non_finite_features_stay_inside_their_event():
             assert e_lg <= tol and e_rg <= tol, (precision, e, e_lg, e_rg)
 
 
+def test_concurrent_calls_from_host_threads_on_their_own_streams():
+    """include/mlpf.h: concurrent mlpf_infer calls on DIFFERENT streams of one handle are safe (one workspace per stream, the
+    enqueue serialised by the handle's mutex).  Four host threads, one stream each, ragged batches of different sizes; every
+    result bit-identical to the same batch run alone afterwards."""
+    import threading
+    m = synth.model_cfg("cfg2")
+    W = synth.make_weights("cfg2")
+    mod = P.Mlpf(W, m)
+    rng = np.random.default_rng(3)
+    batches = []
+    for i in range(16):
+        lens = [int(x) for x in rng.integers(0, 700, int(rng.integers(1, 10)))]
+        X, off = synth.make_events(lens, seed=100 + i, pad_frac=float(rng.choice([0.0, 0.1])))
+        if X.shape[0]:
+            batches.append((torch.from_numpy(X).cuda(), off))
+    results, errors = {}, []
+
+    def worker(tid):
+        try:
+            st = torch.cuda.Stream()
+            for rep in range(4):
+                for bi in range(tid, len(batches), 4):
+                    Xd, off = batches[bi]
+                    lg, rg = mod.infer(Xd, off, stream=st)
+                    st.synchronize()
+                    results[(bi, rep)] = (lg.clone(), rg.clone())
+        except Exception as e:                      # surfaced in the main thread below
+            errors.append(e)
+
+    threads = [threading.Thread(target=worker, args=(t,)) for t in range(4)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    for bi, (Xd, off) in enumerate(batches):
+        lg, rg = mod.infer(Xd, off)
+        torch.cuda.synchronize()
+        for rep in range(4):
+            a, b = results[(bi, rep)]
+            assert torch.equal(a, lg) and torch.equal(b, rg), (bi, rep)
+
+
 # ------------------------------------------------------------------------------------------- random shapes
 @pytest.mark.parametrize("seed", [101, 102, 103, 104])
 def test_random_models_and_ragged_batches_against_the_oracle(seed):
