@@ -195,8 +195,8 @@ int64_t mlpf_candidates_static_limit(int32_t which);   /* 0: max elements, 1: ma
 #define MLPF_OPT_FUSE        7   /* 1 (default): where the shape allows (d_model <= 256, d_ff % 128 == 0, all activations split)
                                     the post-attention half of every block runs as ONE kernel (out-projection + residual +
                                     LN2 + FFN1 + activation + FFN2 + residual + next LayerNorm); 0: one kernel per step   */
-#define MLPF_OPT_ATTN        8   /* attention kernel: 1 (default) = tc_attn2.cu (no running maximum: Cauchy-Schwarz bound from a norms
-                                    pre-pass, exact two-sweep path when the bound is too loose; two threads per query row);
+#define MLPF_OPT_ATTN        8   /* attention kernel: 1 (default) = tc_attn2.cu (no running maximum: Cauchy-Schwarz bound from row norms
+                                    (MLPF_OPT_EPI_NORMS), exact two-sweep path when the bound is too loose; two threads per query row);
                                     2 = the same with the exact path forced for every CTA; 0 = round 1's lazy-rescale kernel */
 #define MLPF_OPT_ATTN_POLY   9   /* tuning (process-wide): n of every 16 pairs of softmax exponentials run as a polynomial on the
                                     FMA pipe instead of the MUFU: 0 (none), 4, 7, 8, 9; -1 (default) = 8 in the model path (scores prescaled by a3's
