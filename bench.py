@@ -430,7 +430,7 @@ def run_ours(args):
     roofline = {"bound": "alu", "kernel": "k_tc_attn2 (a4)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": (achieved / peak) if achieved else None, "traffic": traffic, "traffic_source": traffic_note,
                 "peak_source": f"{peaks['source']} bf16_tflops_sustained (dense bf16 tensor peak; the kernel is a contraction)",
-                "alu": {"binding_pipe": "softmax exponentials, one per 4*hd tensor FLOPs, split over the XU (MUFU ex2) queue and the FMA pipe (packed polynomial): ~65 % busy each, limiting one another (DESIGN.md section 6)",
+                "alu": {"binding_pipe": "issue slots of the softmax warps: exponentials on XU (MUFU ex2) + FMA pipes, one per 4*hd tensor FLOPs; packed and 16-lane instructions take two issue cycles",
                         "mufu_ex2_per_clk_per_sm_measured": mufu_rate, "mufu_ex2_bf16x2_per_clk_per_sm_measured": bf16x2_rate,
                         "fma_poly_exp_per_clk_per_sm_measured": poly_rate,
                         "sm_clock_hz": clk, "poly_share": poly_share,
